@@ -1,0 +1,331 @@
+/*
+ * mf_oracle.c — plain, slow, fp64 CPU ORACLE for the MoreFit NLL + analytic gradient.
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT PRODUCT CODE.  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may build, link or call it.  It
+ * shares no code, header, table or constant with paper_2505_12414_b200/ (the CUDA path)
+ * and neither includes the other.
+ *
+ * What it computes (the plain definitions, PAPER.md line numbers):
+ *   Eq. 1      -ln L(lambda) = - sum_i ln P(x_i | lambda)
+ *   Eq. 2   mass model  P = f G/N1 + (1-f) e^{tau m}/N2
+ *   Eq. 4 angular model d^3Gamma/dcos(theta_l) dcos(theta_K) dphi
+ *   4D model (BASELINE.json configs[3]; not in the paper) P = f (G/N1) A + (1-f) (E/N2) L
+ * and the hand-derived d ln P / d lambda_k of each.
+ *
+ * Deliberately NOT done here (those are the optimisations under test):
+ * no parameter-only constants hoisted out of the event loop, no cached event-only
+ * terms, no algebraic merging of the angular terms, no blocking or fusion.  Every event
+ * re-evaluates the normalisations from the formulas.  Per-event arithmetic is IEEE
+ * double (the paper's precision); sums over events are accumulated
+ * in long double (x87 80-bit) so that the summation error of the oracle itself is
+ * negligible against the 1e-11 / 1e-9 parity tolerances.  With OpenMP (nthreads > 1)
+ * events are split into `nthreads` contiguous static chunks whose long-double sums
+ * are combined in chunk order.
+ *
+ * Readings of the paper taken here:
+ *   R6  N2 is evaluated as e^{tau a} expm1(tau (b-a)) / tau (tau != 0) and (b-a) at tau == 0;
+ *       d ln N2 / d tau = a + w h(tau w), h(u) = 1/(1-e^{-u}) - 1/u evaluated in long
+ *       double, by its Taylor series for |u| < 1e-2 (cancellation), h(0) = 1/2.
+ *   R9  no extended (Poisson) term, unweighted events.
+ *   R15 an event with P <= 0 (or NaN) makes -ln L = +inf and every gradient component NaN;
+ *       the number of such events is returned.
+ *
+ * Pins (tests/test_oracle_*.py): unit integral by quadrature, positivity, score identity,
+ * finite differences, scipy truncnorm/truncexpon, Gaussian closed-form MLE, the printed
+ * constants of Listing 4, closed-form angular marginals, hand-evaluated points of Eq. 4.
+ */
+#include <math.h>
+#include <stddef.h>
+#include <stdint.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define MFO_MASS 0
+#define MFO_ANGULAR 1
+#define MFO_4D 2
+#define MFO_MAXK 16
+
+static const double MFO_PI = 3.14159265358979323846264338327950288;
+
+/* ---------------------------------------------------------------- mass, Eq. 2 */
+
+/* N1(mu, sigma) */
+static double norm_gauss(double mu, double sigma, double a, double b)
+{
+    const double s2 = sqrt(2.0) * sigma;
+    return 0.5 * (erf((mu - a) / s2) - erf((mu - b) / s2));
+}
+
+/* g(x) = Gaussian density */
+static double gauss_density(double x, double mu, double sigma)
+{
+    const double d = x - mu;
+    return exp(-(d * d) / (2.0 * sigma * sigma)) / (sqrt(2.0 * MFO_PI) * sigma);
+}
+
+/* dN1/dmu = g(a) - g(b);  dN1/dsigma = [(a-mu) g(a) - (b-mu) g(b)] / sigma */
+static double dnorm_gauss_dmu(double mu, double sigma, double a, double b)
+{
+    return gauss_density(a, mu, sigma) - gauss_density(b, mu, sigma);
+}
+static double dnorm_gauss_dsigma(double mu, double sigma, double a, double b)
+{
+    return ((a - mu) * gauss_density(a, mu, sigma) - (b - mu) * gauss_density(b, mu, sigma)) / sigma;
+}
+
+/* N2(tau), reading R6 */
+static double norm_exp(double tau, double a, double b)
+{
+    if (tau == 0.0) return b - a;
+    return exp(tau * a) * expm1(tau * (b - a)) / tau;
+}
+
+/* d ln N2 / d tau = mean of m under the truncated exponential, reading R6 */
+static double dlognorm_exp_dtau(double tau, double a, double b)
+{
+    const long double w = (long double)b - (long double)a;
+    const long double u = (long double)tau * w;
+    long double h;
+    if (fabsl(u) < 1e-2L) {
+        const long double u2 = u * u;
+        /* 1/(1-e^-u) - 1/u = 1/2 + u/12 - u^3/720 + u^5/30240 - u^7/1209600 + ... */
+        h = 0.5L + u * (1.0L / 12.0L + u2 * (-1.0L / 720.0L + u2 * (1.0L / 30240.0L + u2 * (-1.0L / 1209600.0L))));
+    } else {
+        h = -1.0L / expm1l(-u) - 1.0L / u;
+    }
+    return (double)((long double)a + w * h);
+}
+
+/* P and d ln P / d(f, mu, sigma, tau) for one event.  g may be NULL. */
+static double mass_event(double m, const double *lam, double a, double b, double *g)
+{
+    const double f = lam[0], mu = lam[1], sigma = lam[2], tau = lam[3];
+    const double G = gauss_density(m, mu, sigma);
+    const double N1 = norm_gauss(mu, sigma, a, b);
+    const double E = exp(tau * m);
+    const double N2 = norm_exp(tau, a, b);
+    const double S = f * G / N1;
+    const double B = (1.0 - f) * E / N2;
+    const double P = S + B;
+    if (g) {
+        g[0] = (G / N1 - E / N2) / P;
+        g[1] = S * ((m - mu) / (sigma * sigma) - dnorm_gauss_dmu(mu, sigma, a, b) / N1) / P;
+        g[2] = S * ((m - mu) * (m - mu) / (sigma * sigma * sigma) - 1.0 / sigma
+                    - dnorm_gauss_dsigma(mu, sigma, a, b) / N1) / P;
+        g[3] = B * (m - dlognorm_exp_dtau(tau, a, b)) / P;
+    }
+    return P;
+}
+
+/* ------------------------------------------------------------ angular, Eq. 4 */
+
+/* The eleven angular terms of Eq. 4 in the order printed, WITHOUT the
+ * coefficients: term[0..3] carry (1-FL), FL, (1-FL), -FL; term[4..10] carry
+ * S3, S4, S5, AFB, S7, S8, S9.  The 4/3 of the AFB term is kept with the term. */
+static void angular_terms(double cl, double ck, double phi, double t[11])
+{
+    const double cos2_l = cl * cl, cos2_k = ck * ck;
+    const double sin2_l = 1.0 - cos2_l, sin2_k = 1.0 - cos2_k; /* sin^2 theta */
+    const double sin_l = sqrt(sin2_l), sin_k = sqrt(sin2_k);   /* theta in [0,pi]: sin >= 0 */
+    const double cos2theta_l = 2.0 * cos2_l - 1.0;             /* cos 2theta_l */
+    const double sin2theta_l = 2.0 * sin_l * cl;               /* sin 2theta_l */
+    const double sin2theta_k = 2.0 * sin_k * ck;               /* sin 2theta_K */
+    t[0] = 0.75 * sin2_k;
+    t[1] = cos2_k;
+    t[2] = 0.25 * sin2_k * cos2theta_l;
+    t[3] = cos2_k * cos2theta_l;
+    t[4] = sin2_k * sin2_l * cos(2.0 * phi);
+    t[5] = sin2theta_k * sin2theta_l * cos(phi);
+    t[6] = sin2theta_k * sin_l * cos(phi);
+    t[7] = (4.0 / 3.0) * sin2_k * cl;
+    t[8] = sin2theta_k * sin_l * sin(phi);
+    t[9] = sin2theta_k * sin2theta_l * sin(phi);
+    t[10] = sin2_k * sin2_l * sin(2.0 * phi);
+}
+
+/* A(Omega) and dA/d(FL,S3,S4,S5,AFB,S7,S8,S9) (NOT divided by A).  dA may be NULL. */
+static double angular_value(double cl, double ck, double phi, const double *a, double *dA)
+{
+    const double c = 9.0 / (32.0 * MFO_PI);
+    double t[11];
+    angular_terms(cl, ck, phi, t);
+    const double FL = a[0];
+    double A = (1.0 - FL) * t[0] + FL * t[1] + (1.0 - FL) * t[2] - FL * t[3];
+    for (int k = 1; k < 8; ++k) A += a[k] * t[3 + k];
+    A *= c;
+    if (dA) {
+        dA[0] = c * (-t[0] + t[1] - t[2] - t[3]);
+        for (int k = 1; k < 8; ++k) dA[k] = c * t[3 + k];
+    }
+    return A;
+}
+
+static double angular_event(double cl, double ck, double phi, const double *lam, double *g)
+{
+    double dA[8];
+    const double A = angular_value(cl, ck, phi, lam, dA);
+    if (g)
+        for (int k = 0; k < 8; ++k) g[k] = dA[k] / A;
+    return A;
+}
+
+/* ------------------------------------------- 4D, BASELINE.json configs[3] */
+
+/* l(x; c1, c2) = 1/2 [1 + c1 P1(x) + c2 P2(x)], normalised on [-1,1] */
+static double legendre2(double x, double c1, double c2)
+{
+    return 0.5 * (1.0 + c1 * x + c2 * 0.5 * (3.0 * x * x - 1.0));
+}
+
+/* lambda = (f, mu, sigma, tau, FL..S9, cl1, cl2, ck1, ck2) */
+static double fourd_event(double m, double cl, double ck, double phi, const double *lam,
+                          double a, double b, double *g)
+{
+    const double f = lam[0], mu = lam[1], sigma = lam[2], tau = lam[3];
+    const double *ang = lam + 4;
+    const double cl1 = lam[12], cl2 = lam[13], ck1 = lam[14], ck2 = lam[15];
+    const double G = gauss_density(m, mu, sigma);
+    const double N1 = norm_gauss(mu, sigma, a, b);
+    const double E = exp(tau * m);
+    const double N2 = norm_exp(tau, a, b);
+    double dA[8];
+    const double A = angular_value(cl, ck, phi, ang, dA);
+    const double Ll = legendre2(cl, cl1, cl2), Lk = legendre2(ck, ck1, ck2);
+    const double L = Ll * Lk / (2.0 * MFO_PI);
+    const double S = f * (G / N1) * A;
+    const double B = (1.0 - f) * (E / N2) * L;
+    const double P = S + B;
+    if (g) {
+        g[0] = ((G / N1) * A - (E / N2) * L) / P;
+        g[1] = S * ((m - mu) / (sigma * sigma) - dnorm_gauss_dmu(mu, sigma, a, b) / N1) / P;
+        g[2] = S * ((m - mu) * (m - mu) / (sigma * sigma * sigma) - 1.0 / sigma
+                    - dnorm_gauss_dsigma(mu, sigma, a, b) / N1) / P;
+        g[3] = B * (m - dlognorm_exp_dtau(tau, a, b)) / P;
+        for (int k = 0; k < 8; ++k) g[4 + k] = f * (G / N1) * dA[k] / P;
+        const double Bm = (1.0 - f) * (E / N2) / (2.0 * MFO_PI);
+        g[12] = Bm * (0.5 * cl) * Lk / P;
+        g[13] = Bm * (0.5 * 0.5 * (3.0 * cl * cl - 1.0)) * Lk / P;
+        g[14] = Bm * Ll * (0.5 * ck) / P;
+        g[15] = Bm * Ll * (0.5 * 0.5 * (3.0 * ck * ck - 1.0)) / P;
+    }
+    return P;
+}
+
+/* ------------------------------------------------------------------- API */
+
+int mfo_nparams(int kind)
+{
+    return kind == MFO_MASS ? 4 : kind == MFO_ANGULAR ? 8 : kind == MFO_4D ? 16 : -1;
+}
+int mfo_ndim(int kind)
+{
+    return kind == MFO_MASS ? 1 : kind == MFO_ANGULAR ? 3 : kind == MFO_4D ? 4 : -1;
+}
+
+static double eval_event(int kind, const double *const *cols, int64_t i, const double *lam,
+                         double lo, double hi, double *g)
+{
+    switch (kind) {
+    case MFO_MASS: return mass_event(cols[0][i], lam, lo, hi, g);
+    case MFO_ANGULAR: return angular_event(cols[0][i], cols[1][i], cols[2][i], lam, g);
+    default: return fourd_event(cols[0][i], cols[1][i], cols[2][i], cols[3][i], lam, lo, hi, g);
+    }
+}
+
+/* Per-event P(x_i | lambda) and d ln P / d lambda_k (dlnp laid out [K][n], may be NULL). */
+int mfo_pdf(int kind, int64_t n, const double *const *cols, const double *lam, double lo,
+            double hi, double *p, double *dlnp)
+{
+    const int K = mfo_nparams(kind);
+    if (K < 0) return -1;
+    for (int64_t i = 0; i < n; ++i) {
+        double g[MFO_MAXK];
+        p[i] = eval_event(kind, cols, i, lam, lo, hi, dlnp ? g : NULL);
+        if (dlnp)
+            for (int k = 0; k < K; ++k) dlnp[(int64_t)k * n + i] = g[k];
+    }
+    return 0;
+}
+
+/* The two normalisations and their derivatives, exposed so that tests can pin them. */
+void mfo_mass_norms(const double *lam, double lo, double hi, double *out /*[5]*/)
+{
+    out[0] = norm_gauss(lam[1], lam[2], lo, hi);
+    out[1] = dnorm_gauss_dmu(lam[1], lam[2], lo, hi);
+    out[2] = dnorm_gauss_dsigma(lam[1], lam[2], lo, hi);
+    out[3] = norm_exp(lam[3], lo, hi);
+    out[4] = dlognorm_exp_dtau(lam[3], lo, hi);
+}
+
+/* The eleven terms of Eq. 4 times c = 9/(32 pi), exposed so that tests can pin them. */
+void mfo_angular_terms(double cl, double ck, double phi, double *out /*[11]*/)
+{
+    angular_terms(cl, ck, phi, out);
+    for (int j = 0; j < 11; ++j) out[j] *= 9.0 / (32.0 * MFO_PI);
+}
+
+static void chunk_sums(int kind, const double *const *cols, int64_t i0, int64_t i1, const double *lam,
+                       double lo, double hi, int K, int want_grad, long double *acc /*[K+1]*/, int64_t *nbad)
+{
+    for (int k = 0; k <= K; ++k) acc[k] = 0.0L;
+    int64_t bad = 0;
+    for (int64_t i = i0; i < i1; ++i) {
+        double g[MFO_MAXK];
+        const double P = eval_event(kind, cols, i, lam, lo, hi, want_grad ? g : NULL);
+        if (!(P > 0.0)) { ++bad; continue; }
+        acc[0] += (long double)log(P);
+        if (want_grad)
+            for (int k = 0; k < K; ++k) acc[1 + k] += (long double)g[k];
+    }
+    *nbad = bad;
+}
+
+/*
+ * -ln L and its gradient over n events (Eq. 1).  cols: ndim pointers to n doubles each.
+ * grad may be NULL.  Returns the number of events with P <= 0 or NaN (then *nll = +inf,
+ * grad = NaN), or -1 on a bad argument.
+ */
+int64_t mfo_nll_grad(int kind, int64_t n, const double *const *cols, const double *lam, double lo,
+                     double hi, int nthreads, double *nll, double *grad)
+{
+    const int K = mfo_nparams(kind);
+    if (K < 0 || n < 0) return -1;
+    if (nthreads < 1) nthreads = 1;
+    if (nthreads > 1024) nthreads = 1024;
+    long double part[1024][MFO_MAXK + 1];
+    int64_t bad[1024];
+    const int want_grad = grad != NULL;
+#ifdef _OPENMP
+#pragma omp parallel for num_threads(nthreads) schedule(static, 1)
+#endif
+    for (int c = 0; c < nthreads; ++c) {
+        const int64_t i0 = n * c / nthreads, i1 = n * (c + 1) / nthreads;
+        chunk_sums(kind, cols, i0, i1, lam, lo, hi, K, want_grad, part[c], &bad[c]);
+    }
+    long double tot[MFO_MAXK + 1];
+    int64_t nbad = 0;
+    for (int k = 0; k <= K; ++k) tot[k] = 0.0L;
+    for (int c = 0; c < nthreads; ++c) { /* chunk order: deterministic */
+        nbad += bad[c];
+        for (int k = 0; k <= K; ++k) tot[k] += part[c][k];
+    }
+    if (nbad) {
+        *nll = INFINITY;
+        if (grad) for (int k = 0; k < K; ++k) grad[k] = NAN;
+        return nbad;
+    }
+    *nll = (double)(-tot[0]);
+    if (grad) for (int k = 0; k < K; ++k) grad[k] = (double)(-tot[1 + k]);
+    return 0;
+}
+
+int mfo_max_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
