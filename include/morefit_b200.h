@@ -1,0 +1,187 @@
+/*
+ * morefit_b200.h — C-ABI boundary of the B200-native MoreFit hot path.
+ *
+ * The path: fused evaluation of the unbinned negative log-likelihood
+ *     -ln L(lambda) = - sum_i ln P(x_i | lambda)            (Eq. 1)
+ * and of its analytic gradient d(-ln L)/d lambda_k over N independent
+ * events, for the model families named in BASELINE.json, plus the host quasi-Newton fit
+ * driver that calls it.  SURVEY.md §8(a) lists the steps S0..S6, §8(b) this
+ * boundary.  Every step of the path runs in the library's own sm_100a kernels; there is no
+ * CPU fallback: without a CUDA device every compute entry point returns MF_ERR_CUDA.
+ *
+ * Conventions
+ *   * All floating point is IEEE double (kernelT = evalT = double).
+ *   * "host" / "device" beside a pointer says which memory it must point to.
+ *   * The library copies what it needs: every caller array may be freed on return.
+ *   * No call throws; every call returns an mf_status.  mf_last_error() gives a text for
+ *     the last non-OK status of that context (valid until the next call on the context).
+ *   * All device work of a context is enqueued on the CUDA stream given at creation
+ *     (borrowed, e.g. torch.cuda.current_stream().cuda_stream; NULL = the legacy default
+ *     stream).  Calls on one context must not be made concurrently from several threads.
+ *   * Results are bit-identical for identical inputs on the same GPU: per-thread, per-warp,
+ *     per-block and final sums are all taken in a fixed order (PAPER.md:65 uses Kahan
+ *     reduction kernels; here one compensated fixed-order pass).
+ */
+#ifndef MOREFIT_B200_H
+#define MOREFIT_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    MF_OK = 0,
+    MF_ERR_ARG = 1,          /* NULL pointer, wrong ndim / kind / size */
+    MF_ERR_CUDA = 2,         /* CUDA runtime error or no device; text in mf_last_error */
+    MF_ERR_OOM = 3,          /* host or device allocation failed */
+    MF_ERR_DATA_RANGE = 4,   /* an event is non-finite or outside [lo, hi] */
+    MF_ERR_PARAM_DOMAIN = 5, /* non-finite lambda, sigma <= 0 or f outside [0,1]: outputs untouched */
+    MF_NONPOSITIVE_PDF = 6   /* P(x_i|lambda) <= 0 or NaN for >= 1 event: nll = +inf, grad = NaN */
+} mf_status;
+
+/* Model families (BASELINE.json configs; parameter order = SURVEY.md §8(b)).
+ *   MF_MASS_GAUSS_EXP   ndim 1 (m), K = 4: f, mu, sigma, tau.            PAPER.md:83-88 (Eq. 2)
+ *   MF_ANGULAR_KSTMUMU  ndim 3 (cos theta_l, cos theta_K, phi), K = 8:
+ *                       FL, S3, S4, S5, AFB, S7, S8, S9.                 PAPER.md:116-118 (Eq. 4)
+ *   MF_MASS_X_ANGULAR   ndim 4 (m, cos theta_l, cos theta_K, phi), K = 16:
+ *                       f, mu, sigma, tau, the 8 angular, cl1, cl2, ck1, ck2
+ *                       P = f (G/N1) A + (1-f) (E/N2) L, L = l(cos theta_l) l(cos theta_K)/(2 pi),
+ *                       l(x; c1, c2) = 1/2 [1 + c1 x + c2 (3x^2-1)/2]   (BASELINE.json configs[3]) */
+typedef enum {
+    MF_MASS_GAUSS_EXP = 0,
+    MF_ANGULAR_KSTMUMU = 1,
+    MF_MASS_X_ANGULAR = 2
+} mf_model_kind;
+
+typedef enum { MF_HOST = 0, MF_DEVICE = 1 } mf_mem;
+
+#define MF_MAX_PARAMS 16
+#define MF_MAX_DIMS 4
+
+typedef struct mf_ctx mf_ctx;
+typedef struct mf_dataset mf_dataset;
+typedef struct mf_model mf_model;
+
+/* ---- context ------------------------------------------------------------------------- */
+
+/* Binds CUDA device `device` and the borrowed stream `cuda_stream` (a cudaStream_t, may be
+ * NULL).  *out is set only on MF_OK.  MF_ERR_CUDA if the device cannot be used. */
+mf_status mf_ctx_create(int device, void* cuda_stream, mf_ctx** out);
+/* Frees the context.  Datasets and models made from it must be destroyed first. */
+void mf_ctx_destroy(mf_ctx* ctx);
+/* Text of the last error on this context ("" if none).  Never NULL.  ctx may be NULL. */
+const char* mf_last_error(const mf_ctx* ctx);
+/* Number of this library's kernels launched on the context since creation (bench.py's
+ * gpu_launches claim is read from here). */
+int64_t mf_ctx_kernel_launches(const mf_ctx* ctx);
+
+/* ---- S0: data (PAPER.md:65 structure of arrays, padded) ------------ */
+
+/* Copies `ndim` event columns to the device as a padded structure of arrays.
+ *   columns[j]   host array of ndim pointers (always host); columns[j] points, in `where`
+ *                memory, to n_toys*n_events doubles, toy-major (toy t at [t*n_events, (t+1)*n_events)).
+ *   n_toys       1 for one dataset, T for T pseudo-experiments of n_events events each.
+ *   lo, hi       host, ndim each: closed ranges.  For the mass dimension they are the
+ *                normalisation range [m_a, m_b] of Eq. 2; the angular dimensions must be
+ *                [-1,1], [-1,1], [-pi,pi] (checked to 1e-12).  NULL = those defaults (mass: error).
+ * Each toy is padded to a multiple of 64 events with copies of its last event; padded
+ * lanes are predicated to contribute exactly 0 (SURVEY.md §8(c) reading 10).
+ * n_events == 0 is allowed (every sum is then 0).
+ * MF_ERR_DATA_RANGE if any event is NaN/inf or outside its range (checked on the device). */
+mf_status mf_dataset_upload(mf_ctx* ctx, int ndim, int64_t n_events, int64_t n_toys,
+                            const double* const* columns, mf_mem where,
+                            const double* lo, const double* hi, mf_dataset** out);
+void mf_dataset_destroy(mf_dataset* ds);
+int64_t mf_dataset_n_events(const mf_dataset* ds);
+int64_t mf_dataset_n_toys(const mf_dataset* ds);
+
+/* ---- S1: model (event-only precompute, Listing 4) --- */
+
+/* Binds a model family to a dataset (ndim must match the kind) and runs the event-only
+ * precompute once: for the angular kinds the nine merged basis columns
+ * h_k = 9/(32 pi) g_k are cached in HBM.  The model keeps its own
+ * reference to the dataset's device buffers: the dataset may be destroyed afterwards. */
+mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_dataset* ds, mf_model** out);
+void mf_model_destroy(mf_model* model);
+int mf_model_nparams(const mf_model* model);
+int64_t mf_model_n_events(const mf_model* model);
+int64_t mf_model_n_toys(const mf_model* model);
+
+/* ---- S2..S6: value + gradient ------------------------------------------------------------ */
+
+/* -ln L and d(-ln L)/d lambda_k at `lambda` over all events of a 1-toy dataset.
+ *   lambda  host, K doubles.   nll  host, 1 double.   grad  host, K doubles or NULL.
+ * One kernel launch (parameter-only constants of Eq. 3, are computed on
+ * the host and passed as kernel arguments), then one stream synchronise.
+ * MF_ERR_ARG if the dataset has n_toys != 1.  See mf_status for the domain / P<=0 cases. */
+mf_status mf_nll_grad(mf_model* model, const double* lambda, double* nll, double* grad);
+
+/* Same evaluation without a host synchronisation: enqueues the launch on the context's
+ * stream and writes K+2 doubles to out_dev (DEVICE): [-ln L, grad[0..K-1], n_bad], where
+ * n_bad is the number of events with P <= 0 (then -ln L = +inf, grad = NaN).  The
+ * parameter-domain check is still made on the host before the launch. */
+mf_status mf_nll_grad_async(mf_model* model, const double* lambda, double* out_dev);
+
+/* T pseudo-experiments at their own parameter points in ONE launch (BASELINE.json
+ * configs[4]): a CTA tile is (toy, event chunk); each CTA derives its toy's
+ * parameter-only constants in a short prologue.
+ *   n_toys   must equal the dataset's n_toys.
+ *   lambdas  host, [n_toys][K].   active  host, n_toys bytes or NULL (= all active).
+ *   nll      host, [n_toys].      grad    host, [n_toys][K] or NULL.
+ * Inactive toys are skipped and their outputs left untouched.  A toy whose lambda is
+ * outside the parameter domain, or that has an event with P <= 0, gets nll = +inf and
+ * grad = NaN; the call still returns MF_OK. */
+mf_status mf_nll_grad_batch(mf_model* model, int64_t n_toys, const double* lambdas,
+                            const uint8_t* active, double* nll, double* grad);
+
+/* ---- fit driver (host quasi-Newton over the GPU value+gradient) ------- */
+
+typedef struct {
+    int max_iter;          /* BFGS iterations (default 200) */
+    double edm_tol;        /* leave BFGS for the Newton polish when g^T H^-1 g / 2 < edm_tol (1e-5) */
+    double armijo_c1;      /* sufficient-decrease constant (1e-4) */
+    double backtrack;      /* step shrink factor (0.5) */
+    int max_backtracks;    /* (40) */
+    double polish_tol;     /* converged when max_k |Newton step_k| / sigma_k < polish_tol (1e-9) */
+    int max_polish;        /* finite-difference Hessians in the polish (8) */
+    int max_chord;         /* Newton steps per Hessian (8) */
+    double fd_rel;         /* first FD step: fd_rel * max(|lambda_k|, 1) (1e-5) */
+    double fd_sigma;       /* later FD steps: fd_sigma * sigma_k (1e-4) */
+} mf_fit_opts;
+
+/* Fills *opts with the defaults above. */
+void mf_fit_opts_default(mf_fit_opts* opts);
+
+typedef struct {
+    double lambda_hat[MF_MAX_PARAMS];               /* fitted parameters (fixed ones = start) */
+    double cov[MF_MAX_PARAMS * MF_MAX_PARAMS];      /* row-major K x K inverse Hessian (HESSE); 0 for fixed */
+    double nll_min;
+    int n_calls;                                    /* value+gradient evaluations used */
+    int n_iter;                                     /* BFGS iterations */
+    int converged;                                  /* 1 = polish criterion met */
+} mf_fit_result;
+
+/* Minimises -ln L from `start` (host, K).  fixed: host, K bytes (1 = keep at start; paper:
+ * the parameter `constant` flag) or NULL.  opts NULL = defaults.
+ * Algorithm (SURVEY.md §8(c) "Fit"): central-difference Hessian of the analytic gradient
+ * at the start point seeds the inverse metric; BFGS with Armijo backtracking that rejects
+ * domain errors and P<=0 points; then Newton steps on a fresh central-difference Hessian
+ * until the step is below polish_tol sigma; cov = H^-1.
+ * MF_ERR_PARAM_DOMAIN / MF_NONPOSITIVE_PDF if the start point itself is invalid. */
+mf_status mf_fit(mf_model* model, const double* start, const uint8_t* fixed,
+                 const mf_fit_opts* opts, mf_fit_result* result);
+
+/* Fits all T toys of the model's dataset concurrently: T independent fit states advance
+ * in lock step, one mf_nll_grad_batch launch per round with the finished toys masked out.
+ *   starts   host, [n_toys][K].   results  host, n_toys entries.
+ * A toy whose start point is invalid gets converged = 0 and n_calls = 1. */
+mf_status mf_fit_batch(mf_model* model, int64_t n_toys, const double* starts,
+                       const uint8_t* fixed, const mf_fit_opts* opts, mf_fit_result* results);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MOREFIT_B200_H */

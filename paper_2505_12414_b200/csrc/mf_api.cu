@@ -1,0 +1,446 @@
+// mf_api.cu — C-ABI entry points of include/morefit_b200.h: context, S0 upload, S1 model
+// creation, and the launches of the fused kernels (S2..S6).  The fit driver is mf_fit.cpp.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "mf_internal.h"
+#include "mf_kernels.cuh"
+
+using namespace mf;
+
+mf_status mf_fail(mf_ctx* ctx, mf_status st, const std::string& msg)
+{
+    if (ctx) ctx->err = msg;
+    return st;
+}
+
+#define MF_CUDA(ctx, call)                                                                              \
+    do {                                                                                                \
+        cudaError_t e__ = (call);                                                                       \
+        if (e__ != cudaSuccess) {                                                                       \
+            const mf_status st__ = (e__ == cudaErrorMemoryAllocation) ? MF_ERR_OOM : MF_ERR_CUDA;       \
+            return mf_fail(ctx, st__, std::string(#call) + ": " + cudaGetErrorString(e__));             \
+        }                                                                                               \
+    } while (0)
+
+static inline int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
+
+static void devbuf_release(mf_devbuf* b)
+{
+    if (b && --b->refs == 0) {
+        if (b->p) cudaFree(b->p);
+        delete b;
+    }
+}
+
+// ------------------------------------------------------------------------------ context
+
+extern "C" mf_status mf_ctx_create(int device, void* cuda_stream, mf_ctx** out)
+{
+    if (!out) return MF_ERR_ARG;
+    int count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) {
+        cudaGetLastError();
+        return MF_ERR_CUDA;
+    }
+    mf_ctx* ctx = new (std::nothrow) mf_ctx();
+    if (!ctx) return MF_ERR_OOM;
+    ctx->device = device;
+    ctx->stream = static_cast<cudaStream_t>(cuda_stream);
+    if (cudaSetDevice(device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) {
+        cudaGetLastError();
+        delete ctx;
+        return MF_ERR_CUDA;
+    }
+    *out = ctx;
+    return MF_OK;
+}
+
+extern "C" void mf_ctx_destroy(mf_ctx* ctx) { delete ctx; }
+
+extern "C" const char* mf_last_error(const mf_ctx* ctx) { return ctx ? ctx->err.c_str() : ""; }
+
+extern "C" int64_t mf_ctx_kernel_launches(const mf_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+// ------------------------------------------------------------------------------ S0: data
+
+extern "C" mf_status mf_dataset_upload(mf_ctx* ctx, int ndim, int64_t n_events, int64_t n_toys,
+                                       const double* const* columns, mf_mem where, const double* lo,
+                                       const double* hi, mf_dataset** out)
+{
+    if (!ctx || !out || !columns) return mf_fail(ctx, MF_ERR_ARG, "mf_dataset_upload: NULL argument");
+    if (!(ndim == 1 || ndim == 3 || ndim == 4) || n_events < 0 || n_toys < 1)
+        return mf_fail(ctx, MF_ERR_ARG, "mf_dataset_upload: ndim must be 1, 3 or 4; n_events >= 0; n_toys >= 1");
+    for (int j = 0; j < ndim; ++j)
+        if (!columns[j] && n_events > 0) return mf_fail(ctx, MF_ERR_ARG, "mf_dataset_upload: NULL column");
+    const bool has_mass = (ndim == 1 || ndim == 4);
+    if (has_mass && (!lo || !hi)) return mf_fail(ctx, MF_ERR_ARG, "mf_dataset_upload: the mass range lo/hi is required");
+    double rlo[MF_MAX_DIMS], rhi[MF_MAX_DIMS];
+    const double ang_lo[3] = {-1.0, -1.0, -kPi}, ang_hi[3] = {1.0, 1.0, kPi};
+    for (int j = 0; j < ndim; ++j) {
+        const bool is_ang = (ndim == 3) || (ndim == 4 && j > 0);
+        const int ja = (ndim == 3) ? j : j - 1;
+        if (is_ang) {
+            rlo[j] = ang_lo[ja];
+            rhi[j] = ang_hi[ja];
+            if (lo && hi && (std::fabs(lo[j] - rlo[j]) > 1e-12 || std::fabs(hi[j] - rhi[j]) > 1e-12))
+                return mf_fail(ctx, MF_ERR_ARG, "mf_dataset_upload: angular ranges must be [-1,1], [-1,1], [-pi,pi]");
+        } else {
+            rlo[j] = lo[j];
+            rhi[j] = hi[j];
+            if (!(std::isfinite(rlo[j]) && std::isfinite(rhi[j]) && rlo[j] < rhi[j]))
+                return mf_fail(ctx, MF_ERR_ARG, "mf_dataset_upload: mass range must be finite with lo < hi");
+        }
+    }
+    MF_CUDA(ctx, cudaSetDevice(ctx->device));
+
+    mf_dataset* ds = new (std::nothrow) mf_dataset();
+    mf_devbuf* buf = new (std::nothrow) mf_devbuf();
+    if (!ds || !buf) {
+        delete ds;
+        delete buf;
+        return mf_fail(ctx, MF_ERR_OOM, "mf_dataset_upload: host allocation failed");
+    }
+    ds->ctx = ctx;
+    ds->ndim = ndim;
+    ds->n_events = n_events;
+    ds->n_pad = round_up(n_events, kItem);
+    ds->n_toys = n_toys;
+    for (int j = 0; j < ndim; ++j) {
+        ds->lo[j] = rlo[j];
+        ds->hi[j] = rhi[j];
+    }
+    ds->raw = buf;
+    const int64_t per_dim = ds->n_pad * n_toys;
+    buf->bytes = (size_t)std::max<int64_t>(per_dim * ndim, 1) * sizeof(double);
+    unsigned long long* d_count = nullptr;
+    auto cleanup = [&]() {
+        if (d_count) cudaFree(d_count);
+        devbuf_release(buf);
+        delete ds;
+    };
+#define MF_CUDA_C(call)                                                                               \
+    do {                                                                                              \
+        cudaError_t e__ = (call);                                                                     \
+        if (e__ != cudaSuccess) {                                                                     \
+            cleanup();                                                                                \
+            const mf_status st__ = (e__ == cudaErrorMemoryAllocation) ? MF_ERR_OOM : MF_ERR_CUDA;     \
+            return mf_fail(ctx, st__, std::string(#call) + ": " + cudaGetErrorString(e__));           \
+        }                                                                                             \
+    } while (0)
+    MF_CUDA_C(cudaMalloc(&buf->p, buf->bytes));
+    MF_CUDA_C(cudaMalloc(&d_count, sizeof(unsigned long long)));
+    MF_CUDA_C(cudaMemsetAsync(d_count, 0, sizeof(unsigned long long), ctx->stream));
+    if (n_events > 0) {
+        const cudaMemcpyKind kind = (where == MF_HOST) ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+        for (int j = 0; j < ndim; ++j) {
+            double* dst = buf->p + (int64_t)j * per_dim;
+            // toy rows of n_events doubles -> rows of n_pad doubles
+            MF_CUDA_C(cudaMemcpy2DAsync(dst, (size_t)ds->n_pad * sizeof(double), columns[j],
+                                        (size_t)n_events * sizeof(double), (size_t)n_events * sizeof(double),
+                                        (size_t)n_toys, kind, ctx->stream));
+        }
+        if (ds->n_pad > n_events) {
+            const int64_t rows = (int64_t)ndim * n_toys;
+            const int64_t work = rows * (ds->n_pad - n_events);
+            const int grid = (int)std::min<int64_t>((work + 255) / 256, 4096);
+            pad_rows_kernel<<<grid, 256, 0, ctx->stream>>>(buf->p, rows, n_events, ds->n_pad);
+            ++ctx->launches;
+        }
+        for (int j = 0; j < ndim; ++j) {
+            const int grid = (int)std::min<int64_t>((n_toys * n_events + 255) / 256, 8 * (int64_t)ctx->sm_count);
+            range_check_kernel<<<grid, 256, 0, ctx->stream>>>(buf->p + (int64_t)j * per_dim, n_toys, n_events, ds->n_pad,
+                                                              rlo[j], rhi[j], d_count);
+            ++ctx->launches;
+        }
+        MF_CUDA_C(cudaGetLastError());
+    }
+    unsigned long long n_out = 0;
+    MF_CUDA_C(cudaMemcpyAsync(&n_out, d_count, sizeof(n_out), cudaMemcpyDeviceToHost, ctx->stream));
+    MF_CUDA_C(cudaStreamSynchronize(ctx->stream));
+#undef MF_CUDA_C
+    cudaFree(d_count);
+    d_count = nullptr;
+    if (n_out) {
+        cleanup();
+        return mf_fail(ctx, MF_ERR_DATA_RANGE,
+                       "mf_dataset_upload: " + std::to_string(n_out) + " values are non-finite or outside their range");
+    }
+    *out = ds;
+    return MF_OK;
+}
+
+extern "C" void mf_dataset_destroy(mf_dataset* ds)
+{
+    if (!ds) return;
+    devbuf_release(ds->raw);
+    delete ds;
+}
+extern "C" int64_t mf_dataset_n_events(const mf_dataset* ds) { return ds ? ds->n_events : 0; }
+extern "C" int64_t mf_dataset_n_toys(const mf_dataset* ds) { return ds ? ds->n_toys : 0; }
+
+// ------------------------------------------------------------------------------ S1: model
+
+extern "C" void mf_model_destroy(mf_model* m)
+{
+    if (!m) return;
+    cudaFree(m->cache);
+    cudaFree(m->partials);
+    cudaFree(m->bad_partials);
+    cudaFree(m->ticket);
+    cudaFree(m->b_partials);
+    cudaFree(m->b_bad);
+    cudaFree(m->d_lam);
+    cudaFree(m->d_ids);
+    cudaFree(m->d_bout);
+    if (m->h_out) cudaFreeHost(m->h_out);
+    if (m->h_lam) cudaFreeHost(m->h_lam);
+    if (m->h_ids) cudaFreeHost(m->h_ids);
+    if (m->h_bout) cudaFreeHost(m->h_bout);
+    devbuf_release(m->raw);
+    cudaGetLastError();
+    delete m;
+}
+
+extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_dataset* ds, mf_model** out)
+{
+    if (!ctx || !ds || !out) return mf_fail(ctx, MF_ERR_ARG, "mf_model_create: NULL argument");
+    if (ds->ctx != ctx) return mf_fail(ctx, MF_ERR_ARG, "mf_model_create: dataset belongs to another context");
+    int K, ncol, ndim;
+    switch (kind) {
+    case MF_MASS_GAUSS_EXP: K = 4, ncol = 1, ndim = 1; break;
+    case MF_ANGULAR_KSTMUMU: K = 8, ncol = 9, ndim = 3; break;
+    case MF_MASS_X_ANGULAR: K = 16, ncol = 12, ndim = 4; break;
+    default: return mf_fail(ctx, MF_ERR_ARG, "mf_model_create: unknown model kind");
+    }
+    if (ds->ndim != ndim) return mf_fail(ctx, MF_ERR_ARG, "mf_model_create: dataset ndim does not match the model kind");
+    MF_CUDA(ctx, cudaSetDevice(ctx->device));
+    mf_model* m = new (std::nothrow) mf_model();
+    if (!m) return mf_fail(ctx, MF_ERR_OOM, "mf_model_create: host allocation failed");
+    m->ctx = ctx;
+    m->kind = kind;
+    m->K = K;
+    m->nacc = K + 1;
+    m->ncol = ncol;
+    m->n_events = ds->n_events;
+    m->n_pad = ds->n_pad;
+    m->n_toys = ds->n_toys;
+    m->ma = ds->lo[0];
+    m->mb = ds->hi[0];
+    m->raw = ds->raw;
+    ++m->raw->refs;
+#define MF_CUDA_M(call)                                                                               \
+    do {                                                                                              \
+        cudaError_t e__ = (call);                                                                     \
+        if (e__ != cudaSuccess) {                                                                     \
+            mf_model_destroy(m);                                                                      \
+            const mf_status st__ = (e__ == cudaErrorMemoryAllocation) ? MF_ERR_OOM : MF_ERR_CUDA;     \
+            return mf_fail(ctx, st__, std::string(#call) + ": " + cudaGetErrorString(e__));           \
+        }                                                                                             \
+    } while (0)
+    const int64_t per_dim = m->n_pad * m->n_toys;
+    const double* raw = m->raw->p;
+    if (kind == MF_MASS_GAUSS_EXP) {
+        m->col[0] = raw;
+    } else {
+        // S1: cache the nine merged angular basis columns
+        MF_CUDA_M(cudaMalloc(&m->cache, (size_t)std::max<int64_t>(9 * per_dim, 1) * sizeof(double)));
+        const int a0 = (kind == MF_ANGULAR_KSTMUMU) ? 0 : 1;  // first angular dimension
+        if (per_dim > 0) {
+            const int grid = (int)std::min<int64_t>((per_dim + 255) / 256, 16 * (int64_t)ctx->sm_count);
+            angular_precompute_kernel<<<grid, 256, 0, ctx->stream>>>(raw + (a0 + 0) * per_dim, raw + (a0 + 1) * per_dim,
+                                                                     raw + (a0 + 2) * per_dim, m->cache, per_dim);
+            ++ctx->launches;
+            MF_CUDA_M(cudaGetLastError());
+        }
+        int c = 0;
+        if (kind == MF_MASS_X_ANGULAR) {
+            m->col[c++] = raw;                // m
+            m->col[c++] = raw + 1 * per_dim;  // cos theta_l
+            m->col[c++] = raw + 2 * per_dim;  // cos theta_K
+        }
+        for (int k = 0; k < 9; ++k) m->col[c++] = m->cache + k * per_dim;
+    }
+    // launch geometry: persistent-style grid, 2 CTAs per SM, never more CTAs than 8-warp groups of items
+    const int64_t n_items = m->n_pad / kItem;
+    m->grid = (int)std::max<int64_t>(1, std::min<int64_t>((n_items + kWarps - 1) / kWarps, 2 * (int64_t)ctx->sm_count));
+    // batch geometry: one CTA per toy up to 32768 events per toy, else split
+    m->chunks = (int)std::max<int64_t>(1, std::min<int64_t>((m->n_pad + 32767) / 32768, 64));
+    MF_CUDA_M(cudaMalloc(&m->partials, sizeof(double) * m->nacc * m->grid));
+    MF_CUDA_M(cudaMalloc(&m->bad_partials, sizeof(unsigned) * m->grid));
+    MF_CUDA_M(cudaMalloc(&m->ticket, sizeof(unsigned) * (1 + m->n_toys)));
+    MF_CUDA_M(cudaMemsetAsync(m->ticket, 0, sizeof(unsigned) * (1 + m->n_toys), ctx->stream));
+    MF_CUDA_M(cudaHostAlloc(&m->h_out, sizeof(double) * (MF_MAX_PARAMS + 2), cudaHostAllocMapped));
+    MF_CUDA_M(cudaHostGetDevicePointer(&m->d_out_mapped, m->h_out, 0));
+    if (m->n_toys > 1) {
+        const int64_t T = m->n_toys;
+        if (m->chunks > 1) {
+            MF_CUDA_M(cudaMalloc(&m->b_partials, sizeof(double) * T * m->nacc * m->chunks));
+            MF_CUDA_M(cudaMalloc(&m->b_bad, sizeof(unsigned) * T * m->chunks));
+        }
+        MF_CUDA_M(cudaMalloc(&m->d_lam, sizeof(double) * T * K));
+        MF_CUDA_M(cudaMalloc(&m->d_ids, sizeof(int) * T));
+        MF_CUDA_M(cudaMalloc(&m->d_bout, sizeof(double) * T * (K + 2)));
+        MF_CUDA_M(cudaHostAlloc(&m->h_lam, sizeof(double) * T * K, cudaHostAllocDefault));
+        MF_CUDA_M(cudaHostAlloc(&m->h_ids, sizeof(int) * T, cudaHostAllocDefault));
+        MF_CUDA_M(cudaHostAlloc(&m->h_bout, sizeof(double) * T * (K + 2), cudaHostAllocDefault));
+    }
+    MF_CUDA_M(cudaStreamSynchronize(ctx->stream));
+#undef MF_CUDA_M
+    *out = m;
+    return MF_OK;
+}
+
+extern "C" int mf_model_nparams(const mf_model* m) { return m ? m->K : 0; }
+extern "C" int64_t mf_model_n_events(const mf_model* m) { return m ? m->n_events : 0; }
+extern "C" int64_t mf_model_n_toys(const mf_model* m) { return m ? m->n_toys : 0; }
+
+// ------------------------------------------------------------------------------ S2..S6
+
+template <class M>
+static bool host_consts(const mf_model* m, const double* lam, typename M::Consts& c);
+template <>
+bool host_consts<MassModel>(const mf_model* m, const double* lam, MassConsts& c)
+{
+    return mass_consts(lam, m->ma, m->mb, c);
+}
+template <>
+bool host_consts<AngularModel>(const mf_model*, const double* lam, AngularConsts& c)
+{
+    return angular_consts(lam, c);
+}
+template <>
+bool host_consts<FourDModel>(const mf_model* m, const double* lam, FourDConsts& c)
+{
+    return fourd_consts(lam, m->ma, m->mb, c);
+}
+
+template <class M>
+static mf_status launch_single(mf_model* m, const double* lam, double* out_dev)
+{
+    mf_ctx* ctx = m->ctx;
+    EvalArgs<M> a;
+    if (!host_consts<M>(m, lam, a.c)) return mf_fail(ctx, MF_ERR_PARAM_DOMAIN, "lambda outside the parameter domain");
+    for (int i = 0; i < M::NCOL; ++i) a.col[i] = m->col[i];
+    a.n = m->n_events;
+    a.n_items = m->n_pad / kItem;
+    a.partials = m->partials;
+    a.bad_partials = m->bad_partials;
+    a.ticket = m->ticket;
+    a.out = out_dev;
+    nll_grad_kernel<M><<<m->grid, kBlock, 0, ctx->stream>>>(a);
+    ++ctx->launches;
+    MF_CUDA(ctx, cudaGetLastError());
+    return MF_OK;
+}
+
+static mf_status dispatch_single(mf_model* m, const double* lam, double* out_dev)
+{
+    switch (m->kind) {
+    case MF_MASS_GAUSS_EXP: return launch_single<MassModel>(m, lam, out_dev);
+    case MF_ANGULAR_KSTMUMU: return launch_single<AngularModel>(m, lam, out_dev);
+    default: return launch_single<FourDModel>(m, lam, out_dev);
+    }
+}
+
+extern "C" mf_status mf_nll_grad_async(mf_model* m, const double* lambda, double* out_dev)
+{
+    if (!m || !lambda || !out_dev) return mf_fail(m ? m->ctx : nullptr, MF_ERR_ARG, "mf_nll_grad_async: NULL argument");
+    if (m->n_toys != 1) return mf_fail(m->ctx, MF_ERR_ARG, "mf_nll_grad_async: dataset has n_toys != 1; use mf_nll_grad_batch");
+    return dispatch_single(m, lambda, out_dev);
+}
+
+extern "C" mf_status mf_nll_grad(mf_model* m, const double* lambda, double* nll, double* grad)
+{
+    if (!m || !lambda || !nll) return mf_fail(m ? m->ctx : nullptr, MF_ERR_ARG, "mf_nll_grad: NULL argument");
+    if (m->n_toys != 1) return mf_fail(m->ctx, MF_ERR_ARG, "mf_nll_grad: dataset has n_toys != 1; use mf_nll_grad_batch");
+    mf_ctx* ctx = m->ctx;
+    const mf_status st = dispatch_single(m, lambda, m->d_out_mapped);  // the last CTA writes to mapped pinned memory
+    if (st != MF_OK) return st;
+    MF_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    *nll = m->h_out[0];
+    if (grad) std::memcpy(grad, m->h_out + 1, sizeof(double) * m->K);
+    if (m->h_out[m->K + 1] != 0.0)
+        return mf_fail(ctx, MF_NONPOSITIVE_PDF,
+                       "P <= 0 for " + std::to_string((long long)m->h_out[m->K + 1]) + " events at this lambda");
+    return MF_OK;
+}
+
+template <class M>
+static mf_status launch_batch(mf_model* m, int n_active)
+{
+    mf_ctx* ctx = m->ctx;
+    BatchArgs<M> a;
+    for (int i = 0; i < M::NCOL; ++i) a.col[i] = m->col[i];
+    a.toy_stride = m->n_pad;
+    a.n = m->n_events;
+    a.n_items = m->n_pad / kItem;
+    a.chunks = m->chunks;
+    a.ma = m->ma;
+    a.mb = m->mb;
+    a.lam = m->d_lam;
+    a.ids = m->d_ids;
+    a.partials = m->b_partials;
+    a.bad_partials = m->b_bad;
+    a.ticket = m->ticket + 1;
+    a.out = m->d_bout;
+    nll_grad_batch_kernel<M><<<n_active * m->chunks, kBlock, 0, ctx->stream>>>(a);
+    ++ctx->launches;
+    MF_CUDA(ctx, cudaGetLastError());
+    return MF_OK;
+}
+
+extern "C" mf_status mf_nll_grad_batch(mf_model* m, int64_t n_toys, const double* lambdas, const uint8_t* active,
+                                       double* nll, double* grad)
+{
+    if (!m || !lambdas || !nll) return mf_fail(m ? m->ctx : nullptr, MF_ERR_ARG, "mf_nll_grad_batch: NULL argument");
+    mf_ctx* ctx = m->ctx;
+    if (n_toys != m->n_toys) return mf_fail(ctx, MF_ERR_ARG, "mf_nll_grad_batch: n_toys does not match the dataset");
+    if (m->n_toys < 2 && !m->d_lam) {
+        // a 1-toy dataset evaluated through the batch entry: same result as mf_nll_grad
+        if (active && !active[0]) return MF_OK;
+        double g[MF_MAX_PARAMS];
+        const mf_status st = mf_nll_grad(m, lambdas, nll, g);
+        if (st == MF_ERR_PARAM_DOMAIN || st == MF_NONPOSITIVE_PDF) {
+            *nll = INFINITY;
+            if (grad) for (int k = 0; k < m->K; ++k) grad[k] = NAN;
+            return MF_OK;
+        }
+        if (st == MF_OK && grad) std::memcpy(grad, g, sizeof(double) * m->K);
+        return st;
+    }
+    const int K = m->K;
+    int n_active = 0;
+    for (int64_t t = 0; t < n_toys; ++t) {
+        if (active && !active[t]) continue;
+        m->h_ids[n_active] = (int)t;
+        std::memcpy(m->h_lam + (int64_t)n_active * K, lambdas + t * K, sizeof(double) * K);
+        ++n_active;
+    }
+    if (n_active == 0) return MF_OK;
+    MF_CUDA(ctx, cudaMemcpyAsync(m->d_lam, m->h_lam, sizeof(double) * n_active * K, cudaMemcpyHostToDevice, ctx->stream));
+    MF_CUDA(ctx, cudaMemcpyAsync(m->d_ids, m->h_ids, sizeof(int) * n_active, cudaMemcpyHostToDevice, ctx->stream));
+    mf_status st;
+    switch (m->kind) {
+    case MF_MASS_GAUSS_EXP: st = launch_batch<MassModel>(m, n_active); break;
+    case MF_ANGULAR_KSTMUMU: st = launch_batch<AngularModel>(m, n_active); break;
+    default: st = launch_batch<FourDModel>(m, n_active); break;
+    }
+    if (st != MF_OK) return st;
+    MF_CUDA(ctx, cudaMemcpyAsync(m->h_bout, m->d_bout, sizeof(double) * n_active * (K + 2), cudaMemcpyDeviceToHost,
+                                 ctx->stream));
+    MF_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    for (int s = 0; s < n_active; ++s) {
+        const int64_t t = m->h_ids[s];
+        const double* o = m->h_bout + (int64_t)s * (K + 2);
+        nll[t] = o[0];
+        if (grad) std::memcpy(grad + t * K, o + 1, sizeof(double) * K);
+    }
+    return MF_OK;
+}

@@ -1,0 +1,66 @@
+// mf_internal.h — host-side objects behind the opaque handles of include/morefit_b200.h.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <string>
+
+#include "../../include/morefit_b200.h"
+
+struct mf_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    int sm_count = 0;
+    int64_t launches = 0;
+    std::string err;
+};
+
+// Reference-counted device buffer so that a model can outlive the dataset handle.
+struct mf_devbuf {
+    double* p = nullptr;
+    size_t bytes = 0;
+    int refs = 1;
+};
+
+struct mf_dataset {
+    mf_ctx* ctx = nullptr;
+    int ndim = 0;
+    int64_t n_events = 0;  // per toy
+    int64_t n_pad = 0;     // per toy, multiple of 64
+    int64_t n_toys = 1;
+    double lo[MF_MAX_DIMS] = {0, 0, 0, 0}, hi[MF_MAX_DIMS] = {0, 0, 0, 0};
+    mf_devbuf* raw = nullptr;  // [ndim][n_toys][n_pad]
+};
+
+constexpr int MF_MAX_COLS = 12;
+
+struct mf_model {
+    mf_ctx* ctx = nullptr;
+    mf_model_kind kind = MF_MASS_GAUSS_EXP;
+    int K = 0, nacc = 0, ncol = 0;
+    int64_t n_events = 0, n_pad = 0, n_toys = 1;
+    double ma = 0, mb = 0;            // mass normalisation range [m_a, m_b]
+    mf_devbuf* raw = nullptr;         // shared with the dataset
+    double* cache = nullptr;          // [9][n_toys][n_pad] angular basis columns (S1), or NULL
+    const double* col[MF_MAX_COLS] = {};  // column base pointers, stride between toys = n_pad
+    // single-dataset evaluation
+    int grid = 1;                     // CTAs of the fused kernel
+    double* partials = nullptr;       // device [nacc][grid]
+    unsigned* bad_partials = nullptr; // device [grid]
+    unsigned* ticket = nullptr;       // device, 1 (single) + n_toys (batch)
+    double* h_out = nullptr;          // pinned + mapped host, MF_MAX_PARAMS+2
+    double* d_out_mapped = nullptr;   // device alias of h_out
+    // batched evaluation
+    int chunks = 1;                   // CTAs per toy
+    double* b_partials = nullptr;     // device [n_toys][nacc][chunks] (chunks > 1 only)
+    unsigned* b_bad = nullptr;        // device [n_toys][chunks]
+    double* d_lam = nullptr;          // device [n_toys][K]
+    int* d_ids = nullptr;             // device [n_toys]
+    double* d_bout = nullptr;         // device [n_toys][K+2]
+    double* h_lam = nullptr;          // pinned [n_toys][K]
+    int* h_ids = nullptr;             // pinned [n_toys]
+    double* h_bout = nullptr;         // pinned [n_toys][K+2]
+};
+
+// Sets ctx->err and returns st (mf_api.cu).
+mf_status mf_fail(mf_ctx* ctx, mf_status st, const std::string& msg);

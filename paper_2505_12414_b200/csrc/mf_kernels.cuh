@@ -1,0 +1,368 @@
+// mf_kernels.cuh — the fused NLL + gradient kernels (S3..S6 of SURVEY.md §8(a)).
+//
+// Work decomposition (both kernels).  The unit of work is a WARP ITEM: 64 consecutive
+// events, lane l owning events 2l and 2l+1, read from every column as ONE coalesced
+// 16-byte load per lane (512 contiguous bytes per warp per column; PAPER.md:65 structure
+// of arrays).  Items are dealt block-cyclically — item j goes to CTA j % G, warp
+// (j / G) % 8 — so that the leftover of the last round spreads over all SMs instead of
+// queueing behind a few CTAs.  Each thread keeps K+1 plain fp64 sums over its few dozen
+// events (SURVEY.md §7 "register budget"); compensation is applied where the long sums
+// are: across block partials (Kahan, fixed order).
+//
+// Reduction (S4, S5; PAPER.md:65 does this with repeated Kahan reduction kernels, each a
+// submission — here it is part of the same launch):
+//   thread sums -> xor-shuffle tree per warp -> 8 warp sums added in warp order ->
+//   block partial in global memory -> the CTA that takes the last ticket combines all
+//   block partials: lane l Kahan-sums partials l, l+32, ... in index order, the 32
+//   (sum, compensation) pairs are merged by a fixed two-sum tree.
+// The order never depends on which CTA finishes last, so results are bit-reproducible.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "mf_models.cuh"
+
+namespace mf {
+
+constexpr int kBlock = 256;
+constexpr int kWarps = kBlock / 32;
+constexpr int kItem = 64;  // events per warp item
+
+template <class M>
+struct EvalArgs {
+    const double* col[M::NCOL];  // column bases (this toy's row for the single kernel)
+    int64_t n;                   // valid events
+    int64_t n_items;             // n_pad / 64
+    typename M::Consts c;        // parameter-only constants (S2), computed on the host
+    double* partials;            // [NACC][gridDim.x]
+    unsigned* bad_partials;      // [gridDim.x]
+    unsigned* ticket;            // zero on entry, reset to zero by the last CTA
+    double* out;                 // [K+2]: -lnL, grad, n_bad
+};
+
+template <class M>
+struct BatchArgs {
+    const double* col[M::NCOL];  // column bases of toy 0; toy t is at + t * toy_stride
+    int64_t toy_stride;          // n_pad
+    int64_t n;                   // valid events per toy
+    int64_t n_items;             // n_pad / 64 per toy
+    int chunks;                  // CTAs per toy
+    double ma, mb;               // mass range for the constants prologue
+    const double* lam;           // [n_active][K]
+    const int* ids;              // [n_active] toy index of each active slot
+    double* partials;            // [n_active][NACC][chunks]   (chunks > 1)
+    unsigned* bad_partials;      // [n_active][chunks]
+    unsigned* ticket;            // [n_active]
+    double* out;                 // [n_active][K+2]
+};
+
+template <class M>
+__device__ __forceinline__ bool make_consts(const double* lam, double ma, double mb, typename M::Consts& c);
+template <>
+__device__ __forceinline__ bool make_consts<MassModel>(const double* lam, double ma, double mb, MassConsts& c)
+{
+    return mass_consts(lam, ma, mb, c);
+}
+template <>
+__device__ __forceinline__ bool make_consts<AngularModel>(const double* lam, double, double, AngularConsts& c)
+{
+    return angular_consts(lam, c);
+}
+template <>
+__device__ __forceinline__ bool make_consts<FourDModel>(const double* lam, double ma, double mb, FourDConsts& c)
+{
+    return fourd_consts(lam, ma, mb, c);
+}
+
+// ---- S3: the event loop of one warp ---------------------------------------------------------
+
+template <class M>
+__device__ __forceinline__ void load_item(const double* const* col, int64_t j, int lane, double* xa, double* xb)
+{
+#pragma unroll
+    for (int c = 0; c < M::NCOL; ++c) {
+        const double2 v = __ldg(reinterpret_cast<const double2*>(col[c] + kItem * j) + lane);
+        xa[c] = v.x;
+        xb[c] = v.y;
+    }
+}
+
+// Items j0, j0 + step, j0 + 2 step, ... < n_items; only item n_items - 1 can be ragged.
+template <class M>
+__device__ __forceinline__ void accumulate(const double* const* col, int64_t n, int64_t n_items, int64_t j0,
+                                           int64_t step, const typename M::Consts& c, double* acc, unsigned& bad)
+{
+    const int lane = threadIdx.x & 31;
+    int64_t j = j0;
+    for (; j + step < n_items; j += 2 * step) {
+        double xa[M::NCOL], xb[M::NCOL], ya[M::NCOL], yb[M::NCOL];
+        load_item<M>(col, j, lane, xa, xb);
+        load_item<M>(col, j + step, lane, ya, yb);
+        M::template event<false>(xa, c, acc, bad, true);
+        M::template event<false>(xb, c, acc, bad, true);
+        if (kItem * (j + step + 1) <= n) {
+            M::template event<false>(ya, c, acc, bad, true);
+            M::template event<false>(yb, c, acc, bad, true);
+        } else {
+            const int64_t e = kItem * (j + step) + 2 * lane;
+            M::template event<true>(ya, c, acc, bad, e < n);
+            M::template event<true>(yb, c, acc, bad, e + 1 < n);
+        }
+    }
+    if (j < n_items) {
+        double xa[M::NCOL], xb[M::NCOL];
+        load_item<M>(col, j, lane, xa, xb);
+        if (kItem * (j + 1) <= n) {
+            M::template event<false>(xa, c, acc, bad, true);
+            M::template event<false>(xb, c, acc, bad, true);
+        } else {
+            const int64_t e = kItem * j + 2 * lane;
+            M::template event<true>(xa, c, acc, bad, e < n);
+            M::template event<true>(xb, c, acc, bad, e + 1 < n);
+        }
+    }
+}
+
+// ---- S4: thread -> warp -> block ---------------------------------------------------------------
+
+// After the call threads 0..NACC-1 hold the block sum of quantity threadIdx.x, thread NACC the
+// block's bad-event count (in *bad_out).
+template <int NACC>
+__device__ __forceinline__ double block_reduce(double* acc, unsigned bad, double (*sm)[NACC], unsigned* sm_bad,
+                                               unsigned* bad_out)
+{
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < NACC; ++k) {
+        double v = acc[k];
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+        acc[k] = v;
+    }
+    bad = __reduce_add_sync(0xffffffffu, bad);
+    if (lane == 0) {
+#pragma unroll
+        for (int k = 0; k < NACC; ++k) sm[w][k] = acc[k];
+        sm_bad[w] = bad;
+    }
+    __syncthreads();
+    double s = 0.0;
+    if (threadIdx.x < NACC) {
+#pragma unroll
+        for (int i = 0; i < kWarps; ++i) s += sm[i][threadIdx.x];
+    } else if (threadIdx.x == NACC) {
+        unsigned b = 0;
+#pragma unroll
+        for (int i = 0; i < kWarps; ++i) b += sm_bad[i];
+        *bad_out = b;
+    }
+    return s;
+}
+
+// ---- S5: fixed-order compensated combine of `count` partials per quantity ---------------------
+
+// Warp w combines quantities w, w + 8, ...; partial i of quantity k is at p[k * stride_k + i].
+// Writes out[0] = -sum_0 (= -ln L), out[1+k] = -sum_{1+k}, out[NACC] = n_bad; +inf / NaN if n_bad.
+template <int NACC>
+__device__ __forceinline__ void final_combine(const double* p, int64_t stride_k, int count, const unsigned* badp,
+                                              double* out)
+{
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    unsigned nb = 0;
+    for (int i = lane; i < count; i += 32) nb += __ldcg(badp + i);
+    nb = __reduce_add_sync(0xffffffffu, nb);
+    for (int k = w; k < NACC; k += kWarps) {
+        const double* pk = p + k * stride_k;
+        double s = 0.0, c = 0.0;  // Kahan: true sum ~ s - c
+        for (int i = lane; i < count; i += 32) {
+            const double y = __ldcg(pk + i) - c;
+            const double t = s + y;
+            c = (t - s) - y;
+            s = t;
+        }
+        double lo = -c;
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+            const double s2 = __shfl_down_sync(0xffffffffu, s, off);
+            const double lo2 = __shfl_down_sync(0xffffffffu, lo, off);
+            const double t = s + s2;  // two-sum
+            const double bb = t - s;
+            const double e = (s - (t - bb)) + (s2 - bb);
+            lo = (lo + lo2) + e;
+            s = t;
+        }
+        if (lane == 0) {
+            double v = -(s + lo);
+            if (nb) v = (k == 0) ? __longlong_as_double(0x7ff0000000000000LL) : __longlong_as_double(0x7ff8000000000000LL);
+            out[k] = v;
+        }
+    }
+    if (threadIdx.x == 0) out[NACC] = (double)nb;
+}
+
+// ---- the fused single-dataset kernel (mf_nll_grad) ----------------------------------------------
+
+template <class M>
+__global__ void __launch_bounds__(kBlock, 2) nll_grad_kernel(const __grid_constant__ EvalArgs<M> a)
+{
+    constexpr int NACC = M::NACC;
+    __shared__ double sm[kWarps][NACC];
+    __shared__ unsigned sm_bad[kWarps];
+    __shared__ unsigned s_bad_block;
+    __shared__ bool s_last;
+
+    double acc[NACC];
+#pragma unroll
+    for (int k = 0; k < NACC; ++k) acc[k] = 0.0;
+    unsigned bad = 0;
+    const int64_t G = gridDim.x;
+    accumulate<M>(a.col, a.n, a.n_items, blockIdx.x + G * (threadIdx.x >> 5), G * kWarps, a.c, acc, bad);
+
+    const double s = block_reduce<NACC>(acc, bad, sm, sm_bad, &s_bad_block);
+    if (threadIdx.x < NACC) {
+        a.partials[threadIdx.x * G + blockIdx.x] = s;
+        __threadfence();
+    } else if (threadIdx.x == NACC) {
+        a.bad_partials[blockIdx.x] = s_bad_block;
+        __threadfence();
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = (atomicAdd(a.ticket, 1u) == gridDim.x - 1);
+    __syncthreads();
+    if (s_last) {
+        __threadfence();
+        final_combine<NACC>(a.partials, G, (int)G, a.bad_partials, a.out);
+        if (threadIdx.x == 0) *a.ticket = 0u;
+    }
+}
+
+// ---- the batched-toy kernel (mf_nll_grad_batch): CTA <-> (toy, event chunk) ----------------------
+
+template <class M>
+__global__ void __launch_bounds__(kBlock, 2) nll_grad_batch_kernel(const __grid_constant__ BatchArgs<M> a)
+{
+    constexpr int NACC = M::NACC;
+    constexpr int K = M::K;
+    __shared__ double sm[kWarps][NACC];
+    __shared__ unsigned sm_bad[kWarps];
+    __shared__ unsigned s_bad_block;
+    __shared__ bool s_last;
+    __shared__ typename M::Consts s_c;
+    __shared__ int s_ok;
+
+    const int slot = blockIdx.x / a.chunks, chunk = blockIdx.x % a.chunks;
+    // S2 for this toy: parameter-only constants from lambda_t, once per CTA
+    if (threadIdx.x == 0) s_ok = make_consts<M>(a.lam + (int64_t)slot * K, a.ma, a.mb, s_c) ? 1 : 0;
+    __syncthreads();
+    double* out = a.out + (int64_t)slot * (K + 2);
+    if (!s_ok) {  // outside the parameter domain: +inf / NaN, n_bad = -1
+        if (chunk == 0 && threadIdx.x <= K + 1)
+            out[threadIdx.x] = threadIdx.x == 0       ? __longlong_as_double(0x7ff0000000000000LL)
+                               : threadIdx.x == K + 1 ? -1.0
+                                                      : __longlong_as_double(0x7ff8000000000000LL);
+        return;
+    }
+    const typename M::Consts c = s_c;
+    const int64_t toy = a.ids[slot];
+    const double* col[M::NCOL];
+#pragma unroll
+    for (int i = 0; i < M::NCOL; ++i) col[i] = a.col[i] + toy * a.toy_stride;
+
+    double acc[NACC];
+#pragma unroll
+    for (int k = 0; k < NACC; ++k) acc[k] = 0.0;
+    unsigned bad = 0;
+    const int64_t C = a.chunks;
+    accumulate<M>(col, a.n, a.n_items, chunk + C * (threadIdx.x >> 5), C * kWarps, c, acc, bad);
+
+    const double s = block_reduce<NACC>(acc, bad, sm, sm_bad, &s_bad_block);
+    if (a.chunks == 1) {  // the CTA holds the toy's complete sums: no cross-CTA pass
+        __syncthreads();
+        const unsigned nb = s_bad_block;
+        if (threadIdx.x < NACC) {
+            double v = -s;
+            if (nb) v = (threadIdx.x == 0) ? __longlong_as_double(0x7ff0000000000000LL) : __longlong_as_double(0x7ff8000000000000LL);
+            out[threadIdx.x] = v;
+        } else if (threadIdx.x == NACC) {
+            out[NACC] = (double)nb;
+        }
+        return;
+    }
+    double* part = a.partials + (int64_t)slot * NACC * C;
+    unsigned* badp = a.bad_partials + (int64_t)slot * C;
+    if (threadIdx.x < NACC) {
+        part[threadIdx.x * C + chunk] = s;
+        __threadfence();
+    } else if (threadIdx.x == NACC) {
+        badp[chunk] = s_bad_block;
+        __threadfence();
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = (atomicAdd(a.ticket + slot, 1u) == (unsigned)a.chunks - 1);
+    __syncthreads();
+    if (s_last) {
+        __threadfence();
+        final_combine<NACC>(part, C, (int)C, badp, out);
+        if (threadIdx.x == 0) a.ticket[slot] = 0u;
+    }
+}
+
+// ---- S1: event-only precompute (Listing 4) ------------------
+
+// Writes the nine merged angular basis columns h_k = 9/(32 pi) g_k for every (padded) event.
+// cl, ck, phi and h are [rows][n_pad] flattened; h column k is at h + k * total.
+__global__ void __launch_bounds__(256) angular_precompute_kernel(const double* __restrict__ cl_,
+                                                                 const double* __restrict__ ck_,
+                                                                 const double* __restrict__ phi_, double* __restrict__ h,
+                                                                 int64_t total)
+{
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+        const double cl = cl_[i], ck = ck_[i], phi = phi_[i];
+        const double cl2 = cl * cl, ck2 = ck * ck;
+        const double sl2 = 1.0 - cl2, sk2 = 1.0 - ck2;
+        const double sl = sqrt(sl2), sk = sqrt(sk2);  // theta in [0, pi]: sin theta >= 0
+        double sp, cp;
+        sincos(phi, &sp, &cp);
+        const double c2p = (cp - sp) * (cp + sp), s2p = 2.0 * sp * cp;  // cos 2phi, sin 2phi
+        const double g0 = 0.5 * sk2 * (1.0 + cl2);
+        const double sksl = sk * ck * sl;  // sin(2 theta_K) sin(theta_l) / 2
+        h[0 * total + i] = kAngNorm * g0;
+        h[1 * total + i] = kAngNorm * (2.0 * ck2 * sl2 - g0);
+        h[2 * total + i] = kAngNorm * (sk2 * sl2 * c2p);
+        h[3 * total + i] = kAngNorm * (4.0 * sksl * cl * cp);
+        h[4 * total + i] = kAngNorm * (2.0 * sksl * cp);
+        h[5 * total + i] = kAngNorm * ((4.0 / 3.0) * sk2 * cl);
+        h[6 * total + i] = kAngNorm * (2.0 * sksl * sp);
+        h[7 * total + i] = kAngNorm * (4.0 * sksl * cl * sp);
+        h[8 * total + i] = kAngNorm * (sk2 * sl2 * s2p);
+    }
+}
+
+// ---- S0 helpers -----------------------------------------------------------------------------------
+
+// Fills the padding of every toy row with that row's last valid event (rows = ndim * n_toys).
+__global__ void pad_rows_kernel(double* data, int64_t rows, int64_t n, int64_t n_pad)
+{
+    const int64_t npadding = n_pad - n;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < rows * npadding;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t r = i / npadding, o = i % npadding;
+        data[r * n_pad + n + o] = (n > 0) ? data[r * n_pad + n - 1] : 0.0;
+    }
+}
+
+// Counts entries of one dimension ([n_toys][n_pad], valid part only) that are not inside [lo, hi].
+__global__ void range_check_kernel(const double* data, int64_t n_toys, int64_t n, int64_t n_pad, double lo, double hi,
+                                   unsigned long long* count)
+{
+    unsigned long long local = 0;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n_toys * n;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        const double v = data[(i / n) * n_pad + (i % n)];
+        if (!(v >= lo && v <= hi)) ++local;
+    }
+    if (local) atomicAdd(count, local);
+}
+
+}  // namespace mf

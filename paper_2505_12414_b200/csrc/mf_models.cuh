@@ -1,0 +1,278 @@
+// mf_models.cuh — the three PDF families of the hot path: parameter-only constants (S2) and
+// the per-event value + gradient body (S3).  SURVEY.md §8(a); Eq. 2 (83-88),
+// Eq. 3 (90-100), Eq. 4 (116-118), Listing 5 (351-385).
+//
+// Notation follows the paper: f = f_sig, mu, sigma = sigma_m, tau = alpha (BASELINE.json
+// calls the slope tau), N1 / N2 the two normalisations of Eq. 2, [m_a, m_b] the mass range.
+//
+// What is NOT the paper's kernel:
+//  * value and all K derivatives are produced in one pass in registers (the paper emits
+//    one kernel per quantity from its differentiated graph);
+//  * the mass mixture is evaluated in ratio form with ONE exponential per event:
+//        R   = (G/N1)/(E/N2) = exp(-b0 (m-mu)^2 - tau m + ln(c1/c2))
+//        P   = (E/N2) [(1-f) + f R],   ln P = tau m + ln c2 + ln[(1-f) + f R]
+//    instead of Eq. 3's b1 exp(..) + b2 exp(..) (two exponentials); b0, c1, c2 and the
+//    derivatives of ln N1, ln N2 are the buffered parameter-only terms;
+//  * the eleven angular terms of Listing 4 are merged into nine columns h_0..h_8 with
+//    P = h0 + FL h1 + S3 h2 + S4 h3 + S5 h4 + AFB h5 + S7 h6 + S8 h7 + S9 h8.
+#pragma once
+#include <cmath>
+#include <cstdint>
+
+#ifdef __CUDACC__
+#include "mf_math.cuh"
+#define MF_HD __host__ __device__
+#define MF_D __device__ __forceinline__
+#else
+#define MF_HD
+#endif
+
+namespace mf {
+
+constexpr double kPi = 3.141592653589793238462643383279502884;
+constexpr double kLnSqrt2Pi = 0.918938533204672741780329736405617639;  // ln sqrt(2 pi)
+constexpr double kSqrt2Pi = 2.506628274631000502415765284811045253;
+constexpr double kSqrtHalf = 0.707106781186547524400844362104849039;
+constexpr double kAngNorm = 9.0 / (32.0 * kPi);                        // 9/(32 pi), Eq. 4
+constexpr double kInv8Pi = 1.0 / (8.0 * kPi);
+
+// ------------------------------------------------------------------------------------------
+// Parameter-only constants (S2).  One MF_HD implementation: the host runs it once per
+// mf_nll_grad call ("calculating these terms only once on the host for each
+// parameter update"), the batched-toy kernel runs it once per CTA for its toy's lambda_t.
+// ------------------------------------------------------------------------------------------
+
+// Langevin function coth(x) - 1/x without cancellation: continued fraction
+// x/(3 + x^2/(5 + x^2/(7 + ...))) for |x| <= 2, closed form beyond.
+MF_HD inline double langevin(double x)
+{
+    const double ax = fabs(x);
+    if (ax > 2.0) {
+        // coth(x) = 1 + 2/expm1(2x); no cancellation against 1/x here (coth >= 1, 1/x <= 0.5)
+        const double cth = 1.0 + 2.0 / expm1(2.0 * ax);
+        const double v = cth - 1.0 / ax;
+        return x < 0.0 ? -v : v;
+    }
+    const double x2 = x * x;
+    double t = 43.0;  // depth 20: truncation error < 1e-30 for |x| <= 2
+    for (int n = 41; n >= 3; n -= 2) t = (double)n + x2 / t;
+    return x / t;
+}
+
+struct MassConsts {
+    double f, omf;   // f_sig, 1 - f_sig
+    double mu, tau;
+    double nb0;      // -b0 = -1/(2 sigma^2)                       (Eq. 3 b0)
+    double lnk;      // ln(c1/c2), c1 = 1/(sqrt(2pi) sigma N1), c2 = 1/N2   (Eq. 3 b1/f, b2/(1-f))
+    double lnc2;     // -ln N2
+    double is2;      // 1/sigma^2
+    double is3;      // 1/sigma^3
+    double kmu;      // d ln N1 / d mu
+    double ksig;     // 1/sigma + d ln N1 / d sigma
+    double ma;       // m_a (reference point for the tau derivative)
+    double ktau;     // d ln N2 / d tau - m_a = w [1/2 + Langevin(tau w / 2)/2],  w = m_b - m_a
+};
+
+// Returns false if lambda = (f, mu, sigma, tau) is outside the parameter domain
+// (non-finite, sigma <= 0, f outside [0,1]).
+MF_HD inline bool mass_consts(const double* lam, double ma, double mb, MassConsts& c)
+{
+    const double f = lam[0], mu = lam[1], sigma = lam[2], tau = lam[3];
+    if (!(isfinite(f) && isfinite(mu) && isfinite(sigma) && isfinite(tau))) return false;
+    if (!(f >= 0.0 && f <= 1.0) || !(sigma > 0.0)) return false;
+    const double is = 1.0 / sigma;
+    // N1
+    const double za = (mu - ma) * is * kSqrtHalf, zb = (mu - mb) * is * kSqrtHalf;
+    const double N1 = 0.5 * (erf(za) - erf(zb));
+    // Gaussian density at the range ends: dN1/dmu = g(a) - g(b); dN1/dsigma = [(a-mu)g(a) - (b-mu)g(b)]/sigma
+    const double ga = exp(-za * za) * is / kSqrt2Pi, gb = exp(-zb * zb) * is / kSqrt2Pi;
+    const double iN1 = 1.0 / N1;
+    // N2, cancellation-free (SURVEY §8(c) reading 6)
+    const double w = mb - ma;
+    const double lnN2 = (tau == 0.0) ? log(w) : tau * ma + log(expm1(tau * w) / tau);
+    c.f = f;
+    c.omf = 1.0 - f;
+    c.mu = mu;
+    c.tau = tau;
+    c.nb0 = -0.5 * is * is;
+    c.lnc2 = -lnN2;
+    c.lnk = (-kLnSqrt2Pi - log(sigma) - log(N1)) + lnN2;
+    c.is2 = is * is;
+    c.is3 = is * is * is;
+    c.kmu = (ga - gb) * iN1;
+    c.ksig = is + ((ma - mu) * ga - (mb - mu) * gb) * is * iN1;
+    c.ma = ma;
+    c.ktau = w * (0.5 + 0.5 * langevin(0.5 * tau * w));
+    return true;
+}
+
+struct AngularConsts {
+    double a[8];  // FL, S3, S4, S5, AFB, S7, S8, S9 (PAPER.md:369-376 order)
+};
+
+MF_HD inline bool angular_consts(const double* lam, AngularConsts& c)
+{
+    bool ok = true;
+    for (int k = 0; k < 8; ++k) {
+        c.a[k] = lam[k];
+        ok = ok && isfinite(lam[k]);
+    }
+    return ok;
+}
+
+struct FourDConsts {
+    MassConsts m;
+    double a[8];                // angular coefficients
+    double cl1, cl2, ck1, ck2;  // Legendre coefficients of the background
+    double kappa;               // (1-f)/(8 pi): (1-f) L = kappa * ll * lk with ll = 2 l(cos theta_l) etc.
+};
+
+MF_HD inline bool fourd_consts(const double* lam, double ma, double mb, FourDConsts& c)
+{
+    bool ok = mass_consts(lam, ma, mb, c.m);
+    for (int k = 0; k < 8; ++k) {
+        c.a[k] = lam[4 + k];
+        ok = ok && isfinite(lam[4 + k]);
+    }
+    c.cl1 = lam[12];
+    c.cl2 = lam[13];
+    c.ck1 = lam[14];
+    c.ck2 = lam[15];
+    ok = ok && isfinite(c.cl1) && isfinite(c.cl2) && isfinite(c.ck1) && isfinite(c.ck2);
+    c.kappa = ok ? c.m.omf * kInv8Pi : 0.0;
+    return ok;
+}
+
+#ifdef __CUDACC__
+// ------------------------------------------------------------------------------------------
+// Per-event bodies (S3).  Each adds ln P_i to acc[0] and d ln P_i / d lambda_k to acc[1+k];
+// `bad` counts events with P <= 0 or NaN (SURVEY.md §8(c) reading 15); when it ends up
+// non-zero the sums are discarded by the final pass, so they are accumulated unconditionally.  PRED = true is the
+// ragged-tail variant: lanes with valid == false contribute exactly 0 (reading 10).
+// ------------------------------------------------------------------------------------------
+
+struct MassModel {
+    static constexpr int K = 4;
+    static constexpr int NCOL = 1;  // m
+    static constexpr int NACC = 5;
+    using Consts = MassConsts;
+
+    template <bool PRED>
+    static MF_D void event(const double* x, const Consts& c, double* acc, unsigned& bad, bool valid)
+    {
+        const double m = x[0];
+        const double d = m - c.mu;
+        const double t = d * d;
+        // ln R = -b0 d^2 - tau m + ln(c1/c2); clamped so R stays finite
+        const double arg = fmin(fma(c.nb0, t, fma(-c.tau, m, c.lnk)), 700.0);
+        const double R = mf_exp(arg);
+        const double D = fma(c.f, R, c.omf);  // P N2 e^{-tau m} = (1-f) + f R
+        const double r = mf_rcp(D);
+        const double lnP = fma(c.tau, m, c.lnc2) + mf_log(D);
+        const double u = R * r;               // (G/N1)/P
+        const double ws = c.f * u;            // signal weight  f (G/N1) / P
+        const double wb = c.omf * r;          // background weight (1-f)(E/N2)/P
+        const double gf = u - r;              // [(G/N1) - (E/N2)]/P
+        const double hmu = fma(d, c.is2, -c.kmu);
+        const double hsig = fma(t, c.is3, -c.ksig);
+        const double htau = (m - c.ma) - c.ktau;
+        const bool good = D > 0.0;
+        if (!PRED || valid) {
+            bad += good ? 0u : 1u;
+            {
+                acc[0] += lnP;
+                acc[1] += gf;
+                acc[2] = fma(ws, hmu, acc[2]);
+                acc[3] = fma(ws, hsig, acc[3]);
+                acc[4] = fma(wb, htau, acc[4]);
+            }
+        }
+    }
+};
+
+struct AngularModel {
+    static constexpr int K = 8;
+    static constexpr int NCOL = 9;  // h_0..h_8 (cached, already times 9/(32 pi))
+    static constexpr int NACC = 9;
+    using Consts = AngularConsts;
+
+    template <bool PRED>
+    static MF_D void event(const double* x, const Consts& c, double* acc, unsigned& bad, bool valid)
+    {
+        double P = fma(c.a[0], x[1], x[0]);
+#pragma unroll
+        for (int k = 1; k < 8; ++k) P = fma(c.a[k], x[1 + k], P);
+        const double r = mf_rcp(P);
+        const double lnP = mf_log(P);
+        const bool good = P > 0.0;
+        if (!PRED || valid) {
+            bad += good ? 0u : 1u;
+            {
+                acc[0] += lnP;
+#pragma unroll
+                for (int k = 0; k < 8; ++k) acc[1 + k] = fma(x[1 + k], r, acc[1 + k]);
+            }
+        }
+    }
+};
+
+struct FourDModel {
+    static constexpr int K = 16;
+    static constexpr int NCOL = 12;  // m, cos theta_l, cos theta_K, h_0..h_8
+    static constexpr int NACC = 17;
+    using Consts = FourDConsts;
+
+    template <bool PRED>
+    static MF_D void event(const double* x, const Consts& c, double* acc, unsigned& bad, bool valid)
+    {
+        const MassConsts& q = c.m;
+        const double m = x[0], cl = x[1], ck = x[2];
+        const double* h = x + 3;
+        // angular signal A(Omega)
+        double A = fma(c.a[0], h[1], h[0]);
+#pragma unroll
+        for (int k = 1; k < 8; ++k) A = fma(c.a[k], h[1 + k], A);
+        // background angles: ll = 2 l(cos theta_l), lk = 2 l(cos theta_K); L = ll lk / (8 pi)
+        const double p2l = fma(1.5 * cl, cl, -0.5), p2k = fma(1.5 * ck, ck, -0.5);
+        const double ll = fma(c.cl2, p2l, fma(c.cl1, cl, 1.0));
+        const double lk = fma(c.ck2, p2k, fma(c.ck1, ck, 1.0));
+        const double d = m - q.mu;
+        const double t = d * d;
+        const double arg = fmin(fma(q.nb0, t, fma(-q.tau, m, q.lnk)), 700.0);
+        const double R = mf_exp(arg);          // (G/N1)/(E/N2)
+        const double omfL = c.kappa * (ll * lk);  // (1-f) L
+        const double fR = q.f * R;
+        const double D = fma(fR, A, omfL);     // P N2 e^{-tau m}
+        const double r = mf_rcp(D);
+        const double lnP = fma(q.tau, m, q.lnc2) + mf_log(D);
+        const double ws = fR * A * r;          // f (G/N1) A / P
+        const double wb = omfL * r;            // (1-f)(E/N2) L / P
+        const double gf = fma(R * A, r, -(ll * lk) * kInv8Pi * r);
+        const double hmu = fma(d, q.is2, -q.kmu);
+        const double hsig = fma(t, q.is3, -q.ksig);
+        const double htau = (m - q.ma) - q.ktau;
+        const double qa = fR * r;              // f (G/N1) / P
+        const double qb = c.kappa * r;         // (1-f)(E/N2)/(8 pi P)
+        const double qbl = qb * lk, qbk = qb * ll;
+        const bool good = D > 0.0;
+        if (!PRED || valid) {
+            bad += good ? 0u : 1u;
+            {
+                acc[0] += lnP;
+                acc[1] += gf;
+                acc[2] = fma(ws, hmu, acc[2]);
+                acc[3] = fma(ws, hsig, acc[3]);
+                acc[4] = fma(wb, htau, acc[4]);
+#pragma unroll
+                for (int k = 0; k < 8; ++k) acc[5 + k] = fma(qa, h[1 + k], acc[5 + k]);
+                acc[13] = fma(qbl, cl, acc[13]);
+                acc[14] = fma(qbl, p2l, acc[14]);
+                acc[15] = fma(qbk, ck, acc[15]);
+                acc[16] = fma(qbk, p2k, acc[16]);
+            }
+        }
+    }
+};
+#endif  // __CUDACC__
+
+}  // namespace mf

@@ -1,0 +1,263 @@
+"""GPU parity: the CUDA path (through the C-ABI library) against the CPU oracle, element by
+element on the same seeded inputs.  Tolerances are BASELINE.json's north_star:
+|d(-lnL)| / |-lnL| <= 1e-11, |d g_k| <= 1e-9 (1 + |g_k|), fitted lambda within 1e-6 sigma_stat."""
+import math
+
+import numpy as np
+import pytest
+
+import mf_datagen as dg
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+NLL_RTOL = 1e-11
+GRAD_TOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def mf():
+    import paper_2505_12414_b200 as mf
+    return mf
+
+
+@pytest.fixture(scope="module")
+def ctx(mf):
+    c = mf.Context(0)
+    yield c
+    c.close()
+
+
+def assert_parity(nll, grad, o_nll, o_grad, what=""):
+    assert abs(nll - o_nll) <= NLL_RTOL * abs(o_nll) + 1e-300, f"{what}: nll {nll!r} vs oracle {o_nll!r}"
+    err = np.abs(grad - o_grad)
+    tol = GRAD_TOL * (1.0 + np.abs(o_grad))
+    assert np.all(err <= tol), f"{what}: grad err {err} tol {tol}"
+
+
+MASS_POINTS = [
+    dg.MASS_TRUTH,
+    dg.MASS_START,
+    (0.4, 5.05, 0.1, 0.7),      # N1 = 0.69: the erf normalisation and its derivatives matter
+    (0.3, 5.28, 0.02, 0.0),     # tau == 0 branch of N2
+    (0.3, 5.28, 0.02, 1e-9),    # tiny tau: cancellation-free forms
+    (0.0, 5.28, 0.02, -1.5),    # f = 0
+    (1.0, 5.3, 0.2, -1.5),      # f = 1
+    (0.7, 5.58, 0.05, 3.0),     # peak at the range edge
+]
+
+
+@pytest.mark.parametrize("n", [10_000, 10_007, 1, 63, 64, 65, 129])
+def test_mass_parity_sizes(mf, ctx, n):
+    m = dg.gen_mass(n, seed=0)
+    ds = ctx.dataset_upload(m, dg.MASS_LO, dg.MASS_HI)
+    model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ds)
+    for lam in MASS_POINTS:
+        o_nll, o_g, nbad = oracle.nll_grad(oracle.MASS, m, lam, dg.MASS_LO, dg.MASS_HI)
+        assert nbad == 0
+        nll, g = model.nll_grad(lam)
+        assert_parity(nll, g, o_nll, o_g, f"mass n={n} lam={lam}")
+
+
+def test_mass_empty_dataset(mf, ctx):
+    ds = ctx.dataset_upload(np.zeros(0), dg.MASS_LO, dg.MASS_HI)
+    model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ds)
+    nll, g = model.nll_grad(dg.MASS_TRUTH)
+    assert nll == 0.0 and np.all(g == 0.0)
+
+
+def test_mass_paper_range_point(mf, ctx):
+    """The paper's own benchmark values: range [5,7], sigma 0.06, alpha -1."""
+    lam = (0.3, 5.28, 0.06, -1.0)
+    m = dg.gen_mass(20_000, seed=11, lam=lam, lo=5.0, hi=7.0)
+    ds = ctx.dataset_upload(m, 5.0, 7.0)
+    model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ds)
+    for pt in [lam, (0.35, 5.3, 0.07, -0.8)]:
+        o_nll, o_g, _ = oracle.nll_grad(oracle.MASS, m, pt, 5.0, 7.0)
+        nll, g = model.nll_grad(pt)
+        assert_parity(nll, g, o_nll, o_g, f"paper range {pt}")
+
+
+def test_mass_device_columns(mf, ctx):
+    import torch
+    m = dg.gen_mass(5000, seed=3)
+    t = torch.from_numpy(m).cuda()
+    ds = ctx.dataset_upload([t], dg.MASS_LO, dg.MASS_HI)
+    model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ds)
+    ds.close()  # the model keeps its own reference
+    o_nll, o_g, _ = oracle.nll_grad(oracle.MASS, m, dg.MASS_TRUTH, dg.MASS_LO, dg.MASS_HI)
+    nll, g = model.nll_grad(dg.MASS_TRUTH)
+    assert_parity(nll, g, o_nll, o_g, "device columns")
+
+
+ANG_POINTS = [
+    dg.ANG_TRUTH,
+    (0.5, 0, 0, 0, 0, 0, 0, 0),
+    (0.7, 0.05, -0.1, 0.1, 0.1, 0.03, 0.04, -0.05),
+]
+
+
+@pytest.mark.parametrize("n", [20_000, 20_011, 37])
+def test_angular_parity(mf, ctx, n):
+    ev = dg.gen_angular(n, seed=2)
+    ds = ctx.dataset_upload(ev)
+    model = ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ds)
+    for lam in ANG_POINTS:
+        o_nll, o_g, nbad = oracle.nll_grad(oracle.ANGULAR, ev, lam)
+        assert nbad == 0
+        nll, g = model.nll_grad(lam)
+        assert_parity(nll, g, o_nll, o_g, f"angular n={n} lam={lam}")
+
+
+FOURD_POINTS = [
+    dg.FOURD_TRUTH,
+    (0.25, 5.27, 0.025, -1.2, 0.55, 0.01, -0.1, -0.15, -0.02, 0.02, 0.0, 0.03, 0.15, -0.1, 0.05, 0.02),
+    (0.4, 5.05, 0.1, 0.7) + dg.ANG_TRUTH + (-0.2, 0.1, 0.3, 0.2),
+]
+
+
+@pytest.mark.parametrize("n", [30_000, 30_001])
+def test_fourd_parity(mf, ctx, n):
+    ev = dg.gen_4d(n, seed=3)
+    ds = ctx.dataset_upload(ev, dg.MASS_LO, dg.MASS_HI)
+    model = ctx.model_create(mf.MF_MASS_X_ANGULAR, ds)
+    for lam in FOURD_POINTS:
+        o_nll, o_g, nbad = oracle.nll_grad(oracle.FOURD, ev, lam, dg.MASS_LO, dg.MASS_HI)
+        assert nbad == 0
+        nll, g = model.nll_grad(lam)
+        assert_parity(nll, g, o_nll, o_g, f"4d n={n}")
+
+
+def test_bitwise_reproducible(mf, ctx):
+    ev = dg.gen_4d(50_000, seed=5)
+    ds = ctx.dataset_upload(ev, dg.MASS_LO, dg.MASS_HI)
+    model = ctx.model_create(mf.MF_MASS_X_ANGULAR, ds)
+    ref = model.nll_grad(dg.FOURD_TRUTH)
+    for _ in range(20):
+        nll, g = model.nll_grad(dg.FOURD_TRUTH)
+        assert nll == ref[0] and np.array_equal(g, ref[1])
+
+
+def test_status_codes(mf, ctx):
+    m = dg.gen_mass(1000, seed=0)
+    ds = ctx.dataset_upload(m, dg.MASS_LO, dg.MASS_HI)
+    model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ds)
+    for bad in [(1.2, 5.28, 0.02, -1.5), (0.3, 5.28, -0.02, -1.5), (0.3, 5.28, 0.0, -1.5), (0.3, math.nan, 0.02, -1.5)]:
+        st, nll, g = model.nll_grad_status(bad)
+        assert st == mf.MF_ERR_PARAM_DOMAIN
+        assert math.isnan(nll) and np.all(np.isnan(g))  # outputs untouched
+        assert not oracle.check_domain(oracle.MASS, bad)
+    # angular coefficients that make P negative for some events
+    ev = dg.gen_angular(5000, seed=2)
+    ads = ctx.dataset_upload(ev)
+    amodel = ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ads)
+    lam = (0.6, 0.9, 0.9, -0.9, 0.9, 0.9, 0.9, 0.9)
+    _, _, nbad = oracle.nll_grad(oracle.ANGULAR, ev, lam)
+    assert nbad > 0
+    st, nll, g = amodel.nll_grad_status(lam)
+    assert st == mf.MF_NONPOSITIVE_PDF and nll == math.inf and np.all(np.isnan(g))
+    # next call is clean again
+    nll, g = amodel.nll_grad(dg.ANG_TRUTH)
+    o_nll, o_g, _ = oracle.nll_grad(oracle.ANGULAR, ev, dg.ANG_TRUTH)
+    assert_parity(nll, g, o_nll, o_g, "after a P<=0 call")
+    # data outside the range
+    with pytest.raises(mf.MoreFitError) as e:
+        ctx.dataset_upload(np.array([5.1, 5.7, 5.2]), dg.MASS_LO, dg.MASS_HI)
+    assert e.value.status == mf.MF_ERR_DATA_RANGE
+    with pytest.raises(mf.MoreFitError) as e:
+        ctx.dataset_upload(np.array([5.1, math.nan]), dg.MASS_LO, dg.MASS_HI)
+    assert e.value.status == mf.MF_ERR_DATA_RANGE
+    with pytest.raises(mf.MoreFitError) as e:
+        ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ds)  # ndim mismatch
+    assert e.value.status == mf.MF_ERR_ARG
+
+
+@pytest.mark.parametrize("n_events", [1000, 1003, 70_001])
+def test_batch_parity(mf, ctx, n_events):
+    """mf_nll_grad_batch: every toy at its own lambda_t in one launch (70,001 events: several CTAs per toy)."""
+    T = 7
+    toys = dg.gen_mass_toys(T, n_events, first_seed=100)
+    ds = ctx.dataset_upload(toys, dg.MASS_LO, dg.MASS_HI, n_toys=T)
+    model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ds)
+    lams = dg.gen_lambda_points(T, 5, dg.MASS_TRUTH, 3 * dg.mass_sigma_stat(n_events))
+    lams[1] = (0.4, 5.05, 0.1, 0.7)
+    lams[2] = (0.3, 5.28, 0.02, 0.0)
+    active = np.ones(T, dtype=np.uint8)
+    active[3] = 0
+    nll, g = model.nll_grad_batch(lams, active)
+    assert math.isnan(nll[3]) and np.all(np.isnan(g[3]))   # untouched
+    for t in range(T):
+        if not active[t]:
+            continue
+        o_nll, o_g, _ = oracle.nll_grad(oracle.MASS, toys[t], lams[t], dg.MASS_LO, dg.MASS_HI)
+        assert_parity(nll[t], g[t], o_nll, o_g, f"toy {t}")
+    # a toy outside the domain gets +inf / NaN, the others are unaffected
+    lams2 = lams.copy()
+    lams2[0] = (0.3, 5.28, -1.0, -1.5)
+    nll2, g2 = model.nll_grad_batch(lams2)
+    assert nll2[0] == math.inf and np.all(np.isnan(g2[0]))
+    assert nll2[1] == nll[1] and np.array_equal(g2[1], g[1])
+
+
+def test_batch_angular_parity(mf, ctx):
+    T, n = 3, 4000
+    ev = np.stack([dg.gen_angular(n, seed=40 + t) for t in range(T)], axis=1)  # [3][T][n]
+    ds = ctx.dataset_upload(ev, n_toys=T)
+    model = ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ds)
+    lams = np.array(ANG_POINTS)
+    nll, g = model.nll_grad_batch(lams)
+    for t in range(T):
+        o_nll, o_g, _ = oracle.nll_grad(oracle.ANGULAR, ev[:, t, :], lams[t])
+        assert_parity(nll[t], g[t], o_nll, o_g, f"angular toy {t}")
+
+
+def _assert_fit_agrees(r, o):
+    assert r.converged and o.converged
+    assert np.max(np.abs(r.lam - o.lam) / o.sigma) < 1e-6, (r.lam, o.lam, o.sigma)
+    np.testing.assert_allclose(r.sigma, o.sigma, rtol=1e-4)
+    assert abs(r.nll - o.nll) <= 1e-11 * abs(o.nll)
+
+
+def test_fit_c0(mf, ctx):
+    """BASELINE.json configs[0]: full fit from (0.5, 5.27, 0.03, -1.0)."""
+    m = dg.gen_mass(10_000, seed=0)
+    ds = ctx.dataset_upload(m, dg.MASS_LO, dg.MASS_HI)
+    model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ds)
+    r = model.fit(dg.MASS_START)
+    o = oracle.fit(oracle.MASS, m, dg.MASS_START, lo=dg.MASS_LO, hi=dg.MASS_HI)
+    _assert_fit_agrees(r, o)
+    # fixed parameters stay put and get zero covariance
+    r2 = model.fit(dg.MASS_START, fixed=[0, 0, 0, 1])
+    o2 = oracle.fit(oracle.MASS, m, dg.MASS_START, fixed=[0, 0, 0, 1], lo=dg.MASS_LO, hi=dg.MASS_HI)
+    assert r2.lam[3] == dg.MASS_START[3] and np.all(r2.cov[3] == 0)
+    assert np.max(np.abs(r2.lam[:3] - o2.lam[:3]) / o2.sigma[:3]) < 1e-6
+
+
+def test_fit_angular(mf, ctx):
+    ev = dg.gen_angular(20_000, seed=2)
+    ds = ctx.dataset_upload(ev)
+    model = ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ds)
+    r = model.fit(dg.ANG_TRUTH)
+    o = oracle.fit(oracle.ANGULAR, ev, dg.ANG_TRUTH)
+    _assert_fit_agrees(r, o)
+
+
+def test_fit_fourd(mf, ctx):
+    ev = dg.gen_4d(20_000, seed=3)
+    ds = ctx.dataset_upload(ev, dg.MASS_LO, dg.MASS_HI)
+    model = ctx.model_create(mf.MF_MASS_X_ANGULAR, ds)
+    r = model.fit(dg.FOURD_TRUTH)
+    o = oracle.fit(oracle.FOURD, ev, dg.FOURD_TRUTH, lo=dg.MASS_LO, hi=dg.MASS_HI, nthreads=oracle.max_threads())
+    _assert_fit_agrees(r, o)
+
+
+def test_fit_batch_small(mf, ctx):
+    """mf_fit_batch: concurrent toy fits agree with one oracle fit per toy."""
+    T, n = 6, 2000
+    toys = dg.gen_mass_toys(T, n, first_seed=0)
+    ds = ctx.dataset_upload(toys, dg.MASS_LO, dg.MASS_HI, n_toys=T)
+    model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ds)
+    res = model.fit_batch(np.array(dg.MASS_TRUTH))
+    for t in range(T):
+        o = oracle.fit(oracle.MASS, toys[t], dg.MASS_TRUTH, lo=dg.MASS_LO, hi=dg.MASS_HI)
+        _assert_fit_agrees(res[t], o)
