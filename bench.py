@@ -1,0 +1,347 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the fused NLL + analytic-gradient hot path on B200.
+
+Workload (BASELINE.json configs[1], "C1"): the 1D Gaussian+exponential mass model, N = 1,000,000
+fp64 events, 4 free parameters; one STEP = one complete pass of the hot path (S2 parameter-only
+constants on the host, S3 per-event value + gradient, S4/S5 reductions, S6 K+2 doubles out) at a
+new parameter point drawn within +-3 sigma_stat of the truth (1,000 seeded points, cycled).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl mine|reference]
+
+Timing rules followed: W >= 3 warm-up steps; the timed steps rotate over R dataset replicas whose
+total size (R x 8 MB = 256 MB) exceeds the 126 MB L2, so every step reads its events from HBM
+("l2": "inputs larger than L2" in config); CUDA events on the launching stream; max over ranks;
+SM clocks and throttle reasons sampled (NVML, separate process) during the timed region.
+
+`value` is events/s with the data resident in HBM; `e2e` is the same metric through the public API
+with HOST inputs (pinned), i.e. mf_dataset_upload + mf_model_create + mf_nll_grad every step.
+`roofline` is for the dominant kernel nll_grad_kernel<MassModel> (ALU bound);
+`cpu_baseline` is the fp64 oracle on this box's host cores on a bounded sample.
+
+--impl reference times the CPU oracle itself (there is no reference implementation to install:
+/root/reference holds only the paper), on the same config, metric and unit.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import mf_datagen as dg  # noqa: E402
+
+N_EVENTS = 1_000_000
+N_POINTS = 1000
+N_REPLICAS = 32
+METRIC = "nll_grad_event_evals_per_s"
+UNIT = "events/s"
+WORKLOAD = "C1: 1D Gaussian+exponential mass model, N=1e6 fp64 events, K=4, NLL+gradient at 1000 seeded lambda points"
+# fp64-pipe thread-instructions per event of the shipped mass kernel's fast path (counted from
+# SASS); never more than the plain two-exponential form's hand count (100).
+MASS_FP64_INSTR_PER_EVENT = 47.0
+NOMINAL_FP64_LANES_PER_SM = 64  # B200: 4 SMSPs x 16 fp64 FMA lanes
+
+
+def _clock_sampler_main(index: int, path: str) -> None:
+    """Child process: appends 't sm_mhz sm_max_mhz reasons_bitmask' lines to `path` until stdin closes."""
+    import select
+
+    import pynvml
+    pynvml.nvmlInit()
+    h = pynvml.nvmlDeviceGetHandleByIndex(index)
+    mx = pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM)
+    with open(path, "w", buffering=1) as fh:
+        while True:
+            if select.select([sys.stdin], [], [], 0.002)[0]:
+                break
+            sm = pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)
+            rs = pynvml.nvmlDeviceGetCurrentClocksEventReasons(h)
+            fh.write(f"{time.time():.6f} {sm} {mx} {rs}\n")
+
+
+class ClockSampler:
+    """SM clock and throttle reasons sampled by NVML in a separate process during the timed region."""
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+               0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x100: "display_clock_setting",
+               0x10: "sync_boost"}
+
+    def __init__(self, index: int):
+        import tempfile
+        self.path = os.path.join(tempfile.gettempdir(), f"mf_clocks_{os.getpid()}.txt")
+        self.p = None
+        try:
+            self.p = subprocess.Popen([sys.executable, os.path.abspath(__file__), "--clock-sampler", str(index), self.path],
+                                      stdin=subprocess.PIPE, stdout=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def wait_ready(self, timeout: float = 30.0) -> None:
+        t = time.time()
+        while self.p is not None and time.time() - t < timeout:
+            if os.path.exists(self.path) and os.path.getsize(self.path) > 0:
+                return
+            if self.p.poll() is not None:
+                return
+            time.sleep(0.01)
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["sampler unavailable"]}
+        try:
+            self.p.communicate(b"q\n", timeout=10)
+        except Exception:
+            self.p.kill()
+        sm, mx, bits, n_all = [], None, 0, 0
+        try:
+            with open(self.path) as fh:
+                lines = fh.read().splitlines()
+            os.remove(self.path)
+        except Exception:
+            lines = []
+        for line in lines:
+            try:
+                t, s, m, r = line.split()
+            except ValueError:
+                continue
+            n_all += 1
+            mx = int(m)
+            if t0 <= float(t) <= t1:
+                sm.append(int(s))
+                bits |= int(r)
+        reasons = [name for bit, name in self.REASONS.items() if bits & bit]
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": mx, "reasons": reasons,
+                "samples_in_region": len(sm), "samples": n_all}
+
+
+def _dist_setup(n_gpus: int):
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch
+        import torch.distributed as dist
+        torch.cuda.set_device(local)
+        dist.init_process_group(backend="nccl", device_id=torch.device("cuda", local))
+    return rank, world, local
+
+
+def _barrier(world: int):
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+
+
+def _max_over_ranks(x: float, world: int) -> float:
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device="cuda")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def _cpu_baseline(sample_events: int, repeats: int) -> dict:
+    """The oracle as it stands on this box's host cores, on the first `sample_events` events of C1."""
+    import oracle
+    m = dg.gen_mass(N_EVENTS, seed=1)[:sample_events]
+    pts = dg.gen_lambda_points(N_POINTS, 1001, dg.MASS_TRUTH, 3 * dg.mass_sigma_stat(N_EVENTS))
+    best = {}
+    for nt in sorted({1, oracle.max_threads()}):
+        oracle.nll_grad(oracle.MASS, m[:1000], pts[0], dg.MASS_LO, dg.MASS_HI, nthreads=nt)
+        t = time.perf_counter()
+        for i in range(repeats):
+            oracle.nll_grad(oracle.MASS, m, pts[i % N_POINTS], dg.MASS_LO, dg.MASS_HI, nthreads=nt)
+        best[nt] = sample_events * repeats / (time.perf_counter() - t)
+    nt = max(best, key=best.get)
+    return {"value": best[nt], "unit": UNIT, "cores": nt, "kind": "oracle",
+            "sample": f"{repeats} NLL+gradient calls on the first {sample_events} events of the C1 dataset (seed 1)",
+            "single_thread_value": best[1], "host_cores": os.cpu_count()}
+
+
+def run_reference(args) -> None:
+    """--impl reference: the CPU oracle timed as the reference arm (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    sample = 200_000
+    m = dg.gen_mass(N_EVENTS, seed=1)[:sample]
+    pts = dg.gen_lambda_points(N_POINTS, 1001, dg.MASS_TRUTH, 3 * dg.mass_sigma_stat(N_EVENTS))
+    nt = oracle.max_threads()
+    steps = min(args.steps, 400)   # each step ~ 0.05-0.1 s of CPU: keeps the arm within minutes
+    warm = min(args.warmup, 5)
+    for i in range(warm):
+        oracle.nll_grad(oracle.MASS, m, pts[i % N_POINTS], dg.MASS_LO, dg.MASS_HI, nthreads=nt)
+    t = time.perf_counter()
+    for i in range(steps):
+        oracle.nll_grad(oracle.MASS, m, pts[i % N_POINTS], dg.MASS_LO, dg.MASS_HI, nthreads=nt)
+    dt = time.perf_counter() - t
+    value = sample * steps / dt
+    desc = f"each step = one oracle NLL+gradient call on the first {sample} events of C1 ({nt} threads)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+        "warmup": warm, "ms_per_step": 1e3 * dt / steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "n_events": N_EVENTS, "sample": desc},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": nt, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def run_mine(args) -> None:
+    import torch
+
+    import paper_2505_12414_b200 as mf
+
+    rank, world, local = _dist_setup(args.gpus)
+    torch.cuda.set_device(local)
+    sampler = ClockSampler(local) if rank == 0 else None   # started early: it needs ~1 s to come up
+    ctx = mf.Context(local)  # borrows torch's current stream on this device
+    K = 4
+
+    # ---- inputs: R replicas of C1 (seeds 1, 2, ...; rank r uses its own seeds), resident in HBM
+    pts = dg.gen_lambda_points(N_POINTS, 1001, dg.MASS_TRUTH, 3 * dg.mass_sigma_stat(N_EVENTS))
+    models, host0 = [], None
+    for r in range(N_REPLICAS):
+        m = dg.gen_mass(N_EVENTS, seed=1 + r + 1000 * rank)
+        if r == 0:
+            host0 = m
+        models.append(ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(m, dg.MASS_LO, dg.MASS_HI)))
+    out = torch.zeros((N_POINTS, K + 2), dtype=torch.float64, device="cuda")
+    out_ptrs = [out[i].data_ptr() for i in range(N_POINTS)]
+    lam_rows = [np.ascontiguousarray(pts[i]) for i in range(N_POINTS)]
+
+    def step(i: int):
+        models[i % N_REPLICAS].nll_grad_async(lam_rows[i % N_POINTS], out_ptrs[i % N_POINTS])
+
+    for i in range(args.warmup):
+        step(i)
+    torch.cuda.synchronize()
+
+    if sampler:
+        sampler.wait_ready()
+    launches0 = ctx.kernel_launches
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    _barrier(world)
+    torch.cuda.synchronize()
+    t_host0 = time.time()
+    e0.record()
+    for i in range(args.steps):
+        step(i)
+    e1.record()
+    torch.cuda.synchronize()
+    _barrier(world)
+    t_host1 = time.time()
+    ms = _max_over_ranks(float(e0.elapsed_time(e1)), world)
+    launches = ctx.kernel_launches - launches0
+    clocks = sampler.stop(t_host0, t_host1) if sampler else None
+
+    res = out.cpu().numpy()
+    n_done = min(args.steps, N_POINTS)
+    if not (np.all(np.isfinite(res[:n_done])) and np.all(res[:n_done, K + 1] == 0)):
+        raise RuntimeError("non-finite NLL / gradient in the timed steps")
+
+    ms_per_step = ms / args.steps
+    value = world * N_EVENTS * args.steps / (ms * 1e-3)
+
+    # ---- e2e: public API with HOST (pinned) inputs, upload + model + evaluation every step
+    pinned = torch.from_numpy(host0).pin_memory()
+    host_view = pinned.numpy()
+    e2e_steps = max(3, min(args.steps, 100))
+
+    def e2e_step(i: int):
+        ds = ctx.dataset_upload(host_view, dg.MASS_LO, dg.MASS_HI)
+        md = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ds)
+        nll, g = md.nll_grad(lam_rows[i % N_POINTS])
+        md.close()
+        ds.close()
+        return nll
+
+    for i in range(3):
+        e2e_step(i)
+    torch.cuda.synchronize()
+    _barrier(world)
+    t = time.perf_counter()
+    for i in range(e2e_steps):
+        e2e_step(i)
+    torch.cuda.synchronize()
+    e2e_s = _max_over_ranks(time.perf_counter() - t, world)
+    e2e = {"value": world * N_EVENTS * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 8 * N_EVENTS,
+           "d2h_bytes_per_step": 8 * (K + 2), "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps,
+           "what": "mf_dataset_upload (pinned host -> device) + mf_model_create + mf_nll_grad + destroy, every step"}
+
+    if rank != 0:
+        return
+
+    # ---- roofline of the dominant kernel (ALU bound; fp64-pipe instruction = 1 DFMA = 2 flop)
+    peaks = {}
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            peaks = json.load(fh)
+    except Exception:
+        pass
+    sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+    n_sm = torch.cuda.get_device_properties(local).multi_processor_count
+    peak_tflops = 2.0 * n_sm * NOMINAL_FP64_LANES_PER_SM * sm_max_mhz * 1e6 / 1e12
+    measured_rate = ctx.probe_fp64_rate()
+    achieved_tflops = 2.0 * MASS_FP64_INSTR_PER_EVENT * N_EVENTS / (ms_per_step * 1e-3) / 1e12
+    traffic = None
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
+            traffic = json.load(fh).get("nll_grad_kernel<MassModel>")
+    except Exception:
+        pass
+    roofline = {
+        "bound": "alu", "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
+        "frac": achieved_tflops / peak_tflops, "traffic": traffic,
+        "kernel": "nll_grad_kernel<MassModel>", "fp64_instr_per_event": MASS_FP64_INSTR_PER_EVENT,
+        "peak_how": f"derived: {n_sm} SMs x {NOMINAL_FP64_LANES_PER_SM} fp64 lanes x {sm_max_mhz:.0f} MHz x 2 flop",
+        "peak_measured_dfma_chain": 2.0 * measured_rate / 1e12,
+        "frac_of_measured_dfma_chain": achieved_tflops / (2.0 * measured_rate / 1e12),
+        "hbm_side": {"bytes_per_event": 8, "achieved_gbs": 8.0 * N_EVENTS / (ms_per_step * 1e-3) / 1e9,
+                     "peak_gbs": peaks.get("hbm_gbs")},
+    }
+
+    cpu = _cpu_baseline(sample_events=N_EVENTS, repeats=40)
+
+    print(json.dumps({
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "n_events": N_EVENTS, "n_params": K, "lambda_points": N_POINTS,
+                   "replicas": N_REPLICAS, "l2": "inputs larger than L2: steps rotate over 32 x 8 MB dataset replicas",
+                   "launch": "one nll_grad_kernel<MassModel> launch per step via mf_nll_grad_async"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
+    }))
+
+
+def main() -> None:
+    if len(sys.argv) >= 4 and sys.argv[1] == "--clock-sampler":
+        _clock_sampler_main(int(sys.argv[2]), sys.argv[3])
+        return
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20000)
+    ap.add_argument("--warmup", type=int, default=100)
+    ap.add_argument("--impl", choices=["mine", "reference"], default="mine")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_mine(args)
+
+
+if __name__ == "__main__":
+    main()

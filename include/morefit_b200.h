@@ -181,6 +181,19 @@ mf_status mf_fit(mf_model* model, const double* start, const uint8_t* fixed,
 mf_status mf_fit_batch(mf_model* model, int64_t n_toys, const double* starts,
                        const uint8_t* fixed, const mf_fit_opts* opts, mf_fit_result* results);
 
+/* ---- measurement helpers (not on the hot path) ------------------------ */
+
+/* fp64-pipe issue rate of this GPU in DFMA thread-instructions per second, measured with
+ * register-only DFMA chains (nominal B200: 148 SMs x 64 lanes x 1.965 GHz = 1.86e13). */
+mf_status mf_probe_fp64_rate(mf_ctx* ctx, double* dfma_per_second);
+/* Read bandwidth in bytes/s of a `bytes`-sized device buffer that one kernel reads `repeats`
+ * times with 16-byte loads: L2 bandwidth when bytes fits the L2 and repeats > 1, HBM otherwise. */
+mf_status mf_probe_read_bandwidth(mf_ctx* ctx, size_t bytes, int repeats, double* bytes_per_second);
+/* Evaluates the kernels' own device math element by element, for the accuracy tests:
+ * op 0 = exp (finite x < 709; x <= -708 gives 0), 1 = log (positive normal x), 2 = reciprocal.
+ * x_host, y_host: host, n doubles. */
+mf_status mf_probe_math(mf_ctx* ctx, int op, int64_t n, const double* x_host, double* y_host);
+
 #ifdef __cplusplus
 }
 #endif

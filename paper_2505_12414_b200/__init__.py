@@ -35,6 +35,7 @@ EXPORTS = [
     "mf_model_create", "mf_model_destroy", "mf_model_nparams", "mf_model_n_events", "mf_model_n_toys",
     "mf_nll_grad", "mf_nll_grad_async", "mf_nll_grad_batch",
     "mf_fit_opts_default", "mf_fit", "mf_fit_batch",
+    "mf_probe_fp64_rate", "mf_probe_read_bandwidth", "mf_probe_math",
 ]
 
 
@@ -133,6 +134,12 @@ def load_library() -> ctypes.CDLL:
     lib.mf_fit.argtypes = [vp, dp, u8p, ctypes.POINTER(FitOpts), ctypes.POINTER(_FitResultC)]
     lib.mf_fit_batch.restype = ctypes.c_int
     lib.mf_fit_batch.argtypes = [vp, i64, dp, u8p, ctypes.POINTER(FitOpts), ctypes.POINTER(_FitResultC)]
+    lib.mf_probe_fp64_rate.restype = ctypes.c_int
+    lib.mf_probe_fp64_rate.argtypes = [vp, dp]
+    lib.mf_probe_read_bandwidth.restype = ctypes.c_int
+    lib.mf_probe_read_bandwidth.argtypes = [vp, ctypes.c_size_t, ctypes.c_int, dp]
+    lib.mf_probe_math.restype = ctypes.c_int
+    lib.mf_probe_math.argtypes = [vp, ctypes.c_int, i64, dp, dp]
     _lib = lib
     return lib
 
@@ -174,6 +181,25 @@ class Context:
     @property
     def kernel_launches(self) -> int:
         return int(self._lib.mf_ctx_kernel_launches(self._h))
+
+    def probe_fp64_rate(self) -> float:
+        """Measured fp64-pipe rate (DFMA thread-instructions per second)."""
+        v = ctypes.c_double()
+        self._check(self._lib.mf_probe_fp64_rate(self._h, ctypes.byref(v)))
+        return float(v.value)
+
+    def probe_read_bandwidth(self, nbytes: int, repeats: int = 1) -> float:
+        """Measured read bandwidth (bytes/s) of an nbytes working set read `repeats` times."""
+        v = ctypes.c_double()
+        self._check(self._lib.mf_probe_read_bandwidth(self._h, int(nbytes), int(repeats), ctypes.byref(v)))
+        return float(v.value)
+
+    def probe_math(self, op: str, x) -> np.ndarray:
+        """The kernels' device exp / log / rcp evaluated element-wise (accuracy tests)."""
+        x = np.ascontiguousarray(x, dtype=np.float64)
+        y = np.empty_like(x)
+        self._check(self._lib.mf_probe_math(self._h, {"exp": 0, "log": 1, "rcp": 2}[op], x.size, _dp(x), _dp(y)))
+        return y
 
     def dataset_upload(self, columns, lo=None, hi=None, n_toys: int = 1) -> "Dataset":
         """columns: numpy array [ndim][n_toys*n_events] (or 1-D for ndim = 1; [n_toys][n_events] for

@@ -267,9 +267,11 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
         }
         for (int k = 0; k < 9; ++k) m->col[c++] = m->cache + k * per_dim;
     }
-    // launch geometry: persistent-style grid, 2 CTAs per SM, never more CTAs than 8-warp groups of items
+    // launch geometry: persistent-style grid, CTAS_PER_SM CTAs per SM (one wave), never more CTAs than 8-warp groups of items
     const int64_t n_items = m->n_pad / kItem;
-    m->grid = (int)std::max<int64_t>(1, std::min<int64_t>((n_items + kWarps - 1) / kWarps, 2 * (int64_t)ctx->sm_count));
+    const int ctas_per_sm = (kind == MF_MASS_X_ANGULAR) ? FourDModel::CTAS_PER_SM
+                            : (kind == MF_ANGULAR_KSTMUMU) ? AngularModel::CTAS_PER_SM : MassModel::CTAS_PER_SM;
+    m->grid = (int)std::max<int64_t>(1, std::min<int64_t>((n_items + kWarps - 1) / kWarps, ctas_per_sm * (int64_t)ctx->sm_count));
     // batch geometry: one CTA per toy up to 32768 events per toy, else split
     m->chunks = (int)std::max<int64_t>(1, std::min<int64_t>((m->n_pad + 32767) / 32768, 64));
     MF_CUDA_M(cudaMalloc(&m->partials, sizeof(double) * m->nacc * m->grid));

@@ -28,6 +28,7 @@ namespace mf {
 constexpr int kBlock = 256;
 constexpr int kWarps = kBlock / 32;
 constexpr int kItem = 64;  // events per warp item
+constexpr int kFinalBatch = 10;  // partials per lane loaded together in the final pass (covers 2 CTAs/SM x 148 SMs)
 
 template <class M>
 struct EvalArgs {
@@ -88,40 +89,66 @@ __device__ __forceinline__ void load_item(const double* const* col, int64_t j, i
     }
 }
 
-// Items j0, j0 + step, j0 + 2 step, ... < n_items; only item n_items - 1 can be ragged.
+// One group = U items (j, j + step, ...) of this warp; only item n_items - 1 can be ragged.
+template <class M, int U>
+__device__ __forceinline__ void load_group(const double* const* col, int64_t n_items, int64_t j, int64_t step, int lane,
+                                           double (&buf)[U][2][M::NCOL])
+{
+#pragma unroll
+    for (int u = 0; u < U; ++u)
+        if (j + u * step < n_items) load_item<M>(col, j + u * step, lane, buf[u][0], buf[u][1]);
+}
+
+template <class M, int U>
+__device__ __forceinline__ void compute_group(int64_t n, int64_t n_items, int64_t j, int64_t step, int lane,
+                                              const double (&buf)[U][2][M::NCOL], const typename M::Consts& c,
+                                              double* acc, int& esum, unsigned& bad, const double2* __restrict__ tab)
+{
+    const int64_t jl = j + (U - 1) * step;  // last item of the group
+    if (jl < n_items && kItem * (jl + 1) <= n) {
+        // fast path: 2U independent events, no predicates, free for the compiler to interleave
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            M::template event<false>(buf[u][0], c, acc, esum, bad, true, tab);
+            M::template event<false>(buf[u][1], c, acc, esum, bad, true, tab);
+        }
+    } else {
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int64_t ju = j + u * step;
+            if (ju < n_items) {
+                const int64_t e = kItem * ju + 2 * lane;
+                M::template event<true>(buf[u][0], c, acc, esum, bad, e < n, tab);
+                M::template event<true>(buf[u][1], c, acc, esum, bad, e + 1 < n, tab);
+            }
+        }
+    }
+}
+
+// Items j0, j0 + step, j0 + 2 step, ... < n_items, U per iteration, software-pipelined: the
+// loads of the next group are in flight while the current group is evaluated (two register
+// buffers, ping-pong).
 template <class M>
 __device__ __forceinline__ void accumulate(const double* const* col, int64_t n, int64_t n_items, int64_t j0,
-                                           int64_t step, const typename M::Consts& c, double* acc, unsigned& bad)
+                                           int64_t step, const typename M::Consts& c, double* acc, unsigned& bad,
+                                           const double2* __restrict__ tab)
 {
+    constexpr int U = M::ITEMS_PER_ITER;
     const int lane = threadIdx.x & 31;
+    int esum = 0;
+    double A[U][2][M::NCOL], B[U][2][M::NCOL];
     int64_t j = j0;
-    for (; j + step < n_items; j += 2 * step) {
-        double xa[M::NCOL], xb[M::NCOL], ya[M::NCOL], yb[M::NCOL];
-        load_item<M>(col, j, lane, xa, xb);
-        load_item<M>(col, j + step, lane, ya, yb);
-        M::template event<false>(xa, c, acc, bad, true);
-        M::template event<false>(xb, c, acc, bad, true);
-        if (kItem * (j + step + 1) <= n) {
-            M::template event<false>(ya, c, acc, bad, true);
-            M::template event<false>(yb, c, acc, bad, true);
-        } else {
-            const int64_t e = kItem * (j + step) + 2 * lane;
-            M::template event<true>(ya, c, acc, bad, e < n);
-            M::template event<true>(yb, c, acc, bad, e + 1 < n);
-        }
+    load_group<M, U>(col, n_items, j, step, lane, A);
+    while (j < n_items) {
+        load_group<M, U>(col, n_items, j + U * step, step, lane, B);
+        compute_group<M, U>(n, n_items, j, step, lane, A, c, acc, esum, bad, tab);
+        j += U * step;
+        if (j >= n_items) break;
+        load_group<M, U>(col, n_items, j + U * step, step, lane, A);
+        compute_group<M, U>(n, n_items, j, step, lane, B, c, acc, esum, bad, tab);
+        j += U * step;
     }
-    if (j < n_items) {
-        double xa[M::NCOL], xb[M::NCOL];
-        load_item<M>(col, j, lane, xa, xb);
-        if (kItem * (j + 1) <= n) {
-            M::template event<false>(xa, c, acc, bad, true);
-            M::template event<false>(xb, c, acc, bad, true);
-        } else {
-            const int64_t e = kItem * j + 2 * lane;
-            M::template event<true>(xa, c, acc, bad, e < n);
-            M::template event<true>(xb, c, acc, bad, e + 1 < n);
-        }
-    }
+    acc[0] = fma((double)esum, MF_LN2, acc[0]);  // the binary exponents of the P_i, summed exactly
 }
 
 // ---- S4: thread -> warp -> block ---------------------------------------------------------------
@@ -175,11 +202,20 @@ __device__ __forceinline__ void final_combine(const double* p, int64_t stride_k,
     for (int k = w; k < NACC; k += kWarps) {
         const double* pk = p + k * stride_k;
         double s = 0.0, c = 0.0;  // Kahan: true sum ~ s - c
-        for (int i = lane; i < count; i += 32) {
-            const double y = __ldcg(pk + i) - c;
-            const double t = s + y;
-            c = (t - s) - y;
-            s = t;
+        for (int i0 = lane; i0 < count; i0 += 32 * kFinalBatch) {
+            double v[kFinalBatch];  // issue the loads of a batch together, then add them in index order
+#pragma unroll
+            for (int u = 0; u < kFinalBatch; ++u) {
+                const int i = i0 + 32 * u;
+                v[u] = (i < count) ? __ldcg(pk + i) : 0.0;
+            }
+#pragma unroll
+            for (int u = 0; u < kFinalBatch; ++u) {
+                const double y = v[u] - c;
+                const double t = s + y;
+                c = (t - s) - y;
+                s = t;
+            }
         }
         double lo = -c;
 #pragma unroll
@@ -204,20 +240,23 @@ __device__ __forceinline__ void final_combine(const double* p, int64_t stride_k,
 // ---- the fused single-dataset kernel (mf_nll_grad) ----------------------------------------------
 
 template <class M>
-__global__ void __launch_bounds__(kBlock, 2) nll_grad_kernel(const __grid_constant__ EvalArgs<M> a)
+__global__ void __launch_bounds__(kBlock, M::CTAS_PER_SM) nll_grad_kernel(const __grid_constant__ EvalArgs<M> a)
 {
     constexpr int NACC = M::NACC;
     __shared__ double sm[kWarps][NACC];
     __shared__ unsigned sm_bad[kWarps];
     __shared__ unsigned s_bad_block;
     __shared__ bool s_last;
+    __shared__ double2 s_tab[kLogTableSize];
 
+    load_log_table(s_tab);
+    __syncthreads();
     double acc[NACC];
 #pragma unroll
     for (int k = 0; k < NACC; ++k) acc[k] = 0.0;
     unsigned bad = 0;
     const int64_t G = gridDim.x;
-    accumulate<M>(a.col, a.n, a.n_items, blockIdx.x + G * (threadIdx.x >> 5), G * kWarps, a.c, acc, bad);
+    accumulate<M>(a.col, a.n, a.n_items, blockIdx.x + G * (threadIdx.x >> 5), G * kWarps, a.c, acc, bad, s_tab);
 
     const double s = block_reduce<NACC>(acc, bad, sm, sm_bad, &s_bad_block);
     if (threadIdx.x < NACC) {
@@ -240,7 +279,7 @@ __global__ void __launch_bounds__(kBlock, 2) nll_grad_kernel(const __grid_consta
 // ---- the batched-toy kernel (mf_nll_grad_batch): CTA <-> (toy, event chunk) ----------------------
 
 template <class M>
-__global__ void __launch_bounds__(kBlock, 2) nll_grad_batch_kernel(const __grid_constant__ BatchArgs<M> a)
+__global__ void __launch_bounds__(kBlock, M::CTAS_PER_SM) nll_grad_batch_kernel(const __grid_constant__ BatchArgs<M> a)
 {
     constexpr int NACC = M::NACC;
     constexpr int K = M::K;
@@ -250,7 +289,9 @@ __global__ void __launch_bounds__(kBlock, 2) nll_grad_batch_kernel(const __grid_
     __shared__ bool s_last;
     __shared__ typename M::Consts s_c;
     __shared__ int s_ok;
+    __shared__ double2 s_tab[kLogTableSize];
 
+    load_log_table(s_tab);
     const int slot = blockIdx.x / a.chunks, chunk = blockIdx.x % a.chunks;
     // S2 for this toy: parameter-only constants from lambda_t, once per CTA
     if (threadIdx.x == 0) s_ok = make_consts<M>(a.lam + (int64_t)slot * K, a.ma, a.mb, s_c) ? 1 : 0;
@@ -274,7 +315,7 @@ __global__ void __launch_bounds__(kBlock, 2) nll_grad_batch_kernel(const __grid_
     for (int k = 0; k < NACC; ++k) acc[k] = 0.0;
     unsigned bad = 0;
     const int64_t C = a.chunks;
-    accumulate<M>(col, a.n, a.n_items, chunk + C * (threadIdx.x >> 5), C * kWarps, c, acc, bad);
+    accumulate<M>(col, a.n, a.n_items, chunk + C * (threadIdx.x >> 5), C * kWarps, c, acc, bad, s_tab);
 
     const double s = block_reduce<NACC>(acc, bad, sm, sm_bad, &s_bad_block);
     if (a.chunks == 1) {  // the CTA holds the toy's complete sums: no cross-CTA pass

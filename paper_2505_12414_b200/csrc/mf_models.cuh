@@ -103,6 +103,14 @@ MF_HD inline bool mass_consts(const double* lam, double ma, double mb, MassConst
     c.ksig = is + ((ma - mu) * ga - (mb - mu) * gb) * is * iN1;
     c.ma = ma;
     c.ktau = w * (0.5 + 0.5 * langevin(0.5 * tau * w));
+    // The kernels evaluate R = exp(-b0 (m-mu)^2 - tau m + lnk) with a range-restricted exp: refuse
+    // parameter points whose normalisations are not representable (N1 or N2 under/overflow) or
+    // whose largest possible exponent argument leaves the finite range.
+    if (!(isfinite(c.lnk) && isfinite(c.lnc2) && isfinite(c.kmu) && isfinite(c.ksig) && isfinite(c.nb0) &&
+          isfinite(c.is3)))
+        return false;
+    const double mmax = fmax(fabs(ma), fabs(mb));
+    if (!(c.lnk + fabs(tau) * mmax < 700.0)) return false;
     return true;
 }
 
@@ -146,7 +154,8 @@ MF_HD inline bool fourd_consts(const double* lam, double ma, double mb, FourDCon
 #ifdef __CUDACC__
 // ------------------------------------------------------------------------------------------
 // Per-event bodies (S3).  Each adds ln P_i to acc[0] and d ln P_i / d lambda_k to acc[1+k];
-// `bad` counts events with P <= 0 or NaN (SURVEY.md §8(c) reading 15); when it ends up
+// ln P_i is accumulated as (fraction in acc[0]) + (binary exponent in esum) * ln2, the exponent sum
+// being converted once per thread.  `bad` counts events with P <= 0 or NaN (SURVEY.md §8(c) reading 15); when it ends up
 // non-zero the sums are discarded by the final pass, so they are accumulated unconditionally.  PRED = true is the
 // ragged-tail variant: lanes with valid == false contribute exactly 0 (reading 10).
 // ------------------------------------------------------------------------------------------
@@ -155,20 +164,24 @@ struct MassModel {
     static constexpr int K = 4;
     static constexpr int NCOL = 1;  // m
     static constexpr int NACC = 5;
+    static constexpr int ITEMS_PER_ITER = 2;  // 4 independent events in flight per thread (ALU bound)
+    static constexpr int CTAS_PER_SM = 2;
     using Consts = MassConsts;
 
     template <bool PRED>
-    static MF_D void event(const double* x, const Consts& c, double* acc, unsigned& bad, bool valid)
+    static MF_D void event(const double* x, const Consts& c, double* acc, int& esum, unsigned& bad, bool valid,
+                           const double2* __restrict__ tab)
     {
         const double m = x[0];
         const double d = m - c.mu;
         const double t = d * d;
-        // ln R = -b0 d^2 - tau m + ln(c1/c2); clamped so R stays finite
-        const double arg = fmin(fma(c.nb0, t, fma(-c.tau, m, c.lnk)), 700.0);
+        // ln R = -b0 d^2 - tau m + ln(c1/c2)
+        const double arg = fma(c.nb0, t, fma(-c.tau, m, c.lnk));  // < 700 by the check in mass_consts
         const double R = mf_exp(arg);
         const double D = fma(c.f, R, c.omf);  // P N2 e^{-tau m} = (1-f) + f R
         const double r = mf_rcp(D);
-        const double lnP = fma(c.tau, m, c.lnc2) + mf_log(D);
+        int e = 0;
+        const double lnP = fma(c.tau, m, c.lnc2) + mf_log_frac(D, tab, e);  // + e ln2, summed as an integer
         const double u = R * r;               // (G/N1)/P
         const double ws = c.f * u;            // signal weight  f (G/N1) / P
         const double wb = c.omf * r;          // background weight (1-f)(E/N2)/P
@@ -179,6 +192,7 @@ struct MassModel {
         const bool good = D > 0.0;
         if (!PRED || valid) {
             bad += good ? 0u : 1u;
+            esum += e;
             {
                 acc[0] += lnP;
                 acc[1] += gf;
@@ -194,19 +208,24 @@ struct AngularModel {
     static constexpr int K = 8;
     static constexpr int NCOL = 9;  // h_0..h_8 (cached, already times 9/(32 pi))
     static constexpr int NACC = 9;
+    static constexpr int ITEMS_PER_ITER = 1;  // memory bound: depth comes from the prefetched next item
+    static constexpr int CTAS_PER_SM = 2;
     using Consts = AngularConsts;
 
     template <bool PRED>
-    static MF_D void event(const double* x, const Consts& c, double* acc, unsigned& bad, bool valid)
+    static MF_D void event(const double* x, const Consts& c, double* acc, int& esum, unsigned& bad, bool valid,
+                           const double2* __restrict__ tab)
     {
         double P = fma(c.a[0], x[1], x[0]);
 #pragma unroll
         for (int k = 1; k < 8; ++k) P = fma(c.a[k], x[1 + k], P);
         const double r = mf_rcp(P);
-        const double lnP = mf_log(P);
+        int e = 0;
+        const double lnP = mf_log_frac(P, tab, e);
         const bool good = P > 0.0;
         if (!PRED || valid) {
             bad += good ? 0u : 1u;
+            esum += e;
             {
                 acc[0] += lnP;
 #pragma unroll
@@ -220,10 +239,13 @@ struct FourDModel {
     static constexpr int K = 16;
     static constexpr int NCOL = 12;  // m, cos theta_l, cos theta_K, h_0..h_8
     static constexpr int NACC = 17;
+    static constexpr int ITEMS_PER_ITER = 1;
+    static constexpr int CTAS_PER_SM = 1;  // 17 sums + two 12-column register buffers: needs > 128 registers
     using Consts = FourDConsts;
 
     template <bool PRED>
-    static MF_D void event(const double* x, const Consts& c, double* acc, unsigned& bad, bool valid)
+    static MF_D void event(const double* x, const Consts& c, double* acc, int& esum, unsigned& bad, bool valid,
+                           const double2* __restrict__ tab)
     {
         const MassConsts& q = c.m;
         const double m = x[0], cl = x[1], ck = x[2];
@@ -238,13 +260,14 @@ struct FourDModel {
         const double lk = fma(c.ck2, p2k, fma(c.ck1, ck, 1.0));
         const double d = m - q.mu;
         const double t = d * d;
-        const double arg = fmin(fma(q.nb0, t, fma(-q.tau, m, q.lnk)), 700.0);
+        const double arg = fma(q.nb0, t, fma(-q.tau, m, q.lnk));  // < 700 by the check in mass_consts
         const double R = mf_exp(arg);          // (G/N1)/(E/N2)
         const double omfL = c.kappa * (ll * lk);  // (1-f) L
         const double fR = q.f * R;
         const double D = fma(fR, A, omfL);     // P N2 e^{-tau m}
         const double r = mf_rcp(D);
-        const double lnP = fma(q.tau, m, q.lnc2) + mf_log(D);
+        int e = 0;
+        const double lnP = fma(q.tau, m, q.lnc2) + mf_log_frac(D, tab, e);
         const double ws = fR * A * r;          // f (G/N1) A / P
         const double wb = omfL * r;            // (1-f)(E/N2) L / P
         const double gf = fma(R * A, r, -(ll * lk) * kInv8Pi * r);
@@ -257,6 +280,7 @@ struct FourDModel {
         const bool good = D > 0.0;
         if (!PRED || valid) {
             bad += good ? 0u : 1u;
+            esum += e;
             {
                 acc[0] += lnP;
                 acc[1] += gf;

@@ -1,0 +1,143 @@
+// mf_probe.cu — the two roofline denominators that MEASURED_PEAKS.json does not hold
+// (SURVEY.md §7 step 0): the fp64-pipe issue rate (register-only DFMA chains) and the read
+// bandwidth of a working set that is re-read in a loop (L2-resident when it fits the 126 MB
+// L2, HBM otherwise).  Measurement helpers only; nothing on the hot path calls them.
+#include <cuda_runtime.h>
+
+#include <string>
+
+#include "mf_internal.h"
+#include "mf_math.cuh"
+
+namespace {
+
+// 8 independent DFMA chains per thread: enough ILP to cover the pipe latency at any occupancy.
+__global__ void __launch_bounds__(256) dfma_chain_kernel(double* out, int iters, double a, double b)
+{
+    double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+#pragma unroll 1
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+            x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+        }
+    }
+    const double s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+    if (s == 123.456) out[0] = s;  // never true for these inputs; keeps the chains alive
+}
+
+__global__ void __launch_bounds__(256) read_kernel(const double2* __restrict__ p, size_t n_vec, int repeats, double* out)
+{
+    double s = 0.0;
+    for (int r = 0; r < repeats; ++r)
+        for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n_vec; i += (size_t)gridDim.x * blockDim.x) {
+            const double2 v = __ldg(p + i);
+            s += v.x + v.y;
+        }
+    if (s == 123.456) out[0] = s;
+}
+
+
+// Element-wise evaluation of the device math of mf_math.cuh (op 0: mf_exp, 1: mf_log, 2: mf_rcp).
+__global__ void __launch_bounds__(256) math_kernel(int op, int64_t n, const double* __restrict__ x, double* __restrict__ y)
+{
+    __shared__ double2 s_tab[mf::kLogTableSize];
+    mf::load_log_table(s_tab);
+    __syncthreads();
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const double v = x[i];
+        y[i] = op == 0 ? mf::mf_exp(v) : op == 1 ? mf::mf_log(v, s_tab) : mf::mf_rcp(v);
+    }
+}
+
+}  // namespace
+
+#define MF_CUDA(ctx, call)                                                                        \
+    do {                                                                                          \
+        cudaError_t e__ = (call);                                                                 \
+        if (e__ != cudaSuccess)                                                                   \
+            return mf_fail(ctx, MF_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e__)); \
+    } while (0)
+
+extern "C" mf_status mf_probe_fp64_rate(mf_ctx* ctx, double* dfma_per_second)
+{
+    if (!ctx || !dfma_per_second) return mf_fail(ctx, MF_ERR_ARG, "mf_probe_fp64_rate: NULL argument");
+    MF_CUDA(ctx, cudaSetDevice(ctx->device));
+    double* d_out = nullptr;
+    MF_CUDA(ctx, cudaMalloc(&d_out, sizeof(double)));
+    cudaEvent_t e0, e1;
+    MF_CUDA(ctx, cudaEventCreate(&e0));
+    MF_CUDA(ctx, cudaEventCreate(&e1));
+    const int grid = ctx->sm_count * 4, iters = 4096;
+    double best = 0.0;
+    for (int rep = 0; rep < 6; ++rep) {
+        MF_CUDA(ctx, cudaEventRecord(e0, ctx->stream));
+        dfma_chain_kernel<<<grid, 256, 0, ctx->stream>>>(d_out, iters, 0.999999, 1e-9);
+        ++ctx->launches;
+        MF_CUDA(ctx, cudaEventRecord(e1, ctx->stream));
+        MF_CUDA(ctx, cudaEventSynchronize(e1));
+        float ms = 0;
+        MF_CUDA(ctx, cudaEventElapsedTime(&ms, e0, e1));
+        const double rate = (double)grid * 256.0 * 64.0 * iters / (ms * 1e-3);
+        if (rep > 0 && rate > best) best = rate;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(d_out);
+    *dfma_per_second = best;
+    return MF_OK;
+}
+
+extern "C" mf_status mf_probe_read_bandwidth(mf_ctx* ctx, size_t bytes, int repeats, double* bytes_per_second)
+{
+    if (!ctx || !bytes_per_second || bytes < 4096 || repeats < 1)
+        return mf_fail(ctx, MF_ERR_ARG, "mf_probe_read_bandwidth: bad argument");
+    MF_CUDA(ctx, cudaSetDevice(ctx->device));
+    const size_t n_vec = bytes / sizeof(double2);
+    double2* buf = nullptr;
+    double* d_out = nullptr;
+    MF_CUDA(ctx, cudaMalloc(&buf, n_vec * sizeof(double2)));
+    MF_CUDA(ctx, cudaMalloc(&d_out, sizeof(double)));
+    MF_CUDA(ctx, cudaMemsetAsync(buf, 0, n_vec * sizeof(double2), ctx->stream));
+    cudaEvent_t e0, e1;
+    MF_CUDA(ctx, cudaEventCreate(&e0));
+    MF_CUDA(ctx, cudaEventCreate(&e1));
+    const int grid = ctx->sm_count * 8;
+    double best = 0.0;
+    for (int rep = 0; rep < 4; ++rep) {
+        MF_CUDA(ctx, cudaEventRecord(e0, ctx->stream));
+        read_kernel<<<grid, 256, 0, ctx->stream>>>(buf, n_vec, repeats, d_out);
+        ++ctx->launches;
+        MF_CUDA(ctx, cudaEventRecord(e1, ctx->stream));
+        MF_CUDA(ctx, cudaEventSynchronize(e1));
+        float ms = 0;
+        MF_CUDA(ctx, cudaEventElapsedTime(&ms, e0, e1));
+        const double rate = (double)n_vec * sizeof(double2) * repeats / (ms * 1e-3);
+        if (rep > 0 && rate > best) best = rate;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(buf);
+    cudaFree(d_out);
+    *bytes_per_second = best;
+    return MF_OK;
+}
+
+extern "C" mf_status mf_probe_math(mf_ctx* ctx, int op, int64_t n, const double* x_host, double* y_host)
+{
+    if (!ctx || !x_host || !y_host || n < 1 || op < 0 || op > 2) return mf_fail(ctx, MF_ERR_ARG, "mf_probe_math: bad argument");
+    MF_CUDA(ctx, cudaSetDevice(ctx->device));
+    double *dx = nullptr, *dy = nullptr;
+    MF_CUDA(ctx, cudaMalloc(&dx, sizeof(double) * n));
+    MF_CUDA(ctx, cudaMalloc(&dy, sizeof(double) * n));
+    MF_CUDA(ctx, cudaMemcpyAsync(dx, x_host, sizeof(double) * n, cudaMemcpyHostToDevice, ctx->stream));
+    math_kernel<<<(int)((n + 255) / 256 > 1184 ? 1184 : (n + 255) / 256), 256, 0, ctx->stream>>>(op, n, dx, dy);
+    ++ctx->launches;
+    MF_CUDA(ctx, cudaGetLastError());
+    MF_CUDA(ctx, cudaMemcpyAsync(y_host, dy, sizeof(double) * n, cudaMemcpyDeviceToHost, ctx->stream));
+    MF_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    cudaFree(dx);
+    cudaFree(dy);
+    return MF_OK;
+}

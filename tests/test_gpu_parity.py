@@ -261,3 +261,25 @@ def test_fit_batch_small(mf, ctx):
     for t in range(T):
         o = oracle.fit(oracle.MASS, toys[t], dg.MASS_TRUTH, lo=dg.MASS_LO, hi=dg.MASS_HI)
         _assert_fit_agrees(res[t], o)
+
+
+def _ulp_err(y, ref):
+    return np.abs(y - ref) / np.spacing(np.abs(ref))
+
+
+def test_device_math_accuracy(mf, ctx):
+    """The kernels' own exp / log / reciprocal (mf_math.cuh) against numpy's libm: a few ulp at most."""
+    rng = np.random.default_rng(0)
+    x = np.concatenate([rng.uniform(-707.9, 700.0, 200_000), rng.uniform(-5, 5, 200_000), [0.0, -0.0, 1e-300, -1e-300]])
+    y = ctx.probe_math("exp", x)
+    assert np.max(_ulp_err(y, np.exp(x))) <= 2.0
+    assert np.all(ctx.probe_math("exp", np.array([-708.0, -750.0, -1e4, -1e300])) == 0.0)
+    v = np.concatenate([np.exp(rng.uniform(-700, 700, 200_000)), rng.uniform(0.5, 2.0, 200_000),
+                        1.0 + rng.uniform(-1e-3, 1e-3, 100_000), [1.0, 2.0, 0.5, 2.2250738585072014e-308]])
+    lg = ctx.probe_math("log", v)
+    ref = np.log(v)
+    # absolute error matters for sums of ln P: <= 2 ulp of max(|ln v|, ~0.35) (log is exact at 1)
+    assert np.max(np.abs(lg - ref) / np.spacing(np.maximum(np.abs(ref), 0.35))) <= 2.0
+    assert ctx.probe_math("log", np.array([1.0]))[0] == 0.0
+    r = ctx.probe_math("rcp", v)
+    assert np.max(_ulp_err(r, 1.0 / v)) <= 2.0
