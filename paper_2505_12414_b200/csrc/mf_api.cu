@@ -4,6 +4,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -305,6 +306,29 @@ extern "C" int64_t mf_model_n_toys(const mf_model* m) { return m ? m->n_toys : 0
 
 // ------------------------------------------------------------------------------ S2..S6
 
+// Launch with programmatic stream serialisation: the kernel may begin while its predecessor on the
+// stream (if that is one of ours) is still in its tail; see pdl_wait() in mf_kernels.cuh.
+template <class Args>
+static cudaError_t launch_pdl(void (*kernel)(const Args), int grid, cudaStream_t stream, const Args& a)
+{
+    static const bool no_pdl = std::getenv("MF_NO_PDL") != nullptr;  // ablation switch: plain stream order
+    if (no_pdl) {
+        kernel<<<grid, kBlock, 0, stream>>>(a);
+        return cudaGetLastError();
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(kBlock);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, a);
+}
+
 template <class M>
 static bool host_consts(const mf_model* m, const double* lam, typename M::Consts& c);
 template <>
@@ -332,13 +356,13 @@ static mf_status launch_single(mf_model* m, const double* lam, double* out_dev)
     for (int i = 0; i < M::NCOL; ++i) a.col[i] = m->col[i];
     a.n = m->n_events;
     a.n_items = m->n_pad / kItem;
+    a.lnp_offset = (double)m->n_events * M::lnp_const(a.c);
     a.partials = m->partials;
     a.bad_partials = m->bad_partials;
     a.ticket = m->ticket;
     a.out = out_dev;
-    nll_grad_kernel<M><<<m->grid, kBlock, 0, ctx->stream>>>(a);
+    MF_CUDA(ctx, launch_pdl(nll_grad_kernel<M>, m->grid, ctx->stream, a));
     ++ctx->launches;
-    MF_CUDA(ctx, cudaGetLastError());
     return MF_OK;
 }
 
@@ -392,9 +416,8 @@ static mf_status launch_batch(mf_model* m, int n_active)
     a.bad_partials = m->b_bad;
     a.ticket = m->ticket + 1;
     a.out = m->d_bout;
-    nll_grad_batch_kernel<M><<<n_active * m->chunks, kBlock, 0, ctx->stream>>>(a);
+    MF_CUDA(ctx, launch_pdl(nll_grad_batch_kernel<M>, n_active * m->chunks, ctx->stream, a));
     ++ctx->launches;
-    MF_CUDA(ctx, cudaGetLastError());
     return MF_OK;
 }
 

@@ -36,6 +36,7 @@ struct EvalArgs {
     int64_t n;                   // valid events
     int64_t n_items;             // n_pad / 64
     typename M::Consts c;        // parameter-only constants (S2), computed on the host
+    double lnp_offset;           // N * (per-event constant of ln P), added once in the final pass
     double* partials;            // [NACC][gridDim.x]
     unsigned* bad_partials;      // [gridDim.x]
     unsigned* ticket;            // zero on entry, reset to zero by the last CTA
@@ -76,6 +77,14 @@ __device__ __forceinline__ bool make_consts<FourDModel>(const double* lam, doubl
     return fourd_consts(lam, ma, mb, c);
 }
 
+// ---- programmatic dependent launch (back-to-back evaluations on one stream) --------------------
+// The event loop only reads the immutable dataset columns, so it may run while the previous
+// evaluation is still reducing: every kernel lets its successor start at once and waits for
+// its predecessor to complete only before it touches the shared scratch (partials, ticket) and
+// the output.  Without the launch attribute both instructions are no-ops.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // ---- S3: the event loop of one warp ---------------------------------------------------------
 
 template <class M>
@@ -102,15 +111,15 @@ __device__ __forceinline__ void load_group(const double* const* col, int64_t n_i
 template <class M, int U>
 __device__ __forceinline__ void compute_group(int64_t n, int64_t n_items, int64_t j, int64_t step, int lane,
                                               const double (&buf)[U][2][M::NCOL], const typename M::Consts& c,
-                                              double* acc, int& esum, unsigned& bad, const double2* __restrict__ tab)
+                                              double* acc, LogProd& lp, unsigned& bad)
 {
     const int64_t jl = j + (U - 1) * step;  // last item of the group
     if (jl < n_items && kItem * (jl + 1) <= n) {
         // fast path: 2U independent events, no predicates, free for the compiler to interleave
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            M::template event<false>(buf[u][0], c, acc, esum, bad, true, tab);
-            M::template event<false>(buf[u][1], c, acc, esum, bad, true, tab);
+            M::template event<false>(buf[u][0], c, acc, lp, bad, true);
+            M::template event<false>(buf[u][1], c, acc, lp, bad, true);
         }
     } else {
 #pragma unroll
@@ -118,11 +127,12 @@ __device__ __forceinline__ void compute_group(int64_t n, int64_t n_items, int64_
             const int64_t ju = j + u * step;
             if (ju < n_items) {
                 const int64_t e = kItem * ju + 2 * lane;
-                M::template event<true>(buf[u][0], c, acc, esum, bad, e < n, tab);
-                M::template event<true>(buf[u][1], c, acc, esum, bad, e + 1 < n, tab);
+                M::template event<true>(buf[u][0], c, acc, lp, bad, e < n);
+                M::template event<true>(buf[u][1], c, acc, lp, bad, e + 1 < n);
             }
         }
     }
+    lp.renorm();  // at most 2U mantissas in [1,2) since the last one
 }
 
 // Items j0, j0 + step, j0 + 2 step, ... < n_items, U per iteration, software-pipelined: the
@@ -130,25 +140,24 @@ __device__ __forceinline__ void compute_group(int64_t n, int64_t n_items, int64_
 // buffers, ping-pong).
 template <class M>
 __device__ __forceinline__ void accumulate(const double* const* col, int64_t n, int64_t n_items, int64_t j0,
-                                           int64_t step, const typename M::Consts& c, double* acc, unsigned& bad,
-                                           const double2* __restrict__ tab)
+                                           int64_t step, const typename M::Consts& c, double* acc, unsigned& bad)
 {
     constexpr int U = M::ITEMS_PER_ITER;
     const int lane = threadIdx.x & 31;
-    int esum = 0;
+    LogProd lp;
     double A[U][2][M::NCOL], B[U][2][M::NCOL];
     int64_t j = j0;
     load_group<M, U>(col, n_items, j, step, lane, A);
     while (j < n_items) {
         load_group<M, U>(col, n_items, j + U * step, step, lane, B);
-        compute_group<M, U>(n, n_items, j, step, lane, A, c, acc, esum, bad, tab);
+        compute_group<M, U>(n, n_items, j, step, lane, A, c, acc, lp, bad);
         j += U * step;
         if (j >= n_items) break;
         load_group<M, U>(col, n_items, j + U * step, step, lane, A);
-        compute_group<M, U>(n, n_items, j, step, lane, B, c, acc, esum, bad, tab);
+        compute_group<M, U>(n, n_items, j, step, lane, B, c, acc, lp, bad);
         j += U * step;
     }
-    acc[0] = fma((double)esum, MF_LN2, acc[0]);  // the binary exponents of the P_i, summed exactly
+    acc[0] += lp.log();  // the one logarithm of this thread
 }
 
 // ---- S4: thread -> warp -> block ---------------------------------------------------------------
@@ -190,10 +199,10 @@ __device__ __forceinline__ double block_reduce(double* acc, unsigned bad, double
 // ---- S5: fixed-order compensated combine of `count` partials per quantity ---------------------
 
 // Warp w combines quantities w, w + 8, ...; partial i of quantity k is at p[k * stride_k + i].
-// Writes out[0] = -sum_0 (= -ln L), out[1+k] = -sum_{1+k}, out[NACC] = n_bad; +inf / NaN if n_bad.
+// Writes out[0] = -(sum_0 + offset0) (= -ln L), out[1+k] = -sum_{1+k}, out[NACC] = n_bad; +inf / NaN if n_bad.
 template <int NACC>
 __device__ __forceinline__ void final_combine(const double* p, int64_t stride_k, int count, const unsigned* badp,
-                                              double* out)
+                                              double offset0, double* out)
 {
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     unsigned nb = 0;
@@ -229,7 +238,7 @@ __device__ __forceinline__ void final_combine(const double* p, int64_t stride_k,
             s = t;
         }
         if (lane == 0) {
-            double v = -(s + lo);
+            double v = -((s + lo) + (k == 0 ? offset0 : 0.0));
             if (nb) v = (k == 0) ? __longlong_as_double(0x7ff0000000000000LL) : __longlong_as_double(0x7ff8000000000000LL);
             out[k] = v;
         }
@@ -247,18 +256,17 @@ __global__ void __launch_bounds__(kBlock, M::CTAS_PER_SM) nll_grad_kernel(const 
     __shared__ unsigned sm_bad[kWarps];
     __shared__ unsigned s_bad_block;
     __shared__ bool s_last;
-    __shared__ double2 s_tab[kLogTableSize];
 
-    load_log_table(s_tab);
-    __syncthreads();
+    pdl_launch_dependents();
     double acc[NACC];
 #pragma unroll
     for (int k = 0; k < NACC; ++k) acc[k] = 0.0;
     unsigned bad = 0;
     const int64_t G = gridDim.x;
-    accumulate<M>(a.col, a.n, a.n_items, blockIdx.x + G * (threadIdx.x >> 5), G * kWarps, a.c, acc, bad, s_tab);
+    accumulate<M>(a.col, a.n, a.n_items, blockIdx.x + G * (threadIdx.x >> 5), G * kWarps, a.c, acc, bad);
 
     const double s = block_reduce<NACC>(acc, bad, sm, sm_bad, &s_bad_block);
+    pdl_wait();
     if (threadIdx.x < NACC) {
         a.partials[threadIdx.x * G + blockIdx.x] = s;
         __threadfence();
@@ -271,7 +279,7 @@ __global__ void __launch_bounds__(kBlock, M::CTAS_PER_SM) nll_grad_kernel(const 
     __syncthreads();
     if (s_last) {
         __threadfence();
-        final_combine<NACC>(a.partials, G, (int)G, a.bad_partials, a.out);
+        final_combine<NACC>(a.partials, G, (int)G, a.bad_partials, a.lnp_offset, a.out);
         if (threadIdx.x == 0) *a.ticket = 0u;
     }
 }
@@ -289,15 +297,15 @@ __global__ void __launch_bounds__(kBlock, M::CTAS_PER_SM) nll_grad_batch_kernel(
     __shared__ bool s_last;
     __shared__ typename M::Consts s_c;
     __shared__ int s_ok;
-    __shared__ double2 s_tab[kLogTableSize];
 
-    load_log_table(s_tab);
+    pdl_launch_dependents();
     const int slot = blockIdx.x / a.chunks, chunk = blockIdx.x % a.chunks;
     // S2 for this toy: parameter-only constants from lambda_t, once per CTA
     if (threadIdx.x == 0) s_ok = make_consts<M>(a.lam + (int64_t)slot * K, a.ma, a.mb, s_c) ? 1 : 0;
     __syncthreads();
     double* out = a.out + (int64_t)slot * (K + 2);
     if (!s_ok) {  // outside the parameter domain: +inf / NaN, n_bad = -1
+        pdl_wait();
         if (chunk == 0 && threadIdx.x <= K + 1)
             out[threadIdx.x] = threadIdx.x == 0       ? __longlong_as_double(0x7ff0000000000000LL)
                                : threadIdx.x == K + 1 ? -1.0
@@ -315,14 +323,16 @@ __global__ void __launch_bounds__(kBlock, M::CTAS_PER_SM) nll_grad_batch_kernel(
     for (int k = 0; k < NACC; ++k) acc[k] = 0.0;
     unsigned bad = 0;
     const int64_t C = a.chunks;
-    accumulate<M>(col, a.n, a.n_items, chunk + C * (threadIdx.x >> 5), C * kWarps, c, acc, bad, s_tab);
+    accumulate<M>(col, a.n, a.n_items, chunk + C * (threadIdx.x >> 5), C * kWarps, c, acc, bad);
 
     const double s = block_reduce<NACC>(acc, bad, sm, sm_bad, &s_bad_block);
+    const double offset0 = (double)a.n * M::lnp_const(c);
+    pdl_wait();
     if (a.chunks == 1) {  // the CTA holds the toy's complete sums: no cross-CTA pass
         __syncthreads();
         const unsigned nb = s_bad_block;
         if (threadIdx.x < NACC) {
-            double v = -s;
+            double v = -(s + (threadIdx.x == 0 ? offset0 : 0.0));
             if (nb) v = (threadIdx.x == 0) ? __longlong_as_double(0x7ff0000000000000LL) : __longlong_as_double(0x7ff8000000000000LL);
             out[threadIdx.x] = v;
         } else if (threadIdx.x == NACC) {
@@ -344,7 +354,7 @@ __global__ void __launch_bounds__(kBlock, M::CTAS_PER_SM) nll_grad_batch_kernel(
     __syncthreads();
     if (s_last) {
         __threadfence();
-        final_combine<NACC>(part, C, (int)C, badp, out);
+        final_combine<NACC>(part, C, (int)C, badp, offset0, out);
         if (threadIdx.x == 0) a.ticket[slot] = 0u;
     }
 }

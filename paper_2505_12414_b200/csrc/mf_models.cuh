@@ -153,9 +153,10 @@ MF_HD inline bool fourd_consts(const double* lam, double ma, double mb, FourDCon
 
 #ifdef __CUDACC__
 // ------------------------------------------------------------------------------------------
-// Per-event bodies (S3).  Each adds ln P_i to acc[0] and d ln P_i / d lambda_k to acc[1+k];
-// ln P_i is accumulated as (fraction in acc[0]) + (binary exponent in esum) * ln2, the exponent sum
-// being converted once per thread.  `bad` counts events with P <= 0 or NaN (SURVEY.md §8(c) reading 15); when it ends up
+// Per-event bodies (S3).  Each adds d ln P_i / d lambda_k to acc[1+k].  ln P_i is split: the factor of
+// P_i that needs a logarithm is multiplied into lp (LogProd, mf_math.cuh: sum of logs = log of the
+// product, taken once per thread), the part that is linear in the event goes to acc[0], and the
+// per-event constant is added once per call as N * Consts::lnp_const().  `bad` counts events with P <= 0 or NaN (SURVEY.md §8(c) reading 15); when it ends up
 // non-zero the sums are discarded by the final pass, so they are accumulated unconditionally.  PRED = true is the
 // ragged-tail variant: lanes with valid == false contribute exactly 0 (reading 10).
 // ------------------------------------------------------------------------------------------
@@ -168,9 +169,11 @@ struct MassModel {
     static constexpr int CTAS_PER_SM = 2;
     using Consts = MassConsts;
 
+    // ln P = [tau m] + [-ln N2] + ln D
+    static MF_HD double lnp_const(const Consts& c) { return c.lnc2; }
+
     template <bool PRED>
-    static MF_D void event(const double* x, const Consts& c, double* acc, int& esum, unsigned& bad, bool valid,
-                           const double2* __restrict__ tab)
+    static MF_D void event(const double* x, const Consts& c, double* acc, LogProd& lp, unsigned& bad, bool valid)
     {
         const double m = x[0];
         const double d = m - c.mu;
@@ -180,8 +183,6 @@ struct MassModel {
         const double R = mf_exp(arg);
         const double D = fma(c.f, R, c.omf);  // P N2 e^{-tau m} = (1-f) + f R
         const double r = mf_rcp(D);
-        int e = 0;
-        const double lnP = fma(c.tau, m, c.lnc2) + mf_log_frac(D, tab, e);  // + e ln2, summed as an integer
         const double u = R * r;               // (G/N1)/P
         const double ws = c.f * u;            // signal weight  f (G/N1) / P
         const double wb = c.omf * r;          // background weight (1-f)(E/N2)/P
@@ -192,14 +193,12 @@ struct MassModel {
         const bool good = D > 0.0;
         if (!PRED || valid) {
             bad += good ? 0u : 1u;
-            esum += e;
-            {
-                acc[0] += lnP;
-                acc[1] += gf;
-                acc[2] = fma(ws, hmu, acc[2]);
-                acc[3] = fma(ws, hsig, acc[3]);
-                acc[4] = fma(wb, htau, acc[4]);
-            }
+            lp.mul(D);
+            acc[0] = fma(c.tau, m, acc[0]);
+            acc[1] += gf;
+            acc[2] = fma(ws, hmu, acc[2]);
+            acc[3] = fma(ws, hsig, acc[3]);
+            acc[4] = fma(wb, htau, acc[4]);
         }
     }
 };
@@ -212,25 +211,21 @@ struct AngularModel {
     static constexpr int CTAS_PER_SM = 2;
     using Consts = AngularConsts;
 
+    static MF_HD double lnp_const(const Consts&) { return 0.0; }
+
     template <bool PRED>
-    static MF_D void event(const double* x, const Consts& c, double* acc, int& esum, unsigned& bad, bool valid,
-                           const double2* __restrict__ tab)
+    static MF_D void event(const double* x, const Consts& c, double* acc, LogProd& lp, unsigned& bad, bool valid)
     {
         double P = fma(c.a[0], x[1], x[0]);
 #pragma unroll
         for (int k = 1; k < 8; ++k) P = fma(c.a[k], x[1 + k], P);
         const double r = mf_rcp(P);
-        int e = 0;
-        const double lnP = mf_log_frac(P, tab, e);
         const bool good = P > 0.0;
         if (!PRED || valid) {
             bad += good ? 0u : 1u;
-            esum += e;
-            {
-                acc[0] += lnP;
+            lp.mul(P);  // acc[0] stays 0: ln P is all in the product
 #pragma unroll
-                for (int k = 0; k < 8; ++k) acc[1 + k] = fma(x[1 + k], r, acc[1 + k]);
-            }
+            for (int k = 0; k < 8; ++k) acc[1 + k] = fma(x[1 + k], r, acc[1 + k]);
         }
     }
 };
@@ -243,9 +238,10 @@ struct FourDModel {
     static constexpr int CTAS_PER_SM = 1;  // 17 sums + two 12-column register buffers: needs > 128 registers
     using Consts = FourDConsts;
 
+    static MF_HD double lnp_const(const Consts& c) { return c.m.lnc2; }
+
     template <bool PRED>
-    static MF_D void event(const double* x, const Consts& c, double* acc, int& esum, unsigned& bad, bool valid,
-                           const double2* __restrict__ tab)
+    static MF_D void event(const double* x, const Consts& c, double* acc, LogProd& lp, unsigned& bad, bool valid)
     {
         const MassConsts& q = c.m;
         const double m = x[0], cl = x[1], ck = x[2];
@@ -266,8 +262,6 @@ struct FourDModel {
         const double fR = q.f * R;
         const double D = fma(fR, A, omfL);     // P N2 e^{-tau m}
         const double r = mf_rcp(D);
-        int e = 0;
-        const double lnP = fma(q.tau, m, q.lnc2) + mf_log_frac(D, tab, e);
         const double ws = fR * A * r;          // f (G/N1) A / P
         const double wb = omfL * r;            // (1-f)(E/N2) L / P
         const double gf = fma(R * A, r, -(ll * lk) * kInv8Pi * r);
@@ -280,20 +274,18 @@ struct FourDModel {
         const bool good = D > 0.0;
         if (!PRED || valid) {
             bad += good ? 0u : 1u;
-            esum += e;
-            {
-                acc[0] += lnP;
-                acc[1] += gf;
-                acc[2] = fma(ws, hmu, acc[2]);
-                acc[3] = fma(ws, hsig, acc[3]);
-                acc[4] = fma(wb, htau, acc[4]);
+            lp.mul(D);
+            acc[0] = fma(q.tau, m, acc[0]);
+            acc[1] += gf;
+            acc[2] = fma(ws, hmu, acc[2]);
+            acc[3] = fma(ws, hsig, acc[3]);
+            acc[4] = fma(wb, htau, acc[4]);
 #pragma unroll
-                for (int k = 0; k < 8; ++k) acc[5 + k] = fma(qa, h[1 + k], acc[5 + k]);
-                acc[13] = fma(qbl, cl, acc[13]);
-                acc[14] = fma(qbl, p2l, acc[14]);
-                acc[15] = fma(qbk, ck, acc[15]);
-                acc[16] = fma(qbk, p2k, acc[16]);
-            }
+            for (int k = 0; k < 8; ++k) acc[5 + k] = fma(qa, h[1 + k], acc[5 + k]);
+            acc[13] = fma(qbl, cl, acc[13]);
+            acc[14] = fma(qbl, p2l, acc[14]);
+            acc[15] = fma(qbk, ck, acc[15]);
+            acc[16] = fma(qbk, p2k, acc[16]);
         }
     }
 };
