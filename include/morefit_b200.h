@@ -125,6 +125,13 @@ mf_status mf_nll_grad(mf_model* model, const double* lambda, double* nll, double
  * parameter-domain check is still made on the host before the launch. */
 mf_status mf_nll_grad_async(mf_model* model, const double* lambda, double* out_dev);
 
+/* n_points evaluations of the same dataset at n_points parameter points (BASELINE.json configs[1]:
+ * "repeated NLL+gradient calls at 1,000 random parameter points"), enqueued back to back without a host
+ * synchronisation: exactly mf_nll_grad_async called n_points times, the loop being inside the library.
+ *   lambdas  host, [n_points][K].   out_dev  DEVICE, [n_points][K+2], row p = [-ln L, grad, n_bad] at point p.
+ * Stops at the first point outside the parameter domain (MF_ERR_PARAM_DOMAIN; earlier points are enqueued). */
+mf_status mf_nll_grad_points(mf_model* model, int64_t n_points, const double* lambdas, double* out_dev);
+
 /* T pseudo-experiments at their own parameter points in ONE launch (BASELINE.json
  * configs[4]): a CTA tile is (toy, event chunk); each CTA derives its toy's
  * parameter-only constants in a short prologue.

@@ -33,7 +33,7 @@ EXPORTS = [
     "mf_ctx_create", "mf_ctx_destroy", "mf_last_error", "mf_ctx_kernel_launches",
     "mf_dataset_upload", "mf_dataset_destroy", "mf_dataset_n_events", "mf_dataset_n_toys",
     "mf_model_create", "mf_model_destroy", "mf_model_nparams", "mf_model_n_events", "mf_model_n_toys",
-    "mf_nll_grad", "mf_nll_grad_async", "mf_nll_grad_batch",
+    "mf_nll_grad", "mf_nll_grad_async", "mf_nll_grad_points", "mf_nll_grad_batch",
     "mf_fit_opts_default", "mf_fit", "mf_fit_batch",
     "mf_probe_fp64_rate", "mf_probe_read_bandwidth", "mf_probe_math",
 ]
@@ -126,6 +126,8 @@ def load_library() -> ctypes.CDLL:
     lib.mf_nll_grad.argtypes = [vp, dp, dp, dp]
     lib.mf_nll_grad_async.restype = ctypes.c_int
     lib.mf_nll_grad_async.argtypes = [vp, dp, vp]
+    lib.mf_nll_grad_points.restype = ctypes.c_int
+    lib.mf_nll_grad_points.argtypes = [vp, i64, dp, vp]
     lib.mf_nll_grad_batch.restype = ctypes.c_int
     lib.mf_nll_grad_batch.argtypes = [vp, i64, dp, u8p, dp, dp]
     lib.mf_fit_opts_default.restype = None
@@ -303,6 +305,14 @@ class Model:
         """Enqueues one evaluation; K+2 doubles are written to the device pointer out_dev_ptr."""
         lam = np.ascontiguousarray(lam, dtype=np.float64)
         self._ctx._check(self._lib.mf_nll_grad_async(self._h, _dp(lam), ctypes.c_void_p(out_dev_ptr)))
+
+    def nll_grad_points(self, lambdas, out_dev_ptr: int):
+        """Enqueues len(lambdas) evaluations back to back; row p of the device array [n][K+2] at
+        out_dev_ptr receives [-ln L, gradient, n_bad] at lambdas[p]."""
+        lam = np.ascontiguousarray(lambdas, dtype=np.float64)
+        if lam.ndim != 2 or lam.shape[1] != self.K:
+            raise ValueError(f"lambdas must be [n][{self.K}]")
+        self._ctx._check(self._lib.mf_nll_grad_points(self._h, lam.shape[0], _dp(lam), ctypes.c_void_p(out_dev_ptr)))
 
     def nll_grad_batch(self, lambdas, active=None):
         """lambdas [T][K] -> (nll [T], grad [T][K]); inactive toys are NaN in the returned arrays."""

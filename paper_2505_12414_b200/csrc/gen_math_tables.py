@@ -77,6 +77,17 @@ def main():
     print(f"exp: degree-11 relative error with double coefficients = {mp.nstr(err, 4)}")
     out.append("// exp(r) = 1 + r + r^2 (c[0] + c[1] r + ... + c[9] r^9) on |r| <= ln2/2; max rel. error %s" % mp.nstr(err, 3))
     out.append("#define MF_EXP_POLY { " + ", ".join(hexlit(c) for c in q_exp_d) + " }")
+    # ---- exp with a 32-entry table: exp(x) = 2^e 2^(j/32) exp(r), |r| <= ln2/64
+    R32 = mp.log(2) / 64 * (1 + mp.mpf(2) ** -12)
+    q32 = cheb_fit(lambda r: (mp.exp(r) - 1 - r) / r ** 2 if abs(r) > mp.mpf(10) ** -30 else mp.mpf(1) / 2 + r / 6, -R32, R32, 4)
+    q32_d = [to_double(c) for c in q32]
+    err = max_err(lambda r: 1 + r + r * r * horner([mp.mpf(c) for c in q32_d], r), mp.exp, -R32, R32)
+    print(f"exp32: degree-6 relative error with double coefficients = {mp.nstr(err, 4)}")
+    assert err < mp.mpf(2) ** -58
+    out.append("// exp(r) - 1 = r + r^2 (c[0] + ... + c[4] r^4) on |r| <= ln2/64; max rel. error of exp %s" % mp.nstr(err, 3))
+    out.append("#define MF_EXP32_POLY { " + ", ".join(hexlit(c) for c in q32_d) + " }")
+    out.append("// 2^(j/32), j = 0..31, rounded to nearest")
+    out.append("#define MF_EXP2_32_TABLE { " + ", ".join(hexlit(to_double(mp.mpf(2) ** (mp.mpf(j) / 32))) for j in range(32)) + " }")
     # ---- log1p on the table residual
     lo_hi = []
     tab = []

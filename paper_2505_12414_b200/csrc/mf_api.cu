@@ -195,6 +195,7 @@ extern "C" void mf_model_destroy(mf_model* m)
     cudaFree(m->partials);
     cudaFree(m->bad_partials);
     cudaFree(m->ticket);
+    cudaFree(m->gen);
     cudaFree(m->b_partials);
     cudaFree(m->b_bad);
     cudaFree(m->d_lam);
@@ -275,10 +276,12 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
     m->grid = (int)std::max<int64_t>(1, std::min<int64_t>((n_items + kWarps - 1) / kWarps, ctas_per_sm * (int64_t)ctx->sm_count));
     // batch geometry: one CTA per toy up to 32768 events per toy, else split
     m->chunks = (int)std::max<int64_t>(1, std::min<int64_t>((m->n_pad + 32767) / 32768, 64));
-    MF_CUDA_M(cudaMalloc(&m->partials, sizeof(double) * m->nacc * m->grid));
-    MF_CUDA_M(cudaMalloc(&m->bad_partials, sizeof(unsigned) * m->grid));
-    MF_CUDA_M(cudaMalloc(&m->ticket, sizeof(unsigned) * (1 + m->n_toys)));
-    MF_CUDA_M(cudaMemsetAsync(m->ticket, 0, sizeof(unsigned) * (1 + m->n_toys), ctx->stream));
+    MF_CUDA_M(cudaMalloc(&m->partials, sizeof(double) * kRing * m->nacc * m->grid));
+    MF_CUDA_M(cudaMalloc(&m->bad_partials, sizeof(unsigned) * kRing * m->grid));
+    MF_CUDA_M(cudaMalloc(&m->ticket, sizeof(unsigned) * (kRing + m->n_toys)));
+    MF_CUDA_M(cudaMemsetAsync(m->ticket, 0, sizeof(unsigned) * (kRing + m->n_toys), ctx->stream));
+    MF_CUDA_M(cudaMalloc(&m->gen, sizeof(unsigned long long) * kRing));
+    MF_CUDA_M(cudaMemsetAsync(m->gen, 0, sizeof(unsigned long long) * kRing, ctx->stream));
     MF_CUDA_M(cudaHostAlloc(&m->h_out, sizeof(double) * (MF_MAX_PARAMS + 2), cudaHostAllocMapped));
     MF_CUDA_M(cudaHostGetDevicePointer(&m->d_out_mapped, m->h_out, 0));
     if (m->n_toys > 1) {
@@ -357,11 +360,15 @@ static mf_status launch_single(mf_model* m, const double* lam, double* out_dev)
     a.n = m->n_events;
     a.n_items = m->n_pad / kItem;
     a.lnp_offset = (double)m->n_events * M::lnp_const(a.c);
-    a.partials = m->partials;
-    a.bad_partials = m->bad_partials;
-    a.ticket = m->ticket;
+    const int slot = (int)(m->seq % kRing);
+    a.partials = m->partials + (int64_t)slot * m->nacc * m->grid;
+    a.bad_partials = m->bad_partials + (int64_t)slot * m->grid;
+    a.ticket = m->ticket + slot;
+    a.gen = m->gen + slot;
+    a.need = m->seq / kRing;
     a.out = out_dev;
     MF_CUDA(ctx, launch_pdl(nll_grad_kernel<M>, m->grid, ctx->stream, a));
+    ++m->seq;
     ++ctx->launches;
     return MF_OK;
 }
@@ -380,6 +387,18 @@ extern "C" mf_status mf_nll_grad_async(mf_model* m, const double* lambda, double
     if (!m || !lambda || !out_dev) return mf_fail(m ? m->ctx : nullptr, MF_ERR_ARG, "mf_nll_grad_async: NULL argument");
     if (m->n_toys != 1) return mf_fail(m->ctx, MF_ERR_ARG, "mf_nll_grad_async: dataset has n_toys != 1; use mf_nll_grad_batch");
     return dispatch_single(m, lambda, out_dev);
+}
+
+extern "C" mf_status mf_nll_grad_points(mf_model* m, int64_t n_points, const double* lambdas, double* out_dev)
+{
+    if (!m || !lambdas || !out_dev || n_points < 0)
+        return mf_fail(m ? m->ctx : nullptr, MF_ERR_ARG, "mf_nll_grad_points: bad argument");
+    if (m->n_toys != 1) return mf_fail(m->ctx, MF_ERR_ARG, "mf_nll_grad_points: dataset has n_toys != 1");
+    for (int64_t p = 0; p < n_points; ++p) {
+        const mf_status st = dispatch_single(m, lambdas + p * m->K, out_dev + p * (m->K + 2));
+        if (st != MF_OK) return st;
+    }
+    return MF_OK;
 }
 
 extern "C" mf_status mf_nll_grad(mf_model* m, const double* lambda, double* nll, double* grad)
@@ -414,7 +433,7 @@ static mf_status launch_batch(mf_model* m, int n_active)
     a.ids = m->d_ids;
     a.partials = m->b_partials;
     a.bad_partials = m->b_bad;
-    a.ticket = m->ticket + 1;
+    a.ticket = m->ticket + kRing;
     a.out = m->d_bout;
     MF_CUDA(ctx, launch_pdl(nll_grad_batch_kernel<M>, n_active * m->chunks, ctx->stream, a));
     ++ctx->launches;

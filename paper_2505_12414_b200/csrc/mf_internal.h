@@ -45,9 +45,11 @@ struct mf_model {
     const double* col[MF_MAX_COLS] = {};  // column base pointers, stride between toys = n_pad
     // single-dataset evaluation
     int grid = 1;                     // CTAs of the fused kernel
-    double* partials = nullptr;       // device [nacc][grid]
-    unsigned* bad_partials = nullptr; // device [grid]
-    unsigned* ticket = nullptr;       // device, 1 (single) + n_toys (batch)
+    double* partials = nullptr;       // device [kRing][nacc][grid]
+    unsigned* bad_partials = nullptr; // device [kRing][grid]
+    unsigned* ticket = nullptr;       // device, kRing (single) + n_toys (batch)
+    unsigned long long* gen = nullptr;  // device [kRing]: evaluations completed per scratch slot
+    unsigned long long seq = 0;       // evaluations enqueued so far (evaluation e uses slot e % kRing)
     double* h_out = nullptr;          // pinned + mapped host, MF_MAX_PARAMS+2
     double* d_out_mapped = nullptr;   // device alias of h_out
     // batched evaluation

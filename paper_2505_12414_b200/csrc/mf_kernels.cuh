@@ -28,6 +28,7 @@ namespace mf {
 constexpr int kBlock = 256;
 constexpr int kWarps = kBlock / 32;
 constexpr int kItem = 64;  // events per warp item
+constexpr int kRing = 4;    // scratch slots of the single-dataset kernel: evaluation e uses slot e % kRing
 constexpr int kFinalBatch = 10;  // partials per lane loaded together in the final pass (covers 2 CTAs/SM x 148 SMs)
 
 template <class M>
@@ -37,9 +38,13 @@ struct EvalArgs {
     int64_t n_items;             // n_pad / 64
     typename M::Consts c;        // parameter-only constants (S2), computed on the host
     double lnp_offset;           // N * (per-event constant of ln P), added once in the final pass
+    // scratch slot of this evaluation (ring of kRing slots, so that successive evaluations do not
+    // serialise on one scratch area; see "pipelining" below)
     double* partials;            // [NACC][gridDim.x]
     unsigned* bad_partials;      // [gridDim.x]
     unsigned* ticket;            // zero on entry, reset to zero by the last CTA
+    unsigned long long* gen;     // evaluations completed on this slot
+    unsigned long long need;     // value of *gen at which the slot is free for this evaluation
     double* out;                 // [K+2]: -lnL, grad, n_bad
 };
 
@@ -77,13 +82,43 @@ __device__ __forceinline__ bool make_consts<FourDModel>(const double* lam, doubl
     return fourd_consts(lam, ma, mb, c);
 }
 
-// ---- programmatic dependent launch (back-to-back evaluations on one stream) --------------------
-// The event loop only reads the immutable dataset columns, so it may run while the previous
-// evaluation is still reducing: every kernel lets its successor start at once and waits for
-// its predecessor to complete only before it touches the shared scratch (partials, ticket) and
-// the output.  Without the launch attribute both instructions are no-ops.
+// ---- pipelining of back-to-back evaluations on one stream (programmatic dependent launch) -------
+// Every kernel lets its successor start at once (launch_dependents at entry) and waits for its
+// predecessor to COMPLETE (griddepcontrol.wait) only where stream order matters:
+//   * single-dataset kernel: the event loop reads only the immutable columns, partial sums go to
+//     this evaluation's own scratch slot (ring of kRing), so only the CTA that does the final
+//     combine waits, immediately before it writes the output.  Kernels therefore complete in
+//     stream order, outputs land in stream order, and everything else overlaps.  A slot is reused
+//     by evaluation e + kRing; its CTAs check the slot's completion counter first (it is always
+//     already there unless > kRing evaluations are in flight; the kernel they would wait for has
+//     all its CTAs running, because a dependent grid is only launched after every CTA of its
+//     predecessor has started, so the check cannot deadlock);
+//   * batched kernel: waits before its first global write.
+// Without the launch attribute both instructions are no-ops.
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+// Ticket with release/acquire semantics at GPU scope.  Called by ONE thread after a __syncthreads():
+// the barrier orders the CTA's partial-sum stores before the release, and the CTA that draws the last
+// ticket acquires every other CTA's stores (then a second __syncthreads() hands them to its threads,
+// which read the partials with L1-bypassing loads).  One fence per CTA instead of one
+// sequentially-consistent fence per storing thread.
+__device__ __forceinline__ unsigned long long gen_load(const unsigned long long* g)
+{
+    unsigned long long v;
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(g) : "memory");
+    return v;
+}
+__device__ __forceinline__ void gen_store(unsigned long long* g, unsigned long long v)
+{
+    asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(g), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned ticket_take(unsigned* ticket)
+{
+    unsigned old;
+    asm volatile("atom.add.acq_rel.gpu.global.u32 %0, [%1], 1;" : "=r"(old) : "l"(ticket) : "memory");
+    return old;
+}
 
 // ---- S3: the event loop of one warp ---------------------------------------------------------
 
@@ -237,19 +272,21 @@ __device__ __forceinline__ void final_combine(const double* p, int64_t stride_k,
             lo = (lo + lo2) + e;
             s = t;
         }
+        pdl_wait();  // outputs land in stream order
         if (lane == 0) {
             double v = -((s + lo) + (k == 0 ? offset0 : 0.0));
             if (nb) v = (k == 0) ? __longlong_as_double(0x7ff0000000000000LL) : __longlong_as_double(0x7ff8000000000000LL);
             out[k] = v;
         }
     }
+    pdl_wait();
     if (threadIdx.x == 0) out[NACC] = (double)nb;
 }
 
 // ---- the fused single-dataset kernel (mf_nll_grad) ----------------------------------------------
 
 template <class M>
-__global__ void __launch_bounds__(kBlock, M::CTAS_PER_SM) nll_grad_kernel(const __grid_constant__ EvalArgs<M> a)
+__global__ void __launch_bounds__(kBlock, M::RESIDENT_CTAS) nll_grad_kernel(const __grid_constant__ EvalArgs<M> a)
 {
     constexpr int NACC = M::NACC;
     __shared__ double sm[kWarps][NACC];
@@ -265,29 +302,30 @@ __global__ void __launch_bounds__(kBlock, M::CTAS_PER_SM) nll_grad_kernel(const 
     const int64_t G = gridDim.x;
     accumulate<M>(a.col, a.n, a.n_items, blockIdx.x + G * (threadIdx.x >> 5), G * kWarps, a.c, acc, bad);
 
-    const double s = block_reduce<NACC>(acc, bad, sm, sm_bad, &s_bad_block);
-    pdl_wait();
-    if (threadIdx.x < NACC) {
+    if (threadIdx.x == 0)
+        while (gen_load(a.gen) < a.need) __nanosleep(64);  // slot still in use by evaluation e - kRing (rare)
+    const double s = block_reduce<NACC>(acc, bad, sm, sm_bad, &s_bad_block);  // contains a __syncthreads()
+    if (threadIdx.x < NACC)
         a.partials[threadIdx.x * G + blockIdx.x] = s;
-        __threadfence();
-    } else if (threadIdx.x == NACC) {
+    else if (threadIdx.x == NACC)
         a.bad_partials[blockIdx.x] = s_bad_block;
-        __threadfence();
-    }
     __syncthreads();
-    if (threadIdx.x == 0) s_last = (atomicAdd(a.ticket, 1u) == gridDim.x - 1);
+    if (threadIdx.x == 0) s_last = (ticket_take(a.ticket) == gridDim.x - 1);
     __syncthreads();
     if (s_last) {
-        __threadfence();
         final_combine<NACC>(a.partials, G, (int)G, a.bad_partials, a.lnp_offset, a.out);
-        if (threadIdx.x == 0) *a.ticket = 0u;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            *a.ticket = 0u;
+            gen_store(a.gen, a.need + 1);  // releases the slot (and the ticket reset) to evaluation e + kRing
+        }
     }
 }
 
 // ---- the batched-toy kernel (mf_nll_grad_batch): CTA <-> (toy, event chunk) ----------------------
 
 template <class M>
-__global__ void __launch_bounds__(kBlock, M::CTAS_PER_SM) nll_grad_batch_kernel(const __grid_constant__ BatchArgs<M> a)
+__global__ void __launch_bounds__(kBlock, M::RESIDENT_CTAS) nll_grad_batch_kernel(const __grid_constant__ BatchArgs<M> a)
 {
     constexpr int NACC = M::NACC;
     constexpr int K = M::K;
@@ -342,18 +380,14 @@ __global__ void __launch_bounds__(kBlock, M::CTAS_PER_SM) nll_grad_batch_kernel(
     }
     double* part = a.partials + (int64_t)slot * NACC * C;
     unsigned* badp = a.bad_partials + (int64_t)slot * C;
-    if (threadIdx.x < NACC) {
+    if (threadIdx.x < NACC)
         part[threadIdx.x * C + chunk] = s;
-        __threadfence();
-    } else if (threadIdx.x == NACC) {
+    else if (threadIdx.x == NACC)
         badp[chunk] = s_bad_block;
-        __threadfence();
-    }
     __syncthreads();
-    if (threadIdx.x == 0) s_last = (atomicAdd(a.ticket + slot, 1u) == (unsigned)a.chunks - 1);
+    if (threadIdx.x == 0) s_last = (ticket_take(a.ticket + slot) == (unsigned)a.chunks - 1);
     __syncthreads();
     if (s_last) {
-        __threadfence();
         final_combine<NACC>(part, C, (int)C, badp, offset0, out);
         if (threadIdx.x == 0) a.ticket[slot] = 0u;
     }

@@ -165,8 +165,9 @@ struct MassModel {
     static constexpr int K = 4;
     static constexpr int NCOL = 1;  // m
     static constexpr int NACC = 5;
-    static constexpr int ITEMS_PER_ITER = 2;  // 4 independent events in flight per thread (ALU bound)
-    static constexpr int CTAS_PER_SM = 2;
+    static constexpr int ITEMS_PER_ITER = 1;  // 2 independent events in flight per thread
+    static constexpr int CTAS_PER_SM = 2;     // grid of one evaluation: CTAs per SM
+    static constexpr int RESIDENT_CTAS = 3;   // register budget: CTAs of the next evaluation co-reside under PDL
     using Consts = MassConsts;
 
     // ln P = [tau m] + [-ln N2] + ln D
@@ -209,6 +210,7 @@ struct AngularModel {
     static constexpr int NACC = 9;
     static constexpr int ITEMS_PER_ITER = 1;  // memory bound: depth comes from the prefetched next item
     static constexpr int CTAS_PER_SM = 2;
+    static constexpr int RESIDENT_CTAS = 2;
     using Consts = AngularConsts;
 
     static MF_HD double lnp_const(const Consts&) { return 0.0; }
@@ -235,6 +237,7 @@ struct FourDModel {
     static constexpr int NCOL = 12;  // m, cos theta_l, cos theta_K, h_0..h_8
     static constexpr int NACC = 17;
     static constexpr int ITEMS_PER_ITER = 1;
+    static constexpr int RESIDENT_CTAS = 1;
     static constexpr int CTAS_PER_SM = 1;  // 17 sums + two 12-column register buffers: needs > 128 registers
     using Consts = FourDConsts;
 
