@@ -197,7 +197,8 @@ mf_status mf_probe_fp64_rate(mf_ctx* ctx, double* dfma_per_second);
  * times with 16-byte loads: L2 bandwidth when bytes fits the L2 and repeats > 1, HBM otherwise. */
 mf_status mf_probe_read_bandwidth(mf_ctx* ctx, size_t bytes, int repeats, double* bytes_per_second);
 /* Evaluates the kernels' own device math element by element, for the accuracy tests:
- * op 0 = exp (finite x < 709; x <= -708 gives 0), 1 = log (positive normal x), 2 = reciprocal.
+ * op 0 = exp (finite x < 709; x <= -708 gives 0), 1 = log (positive normal x), 2 = reciprocal,
+ * 3 = the table-by-shuffle exp the event loops use (same domain as op 0).
  * x_host, y_host: host, n doubles. */
 mf_status mf_probe_math(mf_ctx* ctx, int op, int64_t n, const double* x_host, double* y_host);
 

@@ -200,7 +200,7 @@ class Context:
         """The kernels' device exp / log / rcp evaluated element-wise (accuracy tests)."""
         x = np.ascontiguousarray(x, dtype=np.float64)
         y = np.empty_like(x)
-        self._check(self._lib.mf_probe_math(self._h, {"exp": 0, "log": 1, "rcp": 2}[op], x.size, _dp(x), _dp(y)))
+        self._check(self._lib.mf_probe_math(self._h, {"exp": 0, "log": 1, "rcp": 2, "exp32": 3}[op], x.size, _dp(x), _dp(y)))
         return y
 
     def dataset_upload(self, columns, lo=None, hi=None, n_toys: int = 1) -> "Dataset":

@@ -192,6 +192,7 @@ extern "C" void mf_model_destroy(mf_model* m)
 {
     if (!m) return;
     cudaFree(m->cache);
+    cudaFree(m->d_sum_m);
     cudaFree(m->partials);
     cudaFree(m->bad_partials);
     cudaFree(m->ticket);
@@ -268,6 +269,14 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
             m->col[c++] = raw + 2 * per_dim;  // cos theta_K
         }
         for (int k = 0; k < 9; ++k) m->col[c++] = m->cache + k * per_dim;
+    }
+    if (kind != MF_ANGULAR_KSTMUMU) {
+        // S1: sum_i m_i per toy (ln P_i contains tau m_i: its sum is an event-only constant times tau)
+        MF_CUDA_M(cudaMalloc(&m->d_sum_m, sizeof(double) * m->n_toys));
+        column_sum_kernel<<<(unsigned)m->n_toys, 256, 0, ctx->stream>>>(raw, m->n_events, m->n_pad, m->d_sum_m);
+        ++ctx->launches;
+        MF_CUDA_M(cudaGetLastError());
+        MF_CUDA_M(cudaMemcpyAsync(&m->h_sum_m, m->d_sum_m, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     }
     // launch geometry: persistent-style grid, CTAS_PER_SM CTAs per SM (one wave), never more CTAs than 8-warp groups of items
     const int64_t n_items = m->n_pad / kItem;
@@ -359,7 +368,7 @@ static mf_status launch_single(mf_model* m, const double* lam, double* out_dev)
     for (int i = 0; i < M::NCOL; ++i) a.col[i] = m->col[i];
     a.n = m->n_events;
     a.n_items = m->n_pad / kItem;
-    a.lnp_offset = (double)m->n_events * M::lnp_const(a.c);
+    a.sum_m = m->h_sum_m;
     const int slot = (int)(m->seq % kRing);
     a.partials = m->partials + (int64_t)slot * m->nacc * m->grid;
     a.bad_partials = m->bad_partials + (int64_t)slot * m->grid;
@@ -429,6 +438,7 @@ static mf_status launch_batch(mf_model* m, int n_active)
     a.chunks = m->chunks;
     a.ma = m->ma;
     a.mb = m->mb;
+    a.sum_m = m->d_sum_m;
     a.lam = m->d_lam;
     a.ids = m->d_ids;
     a.partials = m->b_partials;

@@ -37,7 +37,7 @@ struct EvalArgs {
     int64_t n;                   // valid events
     int64_t n_items;             // n_pad / 64
     typename M::Consts c;        // parameter-only constants (S2), computed on the host
-    double lnp_offset;           // N * (per-event constant of ln P), added once in the final pass
+    double sum_m;                // event-only constant sum_i m_i (0 for models without a mass dimension)
     // scratch slot of this evaluation (ring of kRing slots, so that successive evaluations do not
     // serialise on one scratch area; see "pipelining" below)
     double* partials;            // [NACC][gridDim.x]
@@ -56,6 +56,7 @@ struct BatchArgs {
     int64_t n_items;             // n_pad / 64 per toy
     int chunks;                  // CTAs per toy
     double ma, mb;               // mass range for the constants prologue
+    const double* sum_m;         // [n_toys] event-only constants sum_i m_i per toy, or NULL
     const double* lam;           // [n_active][K]
     const int* ids;              // [n_active] toy index of each active slot
     double* partials;            // [n_active][NACC][chunks]   (chunks > 1)
@@ -146,15 +147,15 @@ __device__ __forceinline__ void load_group(const double* const* col, int64_t n_i
 template <class M, int U>
 __device__ __forceinline__ void compute_group(int64_t n, int64_t n_items, int64_t j, int64_t step, int lane,
                                               const double (&buf)[U][2][M::NCOL], const typename M::Consts& c,
-                                              double* acc, LogProd& lp, unsigned& bad)
+                                              double* acc, LogProd& lp, unsigned& bad, double t_lane)
 {
     const int64_t jl = j + (U - 1) * step;  // last item of the group
     if (jl < n_items && kItem * (jl + 1) <= n) {
         // fast path: 2U independent events, no predicates, free for the compiler to interleave
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            M::template event<false>(buf[u][0], c, acc, lp, bad, true);
-            M::template event<false>(buf[u][1], c, acc, lp, bad, true);
+            M::template event<false>(buf[u][0], c, acc, lp, bad, true, t_lane);
+            M::template event<false>(buf[u][1], c, acc, lp, bad, true, t_lane);
         }
     } else {
 #pragma unroll
@@ -162,37 +163,73 @@ __device__ __forceinline__ void compute_group(int64_t n, int64_t n_items, int64_
             const int64_t ju = j + u * step;
             if (ju < n_items) {
                 const int64_t e = kItem * ju + 2 * lane;
-                M::template event<true>(buf[u][0], c, acc, lp, bad, e < n);
-                M::template event<true>(buf[u][1], c, acc, lp, bad, e + 1 < n);
+                M::template event<true>(buf[u][0], c, acc, lp, bad, e < n, t_lane);
+                M::template event<true>(buf[u][1], c, acc, lp, bad, e + 1 < n, t_lane);
             }
         }
     }
     lp.renorm();  // at most 2U mantissas in [1,2) since the last one
 }
 
-// Items j0, j0 + step, j0 + 2 step, ... < n_items, U per iteration, software-pipelined: the
-// loads of the next group are in flight while the current group is evaluated (two register
-// buffers, ping-pong).
+// Items j0, j0 + step, j0 + 2 step, ... < n_items.  Two schedules:
+//  * PREFETCH == 0 (many columns, HBM bound): U items per iteration, software-pipelined with two register
+//    buffers (the loads of the next group are in flight while the current group is evaluated);
+//  * PREFETCH == D > 0 (one column, ALU bound): a rolling window of D items per thread — the slot of the
+//    item being evaluated is refilled at once with the item D steps ahead, so D 16-byte loads per
+//    thread stay in flight (memory latency x bandwidth needs ~44 KB in flight per SM).
 template <class M>
 __device__ __forceinline__ void accumulate(const double* const* col, int64_t n, int64_t n_items, int64_t j0,
                                            int64_t step, const typename M::Consts& c, double* acc, unsigned& bad)
 {
-    constexpr int U = M::ITEMS_PER_ITER;
     const int lane = threadIdx.x & 31;
+    const double t_lane = mf_exp32_lane_entry();
     LogProd lp;
-    double A[U][2][M::NCOL], B[U][2][M::NCOL];
-    int64_t j = j0;
-    load_group<M, U>(col, n_items, j, step, lane, A);
-    while (j < n_items) {
-        load_group<M, U>(col, n_items, j + U * step, step, lane, B);
-        compute_group<M, U>(n, n_items, j, step, lane, A, c, acc, lp, bad);
-        j += U * step;
-        if (j >= n_items) break;
-        load_group<M, U>(col, n_items, j + U * step, step, lane, A);
-        compute_group<M, U>(n, n_items, j, step, lane, B, c, acc, lp, bad);
-        j += U * step;
+    if constexpr (M::PREFETCH > 0) {
+        constexpr int D = M::PREFETCH;
+        double buf[D][2][M::NCOL];
+#pragma unroll
+        for (int u = 0; u < D; ++u)
+            if (j0 + u * step < n_items) load_item<M>(col, j0 + u * step, lane, buf[u][0], buf[u][1]);
+        for (int64_t j = j0; j < n_items; j += D * step) {
+#pragma unroll
+            for (int u = 0; u < D; ++u) {
+                const int64_t ju = j + u * step;
+                if (ju < n_items) {
+                    double xa[M::NCOL], xb[M::NCOL];
+#pragma unroll
+                    for (int q = 0; q < M::NCOL; ++q) {
+                        xa[q] = buf[u][0][q];
+                        xb[q] = buf[u][1][q];
+                    }
+                    if (ju + D * step < n_items) load_item<M>(col, ju + D * step, lane, buf[u][0], buf[u][1]);
+                    if (kItem * (ju + 1) <= n) {
+                        M::template event<false>(xa, c, acc, lp, bad, true, t_lane);
+                        M::template event<false>(xb, c, acc, lp, bad, true, t_lane);
+                    } else {
+                        const int64_t e = kItem * ju + 2 * lane;
+                        M::template event<true>(xa, c, acc, lp, bad, e < n, t_lane);
+                        M::template event<true>(xb, c, acc, lp, bad, e + 1 < n, t_lane);
+                    }
+                    lp.renorm();
+                }
+            }
+        }
+    } else {
+        constexpr int U = M::ITEMS_PER_ITER;
+        double A[U][2][M::NCOL], B[U][2][M::NCOL];
+        int64_t j = j0;
+        load_group<M, U>(col, n_items, j, step, lane, A);
+        while (j < n_items) {
+            load_group<M, U>(col, n_items, j + U * step, step, lane, B);
+            compute_group<M, U>(n, n_items, j, step, lane, A, c, acc, lp, bad, t_lane);
+            j += U * step;
+            if (j >= n_items) break;
+            load_group<M, U>(col, n_items, j + U * step, step, lane, A);
+            compute_group<M, U>(n, n_items, j, step, lane, B, c, acc, lp, bad, t_lane);
+            j += U * step;
+        }
     }
-    acc[0] += lp.log();  // the one logarithm of this thread
+    acc[0] = lp.log();  // the one logarithm of this thread
 }
 
 // ---- S4: thread -> warp -> block ---------------------------------------------------------------
@@ -231,21 +268,27 @@ __device__ __forceinline__ double block_reduce(double* acc, unsigned bad, double
     return s;
 }
 
-// ---- S5: fixed-order compensated combine of `count` partials per quantity ---------------------
+// ---- S5: fixed-order compensated combine of `count` partials per quantity, then M::finish ---------
 
-// Warp w combines quantities w, w + 8, ...; partial i of quantity k is at p[k * stride_k + i].
-// Writes out[0] = -(sum_0 + offset0) (= -ln L), out[1+k] = -sum_{1+k}, out[NACC] = n_bad; +inf / NaN if n_bad.
-template <int NACC>
+// Called by every thread of the CTA that drew the last ticket.  Warp w combines quantities w, w + 8,
+// ...; partial i of quantity k is at p[k * stride_k + i].  Thread 0 then turns the NACC sums into
+// out[0] = -ln L, out[1..K] = gradient, out[K+1] = n_bad (+inf / NaN if n_bad), after waiting for the
+// previous kernel on the stream (outputs land in stream order).
+template <class M>
 __device__ __forceinline__ void final_combine(const double* p, int64_t stride_k, int count, const unsigned* badp,
-                                              double offset0, double* out)
+                                              const typename M::Consts& c, double n, double sum_m, double* s_sum,
+                                              double* out)
 {
+    constexpr int NACC = M::NACC, K = M::K;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     unsigned nb = 0;
-    for (int i = lane; i < count; i += 32) nb += __ldcg(badp + i);
-    nb = __reduce_add_sync(0xffffffffu, nb);
+    if (w == 0) {
+        for (int i = lane; i < count; i += 32) nb += __ldcg(badp + i);
+        nb = __reduce_add_sync(0xffffffffu, nb);
+    }
     for (int k = w; k < NACC; k += kWarps) {
         const double* pk = p + k * stride_k;
-        double s = 0.0, c = 0.0;  // Kahan: true sum ~ s - c
+        double s = 0.0, cc = 0.0;  // Kahan: true sum ~ s - cc
         for (int i0 = lane; i0 < count; i0 += 32 * kFinalBatch) {
             double v[kFinalBatch];  // issue the loads of a batch together, then add them in index order
 #pragma unroll
@@ -255,13 +298,13 @@ __device__ __forceinline__ void final_combine(const double* p, int64_t stride_k,
             }
 #pragma unroll
             for (int u = 0; u < kFinalBatch; ++u) {
-                const double y = v[u] - c;
+                const double y = v[u] - cc;
                 const double t = s + y;
-                c = (t - s) - y;
+                cc = (t - s) - y;
                 s = t;
             }
         }
-        double lo = -c;
+        double lo = -cc;
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) {
             const double s2 = __shfl_down_sync(0xffffffffu, s, off);
@@ -272,15 +315,18 @@ __device__ __forceinline__ void final_combine(const double* p, int64_t stride_k,
             lo = (lo + lo2) + e;
             s = t;
         }
-        pdl_wait();  // outputs land in stream order
-        if (lane == 0) {
-            double v = -((s + lo) + (k == 0 ? offset0 : 0.0));
-            if (nb) v = (k == 0) ? __longlong_as_double(0x7ff0000000000000LL) : __longlong_as_double(0x7ff8000000000000LL);
-            out[k] = v;
-        }
+        if (lane == 0) s_sum[k] = s + lo;
     }
-    pdl_wait();
-    if (threadIdx.x == 0) out[NACC] = (double)nb;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double o[K + 1];
+        M::finish(c, s_sum, n, sum_m, o);
+        pdl_wait();
+#pragma unroll
+        for (int k = 0; k <= K; ++k)
+            out[k] = !nb ? o[k] : (k == 0) ? __longlong_as_double(0x7ff0000000000000LL) : __longlong_as_double(0x7ff8000000000000LL);
+        out[K + 1] = (double)nb;
+    }
 }
 
 // ---- the fused single-dataset kernel (mf_nll_grad) ----------------------------------------------
@@ -290,6 +336,7 @@ __global__ void __launch_bounds__(kBlock, M::RESIDENT_CTAS) nll_grad_kernel(cons
 {
     constexpr int NACC = M::NACC;
     __shared__ double sm[kWarps][NACC];
+    __shared__ double s_sum[NACC];
     __shared__ unsigned sm_bad[kWarps];
     __shared__ unsigned s_bad_block;
     __shared__ bool s_last;
@@ -313,9 +360,8 @@ __global__ void __launch_bounds__(kBlock, M::RESIDENT_CTAS) nll_grad_kernel(cons
     if (threadIdx.x == 0) s_last = (ticket_take(a.ticket) == gridDim.x - 1);
     __syncthreads();
     if (s_last) {
-        final_combine<NACC>(a.partials, G, (int)G, a.bad_partials, a.lnp_offset, a.out);
-        __syncthreads();
-        if (threadIdx.x == 0) {
+        final_combine<M>(a.partials, G, (int)G, a.bad_partials, a.c, (double)a.n, a.sum_m, s_sum, a.out);
+        if (threadIdx.x == 0) {  // every partial has been read: final_combine synchronises the CTA before its thread 0 returns
             *a.ticket = 0u;
             gen_store(a.gen, a.need + 1);  // releases the slot (and the ticket reset) to evaluation e + kRing
         }
@@ -330,6 +376,7 @@ __global__ void __launch_bounds__(kBlock, M::RESIDENT_CTAS) nll_grad_batch_kerne
     constexpr int NACC = M::NACC;
     constexpr int K = M::K;
     __shared__ double sm[kWarps][NACC];
+    __shared__ double s_sum[NACC];
     __shared__ unsigned sm_bad[kWarps];
     __shared__ unsigned s_bad_block;
     __shared__ bool s_last;
@@ -352,6 +399,7 @@ __global__ void __launch_bounds__(kBlock, M::RESIDENT_CTAS) nll_grad_batch_kerne
     }
     const typename M::Consts c = s_c;
     const int64_t toy = a.ids[slot];
+    const double sum_m = a.sum_m ? a.sum_m[toy] : 0.0;
     const double* col[M::NCOL];
 #pragma unroll
     for (int i = 0; i < M::NCOL; ++i) col[i] = a.col[i] + toy * a.toy_stride;
@@ -364,20 +412,22 @@ __global__ void __launch_bounds__(kBlock, M::RESIDENT_CTAS) nll_grad_batch_kerne
     accumulate<M>(col, a.n, a.n_items, chunk + C * (threadIdx.x >> 5), C * kWarps, c, acc, bad);
 
     const double s = block_reduce<NACC>(acc, bad, sm, sm_bad, &s_bad_block);
-    const double offset0 = (double)a.n * M::lnp_const(c);
-    pdl_wait();
     if (a.chunks == 1) {  // the CTA holds the toy's complete sums: no cross-CTA pass
+        if (threadIdx.x < NACC) s_sum[threadIdx.x] = s;
         __syncthreads();
-        const unsigned nb = s_bad_block;
-        if (threadIdx.x < NACC) {
-            double v = -(s + (threadIdx.x == 0 ? offset0 : 0.0));
-            if (nb) v = (threadIdx.x == 0) ? __longlong_as_double(0x7ff0000000000000LL) : __longlong_as_double(0x7ff8000000000000LL);
-            out[threadIdx.x] = v;
-        } else if (threadIdx.x == NACC) {
-            out[NACC] = (double)nb;
+        if (threadIdx.x == 0) {
+            const unsigned nb = s_bad_block;
+            double o[K + 1];
+            M::finish(c, s_sum, (double)a.n, sum_m, o);
+            pdl_wait();
+#pragma unroll
+            for (int k = 0; k <= K; ++k)
+                out[k] = !nb ? o[k] : (k == 0) ? __longlong_as_double(0x7ff0000000000000LL) : __longlong_as_double(0x7ff8000000000000LL);
+            out[K + 1] = (double)nb;
         }
         return;
     }
+    pdl_wait();
     double* part = a.partials + (int64_t)slot * NACC * C;
     unsigned* badp = a.bad_partials + (int64_t)slot * C;
     if (threadIdx.x < NACC)
@@ -388,9 +438,42 @@ __global__ void __launch_bounds__(kBlock, M::RESIDENT_CTAS) nll_grad_batch_kerne
     if (threadIdx.x == 0) s_last = (ticket_take(a.ticket + slot) == (unsigned)a.chunks - 1);
     __syncthreads();
     if (s_last) {
-        final_combine<NACC>(part, C, (int)C, badp, offset0, out);
+        final_combine<M>(part, C, (int)C, badp, c, (double)a.n, sum_m, s_sum, out);
         if (threadIdx.x == 0) a.ticket[slot] = 0u;
     }
+}
+
+// ---- S1: event-only constants: sum_i m_i per toy ------------------------------
+
+// One CTA per toy; deterministic: thread t Kahan-sums events t, t + 256, ..., the 256 (sum, compensation)
+// pairs are merged by a fixed two-sum tree in shared memory.
+__global__ void __launch_bounds__(256) column_sum_kernel(const double* __restrict__ col, int64_t n, int64_t n_pad,
+                                                         double* __restrict__ out)
+{
+    __shared__ double sh[256], sl[256];
+    const double* x = col + (int64_t)blockIdx.x * n_pad;
+    double s = 0.0, cc = 0.0;
+    for (int64_t i = threadIdx.x; i < n; i += 256) {
+        const double y = x[i] - cc;
+        const double t = s + y;
+        cc = (t - s) - y;
+        s = t;
+    }
+    sh[threadIdx.x] = s;
+    sl[threadIdx.x] = -cc;
+    __syncthreads();
+    for (int off = 128; off > 0; off >>= 1) {
+        if (threadIdx.x < off) {
+            const double a = sh[threadIdx.x], b = sh[threadIdx.x + off];
+            const double t = a + b;
+            const double bb = t - a;
+            const double e = (a - (t - bb)) + (b - bb);
+            sl[threadIdx.x] = (sl[threadIdx.x] + sl[threadIdx.x + off]) + e;
+            sh[threadIdx.x] = t;
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) out[blockIdx.x] = sh[0] + sl[0];
 }
 
 // ---- S1: event-only precompute (Listing 4) ------------------

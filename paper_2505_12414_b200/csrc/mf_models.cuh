@@ -153,98 +153,121 @@ MF_HD inline bool fourd_consts(const double* lam, double ma, double mb, FourDCon
 
 #ifdef __CUDACC__
 // ------------------------------------------------------------------------------------------
-// Per-event bodies (S3).  Each adds d ln P_i / d lambda_k to acc[1+k].  ln P_i is split: the factor of
-// P_i that needs a logarithm is multiplied into lp (LogProd, mf_math.cuh: sum of logs = log of the
-// product, taken once per thread), the part that is linear in the event goes to acc[0], and the
-// per-event constant is added once per call as N * Consts::lnp_const().  `bad` counts events with P <= 0 or NaN (SURVEY.md §8(c) reading 15); when it ends up
-// non-zero the sums are discarded by the final pass, so they are accumulated unconditionally.  PRED = true is the
-// ragged-tail variant: lanes with valid == false contribute exactly 0 (reading 10).
+// Per-event bodies (S3) and the per-call finish.
+//
+// The kernels keep NACC running sums per thread.  Sum 0 is always ln of the product of the factor
+// of P_i that needs a logarithm (LogProd, mf_math.cuh: sum of logs = log of the product, one
+// logarithm per thread).  Sums 1..NACC-1 are model specific.  After the fixed-order reduction ONE
+// thread per evaluation calls M::finish(), which turns the NACC sums into -ln L and the K gradient
+// components using the parameter-only constants and the event-only constant sum_m = sum_i m_i
+// (precomputed once per dataset: ln P_i contains tau m_i, so its sum needs no
+// per-event work).  `bad` counts events whose P is not a positive normal number (SURVEY.md §8(c)
+// reading 15); when it ends up non-zero the sums are discarded, so they are accumulated
+// unconditionally.  PRED = true is the ragged-tail variant: lanes with valid == false contribute
+// exactly 0 (reading 10).  t_lane is this lane's entry of the exp table (mf_exp32).
 // ------------------------------------------------------------------------------------------
+
+// a b - c d with the rounding errors of both products recovered (the two terms nearly cancel at a
+// likelihood maximum)
+MF_D double diff_of_products(double a, double b, double c, double d)
+{
+    const double p = a * b, q = c * d;
+    const double ep = fma(a, b, -p), eq = fma(c, d, -q);
+    return (p - q) + (ep - eq);
+}
 
 struct MassModel {
     static constexpr int K = 4;
     static constexpr int NCOL = 1;  // m
-    static constexpr int NACC = 5;
+    static constexpr int NACC = 6;  // ln prod D, and with u = (G/N1)/P', r = (E/N2)/P' (P' = P N2 e^{-tau m}, d = m - mu):
+                                    // sum u, sum r, sum u d, sum u d^2, sum r d
     static constexpr int ITEMS_PER_ITER = 1;  // 2 independent events in flight per thread
+    static constexpr int PREFETCH = 4;        // rolling window: 4 x 16 B in flight per thread
     static constexpr int CTAS_PER_SM = 2;     // grid of one evaluation: CTAs per SM
     static constexpr int RESIDENT_CTAS = 3;   // register budget: CTAs of the next evaluation co-reside under PDL
     using Consts = MassConsts;
 
-    // ln P = [tau m] + [-ln N2] + ln D
-    static MF_HD double lnp_const(const Consts& c) { return c.lnc2; }
-
     template <bool PRED>
-    static MF_D void event(const double* x, const Consts& c, double* acc, LogProd& lp, unsigned& bad, bool valid)
+    static MF_D void event(const double* x, const Consts& c, double* acc, LogProd& lp, unsigned& bad, bool valid,
+                           double t_lane)
     {
         const double m = x[0];
         const double d = m - c.mu;
         const double t = d * d;
         // ln R = -b0 d^2 - tau m + ln(c1/c2)
         const double arg = fma(c.nb0, t, fma(-c.tau, m, c.lnk));  // < 700 by the check in mass_consts
-        const double R = mf_exp(arg);
-        const double D = fma(c.f, R, c.omf);  // P N2 e^{-tau m} = (1-f) + f R
+        const double R = mf_exp32(arg, t_lane);  // (G/N1)/(E/N2)
+        const double D = fma(c.f, R, c.omf);     // P N2 e^{-tau m} = (1-f) + f R
         const double r = mf_rcp(D);
-        const double u = R * r;               // (G/N1)/P
-        const double ws = c.f * u;            // signal weight  f (G/N1) / P
-        const double wb = c.omf * r;          // background weight (1-f)(E/N2)/P
-        const double gf = u - r;              // [(G/N1) - (E/N2)]/P
-        const double hmu = fma(d, c.is2, -c.kmu);
-        const double hsig = fma(t, c.is3, -c.ksig);
-        const double htau = (m - c.ma) - c.ktau;
-        const bool good = D > 0.0;
+        const double u = R * r;
         if (!PRED || valid) {
-            bad += good ? 0u : 1u;
-            lp.mul(D);
-            acc[0] = fma(c.tau, m, acc[0]);
-            acc[1] += gf;
-            acc[2] = fma(ws, hmu, acc[2]);
-            acc[3] = fma(ws, hsig, acc[3]);
-            acc[4] = fma(wb, htau, acc[4]);
+            lp.mul(D, bad);
+            acc[1] += u;
+            acc[2] += r;
+            acc[3] = fma(u, d, acc[3]);
+            acc[4] = fma(u, t, acc[4]);
+            acc[5] = fma(r, d, acc[5]);
         }
+    }
+
+    // ln P = tau m - ln N2 + ln D
+    // d ln P/df = u - r;  d/dmu = f u (d/sigma^2 - kmu);  d/dsigma = f u (d^2/sigma^3 - ksig);
+    // d/dtau = (1-f) r (m - m_a - ktau) = (1-f) r (d + mu - m_a - ktau)
+    static MF_D void finish(const Consts& c, const double* s, double n, double sum_m, double* out)
+    {
+        out[0] = -(s[0] + fma(c.tau, sum_m, n * c.lnc2));
+        out[1] = -(s[1] - s[2]);
+        out[2] = -c.f * diff_of_products(c.is2, s[3], c.kmu, s[1]);
+        out[3] = -c.f * diff_of_products(c.is3, s[4], c.ksig, s[1]);
+        out[4] = -c.omf * fma((c.mu - c.ma) - c.ktau, s[2], s[5]);
     }
 };
 
 struct AngularModel {
     static constexpr int K = 8;
     static constexpr int NCOL = 9;  // h_0..h_8 (cached, already times 9/(32 pi))
-    static constexpr int NACC = 9;
+    static constexpr int NACC = 9;  // ln prod P, sum h_k / P
     static constexpr int ITEMS_PER_ITER = 1;  // memory bound: depth comes from the prefetched next item
+    static constexpr int PREFETCH = 0;
     static constexpr int CTAS_PER_SM = 2;
     static constexpr int RESIDENT_CTAS = 2;
     using Consts = AngularConsts;
 
-    static MF_HD double lnp_const(const Consts&) { return 0.0; }
-
     template <bool PRED>
-    static MF_D void event(const double* x, const Consts& c, double* acc, LogProd& lp, unsigned& bad, bool valid)
+    static MF_D void event(const double* x, const Consts& c, double* acc, LogProd& lp, unsigned& bad, bool valid,
+                           double)
     {
         double P = fma(c.a[0], x[1], x[0]);
 #pragma unroll
         for (int k = 1; k < 8; ++k) P = fma(c.a[k], x[1 + k], P);
         const double r = mf_rcp(P);
-        const bool good = P > 0.0;
         if (!PRED || valid) {
-            bad += good ? 0u : 1u;
-            lp.mul(P);  // acc[0] stays 0: ln P is all in the product
+            lp.mul(P, bad);
 #pragma unroll
             for (int k = 0; k < 8; ++k) acc[1 + k] = fma(x[1 + k], r, acc[1 + k]);
         }
+    }
+
+    static MF_D void finish(const Consts&, const double* s, double, double, double* out)
+    {
+#pragma unroll
+        for (int k = 0; k < NACC; ++k) out[k] = -s[k];
     }
 };
 
 struct FourDModel {
     static constexpr int K = 16;
     static constexpr int NCOL = 12;  // m, cos theta_l, cos theta_K, h_0..h_8
-    static constexpr int NACC = 17;
+    static constexpr int NACC = 17;  // ln prod D, then sum d ln P / d lambda_k
     static constexpr int ITEMS_PER_ITER = 1;
+    static constexpr int PREFETCH = 0;
     static constexpr int RESIDENT_CTAS = 1;
     static constexpr int CTAS_PER_SM = 1;  // 17 sums + two 12-column register buffers: needs > 128 registers
     using Consts = FourDConsts;
 
-    static MF_HD double lnp_const(const Consts& c) { return c.m.lnc2; }
-
     template <bool PRED>
-    static MF_D void event(const double* x, const Consts& c, double* acc, LogProd& lp, unsigned& bad, bool valid)
+    static MF_D void event(const double* x, const Consts& c, double* acc, LogProd& lp, unsigned& bad, bool valid,
+                           double t_lane)
     {
         const MassConsts& q = c.m;
         const double m = x[0], cl = x[1], ck = x[2];
@@ -260,25 +283,22 @@ struct FourDModel {
         const double d = m - q.mu;
         const double t = d * d;
         const double arg = fma(q.nb0, t, fma(-q.tau, m, q.lnk));  // < 700 by the check in mass_consts
-        const double R = mf_exp(arg);          // (G/N1)/(E/N2)
+        const double R = mf_exp32(arg, t_lane);   // (G/N1)/(E/N2)
         const double omfL = c.kappa * (ll * lk);  // (1-f) L
         const double fR = q.f * R;
-        const double D = fma(fR, A, omfL);     // P N2 e^{-tau m}
+        const double D = fma(fR, A, omfL);        // P N2 e^{-tau m}
         const double r = mf_rcp(D);
-        const double ws = fR * A * r;          // f (G/N1) A / P
-        const double wb = omfL * r;            // (1-f)(E/N2) L / P
+        const double ws = fR * A * r;             // f (G/N1) A / P
+        const double wb = omfL * r;               // (1-f)(E/N2) L / P
         const double gf = fma(R * A, r, -(ll * lk) * kInv8Pi * r);
         const double hmu = fma(d, q.is2, -q.kmu);
         const double hsig = fma(t, q.is3, -q.ksig);
         const double htau = (m - q.ma) - q.ktau;
-        const double qa = fR * r;              // f (G/N1) / P
-        const double qb = c.kappa * r;         // (1-f)(E/N2)/(8 pi P)
+        const double qa = fR * r;                 // f (G/N1) / P
+        const double qb = c.kappa * r;            // (1-f)(E/N2)/(8 pi P)
         const double qbl = qb * lk, qbk = qb * ll;
-        const bool good = D > 0.0;
         if (!PRED || valid) {
-            bad += good ? 0u : 1u;
-            lp.mul(D);
-            acc[0] = fma(q.tau, m, acc[0]);
+            lp.mul(D, bad);
             acc[1] += gf;
             acc[2] = fma(ws, hmu, acc[2]);
             acc[3] = fma(ws, hsig, acc[3]);
@@ -290,6 +310,14 @@ struct FourDModel {
             acc[15] = fma(qbk, ck, acc[15]);
             acc[16] = fma(qbk, p2k, acc[16]);
         }
+    }
+
+    // ln P = tau m - ln N2 + ln D
+    static MF_D void finish(const Consts& c, const double* s, double n, double sum_m, double* out)
+    {
+        out[0] = -(s[0] + fma(c.m.tau, sum_m, n * c.m.lnc2));
+#pragma unroll
+        for (int k = 1; k < NACC; ++k) out[k] = -s[k];
     }
 };
 #endif  // __CUDACC__

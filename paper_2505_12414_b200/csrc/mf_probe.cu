@@ -39,15 +39,19 @@ __global__ void __launch_bounds__(256) read_kernel(const double2* __restrict__ p
 }
 
 
-// Element-wise evaluation of the device math of mf_math.cuh (op 0: mf_exp, 1: mf_log, 2: mf_rcp).
+// Element-wise evaluation of the device math of mf_math.cuh (op 0: mf_exp, 1: mf_log, 2: mf_rcp, 3: mf_exp32).
 __global__ void __launch_bounds__(256) math_kernel(int op, int64_t n, const double* __restrict__ x, double* __restrict__ y)
 {
     __shared__ double2 s_tab[mf::kLogTableSize];
     mf::load_log_table(s_tab);
     __syncthreads();
-    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-        const double v = x[i];
-        y[i] = op == 0 ? mf::mf_exp(v) : op == 1 ? mf::mf_log(v, s_tab) : mf::mf_rcp(v);
+    const double t_lane = mf::mf_exp32_lane_entry();
+    // whole warps iterate together (mf_exp32 shuffles across the warp); lanes past n compute on 0
+    const int64_t n_round = (n + 31) / 32 * 32;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n_round; i += (int64_t)gridDim.x * blockDim.x) {
+        const double v = i < n ? x[i] : 0.0;
+        const double r = op == 3 ? mf::mf_exp32(v, t_lane) : op == 0 ? mf::mf_exp(v) : op == 1 ? mf::mf_log(v, s_tab) : mf::mf_rcp(v);
+        if (i < n) y[i] = r;
     }
 }
 
@@ -126,7 +130,7 @@ extern "C" mf_status mf_probe_read_bandwidth(mf_ctx* ctx, size_t bytes, int repe
 
 extern "C" mf_status mf_probe_math(mf_ctx* ctx, int op, int64_t n, const double* x_host, double* y_host)
 {
-    if (!ctx || !x_host || !y_host || n < 1 || op < 0 || op > 2) return mf_fail(ctx, MF_ERR_ARG, "mf_probe_math: bad argument");
+    if (!ctx || !x_host || !y_host || n < 1 || op < 0 || op > 3) return mf_fail(ctx, MF_ERR_ARG, "mf_probe_math: bad argument");
     MF_CUDA(ctx, cudaSetDevice(ctx->device));
     double *dx = nullptr, *dy = nullptr;
     MF_CUDA(ctx, cudaMalloc(&dx, sizeof(double) * n));
