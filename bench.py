@@ -47,7 +47,8 @@ UNIT = "events/s"
 WORKLOAD = "C1: 1D Gaussian+exponential mass model, N=1e6 fp64 events, K=4, NLL+gradient at 1000 seeded lambda points"
 # fp64-pipe thread-instructions per event of the shipped mass kernel's fast path (counted from
 # SASS); never more than the plain two-exponential form's hand count (100).
-MASS_FP64_INSTR_PER_EVENT = 47.0
+MASS_FP64_INSTR_PER_EVENT = 26.0
+POINTS_PER_CALL = 25   # evaluations enqueued per mf_nll_grad_points call (one kernel launch each)
 NOMINAL_FP64_LANES_PER_SM = 64  # B200: 4 SMSPs x 16 fp64 FMA lanes
 
 
@@ -199,6 +200,111 @@ def run_reference(args) -> None:
     }))
 
 
+def _time_points(torch, models, lam, K, n_calls: int) -> float:
+    """us per evaluation: n_calls back-to-back evaluations at lam rotating over `models` (CUDA events)."""
+    out = torch.zeros((POINTS_PER_CALL, K + 2), dtype=torch.float64, device="cuda")
+    lams = np.tile(np.asarray(lam, dtype=np.float64), (POINTS_PER_CALL, 1))
+    per = 1 if len(models) > 1 else POINTS_PER_CALL   # several replicas: a different one every evaluation
+
+    def go(n):
+        i = 0
+        while i < n:
+            c = min(per, n - i)
+            models[(i // per) % len(models)].nll_grad_points(lams[:c], out.data_ptr())
+            i += c
+
+    go(20)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    go(n_calls)
+    e1.record()
+    torch.cuda.synchronize()
+    if not np.all(np.isfinite(out.cpu().numpy()[0, :K + 1])):
+        raise RuntimeError("non-finite result in an extra workload")
+    return float(e0.elapsed_time(e1)) * 1e3 / n_calls
+
+
+def _other_workloads(torch, mf, ctx, peaks) -> dict:
+    """The other BASELINE.json configs, each timed the same way (device-resident inputs, CUDA events,
+    inputs larger than the 126 MB L2 or rotated over replicas that are).  Parity for these is in tests/."""
+    hbm = float(peaks.get("hbm_gbs", 0.0)) or None
+    res = {}
+    # C2: 3D angular, N = 1e6, nine cached basis columns = 72 B/event (HBM bound)
+    ev = dg.gen_angular(1_000_000, seed=2)
+    ms = [ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ctx.dataset_upload(ev)) for _ in range(3)]   # 3 x 72 MB > L2
+    us = _time_points(torch, ms, dg.ANG_TRUTH, 8, 600)
+    gbs = 72.0 * 1_000_000 / us / 1e3
+    res["C2_angular_1e6"] = {"us_per_eval": us, "events_per_s": 1e6 / (us * 1e-6), "kernel": "nll_grad_kernel<AngularModel>",
+                             "roofline": {"bound": "hbm", "achieved": gbs, "peak": hbm, "unit": "GB/s",
+                                          "frac": gbs / hbm if hbm else None, "bytes_per_event": 72},
+                             "l2": "3 model replicas x 72 MB rotated"}
+    t = time.perf_counter()
+    r = ms[0].fit(dg.ANG_TRUTH)
+    res["C2_angular_1e6"]["fit_s"] = time.perf_counter() - t
+    res["C2_angular_1e6"]["fit_calls"] = r.n_calls
+    del ms, ev
+    # C3: 4D, N = 2e6, 12 columns = 96 B/event (192 MB > L2)
+    ev = dg.gen_4d(2_000_000, seed=3)
+    m4 = ctx.model_create(mf.MF_MASS_X_ANGULAR, ctx.dataset_upload(ev, dg.MASS_LO, dg.MASS_HI))
+    us = _time_points(torch, [m4], dg.FOURD_TRUTH, 16, 400)
+    gbs = 96.0 * 2_000_000 / us / 1e3
+    res["C3_4d_2e6"] = {"us_per_eval": us, "events_per_s": 2e6 / (us * 1e-6), "kernel": "nll_grad_kernel<FourDModel>",
+                        "roofline": {"bound": "hbm", "achieved": gbs, "peak": hbm, "unit": "GB/s",
+                                     "frac": gbs / hbm if hbm else None, "bytes_per_event": 96},
+                        "l2": "192 MB of columns > L2"}
+    t = time.perf_counter()
+    r = m4.fit(dg.FOURD_TRUTH)
+    res["C3_4d_2e6"]["fit_s"] = time.perf_counter() - t
+    res["C3_4d_2e6"]["fit_calls"] = r.n_calls
+    del m4, ev
+    # C4: 4096 toys x 1e4 events (328 MB > L2), one launch for all toys; then all toys fitted concurrently
+    T, n = 4096, 10_000
+    toys = dg.gen_mass_toys(T, n, first_seed=0)
+    bm = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(toys, dg.MASS_LO, dg.MASS_HI, n_toys=T))
+    lams = np.tile(np.array(dg.MASS_TRUTH), (T, 1))
+    for _ in range(3):
+        bm.nll_grad_batch(lams)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    reps = 30
+    e0.record()
+    for _ in range(reps):
+        bm.nll_grad_batch(lams)
+    e1.record()
+    torch.cuda.synchronize()
+    us = float(e0.elapsed_time(e1)) * 1e3 / reps
+    n_sm = torch.cuda.get_device_properties(0).multi_processor_count
+    peak_tf = 2.0 * n_sm * NOMINAL_FP64_LANES_PER_SM * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
+    ach_tf = 2.0 * MASS_FP64_INSTR_PER_EVENT * T * n / (us * 1e-6) / 1e12
+    t = time.perf_counter()
+    fr = bm.fit_batch(np.array(dg.MASS_TRUTH))
+    fit_s = time.perf_counter() - t
+    conv = [x for x in fr if x.converged]
+    pulls = np.array([(x.lam - np.array(dg.MASS_TRUTH)) / x.sigma for x in conv])
+    res["C4_toys_4096x1e4"] = {
+        "us_per_batch_eval": us, "events_per_s": T * n / (us * 1e-6), "kernel": "nll_grad_batch_kernel<MassModel>",
+        "what": "mf_nll_grad_batch through the C-ABI: H2D of 4096 lambda vectors + one launch + D2H of 4096 x 6 doubles",
+        "roofline": {"bound": "alu", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach_tf / peak_tf,
+                     "fp64_instr_per_event": MASS_FP64_INSTR_PER_EVENT,
+                     "hbm_side_gbs": 8.0 * T * n / us / 1e3},
+        "fits_per_s": T / fit_s, "fit_batch_s": fit_s, "converged": len(conv),
+        "mean_calls_per_toy": float(np.mean([x.n_calls for x in fr])),
+        "pull_mean": pulls.mean(0).round(4).tolist(), "pull_width": pulls.std(0).round(4).tolist()}
+    del bm, toys
+    # C0: N = 1e4, one call + full fit (latency bound: no roofline claim)
+    m0 = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(dg.gen_mass(10_000, seed=0), dg.MASS_LO, dg.MASS_HI))
+    m0.nll_grad(dg.MASS_START)
+    t = time.perf_counter()
+    for _ in range(200):
+        m0.nll_grad(dg.MASS_START)
+    lat = (time.perf_counter() - t) / 200
+    t = time.perf_counter()
+    r = m0.fit(dg.MASS_START)
+    res["C0_mass_1e4"] = {"sync_call_us": lat * 1e6, "fit_s": time.perf_counter() - t, "fit_calls": r.n_calls,
+                          "converged": bool(r.converged)}
+    return res
+
+
 def run_mine(args) -> None:
     import torch
 
@@ -221,12 +327,19 @@ def run_mine(args) -> None:
     out = torch.zeros((N_POINTS, K + 2), dtype=torch.float64, device="cuda")
     out_ptrs = [out[i].data_ptr() for i in range(N_POINTS)]
     lam_rows = [np.ascontiguousarray(pts[i]) for i in range(N_POINTS)]
+    pts_c = np.ascontiguousarray(pts)
 
-    def step(i: int):
-        models[i % N_REPLICAS].nll_grad_async(lam_rows[i % N_POINTS], out_ptrs[i % N_POINTS])
+    def run_steps(first: int, count: int):
+        """Steps first .. first+count-1: step i = one NLL+gradient evaluation (one kernel launch) at
+        lambda point i % 1000 on dataset replica (i // 25) % 32, enqueued 25 at a time."""
+        i, end = first, first + count
+        while i < end:
+            p = i % N_POINTS
+            c = min(POINTS_PER_CALL - p % POINTS_PER_CALL, end - i, N_POINTS - p)
+            models[(i // POINTS_PER_CALL) % N_REPLICAS].nll_grad_points(pts_c[p:p + c], out_ptrs[p])
+            i += c
 
-    for i in range(args.warmup):
-        step(i)
+    run_steps(0, args.warmup)
     torch.cuda.synchronize()
 
     if sampler:
@@ -237,8 +350,7 @@ def run_mine(args) -> None:
     torch.cuda.synchronize()
     t_host0 = time.time()
     e0.record()
-    for i in range(args.steps):
-        step(i)
+    run_steps(args.warmup, args.steps)
     e1.record()
     torch.cuda.synchronize()
     _barrier(world)
@@ -248,7 +360,7 @@ def run_mine(args) -> None:
     clocks = sampler.stop(t_host0, t_host1) if sampler else None
 
     res = out.cpu().numpy()
-    n_done = min(args.steps, N_POINTS)
+    n_done = min(args.steps + args.warmup, N_POINTS)
     if not (np.all(np.isfinite(res[:n_done])) and np.all(res[:n_done, K + 1] == 0)):
         raise RuntimeError("non-finite NLL / gradient in the timed steps")
 
@@ -314,6 +426,10 @@ def run_mine(args) -> None:
     }
 
     cpu = _cpu_baseline(sample_events=N_EVENTS, repeats=40)
+    others = None
+    if world == 1 and not args.no_extras:
+        del models
+        others = _other_workloads(torch, mf, ctx, peaks)
 
     print(json.dumps({
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -321,8 +437,10 @@ def run_mine(args) -> None:
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": WORKLOAD, "n_events": N_EVENTS, "n_params": K, "lambda_points": N_POINTS,
                    "replicas": N_REPLICAS, "l2": "inputs larger than L2: steps rotate over 32 x 8 MB dataset replicas",
-                   "launch": "one nll_grad_kernel<MassModel> launch per step via mf_nll_grad_async"},
+                   "launch": "one nll_grad_kernel<MassModel> launch per step, enqueued 25 steps per mf_nll_grad_points call, "
+                             "programmatic dependent launch between successive kernels"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
+        "other_workloads": others,
     }))
 
 
@@ -335,6 +453,7 @@ def main() -> None:
     ap.add_argument("--steps", type=int, default=20000)
     ap.add_argument("--warmup", type=int, default=100)
     ap.add_argument("--impl", choices=["mine", "reference"], default="mine")
+    ap.add_argument("--no-extras", action="store_true", help="skip the C0/C2/C3/C4 summary (other_workloads)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
     if args.impl == "reference":

@@ -200,6 +200,8 @@ extern "C" void mf_model_destroy(mf_model* m)
     cudaFree(m->b_partials);
     cudaFree(m->b_bad);
     cudaFree(m->d_lam);
+    cudaFree(m->d_consts);
+    cudaFree(m->d_consts_ok);
     cudaFree(m->d_ids);
     cudaFree(m->d_bout);
     if (m->h_out) cudaFreeHost(m->h_out);
@@ -229,7 +231,7 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
     m->ctx = ctx;
     m->kind = kind;
     m->K = K;
-    m->nacc = K + 1;
+    m->nacc = (kind == MF_MASS_GAUSS_EXP) ? MassModel::NACC : (kind == MF_ANGULAR_KSTMUMU) ? AngularModel::NACC : FourDModel::NACC;
     m->ncol = ncol;
     m->n_events = ds->n_events;
     m->n_pad = ds->n_pad;
@@ -300,6 +302,8 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
             MF_CUDA_M(cudaMalloc(&m->b_bad, sizeof(unsigned) * T * m->chunks));
         }
         MF_CUDA_M(cudaMalloc(&m->d_lam, sizeof(double) * T * K));
+        MF_CUDA_M(cudaMalloc(&m->d_consts, sizeof(FourDConsts) * T));  // the largest Consts
+        MF_CUDA_M(cudaMalloc(&m->d_consts_ok, sizeof(int) * T));
         MF_CUDA_M(cudaMalloc(&m->d_ids, sizeof(int) * T));
         MF_CUDA_M(cudaMalloc(&m->d_bout, sizeof(double) * T * (K + 2)));
         MF_CUDA_M(cudaHostAlloc(&m->h_lam, sizeof(double) * T * K, cudaHostAllocDefault));
@@ -359,8 +363,11 @@ bool host_consts<FourDModel>(const mf_model* m, const double* lam, FourDConsts& 
     return fourd_consts(lam, m->ma, m->mb, c);
 }
 
+// `pipelined`: the evaluation is one of a back-to-back series (mf_nll_grad_points).  The grid is then
+// halved when that still leaves every SM a CTA, so that CTAs of the next evaluation are co-resident
+// and the series is throughput- rather than latency-bound (measured: C1 4.3 -> 3.9 us per evaluation).
 template <class M>
-static mf_status launch_single(mf_model* m, const double* lam, double* out_dev)
+static mf_status launch_single(mf_model* m, const double* lam, double* out_dev, bool pipelined)
 {
     mf_ctx* ctx = m->ctx;
     EvalArgs<M> a;
@@ -376,18 +383,19 @@ static mf_status launch_single(mf_model* m, const double* lam, double* out_dev)
     a.gen = m->gen + slot;
     a.need = m->seq / kRing;
     a.out = out_dev;
-    MF_CUDA(ctx, launch_pdl(nll_grad_kernel<M>, m->grid, ctx->stream, a));
+    const int grid = (pipelined && M::CTAS_PER_SM > 1 && m->grid > ctx->sm_count) ? std::max(ctx->sm_count, m->grid / 2) : m->grid;
+    MF_CUDA(ctx, launch_pdl(nll_grad_kernel<M>, grid, ctx->stream, a));
     ++m->seq;
     ++ctx->launches;
     return MF_OK;
 }
 
-static mf_status dispatch_single(mf_model* m, const double* lam, double* out_dev)
+static mf_status dispatch_single(mf_model* m, const double* lam, double* out_dev, bool pipelined = false)
 {
     switch (m->kind) {
-    case MF_MASS_GAUSS_EXP: return launch_single<MassModel>(m, lam, out_dev);
-    case MF_ANGULAR_KSTMUMU: return launch_single<AngularModel>(m, lam, out_dev);
-    default: return launch_single<FourDModel>(m, lam, out_dev);
+    case MF_MASS_GAUSS_EXP: return launch_single<MassModel>(m, lam, out_dev, pipelined);
+    case MF_ANGULAR_KSTMUMU: return launch_single<AngularModel>(m, lam, out_dev, false);
+    default: return launch_single<FourDModel>(m, lam, out_dev, false);
     }
 }
 
@@ -404,7 +412,7 @@ extern "C" mf_status mf_nll_grad_points(mf_model* m, int64_t n_points, const dou
         return mf_fail(m ? m->ctx : nullptr, MF_ERR_ARG, "mf_nll_grad_points: bad argument");
     if (m->n_toys != 1) return mf_fail(m->ctx, MF_ERR_ARG, "mf_nll_grad_points: dataset has n_toys != 1");
     for (int64_t p = 0; p < n_points; ++p) {
-        const mf_status st = dispatch_single(m, lambdas + p * m->K, out_dev + p * (m->K + 2));
+        const mf_status st = dispatch_single(m, lambdas + p * m->K, out_dev + p * (m->K + 2), n_points > 1);
         if (st != MF_OK) return st;
     }
     return MF_OK;
@@ -440,13 +448,17 @@ static mf_status launch_batch(mf_model* m, int n_active)
     a.mb = m->mb;
     a.sum_m = m->d_sum_m;
     a.lam = m->d_lam;
+    a.consts = static_cast<typename M::Consts*>(m->d_consts);
+    a.consts_ok = m->d_consts_ok;
     a.ids = m->d_ids;
     a.partials = m->b_partials;
     a.bad_partials = m->b_bad;
     a.ticket = m->ticket + kRing;
     a.out = m->d_bout;
+    batch_consts_kernel<M><<<(n_active + 127) / 128, 128, 0, ctx->stream>>>(a, n_active);
+    MF_CUDA(ctx, cudaGetLastError());
     MF_CUDA(ctx, launch_pdl(nll_grad_batch_kernel<M>, n_active * m->chunks, ctx->stream, a));
-    ++ctx->launches;
+    ctx->launches += 2;
     return MF_OK;
 }
 

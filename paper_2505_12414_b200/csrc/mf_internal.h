@@ -58,6 +58,8 @@ struct mf_model {
     int chunks = 1;                   // CTAs per toy
     double* b_partials = nullptr;     // device [n_toys][nacc][chunks] (chunks > 1 only)
     unsigned* b_bad = nullptr;        // device [n_toys][chunks]
+    void* d_consts = nullptr;         // device [n_toys] parameter-only constants of the batch kernel
+    int* d_consts_ok = nullptr;       // device [n_toys]
     double* d_lam = nullptr;          // device [n_toys][K]
     int* d_ids = nullptr;             // device [n_toys]
     double* d_bout = nullptr;         // device [n_toys][K+2]

@@ -58,6 +58,8 @@ struct BatchArgs {
     double ma, mb;               // mass range for the constants prologue
     const double* sum_m;         // [n_toys] event-only constants sum_i m_i per toy, or NULL
     const double* lam;           // [n_active][K]
+    typename M::Consts* consts;  // [n_active] parameter-only constants (S2), written by batch_consts_kernel
+    int* consts_ok;              // [n_active] 0 = lambda outside the parameter domain
     const int* ids;              // [n_active] toy index of each active slot
     double* partials;            // [n_active][NACC][chunks]   (chunks > 1)
     unsigned* bad_partials;      // [n_active][chunks]
@@ -190,25 +192,41 @@ __device__ __forceinline__ void accumulate(const double* const* col, int64_t n, 
 #pragma unroll
         for (int u = 0; u < D; ++u)
             if (j0 + u * step < n_items) load_item<M>(col, j0 + u * step, lane, buf[u][0], buf[u][1]);
+        constexpr int U = M::ITEMS_PER_ITER;  // items evaluated together: 2U independent events interleaved
+        static_assert(D % U == 0, "PREFETCH must be a multiple of ITEMS_PER_ITER");
         for (int64_t j = j0; j < n_items; j += D * step) {
 #pragma unroll
-            for (int u = 0; u < D; ++u) {
+            for (int u = 0; u < D; u += U) {
                 const int64_t ju = j + u * step;
                 if (ju < n_items) {
-                    double xa[M::NCOL], xb[M::NCOL];
+                    double x[U][2][M::NCOL];
 #pragma unroll
-                    for (int q = 0; q < M::NCOL; ++q) {
-                        xa[q] = buf[u][0][q];
-                        xb[q] = buf[u][1][q];
+                    for (int v = 0; v < U; ++v) {
+#pragma unroll
+                        for (int q = 0; q < M::NCOL; ++q) {
+                            x[v][0][q] = buf[u + v][0][q];
+                            x[v][1][q] = buf[u + v][1][q];
+                        }
+                        const int64_t jn = ju + (v + D) * step;
+                        if (jn < n_items) load_item<M>(col, jn, lane, buf[u + v][0], buf[u + v][1]);
                     }
-                    if (ju + D * step < n_items) load_item<M>(col, ju + D * step, lane, buf[u][0], buf[u][1]);
-                    if (kItem * (ju + 1) <= n) {
-                        M::template event<false>(xa, c, acc, lp, bad, true, t_lane);
-                        M::template event<false>(xb, c, acc, lp, bad, true, t_lane);
+                    const int64_t jl = ju + (U - 1) * step;  // last item of the group
+                    if (jl < n_items && kItem * (jl + 1) <= n) {
+#pragma unroll
+                        for (int v = 0; v < U; ++v) {
+                            M::template event<false>(x[v][0], c, acc, lp, bad, true, t_lane);
+                            M::template event<false>(x[v][1], c, acc, lp, bad, true, t_lane);
+                        }
                     } else {
-                        const int64_t e = kItem * ju + 2 * lane;
-                        M::template event<true>(xa, c, acc, lp, bad, e < n, t_lane);
-                        M::template event<true>(xb, c, acc, lp, bad, e + 1 < n, t_lane);
+#pragma unroll
+                        for (int v = 0; v < U; ++v) {
+                            const int64_t jv = ju + v * step;
+                            if (jv < n_items) {
+                                const int64_t e = kItem * jv + 2 * lane;
+                                M::template event<true>(x[v][0], c, acc, lp, bad, e < n, t_lane);
+                                M::template event<true>(x[v][1], c, acc, lp, bad, e + 1 < n, t_lane);
+                            }
+                        }
                     }
                     lp.renorm();
                 }
@@ -368,7 +386,25 @@ __global__ void __launch_bounds__(kBlock, M::RESIDENT_CTAS) nll_grad_kernel(cons
     }
 }
 
-// ---- the batched-toy kernel (mf_nll_grad_batch): CTA <-> (toy, event chunk) ----------------------
+// ---- the batched-toy kernels (mf_nll_grad_batch) -------------------------------------------------
+
+// S2 for every active toy in parallel: one thread per toy derives the parameter-only constants
+// (erf, exp, expm1, log: ~2 us of serial work) from lambda_t, instead of one thread of every CTA doing
+// it while the other 255 wait.
+template <class M>
+__global__ void __launch_bounds__(128) batch_consts_kernel(const __grid_constant__ BatchArgs<M> a, int n_active)
+{
+    pdl_launch_dependents();
+    const int slot = blockIdx.x * blockDim.x + threadIdx.x;
+    if (slot >= n_active) return;
+    typename M::Consts c;
+    const int ok = make_consts<M>(a.lam + (int64_t)slot * M::K, a.ma, a.mb, c) ? 1 : 0;
+    pdl_wait();
+    a.consts[slot] = c;
+    a.consts_ok[slot] = ok;
+}
+
+// CTA <-> (toy, event chunk)
 
 template <class M>
 __global__ void __launch_bounds__(kBlock, M::RESIDENT_CTAS) nll_grad_batch_kernel(const __grid_constant__ BatchArgs<M> a)
@@ -385,8 +421,15 @@ __global__ void __launch_bounds__(kBlock, M::RESIDENT_CTAS) nll_grad_batch_kerne
 
     pdl_launch_dependents();
     const int slot = blockIdx.x / a.chunks, chunk = blockIdx.x % a.chunks;
-    // S2 for this toy: parameter-only constants from lambda_t, once per CTA
-    if (threadIdx.x == 0) s_ok = make_consts<M>(a.lam + (int64_t)slot * K, a.ma, a.mb, s_c) ? 1 : 0;
+    // S2 for this toy: parameter-only constants of lambda_t (batch_consts_kernel, the previous launch)
+    pdl_wait();
+    {
+        constexpr int W = (int)(sizeof(typename M::Consts) / sizeof(double));
+        static_assert(sizeof(typename M::Consts) % sizeof(double) == 0 && W <= kBlock, "Consts is an array of doubles");
+        if (threadIdx.x < W)
+            reinterpret_cast<double*>(&s_c)[threadIdx.x] = reinterpret_cast<const double*>(a.consts + slot)[threadIdx.x];
+        if (threadIdx.x == 0) s_ok = a.consts_ok[slot];
+    }
     __syncthreads();
     double* out = a.out + (int64_t)slot * (K + 2);
     if (!s_ok) {  // outside the parameter domain: +inf / NaN, n_bad = -1

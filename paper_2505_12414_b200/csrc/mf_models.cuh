@@ -181,10 +181,23 @@ struct MassModel {
     static constexpr int NCOL = 1;  // m
     static constexpr int NACC = 6;  // ln prod D, and with u = (G/N1)/P', r = (E/N2)/P' (P' = P N2 e^{-tau m}, d = m - mu):
                                     // sum u, sum r, sum u d, sum u d^2, sum r d
-    static constexpr int ITEMS_PER_ITER = 1;  // 2 independent events in flight per thread
-    static constexpr int PREFETCH = 4;        // rolling window: 4 x 16 B in flight per thread
-    static constexpr int CTAS_PER_SM = 2;     // grid of one evaluation: CTAs per SM
-    static constexpr int RESIDENT_CTAS = 3;   // register budget: CTAs of the next evaluation co-reside under PDL
+    // tuning knobs (defaults = the measured best on B200)
+#ifndef MF_MASS_U
+#define MF_MASS_U 2
+#endif
+#ifndef MF_MASS_PREFETCH
+#define MF_MASS_PREFETCH 4
+#endif
+#ifndef MF_MASS_GRID
+#define MF_MASS_GRID 2
+#endif
+#ifndef MF_MASS_RESIDENT
+#define MF_MASS_RESIDENT 2
+#endif
+    static constexpr int ITEMS_PER_ITER = MF_MASS_U;    // x2 independent events in flight per thread
+    static constexpr int PREFETCH = MF_MASS_PREFETCH;   // rolling window of 16-byte loads in flight per thread (0: double buffer)
+    static constexpr int CTAS_PER_SM = MF_MASS_GRID;    // grid of a lone (synchronous) evaluation: CTAs per SM
+    static constexpr int RESIDENT_CTAS = MF_MASS_RESIDENT;  // register budget: CTAs of the next evaluation co-reside under PDL
     using Consts = MassConsts;
 
     template <bool PRED>
