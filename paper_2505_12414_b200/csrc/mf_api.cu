@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -293,7 +294,8 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
     MF_CUDA_M(cudaMemsetAsync(m->ticket, 0, sizeof(unsigned) * (kRing + m->n_toys), ctx->stream));
     MF_CUDA_M(cudaMalloc(&m->gen, sizeof(unsigned long long) * kRing));
     MF_CUDA_M(cudaMemsetAsync(m->gen, 0, sizeof(unsigned long long) * kRing, ctx->stream));
-    MF_CUDA_M(cudaHostAlloc(&m->h_out, sizeof(double) * (MF_MAX_PARAMS + 2), cudaHostAllocMapped));
+    MF_CUDA_M(cudaHostAlloc(&m->h_out, sizeof(double) * (MF_MAX_PARAMS + 3), cudaHostAllocMapped));
+    std::memset(m->h_out, 0, sizeof(double) * (MF_MAX_PARAMS + 3));
     MF_CUDA_M(cudaHostGetDevicePointer(&m->d_out_mapped, m->h_out, 0));
     if (m->n_toys > 1) {
         const int64_t T = m->n_toys;
@@ -367,7 +369,7 @@ bool host_consts<FourDModel>(const mf_model* m, const double* lam, FourDConsts& 
 // halved when that still leaves every SM a CTA, so that CTAs of the next evaluation are co-resident
 // and the series is throughput- rather than latency-bound (measured: C1 4.3 -> 3.9 us per evaluation).
 template <class M>
-static mf_status launch_single(mf_model* m, const double* lam, double* out_dev, bool pipelined)
+static mf_status launch_single(mf_model* m, const double* lam, double* out_dev, bool pipelined, bool signal_host)
 {
     mf_ctx* ctx = m->ctx;
     EvalArgs<M> a;
@@ -383,6 +385,8 @@ static mf_status launch_single(mf_model* m, const double* lam, double* out_dev, 
     a.gen = m->gen + slot;
     a.need = m->seq / kRing;
     a.out = out_dev;
+    a.done_flag = signal_host ? reinterpret_cast<unsigned long long*>(m->d_out_mapped + MF_MAX_PARAMS + 2) : nullptr;
+    a.done_value = m->seq + 1;
     const int grid = (pipelined && M::CTAS_PER_SM > 1 && m->grid > ctx->sm_count) ? std::max(ctx->sm_count, m->grid / 2) : m->grid;
     MF_CUDA(ctx, launch_pdl(nll_grad_kernel<M>, grid, ctx->stream, a));
     ++m->seq;
@@ -390,12 +394,13 @@ static mf_status launch_single(mf_model* m, const double* lam, double* out_dev, 
     return MF_OK;
 }
 
-static mf_status dispatch_single(mf_model* m, const double* lam, double* out_dev, bool pipelined = false)
+static mf_status dispatch_single(mf_model* m, const double* lam, double* out_dev, bool pipelined = false,
+                                 bool signal_host = false)
 {
     switch (m->kind) {
-    case MF_MASS_GAUSS_EXP: return launch_single<MassModel>(m, lam, out_dev, pipelined);
-    case MF_ANGULAR_KSTMUMU: return launch_single<AngularModel>(m, lam, out_dev, false);
-    default: return launch_single<FourDModel>(m, lam, out_dev, false);
+    case MF_MASS_GAUSS_EXP: return launch_single<MassModel>(m, lam, out_dev, pipelined, signal_host);
+    case MF_ANGULAR_KSTMUMU: return launch_single<AngularModel>(m, lam, out_dev, false, signal_host);
+    default: return launch_single<FourDModel>(m, lam, out_dev, false, signal_host);
     }
 }
 
@@ -423,9 +428,22 @@ extern "C" mf_status mf_nll_grad(mf_model* m, const double* lambda, double* nll,
     if (!m || !lambda || !nll) return mf_fail(m ? m->ctx : nullptr, MF_ERR_ARG, "mf_nll_grad: NULL argument");
     if (m->n_toys != 1) return mf_fail(m->ctx, MF_ERR_ARG, "mf_nll_grad: dataset has n_toys != 1; use mf_nll_grad_batch");
     mf_ctx* ctx = m->ctx;
-    const mf_status st = dispatch_single(m, lambda, m->d_out_mapped);  // the last CTA writes to mapped pinned memory
+    // the last CTA writes the result, then the done word, to mapped pinned memory; the host spins on the
+    // done word (a stream synchronise costs ~20 us of driver latency per call, the kernel 4-30 us)
+    const mf_status st = dispatch_single(m, lambda, m->d_out_mapped, false, true);
     if (st != MF_OK) return st;
-    MF_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    volatile unsigned long long* done = reinterpret_cast<volatile unsigned long long*>(m->h_out + MF_MAX_PARAMS + 2);
+    const unsigned long long want = m->seq;
+    for (unsigned spins = 1; *done != want; ++spins) {
+        if ((spins & 0xFFFF) == 0) {  // every ~65k polls: make sure the stream is still alive
+            const cudaError_t q = cudaStreamQuery(ctx->stream);
+            if (q != cudaErrorNotReady && *done != want) {
+                if (q == cudaSuccess) continue;  // completed: the word is on its way
+                return mf_fail(ctx, MF_ERR_CUDA, std::string("mf_nll_grad: ") + cudaGetErrorString(q));
+            }
+        }
+    }
+    std::atomic_thread_fence(std::memory_order_acquire);
     *nll = m->h_out[0];
     if (grad) std::memcpy(grad, m->h_out + 1, sizeof(double) * m->K);
     if (m->h_out[m->K + 1] != 0.0)

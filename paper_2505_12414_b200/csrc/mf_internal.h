@@ -52,7 +52,7 @@ struct mf_model {
     unsigned* ticket = nullptr;       // device, kRing (single) + n_toys (batch)
     unsigned long long* gen = nullptr;  // device [kRing]: evaluations completed per scratch slot
     unsigned long long seq = 0;       // evaluations enqueued so far (evaluation e uses slot e % kRing)
-    double* h_out = nullptr;          // pinned + mapped host, MF_MAX_PARAMS+2
+    double* h_out = nullptr;          // pinned + mapped host, MF_MAX_PARAMS+2 doubles, then the 64-bit done word
     double* d_out_mapped = nullptr;   // device alias of h_out
     // batched evaluation
     int chunks = 1;                   // CTAs per toy

@@ -46,6 +46,8 @@ struct EvalArgs {
     unsigned long long* gen;     // evaluations completed on this slot
     unsigned long long need;     // value of *gen at which the slot is free for this evaluation
     double* out;                 // [K+2]: -lnL, grad, n_bad
+    unsigned long long* done_flag;   // mapped host word that receives done_value after `out` is written, or NULL
+    unsigned long long done_value;
 };
 
 template <class M>
@@ -295,7 +297,8 @@ __device__ __forceinline__ double block_reduce(double* acc, unsigned bad, double
 template <class M>
 __device__ __forceinline__ void final_combine(const double* p, int64_t stride_k, int count, const unsigned* badp,
                                               const typename M::Consts& c, double n, double sum_m, double* s_sum,
-                                              double* out)
+                                              double* out, unsigned long long* done_flag = nullptr,
+                                              unsigned long long done_value = 0)
 {
     constexpr int NACC = M::NACC, K = M::K;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -344,6 +347,10 @@ __device__ __forceinline__ void final_combine(const double* p, int64_t stride_k,
         for (int k = 0; k <= K; ++k)
             out[k] = !nb ? o[k] : (k == 0) ? __longlong_as_double(0x7ff0000000000000LL) : __longlong_as_double(0x7ff8000000000000LL);
         out[K + 1] = (double)nb;
+        if (done_flag) {  // synchronous call: the host spins on this word instead of a stream synchronise
+            __threadfence_system();
+            *reinterpret_cast<volatile unsigned long long*>(done_flag) = done_value;
+        }
     }
 }
 
@@ -378,7 +385,8 @@ __global__ void __launch_bounds__(kBlock, M::RESIDENT_CTAS) nll_grad_kernel(cons
     if (threadIdx.x == 0) s_last = (ticket_take(a.ticket) == gridDim.x - 1);
     __syncthreads();
     if (s_last) {
-        final_combine<M>(a.partials, G, (int)G, a.bad_partials, a.c, (double)a.n, a.sum_m, s_sum, a.out);
+        final_combine<M>(a.partials, G, (int)G, a.bad_partials, a.c, (double)a.n, a.sum_m, s_sum, a.out, a.done_flag,
+                         a.done_value);
         if (threadIdx.x == 0) {  // every partial has been read: final_combine synchronises the CTA before its thread 0 returns
             *a.ticket = 0u;
             gen_store(a.gen, a.need + 1);  // releases the slot (and the ticket reset) to evaluation e + kRing
