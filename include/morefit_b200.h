@@ -39,7 +39,8 @@ typedef enum {
     MF_ERR_OOM = 3,          /* host or device allocation failed */
     MF_ERR_DATA_RANGE = 4,   /* an event is non-finite or outside [lo, hi] */
     MF_ERR_PARAM_DOMAIN = 5, /* non-finite lambda, sigma <= 0 or f outside [0,1]: outputs untouched */
-    MF_NONPOSITIVE_PDF = 6   /* P(x_i|lambda) <= 0 or NaN for >= 1 event: nll = +inf, grad = NaN */
+    MF_NONPOSITIVE_PDF = 6   /* P(x_i|lambda) <= 0, NaN, or underflowed (P N2 e^{-tau m} < 2^-1000) for >= 1 event:
+                                nll = +inf, grad = NaN */
 } mf_status;
 
 /* Model families (BASELINE.json configs; parameter order = SURVEY.md §8(b)).
@@ -198,7 +199,8 @@ mf_status mf_probe_fp64_rate(mf_ctx* ctx, double* dfma_per_second);
 mf_status mf_probe_read_bandwidth(mf_ctx* ctx, size_t bytes, int repeats, double* bytes_per_second);
 /* Evaluates the kernels' own device math element by element, for the accuracy tests:
  * op 0 = exp (finite x < 709; x <= -708 gives 0), 1 = log (positive normal x), 2 = reciprocal,
- * 3 = the table-by-shuffle exp the event loops use (same domain as op 0).
+ * 3 = the table-by-shuffle exp the event loops use (same domain; x below about -708 gives a value in
+ *     [2^-1022, 2^-1021], which the kernels treat as zero, instead of 0).
  * x_host, y_host: host, n doubles. */
 mf_status mf_probe_math(mf_ctx* ctx, int op, int64_t n, const double* x_host, double* y_host);
 

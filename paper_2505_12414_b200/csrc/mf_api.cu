@@ -252,6 +252,7 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
     } while (0)
     const int64_t per_dim = m->n_pad * m->n_toys;
     const double* raw = m->raw->p;
+    double2* d_part = nullptr;  // scratch of the column sum, freed after the synchronise below
     if (kind == MF_MASS_GAUSS_EXP) {
         m->col[0] = raw;
     } else {
@@ -276,8 +277,16 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
     if (kind != MF_ANGULAR_KSTMUMU) {
         // S1: sum_i m_i per toy (ln P_i contains tau m_i: its sum is an event-only constant times tau)
         MF_CUDA_M(cudaMalloc(&m->d_sum_m, sizeof(double) * m->n_toys));
-        column_sum_kernel<<<(unsigned)m->n_toys, 256, 0, ctx->stream>>>(raw, m->n_events, m->n_pad, m->d_sum_m);
+        const int chunks = (int)std::max<int64_t>(1, std::min<int64_t>(m->n_pad / 8192, 512));
+        if (chunks > 1) MF_CUDA_M(cudaMalloc(&d_part, sizeof(double2) * m->n_toys * chunks));
+        column_sum_kernel<<<(unsigned)(m->n_toys * chunks), 256, 0, ctx->stream>>>(raw, m->n_events, m->n_pad, chunks, d_part,
+                                                                                 m->d_sum_m);
         ++ctx->launches;
+        if (chunks > 1) {
+            column_sum_finish_kernel<<<(unsigned)((m->n_toys + 127) / 128), 128, 0, ctx->stream>>>(d_part, chunks, m->n_toys,
+                                                                                                 m->d_sum_m);
+            ++ctx->launches;
+        }
         MF_CUDA_M(cudaGetLastError());
         MF_CUDA_M(cudaMemcpyAsync(&m->h_sum_m, m->d_sum_m, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     }
@@ -312,7 +321,11 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
         MF_CUDA_M(cudaHostAlloc(&m->h_ids, sizeof(int) * T, cudaHostAllocDefault));
         MF_CUDA_M(cudaHostAlloc(&m->h_bout, sizeof(double) * T * (K + 2), cudaHostAllocDefault));
     }
-    MF_CUDA_M(cudaStreamSynchronize(ctx->stream));
+    {
+        const cudaError_t e_sync = cudaStreamSynchronize(ctx->stream);
+        cudaFree(d_part);
+        MF_CUDA_M(e_sync);
+    }
 #undef MF_CUDA_M
     *out = m;
     return MF_OK;

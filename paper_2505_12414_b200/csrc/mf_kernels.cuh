@@ -196,11 +196,14 @@ __device__ __forceinline__ void accumulate(const double* const* col, int64_t n, 
             if (j0 + u * step < n_items) load_item<M>(col, j0 + u * step, lane, buf[u][0], buf[u][1]);
         constexpr int U = M::ITEMS_PER_ITER;  // items evaluated together: 2U independent events interleaved
         static_assert(D % U == 0, "PREFETCH must be a multiple of ITEMS_PER_ITER");
+        const int64_t n_full = n / kItem;  // items 0 .. n_full-1 have 64 valid events
         for (int64_t j = j0; j < n_items; j += D * step) {
 #pragma unroll
             for (int u = 0; u < D; u += U) {
                 const int64_t ju = j + u * step;
                 if (ju < n_items) {
+                    // take the group out of the window and refill its slots at once (measured: refilling
+                    // after the evaluation saves the copies but costs the HBM-fed batch kernel 15%)
                     double x[U][2][M::NCOL];
 #pragma unroll
                     for (int v = 0; v < U; ++v) {
@@ -212,8 +215,7 @@ __device__ __forceinline__ void accumulate(const double* const* col, int64_t n, 
                         const int64_t jn = ju + (v + D) * step;
                         if (jn < n_items) load_item<M>(col, jn, lane, buf[u + v][0], buf[u + v][1]);
                     }
-                    const int64_t jl = ju + (U - 1) * step;  // last item of the group
-                    if (jl < n_items && kItem * (jl + 1) <= n) {
+                    if (ju + (U - 1) * step < n_full) {
 #pragma unroll
                         for (int v = 0; v < U; ++v) {
                             M::template event<false>(x[v][0], c, acc, lp, bad, true, t_lane);
@@ -496,15 +498,29 @@ __global__ void __launch_bounds__(kBlock, M::RESIDENT_CTAS) nll_grad_batch_kerne
 
 // ---- S1: event-only constants: sum_i m_i per toy ------------------------------
 
-// One CTA per toy; deterministic: thread t Kahan-sums events t, t + 256, ..., the 256 (sum, compensation)
-// pairs are merged by a fixed two-sum tree in shared memory.
+// Deterministic two-level sum.  Level 1: CTA (toy, chunk) sums events [chunk * len, (chunk+1) * len) of its
+// toy — thread t Kahan-sums events t, t + 256, ..., the 256 (sum, compensation) pairs are merged by a
+// fixed two-sum tree in shared memory — and writes the pair to part[toy][chunk].  Level 2 (chunks > 1):
+// one thread per toy adds the chunk pairs in chunk order.
+__device__ __forceinline__ void two_sum_acc(double& s, double& lo, double b, double blo)
+{
+    const double t = s + b;
+    const double bb = t - s;
+    const double e = (s - (t - bb)) + (b - bb);
+    lo = (lo + blo) + e;
+    s = t;
+}
+
 __global__ void __launch_bounds__(256) column_sum_kernel(const double* __restrict__ col, int64_t n, int64_t n_pad,
-                                                         double* __restrict__ out)
+                                                         int chunks, double2* __restrict__ part, double* __restrict__ out)
 {
     __shared__ double sh[256], sl[256];
-    const double* x = col + (int64_t)blockIdx.x * n_pad;
+    const int toy = blockIdx.x / chunks, chunk = blockIdx.x % chunks;
+    const int64_t len = (n + chunks - 1) / chunks;
+    const int64_t lo_i = chunk * len, hi_i = (lo_i + len < n) ? lo_i + len : n;
+    const double* x = col + (int64_t)toy * n_pad;
     double s = 0.0, cc = 0.0;
-    for (int64_t i = threadIdx.x; i < n; i += 256) {
+    for (int64_t i = lo_i + threadIdx.x; i < hi_i; i += 256) {
         const double y = x[i] - cc;
         const double t = s + y;
         cc = (t - s) - y;
@@ -515,16 +531,31 @@ __global__ void __launch_bounds__(256) column_sum_kernel(const double* __restric
     __syncthreads();
     for (int off = 128; off > 0; off >>= 1) {
         if (threadIdx.x < off) {
-            const double a = sh[threadIdx.x], b = sh[threadIdx.x + off];
-            const double t = a + b;
-            const double bb = t - a;
-            const double e = (a - (t - bb)) + (b - bb);
-            sl[threadIdx.x] = (sl[threadIdx.x] + sl[threadIdx.x + off]) + e;
-            sh[threadIdx.x] = t;
+            double a = sh[threadIdx.x], alo = sl[threadIdx.x];
+            two_sum_acc(a, alo, sh[threadIdx.x + off], sl[threadIdx.x + off]);
+            sh[threadIdx.x] = a;
+            sl[threadIdx.x] = alo;
         }
         __syncthreads();
     }
-    if (threadIdx.x == 0) out[blockIdx.x] = sh[0] + sl[0];
+    if (threadIdx.x == 0) {
+        if (chunks == 1)
+            out[toy] = sh[0] + sl[0];
+        else
+            part[blockIdx.x] = make_double2(sh[0], sl[0]);
+    }
+}
+
+__global__ void column_sum_finish_kernel(const double2* __restrict__ part, int chunks, int64_t n_toys, double* __restrict__ out)
+{
+    const int64_t toy = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (toy >= n_toys) return;
+    double s = 0.0, lo = 0.0;
+    for (int c = 0; c < chunks; ++c) {
+        const double2 p = part[toy * chunks + c];
+        two_sum_acc(s, lo, p.x, p.y);
+    }
+    out[toy] = s + lo;
 }
 
 // ---- S1: event-only precompute (Listing 4) ------------------

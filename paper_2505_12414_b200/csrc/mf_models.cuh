@@ -111,6 +111,9 @@ MF_HD inline bool mass_consts(const double* lam, double ma, double mb, MassConst
         return false;
     const double mmax = fmax(fabs(ma), fabs(mb));
     if (!(c.lnk + fabs(tau) * mmax < 700.0)) return false;
+    // ... and whose most negative one is beyond the range in which mf_exp32 reduces its argument
+    const double dmax = fmax(fabs(ma - mu), fabs(mb - mu));
+    if (!(-c.nb0 * dmax * dmax + fabs(tau) * mmax + fabs(c.lnk) < 1e12)) return false;
     return true;
 }
 
