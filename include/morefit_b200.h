@@ -134,8 +134,8 @@ mf_status mf_nll_grad_async(mf_model* model, const double* lambda, double* out_d
 mf_status mf_nll_grad_points(mf_model* model, int64_t n_points, const double* lambdas, double* out_dev);
 
 /* T pseudo-experiments at their own parameter points in ONE launch (BASELINE.json
- * configs[4]): a CTA tile is (toy, event chunk); each CTA derives its toy's
- * parameter-only constants in a short prologue.
+ * configs[4]): a CTA tile is (toy, event chunk); the toys' parameter-only constants are
+ * derived on the device by a small kernel launched just before it.
  *   n_toys   must equal the dataset's n_toys.
  *   lambdas  host, [n_toys][K].   active  host, n_toys bytes or NULL (= all active).
  *   nll      host, [n_toys].      grad    host, [n_toys][K] or NULL.
@@ -144,6 +144,11 @@ mf_status mf_nll_grad_points(mf_model* model, int64_t n_points, const double* la
  * grad = NaN; the call still returns MF_OK. */
 mf_status mf_nll_grad_batch(mf_model* model, int64_t n_toys, const double* lambdas,
                             const uint8_t* active, double* nll, double* grad);
+
+/* The same evaluation for ALL toys without host copies or synchronisation: lambdas_dev is DEVICE [n_toys][K],
+ * out_dev DEVICE [n_toys][K+2], row t = [-ln L, grad, n_bad] of toy t (n_bad = -1: lambda_t outside the domain).
+ * Two launches are enqueued on the context's stream (parameter-only constants, then the fused kernel). */
+mf_status mf_nll_grad_batch_async(mf_model* model, int64_t n_toys, const double* lambdas_dev, double* out_dev);
 
 /* ---- fit driver (host quasi-Newton over the GPU value+gradient) ------- */
 

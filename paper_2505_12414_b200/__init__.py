@@ -33,7 +33,7 @@ EXPORTS = [
     "mf_ctx_create", "mf_ctx_destroy", "mf_last_error", "mf_ctx_kernel_launches",
     "mf_dataset_upload", "mf_dataset_destroy", "mf_dataset_n_events", "mf_dataset_n_toys",
     "mf_model_create", "mf_model_destroy", "mf_model_nparams", "mf_model_n_events", "mf_model_n_toys",
-    "mf_nll_grad", "mf_nll_grad_async", "mf_nll_grad_points", "mf_nll_grad_batch",
+    "mf_nll_grad", "mf_nll_grad_async", "mf_nll_grad_points", "mf_nll_grad_batch", "mf_nll_grad_batch_async",
     "mf_fit_opts_default", "mf_fit", "mf_fit_batch",
     "mf_probe_fp64_rate", "mf_probe_read_bandwidth", "mf_probe_math",
 ]
@@ -130,6 +130,8 @@ def load_library() -> ctypes.CDLL:
     lib.mf_nll_grad_points.argtypes = [vp, i64, dp, vp]
     lib.mf_nll_grad_batch.restype = ctypes.c_int
     lib.mf_nll_grad_batch.argtypes = [vp, i64, dp, u8p, dp, dp]
+    lib.mf_nll_grad_batch_async.restype = ctypes.c_int
+    lib.mf_nll_grad_batch_async.argtypes = [vp, i64, vp, vp]
     lib.mf_fit_opts_default.restype = None
     lib.mf_fit_opts_default.argtypes = [ctypes.POINTER(FitOpts)]
     lib.mf_fit.restype = ctypes.c_int
@@ -325,6 +327,11 @@ class Model:
         grad = np.full((T, self.K), np.nan)
         self._ctx._check(self._lib.mf_nll_grad_batch(self._h, T, _dp(lam), _u8p(act), _dp(nll), _dp(grad)))
         return nll, grad
+
+    def nll_grad_batch_async(self, lambdas_dev_ptr: int, out_dev_ptr: int):
+        """All toys, device pointers in ([T][K]) and out ([T][K+2]), no host synchronisation."""
+        self._ctx._check(self._lib.mf_nll_grad_batch_async(self._h, self.n_toys, ctypes.c_void_p(lambdas_dev_ptr),
+                                                           ctypes.c_void_p(out_dev_ptr)))
 
     def fit(self, start, fixed=None, opts: FitOpts | None = None) -> FitResult:
         start = np.ascontiguousarray(start, dtype=np.float64)

@@ -466,7 +466,7 @@ extern "C" mf_status mf_nll_grad(mf_model* m, const double* lambda, double* nll,
 }
 
 template <class M>
-static mf_status launch_batch(mf_model* m, int n_active)
+static mf_status launch_batch(mf_model* m, int n_active, const double* lam_dev = nullptr, double* out_dev = nullptr)
 {
     mf_ctx* ctx = m->ctx;
     BatchArgs<M> a;
@@ -478,19 +478,31 @@ static mf_status launch_batch(mf_model* m, int n_active)
     a.ma = m->ma;
     a.mb = m->mb;
     a.sum_m = m->d_sum_m;
-    a.lam = m->d_lam;
+    a.lam = lam_dev ? lam_dev : m->d_lam;
     a.consts = static_cast<typename M::Consts*>(m->d_consts);
     a.consts_ok = m->d_consts_ok;
-    a.ids = m->d_ids;
+    a.ids = (n_active == m->n_toys) ? nullptr : m->d_ids;
     a.partials = m->b_partials;
     a.bad_partials = m->b_bad;
     a.ticket = m->ticket + kRing;
-    a.out = m->d_bout;
+    a.out = out_dev ? out_dev : m->d_bout;
     batch_consts_kernel<M><<<(n_active + 127) / 128, 128, 0, ctx->stream>>>(a, n_active);
     MF_CUDA(ctx, cudaGetLastError());
     MF_CUDA(ctx, launch_pdl(nll_grad_batch_kernel<M>, n_active * m->chunks, ctx->stream, a));
     ctx->launches += 2;
     return MF_OK;
+}
+
+extern "C" mf_status mf_nll_grad_batch_async(mf_model* m, int64_t n_toys, const double* lambdas_dev, double* out_dev)
+{
+    if (!m || !lambdas_dev || !out_dev) return mf_fail(m ? m->ctx : nullptr, MF_ERR_ARG, "mf_nll_grad_batch_async: NULL argument");
+    if (n_toys != m->n_toys || m->n_toys < 2 || !m->d_lam)
+        return mf_fail(m->ctx, MF_ERR_ARG, "mf_nll_grad_batch_async: needs a dataset with n_toys > 1 and n_toys equal to it");
+    switch (m->kind) {
+    case MF_MASS_GAUSS_EXP: return launch_batch<MassModel>(m, (int)n_toys, lambdas_dev, out_dev);
+    case MF_ANGULAR_KSTMUMU: return launch_batch<AngularModel>(m, (int)n_toys, lambdas_dev, out_dev);
+    default: return launch_batch<FourDModel>(m, (int)n_toys, lambdas_dev, out_dev);
+    }
 }
 
 extern "C" mf_status mf_nll_grad_batch(mf_model* m, int64_t n_toys, const double* lambdas, const uint8_t* active,
@@ -522,7 +534,8 @@ extern "C" mf_status mf_nll_grad_batch(mf_model* m, int64_t n_toys, const double
     }
     if (n_active == 0) return MF_OK;
     MF_CUDA(ctx, cudaMemcpyAsync(m->d_lam, m->h_lam, sizeof(double) * n_active * K, cudaMemcpyHostToDevice, ctx->stream));
-    MF_CUDA(ctx, cudaMemcpyAsync(m->d_ids, m->h_ids, sizeof(int) * n_active, cudaMemcpyHostToDevice, ctx->stream));
+    if (n_active < n_toys)
+        MF_CUDA(ctx, cudaMemcpyAsync(m->d_ids, m->h_ids, sizeof(int) * n_active, cudaMemcpyHostToDevice, ctx->stream));
     mf_status st;
     switch (m->kind) {
     case MF_MASS_GAUSS_EXP: st = launch_batch<MassModel>(m, n_active); break;

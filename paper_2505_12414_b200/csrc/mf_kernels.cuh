@@ -62,7 +62,7 @@ struct BatchArgs {
     const double* lam;           // [n_active][K]
     typename M::Consts* consts;  // [n_active] parameter-only constants (S2), written by batch_consts_kernel
     int* consts_ok;              // [n_active] 0 = lambda outside the parameter domain
-    const int* ids;              // [n_active] toy index of each active slot
+    const int* ids;              // [n_active] toy index of each active slot; NULL = identity (all toys active)
     double* partials;            // [n_active][NACC][chunks]   (chunks > 1)
     unsigned* bad_partials;      // [n_active][chunks]
     unsigned* ticket;            // [n_active]
@@ -417,7 +417,7 @@ __global__ void __launch_bounds__(128) batch_consts_kernel(const __grid_constant
 // CTA <-> (toy, event chunk)
 
 template <class M>
-__global__ void __launch_bounds__(kBlock, M::RESIDENT_CTAS) nll_grad_batch_kernel(const __grid_constant__ BatchArgs<M> a)
+__global__ void __launch_bounds__(kBlock, M::BATCH_RESIDENT_CTAS) nll_grad_batch_kernel(const __grid_constant__ BatchArgs<M> a)
 {
     constexpr int NACC = M::NACC;
     constexpr int K = M::K;
@@ -431,6 +431,17 @@ __global__ void __launch_bounds__(kBlock, M::RESIDENT_CTAS) nll_grad_batch_kerne
 
     pdl_launch_dependents();
     const int slot = blockIdx.x / a.chunks, chunk = blockIdx.x % a.chunks;
+    const int64_t toy = a.ids ? a.ids[slot] : slot;  // ids == NULL: every toy is active
+    if (a.chunks == 1) {
+        // this CTA streams its toy's columns once from HBM: ask for them now (L2 prefetch, 128-byte lines), so
+        // that they arrive while the constants are fetched and the first loads of the event loop hit L2
+        const int64_t lines = (a.n_items * kItem * (int64_t)sizeof(double) + 127) / 128;
+#pragma unroll
+        for (int q = 0; q < M::NCOL; ++q) {
+            const char* base = reinterpret_cast<const char*>(a.col[q] + toy * a.toy_stride);
+            for (int64_t l = threadIdx.x; l < lines; l += kBlock) asm volatile("prefetch.global.L2 [%0];" ::"l"(base + 128 * l));
+        }
+    }
     // S2 for this toy: parameter-only constants of lambda_t (batch_consts_kernel, the previous launch)
     pdl_wait();
     {
@@ -451,7 +462,6 @@ __global__ void __launch_bounds__(kBlock, M::RESIDENT_CTAS) nll_grad_batch_kerne
         return;
     }
     const typename M::Consts c = s_c;
-    const int64_t toy = a.ids[slot];
     const double sum_m = a.sum_m ? a.sum_m[toy] : 0.0;
     const double* col[M::NCOL];
 #pragma unroll

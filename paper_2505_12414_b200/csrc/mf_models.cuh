@@ -200,6 +200,10 @@ struct MassModel {
     static constexpr int ITEMS_PER_ITER = MF_MASS_U;    // x2 independent events in flight per thread
     static constexpr int PREFETCH = MF_MASS_PREFETCH;   // rolling window of 16-byte loads in flight per thread (0: double buffer)
     static constexpr int CTAS_PER_SM = MF_MASS_GRID;    // grid of a lone (synchronous) evaluation: CTAs per SM
+#ifndef MF_MASS_BATCH_RESIDENT
+#define MF_MASS_BATCH_RESIDENT 3
+#endif
+    static constexpr int BATCH_RESIDENT_CTAS = MF_MASS_BATCH_RESIDENT;  // the batched kernel: more, smaller-budget CTAs
     static constexpr int RESIDENT_CTAS = MF_MASS_RESIDENT;  // register budget: CTAs of the next evaluation co-reside under PDL
     using Consts = MassConsts;
 
@@ -247,6 +251,7 @@ struct AngularModel {
     static constexpr int PREFETCH = 0;
     static constexpr int CTAS_PER_SM = 2;
     static constexpr int RESIDENT_CTAS = 2;
+    static constexpr int BATCH_RESIDENT_CTAS = 2;
     using Consts = AngularConsts;
 
     template <bool PRED>
@@ -278,6 +283,7 @@ struct FourDModel {
     static constexpr int ITEMS_PER_ITER = 1;
     static constexpr int PREFETCH = 0;
     static constexpr int RESIDENT_CTAS = 1;
+    static constexpr int BATCH_RESIDENT_CTAS = 1;
     static constexpr int CTAS_PER_SM = 1;  // 17 sums + two 12-column register buffers: needs > 128 registers
     using Consts = FourDConsts;
 

@@ -288,3 +288,72 @@ def test_device_math_accuracy(mf, ctx):
     assert ctx.probe_math("log", np.array([1.0]))[0] == 0.0
     r = ctx.probe_math("rcp", v)
     assert np.max(_ulp_err(r, 1.0 / v)) <= 2.0
+
+
+def test_points_and_pipelining(mf, ctx):
+    """mf_nll_grad_points: 40 back-to-back evaluations (more than the scratch ring holds, programmatic dependent
+    launch between them) give, point by point, exactly what mf_nll_grad gives, and match the oracle."""
+    import torch
+    n = 100_003
+    m = dg.gen_mass(n, seed=5)
+    model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(m, dg.MASS_LO, dg.MASS_HI))
+    pts = dg.gen_lambda_points(40, 77, dg.MASS_TRUTH, 3 * dg.mass_sigma_stat(n))
+    out = torch.full((40, 6), float("nan"), dtype=torch.float64, device="cuda")
+    for _ in range(3):                      # repeated: the ring wraps many times
+        model.nll_grad_points(pts, out.data_ptr())
+    out2 = torch.full((40, 6), float("nan"), dtype=torch.float64, device="cuda")
+    model.nll_grad_points(pts, out2.data_ptr())
+    torch.cuda.synchronize()
+    res = out.cpu().numpy()
+    assert np.array_equal(res, out2.cpu().numpy())      # a series is bit-reproducible
+    assert np.all(res[:, 5] == 0)
+    for p in (0, 1, 7, 39):
+        nll, g = model.nll_grad(pts[p])   # the lone call uses a larger grid: same value up to summation order
+        assert abs(res[p, 0] - nll) <= 1e-13 * abs(nll) and np.all(np.abs(res[p, 1:5] - g) <= 1e-11 * (1 + np.abs(g)))
+        o_nll, o_g, _ = oracle.nll_grad(oracle.MASS, m, pts[p], dg.MASS_LO, dg.MASS_HI)
+        assert_parity(res[p, 0], res[p, 1:5], o_nll, o_g, f"point {p}")
+    # a point outside the domain stops the series with MF_ERR_PARAM_DOMAIN
+    bad = pts.copy()
+    bad[3, 2] = -1.0
+    with pytest.raises(mf.MoreFitError):
+        model.nll_grad_points(bad, out.data_ptr())
+    torch.cuda.synchronize()
+
+
+def test_batch_async_parity(mf, ctx):
+    """mf_nll_grad_batch_async (device pointers, no host copies) equals mf_nll_grad_batch bit for bit."""
+    import torch
+    T, n = 9, 3000
+    toys = dg.gen_mass_toys(T, n, first_seed=300)
+    model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(toys, dg.MASS_LO, dg.MASS_HI, n_toys=T))
+    lams = dg.gen_lambda_points(T, 6, dg.MASS_TRUTH, 3 * dg.mass_sigma_stat(n))
+    lams[4] = (0.3, 5.28, -2.0, -1.5)       # outside the domain: +inf / NaN / n_bad = -1
+    nll, g = model.nll_grad_batch(lams)
+    d_lam = torch.from_numpy(lams).cuda()
+    d_out = torch.zeros((T, 6), dtype=torch.float64, device="cuda")
+    model.nll_grad_batch_async(d_lam.data_ptr(), d_out.data_ptr())
+    torch.cuda.synchronize()
+    res = d_out.cpu().numpy()
+    ok = np.arange(T) != 4
+    assert np.array_equal(res[ok, 0], nll[ok]) and np.array_equal(res[ok, 1:5], g[ok])
+    assert res[4, 0] == math.inf and np.all(np.isnan(res[4, 1:5])) and res[4, 5] == -1.0
+    o_nll, o_g, _ = oracle.nll_grad(oracle.MASS, toys[2], lams[2], dg.MASS_LO, dg.MASS_HI)
+    assert_parity(res[2, 0], res[2, 1:5], o_nll, o_g, "toy 2")
+
+
+def test_underflowed_pdf_is_flagged(mf, ctx):
+    """f = 1 and an event 60 sigma from the peak: P underflows to 0 in fp64 (oracle: P <= 0 -> +inf); the CUDA
+    path's exponential is clamped, not flushed, and LogProd flags the event instead (reading R15)."""
+    m = np.array([5.10, 5.28, 5.29, 5.27])
+    model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(m, dg.MASS_LO, dg.MASS_HI))
+    lam = (1.0, 5.28, 0.003, -1.5)
+    o_nll, o_g, o_bad = oracle.nll_grad(oracle.MASS, m, lam, dg.MASS_LO, dg.MASS_HI)
+    assert o_bad == 1 and o_nll == math.inf
+    st, nll, g = model.nll_grad_status(lam)
+    assert st == mf.MF_NONPOSITIVE_PDF and nll == math.inf and np.all(np.isnan(g))
+    # with a background component the same event is fine on both sides
+    lam2 = (0.9, 5.28, 0.003, -1.5)
+    nll, g = model.nll_grad(lam2)
+    o_nll, o_g, o_bad = oracle.nll_grad(oracle.MASS, m, lam2, dg.MASS_LO, dg.MASS_HI)
+    assert o_bad == 0
+    assert_parity(nll, g, o_nll, o_g, "f = 0.9")
