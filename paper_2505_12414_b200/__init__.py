@@ -14,6 +14,7 @@ The names mirror the C entry points: ``Context`` (mf_ctx_*), ``Context.dataset_u
 from __future__ import annotations
 
 import ctypes
+import weakref
 import os
 
 import numpy as np
@@ -168,6 +169,7 @@ class Context:
     def __init__(self, device: int = 0, stream: int | None = None):
         self._lib = load_library()
         self._h = ctypes.c_void_p()
+        self._children = weakref.WeakSet()   # live datasets / models, closed before the context
         if stream is None:
             import torch  # device memory / streams come from PyTorch (plumbing only)
             if not torch.cuda.is_available():
@@ -214,7 +216,10 @@ class Context:
         return Model(self, kind, dataset)
 
     def close(self):
+        """Destroys the context after every dataset and model made from it (the C-ABI's required order)."""
         if self._h:
+            for child in list(self._children):
+                child.close()
             self._lib.mf_ctx_destroy(self._h)
             self._h = ctypes.c_void_p()
 
@@ -261,6 +266,7 @@ class Dataset:
                                          ctypes.byref(self._h))
         del keep
         ctx._check(st)
+        ctx._children.add(self)
         self.ndim, self.n_events, self.n_toys = ndim, total // n_toys, int(n_toys)
 
     def close(self):
@@ -280,6 +286,7 @@ class Model:
         self._ctx, self._lib = ctx, ctx._lib
         self._h = ctypes.c_void_p()
         ctx._check(self._lib.mf_model_create(ctx._h, int(kind), dataset._h, ctypes.byref(self._h)))
+        ctx._children.add(self)
         self.kind = int(kind)
         self.K = int(self._lib.mf_model_nparams(self._h))
         self.n_events = int(self._lib.mf_model_n_events(self._h))

@@ -30,12 +30,45 @@ mf_status mf_fail(mf_ctx* ctx, mf_status st, const std::string& msg)
         }                                                                                               \
     } while (0)
 
+// ---- allocation: device memory from the stream-ordered pool (kept warm: creating and destroying a dataset +
+// model per call must not pay cudaMalloc / cudaFree synchronisations), result slots from one pinned, mapped slab.
+template <class T>
+static cudaError_t dev_alloc(mf_ctx* ctx, T** p, size_t bytes)
+{
+    return cudaMallocAsync(reinterpret_cast<void**>(p), bytes ? bytes : 1, ctx->stream);
+}
+static void dev_free(mf_ctx* ctx, void* p)
+{
+    if (p) cudaFreeAsync(p, ctx->stream);
+}
+static cudaError_t host_slot_acquire(mf_ctx* ctx, double** h, double** d)
+{
+    if (!ctx->h_slab) {
+        cudaError_t e = cudaHostAlloc(&ctx->h_slab, sizeof(double) * MF_HOST_SLOT_DOUBLES * MF_HOST_SLOTS, cudaHostAllocMapped);
+        if (e != cudaSuccess) return e;
+        e = cudaHostGetDevicePointer(&ctx->d_slab, ctx->h_slab, 0);
+        if (e != cudaSuccess) return e;
+        for (int i = MF_HOST_SLOTS - 1; i >= 0; --i) ctx->free_slots.push_back(i);
+    }
+    if (ctx->free_slots.empty()) return cudaErrorMemoryAllocation;  // more than MF_HOST_SLOTS live models
+    const int i = ctx->free_slots.back();
+    ctx->free_slots.pop_back();
+    *h = ctx->h_slab + (size_t)i * MF_HOST_SLOT_DOUBLES;
+    *d = ctx->d_slab + (size_t)i * MF_HOST_SLOT_DOUBLES;
+    std::memset(*h, 0, sizeof(double) * MF_HOST_SLOT_DOUBLES);
+    return cudaSuccess;
+}
+static void host_slot_release(mf_ctx* ctx, double* h)
+{
+    if (h && ctx && ctx->h_slab) ctx->free_slots.push_back((int)((h - ctx->h_slab) / MF_HOST_SLOT_DOUBLES));
+}
+
 static inline int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
 
 static void devbuf_release(mf_devbuf* b)
 {
     if (b && --b->refs == 0) {
-        if (b->p) cudaFree(b->p);
+        if (b->p) cudaFreeAsync(b->p, b->stream);
         delete b;
     }
 }
@@ -60,11 +93,26 @@ extern "C" mf_status mf_ctx_create(int device, void* cuda_stream, mf_ctx** out)
         delete ctx;
         return MF_ERR_CUDA;
     }
+    cudaMemPool_t pool;
+    if (cudaDeviceGetDefaultMemPool(&pool, device) == cudaSuccess) {
+        unsigned long long keep = ~0ull;  // freed blocks stay in the pool for the next dataset / model
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    }
+    cudaGetLastError();
     *out = ctx;
     return MF_OK;
 }
 
-extern "C" void mf_ctx_destroy(mf_ctx* ctx) { delete ctx; }
+extern "C" void mf_ctx_destroy(mf_ctx* ctx)
+{
+    if (!ctx) return;
+    if (ctx->h_slab) {
+        cudaStreamSynchronize(ctx->stream);
+        cudaFreeHost(ctx->h_slab);
+    }
+    cudaGetLastError();
+    delete ctx;
+}
 
 extern "C" const char* mf_last_error(const mf_ctx* ctx) { return ctx ? ctx->err.c_str() : ""; }
 
@@ -121,9 +169,10 @@ extern "C" mf_status mf_dataset_upload(mf_ctx* ctx, int ndim, int64_t n_events, 
     ds->raw = buf;
     const int64_t per_dim = ds->n_pad * n_toys;
     buf->bytes = (size_t)std::max<int64_t>(per_dim * ndim, 1) * sizeof(double);
+    buf->stream = ctx->stream;
     unsigned long long* d_count = nullptr;
     auto cleanup = [&]() {
-        if (d_count) cudaFree(d_count);
+        if (d_count) cudaFreeAsync(d_count, ctx->stream);
         devbuf_release(buf);
         delete ds;
     };
@@ -136,8 +185,8 @@ extern "C" mf_status mf_dataset_upload(mf_ctx* ctx, int ndim, int64_t n_events, 
             return mf_fail(ctx, st__, std::string(#call) + ": " + cudaGetErrorString(e__));           \
         }                                                                                             \
     } while (0)
-    MF_CUDA_C(cudaMalloc(&buf->p, buf->bytes));
-    MF_CUDA_C(cudaMalloc(&d_count, sizeof(unsigned long long)));
+    MF_CUDA_C(dev_alloc(ctx, &buf->p, buf->bytes));
+    MF_CUDA_C(dev_alloc(ctx, &d_count, sizeof(unsigned long long)));
     MF_CUDA_C(cudaMemsetAsync(d_count, 0, sizeof(unsigned long long), ctx->stream));
     if (n_events > 0) {
         const cudaMemcpyKind kind = (where == MF_HOST) ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
@@ -167,7 +216,7 @@ extern "C" mf_status mf_dataset_upload(mf_ctx* ctx, int ndim, int64_t n_events, 
     MF_CUDA_C(cudaMemcpyAsync(&n_out, d_count, sizeof(n_out), cudaMemcpyDeviceToHost, ctx->stream));
     MF_CUDA_C(cudaStreamSynchronize(ctx->stream));
 #undef MF_CUDA_C
-    cudaFree(d_count);
+    cudaFreeAsync(d_count, ctx->stream);
     d_count = nullptr;
     if (n_out) {
         cleanup();
@@ -192,20 +241,23 @@ extern "C" int64_t mf_dataset_n_toys(const mf_dataset* ds) { return ds ? ds->n_t
 extern "C" void mf_model_destroy(mf_model* m)
 {
     if (!m) return;
-    cudaFree(m->cache);
-    cudaFree(m->d_sum_m);
-    cudaFree(m->partials);
-    cudaFree(m->bad_partials);
-    cudaFree(m->ticket);
-    cudaFree(m->gen);
-    cudaFree(m->b_partials);
-    cudaFree(m->b_bad);
-    cudaFree(m->d_lam);
-    cudaFree(m->d_consts);
-    cudaFree(m->d_consts_ok);
-    cudaFree(m->d_ids);
-    cudaFree(m->d_bout);
-    if (m->h_out) cudaFreeHost(m->h_out);
+    // device memory is freed in stream order; the pinned result slot is recycled at once, so no evaluation of this
+    // model may still be in flight
+    if (m->seq > 0 || m->n_toys > 1) cudaStreamSynchronize(m->ctx->stream);
+    dev_free(m->ctx, m->cache);
+    dev_free(m->ctx, m->d_sum_m);
+    dev_free(m->ctx, m->partials);
+    dev_free(m->ctx, m->bad_partials);
+    dev_free(m->ctx, m->ticket);
+    dev_free(m->ctx, m->gen);
+    dev_free(m->ctx, m->b_partials);
+    dev_free(m->ctx, m->b_bad);
+    dev_free(m->ctx, m->d_lam);
+    dev_free(m->ctx, m->d_consts);
+    dev_free(m->ctx, m->d_consts_ok);
+    dev_free(m->ctx, m->d_ids);
+    dev_free(m->ctx, m->d_bout);
+    host_slot_release(m->ctx, m->h_out);
     if (m->h_lam) cudaFreeHost(m->h_lam);
     if (m->h_ids) cudaFreeHost(m->h_ids);
     if (m->h_bout) cudaFreeHost(m->h_bout);
@@ -257,7 +309,7 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
         m->col[0] = raw;
     } else {
         // S1: cache the nine merged angular basis columns
-        MF_CUDA_M(cudaMalloc(&m->cache, (size_t)std::max<int64_t>(9 * per_dim, 1) * sizeof(double)));
+        MF_CUDA_M(dev_alloc(ctx, &m->cache, (size_t)std::max<int64_t>(9 * per_dim, 1) * sizeof(double)));
         const int a0 = (kind == MF_ANGULAR_KSTMUMU) ? 0 : 1;  // first angular dimension
         if (per_dim > 0) {
             const int grid = (int)std::min<int64_t>((per_dim + 255) / 256, 16 * (int64_t)ctx->sm_count);
@@ -276,9 +328,9 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
     }
     if (kind != MF_ANGULAR_KSTMUMU) {
         // S1: sum_i m_i per toy (ln P_i contains tau m_i: its sum is an event-only constant times tau)
-        MF_CUDA_M(cudaMalloc(&m->d_sum_m, sizeof(double) * m->n_toys));
+        MF_CUDA_M(dev_alloc(ctx, &m->d_sum_m, sizeof(double) * m->n_toys));
         const int chunks = (int)std::max<int64_t>(1, std::min<int64_t>(m->n_pad / 8192, 512));
-        if (chunks > 1) MF_CUDA_M(cudaMalloc(&d_part, sizeof(double2) * m->n_toys * chunks));
+        if (chunks > 1) MF_CUDA_M(dev_alloc(ctx, &d_part, sizeof(double2) * m->n_toys * chunks));
         column_sum_kernel<<<(unsigned)(m->n_toys * chunks), 256, 0, ctx->stream>>>(raw, m->n_events, m->n_pad, chunks, d_part,
                                                                                  m->d_sum_m);
         ++ctx->launches;
@@ -297,33 +349,31 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
     m->grid = (int)std::max<int64_t>(1, std::min<int64_t>((n_items + kWarps - 1) / kWarps, ctas_per_sm * (int64_t)ctx->sm_count));
     // batch geometry: one CTA per toy up to 32768 events per toy, else split
     m->chunks = (int)std::max<int64_t>(1, std::min<int64_t>((m->n_pad + 32767) / 32768, 64));
-    MF_CUDA_M(cudaMalloc(&m->partials, sizeof(double) * kRing * m->nacc * m->grid));
-    MF_CUDA_M(cudaMalloc(&m->bad_partials, sizeof(unsigned) * kRing * m->grid));
-    MF_CUDA_M(cudaMalloc(&m->ticket, sizeof(unsigned) * (kRing + m->n_toys)));
+    MF_CUDA_M(dev_alloc(ctx, &m->partials, sizeof(double) * kRing * m->nacc * m->grid));
+    MF_CUDA_M(dev_alloc(ctx, &m->bad_partials, sizeof(unsigned) * kRing * m->grid));
+    MF_CUDA_M(dev_alloc(ctx, &m->ticket, sizeof(unsigned) * (kRing + m->n_toys)));
     MF_CUDA_M(cudaMemsetAsync(m->ticket, 0, sizeof(unsigned) * (kRing + m->n_toys), ctx->stream));
-    MF_CUDA_M(cudaMalloc(&m->gen, sizeof(unsigned long long) * kRing));
+    MF_CUDA_M(dev_alloc(ctx, &m->gen, sizeof(unsigned long long) * kRing));
     MF_CUDA_M(cudaMemsetAsync(m->gen, 0, sizeof(unsigned long long) * kRing, ctx->stream));
-    MF_CUDA_M(cudaHostAlloc(&m->h_out, sizeof(double) * (MF_MAX_PARAMS + 3), cudaHostAllocMapped));
-    std::memset(m->h_out, 0, sizeof(double) * (MF_MAX_PARAMS + 3));
-    MF_CUDA_M(cudaHostGetDevicePointer(&m->d_out_mapped, m->h_out, 0));
+    MF_CUDA_M(host_slot_acquire(ctx, &m->h_out, &m->d_out_mapped));
     if (m->n_toys > 1) {
         const int64_t T = m->n_toys;
         if (m->chunks > 1) {
-            MF_CUDA_M(cudaMalloc(&m->b_partials, sizeof(double) * T * m->nacc * m->chunks));
-            MF_CUDA_M(cudaMalloc(&m->b_bad, sizeof(unsigned) * T * m->chunks));
+            MF_CUDA_M(dev_alloc(ctx, &m->b_partials, sizeof(double) * T * m->nacc * m->chunks));
+            MF_CUDA_M(dev_alloc(ctx, &m->b_bad, sizeof(unsigned) * T * m->chunks));
         }
-        MF_CUDA_M(cudaMalloc(&m->d_lam, sizeof(double) * T * K));
-        MF_CUDA_M(cudaMalloc(&m->d_consts, sizeof(FourDConsts) * T));  // the largest Consts
-        MF_CUDA_M(cudaMalloc(&m->d_consts_ok, sizeof(int) * T));
-        MF_CUDA_M(cudaMalloc(&m->d_ids, sizeof(int) * T));
-        MF_CUDA_M(cudaMalloc(&m->d_bout, sizeof(double) * T * (K + 2)));
+        MF_CUDA_M(dev_alloc(ctx, &m->d_lam, sizeof(double) * T * K));
+        MF_CUDA_M(dev_alloc(ctx, &m->d_consts, sizeof(FourDConsts) * T));  // the largest Consts
+        MF_CUDA_M(dev_alloc(ctx, &m->d_consts_ok, sizeof(int) * T));
+        MF_CUDA_M(dev_alloc(ctx, &m->d_ids, sizeof(int) * T));
+        MF_CUDA_M(dev_alloc(ctx, &m->d_bout, sizeof(double) * T * (K + 2)));
         MF_CUDA_M(cudaHostAlloc(&m->h_lam, sizeof(double) * T * K, cudaHostAllocDefault));
         MF_CUDA_M(cudaHostAlloc(&m->h_ids, sizeof(int) * T, cudaHostAllocDefault));
         MF_CUDA_M(cudaHostAlloc(&m->h_bout, sizeof(double) * T * (K + 2), cudaHostAllocDefault));
     }
     {
         const cudaError_t e_sync = cudaStreamSynchronize(ctx->stream);
-        cudaFree(d_part);
+        dev_free(ctx, d_part);
         MF_CUDA_M(e_sync);
     }
 #undef MF_CUDA_M

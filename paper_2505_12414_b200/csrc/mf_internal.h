@@ -4,6 +4,7 @@
 
 #include <cstdint>
 #include <string>
+#include <vector>
 
 #include "../../include/morefit_b200.h"
 
@@ -13,10 +14,18 @@ struct mf_ctx {
     int sm_count = 0;
     int64_t launches = 0;
     std::string err;
+    // pinned + mapped slab of per-model result slots (MF_MAX_PARAMS + 2 doubles and the done word)
+    double* h_slab = nullptr;
+    double* d_slab = nullptr;
+    std::vector<int> free_slots;
 };
+
+constexpr int MF_HOST_SLOT_DOUBLES = 32;  // >= MF_MAX_PARAMS + 3, 256-byte slots
+constexpr int MF_HOST_SLOTS = 4096;
 
 // Reference-counted device buffer so that a model can outlive the dataset handle.
 struct mf_devbuf {
+    cudaStream_t stream = nullptr;  // freed in the order of this stream
     double* p = nullptr;
     size_t bytes = 0;
     int refs = 1;
