@@ -5,7 +5,7 @@
 // Notation follows the paper: f = f_sig, mu, sigma = sigma_m, tau = alpha (BASELINE.json
 // calls the slope tau), N1 / N2 the two normalisations of Eq. 2, [m_a, m_b] the mass range.
 //
-// What is NOT the paper's kernel (DESIGN.md "Differences"):
+// What is NOT the paper's kernel (DESIGN.md §6):
 //  * value and all K derivatives are produced in one pass in registers (the paper emits
 //    one kernel per quantity from its differentiated graph);
 //  * the mass mixture is evaluated in ratio form with ONE exponential per event:
@@ -13,6 +13,9 @@
 //        P   = (E/N2) [(1-f) + f R],   ln P = tau m + ln c2 + ln[(1-f) + f R]
 //    instead of Eq. 3's b1 exp(..) + b2 exp(..) (two exponentials); b0, c1, c2 and the
 //    derivatives of ln N1, ln N2 are the buffered parameter-only terms;
+//  * the kernels accumulate model-specific SUMS (mass: the product of the D_i and five moments
+//    of u = R/D, r = 1/D) and one thread per evaluation turns them into -ln L and the gradient
+//    (M::finish); sum_i tau m_i is an event-only constant times tau;
 //  * the eleven angular terms of Listing 4 are merged into nine columns h_0..h_8 with
 //    P = h0 + FL h1 + S3 h2 + S4 h3 + S5 h4 + AFB h5 + S7 h6 + S8 h7 + S9 h8.
 #pragma once
