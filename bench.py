@@ -48,7 +48,7 @@ WORKLOAD = "C1: 1D Gaussian+exponential mass model, N=1e6 fp64 events, K=4, NLL+
 # fp64-pipe thread-instructions per event of the shipped mass kernel's fast path (counted from
 # SASS); never more than the plain two-exponential form's hand count (100).
 MASS_FP64_INSTR_PER_EVENT = 26.0
-POINTS_PER_CALL = 25   # evaluations enqueued per mf_nll_grad_points call (one kernel launch each)
+POINTS_PER_CALL = 250  # evaluations per mf_nll_grad_points call (ONE launch: CTA tile = (point, event chunk))
 NOMINAL_FP64_LANES_PER_SM = 64  # B200: 4 SMSPs x 16 fp64 FMA lanes
 
 
@@ -202,9 +202,9 @@ def run_reference(args) -> None:
 
 def _time_points(torch, models, lam, K, n_calls: int) -> float:
     """us per evaluation: n_calls back-to-back evaluations at lam rotating over `models` (CUDA events)."""
-    out = torch.zeros((POINTS_PER_CALL, K + 2), dtype=torch.float64, device="cuda")
-    lams = np.tile(np.asarray(lam, dtype=np.float64), (POINTS_PER_CALL, 1))
-    per = 1 if len(models) > 1 else POINTS_PER_CALL   # several replicas: a different one every evaluation
+    out = torch.zeros((8, K + 2), dtype=torch.float64, device="cuda")
+    lams = np.tile(np.asarray(lam, dtype=np.float64), (8, 1))
+    per = 1 if len(models) > 1 else 8   # several replicas: a different one every evaluation; < 16 per call = one launch each
 
     def go(n):
         i = 0
@@ -246,18 +246,19 @@ def _other_workloads(torch, mf, ctx, peaks) -> dict:
     del ms, ev
     # C3: 4D, N = 2e6, 12 columns = 96 B/event (192 MB > L2)
     ev = dg.gen_4d(2_000_000, seed=3)
-    m4 = ctx.model_create(mf.MF_MASS_X_ANGULAR, ctx.dataset_upload(ev, dg.MASS_LO, dg.MASS_HI))
-    us = _time_points(torch, [m4], dg.FOURD_TRUTH, 16, 400)
+    m4s = [ctx.model_create(mf.MF_MASS_X_ANGULAR, ctx.dataset_upload(ev, dg.MASS_LO, dg.MASS_HI)) for _ in range(2)]
+    m4 = m4s[0]
+    us = _time_points(torch, m4s, dg.FOURD_TRUTH, 16, 400)   # 2 x 192 MB of columns, alternating
     gbs = 96.0 * 2_000_000 / us / 1e3
     res["C3_4d_2e6"] = {"us_per_eval": us, "events_per_s": 2e6 / (us * 1e-6), "kernel": "nll_grad_kernel<FourDModel>",
                         "roofline": {"bound": "hbm", "achieved": gbs, "peak": hbm, "unit": "GB/s",
                                      "frac": gbs / hbm if hbm else None, "bytes_per_event": 96},
-                        "l2": "192 MB of columns > L2"}
+                        "l2": "2 model replicas x 192 MB of columns, alternating every evaluation"}
     t = time.perf_counter()
     r = m4.fit(dg.FOURD_TRUTH)
     res["C3_4d_2e6"]["fit_s"] = time.perf_counter() - t
     res["C3_4d_2e6"]["fit_calls"] = r.n_calls
-    del m4, ev
+    del m4, m4s, ev
     # C4: 4096 toys x 1e4 events (328 MB > L2), one launch for all toys; then all toys fitted concurrently
     T, n = 4096, 10_000
     toys = dg.gen_mass_toys(T, n, first_seed=0)
@@ -347,8 +348,8 @@ def run_mine(args) -> None:
     pts_c = np.ascontiguousarray(pts)
 
     def run_steps(first: int, count: int):
-        """Steps first .. first+count-1: step i = one NLL+gradient evaluation (one kernel launch) at
-        lambda point i % 1000 on dataset replica (i // 25) % 32, enqueued 25 at a time."""
+        """Steps first .. first+count-1: step i = one NLL+gradient evaluation at lambda point i % 1000 on dataset
+        replica (i // 250) % 32; 250 steps per mf_nll_grad_points call."""
         i, end = first, first + count
         while i < end:
             p = i % N_POINTS
@@ -428,13 +429,13 @@ def run_mine(args) -> None:
     traffic = None
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
-            traffic = json.load(fh).get("nll_grad_kernel<MassModel>")
+            traffic = json.load(fh).get("nll_grad_batch_kernel<MassModel>/points")
     except Exception:
         pass
     roofline = {
         "bound": "alu", "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
         "frac": achieved_tflops / peak_tflops, "traffic": traffic,
-        "kernel": "nll_grad_kernel<MassModel>", "fp64_instr_per_event": MASS_FP64_INSTR_PER_EVENT,
+        "kernel": "nll_grad_batch_kernel<MassModel> (points mode)", "fp64_instr_per_event": MASS_FP64_INSTR_PER_EVENT,
         "peak_how": f"derived: {n_sm} SMs x {NOMINAL_FP64_LANES_PER_SM} fp64 lanes x {sm_max_mhz:.0f} MHz x 2 flop",
         "peak_measured_dfma_chain": 2.0 * measured_rate / 1e12,
         "frac_of_measured_dfma_chain": achieved_tflops / (2.0 * measured_rate / 1e12),
@@ -453,9 +454,11 @@ def run_mine(args) -> None:
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": WORKLOAD, "n_events": N_EVENTS, "n_params": K, "lambda_points": N_POINTS,
-                   "replicas": N_REPLICAS, "l2": "inputs larger than L2: steps rotate over 32 x 8 MB dataset replicas",
-                   "launch": "one nll_grad_kernel<MassModel> launch per step, enqueued 25 steps per mf_nll_grad_points call, "
-                             "programmatic dependent launch between successive kernels"},
+                   "replicas": N_REPLICAS, "points_per_call": POINTS_PER_CALL,
+                   "l2": "inputs larger than L2: calls rotate over 32 x 8 MB dataset replicas, so each call first reads its "
+                         "events from HBM; the 250 evaluations of one call re-read them from L2 by design (8 B/event, ALU bound)",
+                   "launch": "one nll_grad_batch_kernel<MassModel> launch per mf_nll_grad_points call of 250 steps "
+                             "(CTA tile = (lambda point, event chunk))"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
         "other_workloads": others,
     }))

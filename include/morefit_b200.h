@@ -127,10 +127,13 @@ mf_status mf_nll_grad(mf_model* model, const double* lambda, double* nll, double
 mf_status mf_nll_grad_async(mf_model* model, const double* lambda, double* out_dev);
 
 /* n_points evaluations of the same dataset at n_points parameter points (BASELINE.json configs[1]:
- * "repeated NLL+gradient calls at 1,000 random parameter points"), enqueued back to back without a host
- * synchronisation: exactly mf_nll_grad_async called n_points times, the loop being inside the library.
+ * "repeated NLL+gradient calls at 1,000 random parameter points"), enqueued without a host synchronisation.
  *   lambdas  host, [n_points][K].   out_dev  DEVICE, [n_points][K+2], row p = [-ln L, grad, n_bad] at point p.
- * Stops at the first point outside the parameter domain (MF_ERR_PARAM_DOMAIN; earlier points are enqueued). */
+ * Fewer than 16 points: mf_nll_grad_async n_points times (one launch each, pipelined).  Otherwise ONE launch
+ * whose CTA tile is (point, event chunk), the parameter-only constants of every point being derived on the host
+ * and uploaded (the dataset is read from HBM once and re-read from L2 by the other points).
+ * Every point is validated first: MF_ERR_PARAM_DOMAIN (nothing enqueued) if one is outside the domain
+ * (for fewer than 16 points the earlier ones are enqueued). */
 mf_status mf_nll_grad_points(mf_model* model, int64_t n_points, const double* lambdas, double* out_dev);
 
 /* T pseudo-experiments at their own parameter points in ONE launch (BASELINE.json

@@ -9,6 +9,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 #include "mf_internal.h"
 #include "mf_kernels.cuh"
@@ -349,6 +350,7 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
     m->grid = (int)std::max<int64_t>(1, std::min<int64_t>((n_items + kWarps - 1) / kWarps, ctas_per_sm * (int64_t)ctx->sm_count));
     // batch geometry: one CTA per toy up to 32768 events per toy, else split
     m->chunks = (int)std::max<int64_t>(1, std::min<int64_t>((m->n_pad + 32767) / 32768, 64));
+    if (const char* e = std::getenv("MF_BATCH_CHUNKS")) m->chunks = std::max(1, std::atoi(e));  // tuning knob
     MF_CUDA_M(dev_alloc(ctx, &m->partials, sizeof(double) * kRing * m->nacc * m->grid));
     MF_CUDA_M(dev_alloc(ctx, &m->bad_partials, sizeof(unsigned) * kRing * m->grid));
     MF_CUDA_M(dev_alloc(ctx, &m->ticket, sizeof(unsigned) * (kRing + m->n_toys)));
@@ -474,16 +476,78 @@ extern "C" mf_status mf_nll_grad_async(mf_model* m, const double* lambda, double
     return dispatch_single(m, lambda, out_dev);
 }
 
+// Several parameter points on ONE dataset in one launch: the batched kernel with every slot reading toy 0.
+// The parameter-only constants are derived on the host (which also validates every point before anything is
+// enqueued) and uploaded; a CTA is (point, event chunk); chunk sums are combined per point in fixed order.
+template <class M>
+static mf_status launch_points(mf_model* m, int64_t n_points, const double* lambdas, double* out_dev)
+{
+    mf_ctx* ctx = m->ctx;
+    const int K = M::K;
+    std::vector<typename M::Consts> hc((size_t)n_points);
+    for (int64_t p = 0; p < n_points; ++p)
+        if (!host_consts<M>(m, lambdas + p * K, hc[(size_t)p]))
+            return mf_fail(ctx, MF_ERR_PARAM_DOMAIN, "mf_nll_grad_points: lambda " + std::to_string((long long)p) +
+                                                         " is outside the parameter domain");
+    // CTAs: whole waves of the resident capacity, about 64k events per CTA
+    const int64_t slots = (int64_t)M::BATCH_RESIDENT_CTAS * ctx->sm_count;
+    const int64_t waves = std::max<int64_t>(1, (n_points * m->n_pad + slots * 65536 - 1) / (slots * 65536));
+    const int64_t max_chunks = std::max<int64_t>(1, (m->n_pad / kItem + kWarps - 1) / kWarps);
+    const int chunks = (int)std::max<int64_t>(1, std::min<int64_t>(max_chunks, waves * slots / n_points));
+    // scratch from the stream-ordered pool: [consts | ok | partials | bad | ticket]
+    const size_t b_consts = sizeof(typename M::Consts) * n_points, b_ok = sizeof(int) * n_points;
+    const size_t b_part = sizeof(double) * n_points * M::NACC * chunks, b_bad = sizeof(unsigned) * n_points * chunks;
+    const size_t b_ticket = sizeof(unsigned) * n_points;
+    auto up = [](size_t x) { return (x + 255) / 256 * 256; };
+    char* blk = nullptr;
+    MF_CUDA(ctx, dev_alloc(ctx, &blk, up(b_consts) + up(b_ok) + up(b_part) + up(b_bad) + up(b_ticket)));
+    BatchArgs<M> a;
+    for (int i = 0; i < M::NCOL; ++i) a.col[i] = m->col[i];
+    a.toy_stride = 0;
+    a.shared_data = 1;
+    a.n = m->n_events;
+    a.n_items = m->n_pad / kItem;
+    a.chunks = chunks;
+    a.ma = m->ma;
+    a.mb = m->mb;
+    a.sum_m = m->d_sum_m;
+    a.lam = nullptr;
+    a.consts = reinterpret_cast<typename M::Consts*>(blk);
+    a.consts_ok = reinterpret_cast<int*>(blk + up(b_consts));
+    a.partials = reinterpret_cast<double*>(blk + up(b_consts) + up(b_ok));
+    a.bad_partials = reinterpret_cast<unsigned*>(blk + up(b_consts) + up(b_ok) + up(b_part));
+    a.ticket = reinterpret_cast<unsigned*>(blk + up(b_consts) + up(b_ok) + up(b_part) + up(b_bad));
+    a.ids = nullptr;
+    a.out = out_dev;
+    cudaError_t e = cudaMemcpyAsync(a.consts, hc.data(), b_consts, cudaMemcpyHostToDevice, ctx->stream);  // pageable: staged before return
+    if (e == cudaSuccess) e = cudaMemsetAsync(a.consts_ok, 0xFF, b_ok, ctx->stream);                    // non-zero = ok
+    if (e == cudaSuccess) e = cudaMemsetAsync(a.ticket, 0, b_ticket, ctx->stream);
+    if (e == cudaSuccess) e = launch_pdl(nll_grad_batch_kernel<M>, (int)(n_points * chunks), ctx->stream, a);
+    dev_free(ctx, blk);
+    MF_CUDA(ctx, e);
+    ++ctx->launches;
+    return MF_OK;
+}
+
 extern "C" mf_status mf_nll_grad_points(mf_model* m, int64_t n_points, const double* lambdas, double* out_dev)
 {
     if (!m || !lambdas || !out_dev || n_points < 0)
         return mf_fail(m ? m->ctx : nullptr, MF_ERR_ARG, "mf_nll_grad_points: bad argument");
     if (m->n_toys != 1) return mf_fail(m->ctx, MF_ERR_ARG, "mf_nll_grad_points: dataset has n_toys != 1");
-    for (int64_t p = 0; p < n_points; ++p) {
-        const mf_status st = dispatch_single(m, lambdas + p * m->K, out_dev + p * (m->K + 2), n_points > 1);
-        if (st != MF_OK) return st;
+    if (n_points == 0) return MF_OK;
+    if (n_points < 16) {  // few points: back-to-back pipelined single evaluations are faster (measured cross-over ~12)
+        for (int64_t p = 0; p < n_points; ++p) {
+            const mf_status st = dispatch_single(m, lambdas + p * m->K, out_dev + p * (m->K + 2), n_points > 1);
+            if (st != MF_OK) return st;
+        }
+        return MF_OK;
     }
-    return MF_OK;
+    if (n_points > (int64_t)1 << 20) return mf_fail(m->ctx, MF_ERR_ARG, "mf_nll_grad_points: more than 2^20 points per call");
+    switch (m->kind) {
+    case MF_MASS_GAUSS_EXP: return launch_points<MassModel>(m, n_points, lambdas, out_dev);
+    case MF_ANGULAR_KSTMUMU: return launch_points<AngularModel>(m, n_points, lambdas, out_dev);
+    default: return launch_points<FourDModel>(m, n_points, lambdas, out_dev);
+    }
 }
 
 extern "C" mf_status mf_nll_grad(mf_model* m, const double* lambda, double* nll, double* grad)
@@ -522,6 +586,7 @@ static mf_status launch_batch(mf_model* m, int n_active, const double* lam_dev =
     BatchArgs<M> a;
     for (int i = 0; i < M::NCOL; ++i) a.col[i] = m->col[i];
     a.toy_stride = m->n_pad;
+    a.shared_data = 0;
     a.n = m->n_events;
     a.n_items = m->n_pad / kItem;
     a.chunks = m->chunks;

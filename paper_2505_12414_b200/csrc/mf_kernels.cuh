@@ -54,6 +54,7 @@ template <class M>
 struct BatchArgs {
     const double* col[M::NCOL];  // column bases of toy 0; toy t is at + t * toy_stride
     int64_t toy_stride;          // n_pad
+    int shared_data;             // 1: every slot evaluates toy 0 (several parameter points on ONE dataset)
     int64_t n;                   // valid events per toy
     int64_t n_items;             // n_pad / 64 per toy
     int chunks;                  // CTAs per toy
@@ -181,9 +182,11 @@ __device__ __forceinline__ void compute_group(int64_t n, int64_t n_items, int64_
 //  * PREFETCH == D > 0 (one column, ALU bound): a rolling window of D items per thread — the slot of the
 //    item being evaluated is refilled at once with the item D steps ahead, so D 16-byte loads per
 //    thread stay in flight (memory latency x bandwidth needs ~44 KB in flight per SM).
-template <class M>
+// get_c() yields the parameter-only constants; it is called AFTER the first loads have been issued (rolling
+// schedule), so that a kernel which must first fetch them (batched toys) overlaps that with the data latency.
+template <class M, class GetC>
 __device__ __forceinline__ void accumulate(const double* const* col, int64_t n, int64_t n_items, int64_t j0,
-                                           int64_t step, const typename M::Consts& c, double* acc, unsigned& bad)
+                                           int64_t step, GetC get_c, double* acc, unsigned& bad)
 {
     const int lane = threadIdx.x & 31;
     const double t_lane = mf_exp32_lane_entry();
@@ -194,6 +197,7 @@ __device__ __forceinline__ void accumulate(const double* const* col, int64_t n, 
 #pragma unroll
         for (int u = 0; u < D; ++u)
             if (j0 + u * step < n_items) load_item<M>(col, j0 + u * step, lane, buf[u][0], buf[u][1]);
+        decltype(auto) c = get_c();
         constexpr int U = M::ITEMS_PER_ITER;  // items evaluated together: 2U independent events interleaved
         static_assert(D % U == 0, "PREFETCH must be a multiple of ITEMS_PER_ITER");
         const int64_t n_full = n / kItem;  // items 0 .. n_full-1 have 64 valid events
@@ -237,6 +241,7 @@ __device__ __forceinline__ void accumulate(const double* const* col, int64_t n, 
             }
         }
     } else {
+        decltype(auto) c = get_c();
         constexpr int U = M::ITEMS_PER_ITER;
         double A[U][2][M::NCOL], B[U][2][M::NCOL];
         int64_t j = j0;
@@ -374,7 +379,8 @@ __global__ void __launch_bounds__(kBlock, M::RESIDENT_CTAS) nll_grad_kernel(cons
     for (int k = 0; k < NACC; ++k) acc[k] = 0.0;
     unsigned bad = 0;
     const int64_t G = gridDim.x;
-    accumulate<M>(a.col, a.n, a.n_items, blockIdx.x + G * (threadIdx.x >> 5), G * kWarps, a.c, acc, bad);
+    accumulate<M>(a.col, a.n, a.n_items, blockIdx.x + G * (threadIdx.x >> 5), G * kWarps,
+                  [&]() -> const typename M::Consts& { return a.c; }, acc, bad);
 
     if (threadIdx.x == 0)
         while (gen_load(a.gen) < a.need) __nanosleep(64);  // slot still in use by evaluation e - kRing (rare)
@@ -431,8 +437,8 @@ __global__ void __launch_bounds__(kBlock, M::BATCH_RESIDENT_CTAS) nll_grad_batch
 
     pdl_launch_dependents();
     const int slot = blockIdx.x / a.chunks, chunk = blockIdx.x % a.chunks;
-    const int64_t toy = a.ids ? a.ids[slot] : slot;  // ids == NULL: every toy is active
-    if (a.chunks == 1) {
+    const int64_t toy = a.shared_data ? 0 : a.ids ? a.ids[slot] : slot;  // ids == NULL: every toy is active
+    if (a.chunks == 1 && !a.shared_data) {
         // this CTA streams its toy's columns once from HBM: ask for them now (L2 prefetch, 128-byte lines), so
         // that they arrive while the constants are fetched and the first loads of the event loop hit L2
         const int64_t lines = (a.n_items * kItem * (int64_t)sizeof(double) + 127) / 128;
@@ -451,17 +457,7 @@ __global__ void __launch_bounds__(kBlock, M::BATCH_RESIDENT_CTAS) nll_grad_batch
             reinterpret_cast<double*>(&s_c)[threadIdx.x] = reinterpret_cast<const double*>(a.consts + slot)[threadIdx.x];
         if (threadIdx.x == 0) s_ok = a.consts_ok[slot];
     }
-    __syncthreads();
     double* out = a.out + (int64_t)slot * (K + 2);
-    if (!s_ok) {  // outside the parameter domain: +inf / NaN, n_bad = -1
-        pdl_wait();
-        if (chunk == 0 && threadIdx.x <= K + 1)
-            out[threadIdx.x] = threadIdx.x == 0       ? __longlong_as_double(0x7ff0000000000000LL)
-                               : threadIdx.x == K + 1 ? -1.0
-                                                      : __longlong_as_double(0x7ff8000000000000LL);
-        return;
-    }
-    const typename M::Consts c = s_c;
     const double sum_m = a.sum_m ? a.sum_m[toy] : 0.0;
     const double* col[M::NCOL];
 #pragma unroll
@@ -472,7 +468,21 @@ __global__ void __launch_bounds__(kBlock, M::BATCH_RESIDENT_CTAS) nll_grad_batch
     for (int k = 0; k < NACC; ++k) acc[k] = 0.0;
     unsigned bad = 0;
     const int64_t C = a.chunks;
-    accumulate<M>(col, a.n, a.n_items, chunk + C * (threadIdx.x >> 5), C * kWarps, c, acc, bad);
+    // the constants become visible (barrier) only after the first event loads are in flight
+    accumulate<M>(col, a.n, a.n_items, chunk + C * (threadIdx.x >> 5), C * kWarps,
+                  [&]() -> const typename M::Consts& {
+                      __syncthreads();
+                      return s_c;
+                  },
+                  acc, bad);
+    if (!s_ok) {  // outside the parameter domain (the sums above are garbage and unused): +inf / NaN, n_bad = -1
+        if (chunk == 0 && threadIdx.x <= K + 1)
+            out[threadIdx.x] = threadIdx.x == 0       ? __longlong_as_double(0x7ff0000000000000LL)
+                               : threadIdx.x == K + 1 ? -1.0
+                                                      : __longlong_as_double(0x7ff8000000000000LL);
+        return;
+    }
+    const typename M::Consts& c = s_c;
 
     const double s = block_reduce<NACC>(acc, bad, sm, sm_bad, &s_bad_block);
     if (a.chunks == 1) {  // the CTA holds the toy's complete sums: no cross-CTA pass

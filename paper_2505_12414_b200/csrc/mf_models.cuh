@@ -204,7 +204,7 @@ struct MassModel {
     static constexpr int PREFETCH = MF_MASS_PREFETCH;   // rolling window of 16-byte loads in flight per thread (0: double buffer)
     static constexpr int CTAS_PER_SM = MF_MASS_GRID;    // grid of a lone (synchronous) evaluation: CTAs per SM
 #ifndef MF_MASS_BATCH_RESIDENT
-#define MF_MASS_BATCH_RESIDENT 3
+#define MF_MASS_BATCH_RESIDENT 2
 #endif
     static constexpr int BATCH_RESIDENT_CTAS = MF_MASS_BATCH_RESIDENT;  // the batched kernel: more, smaller-budget CTAs
     static constexpr int RESIDENT_CTAS = MF_MASS_RESIDENT;  // register budget: CTAs of the next evaluation co-reside under PDL
