@@ -392,16 +392,16 @@ extern "C" int64_t mf_model_n_toys(const mf_model* m) { return m ? m->n_toys : 0
 // Launch with programmatic stream serialisation: the kernel may begin while its predecessor on the
 // stream (if that is one of ours) is still in its tail; see pdl_wait() in mf_kernels.cuh.
 template <class Args>
-static cudaError_t launch_pdl(void (*kernel)(const Args), int grid, cudaStream_t stream, const Args& a)
+static cudaError_t launch_pdl(void (*kernel)(const Args), int grid, cudaStream_t stream, const Args& a, int block = kBlock)
 {
     static const bool no_pdl = std::getenv("MF_NO_PDL") != nullptr;  // ablation switch: plain stream order
     if (no_pdl) {
-        kernel<<<grid, kBlock, 0, stream>>>(a);
+        kernel<<<grid, block, 0, stream>>>(a);
         return cudaGetLastError();
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)grid);
-    cfg.blockDim = dim3(kBlock);
+    cfg.blockDim = dim3((unsigned)block);
     cfg.dynamicSmemBytes = 0;
     cfg.stream = stream;
     cudaLaunchAttribute attr[1];
@@ -492,7 +492,7 @@ static mf_status launch_points(mf_model* m, int64_t n_points, const double* lamb
     // CTAs: whole waves of the resident capacity, about 64k events per CTA
     const int64_t slots = (int64_t)M::BATCH_RESIDENT_CTAS * ctx->sm_count;
     const int64_t waves = std::max<int64_t>(1, (n_points * m->n_pad + slots * 65536 - 1) / (slots * 65536));
-    const int64_t max_chunks = std::max<int64_t>(1, (m->n_pad / kItem + kWarps - 1) / kWarps);
+    const int64_t max_chunks = std::max<int64_t>(1, (m->n_pad / kItem + M::BATCH_BLOCK / 32 - 1) / (M::BATCH_BLOCK / 32));
     const int chunks = (int)std::max<int64_t>(1, std::min<int64_t>(max_chunks, waves * slots / n_points));
     // scratch from the stream-ordered pool: [consts | ok | partials | bad | ticket]
     const size_t b_consts = sizeof(typename M::Consts) * n_points, b_ok = sizeof(int) * n_points;
@@ -522,7 +522,7 @@ static mf_status launch_points(mf_model* m, int64_t n_points, const double* lamb
     cudaError_t e = cudaMemcpyAsync(a.consts, hc.data(), b_consts, cudaMemcpyHostToDevice, ctx->stream);  // pageable: staged before return
     if (e == cudaSuccess) e = cudaMemsetAsync(a.consts_ok, 0xFF, b_ok, ctx->stream);                    // non-zero = ok
     if (e == cudaSuccess) e = cudaMemsetAsync(a.ticket, 0, b_ticket, ctx->stream);
-    if (e == cudaSuccess) e = launch_pdl(nll_grad_batch_kernel<M>, (int)(n_points * chunks), ctx->stream, a);
+    if (e == cudaSuccess) e = launch_pdl(nll_grad_batch_kernel<M>, (int)(n_points * chunks), ctx->stream, a, M::BATCH_BLOCK);
     dev_free(ctx, blk);
     MF_CUDA(ctx, e);
     ++ctx->launches;
@@ -603,7 +603,7 @@ static mf_status launch_batch(mf_model* m, int n_active, const double* lam_dev =
     a.out = out_dev ? out_dev : m->d_bout;
     batch_consts_kernel<M><<<(n_active + 127) / 128, 128, 0, ctx->stream>>>(a, n_active);
     MF_CUDA(ctx, cudaGetLastError());
-    MF_CUDA(ctx, launch_pdl(nll_grad_batch_kernel<M>, n_active * m->chunks, ctx->stream, a));
+    MF_CUDA(ctx, launch_pdl(nll_grad_batch_kernel<M>, n_active * m->chunks, ctx->stream, a, M::BATCH_BLOCK));
     ctx->launches += 2;
     return MF_OK;
 }

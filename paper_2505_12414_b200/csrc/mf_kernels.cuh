@@ -220,10 +220,20 @@ __device__ __forceinline__ void accumulate(const double* const* col, int64_t n, 
                         if (jn < n_items) load_item<M>(col, jn, lane, buf[u + v][0], buf[u + v][1]);
                     }
                     if (ju + (U - 1) * step < n_full) {
+                        if constexpr (M::NCOL == 1) {  // one column: the model evaluates the 2U events together
+                            double xs[2 * U];
 #pragma unroll
-                        for (int v = 0; v < U; ++v) {
-                            M::template event<false>(x[v][0], c, acc, lp, bad, true, t_lane);
-                            M::template event<false>(x[v][1], c, acc, lp, bad, true, t_lane);
+                            for (int v = 0; v < U; ++v) {
+                                xs[2 * v] = x[v][0][0];
+                                xs[2 * v + 1] = x[v][1][0];
+                            }
+                            M::template events<2 * U>(xs, c, acc, lp, bad, t_lane);
+                        } else {
+#pragma unroll
+                            for (int v = 0; v < U; ++v) {
+                                M::template event<false>(x[v][0], c, acc, lp, bad, true, t_lane);
+                                M::template event<false>(x[v][1], c, acc, lp, bad, true, t_lane);
+                            }
                         }
                     } else {
 #pragma unroll
@@ -263,7 +273,7 @@ __device__ __forceinline__ void accumulate(const double* const* col, int64_t n, 
 
 // After the call threads 0..NACC-1 hold the block sum of quantity threadIdx.x, thread NACC the
 // block's bad-event count (in *bad_out).
-template <int NACC>
+template <int NACC, int WARPS = kWarps>
 __device__ __forceinline__ double block_reduce(double* acc, unsigned bad, double (*sm)[NACC], unsigned* sm_bad,
                                                unsigned* bad_out)
 {
@@ -285,11 +295,11 @@ __device__ __forceinline__ double block_reduce(double* acc, unsigned bad, double
     double s = 0.0;
     if (threadIdx.x < NACC) {
 #pragma unroll
-        for (int i = 0; i < kWarps; ++i) s += sm[i][threadIdx.x];
+        for (int i = 0; i < WARPS; ++i) s += sm[i][threadIdx.x];
     } else if (threadIdx.x == NACC) {
         unsigned b = 0;
 #pragma unroll
-        for (int i = 0; i < kWarps; ++i) b += sm_bad[i];
+        for (int i = 0; i < WARPS; ++i) b += sm_bad[i];
         *bad_out = b;
     }
     return s;
@@ -301,7 +311,7 @@ __device__ __forceinline__ double block_reduce(double* acc, unsigned bad, double
 // ...; partial i of quantity k is at p[k * stride_k + i].  Thread 0 then turns the NACC sums into
 // out[0] = -ln L, out[1..K] = gradient, out[K+1] = n_bad (+inf / NaN if n_bad), after waiting for the
 // previous kernel on the stream (outputs land in stream order).
-template <class M>
+template <class M, int WARPS = kWarps>
 __device__ __forceinline__ void final_combine(const double* p, int64_t stride_k, int count, const unsigned* badp,
                                               const typename M::Consts& c, double n, double sum_m, double* s_sum,
                                               double* out, unsigned long long* done_flag = nullptr,
@@ -314,7 +324,7 @@ __device__ __forceinline__ void final_combine(const double* p, int64_t stride_k,
         for (int i = lane; i < count; i += 32) nb += __ldcg(badp + i);
         nb = __reduce_add_sync(0xffffffffu, nb);
     }
-    for (int k = w; k < NACC; k += kWarps) {
+    for (int k = w; k < NACC; k += WARPS) {
         const double* pk = p + k * stride_k;
         double s = 0.0, cc = 0.0;  // Kahan: true sum ~ s - cc
         for (int i0 = lane; i0 < count; i0 += 32 * kFinalBatch) {
@@ -423,10 +433,13 @@ __global__ void __launch_bounds__(128) batch_consts_kernel(const __grid_constant
 // CTA <-> (toy, event chunk)
 
 template <class M>
-__global__ void __launch_bounds__(kBlock, M::BATCH_RESIDENT_CTAS) nll_grad_batch_kernel(const __grid_constant__ BatchArgs<M> a)
+__global__ void __launch_bounds__(M::BATCH_BLOCK, M::BATCH_RESIDENT_CTAS)
+    nll_grad_batch_kernel(const __grid_constant__ BatchArgs<M> a)
 {
     constexpr int NACC = M::NACC;
     constexpr int K = M::K;
+    constexpr int kBlock = M::BATCH_BLOCK, kWarps = kBlock / 32;  // this kernel's own CTA size
+    static_assert(kBlock >= 64 && NACC + 1 <= kBlock, "CTA too small for the reduction");
     __shared__ double sm[kWarps][NACC];
     __shared__ double s_sum[NACC];
     __shared__ unsigned sm_bad[kWarps];
@@ -484,7 +497,7 @@ __global__ void __launch_bounds__(kBlock, M::BATCH_RESIDENT_CTAS) nll_grad_batch
     }
     const typename M::Consts& c = s_c;
 
-    const double s = block_reduce<NACC>(acc, bad, sm, sm_bad, &s_bad_block);
+    const double s = block_reduce<NACC, kWarps>(acc, bad, sm, sm_bad, &s_bad_block);
     if (a.chunks == 1) {  // the CTA holds the toy's complete sums: no cross-CTA pass
         if (threadIdx.x < NACC) s_sum[threadIdx.x] = s;
         __syncthreads();
@@ -511,7 +524,7 @@ __global__ void __launch_bounds__(kBlock, M::BATCH_RESIDENT_CTAS) nll_grad_batch
     if (threadIdx.x == 0) s_last = (ticket_take(a.ticket + slot) == (unsigned)a.chunks - 1);
     __syncthreads();
     if (s_last) {
-        final_combine<M>(part, C, (int)C, badp, c, (double)a.n, sum_m, s_sum, out);
+        final_combine<M, kWarps>(part, C, (int)C, badp, c, (double)a.n, sum_m, s_sum, out);
         if (threadIdx.x == 0) a.ticket[slot] = 0u;
     }
 }

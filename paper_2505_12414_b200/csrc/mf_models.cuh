@@ -204,8 +204,12 @@ struct MassModel {
     static constexpr int PREFETCH = MF_MASS_PREFETCH;   // rolling window of 16-byte loads in flight per thread (0: double buffer)
     static constexpr int CTAS_PER_SM = MF_MASS_GRID;    // grid of a lone (synchronous) evaluation: CTAs per SM
 #ifndef MF_MASS_BATCH_RESIDENT
-#define MF_MASS_BATCH_RESIDENT 2
+#define MF_MASS_BATCH_RESIDENT 4
 #endif
+#ifndef MF_MASS_BATCH_BLOCK
+#define MF_MASS_BATCH_BLOCK 128
+#endif
+    static constexpr int BATCH_BLOCK = MF_MASS_BATCH_BLOCK;  // threads per CTA of the batched kernel
     static constexpr int BATCH_RESIDENT_CTAS = MF_MASS_BATCH_RESIDENT;  // the batched kernel: more, smaller-budget CTAs
     static constexpr int RESIDENT_CTAS = MF_MASS_RESIDENT;  // register budget: CTAs of the next evaluation co-reside under PDL
     using Consts = MassConsts;
@@ -233,6 +237,38 @@ struct MassModel {
         }
     }
 
+    // E full events at once (the fast path of the event loop), written operation by operation across the E
+    // events so that the instruction stream is interleaved as issued and constants are shared operands.
+    template <int E>
+    static MF_D void events(const double (&m)[E], const Consts& c, double* acc, LogProd& lp, unsigned& bad, double t_lane)
+    {
+        double d[E], t[E], arg[E], R[E], D[E], r[E], u[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) d[e] = m[e] - c.mu;
+#pragma unroll
+        for (int e = 0; e < E; ++e) arg[e] = fma(-c.tau, m[e], c.lnk);
+#pragma unroll
+        for (int e = 0; e < E; ++e) t[e] = d[e] * d[e];
+#pragma unroll
+        for (int e = 0; e < E; ++e) arg[e] = fma(c.nb0, t[e], arg[e]);
+        mf_exp32_v<E>(arg, t_lane, R);
+#pragma unroll
+        for (int e = 0; e < E; ++e) D[e] = fma(c.f, R[e], c.omf);
+#pragma unroll
+        for (int e = 0; e < E; ++e) r[e] = mf_rcp(D[e]);
+#pragma unroll
+        for (int e = 0; e < E; ++e) u[e] = R[e] * r[e];
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            lp.mul(D[e], bad);
+            acc[1] += u[e];
+            acc[2] += r[e];
+            acc[3] = fma(u[e], d[e], acc[3]);
+            acc[4] = fma(u[e], t[e], acc[4]);
+            acc[5] = fma(r[e], d[e], acc[5]);
+        }
+    }
+
     // ln P = tau m - ln N2 + ln D
     // d ln P/df = u - r;  d/dmu = f u (d/sigma^2 - kmu);  d/dsigma = f u (d^2/sigma^3 - ksig);
     // d/dtau = (1-f) r (m - m_a - ktau) = (1-f) r (d + mu - m_a - ktau)
@@ -255,6 +291,7 @@ struct AngularModel {
     static constexpr int CTAS_PER_SM = 2;
     static constexpr int RESIDENT_CTAS = 2;
     static constexpr int BATCH_RESIDENT_CTAS = 2;
+    static constexpr int BATCH_BLOCK = 256;
     using Consts = AngularConsts;
 
     template <bool PRED>
@@ -287,6 +324,7 @@ struct FourDModel {
     static constexpr int PREFETCH = 0;
     static constexpr int RESIDENT_CTAS = 1;
     static constexpr int BATCH_RESIDENT_CTAS = 1;
+    static constexpr int BATCH_BLOCK = 256;
     static constexpr int CTAS_PER_SM = 1;  // 17 sums + two 12-column register buffers: needs > 128 registers
     using Consts = FourDConsts;
 
