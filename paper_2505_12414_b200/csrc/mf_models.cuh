@@ -189,7 +189,7 @@ struct MassModel {
                                     // sum u, sum r, sum u d, sum u d^2, sum r d
     // tuning knobs (defaults = the measured best on B200)
 #ifndef MF_MASS_U
-#define MF_MASS_U 2
+#define MF_MASS_U 4
 #endif
 #ifndef MF_MASS_PREFETCH
 #define MF_MASS_PREFETCH 4
