@@ -48,7 +48,7 @@ WORKLOAD = "C1: 1D Gaussian+exponential mass model, N=1e6 fp64 events, K=4, NLL+
 # fp64-pipe thread-instructions per event of the shipped mass kernel's fast path (counted from
 # SASS); never more than the plain two-exponential form's hand count (100).
 MASS_FP64_INSTR_PER_EVENT = 26.0
-POINTS_PER_CALL = 250  # evaluations per mf_nll_grad_points call (ONE launch: CTA tile = (point, event chunk))
+POINTS_PER_CALL = 500  # evaluations per mf_nll_grad_points call (ONE launch: CTA tile = (point, event chunk))
 NOMINAL_FP64_LANES_PER_SM = 64  # B200: 4 SMSPs x 16 fp64 FMA lanes
 
 
@@ -349,7 +349,7 @@ def run_mine(args) -> None:
 
     def run_steps(first: int, count: int):
         """Steps first .. first+count-1: step i = one NLL+gradient evaluation at lambda point i % 1000 on dataset
-        replica (i // 250) % 32; 250 steps per mf_nll_grad_points call."""
+        replica (i // 500) % 32; 500 steps per mf_nll_grad_points call."""
         i, end = first, first + count
         while i < end:
             p = i % N_POINTS
@@ -456,8 +456,8 @@ def run_mine(args) -> None:
         "config": {"workload": WORKLOAD, "n_events": N_EVENTS, "n_params": K, "lambda_points": N_POINTS,
                    "replicas": N_REPLICAS, "points_per_call": POINTS_PER_CALL,
                    "l2": "inputs larger than L2: calls rotate over 32 x 8 MB dataset replicas, so each call first reads its "
-                         "events from HBM; the 250 evaluations of one call re-read them from L2 by design (8 B/event, ALU bound)",
-                   "launch": "one nll_grad_batch_kernel<MassModel> launch per mf_nll_grad_points call of 250 steps "
+                         "events from HBM; the 500 evaluations of one call re-read them from L2 by design (8 B/event, ALU bound)",
+                   "launch": "one nll_grad_batch_kernel<MassModel> launch per mf_nll_grad_points call of 500 steps "
                              "(CTA tile = (lambda point, event chunk))"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
         "other_workloads": others,

@@ -491,7 +491,8 @@ static mf_status launch_points(mf_model* m, int64_t n_points, const double* lamb
                                                          " is outside the parameter domain");
     // CTAs: whole waves of the resident capacity, about 64k events per CTA
     const int64_t slots = (int64_t)M::BATCH_RESIDENT_CTAS * ctx->sm_count;
-    const int64_t waves = std::max<int64_t>(1, (n_points * m->n_pad + slots * 65536 - 1) / (slots * 65536));
+    static const int64_t per_cta = std::getenv("MF_POINTS_CTA_EVENTS") ? std::atoll(std::getenv("MF_POINTS_CTA_EVENTS")) : 65536;  // tuning knob
+    const int64_t waves = std::max<int64_t>(1, (n_points * m->n_pad + slots * per_cta - 1) / (slots * per_cta));
     const int64_t max_chunks = std::max<int64_t>(1, (m->n_pad / kItem + M::BATCH_BLOCK / 32 - 1) / (M::BATCH_BLOCK / 32));
     const int chunks = (int)std::max<int64_t>(1, std::min<int64_t>(max_chunks, waves * slots / n_points));
     // scratch from the stream-ordered pool: [consts | ok | partials | bad | ticket]
