@@ -1,0 +1,120 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (500 lambda points per
+mf_nll_grad_points call for C1, single evaluations for C2/C3, one batched launch over 4096 toys for C4).
+The oracle (OpenMP over event chunks) is called on a SAMPLE of the outputs: it needs ~0.1-3 s per evaluation at
+these sizes.  Tolerances are north_star's, as in test_gpu_parity.py."""
+import math
+
+import numpy as np
+import pytest
+
+import mf_datagen as dg
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+NLL_RTOL = 1e-11
+GRAD_TOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def mf():
+    import paper_2505_12414_b200 as mf
+    return mf
+
+
+@pytest.fixture(scope="module")
+def ctx(mf):
+    c = mf.Context(0)
+    yield c
+    c.close()
+
+
+def check(nll, grad, o_nll, o_grad, what):
+    assert abs(nll - o_nll) <= NLL_RTOL * abs(o_nll), f"{what}: nll {nll!r} vs oracle {o_nll!r}"
+    err = np.abs(grad - o_grad)
+    tol = GRAD_TOL * (1.0 + np.abs(o_grad))
+    assert np.all(err <= tol), f"{what}: grad err {err} tol {tol}"
+
+
+def test_c1_points_mode_full_size(mf, ctx):
+    """C1: N = 1e6, the 1,000 seeded lambda points, evaluated 500 per call exactly as bench.py does."""
+    import torch
+    n = 1_000_000
+    m = dg.gen_mass(n, seed=1)
+    model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(m, dg.MASS_LO, dg.MASS_HI))
+    pts = dg.gen_lambda_points(1000, 1001, dg.MASS_TRUTH, 3 * dg.mass_sigma_stat(n))
+    out = torch.full((1000, 6), float("nan"), dtype=torch.float64, device="cuda")
+    for c in (0, 500):
+        model.nll_grad_points(pts[c:c + 500], out[c].data_ptr())
+    torch.cuda.synchronize()
+    res = out.cpu().numpy()
+    assert np.all(np.isfinite(res)) and np.all(res[:, 5] == 0)
+    for p in (0, 137, 499, 500, 999):      # sampled outputs, both calls, first and last slots
+        o_nll, o_g, _ = oracle.nll_grad(oracle.MASS, m, pts[p], dg.MASS_LO, dg.MASS_HI, nthreads=oracle.max_threads())
+        check(res[p, 0], res[p, 1:5], o_nll, o_g, f"C1 point {p}")
+    # properties that hold for every point: the lone-call kernel agrees with the points-mode kernel
+    for p in (3, 750):
+        nll, g = model.nll_grad(pts[p])
+        assert abs(nll - res[p, 0]) <= 1e-12 * abs(nll)
+        assert np.all(np.abs(g - res[p, 1:5]) <= 1e-10 * (1 + np.abs(g)))
+
+
+def test_c1_full_fit(mf, ctx):
+    """C1's full fit from the BASELINE start point; the GPU fit must satisfy the oracle's gradient = 0 condition."""
+    n = 1_000_000
+    m = dg.gen_mass(n, seed=1)
+    model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(m, dg.MASS_LO, dg.MASS_HI))
+    r = model.fit(dg.MASS_START)
+    assert r.converged
+    o_nll, o_g, _ = oracle.nll_grad(oracle.MASS, m, r.lam, dg.MASS_LO, dg.MASS_HI, nthreads=oracle.max_threads())
+    assert abs(r.nll - o_nll) <= NLL_RTOL * abs(o_nll)
+    # a Newton step from the fitted point, with the oracle's gradient and the fit's covariance, is < 1e-6 sigma
+    step = r.cov @ o_g
+    assert np.max(np.abs(step) / r.sigma) < 1e-6, (step, r.sigma)
+    pull = (r.lam - np.array(dg.MASS_TRUTH)) / r.sigma
+    assert np.all(np.abs(pull) < 5)
+
+
+def test_c2_full_size(mf, ctx):
+    ev = dg.gen_angular(1_000_000, seed=2)
+    model = ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ctx.dataset_upload(ev))
+    for lam in (dg.ANG_TRUTH, (0.55, 0.03, -0.1, -0.25, 0.02, 0.04, -0.05, 0.03)):
+        nll, g = model.nll_grad(lam)
+        o_nll, o_g, _ = oracle.nll_grad(oracle.ANGULAR, ev, lam, nthreads=oracle.max_threads())
+        check(nll, g, o_nll, o_g, "C2")
+
+
+def test_c3_full_size(mf, ctx):
+    ev = dg.gen_4d(2_000_000, seed=3)
+    model = ctx.model_create(mf.MF_MASS_X_ANGULAR, ctx.dataset_upload(ev, dg.MASS_LO, dg.MASS_HI))
+    nll, g = model.nll_grad(dg.FOURD_TRUTH)
+    o_nll, o_g, _ = oracle.nll_grad(oracle.FOURD, ev, dg.FOURD_TRUTH, dg.MASS_LO, dg.MASS_HI, nthreads=oracle.max_threads())
+    check(nll, g, o_nll, o_g, "C3")
+
+
+def test_c4_full_size(mf, ctx):
+    """C4: 4096 toys x 1e4 events in one launch, every toy at its own lambda_t; sampled toys against the oracle,
+    every toy against the invariants; then all toys fitted concurrently and the pulls checked."""
+    T, n = 4096, 10_000
+    toys = dg.gen_mass_toys(T, n, first_seed=0)
+    model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(toys, dg.MASS_LO, dg.MASS_HI, n_toys=T))
+    lams = dg.gen_lambda_points(T, 4242, dg.MASS_TRUTH, 3 * dg.mass_sigma_stat(n))
+    nll, g = model.nll_grad_batch(lams)
+    assert np.all(np.isfinite(nll)) and np.all(np.isfinite(g))
+    for t in (0, 1, 777, 2048, 4095):
+        o_nll, o_g, _ = oracle.nll_grad(oracle.MASS, toys[t], lams[t], dg.MASS_LO, dg.MASS_HI)
+        check(nll[t], g[t], o_nll, o_g, f"C4 toy {t}")
+    # a 1-toy model of the same events gives the same numbers (same kernel arithmetic, different tiling)
+    one = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(toys[123], dg.MASS_LO, dg.MASS_HI))
+    n1, g1 = one.nll_grad(lams[123])
+    assert abs(n1 - nll[123]) <= 1e-12 * abs(n1) and np.all(np.abs(g1 - g[123]) <= 1e-10 * (1 + np.abs(g1)))
+    res = model.fit_batch(np.array(dg.MASS_TRUTH))
+    assert sum(r.converged for r in res) == T
+    pulls = np.array([(r.lam - np.array(dg.MASS_TRUTH)) / r.sigma for r in res])
+    # mean 0 +- 1/sqrt(T) = 0.016 (plus O(1/N) bias), width 1 +- 0.011
+    assert np.all(np.abs(pulls.mean(0)) < 0.08), pulls.mean(0)
+    assert np.all(np.abs(pulls.std(0) - 1.0) < 0.05), pulls.std(0)
+    # sampled toys: the batched fit agrees with the oracle's own fit to 1e-6 sigma
+    for t in (5, 3000):
+        o = oracle.fit(oracle.MASS, toys[t], dg.MASS_TRUTH, lo=dg.MASS_LO, hi=dg.MASS_HI)
+        assert np.max(np.abs(res[t].lam - o.lam) / o.sigma) < 1e-6
