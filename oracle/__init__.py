@@ -56,6 +56,10 @@ def _load():
         lib.mfo_pdf.restype = ctypes.c_int
         lib.mfo_pdf.argtypes = [ctypes.c_int, ctypes.c_int64, dpp, dp, ctypes.c_double,
                                 ctypes.c_double, dp, dp]
+        lib.mfo_nll_grad_hess.restype = ctypes.c_int64
+        lib.mfo_nll_grad_hess.argtypes = [ctypes.c_int, ctypes.c_int64, dpp, dp, ctypes.c_double, ctypes.c_double, dp, dp, dp]
+        lib.mfo_mass_hess_points.restype = ctypes.c_int
+        lib.mfo_mass_hess_points.argtypes = [ctypes.c_int64, dp, dp, ctypes.c_double, ctypes.c_double, dp, dp, dp]
         lib.mfo_mass_norms.restype = None
         lib.mfo_mass_norms.argtypes = [dp, ctypes.c_double, ctypes.c_double, dp]
         lib.mfo_angular_terms.restype = None
@@ -116,6 +120,36 @@ def nll_grad(kind: int, events, lam, lo: float = 0.0, hi: float = 0.0, nthreads:
     if nbad < 0:
         raise ValueError("bad argument")
     return float(nll.value), (grad if want_grad else None), int(nbad)
+
+
+def nll_grad_hess(kind: int, events, lam, lo: float = 0.0, hi: float = 0.0):
+    """(-ln L, gradient [K], Hessian [K][K], n_bad) for the mass and angular kinds (analytic second derivatives,
+    PAPER.md:39, 53)."""
+    lib = _load()
+    cols, n = _columns(kind, events)
+    lam = np.ascontiguousarray(lam, dtype=np.float64)
+    if not check_domain(kind, lam):
+        raise ValueError("parameter outside its domain")
+    K = NPARAMS[kind]
+    nll = ctypes.c_double(0.0)
+    grad = np.zeros(K, dtype=np.float64)
+    hess = np.zeros((K, K), dtype=np.float64)
+    nbad = lib.mfo_nll_grad_hess(kind, n, _colptrs(cols), _dptr(lam), lo, hi, ctypes.byref(nll), _dptr(grad), _dptr(hess))
+    if nbad < 0:
+        raise ValueError("bad argument (no analytic Hessian for this kind)")
+    return float(nll.value), grad, hess, int(nbad)
+
+
+def mass_hess_points(m, lam, lo: float, hi: float):
+    """P [n], d ln P/d lambda [n][4] and the packed Hessian of ln P [n][10] (ff, fm, fs, ft, mm, ms, mt, ss, st, tt)."""
+    lib = _load()
+    m = np.ascontiguousarray(m, dtype=np.float64)
+    lam = np.ascontiguousarray(lam, dtype=np.float64)
+    P = np.empty(m.size)
+    g = np.empty((m.size, 4))
+    h = np.empty((m.size, 10))
+    lib.mfo_mass_hess_points(m.size, _dptr(m), _dptr(lam), lo, hi, _dptr(P), _dptr(g), _dptr(h))
+    return P, g, h
 
 
 def pdf(kind: int, events, lam, lo: float = 0.0, hi: float = 0.0, want_grad: bool = True):

@@ -34,6 +34,8 @@
  * Pins (tests/test_oracle_*.py): unit integral by quadrature, positivity, score identity,
  * finite differences, scipy truncnorm/truncexpon, Gaussian closed-form MLE, the printed
  * constants of Listing 4, closed-form angular marginals, hand-evaluated points of Eq. 4.
+ * The analytic Hessian at the end of the file (mass and angular kinds) has its own pins
+ * (tests/test_oracle_hessian.py): finite differences of the pinned gradient and the information identity.
  */
 #include <math.h>
 #include <stddef.h>
@@ -328,4 +330,130 @@ int mfo_max_threads(void)
 #else
     return 1;
 #endif
+}
+
+/* ================================================================================================
+ * Second derivatives (analytic Hessian by symbolic second
+ * differentiation of ln P).  Written through the derivatives of P itself,
+ *     d2 ln P / da db = P_ab / P - P_a P_b / P^2,
+ * with P = f s(m; mu, sigma) + (1 - f) b(m; tau), s = G/N1, b = e^{tau m}/N2.
+ * Pins (tests/test_oracle_hessian.py): Richardson central differences of mfo_nll_grad's gradient, and the
+ * information identity  int P (l_ab + l_a l_b) dm = 0  by quadrature for all ten (a, b).
+ * ================================================================================================ */
+
+/* d^2 ln N2 / d tau^2 = w^2 h'(tau w), h(u) = 1/(1 - e^-u) - 1/u, h'(u) = 1/u^2 - 1/(4 sinh^2(u/2)) */
+static double d2lognorm_exp_dtau2(double tau, double a, double b)
+{
+    const long double w = (long double)b - (long double)a;
+    const long double u = (long double)tau * w;
+    long double hp;
+    if (fabsl(u) < 1e-2L) {
+        const long double u2 = u * u;
+        hp = 1.0L / 12.0L + u2 * (-1.0L / 240.0L + u2 * (1.0L / 6048.0L + u2 * (-1.0L / 172800.0L)));
+    } else {
+        const long double sh = sinhl(0.5L * u);
+        hp = 1.0L / (u * u) - 1.0L / (4.0L * sh * sh);
+    }
+    return (double)(w * w * hp);
+}
+
+/* Hessian of ln P for one mass event, h[10] in the order ff, fm, fs, ft, mm, ms, mt, ss, st, tt
+ * (m = mu, s = sigma, t = tau); g[4] = gradient of ln P.  Returns P. */
+static double mass_event_hess(double m, const double *lam, double a, double b, double *g, double *h)
+{
+    const double f = lam[0], mu = lam[1], sigma = lam[2], tau = lam[3];
+    const double s2 = sigma * sigma, s3 = s2 * sigma, s4 = s2 * s2;
+    const double d = m - mu;
+    const double N1 = norm_gauss(mu, sigma, a, b);
+    const double ga = gauss_density(a, mu, sigma), gb = gauss_density(b, mu, sigma);
+    /* derivatives of N1: dg(x)/dmu = g (x-mu)/sigma^2, dg(x)/dsigma = g ((x-mu)^2/sigma^3 - 1/sigma) */
+    const double da = a - mu, db = b - mu;
+    const double N1_m = ga - gb;
+    const double N1_s = (da * ga - db * gb) / sigma;
+    const double ga_s = ga * (da * da / s3 - 1.0 / sigma), gb_s = gb * (db * db / s3 - 1.0 / sigma);
+    const double N1_mm = ga * da / s2 - gb * db / s2;
+    const double N1_ms = ga_s - gb_s;
+    const double N1_ss = (da * ga_s - db * gb_s) / sigma - (da * ga - db * gb) / s2;
+    /* s = G/N1 and its logarithmic derivatives */
+    const double s = gauss_density(m, mu, sigma) / N1;
+    const double al_m = d / s2 - N1_m / N1;
+    const double al_s = d * d / s3 - 1.0 / sigma - N1_s / N1;
+    const double al_mm = -1.0 / s2 - (N1_mm / N1 - (N1_m / N1) * (N1_m / N1));
+    const double al_ms = -2.0 * d / s3 - (N1_ms / N1 - (N1_m / N1) * (N1_s / N1));
+    const double al_ss = -3.0 * d * d / s4 + 1.0 / s2 - (N1_ss / N1 - (N1_s / N1) * (N1_s / N1));
+    const double s_m = s * al_m, s_s = s * al_s;
+    const double s_mm = s * (al_m * al_m + al_mm), s_ms = s * (al_m * al_s + al_ms), s_ss = s * (al_s * al_s + al_ss);
+    /* b = E/N2 */
+    const double bb = exp(tau * m) / norm_exp(tau, a, b);
+    const double be = m - dlognorm_exp_dtau(tau, a, b);
+    const double b_t = bb * be;
+    const double b_tt = bb * (be * be - d2lognorm_exp_dtau2(tau, a, b));
+    const double P = f * s + (1.0 - f) * bb;
+    const double Pf = s - bb, Pm = f * s_m, Ps = f * s_s, Pt = (1.0 - f) * b_t;
+    const double P1[4] = {Pf, Pm, Ps, Pt};
+    /*                  ff   fm   fs    ft     mm        ms        mt   ss        st   tt */
+    const double P2[10] = {0.0, s_m, s_s, -b_t, f * s_mm, f * s_ms, 0.0, f * s_ss, 0.0, (1.0 - f) * b_tt};
+    if (g) for (int k = 0; k < 4; ++k) g[k] = P1[k] / P;
+    int q = 0;
+    for (int i = 0; i < 4; ++i)
+        for (int j = i; j < 4; ++j, ++q) h[q] = P2[q] / P - (P1[i] / P) * (P1[j] / P);
+    return P;
+}
+
+/* exposed for the quadrature pins: P, gradient and packed Hessian of ln P at mass values m[0..n-1] */
+int mfo_mass_hess_points(int64_t n, const double *m, const double *lam, double lo, double hi, double *P, double *g /*[n][4]*/,
+                         double *h /*[n][10]*/)
+{
+    for (int64_t i = 0; i < n; ++i) P[i] = mass_event_hess(m[i], lam, lo, hi, g + 4 * i, h + 10 * i);
+    return 0;
+}
+
+/*
+ * -ln L, its gradient and its Hessian (row-major K x K, symmetric) over n events, for the mass (K = 4) and
+ * angular (K = 8) kinds.  Angular: P = A is linear in its coefficients, so d2 ln P / da db = -A_a A_b / A^2.
+ * Sums in long double, single pass in event order.  Returns the number of events with P <= 0 (then nll = +inf,
+ * everything else NaN), -1 on a bad argument (including the 4D kind, for which no analytic Hessian is defined here).
+ */
+int64_t mfo_nll_grad_hess(int kind, int64_t n, const double *const *cols, const double *lam, double lo, double hi,
+                          double *nll, double *grad, double *hess)
+{
+    if (!(kind == MFO_MASS || kind == MFO_ANGULAR) || n < 0) return -1;
+    const int K = mfo_nparams(kind);
+    long double s0 = 0.0L, sg[8], sh[64];
+    for (int i = 0; i < 8; ++i) sg[i] = 0.0L;
+    for (int i = 0; i < 64; ++i) sh[i] = 0.0L;
+    int64_t bad = 0;
+    for (int64_t e = 0; e < n; ++e) {
+        double g[8], P;
+        if (kind == MFO_MASS) {
+            double h[10];
+            P = mass_event_hess(cols[0][e], lam, lo, hi, g, h);
+            if (!(P > 0.0)) { ++bad; continue; }
+            int q = 0;
+            for (int i = 0; i < 4; ++i)
+                for (int j = i; j < 4; ++j, ++q) {
+                    sh[i * K + j] += (long double)h[q];
+                    if (j != i) sh[j * K + i] += (long double)h[q];
+                }
+        } else {
+            double dA[8];
+            P = angular_value(cols[0][e], cols[1][e], cols[2][e], lam, dA);
+            if (!(P > 0.0)) { ++bad; continue; }
+            for (int i = 0; i < 8; ++i) g[i] = dA[i] / P;
+            for (int i = 0; i < 8; ++i)
+                for (int j = 0; j < 8; ++j) sh[i * K + j] += (long double)(-(dA[i] / P) * (dA[j] / P));
+        }
+        s0 += (long double)log(P);
+        for (int i = 0; i < K; ++i) sg[i] += (long double)g[i];
+    }
+    if (bad) {
+        *nll = INFINITY;
+        for (int i = 0; i < K; ++i) grad[i] = NAN;
+        for (int i = 0; i < K * K; ++i) hess[i] = NAN;
+        return bad;
+    }
+    *nll = (double)(-s0);
+    for (int i = 0; i < K; ++i) grad[i] = (double)(-sg[i]);
+    for (int i = 0; i < K * K; ++i) hess[i] = (double)(-sh[i]);
+    return 0;
 }

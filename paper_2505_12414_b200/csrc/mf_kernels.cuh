@@ -236,10 +236,20 @@ __device__ __forceinline__ void accumulate(const double* const* col, int64_t n, 
                             }
                         }
                     } else {
+                        // the last, partial group of this warp (and the ragged last item of the dataset): full items
+                        // still go through the vectorised body, two events at a time; only a ragged item is predicated
 #pragma unroll
                         for (int v = 0; v < U; ++v) {
                             const int64_t jv = ju + v * step;
-                            if (jv < n_items) {
+                            if (jv < n_full) {
+                                if constexpr (M::NCOL == 1) {
+                                    const double xs[2] = {x[v][0][0], x[v][1][0]};
+                                    M::template events<2>(xs, c, acc, lp, bad, t_lane);
+                                } else {
+                                    M::template event<false>(x[v][0], c, acc, lp, bad, true, t_lane);
+                                    M::template event<false>(x[v][1], c, acc, lp, bad, true, t_lane);
+                                }
+                            } else if (jv < n_items) {
                                 const int64_t e = kItem * jv + 2 * lane;
                                 M::template event<true>(x[v][0], c, acc, lp, bad, e < n, t_lane);
                                 M::template event<true>(x[v][1], c, acc, lp, bad, e + 1 < n, t_lane);
