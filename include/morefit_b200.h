@@ -153,6 +153,20 @@ mf_status mf_nll_grad_batch(mf_model* model, int64_t n_toys, const double* lambd
  * Two launches are enqueued on the context's stream (parameter-only constants, then the fused kernel). */
 mf_status mf_nll_grad_batch_async(mf_model* model, int64_t n_toys, const double* lambdas_dev, double* out_dev);
 
+/* ---- value + gradient + analytic Hessian ---------------------- */
+
+/* 1 if the model family has the analytic Hessian kernel (this round: MF_MASS_GAUSS_EXP), else 0. */
+int mf_model_has_hessian(const mf_model* model);
+
+/* As mf_nll_grad, plus hess (host, K*K doubles, row-major, symmetric) = d2(-ln L)/d lambda_k d lambda_l, from one
+ * launch that accumulates the second-derivative moment sums beside the value and the gradient.
+ * MF_ERR_ARG for a model family without the Hessian kernel; on MF_NONPOSITIVE_PDF hess is NaN. */
+mf_status mf_nll_grad_hess(mf_model* model, const double* lambda, double* nll, double* grad, double* hess);
+
+/* As mf_nll_grad_batch, plus hess (host, [n_toys][K*K]); inactive toys are left untouched. */
+mf_status mf_nll_grad_hess_batch(mf_model* model, int64_t n_toys, const double* lambdas, const uint8_t* active,
+                                 double* nll, double* grad, double* hess);
+
 /* ---- fit driver (host quasi-Newton over the GPU value+gradient) ------- */
 
 typedef struct {

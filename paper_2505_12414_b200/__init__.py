@@ -35,6 +35,7 @@ EXPORTS = [
     "mf_dataset_upload", "mf_dataset_destroy", "mf_dataset_n_events", "mf_dataset_n_toys",
     "mf_model_create", "mf_model_destroy", "mf_model_nparams", "mf_model_n_events", "mf_model_n_toys",
     "mf_nll_grad", "mf_nll_grad_async", "mf_nll_grad_points", "mf_nll_grad_batch", "mf_nll_grad_batch_async",
+    "mf_model_has_hessian", "mf_nll_grad_hess", "mf_nll_grad_hess_batch",
     "mf_fit_opts_default", "mf_fit", "mf_fit_batch",
     "mf_probe_fp64_rate", "mf_probe_read_bandwidth", "mf_probe_math",
 ]
@@ -133,6 +134,12 @@ def load_library() -> ctypes.CDLL:
     lib.mf_nll_grad_batch.argtypes = [vp, i64, dp, u8p, dp, dp]
     lib.mf_nll_grad_batch_async.restype = ctypes.c_int
     lib.mf_nll_grad_batch_async.argtypes = [vp, i64, vp, vp]
+    lib.mf_model_has_hessian.restype = ctypes.c_int
+    lib.mf_model_has_hessian.argtypes = [vp]
+    lib.mf_nll_grad_hess.restype = ctypes.c_int
+    lib.mf_nll_grad_hess.argtypes = [vp, dp, dp, dp, dp]
+    lib.mf_nll_grad_hess_batch.restype = ctypes.c_int
+    lib.mf_nll_grad_hess_batch.argtypes = [vp, i64, dp, u8p, dp, dp, dp]
     lib.mf_fit_opts_default.restype = None
     lib.mf_fit_opts_default.argtypes = [ctypes.POINTER(FitOpts)]
     lib.mf_fit.restype = ctypes.c_int
@@ -334,6 +341,30 @@ class Model:
         grad = np.full((T, self.K), np.nan)
         self._ctx._check(self._lib.mf_nll_grad_batch(self._h, T, _dp(lam), _u8p(act), _dp(nll), _dp(grad)))
         return nll, grad
+
+    @property
+    def has_hessian(self) -> bool:
+        return bool(self._lib.mf_model_has_hessian(self._h))
+
+    def nll_grad_hess(self, lam):
+        """(-ln L, gradient [K], Hessian [K][K]) from one launch (analytic second derivatives)."""
+        lam = np.ascontiguousarray(lam, dtype=np.float64)
+        nll = ctypes.c_double()
+        grad = np.empty(self.K)
+        hess = np.empty((self.K, self.K))
+        self._ctx._check(self._lib.mf_nll_grad_hess(self._h, _dp(lam), ctypes.byref(nll), _dp(grad), _dp(hess)))
+        return float(nll.value), grad, hess
+
+    def nll_grad_hess_batch(self, lambdas, active=None):
+        """lambdas [T][K] -> (nll [T], grad [T][K], hess [T][K][K]); inactive toys are NaN."""
+        lam = np.ascontiguousarray(lambdas, dtype=np.float64)
+        T = self.n_toys
+        act = None if active is None else np.ascontiguousarray(active, dtype=np.uint8)
+        nll = np.full(T, np.nan)
+        grad = np.full((T, self.K), np.nan)
+        hess = np.full((T, self.K, self.K), np.nan)
+        self._ctx._check(self._lib.mf_nll_grad_hess_batch(self._h, T, _dp(lam), _u8p(act), _dp(nll), _dp(grad), _dp(hess)))
+        return nll, grad, hess
 
     def nll_grad_batch_async(self, lambdas_dev_ptr: int, out_dev_ptr: int):
         """All toys, device pointers in ([T][K]) and out ([T][K+2]), no host synchronisation."""

@@ -285,7 +285,7 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
     m->ctx = ctx;
     m->kind = kind;
     m->K = K;
-    m->nacc = (kind == MF_MASS_GAUSS_EXP) ? MassModel::NACC : (kind == MF_ANGULAR_KSTMUMU) ? AngularModel::NACC : FourDModel::NACC;
+    m->nacc = (kind == MF_MASS_GAUSS_EXP) ? MassHessModel::NACC : (kind == MF_ANGULAR_KSTMUMU) ? AngularModel::NACC : FourDModel::NACC;
     m->ncol = ncol;
     m->n_events = ds->n_events;
     m->n_pad = ds->n_pad;
@@ -368,10 +368,11 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
         MF_CUDA_M(dev_alloc(ctx, &m->d_consts, sizeof(FourDConsts) * T));  // the largest Consts
         MF_CUDA_M(dev_alloc(ctx, &m->d_consts_ok, sizeof(int) * T));
         MF_CUDA_M(dev_alloc(ctx, &m->d_ids, sizeof(int) * T));
-        MF_CUDA_M(dev_alloc(ctx, &m->d_bout, sizeof(double) * T * (K + 2)));
+        const int nout1 = (kind == MF_MASS_GAUSS_EXP ? MassHessModel::NOUT : K + 1) + 1;  // widest output row + n_bad
+        MF_CUDA_M(dev_alloc(ctx, &m->d_bout, sizeof(double) * T * nout1));
         MF_CUDA_M(cudaHostAlloc(&m->h_lam, sizeof(double) * T * K, cudaHostAllocDefault));
         MF_CUDA_M(cudaHostAlloc(&m->h_ids, sizeof(int) * T, cudaHostAllocDefault));
-        MF_CUDA_M(cudaHostAlloc(&m->h_bout, sizeof(double) * T * (K + 2), cudaHostAllocDefault));
+        MF_CUDA_M(cudaHostAlloc(&m->h_bout, sizeof(double) * T * nout1, cudaHostAllocDefault));
     }
     {
         const cudaError_t e_sync = cudaStreamSynchronize(ctx->stream);
@@ -420,6 +421,11 @@ bool host_consts<MassModel>(const mf_model* m, const double* lam, MassConsts& c)
     return mass_consts(lam, m->ma, m->mb, c);
 }
 template <>
+bool host_consts<MassHessModel>(const mf_model* m, const double* lam, MassConsts& c)
+{
+    return mass_consts(lam, m->ma, m->mb, c);
+}
+template <>
 bool host_consts<AngularModel>(const mf_model*, const double* lam, AngularConsts& c)
 {
     return angular_consts(lam, c);
@@ -460,8 +466,13 @@ static mf_status launch_single(mf_model* m, const double* lam, double* out_dev, 
 }
 
 static mf_status dispatch_single(mf_model* m, const double* lam, double* out_dev, bool pipelined = false,
-                                 bool signal_host = false)
+                                 bool signal_host = false, bool hess = false)
 {
+    if (hess) {
+        if (m->kind != MF_MASS_GAUSS_EXP)
+            return mf_fail(m->ctx, MF_ERR_ARG, "the analytic Hessian is implemented for MF_MASS_GAUSS_EXP only");
+        return launch_single<MassHessModel>(m, lam, out_dev, pipelined, signal_host);
+    }
     switch (m->kind) {
     case MF_MASS_GAUSS_EXP: return launch_single<MassModel>(m, lam, out_dev, pipelined, signal_host);
     case MF_ANGULAR_KSTMUMU: return launch_single<AngularModel>(m, lam, out_dev, false, signal_host);
@@ -551,14 +562,14 @@ extern "C" mf_status mf_nll_grad_points(mf_model* m, int64_t n_points, const dou
     }
 }
 
-extern "C" mf_status mf_nll_grad(mf_model* m, const double* lambda, double* nll, double* grad)
+// One synchronous evaluation: value, gradient and (hess != NULL, mass model) the K x K Hessian.
+static mf_status eval_sync(mf_model* m, const double* lambda, double* nll, double* grad, double* hess, const char* who)
 {
-    if (!m || !lambda || !nll) return mf_fail(m ? m->ctx : nullptr, MF_ERR_ARG, "mf_nll_grad: NULL argument");
-    if (m->n_toys != 1) return mf_fail(m->ctx, MF_ERR_ARG, "mf_nll_grad: dataset has n_toys != 1; use mf_nll_grad_batch");
     mf_ctx* ctx = m->ctx;
+    const int K = m->K;
     // the last CTA writes the result, then the done word, to mapped pinned memory; the host spins on the
     // done word (a stream synchronise costs ~20 us of driver latency per call, the kernel 4-30 us)
-    const mf_status st = dispatch_single(m, lambda, m->d_out_mapped, false, true);
+    const mf_status st = dispatch_single(m, lambda, m->d_out_mapped, false, true, hess != nullptr);
     if (st != MF_OK) return st;
     volatile unsigned long long* done = reinterpret_cast<volatile unsigned long long*>(m->h_out + MF_MAX_PARAMS + 2);
     const unsigned long long want = m->seq;
@@ -567,18 +578,40 @@ extern "C" mf_status mf_nll_grad(mf_model* m, const double* lambda, double* nll,
             const cudaError_t q = cudaStreamQuery(ctx->stream);
             if (q != cudaErrorNotReady && *done != want) {
                 if (q == cudaSuccess) continue;  // completed: the word is on its way
-                return mf_fail(ctx, MF_ERR_CUDA, std::string("mf_nll_grad: ") + cudaGetErrorString(q));
+                return mf_fail(ctx, MF_ERR_CUDA, std::string(who) + ": " + cudaGetErrorString(q));
             }
         }
     }
     std::atomic_thread_fence(std::memory_order_acquire);
     *nll = m->h_out[0];
-    if (grad) std::memcpy(grad, m->h_out + 1, sizeof(double) * m->K);
-    if (m->h_out[m->K + 1] != 0.0)
+    if (grad) std::memcpy(grad, m->h_out + 1, sizeof(double) * K);
+    const int nout = hess ? MassHessModel::NOUT : K + 1;
+    if (hess) {
+        int q = 1 + K;
+        for (int i = 0; i < K; ++i)
+            for (int j = i; j < K; ++j, ++q) hess[i * K + j] = hess[j * K + i] = m->h_out[q];
+    }
+    if (m->h_out[nout] != 0.0)
         return mf_fail(ctx, MF_NONPOSITIVE_PDF,
-                       "P <= 0 for " + std::to_string((long long)m->h_out[m->K + 1]) + " events at this lambda");
+                       "P <= 0 for " + std::to_string((long long)m->h_out[nout]) + " events at this lambda");
     return MF_OK;
 }
+
+extern "C" mf_status mf_nll_grad(mf_model* m, const double* lambda, double* nll, double* grad)
+{
+    if (!m || !lambda || !nll) return mf_fail(m ? m->ctx : nullptr, MF_ERR_ARG, "mf_nll_grad: NULL argument");
+    if (m->n_toys != 1) return mf_fail(m->ctx, MF_ERR_ARG, "mf_nll_grad: dataset has n_toys != 1; use mf_nll_grad_batch");
+    return eval_sync(m, lambda, nll, grad, nullptr, "mf_nll_grad");
+}
+
+extern "C" mf_status mf_nll_grad_hess(mf_model* m, const double* lambda, double* nll, double* grad, double* hess)
+{
+    if (!m || !lambda || !nll || !hess) return mf_fail(m ? m->ctx : nullptr, MF_ERR_ARG, "mf_nll_grad_hess: NULL argument");
+    if (m->n_toys != 1) return mf_fail(m->ctx, MF_ERR_ARG, "mf_nll_grad_hess: dataset has n_toys != 1; use mf_nll_grad_hess_batch");
+    return eval_sync(m, lambda, nll, grad, hess, "mf_nll_grad_hess");
+}
+
+extern "C" int mf_model_has_hessian(const mf_model* m) { return m && m->kind == MF_MASS_GAUSS_EXP ? 1 : 0; }
 
 template <class M>
 static mf_status launch_batch(mf_model* m, int n_active, const double* lam_dev = nullptr, double* out_dev = nullptr)
@@ -621,26 +654,29 @@ extern "C" mf_status mf_nll_grad_batch_async(mf_model* m, int64_t n_toys, const 
     }
 }
 
-extern "C" mf_status mf_nll_grad_batch(mf_model* m, int64_t n_toys, const double* lambdas, const uint8_t* active,
-                                       double* nll, double* grad)
+// T toys at their own parameter points; hess != NULL (mass model): also the K x K Hessian per toy.
+static mf_status eval_batch(mf_model* m, int64_t n_toys, const double* lambdas, const uint8_t* active, double* nll,
+                            double* grad, double* hess, const char* who)
 {
-    if (!m || !lambdas || !nll) return mf_fail(m ? m->ctx : nullptr, MF_ERR_ARG, "mf_nll_grad_batch: NULL argument");
     mf_ctx* ctx = m->ctx;
-    if (n_toys != m->n_toys) return mf_fail(ctx, MF_ERR_ARG, "mf_nll_grad_batch: n_toys does not match the dataset");
+    const int K = m->K;
+    if (n_toys != m->n_toys) return mf_fail(ctx, MF_ERR_ARG, std::string(who) + ": n_toys does not match the dataset");
+    if (hess && m->kind != MF_MASS_GAUSS_EXP)
+        return mf_fail(ctx, MF_ERR_ARG, "the analytic Hessian is implemented for MF_MASS_GAUSS_EXP only");
     if (m->n_toys < 2 && !m->d_lam) {
-        // a 1-toy dataset evaluated through the batch entry: same result as mf_nll_grad
+        // a 1-toy dataset evaluated through the batch entry: same result as the single call
         if (active && !active[0]) return MF_OK;
         double g[MF_MAX_PARAMS];
-        const mf_status st = mf_nll_grad(m, lambdas, nll, g);
+        const mf_status st = eval_sync(m, lambdas, nll, g, hess, who);
         if (st == MF_ERR_PARAM_DOMAIN || st == MF_NONPOSITIVE_PDF) {
             *nll = INFINITY;
-            if (grad) for (int k = 0; k < m->K; ++k) grad[k] = NAN;
+            if (grad) for (int k = 0; k < K; ++k) grad[k] = NAN;
+            if (hess) for (int k = 0; k < K * K; ++k) hess[k] = NAN;
             return MF_OK;
         }
-        if (st == MF_OK && grad) std::memcpy(grad, g, sizeof(double) * m->K);
+        if (st == MF_OK && grad) std::memcpy(grad, g, sizeof(double) * K);
         return st;
     }
-    const int K = m->K;
     int n_active = 0;
     for (int64_t t = 0; t < n_toys; ++t) {
         if (active && !active[t]) continue;
@@ -653,20 +689,45 @@ extern "C" mf_status mf_nll_grad_batch(mf_model* m, int64_t n_toys, const double
     if (n_active < n_toys)
         MF_CUDA(ctx, cudaMemcpyAsync(m->d_ids, m->h_ids, sizeof(int) * n_active, cudaMemcpyHostToDevice, ctx->stream));
     mf_status st;
-    switch (m->kind) {
-    case MF_MASS_GAUSS_EXP: st = launch_batch<MassModel>(m, n_active); break;
-    case MF_ANGULAR_KSTMUMU: st = launch_batch<AngularModel>(m, n_active); break;
-    default: st = launch_batch<FourDModel>(m, n_active); break;
+    if (hess) {
+        st = launch_batch<MassHessModel>(m, n_active);
+    } else {
+        switch (m->kind) {
+        case MF_MASS_GAUSS_EXP: st = launch_batch<MassModel>(m, n_active); break;
+        case MF_ANGULAR_KSTMUMU: st = launch_batch<AngularModel>(m, n_active); break;
+        default: st = launch_batch<FourDModel>(m, n_active); break;
+        }
     }
     if (st != MF_OK) return st;
-    MF_CUDA(ctx, cudaMemcpyAsync(m->h_bout, m->d_bout, sizeof(double) * n_active * (K + 2), cudaMemcpyDeviceToHost,
-                                 ctx->stream));
+    const int row = (hess ? MassHessModel::NOUT : K + 1) + 1;
+    MF_CUDA(ctx, cudaMemcpyAsync(m->h_bout, m->d_bout, sizeof(double) * n_active * row, cudaMemcpyDeviceToHost, ctx->stream));
     MF_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     for (int s = 0; s < n_active; ++s) {
         const int64_t t = m->h_ids[s];
-        const double* o = m->h_bout + (int64_t)s * (K + 2);
+        const double* o = m->h_bout + (int64_t)s * row;
         nll[t] = o[0];
         if (grad) std::memcpy(grad + t * K, o + 1, sizeof(double) * K);
+        if (hess) {
+            double* H = hess + t * K * K;
+            int q = 1 + K;
+            for (int i = 0; i < K; ++i)
+                for (int j = i; j < K; ++j, ++q) H[i * K + j] = H[j * K + i] = o[q];
+        }
     }
     return MF_OK;
+}
+
+extern "C" mf_status mf_nll_grad_batch(mf_model* m, int64_t n_toys, const double* lambdas, const uint8_t* active,
+                                       double* nll, double* grad)
+{
+    if (!m || !lambdas || !nll) return mf_fail(m ? m->ctx : nullptr, MF_ERR_ARG, "mf_nll_grad_batch: NULL argument");
+    return eval_batch(m, n_toys, lambdas, active, nll, grad, nullptr, "mf_nll_grad_batch");
+}
+
+extern "C" mf_status mf_nll_grad_hess_batch(mf_model* m, int64_t n_toys, const double* lambdas, const uint8_t* active,
+                                            double* nll, double* grad, double* hess)
+{
+    if (!m || !lambdas || !nll || !hess)
+        return mf_fail(m ? m->ctx : nullptr, MF_ERR_ARG, "mf_nll_grad_hess_batch: NULL argument");
+    return eval_batch(m, n_toys, lambdas, active, nll, grad, hess, "mf_nll_grad_hess_batch");
 }

@@ -45,7 +45,7 @@ struct EvalArgs {
     unsigned* ticket;            // zero on entry, reset to zero by the last CTA
     unsigned long long* gen;     // evaluations completed on this slot
     unsigned long long need;     // value of *gen at which the slot is free for this evaluation
-    double* out;                 // [K+2]: -lnL, grad, n_bad
+    double* out;                 // [NOUT+1]: -lnL, grad (, Hessian), n_bad
     unsigned long long* done_flag;   // mapped host word that receives done_value after `out` is written, or NULL
     unsigned long long done_value;
 };
@@ -74,6 +74,11 @@ template <class M>
 __device__ __forceinline__ bool make_consts(const double* lam, double ma, double mb, typename M::Consts& c);
 template <>
 __device__ __forceinline__ bool make_consts<MassModel>(const double* lam, double ma, double mb, MassConsts& c)
+{
+    return mass_consts(lam, ma, mb, c);
+}
+template <>
+__device__ __forceinline__ bool make_consts<MassHessModel>(const double* lam, double ma, double mb, MassConsts& c)
 {
     return mass_consts(lam, ma, mb, c);
 }
@@ -327,7 +332,7 @@ __device__ __forceinline__ void final_combine(const double* p, int64_t stride_k,
                                               double* out, unsigned long long* done_flag = nullptr,
                                               unsigned long long done_value = 0)
 {
-    constexpr int NACC = M::NACC, K = M::K;
+    constexpr int NACC = M::NACC, NOUT = M::NOUT;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     unsigned nb = 0;
     if (w == 0) {
@@ -367,13 +372,13 @@ __device__ __forceinline__ void final_combine(const double* p, int64_t stride_k,
     }
     __syncthreads();
     if (threadIdx.x == 0) {
-        double o[K + 1];
+        double o[NOUT];
         M::finish(c, s_sum, n, sum_m, o);
         pdl_wait();
 #pragma unroll
-        for (int k = 0; k <= K; ++k)
+        for (int k = 0; k < NOUT; ++k)
             out[k] = !nb ? o[k] : (k == 0) ? __longlong_as_double(0x7ff0000000000000LL) : __longlong_as_double(0x7ff8000000000000LL);
-        out[K + 1] = (double)nb;
+        out[NOUT] = (double)nb;
         if (done_flag) {  // synchronous call: the host spins on this word instead of a stream synchronise
             __threadfence_system();
             *reinterpret_cast<volatile unsigned long long*>(done_flag) = done_value;
@@ -480,7 +485,8 @@ __global__ void __launch_bounds__(M::BATCH_BLOCK, M::BATCH_RESIDENT_CTAS)
             reinterpret_cast<double*>(&s_c)[threadIdx.x] = reinterpret_cast<const double*>(a.consts + slot)[threadIdx.x];
         if (threadIdx.x == 0) s_ok = a.consts_ok[slot];
     }
-    double* out = a.out + (int64_t)slot * (K + 2);
+    constexpr int NOUT = M::NOUT;  // -ln L, gradient (and Hessian for the *Hess models); n_bad follows at [NOUT]
+    double* out = a.out + (int64_t)slot * (NOUT + 1);
     const double sum_m = a.sum_m ? a.sum_m[toy] : 0.0;
     const double* col[M::NCOL];
 #pragma unroll
@@ -499,9 +505,9 @@ __global__ void __launch_bounds__(M::BATCH_BLOCK, M::BATCH_RESIDENT_CTAS)
                   },
                   acc, bad);
     if (!s_ok) {  // outside the parameter domain (the sums above are garbage and unused): +inf / NaN, n_bad = -1
-        if (chunk == 0 && threadIdx.x <= K + 1)
+        if (chunk == 0 && threadIdx.x <= NOUT)
             out[threadIdx.x] = threadIdx.x == 0       ? __longlong_as_double(0x7ff0000000000000LL)
-                               : threadIdx.x == K + 1 ? -1.0
+                               : threadIdx.x == NOUT  ? -1.0
                                                       : __longlong_as_double(0x7ff8000000000000LL);
         return;
     }
@@ -513,13 +519,13 @@ __global__ void __launch_bounds__(M::BATCH_BLOCK, M::BATCH_RESIDENT_CTAS)
         __syncthreads();
         if (threadIdx.x == 0) {
             const unsigned nb = s_bad_block;
-            double o[K + 1];
+            double o[NOUT];
             M::finish(c, s_sum, (double)a.n, sum_m, o);
             pdl_wait();
 #pragma unroll
-            for (int k = 0; k <= K; ++k)
+            for (int k = 0; k < NOUT; ++k)
                 out[k] = !nb ? o[k] : (k == 0) ? __longlong_as_double(0x7ff0000000000000LL) : __longlong_as_double(0x7ff8000000000000LL);
-            out[K + 1] = (double)nb;
+            out[NOUT] = (double)nb;
         }
         return;
     }

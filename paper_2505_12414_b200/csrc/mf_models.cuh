@@ -74,7 +74,23 @@ struct MassConsts {
     double ksig;     // 1/sigma + d ln N1 / d sigma
     double ma;       // m_a (reference point for the tau derivative)
     double ktau;     // d ln N2 / d tau - m_a = w [1/2 + Langevin(tau w / 2)/2],  w = m_b - m_a
+    // second derivatives of the normalisations (analytic Hessian; MassHessModel)
+    double is4;      // 1/sigma^4
+    double ct;       // mu - m_a - ktau:  m - d ln N2/d tau = d + ct
+    double n1mm, n1ms, n1ss;  // d2 ln N1 / d(mu, sigma)^2
+    double n2tt;     // d2 ln N2 / d tau^2 = w^2 L'(tau w / 2) / 4
 };
+
+// derivative of the Langevin function, 1/x^2 - 1/sinh^2(x) (series below |x| = 0.1: cancellation)
+MF_HD inline double langevin_prime(double x)
+{
+    const double x2 = x * x;
+    if (fabs(x) < 0.1)
+        return 1.0 / 3.0 + x2 * (-1.0 / 15.0 + x2 * (2.0 / 189.0 + x2 * (-1.0 / 675.0 + x2 * (2.0 / 10395.0))));
+    if (fabs(x) > 350.0) return 1.0 / x2;
+    const double sh = sinh(x);
+    return 1.0 / x2 - 1.0 / (sh * sh);
+}
 
 // Returns false if lambda = (f, mu, sigma, tau) is outside the parameter domain
 // (non-finite, sigma <= 0, f outside [0,1]).
@@ -106,6 +122,19 @@ MF_HD inline bool mass_consts(const double* lam, double ma, double mb, MassConst
     c.ksig = is + ((ma - mu) * ga - (mb - mu) * gb) * is * iN1;
     c.ma = ma;
     c.ktau = w * (0.5 + 0.5 * langevin(0.5 * tau * w));
+    {
+        const double da = ma - mu, db = mb - mu, is2 = is * is, is3 = is2 * is;
+        const double N1m = ga - gb, N1s = (da * ga - db * gb) * is;
+        const double ga_s = ga * (da * da * is3 - is), gb_s = gb * (db * db * is3 - is);
+        const double N1mm = (ga * da - gb * db) * is2, N1ms = ga_s - gb_s;
+        const double N1ss = (da * ga_s - db * gb_s) * is - (da * ga - db * gb) * is2;
+        c.n1mm = N1mm * iN1 - (N1m * iN1) * (N1m * iN1);
+        c.n1ms = N1ms * iN1 - (N1m * iN1) * (N1s * iN1);
+        c.n1ss = N1ss * iN1 - (N1s * iN1) * (N1s * iN1);
+        c.n2tt = 0.25 * w * w * langevin_prime(0.5 * tau * w);
+        c.is4 = is2 * is2;
+        c.ct = (mu - ma) - c.ktau;
+    }
     // The kernels evaluate R = exp(-b0 (m-mu)^2 - tau m + lnk) with a range-restricted exp: refuse
     // parameter points whose normalisations are not representable (N1 or N2 under/overflow) or
     // whose largest possible exponent argument leaves the finite range.
@@ -185,6 +214,7 @@ MF_D double diff_of_products(double a, double b, double c, double d)
 struct MassModel {
     static constexpr int K = 4;
     static constexpr int NCOL = 1;  // m
+    static constexpr int NOUT = K + 1;  // -ln L, gradient
     static constexpr int NACC = 6;  // ln prod D, and with u = (G/N1)/P', r = (E/N2)/P' (P' = P N2 e^{-tau m}, d = m - mu):
                                     // sum u, sum r, sum u d, sum u d^2, sum r d
     // tuning knobs (defaults = the measured best on B200)
@@ -282,9 +312,128 @@ struct MassModel {
     }
 };
 
+// ------------------------------------------------------------------------------------------
+// Mass model with the analytic Hessian (value, gradient and
+// Hessian in one evaluation give Newton convergence in 2-3 iterations).  With w = f u the signal
+// weight, 1 - w = (1-f) r, A = ln R and q = m - d ln N2/d tau = d + ct:
+//   l_ff = -(u - r)^2                       l_f,theta = u r A_theta            (A_tau = -q)
+//   l_theta,theta' = w (1-w) A_theta A_theta' + w A_theta,theta'   (- (1-w) d2 ln N2/dtau^2 for tau,tau)
+// A_mu = d/s^2 - kmu, A_sigma = d^2/s^3 - ksig are polynomials in d, so the Hessian needs seven more
+// moment sums: sum u^2, r^2, z, z d, z d^2, z d^3, z d^4 with z = u r.  36 fp64 instructions per event.
+// Output: -ln L, gradient[4], then the upper triangle ff, fm, fs, ft, mm, ms, mt, ss, st, tt of d2(-ln L).
+// ------------------------------------------------------------------------------------------
+struct MassHessModel {
+    static constexpr int K = 4;
+    static constexpr int NCOL = 1;
+    static constexpr int NOUT = 1 + 4 + 10;
+    static constexpr int NACC = 13;
+    static constexpr int ITEMS_PER_ITER = 2;  // 4 events at once (13 sums leave fewer registers)
+    static constexpr int PREFETCH = 4;
+    static constexpr int CTAS_PER_SM = 2;
+    static constexpr int RESIDENT_CTAS = 2;
+    static constexpr int BATCH_RESIDENT_CTAS = 4;
+    static constexpr int BATCH_BLOCK = 128;
+    using Consts = MassConsts;
+
+    template <int E>
+    static MF_D void events(const double (&m)[E], const Consts& c, double* acc, LogProd& lp, unsigned& bad, double t_lane)
+    {
+        double d[E], t[E], arg[E], R[E], D[E], r[E], u[E], z[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) d[e] = m[e] - c.mu;
+#pragma unroll
+        for (int e = 0; e < E; ++e) arg[e] = fma(-c.tau, m[e], c.lnk);
+#pragma unroll
+        for (int e = 0; e < E; ++e) t[e] = d[e] * d[e];
+#pragma unroll
+        for (int e = 0; e < E; ++e) arg[e] = fma(c.nb0, t[e], arg[e]);
+        mf_exp32_v<E>(arg, t_lane, R);
+#pragma unroll
+        for (int e = 0; e < E; ++e) D[e] = fma(c.f, R[e], c.omf);
+#pragma unroll
+        for (int e = 0; e < E; ++e) r[e] = mf_rcp(D[e]);
+#pragma unroll
+        for (int e = 0; e < E; ++e) u[e] = R[e] * r[e];
+#pragma unroll
+        for (int e = 0; e < E; ++e) z[e] = u[e] * r[e];
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            lp.mul(D[e], bad);
+            acc[1] += u[e];
+            acc[2] += r[e];
+            acc[3] = fma(u[e], d[e], acc[3]);
+            acc[4] = fma(u[e], t[e], acc[4]);
+            acc[5] = fma(r[e], d[e], acc[5]);
+            acc[6] = fma(u[e], u[e], acc[6]);
+            acc[7] = fma(r[e], r[e], acc[7]);
+            acc[8] += z[e];
+            const double zd = z[e] * d[e];
+            acc[9] += zd;
+            acc[10] = fma(zd, d[e], acc[10]);
+            acc[11] = fma(zd, t[e], acc[11]);
+            acc[12] = fma(z[e] * t[e], t[e], acc[12]);
+        }
+    }
+
+    template <bool PRED>
+    static MF_D void event(const double* x, const Consts& c, double* acc, LogProd& lp, unsigned& bad, bool valid,
+                           double t_lane)
+    {
+        // every lane evaluates (the exponential shuffles across the whole warp); invalid lanes discard the result
+        double tmp[NACC];
+#pragma unroll
+        for (int k = 0; k < NACC; ++k) tmp[k] = 0.0;
+        LogProd lp2;
+        unsigned bad2 = 0;
+        const double m1[1] = {x[0]};
+        events<1>(m1, c, tmp, lp2, bad2, t_lane);
+        if (!PRED || valid) {
+#pragma unroll
+            for (int k = 1; k < NACC; ++k) acc[k] += tmp[k];
+            lp.prod *= lp2.prod;
+            lp.esum += lp2.esum;
+            bad += bad2;
+        }
+    }
+
+    static MF_D void finish(const Consts& c, const double* s, double n, double sum_m, double* out)
+    {
+        MassModel::finish(c, s, n, sum_m, out);
+        const double Su = s[1], Sr = s[2], Sud = s[3], Sud2 = s[4];
+        const double Suu = s[6], Srr = s[7], Sz = s[8], Szd = s[9], Szd2 = s[10], Szd3 = s[11], Szd4 = s[12];
+        const double fo = c.f * c.omf, ct = c.ct, kmu = c.kmu, ksig = c.ksig, is2 = c.is2, is3 = c.is3;
+        const double Szq = fma(ct, Sz, Szd);          // sum z q
+        const double Szdq = fma(ct, Szd, Szd2);       // sum z d q
+        const double Szd2q = fma(ct, Szd2, Szd3);     // sum z d^2 q
+        const double l_ff = -((Suu - 2.0 * Sz) + Srr);
+        const double l_fm = diff_of_products(is2, Szd, kmu, Sz);
+        const double l_fs = diff_of_products(is3, Szd2, ksig, Sz);
+        const double l_ft = -Szq;
+        const double l_mm = fo * (is2 * is2 * Szd2 - 2.0 * is2 * kmu * Szd + kmu * kmu * Sz) - c.f * (is2 + c.n1mm) * Su;
+        const double l_ms = fo * (is2 * is3 * Szd3 - is2 * ksig * Szd - kmu * is3 * Szd2 + kmu * ksig * Sz) -
+                            c.f * (2.0 * is3 * Sud + c.n1ms * Su);
+        const double l_mt = -fo * diff_of_products(is2, Szdq, kmu, Szq);
+        const double l_ss = fo * (is3 * is3 * Szd4 - 2.0 * is3 * ksig * Szd2 + ksig * ksig * Sz) +
+                            c.f * ((is2 - c.n1ss) * Su - 3.0 * c.is4 * Sud2);
+        const double l_st = -fo * diff_of_products(is3, Szd2q, ksig, Szq);
+        const double l_tt = fo * (Szd2 + 2.0 * ct * Szd + ct * ct * Sz) - c.omf * c.n2tt * Sr;
+        out[5] = -l_ff;
+        out[6] = -l_fm;
+        out[7] = -l_fs;
+        out[8] = -l_ft;
+        out[9] = -l_mm;
+        out[10] = -l_ms;
+        out[11] = -l_mt;
+        out[12] = -l_ss;
+        out[13] = -l_st;
+        out[14] = -l_tt;
+    }
+};
+
 struct AngularModel {
     static constexpr int K = 8;
     static constexpr int NCOL = 9;  // h_0..h_8 (cached, already times 9/(32 pi))
+    static constexpr int NOUT = K + 1;
     static constexpr int NACC = 9;  // ln prod P, sum h_k / P
     static constexpr int ITEMS_PER_ITER = 1;  // memory bound: depth comes from the prefetched next item
     static constexpr int PREFETCH = 0;
@@ -319,6 +468,7 @@ struct AngularModel {
 struct FourDModel {
     static constexpr int K = 16;
     static constexpr int NCOL = 12;  // m, cos theta_l, cos theta_K, h_0..h_8
+    static constexpr int NOUT = K + 1;
     static constexpr int NACC = 17;  // ln prod D, then sum d ln P / d lambda_k
     static constexpr int ITEMS_PER_ITER = 1;
     static constexpr int PREFETCH = 0;
