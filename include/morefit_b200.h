@@ -180,6 +180,8 @@ typedef struct {
     int max_chord;         /* Newton steps per Hessian (8) */
     double fd_rel;         /* first FD step: fd_rel * max(|lambda_k|, 1) (1e-5) */
     double fd_sigma;       /* later FD steps: fd_sigma * sigma_k (1e-4) */
+    int analytic_hessian;  /* 1 (default): use the analytic Hessian kernel where the model has one (mf_model_has_hessian):
+                              every evaluation returns the Hessian, Newton steps, no finite-difference phases */
 } mf_fit_opts;
 
 /* Fills *opts with the defaults above. */
@@ -196,7 +198,9 @@ typedef struct {
 
 /* Minimises -ln L from `start` (host, K).  fixed: host, K bytes (1 = keep at start; paper:
  * the parameter `constant` flag) or NULL.  opts NULL = defaults.
- * Algorithm (SURVEY.md §8(c) "Fit"): central-difference Hessian of the analytic gradient
+ * With the analytic Hessian (opts->analytic_hessian, mass model): Newton steps with Armijo backtracking on the
+ * Hessian returned by every evaluation, then Newton polish; cov = H^-1 at the minimum.
+ * Otherwise (SURVEY.md §8(c) "Fit"): central-difference Hessian of the analytic gradient
  * at the start point seeds the inverse metric; BFGS with Armijo backtracking that rejects
  * domain errors and P<=0 points; then Newton steps on a fresh central-difference Hessian
  * until the step is below polish_tol sigma; cov = H^-1.

@@ -52,7 +52,7 @@ class FitOpts(ctypes.Structure):
     _fields_ = [("max_iter", ctypes.c_int), ("edm_tol", ctypes.c_double), ("armijo_c1", ctypes.c_double),
                 ("backtrack", ctypes.c_double), ("max_backtracks", ctypes.c_int), ("polish_tol", ctypes.c_double),
                 ("max_polish", ctypes.c_int), ("max_chord", ctypes.c_int), ("fd_rel", ctypes.c_double),
-                ("fd_sigma", ctypes.c_double)]
+                ("fd_sigma", ctypes.c_double), ("analytic_hessian", ctypes.c_int)]
 
 
 class _FitResultC(ctypes.Structure):
@@ -76,6 +76,38 @@ class FitResult:
     @property
     def sigma(self) -> np.ndarray:
         return np.sqrt(np.diag(self.cov))
+
+
+class BatchFitResult:
+    """Results of mf_fit_batch as arrays: lam [T][K], cov [T][K][K], nll [T], n_calls [T], n_iter [T],
+    converged [T] (bool), sigma [T][K].  Indexing or iterating yields per-toy FitResult-like views."""
+
+    _DT = np.dtype([("lambda_hat", np.float64, (MF_MAX_PARAMS,)), ("cov", np.float64, (MF_MAX_PARAMS * MF_MAX_PARAMS,)),
+                    ("nll_min", np.float64), ("n_calls", np.int32), ("n_iter", np.int32), ("converged", np.int32),
+                    ("_pad", np.int32)])
+
+    def __init__(self, raw, T: int, K: int):
+        assert self._DT.itemsize == ctypes.sizeof(_FitResultC)
+        a = np.frombuffer(raw, dtype=self._DT, count=T)
+        self.lam = a["lambda_hat"][:, :K].copy()
+        self.cov = a["cov"][:, :K * K].reshape(T, K, K).copy()
+        self.nll = a["nll_min"].copy()
+        self.n_calls = a["n_calls"].copy()
+        self.n_iter = a["n_iter"].copy()
+        self.converged = a["converged"] != 0
+        self.sigma = np.sqrt(np.abs(np.diagonal(self.cov, axis1=1, axis2=2)))
+
+    def __len__(self):
+        return self.lam.shape[0]
+
+    def __getitem__(self, t):
+        v = FitResult.__new__(FitResult)
+        v.lam, v.cov, v.nll = self.lam[t], self.cov[t], float(self.nll[t])
+        v.n_calls, v.n_iter, v.converged = int(self.n_calls[t]), int(self.n_iter[t]), bool(self.converged[t])
+        return v
+
+    def __iter__(self):
+        return (self[t] for t in range(len(self)))
 
 
 _lib = None
@@ -380,7 +412,7 @@ class Model:
         self._ctx._check(st)
         return FitResult(res, self.K)
 
-    def fit_batch(self, starts, fixed=None, opts: FitOpts | None = None) -> list[FitResult]:
+    def fit_batch(self, starts, fixed=None, opts: FitOpts | None = None) -> "BatchFitResult":
         T = self.n_toys
         starts = np.ascontiguousarray(starts, dtype=np.float64)
         if starts.shape == (self.K,):
@@ -390,7 +422,7 @@ class Model:
         st = self._lib.mf_fit_batch(self._h, T, _dp(starts), _u8p(fx), None if opts is None else ctypes.byref(opts),
                                     res)
         self._ctx._check(st)
-        return [FitResult(res[t], self.K) for t in range(T)]
+        return BatchFitResult(res, T, self.K)
 
     def close(self):
         if self._h:

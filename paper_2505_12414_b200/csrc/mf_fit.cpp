@@ -22,14 +22,15 @@
 
 namespace {
 
-constexpr int KMAX = MF_MAX_PARAMS;
-
-// Dense symmetric helpers on nf x nf matrices stored row-major with leading dimension KMAX.
-struct Mat {
-    double a[KMAX][KMAX];
+// Dense symmetric helpers on nf x nf matrices stored row-major with leading dimension KM (the capacity of the fit
+// state: 4, 8 or 16 parameters, so that 4096 concurrent 4-parameter toy fits carry 1 KB of state each, not 12 KB).
+template <int KM>
+struct MatT {
+    double a[KM][KM];
 };
 
 // Cholesky factor (lower) of A; false if A is not positive definite.
+template <class Mat>
 bool cholesky(const Mat& A, int n, Mat& L)
 {
     for (int i = 0; i < n; ++i) {
@@ -48,6 +49,7 @@ bool cholesky(const Mat& A, int n, Mat& L)
 }
 
 // inv = A^-1 for positive definite A; false otherwise.
+template <class Mat>
 bool inv_pd(const Mat& A, int n, Mat& inv)
 {
     Mat L;
@@ -73,7 +75,10 @@ bool inv_pd(const Mat& A, int n, Mat& inv)
     return true;
 }
 
-class FitState {
+template <int KMAX>
+class FitStateT {
+    using Mat = MatT<KMAX>;
+
 public:
     void init(int K, const double* start, const uint8_t* fixed, const mf_fit_opts& o)
     {
@@ -95,9 +100,13 @@ public:
     }
     bool done() const { return phase_ == DONE; }
     const double* request() const { return req_; }
+    // Analytic-Hessian mode (model families with the Hessian kernel; likelihood + gradient + Hessian
+    // per iteration): every evaluation also returns d2(-ln L); no finite-difference phases, Newton metric.
+    void use_analytic_hessian() { use_h_ = true; }
 
-    // Result of evaluating request(): ok = finite value and gradient at a valid point.
-    void feed(bool ok, double f, const double* gfull)
+    // Result of evaluating request(): ok = finite value and gradient at a valid point.  hfull: K x K Hessian there
+    // (analytic mode) or NULL.
+    void feed(bool ok, double f, const double* gfull, const double* hfull = nullptr)
     {
         ++calls_;
         double g[KMAX];
@@ -108,6 +117,14 @@ public:
                 ok = ok && std::isfinite(g[a]);
             }
         }
+        Mat Hin{};
+        bool h_ok = use_h_ && ok && hfull != nullptr;
+        if (h_ok)
+            for (int a = 0; a < nf_; ++a)
+                for (int b = 0; b < nf_; ++b) {
+                    Hin.a[a][b] = hfull[idx_[a] * K_ + idx_[b]];
+                    h_ok = h_ok && std::isfinite(Hin.a[a][b]);
+                }
         switch (phase_) {
         case START:
             if (!ok) {
@@ -121,6 +138,14 @@ public:
             if (nf_ == 0) {
                 converged_ = true;
                 phase_ = DONE;
+                return;
+            }
+            if (use_h_) {  // the Hessian at the start point came with this evaluation
+                H_ = Hin;
+                Hx_ = Hin;
+                hx_ok_ = h_ok;
+                fd_ok_ = h_ok;
+                after_seed();
                 return;
             }
             for (int a = 0; a < nf_; ++a) h_[a] = o_.fd_rel * std::max(std::fabs(x_[idx_[a]]), 1.0);
@@ -143,7 +168,10 @@ public:
                     ss += s[a] * s[a];
                     yy += y[a] * y[a];
                 }
-                if (sy > 1e-10 * std::sqrt(ss) * std::sqrt(yy)) {
+                Mat newton;
+                if (use_h_ && h_ok && inv_pd(Hin, nf_, newton)) {
+                    Hinv_ = newton;  // Newton metric at the accepted point
+                } else if (sy > 1e-10 * std::sqrt(ss) * std::sqrt(yy)) {
                     const double rho = 1.0 / sy;
                     double Hy[KMAX];
                     double yHy = 0;
@@ -160,6 +188,8 @@ public:
                 std::memcpy(x_, req_, sizeof(double) * K_);
                 f_ = f;
                 std::memcpy(g_, g, sizeof(double) * nf_);
+                Hx_ = Hin;
+                hx_ok_ = h_ok;
                 begin_bfgs_iter();
                 return;
             }
@@ -180,6 +210,18 @@ public:
             f_ = f;
             std::memcpy(g_, g, sizeof(double) * nf_);
             ++chord_;
+            if (use_h_) {  // a fresh Hessian came with the point: true Newton steps, covariance always current
+                Hx_ = Hin;
+                hx_ok_ = h_ok;
+                Mat c;
+                if (h_ok && inv_pd(Hin, nf_, c)) {
+                    cov_ = c;
+                    for (int a = 0; a < nf_; ++a) {
+                        sig_[a] = std::sqrt(cov_.a[a][a]);
+                        moved_[a] = 0.0;  // the covariance was taken here
+                    }
+                }
+            }
             begin_chord();
             return;
         default: return;
@@ -309,6 +351,12 @@ private:
             return;
         }
         ++polish_;
+        if (use_h_) {  // the Hessian at x_ is already here
+            H_ = Hx_;
+            fd_ok_ = hx_ok_;
+            after_polish_fd();
+            return;
+        }
         begin_fd(POLISH_FD);
     }
     void after_polish_fd()
@@ -368,6 +416,8 @@ private:
     int nbt_ = 0, iter_ = 0, calls_ = 0, polish_ = 0, chord_ = 0;
     double sig_[KMAX] = {}, moved_[KMAX] = {};
     bool converged_ = false, failed_start_ = false;
+    bool use_h_ = false, hx_ok_ = false;
+    Mat Hx_{};  // analytic mode: Hessian at x_
 };
 
 }  // namespace
@@ -385,6 +435,29 @@ extern "C" void mf_fit_opts_default(mf_fit_opts* o)
     o->max_chord = 8;
     o->fd_rel = 1e-5;
     o->fd_sigma = 1e-4;
+    o->analytic_hessian = 1;
+}
+
+template <int KM>
+static mf_status fit_one(mf_model* m, const double* start, const uint8_t* fixed, const mf_fit_opts& o, mf_fit_result* result)
+{
+    FitStateT<KM> st;
+    st.init(m->K, start, fixed, o);
+    const bool analytic = o.analytic_hessian != 0 && mf_model_has_hessian(m);
+    if (analytic) st.use_analytic_hessian();
+    mf_status first = MF_OK;
+    bool is_first = true;
+    while (!st.done()) {
+        double f = 0, g[KM], h[KM * KM];
+        const mf_status rc = analytic ? mf_nll_grad_hess(m, st.request(), &f, g, h) : mf_nll_grad(m, st.request(), &f, g);
+        if (rc != MF_OK && rc != MF_ERR_PARAM_DOMAIN && rc != MF_NONPOSITIVE_PDF) return rc;
+        if (is_first) first = rc;
+        is_first = false;
+        st.feed(rc == MF_OK, f, g, analytic ? h : nullptr);
+    }
+    st.result(result);
+    if (st.failed_start()) return mf_fail(m->ctx, first == MF_OK ? MF_NONPOSITIVE_PDF : first, "mf_fit: invalid start point");
+    return MF_OK;
 }
 
 extern "C" mf_status mf_fit(mf_model* m, const double* start, const uint8_t* fixed, const mf_fit_opts* opts,
@@ -395,20 +468,42 @@ extern "C" mf_status mf_fit(mf_model* m, const double* start, const uint8_t* fix
     mf_fit_opts o;
     if (opts) o = *opts;
     else mf_fit_opts_default(&o);
-    FitState st;
-    st.init(m->K, start, fixed, o);
-    mf_status first = MF_OK;
-    bool is_first = true;
-    while (!st.done()) {
-        double f = 0, g[KMAX];
-        const mf_status rc = mf_nll_grad(m, st.request(), &f, g);
-        if (rc != MF_OK && rc != MF_ERR_PARAM_DOMAIN && rc != MF_NONPOSITIVE_PDF) return rc;
-        if (is_first) first = rc;
-        is_first = false;
-        st.feed(rc == MF_OK, f, g);
+    if (m->K <= 4) return fit_one<4>(m, start, fixed, o, result);
+    if (m->K <= 8) return fit_one<8>(m, start, fixed, o, result);
+    return fit_one<MF_MAX_PARAMS>(m, start, fixed, o, result);
+}
+
+template <int KM>
+static mf_status fit_many(mf_model* m, int64_t n_toys, const double* starts, const uint8_t* fixed, const mf_fit_opts& o,
+                          mf_fit_result* results)
+{
+    const int K = m->K;
+    std::vector<FitStateT<KM>> st((size_t)n_toys);
+    std::vector<double> lam((size_t)n_toys * K), nll((size_t)n_toys), grad((size_t)n_toys * K);
+    std::vector<uint8_t> active((size_t)n_toys);
+    const bool analytic = o.analytic_hessian != 0 && mf_model_has_hessian(m);
+    std::vector<double> hess(analytic ? (size_t)n_toys * K * K : 0);
+    for (int64_t t = 0; t < n_toys; ++t) {
+        st[t].init(K, starts + t * K, fixed, o);
+        if (analytic) st[t].use_analytic_hessian();
     }
-    st.result(result);
-    if (st.failed_start()) return mf_fail(m->ctx, first == MF_OK ? MF_NONPOSITIVE_PDF : first, "mf_fit: invalid start point");
+    for (;;) {
+        int64_t n_active = 0;
+        for (int64_t t = 0; t < n_toys; ++t) {
+            active[t] = st[t].done() ? 0 : 1;
+            if (active[t]) {
+                std::memcpy(&lam[t * K], st[t].request(), sizeof(double) * K);
+                ++n_active;
+            }
+        }
+        if (n_active == 0) break;
+        const mf_status rc = analytic ? mf_nll_grad_hess_batch(m, n_toys, lam.data(), active.data(), nll.data(), grad.data(), hess.data())
+                                      : mf_nll_grad_batch(m, n_toys, lam.data(), active.data(), nll.data(), grad.data());
+        if (rc != MF_OK) return rc;
+        for (int64_t t = 0; t < n_toys; ++t)
+            if (active[t]) st[t].feed(std::isfinite(nll[t]), nll[t], &grad[t * K], analytic ? &hess[t * K * K] : nullptr);
+    }
+    for (int64_t t = 0; t < n_toys; ++t) st[t].result(&results[t]);
     return MF_OK;
 }
 
@@ -420,26 +515,7 @@ extern "C" mf_status mf_fit_batch(mf_model* m, int64_t n_toys, const double* sta
     mf_fit_opts o;
     if (opts) o = *opts;
     else mf_fit_opts_default(&o);
-    const int K = m->K;
-    std::vector<FitState> st((size_t)n_toys);
-    std::vector<double> lam((size_t)n_toys * K), nll((size_t)n_toys), grad((size_t)n_toys * K);
-    std::vector<uint8_t> active((size_t)n_toys);
-    for (int64_t t = 0; t < n_toys; ++t) st[t].init(K, starts + t * K, fixed, o);
-    for (;;) {
-        int64_t n_active = 0;
-        for (int64_t t = 0; t < n_toys; ++t) {
-            active[t] = st[t].done() ? 0 : 1;
-            if (active[t]) {
-                std::memcpy(&lam[t * K], st[t].request(), sizeof(double) * K);
-                ++n_active;
-            }
-        }
-        if (n_active == 0) break;
-        const mf_status rc = mf_nll_grad_batch(m, n_toys, lam.data(), active.data(), nll.data(), grad.data());
-        if (rc != MF_OK) return rc;
-        for (int64_t t = 0; t < n_toys; ++t)
-            if (active[t]) st[t].feed(std::isfinite(nll[t]), nll[t], &grad[t * K]);
-    }
-    for (int64_t t = 0; t < n_toys; ++t) st[t].result(&results[t]);
-    return MF_OK;
+    if (m->K <= 4) return fit_many<4>(m, n_toys, starts, fixed, o, results);
+    if (m->K <= 8) return fit_many<8>(m, n_toys, starts, fixed, o, results);
+    return fit_many<MF_MAX_PARAMS>(m, n_toys, starts, fixed, o, results);
 }
