@@ -80,3 +80,47 @@ def test_hessian_status(mf, ctx):
     with pytest.raises(mf.MoreFitError) as e:
         model.nll_grad_hess((0.3, 5.28, -1.0, -1.5))
     assert e.value.status == mf.MF_ERR_PARAM_DOMAIN
+
+
+def test_fit_analytic_vs_finite_difference_vs_oracle(mf, ctx):
+    """The Newton fit on the analytic Hessian, the BFGS + finite-difference fit and the oracle's own fit reach the same
+    minimum (1e-6 sigma) and the same covariance; the analytic mode needs far fewer evaluations."""
+    m = dg.gen_mass(10_000, seed=0)
+    model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(m, LO, HI))
+    oa, of = mf.default_fit_opts(), mf.default_fit_opts()
+    assert oa.analytic_hessian == 1
+    of.analytic_hessian = 0
+    ra, rf = model.fit(dg.MASS_START, opts=oa), model.fit(dg.MASS_START, opts=of)
+    o = oracle.fit(oracle.MASS, m, dg.MASS_START, lo=LO, hi=HI)
+    assert ra.converged and rf.converged
+    assert np.max(np.abs(ra.lam - o.lam) / o.sigma) < 1e-6 and np.max(np.abs(rf.lam - o.lam) / o.sigma) < 1e-6
+    assert np.max(np.abs(ra.sigma / o.sigma - 1)) < 1e-6      # analytic covariance vs the oracle's FD covariance
+    assert np.max(np.abs(ra.cov - rf.cov) / np.outer(ra.sigma, ra.sigma)) < 1e-5   # FD Hessian error of the other fit
+    assert ra.n_calls <= 15 < rf.n_calls
+    # fixed parameters work in the analytic mode too
+    fx = np.array([0, 0, 0, 1], dtype=np.uint8)
+    r2 = model.fit(dg.MASS_START, fixed=fx, opts=oa)
+    assert r2.converged and r2.lam[3] == dg.MASS_START[3] and r2.cov[3, 3] == 0.0
+    o2 = oracle.fit(oracle.MASS, m, dg.MASS_START, lo=LO, hi=HI, fixed=fx)
+    assert np.max(np.abs(r2.lam[:3] - o2.lam[:3]) / o2.sigma[:3]) < 1e-6
+
+
+def test_fit_batch_analytic(mf, ctx):
+    T, n = 64, 2000
+    toys = dg.gen_mass_toys(T, n, first_seed=900)
+    model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(toys, LO, HI, n_toys=T))
+    oa, of = mf.default_fit_opts(), mf.default_fit_opts()
+    of.analytic_hessian = 0
+    ra, rf = model.fit_batch(np.array(dg.MASS_TRUTH), opts=oa), model.fit_batch(np.array(dg.MASS_TRUTH), opts=of)
+    assert ra.converged.all() and rf.converged.all()
+    assert np.max(np.abs(ra.lam - rf.lam) / rf.sigma) < 1e-6
+    # the other fit's covariance is a finite-difference Hessian taken up to 1e-3 sigma from the minimum: loose bound
+    assert np.max(np.abs(ra.cov - rf.cov) / (ra.sigma[:, :, None] * ra.sigma[:, None, :])) < 2e-3
+    assert ra.n_calls.mean() < 0.5 * rf.n_calls.mean()
+    for t in (0, 63):
+        o = oracle.fit(oracle.MASS, toys[t], dg.MASS_TRUTH, lo=LO, hi=HI)
+        assert np.max(np.abs(ra[t].lam - o.lam) / o.sigma) < 1e-6
+        # HESSE: the returned covariance is the inverse of the (oracle's) analytic Hessian at the fitted point
+        _, _, H, _ = oracle.nll_grad_hess(oracle.MASS, toys[t], ra[t].lam, LO, HI)
+        c = np.linalg.inv(H)
+        assert np.max(np.abs(ra[t].cov - c) / np.outer(ra[t].sigma, ra[t].sigma)) < 1e-7
