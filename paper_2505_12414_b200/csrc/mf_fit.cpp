@@ -10,6 +10,11 @@
 //   3. polish: central-difference Hessian, Newton steps with it until
 //      max_k |step_k| / sigma_k < polish_tol; cov = H^-1 (the HESSE matrix).
 //
+// Where the model family has the analytic Hessian kernel (mf_model_has_hessian) and opts->analytic_hessian is set, every
+// evaluation also returns d2(-ln L): steps 1 and 3 need no finite differences, step 2 uses the Newton metric of the
+// accepted point (BFGS update only if that Hessian is not positive definite), and cov is the inverse of the Hessian at the
+// final point.
+//
 // It is written as a resumable state machine (one FitState per fit: "give me the next point
 // to evaluate" / "here is the value and gradient there") so that the same code drives one fit
 // through mf_nll_grad and T concurrent toy fits through ONE mf_nll_grad_batch launch per round.
