@@ -155,11 +155,13 @@ mf_status mf_nll_grad_batch_async(mf_model* model, int64_t n_toys, const double*
 
 /* ---- value + gradient + analytic Hessian ---------------------- */
 
-/* 1 if the model family has the analytic Hessian kernel (this round: MF_MASS_GAUSS_EXP), else 0. */
+/* 1 if the model family has the analytic Hessian kernel (MF_MASS_GAUSS_EXP, MF_ANGULAR_KSTMUMU), else 0
+ * (MF_MASS_X_ANGULAR: the fit driver then uses finite differences of the gradient). */
 int mf_model_has_hessian(const mf_model* model);
 
 /* As mf_nll_grad, plus hess (host, K*K doubles, row-major, symmetric) = d2(-ln L)/d lambda_k d lambda_l, from one
- * launch that accumulates the second-derivative moment sums beside the value and the gradient.
+ * launch that accumulates the second-derivative sums beside the value and the gradient (mass: seven more moment sums;
+ * angular: the 36 products of the score components).
  * MF_ERR_ARG for a model family without the Hessian kernel; on MF_NONPOSITIVE_PDF hess is NaN. */
 mf_status mf_nll_grad_hess(mf_model* model, const double* lambda, double* nll, double* grad, double* hess);
 

@@ -285,7 +285,7 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
     m->ctx = ctx;
     m->kind = kind;
     m->K = K;
-    m->nacc = (kind == MF_MASS_GAUSS_EXP) ? MassHessModel::NACC : (kind == MF_ANGULAR_KSTMUMU) ? AngularModel::NACC : FourDModel::NACC;
+    m->nacc = (kind == MF_MASS_GAUSS_EXP) ? MassHessModel::NACC : (kind == MF_ANGULAR_KSTMUMU) ? AngularHessModel::NACC : FourDModel::NACC;
     m->ncol = ncol;
     m->n_events = ds->n_events;
     m->n_pad = ds->n_pad;
@@ -368,7 +368,7 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
         MF_CUDA_M(dev_alloc(ctx, &m->d_consts, sizeof(FourDConsts) * T));  // the largest Consts
         MF_CUDA_M(dev_alloc(ctx, &m->d_consts_ok, sizeof(int) * T));
         MF_CUDA_M(dev_alloc(ctx, &m->d_ids, sizeof(int) * T));
-        const int nout1 = (kind == MF_MASS_GAUSS_EXP ? MassHessModel::NOUT : K + 1) + 1;  // widest output row + n_bad
+        const int nout1 = (kind == MF_MASS_GAUSS_EXP ? MassHessModel::NOUT : kind == MF_ANGULAR_KSTMUMU ? AngularHessModel::NOUT : K + 1) + 1;  // widest output row + n_bad
         MF_CUDA_M(dev_alloc(ctx, &m->d_bout, sizeof(double) * T * nout1));
         MF_CUDA_M(cudaHostAlloc(&m->h_lam, sizeof(double) * T * K, cudaHostAllocDefault));
         MF_CUDA_M(cudaHostAlloc(&m->h_ids, sizeof(int) * T, cudaHostAllocDefault));
@@ -431,6 +431,11 @@ bool host_consts<AngularModel>(const mf_model*, const double* lam, AngularConsts
     return angular_consts(lam, c);
 }
 template <>
+bool host_consts<AngularHessModel>(const mf_model*, const double* lam, AngularConsts& c)
+{
+    return angular_consts(lam, c);
+}
+template <>
 bool host_consts<FourDModel>(const mf_model* m, const double* lam, FourDConsts& c)
 {
     return fourd_consts(lam, m->ma, m->mb, c);
@@ -456,7 +461,7 @@ static mf_status launch_single(mf_model* m, const double* lam, double* out_dev, 
     a.gen = m->gen + slot;
     a.need = m->seq / kRing;
     a.out = out_dev;
-    a.done_flag = signal_host ? reinterpret_cast<unsigned long long*>(m->d_out_mapped + MF_MAX_PARAMS + 2) : nullptr;
+    a.done_flag = signal_host ? reinterpret_cast<unsigned long long*>(m->d_out_mapped + MF_HOST_DONE_INDEX) : nullptr;
     a.done_value = m->seq + 1;
     const int grid = (pipelined && M::CTAS_PER_SM > 1 && m->grid > ctx->sm_count) ? std::max(ctx->sm_count, m->grid / 2) : m->grid;
     MF_CUDA(ctx, launch_pdl(nll_grad_kernel<M>, grid, ctx->stream, a));
@@ -469,9 +474,9 @@ static mf_status dispatch_single(mf_model* m, const double* lam, double* out_dev
                                  bool signal_host = false, bool hess = false)
 {
     if (hess) {
-        if (m->kind != MF_MASS_GAUSS_EXP)
-            return mf_fail(m->ctx, MF_ERR_ARG, "the analytic Hessian is implemented for MF_MASS_GAUSS_EXP only");
-        return launch_single<MassHessModel>(m, lam, out_dev, pipelined, signal_host);
+        if (m->kind == MF_MASS_GAUSS_EXP) return launch_single<MassHessModel>(m, lam, out_dev, pipelined, signal_host);
+        if (m->kind == MF_ANGULAR_KSTMUMU) return launch_single<AngularHessModel>(m, lam, out_dev, false, signal_host);
+        return mf_fail(m->ctx, MF_ERR_ARG, "no analytic Hessian kernel for this model family (MF_MASS_X_ANGULAR)");
     }
     switch (m->kind) {
     case MF_MASS_GAUSS_EXP: return launch_single<MassModel>(m, lam, out_dev, pipelined, signal_host);
@@ -571,7 +576,7 @@ static mf_status eval_sync(mf_model* m, const double* lambda, double* nll, doubl
     // done word (a stream synchronise costs ~20 us of driver latency per call, the kernel 4-30 us)
     const mf_status st = dispatch_single(m, lambda, m->d_out_mapped, false, true, hess != nullptr);
     if (st != MF_OK) return st;
-    volatile unsigned long long* done = reinterpret_cast<volatile unsigned long long*>(m->h_out + MF_MAX_PARAMS + 2);
+    volatile unsigned long long* done = reinterpret_cast<volatile unsigned long long*>(m->h_out + MF_HOST_DONE_INDEX);
     const unsigned long long want = m->seq;
     for (unsigned spins = 1; *done != want; ++spins) {
         if ((spins & 0xFFFF) == 0) {  // every ~65k polls: make sure the stream is still alive
@@ -585,7 +590,7 @@ static mf_status eval_sync(mf_model* m, const double* lambda, double* nll, doubl
     std::atomic_thread_fence(std::memory_order_acquire);
     *nll = m->h_out[0];
     if (grad) std::memcpy(grad, m->h_out + 1, sizeof(double) * K);
-    const int nout = hess ? MassHessModel::NOUT : K + 1;
+    const int nout = hess ? 1 + K + K * (K + 1) / 2 : K + 1;
     if (hess) {
         int q = 1 + K;
         for (int i = 0; i < K; ++i)
@@ -611,7 +616,10 @@ extern "C" mf_status mf_nll_grad_hess(mf_model* m, const double* lambda, double*
     return eval_sync(m, lambda, nll, grad, hess, "mf_nll_grad_hess");
 }
 
-extern "C" int mf_model_has_hessian(const mf_model* m) { return m && m->kind == MF_MASS_GAUSS_EXP ? 1 : 0; }
+extern "C" int mf_model_has_hessian(const mf_model* m)
+{
+    return m && (m->kind == MF_MASS_GAUSS_EXP || m->kind == MF_ANGULAR_KSTMUMU) ? 1 : 0;
+}
 
 template <class M>
 static mf_status launch_batch(mf_model* m, int n_active, const double* lam_dev = nullptr, double* out_dev = nullptr)
@@ -661,8 +669,8 @@ static mf_status eval_batch(mf_model* m, int64_t n_toys, const double* lambdas, 
     mf_ctx* ctx = m->ctx;
     const int K = m->K;
     if (n_toys != m->n_toys) return mf_fail(ctx, MF_ERR_ARG, std::string(who) + ": n_toys does not match the dataset");
-    if (hess && m->kind != MF_MASS_GAUSS_EXP)
-        return mf_fail(ctx, MF_ERR_ARG, "the analytic Hessian is implemented for MF_MASS_GAUSS_EXP only");
+    if (hess && !mf_model_has_hessian(m))
+        return mf_fail(ctx, MF_ERR_ARG, "no analytic Hessian kernel for this model family (MF_MASS_X_ANGULAR)");
     if (m->n_toys < 2 && !m->d_lam) {
         // a 1-toy dataset evaluated through the batch entry: same result as the single call
         if (active && !active[0]) return MF_OK;
@@ -690,7 +698,7 @@ static mf_status eval_batch(mf_model* m, int64_t n_toys, const double* lambdas, 
         MF_CUDA(ctx, cudaMemcpyAsync(m->d_ids, m->h_ids, sizeof(int) * n_active, cudaMemcpyHostToDevice, ctx->stream));
     mf_status st;
     if (hess) {
-        st = launch_batch<MassHessModel>(m, n_active);
+        st = (m->kind == MF_MASS_GAUSS_EXP) ? launch_batch<MassHessModel>(m, n_active) : launch_batch<AngularHessModel>(m, n_active);
     } else {
         switch (m->kind) {
         case MF_MASS_GAUSS_EXP: st = launch_batch<MassModel>(m, n_active); break;
@@ -699,7 +707,7 @@ static mf_status eval_batch(mf_model* m, int64_t n_toys, const double* lambdas, 
         }
     }
     if (st != MF_OK) return st;
-    const int row = (hess ? MassHessModel::NOUT : K + 1) + 1;
+    const int row = (hess ? 1 + K + K * (K + 1) / 2 : K + 1) + 1;
     MF_CUDA(ctx, cudaMemcpyAsync(m->h_bout, m->d_bout, sizeof(double) * n_active * row, cudaMemcpyDeviceToHost, ctx->stream));
     MF_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     for (int s = 0; s < n_active; ++s) {

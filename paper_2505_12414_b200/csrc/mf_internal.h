@@ -20,7 +20,8 @@ struct mf_ctx {
     std::vector<int> free_slots;
 };
 
-constexpr int MF_HOST_SLOT_DOUBLES = 32;  // >= MF_MAX_PARAMS + 3, 256-byte slots
+constexpr int MF_HOST_SLOT_DOUBLES = 64;  // widest output row (angular Hessian: 45 + n_bad) and the done word
+constexpr int MF_HOST_DONE_INDEX = 63;    // the 64-bit done word of a synchronous call
 constexpr int MF_HOST_SLOTS = 4096;
 
 // Reference-counted device buffer so that a model can outlive the dataset handle.
@@ -61,7 +62,7 @@ struct mf_model {
     unsigned* ticket = nullptr;       // device, kRing (single) + n_toys (batch)
     unsigned long long* gen = nullptr;  // device [kRing]: evaluations completed per scratch slot
     unsigned long long seq = 0;       // evaluations enqueued so far (evaluation e uses slot e % kRing)
-    double* h_out = nullptr;          // pinned + mapped host, MF_MAX_PARAMS+2 doubles, then the 64-bit done word
+    double* h_out = nullptr;          // pinned + mapped host slot: the output row, the 64-bit done word at MF_HOST_DONE_INDEX
     double* d_out_mapped = nullptr;   // device alias of h_out
     // batched evaluation
     int chunks = 1;                   // CTAs per toy

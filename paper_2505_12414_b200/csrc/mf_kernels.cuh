@@ -88,6 +88,11 @@ __device__ __forceinline__ bool make_consts<AngularModel>(const double* lam, dou
     return angular_consts(lam, c);
 }
 template <>
+__device__ __forceinline__ bool make_consts<AngularHessModel>(const double* lam, double, double, AngularConsts& c)
+{
+    return angular_consts(lam, c);
+}
+template <>
 __device__ __forceinline__ bool make_consts<FourDModel>(const double* lam, double ma, double mb, FourDConsts& c)
 {
     return fourd_consts(lam, ma, mb, c);

@@ -465,6 +465,56 @@ struct AngularModel {
     }
 };
 
+// Angular model with the analytic Hessian.  P is linear in its coefficients, so with the score components
+// s_k = h_k / P:  d2 ln P / da_k da_l = -s_k s_l, i.e. d2(-ln L) = sum_i s_k s_l (positive semi-definite: -ln L is convex).
+// 36 more sums than AngularModel; still one pass over the nine cached columns.
+// Output: -ln L, gradient[8], then the upper triangle (k <= l, row by row) of d2(-ln L).
+struct AngularHessModel {
+    static constexpr int K = 8;
+    static constexpr int NCOL = 9;
+    static constexpr int NOUT = 1 + 8 + 36;
+    static constexpr int NACC = 1 + 8 + 36;
+    static constexpr int ITEMS_PER_ITER = 1;
+    static constexpr int PREFETCH = 0;
+    static constexpr int CTAS_PER_SM = 1;
+    static constexpr int RESIDENT_CTAS = 1;  // 45 sums + two 9-column register buffers
+    static constexpr int BATCH_RESIDENT_CTAS = 1;
+    static constexpr int BATCH_BLOCK = 256;
+    using Consts = AngularConsts;
+
+    template <bool PRED>
+    static MF_D void event(const double* x, const Consts& c, double* acc, LogProd& lp, unsigned& bad, bool valid,
+                           double)
+    {
+        double P = fma(c.a[0], x[1], x[0]);
+#pragma unroll
+        for (int k = 1; k < 8; ++k) P = fma(c.a[k], x[1 + k], P);
+        const double r = mf_rcp(P);
+        if (!PRED || valid) {
+            lp.mul(P, bad);
+            double s[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                s[k] = x[1 + k] * r;
+                acc[1 + k] += s[k];
+            }
+            int q = 9;
+#pragma unroll
+            for (int k = 0; k < 8; ++k)
+#pragma unroll
+                for (int l = k; l < 8; ++l, ++q) acc[q] = fma(s[k], s[l], acc[q]);
+        }
+    }
+
+    static MF_D void finish(const Consts&, const double* s, double, double, double* out)
+    {
+#pragma unroll
+        for (int k = 0; k < 9; ++k) out[k] = -s[k];
+#pragma unroll
+        for (int k = 9; k < NOUT; ++k) out[k] = s[k];
+    }
+};
+
 struct FourDModel {
     static constexpr int K = 16;
     static constexpr int NCOL = 12;  // m, cos theta_l, cos theta_K, h_0..h_8

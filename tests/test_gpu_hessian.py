@@ -69,12 +69,13 @@ def test_mass_hessian_batch_parity(mf, ctx):
 
 
 def test_hessian_status(mf, ctx):
-    ev = dg.gen_angular(1000, seed=2)
-    amodel = ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ctx.dataset_upload(ev))
-    assert not amodel.has_hessian
+    ev = dg.gen_4d(1000, seed=3)
+    amodel = ctx.model_create(mf.MF_MASS_X_ANGULAR, ctx.dataset_upload(ev, LO, HI))
+    assert not amodel.has_hessian                 # no Hessian kernel for the 4D family: the fit uses finite differences
     with pytest.raises(mf.MoreFitError) as e:
-        amodel.nll_grad_hess(dg.ANG_TRUTH)
+        amodel.nll_grad_hess(dg.FOURD_TRUTH)
     assert e.value.status == mf.MF_ERR_ARG
+    assert amodel.fit(dg.FOURD_TRUTH).converged
     m = dg.gen_mass(1000, seed=0)
     model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(m, LO, HI))
     with pytest.raises(mf.MoreFitError) as e:
@@ -124,3 +125,35 @@ def test_fit_batch_analytic(mf, ctx):
         _, _, H, _ = oracle.nll_grad_hess(oracle.MASS, toys[t], ra[t].lam, LO, HI)
         c = np.linalg.inv(H)
         assert np.max(np.abs(ra[t].cov - c) / np.outer(ra[t].sigma, ra[t].sigma)) < 1e-7
+
+
+@pytest.mark.parametrize("n", [20_000, 20_011, 37])
+def test_angular_hessian_parity(mf, ctx, n):
+    ev = dg.gen_angular(n, seed=31)
+    model = ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ctx.dataset_upload(ev))
+    assert model.has_hessian
+    for lam in (dg.ANG_TRUTH, (0.55, 0.03, -0.1, -0.25, 0.02, 0.04, -0.05, 0.03)):
+        nll, g, H = model.nll_grad_hess(lam)
+        o_nll, o_g, o_H, bad = oracle.nll_grad_hess(oracle.ANGULAR, ev, lam)
+        assert bad == 0
+        check(nll, g, H, o_nll, o_g, o_H, f"angular n={n}")
+
+
+def test_angular_hessian_batch_and_fit(mf, ctx):
+    T, n = 3, 4000
+    ev = np.stack([dg.gen_angular(n, seed=60 + t) for t in range(T)], axis=1)  # [3][T][n]
+    model = ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ctx.dataset_upload(ev, n_toys=T))
+    lams = np.tile(np.array(dg.ANG_TRUTH), (T, 1))
+    lams[1, 0] = 0.5
+    nll, g, H = model.nll_grad_hess_batch(lams)
+    for t in range(T):
+        o_nll, o_g, o_H, _ = oracle.nll_grad_hess(oracle.ANGULAR, ev[:, t, :], lams[t])
+        check(nll[t], g[t], H[t], o_nll, o_g, o_H, f"angular toy {t}")
+    # the analytic-mode fit of one dataset against the oracle's fit
+    one = dg.gen_angular(50_000, seed=2)
+    m1 = ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ctx.dataset_upload(one))
+    r = m1.fit(dg.ANG_TRUTH)
+    o = oracle.fit(oracle.ANGULAR, one, dg.ANG_TRUTH)
+    assert r.converged and np.max(np.abs(r.lam - o.lam) / o.sigma) < 1e-6
+    assert np.max(np.abs(r.sigma / o.sigma - 1)) < 1e-5
+    assert r.n_calls <= 12
