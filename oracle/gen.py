@@ -1,0 +1,76 @@
+"""CPU ORACLE of the on-device pseudo-data generator (accept-reject /
+inverse-CDF generation with a counter-based per-work-item RNG) — TEST INFRASTRUCTURE ONLY, like the rest of oracle/.
+
+The recipe, followed step by step, one event at a time:
+
+  RNG     Philox4x32-10 (Salmon et al., "Parallel random numbers: as easy as 1, 2, 3", SC'11), written out below.
+          key = (seed mod 2^32, seed >> 32) with seed = seed0 + toy; counter = (event mod 2^32, event >> 32, draw, 0).
+          One call gives four 32-bit words w0..w3 = two uniforms  u = ((w_hi * 2^32 + w_lo) >> 11 + 1/2) * 2^-53  in (0, 1).
+  event   draw 0: (uA, uB).  Signal if uA < f, else background.
+          background:  m = lo + log1p(uB * expm1(tau w)) / tau   (tau != 0),  lo + uB w  (tau == 0),  w = hi - lo; clamped to [lo, hi].
+          signal: draws k = 1, 2, ...: (u1, u2), z = sqrt(-2 ln u1) cos(2 pi u2), m = mu + sigma z; the first m in [lo, hi] is taken
+          (after 64 rejected draws the last m is clamped into the range).
+
+The CUDA path implements the same recipe in its own code (mf_generate.cu); uniform words are bit-identical, the
+floating-point transforms agree to a few ulp.  Pins (tests/test_oracle_gen.py): the published Philox4x32-10 known-answer
+vectors; Kolmogorov-Smirnov distance of generated samples to the closed-form CDF of Eq. 2.
+"""
+from __future__ import annotations
+
+import math
+
+import numpy as np
+
+_M0, _M1 = 0xD2511F53, 0xCD9E8D57
+_W0, _W1 = 0x9E3779B9, 0xBB67AE85
+_MASK = 0xFFFFFFFF
+
+
+def philox4x32_10(counter, key):
+    """counter: 4 ints, key: 2 ints (32-bit each) -> 4 ints."""
+    c0, c1, c2, c3 = [int(x) & _MASK for x in counter]
+    k0, k1 = [int(x) & _MASK for x in key]
+    for _ in range(10):
+        p0 = _M0 * c0
+        p1 = _M1 * c2
+        hi0, lo0 = p0 >> 32, p0 & _MASK
+        hi1, lo1 = p1 >> 32, p1 & _MASK
+        c0, c1, c2, c3 = (hi1 ^ c1 ^ k0) & _MASK, lo1, (hi0 ^ c3 ^ k1) & _MASK, lo0
+        k0, k1 = (k0 + _W0) & _MASK, (k1 + _W1) & _MASK
+    return c0, c1, c2, c3
+
+
+def _uniform(w_hi: int, w_lo: int) -> float:
+    return (((w_hi << 32) | w_lo) >> 11) * 2.0 ** -53 + 2.0 ** -54
+
+
+def uniforms(seed: int, event: int, draw: int):
+    w = philox4x32_10((event & _MASK, event >> 32, draw, 0), (seed & _MASK, seed >> 32))
+    return _uniform(w[0], w[1]), _uniform(w[2], w[3])
+
+
+def gen_mass_event(seed: int, event: int, lam, lo: float, hi: float):
+    """(m, is_signal, number of draws used) of one event."""
+    f, mu, sigma, tau = [float(x) for x in lam]
+    ua, ub = uniforms(seed, event, 0)
+    if ua < f:
+        m = mu
+        for k in range(1, 65):
+            u1, u2 = uniforms(seed, event, k)
+            z = math.sqrt(-2.0 * math.log(u1)) * math.cos(2.0 * math.pi * u2)
+            m = mu + sigma * z
+            if lo <= m <= hi:
+                return m, True, k + 1
+        return min(max(m, lo), hi), True, 65
+    w = hi - lo
+    m = lo + ub * w if tau == 0.0 else lo + math.log1p(ub * math.expm1(tau * w)) / tau
+    return min(max(m, lo), hi), False, 1
+
+
+def gen_mass_toys(seed0: int, n_toys: int, n_events: int, lam, lo: float, hi: float) -> np.ndarray:
+    """[n_toys][n_events]: toy t uses seed0 + t."""
+    out = np.empty((n_toys, n_events))
+    for t in range(n_toys):
+        for i in range(n_events):
+            out[t, i] = gen_mass_event(seed0 + t, i, lam, lo, hi)[0]
+    return out
