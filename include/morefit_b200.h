@@ -99,6 +99,18 @@ void mf_dataset_destroy(mf_dataset* ds);
 int64_t mf_dataset_n_events(const mf_dataset* ds);
 int64_t mf_dataset_n_toys(const mf_dataset* ds);
 
+/* ---- on-device generation of pseudo-experiments ------------------------- */
+
+/* Generates n_toys pseudo-experiments of n_events events each of the Gaussian + exponential mass model at lambda =
+ * (f, mu, sigma, tau) on [lo, hi], directly into a device dataset (ndim = 1; use it with mf_model_create).  Toy t uses the
+ * counter-based stream Philox4x32-10 keyed by seed0 + t; event i is a pure function of (seed0 + t, i), whatever the launch
+ * geometry.  Recipe: mf_generate.cu.  lam: host, 4 doubles.  MF_ERR_PARAM_DOMAIN as for the mass model. */
+mf_status mf_generate_mass(mf_ctx* ctx, uint64_t seed0, int64_t n_toys, int64_t n_events, const double* lam, double lo,
+                           double hi, mf_dataset** out);
+
+/* Copies a dataset's events to the host: dst [ndim][n_toys][n_events] doubles. */
+mf_status mf_dataset_download(const mf_dataset* ds, double* dst);
+
 /* ---- S1: model (event-only precompute, Listing 4) --- */
 
 /* Binds a model family to a dataset (ndim must match the kind) and runs the event-only

@@ -32,7 +32,7 @@ _STATUS_NAMES = ["MF_OK", "MF_ERR_ARG", "MF_ERR_CUDA", "MF_ERR_OOM", "MF_ERR_DAT
 
 EXPORTS = [
     "mf_ctx_create", "mf_ctx_destroy", "mf_last_error", "mf_ctx_kernel_launches",
-    "mf_dataset_upload", "mf_dataset_destroy", "mf_dataset_n_events", "mf_dataset_n_toys",
+    "mf_dataset_upload", "mf_generate_mass", "mf_dataset_download", "mf_dataset_destroy", "mf_dataset_n_events", "mf_dataset_n_toys",
     "mf_model_create", "mf_model_destroy", "mf_model_nparams", "mf_model_n_events", "mf_model_n_toys",
     "mf_nll_grad", "mf_nll_grad_async", "mf_nll_grad_points", "mf_nll_grad_batch", "mf_nll_grad_batch_async",
     "mf_model_has_hessian", "mf_nll_grad_hess", "mf_nll_grad_hess_batch",
@@ -140,6 +140,10 @@ def load_library() -> ctypes.CDLL:
     lib.mf_dataset_upload.restype = ctypes.c_int
     lib.mf_dataset_upload.argtypes = [vp, ctypes.c_int, i64, i64, ctypes.POINTER(vp), ctypes.c_int, dp, dp,
                                       ctypes.POINTER(vp)]
+    lib.mf_generate_mass.restype = ctypes.c_int
+    lib.mf_generate_mass.argtypes = [vp, ctypes.c_uint64, i64, i64, dp, ctypes.c_double, ctypes.c_double, ctypes.POINTER(vp)]
+    lib.mf_dataset_download.restype = ctypes.c_int
+    lib.mf_dataset_download.argtypes = [vp, dp]
     lib.mf_dataset_destroy.restype = None
     lib.mf_dataset_destroy.argtypes = [vp]
     lib.mf_dataset_n_events.restype = i64
@@ -251,6 +255,17 @@ class Context:
         ndim = 1 with n_toys > 1), or a list of CUDA torch tensors (device pointers, one per dimension)."""
         return Dataset(self, columns, lo, hi, n_toys)
 
+    def generate_mass(self, seed0: int, n_toys: int, n_events: int, lam, lo: float, hi: float) -> "Dataset":
+        """n_toys pseudo-experiments of the mass model generated on the device (no host copy)."""
+        lam = np.ascontiguousarray(lam, dtype=np.float64)
+        ds = Dataset.__new__(Dataset)
+        ds._ctx, ds._lib, ds._h = self, self._lib, ctypes.c_void_p()
+        self._check(self._lib.mf_generate_mass(self._h, int(seed0), int(n_toys), int(n_events), _dp(lam), float(lo), float(hi),
+                                               ctypes.byref(ds._h)))
+        self._children.add(ds)
+        ds.ndim, ds.n_events, ds.n_toys = 1, int(n_events), int(n_toys)
+        return ds
+
     def model_create(self, kind: int, dataset: "Dataset") -> "Model":
         return Model(self, kind, dataset)
 
@@ -307,6 +322,12 @@ class Dataset:
         ctx._check(st)
         ctx._children.add(self)
         self.ndim, self.n_events, self.n_toys = ndim, total // n_toys, int(n_toys)
+
+    def download(self) -> np.ndarray:
+        """The events as a host array [ndim][n_toys][n_events]."""
+        out = np.empty((self.ndim, self.n_toys, self.n_events), dtype=np.float64)
+        self._ctx._check(self._lib.mf_dataset_download(self._h, _dp(out)))
+        return out
 
     def close(self):
         if self._h:

@@ -1,0 +1,154 @@
+// mf_generate.cu — on-device generation of mass-model pseudo-experiments ("a small-state
+// RNG per work item ... events generated on the accelerator", half of the paper's per-toy time at 1M events).
+//
+// Counter-based instead of the paper's jump-seeded Xoshiro streams: event i of toy t draws from Philox4x32-10 with
+// key = seed0 + t and counter = (i, draw), so any thread can generate any event and the result does not depend on the
+// launch geometry.  Recipe (restated independently in oracle/gen.py, which is test infrastructure):
+//   draw 0 -> (uA, uB); signal if uA < f, else background m = lo + log1p(uB expm1(tau w)) / tau  (lo + uB w at tau == 0);
+//   signal: draws 1, 2, ... -> Box-Muller z = sqrt(-2 ln u1) cos(2 pi u2), m = mu + sigma z, first m inside [lo, hi]
+//   (after 64 rejected draws the last one is clamped).  u = ((w_hi 2^32 + w_lo) >> 11 + 1/2) 2^-53.
+// The events are written straight into the dataset's padded structure of arrays: no host copy.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <new>
+#include <string>
+
+#include "mf_internal.h"
+
+namespace {
+
+__device__ __forceinline__ void philox4x32_10(unsigned c0, unsigned c1, unsigned c2, unsigned c3, unsigned k0, unsigned k1,
+                                              unsigned (&out)[4])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const unsigned hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const unsigned hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        const unsigned n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0;
+        c1 = lo1;
+        c2 = n2;
+        c3 = lo0;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0;
+    out[1] = c1;
+    out[2] = c2;
+    out[3] = c3;
+}
+
+__device__ __forceinline__ double uniform53(unsigned hi, unsigned lo)
+{
+    const unsigned long long x = (((unsigned long long)hi << 32) | lo) >> 11;
+    return (double)x * 0x1p-53 + 0x1p-54;
+}
+
+__device__ __forceinline__ void uniforms(unsigned long long seed, unsigned long long event, unsigned draw, double& ua, double& ub)
+{
+    unsigned w[4];
+    philox4x32_10((unsigned)event, (unsigned)(event >> 32), draw, 0u, (unsigned)seed, (unsigned)(seed >> 32), w);
+    ua = uniform53(w[0], w[1]);
+    ub = uniform53(w[2], w[3]);
+}
+
+// data: [n_toys][n_pad]; the padding of each toy row repeats its last event (as mf_dataset_upload does)
+__global__ void __launch_bounds__(256) generate_mass_kernel(double* __restrict__ data, int64_t n_toys, int64_t n, int64_t n_pad,
+                                                            unsigned long long seed0, double f, double mu, double sigma,
+                                                            double tau, double lo, double hi, double em1)
+{
+    const double w = hi - lo;
+    for (int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; idx < n_toys * n_pad; idx += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t toy = idx / n_pad, slot = idx % n_pad;
+        if (n == 0) {
+            data[idx] = 0.0;
+            continue;
+        }
+        const unsigned long long ev = (unsigned long long)(slot < n ? slot : n - 1), seed = seed0 + (unsigned long long)toy;
+        double ua, ub, m;
+        uniforms(seed, ev, 0u, ua, ub);
+        if (ua < f) {
+            m = mu;
+            bool ok = false;
+            for (unsigned k = 1; k <= 64 && !ok; ++k) {
+                double u1, u2;
+                uniforms(seed, ev, k, u1, u2);
+                const double z = sqrt(-2.0 * log(u1)) * cos(2.0 * 3.141592653589793238462643383279502884 * u2);
+                m = fma(sigma, z, mu);
+                ok = (m >= lo && m <= hi);
+            }
+            if (!ok) m = fmin(fmax(m, lo), hi);
+        } else {
+            m = (tau == 0.0) ? fma(ub, w, lo) : lo + log1p(ub * em1) / tau;
+            m = fmin(fmax(m, lo), hi);
+        }
+        data[idx] = m;
+    }
+}
+
+}  // namespace
+
+extern "C" mf_status mf_generate_mass(mf_ctx* ctx, uint64_t seed0, int64_t n_toys, int64_t n_events, const double* lam,
+                                      double lo, double hi, mf_dataset** out)
+{
+    if (!ctx || !lam || !out) return mf_fail(ctx, MF_ERR_ARG, "mf_generate_mass: NULL argument");
+    if (n_toys < 1 || n_events < 0 || !(std::isfinite(lo) && std::isfinite(hi) && lo < hi))
+        return mf_fail(ctx, MF_ERR_ARG, "mf_generate_mass: n_toys >= 1, n_events >= 0 and a finite range lo < hi are required");
+    const double f = lam[0], mu = lam[1], sigma = lam[2], tau = lam[3];
+    if (!(std::isfinite(f) && std::isfinite(mu) && std::isfinite(sigma) && std::isfinite(tau)) || !(f >= 0.0 && f <= 1.0) ||
+        !(sigma > 0.0) || !std::isfinite(std::expm1(tau * (hi - lo))))
+        return mf_fail(ctx, MF_ERR_PARAM_DOMAIN, "mf_generate_mass: lambda outside the parameter domain");
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return mf_fail(ctx, MF_ERR_CUDA, "mf_generate_mass: cudaSetDevice failed");
+    mf_dataset* ds = new (std::nothrow) mf_dataset();
+    mf_devbuf* buf = new (std::nothrow) mf_devbuf();
+    if (!ds || !buf) {
+        delete ds;
+        delete buf;
+        return mf_fail(ctx, MF_ERR_OOM, "mf_generate_mass: host allocation failed");
+    }
+    ds->ctx = ctx;
+    ds->ndim = 1;
+    ds->n_events = n_events;
+    ds->n_pad = (n_events + 63) / 64 * 64;
+    ds->n_toys = n_toys;
+    ds->lo[0] = lo;
+    ds->hi[0] = hi;
+    ds->raw = buf;
+    buf->stream = ctx->stream;
+    const int64_t total = ds->n_pad * n_toys;
+    buf->bytes = (size_t)(total > 0 ? total : 1) * sizeof(double);
+    cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&buf->p), buf->bytes, ctx->stream);
+    if (e == cudaSuccess && total > 0) {
+        const int grid = (int)std::min<int64_t>((total + 255) / 256, 32 * (int64_t)ctx->sm_count);
+        generate_mass_kernel<<<grid, 256, 0, ctx->stream>>>(buf->p, n_toys, n_events, ds->n_pad, seed0, f, mu, sigma, tau, lo, hi,
+                                                             std::expm1(tau * (hi - lo)));
+        ++ctx->launches;
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) {
+        if (buf->p) cudaFreeAsync(buf->p, ctx->stream);
+        delete buf;
+        delete ds;
+        return mf_fail(ctx, e == cudaErrorMemoryAllocation ? MF_ERR_OOM : MF_ERR_CUDA, std::string("mf_generate_mass: ") + cudaGetErrorString(e));
+    }
+    *out = ds;
+    return MF_OK;
+}
+
+// Copies the events of a dataset back to the host (dst: [ndim][n_toys][n_events], dimension-major) — for tests and for
+// users who want to inspect generated pseudo-data.
+extern "C" mf_status mf_dataset_download(const mf_dataset* ds, double* dst)
+{
+    if (!ds || !dst) return MF_ERR_ARG;
+    mf_ctx* ctx = ds->ctx;
+    if (ds->n_events == 0) return MF_OK;
+    const cudaError_t e = cudaMemcpy2DAsync(dst, (size_t)ds->n_events * sizeof(double), ds->raw->p, (size_t)ds->n_pad * sizeof(double),
+                                            (size_t)ds->n_events * sizeof(double), (size_t)(ds->n_toys * ds->ndim),
+                                            cudaMemcpyDeviceToHost, ctx->stream);
+    if (e != cudaSuccess) return mf_fail(ctx, MF_ERR_CUDA, std::string("mf_dataset_download: ") + cudaGetErrorString(e));
+    if (cudaStreamSynchronize(ctx->stream) != cudaSuccess) return mf_fail(ctx, MF_ERR_CUDA, "mf_dataset_download: synchronise failed");
+    return MF_OK;
+}
