@@ -118,3 +118,25 @@ def test_c4_full_size(mf, ctx):
     for t in (5, 3000):
         o = oracle.fit(oracle.MASS, toys[t], dg.MASS_TRUTH, lo=dg.MASS_LO, hi=dg.MASS_HI)
         assert np.max(np.abs(res[t].lam - o.lam) / o.sigma) < 1e-6
+
+
+def test_beyond_4gib_of_events(mf, ctx):
+    """Maximum sizes: one dataset of 5.5e8 events (4.4 GB: element and byte offsets beyond 2^32), generated on the device,
+    evaluated by the lone kernel and the points-mode kernel, and checked against the oracle on the downloaded events."""
+    import torch
+    n = 550_000_000
+    ds = ctx.generate_mass(31, 1, n, dg.MASS_TRUTH, dg.MASS_LO, dg.MASS_HI)
+    model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ds)
+    lam = (0.31, 5.2801, 0.0201, -1.45)
+    nll, g = model.nll_grad(lam)
+    x = ds.download()[0, 0]
+    assert x.size == n and np.all((x >= dg.MASS_LO) & (x <= dg.MASS_HI))
+    o_nll, o_g, bad = oracle.nll_grad(oracle.MASS, x, lam, dg.MASS_LO, dg.MASS_HI, nthreads=oracle.max_threads())
+    assert bad == 0
+    check(nll, g, o_nll, o_g, "5.5e8 events")
+    pts = np.tile(np.array(lam), (16, 1))
+    out = torch.zeros((16, 6), dtype=torch.float64, device="cuda")
+    model.nll_grad_points(pts, out.data_ptr())
+    torch.cuda.synchronize()
+    r = out.cpu().numpy()
+    check(r[15, 0], r[15, 1:5], o_nll, o_g, "5.5e8 events, points mode")
