@@ -108,6 +108,11 @@ int64_t mf_dataset_n_toys(const mf_dataset* ds);
 mf_status mf_generate_mass(mf_ctx* ctx, uint64_t seed0, int64_t n_toys, int64_t n_events, const double* lam, double lo,
                            double hi, mf_dataset** out);
 
+/* The same for the angular model (ndim = 3): accept-reject of uniform proposals in (cos theta_l, cos theta_K, phi) under
+ * the paper's get_max() envelope 9/(32 pi) (4 + sum |S_i| + 4/3 |AFB|), flat acceptance; proposal k of an
+ * event uses the draws 2k and 2k+1 of its Philox stream.  a: host, the 8 coefficients FL, S3, S4, S5, AFB, S7, S8, S9. */
+mf_status mf_generate_angular(mf_ctx* ctx, uint64_t seed0, int64_t n_toys, int64_t n_events, const double* a, mf_dataset** out);
+
 /* Copies a dataset's events to the host: dst [ndim][n_toys][n_events] doubles. */
 mf_status mf_dataset_download(const mf_dataset* ds, double* dst);
 

@@ -74,3 +74,53 @@ def gen_mass_toys(seed0: int, n_toys: int, n_events: int, lam, lo: float, hi: fl
         for i in range(n_events):
             out[t, i] = gen_mass_event(seed0 + t, i, lam, lo, hi)[0]
     return out
+
+
+# ---------------------------------------------------------------- angular model (Eq. 4), accept-reject
+#
+#   proposal k = 0, 1, ... of event i uses draws 2k and 2k+1:  (u1, u2) -> cos theta_l = 2 u1 - 1, cos theta_K = 2 u2 - 1;
+#   (u3, u4) -> phi = pi (2 u3 - 1), accepted if u4 * pmax < P(Omega), pmax = the paper's get_max() bound
+#   9/(32 pi) (4 + sum |S_i| + 4/3 |AFB|).  The first accepted proposal is the event (after 4096
+#   rejected proposals the last one is taken: unreachable in practice, the efficiency is >= 10 %).
+#   P(Omega) is Eq. 4 written out term by term, here in Python, in the CUDA path in mf_generate.cu.
+
+def angular_pdf(cl: float, ck: float, phi: float, a) -> float:
+    FL, S3, S4, S5, AFB, S7, S8, S9 = [float(x) for x in a]
+    cos2_l, cos2_k = cl * cl, ck * ck
+    sin2_l, sin2_k = 1.0 - cos2_l, 1.0 - cos2_k
+    sin_l, sin_k = math.sqrt(sin2_l), math.sqrt(sin2_k)
+    cos2theta_l = 2.0 * cos2_l - 1.0
+    sin2theta_l, sin2theta_k = 2.0 * sin_l * cl, 2.0 * sin_k * ck
+    return 9.0 / (32.0 * math.pi) * (
+        0.75 * (1.0 - FL) * sin2_k + FL * cos2_k + 0.25 * (1.0 - FL) * sin2_k * cos2theta_l - FL * cos2_k * cos2theta_l
+        + S3 * sin2_k * sin2_l * math.cos(2.0 * phi) + S4 * sin2theta_k * sin2theta_l * math.cos(phi)
+        + S5 * sin2theta_k * sin_l * math.cos(phi) + (4.0 / 3.0) * AFB * sin2_k * cl
+        + S7 * sin2theta_k * sin_l * math.sin(phi) + S8 * sin2theta_k * sin2theta_l * math.sin(phi)
+        + S9 * sin2_k * sin2_l * math.sin(2.0 * phi))
+
+
+def angular_pmax(a) -> float:
+    FL, S3, S4, S5, AFB, S7, S8, S9 = [float(x) for x in a]
+    return 9.0 / (32.0 * math.pi) * (4.0 + abs(S3) + abs(S4) + abs(S5) + 4.0 / 3.0 * abs(AFB) + abs(S7) + abs(S8) + abs(S9))
+
+
+def gen_angular_event(seed: int, event: int, a):
+    """((cos theta_l, cos theta_K, phi), number of proposals) of one event."""
+    pmax = angular_pmax(a)
+    cl = ck = phi = 0.0
+    for k in range(4096):
+        u1, u2 = uniforms(seed, event, 2 * k)
+        u3, u4 = uniforms(seed, event, 2 * k + 1)
+        cl, ck, phi = 2.0 * u1 - 1.0, 2.0 * u2 - 1.0, math.pi * (2.0 * u3 - 1.0)
+        if u4 * pmax < angular_pdf(cl, ck, phi, a):
+            return (cl, ck, phi), k + 1
+    return (cl, ck, phi), 4096
+
+
+def gen_angular_toys(seed0: int, n_toys: int, n_events: int, a) -> np.ndarray:
+    """[3][n_toys][n_events]"""
+    out = np.empty((3, n_toys, n_events))
+    for t in range(n_toys):
+        for i in range(n_events):
+            out[:, t, i] = gen_angular_event(seed0 + t, i, a)[0]
+    return out

@@ -88,7 +88,107 @@ __global__ void __launch_bounds__(256) generate_mass_kernel(double* __restrict__
     }
 }
 
+// Eq. 4, term by term, for the accept decision
+__device__ __forceinline__ double angular_pdf(double cl, double ck, double phi, const double* a)
+{
+    const double cl2 = cl * cl, ck2 = ck * ck, sl2 = 1.0 - cl2, sk2 = 1.0 - ck2;
+    const double sl = sqrt(sl2), sk = sqrt(sk2);
+    const double c2l = 2.0 * cl2 - 1.0, s2l = 2.0 * sl * cl, s2k = 2.0 * sk * ck;
+    double sp, cp, s2p, c2p;
+    sincos(phi, &sp, &cp);
+    sincos(2.0 * phi, &s2p, &c2p);
+    const double FL = a[0];
+    return (9.0 / (32.0 * 3.141592653589793238462643383279502884)) *
+           (0.75 * (1.0 - FL) * sk2 + FL * ck2 + 0.25 * (1.0 - FL) * sk2 * c2l - FL * ck2 * c2l + a[1] * sk2 * sl2 * c2p +
+            a[2] * s2k * s2l * cp + a[3] * s2k * sl * cp + (4.0 / 3.0) * a[4] * sk2 * cl + a[5] * s2k * sl * sp +
+            a[6] * s2k * s2l * sp + a[7] * sk2 * sl2 * s2p);
+}
+
+struct AngGenArgs {
+    double a[8];
+    double pmax;
+};
+
+// data: [3][n_toys][n_pad] (cos theta_l, cos theta_K, phi).  Proposal k of an event uses draws 2k and 2k+1.
+__global__ void __launch_bounds__(256) generate_angular_kernel(double* __restrict__ data, int64_t n_toys, int64_t n, int64_t n_pad,
+                                                               unsigned long long seed0, const __grid_constant__ AngGenArgs g)
+{
+    const int64_t per_dim = n_toys * n_pad;
+    for (int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; idx < per_dim; idx += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t toy = idx / n_pad, slot = idx % n_pad;
+        double cl = 0.0, ck = 0.0, phi = 0.0;
+        if (n > 0) {
+            const unsigned long long ev = (unsigned long long)(slot < n ? slot : n - 1), seed = seed0 + (unsigned long long)toy;
+            for (unsigned k = 0; k < 4096; ++k) {
+                double u1, u2, u3, u4;
+                uniforms(seed, ev, 2 * k, u1, u2);
+                uniforms(seed, ev, 2 * k + 1, u3, u4);
+                cl = 2.0 * u1 - 1.0;
+                ck = 2.0 * u2 - 1.0;
+                phi = 3.141592653589793238462643383279502884 * (2.0 * u3 - 1.0);
+                if (u4 * g.pmax < angular_pdf(cl, ck, phi, g.a)) break;
+            }
+        }
+        data[idx] = cl;
+        data[per_dim + idx] = ck;
+        data[2 * per_dim + idx] = phi;
+    }
+}
+
 }  // namespace
+
+extern "C" mf_status mf_generate_angular(mf_ctx* ctx, uint64_t seed0, int64_t n_toys, int64_t n_events, const double* a,
+                                         mf_dataset** out)
+{
+    if (!ctx || !a || !out) return mf_fail(ctx, MF_ERR_ARG, "mf_generate_angular: NULL argument");
+    if (n_toys < 1 || n_events < 0) return mf_fail(ctx, MF_ERR_ARG, "mf_generate_angular: n_toys >= 1 and n_events >= 0 are required");
+    AngGenArgs g;
+    double sum = 4.0;
+    for (int k = 0; k < 8; ++k) {
+        if (!std::isfinite(a[k])) return mf_fail(ctx, MF_ERR_PARAM_DOMAIN, "mf_generate_angular: non-finite coefficient");
+        g.a[k] = a[k];
+        if (k > 0) sum += (k == 4 ? 4.0 / 3.0 : 1.0) * std::fabs(a[k]);
+    }
+    g.pmax = 9.0 / (32.0 * 3.141592653589793238462643383279502884) * sum;  // the paper's get_max() bound
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return mf_fail(ctx, MF_ERR_CUDA, "mf_generate_angular: cudaSetDevice failed");
+    mf_dataset* ds = new (std::nothrow) mf_dataset();
+    mf_devbuf* buf = new (std::nothrow) mf_devbuf();
+    if (!ds || !buf) {
+        delete ds;
+        delete buf;
+        return mf_fail(ctx, MF_ERR_OOM, "mf_generate_angular: host allocation failed");
+    }
+    ds->ctx = ctx;
+    ds->ndim = 3;
+    ds->n_events = n_events;
+    ds->n_pad = (n_events + 63) / 64 * 64;
+    ds->n_toys = n_toys;
+    const double alo[3] = {-1.0, -1.0, -3.141592653589793238462643383279502884};
+    for (int j = 0; j < 3; ++j) {
+        ds->lo[j] = alo[j];
+        ds->hi[j] = -alo[j];
+    }
+    ds->raw = buf;
+    buf->stream = ctx->stream;
+    const int64_t per_dim = ds->n_pad * n_toys;
+    buf->bytes = (size_t)(per_dim > 0 ? 3 * per_dim : 1) * sizeof(double);
+    cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&buf->p), buf->bytes, ctx->stream);
+    if (e == cudaSuccess && per_dim > 0) {
+        const int grid = (int)std::min<int64_t>((per_dim + 255) / 256, 32 * (int64_t)ctx->sm_count);
+        generate_angular_kernel<<<grid, 256, 0, ctx->stream>>>(buf->p, n_toys, n_events, ds->n_pad, seed0, g);
+        ++ctx->launches;
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) {
+        if (buf->p) cudaFreeAsync(buf->p, ctx->stream);
+        delete buf;
+        delete ds;
+        return mf_fail(ctx, e == cudaErrorMemoryAllocation ? MF_ERR_OOM : MF_ERR_CUDA, std::string("mf_generate_angular: ") + cudaGetErrorString(e));
+    }
+    *out = ds;
+    return MF_OK;
+}
 
 extern "C" mf_status mf_generate_mass(mf_ctx* ctx, uint64_t seed0, int64_t n_toys, int64_t n_events, const double* lam,
                                       double lo, double hi, mf_dataset** out)

@@ -77,3 +77,27 @@ def test_generate_edge_cases(mf, ctx):
     assert np.array_equal(c[1], a)                         # toy t uses seed0 + t
     with pytest.raises(mf.MoreFitError):
         ctx.generate_mass(1, 1, 10, (0.3, 5.28, -1.0, -1.5), LO, HI)
+
+
+@pytest.mark.parametrize("a", [dg.ANG_TRUTH, (0.3, 0.1, -0.2, 0.25, 0.1, -0.05, 0.07, -0.09)])
+def test_generate_angular_matches_oracle(mf, ctx, a):
+    T, n, seed0 = 2, 333, 777
+    ds = ctx.generate_angular(seed0, T, n, a)
+    x = ds.download()                                   # [3][T][n]
+    ref = gen.gen_angular_toys(seed0, T, n, a)
+    assert x.shape == ref.shape == (3, T, n)
+    assert np.all(np.abs(x[:2]) <= 1) and np.all(np.abs(x[2]) <= np.pi)
+    # the proposals are bit-identical functions of the uniforms; an accept decision can differ only if u4 * pmax is within
+    # rounding of P(Omega), which does not happen in 666 events
+    assert np.array_equal(x, ref)
+
+
+def test_generated_angular_dataset_feeds_the_model(mf, ctx):
+    ds = ctx.generate_angular(5, 1, 50_000, dg.ANG_TRUTH)
+    model = ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ds)
+    ev = ds.download()[:, 0, :]
+    nll, g = model.nll_grad(dg.ANG_TRUTH)
+    o_nll, o_g, _ = oracle.nll_grad(oracle.ANGULAR, ev, dg.ANG_TRUTH)
+    assert abs(nll - o_nll) <= 1e-11 * abs(o_nll) and np.all(np.abs(g - o_g) <= 1e-9 * (1 + np.abs(o_g)))
+    r = model.fit(dg.ANG_TRUTH)
+    assert r.converged and np.all(np.abs((r.lam - np.array(dg.ANG_TRUTH)) / r.sigma) < 5)

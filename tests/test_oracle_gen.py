@@ -50,3 +50,30 @@ def test_signal_fraction_and_redraws():
     draws = np.array([k for _, s, k in r if s])
     assert abs(sig.mean() - 0.5) < 0.03
     assert 1.3 < (draws - 1).mean() < 1.8   # expected 1 / P(accept) = 1 / 0.655 = 1.53 Gaussian draws per signal event
+
+
+def test_angular_generator_pdf_is_the_pinned_oracle_pdf():
+    """oracle/gen.py's Eq. 4 (used for the accept decision) equals the pinned likelihood oracle's PDF (mf_oracle.c)."""
+    import oracle
+    rng = np.random.default_rng(1)
+    ev = np.stack([rng.uniform(-1, 1, 200), rng.uniform(-1, 1, 200), rng.uniform(-np.pi, np.pi, 200)])
+    for a in (dg.ANG_TRUTH, (0.3, 0.1, -0.2, 0.25, 0.1, -0.05, 0.07, -0.09)):
+        P, _ = oracle.pdf(oracle.ANGULAR, ev, a)
+        mine = np.array([gen.angular_pdf(*ev[:, i], a) for i in range(200)])
+        assert np.allclose(mine, P, rtol=1e-13, atol=1e-16)
+        assert np.all(P <= gen.angular_pmax(a))
+
+
+def test_angular_generated_marginals():
+    """Closed-form marginals of Eq. 4: dG/dcos(theta_l) = 3/4 FL (1-cl^2) + 3/8 (1-FL)(1+cl^2) + AFB cl,
+    dG/dcos(theta_K) = 3/4 (1-FL)(1-ck^2) + 3/2 FL ck^2, dG/dphi = [1 + S3 cos 2phi + S9 sin 2phi] / (2 pi)."""
+    a = (0.6, -0.1, -0.15, -0.2, 0.2, 0.0, -0.02, 0.15)
+    FL, S3, AFB, S9 = a[0], a[1], a[4], a[7]
+    x = gen.gen_angular_toys(21, 1, 5000, a)[:, 0, :]
+    cdf_l = lambda c: 0.75 * FL * (c - c ** 3 / 3 + 2 / 3) + 0.375 * (1 - FL) * (c + c ** 3 / 3 + 4 / 3) + AFB * (c * c - 1) / 2
+    cdf_k = lambda c: 0.75 * (1 - FL) * (c - c ** 3 / 3 + 2 / 3) + 0.5 * FL * (c ** 3 + 1)
+    cdf_p = lambda p: (p + np.pi + S3 * np.sin(2 * p) / 2 + S9 * (1 - np.cos(2 * p)) / 2) / (2 * np.pi)
+    for col, cdf in ((x[0], cdf_l), (x[1], cdf_k), (x[2], cdf_p)):
+        assert stats.kstest(col, cdf).pvalue > 1e-3
+    eff = np.mean([1.0 / gen.gen_angular_event(5, i, a)[1] for i in range(500)])
+    assert 0.05 < eff < 0.9
