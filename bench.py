@@ -375,8 +375,12 @@ def run_mine(args) -> None:
     import torch
 
     import paper_2505_12414_b200 as mf
+    from paper_2505_12414_b200 import build as mf_build
 
+    if int(os.environ.get("LOCAL_RANK", "0")) == 0:
+        mf_build.build()   # no-op when the library is newer than its sources
     rank, world, local = _dist_setup(args.gpus)
+    _barrier(world)
     torch.cuda.set_device(local)
     sampler = ClockSampler(local) if rank == 0 else None   # started early: it needs ~1 s to come up
     ctx = mf.Context(local)  # borrows torch's current stream on this device

@@ -16,6 +16,8 @@ LO, HI = dg.MASS_LO, dg.MASS_HI
 @pytest.fixture(scope="module")
 def mf():
     import paper_2505_12414_b200 as mf
+    from paper_2505_12414_b200 import build
+    build.build()          # no-op when lib/libmorefit_b200.so is newer than its sources (nvcc, sm_100a)
     return mf
 
 

@@ -18,6 +18,8 @@ GRAD_TOL = 1e-9
 @pytest.fixture(scope="module")
 def mf():
     import paper_2505_12414_b200 as mf
+    from paper_2505_12414_b200 import build
+    build.build()          # no-op when lib/libmorefit_b200.so is newer than its sources (nvcc, sm_100a)
     return mf
 
 
