@@ -113,6 +113,13 @@ mf_status mf_generate_mass(mf_ctx* ctx, uint64_t seed0, int64_t n_toys, int64_t 
  * event uses the draws 2k and 2k+1 of its Philox stream.  a: host, the 8 coefficients FL, S3, S4, S5, AFB, S7, S8, S9. */
 mf_status mf_generate_angular(mf_ctx* ctx, uint64_t seed0, int64_t n_toys, int64_t n_events, const double* a, mf_dataset** out);
 
+/* The same for the 4D model (ndim = 4: m, cos theta_l, cos theta_K, phi; BASELINE.json configs[3]).  lam: host, the 16
+ * parameters f, mu, sigma, tau, the 8 angular coefficients, cl1, cl2, ck1, ck2.  Signal (probability f): Gaussian mass and
+ * angular accept-reject as above; background: exponential mass by inverse CDF, flat phi, (cos theta_l, cos theta_K) by
+ * accept-reject of the Legendre product under 1/2 (1 + |c1| + |c2|) per factor.  Draw layout: mf_generate.cu. */
+mf_status mf_generate_4d(mf_ctx* ctx, uint64_t seed0, int64_t n_toys, int64_t n_events, const double* lam, double lo, double hi,
+                         mf_dataset** out);
+
 /* Copies a dataset's events to the host: dst [ndim][n_toys][n_events] doubles. */
 mf_status mf_dataset_download(const mf_dataset* ds, double* dst);
 

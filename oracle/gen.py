@@ -124,3 +124,67 @@ def gen_angular_toys(seed0: int, n_toys: int, n_events: int, a) -> np.ndarray:
         for i in range(n_events):
             out[:, t, i] = gen_angular_event(seed0 + t, i, a)[0]
     return out
+
+
+# ---------------------------------------------------------------- 4D model (BASELINE.json configs[3])
+#
+#   draw 0: (uA, uB).  Signal if uA < f.
+#   signal:      mass from draws 1..64 exactly as in gen_mass_event; angles by the angular accept-reject above with the
+#                proposals taken from draws 100 + 2k, 101 + 2k.
+#   background:  mass from uB by the inverse CDF; draw 1: (u1, -) -> phi = pi (2 u1 - 1);
+#                (cos theta_l, cos theta_K) by accept-reject of the Legendre product l(x; cl1, cl2) l(y; ck1, ck2),
+#                l(x; c1, c2) = 1/2 [1 + c1 x + c2 (3 x^2 - 1)/2], under the bound lmax(c1, c2) = 1/2 (1 + |c1| + |c2|) per factor:
+#                proposal k uses draws 100 + 2k -> (x, y) = (2 u1 - 1, 2 u2 - 1) and 101 + 2k -> (u3, -), accepted if
+#                u3 lmax_l lmax_k < l(x) l(y).
+
+def _legendre2(x: float, c1: float, c2: float) -> float:
+    return 0.5 * (1.0 + c1 * x + c2 * 0.5 * (3.0 * x * x - 1.0))
+
+
+def gen_4d_event(seed: int, event: int, lam, lo: float, hi: float):
+    """((m, cos theta_l, cos theta_K, phi), is_signal)."""
+    lam = [float(x) for x in lam]
+    f, mu, sigma, tau = lam[:4]
+    a = lam[4:12]
+    cl1, cl2, ck1, ck2 = lam[12:16]
+    ua, ub = uniforms(seed, event, 0)
+    if ua < f:
+        m = mu
+        for k in range(1, 65):
+            u1, u2 = uniforms(seed, event, k)
+            m = mu + sigma * (math.sqrt(-2.0 * math.log(u1)) * math.cos(2.0 * math.pi * u2))
+            if lo <= m <= hi:
+                break
+        else:
+            m = min(max(m, lo), hi)
+        pmax = angular_pmax(a)
+        cl = ck = phi = 0.0
+        for k in range(4096):
+            u1, u2 = uniforms(seed, event, 100 + 2 * k)
+            u3, u4 = uniforms(seed, event, 101 + 2 * k)
+            cl, ck, phi = 2.0 * u1 - 1.0, 2.0 * u2 - 1.0, math.pi * (2.0 * u3 - 1.0)
+            if u4 * pmax < angular_pdf(cl, ck, phi, a):
+                break
+        return (m, cl, ck, phi), True
+    w = hi - lo
+    m = lo + ub * w if tau == 0.0 else lo + math.log1p(ub * math.expm1(tau * w)) / tau
+    m = min(max(m, lo), hi)
+    phi = math.pi * (2.0 * uniforms(seed, event, 1)[0] - 1.0)
+    bound = 0.5 * (1.0 + abs(cl1) + abs(cl2)) * 0.5 * (1.0 + abs(ck1) + abs(ck2))
+    x = y = 0.0
+    for k in range(4096):
+        u1, u2 = uniforms(seed, event, 100 + 2 * k)
+        u3, _ = uniforms(seed, event, 101 + 2 * k)
+        x, y = 2.0 * u1 - 1.0, 2.0 * u2 - 1.0
+        if u3 * bound < _legendre2(x, cl1, cl2) * _legendre2(y, ck1, ck2):
+            break
+    return (m, x, y, phi), False
+
+
+def gen_4d_toys(seed0: int, n_toys: int, n_events: int, lam, lo: float, hi: float) -> np.ndarray:
+    """[4][n_toys][n_events]"""
+    out = np.empty((4, n_toys, n_events))
+    for t in range(n_toys):
+        for i in range(n_events):
+            out[:, t, i] = gen_4d_event(seed0 + t, i, lam, lo, hi)[0]
+    return out

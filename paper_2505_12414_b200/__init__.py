@@ -32,7 +32,7 @@ _STATUS_NAMES = ["MF_OK", "MF_ERR_ARG", "MF_ERR_CUDA", "MF_ERR_OOM", "MF_ERR_DAT
 
 EXPORTS = [
     "mf_ctx_create", "mf_ctx_destroy", "mf_last_error", "mf_ctx_kernel_launches",
-    "mf_dataset_upload", "mf_generate_mass", "mf_generate_angular", "mf_dataset_download", "mf_dataset_destroy", "mf_dataset_n_events", "mf_dataset_n_toys",
+    "mf_dataset_upload", "mf_generate_mass", "mf_generate_angular", "mf_generate_4d", "mf_dataset_download", "mf_dataset_destroy", "mf_dataset_n_events", "mf_dataset_n_toys",
     "mf_model_create", "mf_model_destroy", "mf_model_nparams", "mf_model_n_events", "mf_model_n_toys",
     "mf_nll_grad", "mf_nll_grad_async", "mf_nll_grad_points", "mf_nll_grad_batch", "mf_nll_grad_batch_async",
     "mf_model_has_hessian", "mf_nll_grad_hess", "mf_nll_grad_hess_batch",
@@ -144,6 +144,8 @@ def load_library() -> ctypes.CDLL:
     lib.mf_generate_mass.argtypes = [vp, ctypes.c_uint64, i64, i64, dp, ctypes.c_double, ctypes.c_double, ctypes.POINTER(vp)]
     lib.mf_generate_angular.restype = ctypes.c_int
     lib.mf_generate_angular.argtypes = [vp, ctypes.c_uint64, i64, i64, dp, ctypes.POINTER(vp)]
+    lib.mf_generate_4d.restype = ctypes.c_int
+    lib.mf_generate_4d.argtypes = [vp, ctypes.c_uint64, i64, i64, dp, ctypes.c_double, ctypes.c_double, ctypes.POINTER(vp)]
     lib.mf_dataset_download.restype = ctypes.c_int
     lib.mf_dataset_download.argtypes = [vp, dp]
     lib.mf_dataset_destroy.restype = None
@@ -266,6 +268,19 @@ class Context:
                                                ctypes.byref(ds._h)))
         self._children.add(ds)
         ds.ndim, ds.n_events, ds.n_toys = 1, int(n_events), int(n_toys)
+        return ds
+
+    def generate_4d(self, seed0: int, n_toys: int, n_events: int, lam, lo: float, hi: float) -> "Dataset":
+        """n_toys pseudo-experiments of the 4D mass x angular model generated on the device."""
+        lam = np.ascontiguousarray(lam, dtype=np.float64)
+        if lam.shape != (16,):
+            raise ValueError("lam must have 16 entries")
+        ds = Dataset.__new__(Dataset)
+        ds._ctx, ds._lib, ds._h = self, self._lib, ctypes.c_void_p()
+        self._check(self._lib.mf_generate_4d(self._h, int(seed0), int(n_toys), int(n_events), _dp(lam), float(lo), float(hi),
+                                             ctypes.byref(ds._h)))
+        self._children.add(ds)
+        ds.ndim, ds.n_events, ds.n_toys = 4, int(n_events), int(n_toys)
         return ds
 
     def generate_angular(self, seed0: int, n_toys: int, n_events: int, a) -> "Dataset":

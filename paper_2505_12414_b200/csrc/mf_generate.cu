@@ -135,7 +135,143 @@ __global__ void __launch_bounds__(256) generate_angular_kernel(double* __restric
     }
 }
 
+struct FourDGenArgs {
+    double f, mu, sigma, tau, lo, hi, em1;
+    AngGenArgs ang;
+    double cl1, cl2, ck1, ck2, bound;
+};
+
+__device__ __forceinline__ double legendre2(double x, double c1, double c2)
+{
+    return 0.5 * (1.0 + c1 * x + c2 * 0.5 * (3.0 * x * x - 1.0));
+}
+
+// data: [4][n_toys][n_pad] (m, cos theta_l, cos theta_K, phi); recipe: see oracle/gen.py gen_4d_event / the header
+__global__ void __launch_bounds__(256) generate_4d_kernel(double* __restrict__ data, int64_t n_toys, int64_t n, int64_t n_pad,
+                                                          unsigned long long seed0, const __grid_constant__ FourDGenArgs g)
+{
+    const int64_t per_dim = n_toys * n_pad;
+    const double pi = 3.141592653589793238462643383279502884;
+    for (int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; idx < per_dim; idx += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t toy = idx / n_pad, slot = idx % n_pad;
+        double m = 0.0, cl = 0.0, ck = 0.0, phi = 0.0;
+        if (n > 0) {
+            const unsigned long long ev = (unsigned long long)(slot < n ? slot : n - 1), seed = seed0 + (unsigned long long)toy;
+            double ua, ub;
+            uniforms(seed, ev, 0u, ua, ub);
+            if (ua < g.f) {
+                m = g.mu;
+                bool ok = false;
+                for (unsigned k = 1; k <= 64 && !ok; ++k) {
+                    double u1, u2;
+                    uniforms(seed, ev, k, u1, u2);
+                    m = fma(g.sigma, sqrt(-2.0 * log(u1)) * cos(2.0 * pi * u2), g.mu);
+                    ok = (m >= g.lo && m <= g.hi);
+                }
+                if (!ok) m = fmin(fmax(m, g.lo), g.hi);
+                for (unsigned k = 0; k < 4096; ++k) {
+                    double u1, u2, u3, u4;
+                    uniforms(seed, ev, 100 + 2 * k, u1, u2);
+                    uniforms(seed, ev, 101 + 2 * k, u3, u4);
+                    cl = 2.0 * u1 - 1.0;
+                    ck = 2.0 * u2 - 1.0;
+                    phi = pi * (2.0 * u3 - 1.0);
+                    if (u4 * g.ang.pmax < angular_pdf(cl, ck, phi, g.ang.a)) break;
+                }
+            } else {
+                const double w = g.hi - g.lo;
+                m = (g.tau == 0.0) ? fma(ub, w, g.lo) : g.lo + log1p(ub * g.em1) / g.tau;
+                m = fmin(fmax(m, g.lo), g.hi);
+                double u1, u2, u3, u4;
+                uniforms(seed, ev, 1u, u1, u2);
+                phi = pi * (2.0 * u1 - 1.0);
+                for (unsigned k = 0; k < 4096; ++k) {
+                    uniforms(seed, ev, 100 + 2 * k, u1, u2);
+                    uniforms(seed, ev, 101 + 2 * k, u3, u4);
+                    cl = 2.0 * u1 - 1.0;
+                    ck = 2.0 * u2 - 1.0;
+                    if (u3 * g.bound < legendre2(cl, g.cl1, g.cl2) * legendre2(ck, g.ck1, g.ck2)) break;
+                }
+            }
+        }
+        data[idx] = m;
+        data[per_dim + idx] = cl;
+        data[2 * per_dim + idx] = ck;
+        data[3 * per_dim + idx] = phi;
+    }
+}
+
 }  // namespace
+
+extern "C" mf_status mf_generate_4d(mf_ctx* ctx, uint64_t seed0, int64_t n_toys, int64_t n_events, const double* lam, double lo,
+                                    double hi, mf_dataset** out)
+{
+    if (!ctx || !lam || !out) return mf_fail(ctx, MF_ERR_ARG, "mf_generate_4d: NULL argument");
+    if (n_toys < 1 || n_events < 0 || !(std::isfinite(lo) && std::isfinite(hi) && lo < hi))
+        return mf_fail(ctx, MF_ERR_ARG, "mf_generate_4d: n_toys >= 1, n_events >= 0 and a finite range lo < hi are required");
+    for (int k = 0; k < 16; ++k)
+        if (!std::isfinite(lam[k])) return mf_fail(ctx, MF_ERR_PARAM_DOMAIN, "mf_generate_4d: non-finite parameter");
+    if (!(lam[0] >= 0.0 && lam[0] <= 1.0) || !(lam[2] > 0.0) || !std::isfinite(std::expm1(lam[3] * (hi - lo))))
+        return mf_fail(ctx, MF_ERR_PARAM_DOMAIN, "mf_generate_4d: lambda outside the parameter domain");
+    FourDGenArgs g;
+    g.f = lam[0];
+    g.mu = lam[1];
+    g.sigma = lam[2];
+    g.tau = lam[3];
+    g.lo = lo;
+    g.hi = hi;
+    g.em1 = std::expm1(lam[3] * (hi - lo));
+    double sum = 4.0;
+    for (int k = 0; k < 8; ++k) {
+        g.ang.a[k] = lam[4 + k];
+        if (k > 0) sum += (k == 4 ? 4.0 / 3.0 : 1.0) * std::fabs(lam[4 + k]);
+    }
+    g.ang.pmax = 9.0 / (32.0 * 3.141592653589793238462643383279502884) * sum;
+    g.cl1 = lam[12];
+    g.cl2 = lam[13];
+    g.ck1 = lam[14];
+    g.ck2 = lam[15];
+    g.bound = 0.5 * (1.0 + std::fabs(g.cl1) + std::fabs(g.cl2)) * 0.5 * (1.0 + std::fabs(g.ck1) + std::fabs(g.ck2));
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return mf_fail(ctx, MF_ERR_CUDA, "mf_generate_4d: cudaSetDevice failed");
+    mf_dataset* ds = new (std::nothrow) mf_dataset();
+    mf_devbuf* buf = new (std::nothrow) mf_devbuf();
+    if (!ds || !buf) {
+        delete ds;
+        delete buf;
+        return mf_fail(ctx, MF_ERR_OOM, "mf_generate_4d: host allocation failed");
+    }
+    ds->ctx = ctx;
+    ds->ndim = 4;
+    ds->n_events = n_events;
+    ds->n_pad = (n_events + 63) / 64 * 64;
+    ds->n_toys = n_toys;
+    const double alo[4] = {lo, -1.0, -1.0, -3.141592653589793238462643383279502884};
+    const double ahi[4] = {hi, 1.0, 1.0, 3.141592653589793238462643383279502884};
+    for (int j = 0; j < 4; ++j) {
+        ds->lo[j] = alo[j];
+        ds->hi[j] = ahi[j];
+    }
+    ds->raw = buf;
+    buf->stream = ctx->stream;
+    const int64_t per_dim = ds->n_pad * n_toys;
+    buf->bytes = (size_t)(per_dim > 0 ? 4 * per_dim : 1) * sizeof(double);
+    cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&buf->p), buf->bytes, ctx->stream);
+    if (e == cudaSuccess && per_dim > 0) {
+        const int grid = (int)std::min<int64_t>((per_dim + 255) / 256, 32 * (int64_t)ctx->sm_count);
+        generate_4d_kernel<<<grid, 256, 0, ctx->stream>>>(buf->p, n_toys, n_events, ds->n_pad, seed0, g);
+        ++ctx->launches;
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) {
+        if (buf->p) cudaFreeAsync(buf->p, ctx->stream);
+        delete buf;
+        delete ds;
+        return mf_fail(ctx, e == cudaErrorMemoryAllocation ? MF_ERR_OOM : MF_ERR_CUDA, std::string("mf_generate_4d: ") + cudaGetErrorString(e));
+    }
+    *out = ds;
+    return MF_OK;
+}
 
 extern "C" mf_status mf_generate_angular(mf_ctx* ctx, uint64_t seed0, int64_t n_toys, int64_t n_events, const double* a,
                                          mf_dataset** out)

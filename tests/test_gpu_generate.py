@@ -103,3 +103,22 @@ def test_generated_angular_dataset_feeds_the_model(mf, ctx):
     assert abs(nll - o_nll) <= 1e-11 * abs(o_nll) and np.all(np.abs(g - o_g) <= 1e-9 * (1 + np.abs(o_g)))
     r = model.fit(dg.ANG_TRUTH)
     assert r.converged and np.all(np.abs((r.lam - np.array(dg.ANG_TRUTH)) / r.sigma) < 5)
+
+
+def test_generate_4d_matches_oracle_and_feeds_the_model(mf, ctx):
+    T, n, seed0 = 2, 257, 4242
+    lam = dg.FOURD_TRUTH
+    ds = ctx.generate_4d(seed0, T, n, lam, LO, HI)
+    x = ds.download()                                   # [4][T][n]
+    ref = gen.gen_4d_toys(seed0, T, n, lam, LO, HI)
+    assert x.shape == ref.shape == (4, T, n)
+    assert np.array_equal(x[1:], ref[1:])               # angles: bit-identical functions of the uniforms
+    assert np.max(np.abs(x[0] - ref[0])) <= 64 * np.spacing(HI)   # mass: CUDA vs libm transforms
+    big = ctx.generate_4d(9, 1, 100_000, lam, LO, HI)
+    model = ctx.model_create(mf.MF_MASS_X_ANGULAR, big)
+    ev = big.download()[:, 0, :]
+    nll, g = model.nll_grad(lam)
+    o_nll, o_g, _ = oracle.nll_grad(oracle.FOURD, ev, lam, LO, HI, nthreads=oracle.max_threads())
+    assert abs(nll - o_nll) <= 1e-11 * abs(o_nll) and np.all(np.abs(g - o_g) <= 1e-9 * (1 + np.abs(o_g)))
+    r = model.fit(lam)
+    assert r.converged and np.all(np.abs((r.lam - np.array(lam)) / r.sigma) < 5)

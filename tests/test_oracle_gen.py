@@ -77,3 +77,25 @@ def test_angular_generated_marginals():
         assert stats.kstest(col, cdf).pvalue > 1e-3
     eff = np.mean([1.0 / gen.gen_angular_event(5, i, a)[1] for i in range(500)])
     assert 0.05 < eff < 0.9
+
+
+def test_4d_generated_sample_is_consistent_with_the_4d_pdf():
+    """The generated 4D sample maximises its own likelihood near the generating values: the pinned oracle's gradient at
+    the truth, in units of its statistical spread, is O(1) (score test), and the signal fraction and the marginals match."""
+    import oracle
+    lam = dg.FOURD_TRUTH
+    n = 4000
+    ev = gen.gen_4d_toys(77, 1, n, lam, LO, HI)[:, 0, :]
+    assert np.all((ev[0] >= LO) & (ev[0] <= HI)) and np.all(np.abs(ev[1:3]) <= 1) and np.all(np.abs(ev[3]) <= np.pi)
+    sig = np.array([gen.gen_4d_event(77, i, lam, LO, HI)[1] for i in range(n)])
+    assert abs(sig.mean() - lam[0]) < 4 * math.sqrt(lam[0] * (1 - lam[0]) / n)
+    # score test: g_k / sqrt(sum of squared per-event scores) ~ N(0, 1) at the generating point
+    nll, g, bad = oracle.nll_grad(oracle.FOURD, ev, lam, LO, HI)
+    P, dl = oracle.pdf(oracle.FOURD, ev, lam, LO, HI)
+    z = -g / np.sqrt((dl ** 2).sum(axis=1))
+    assert bad == 0 and np.all(np.abs(z) < 4.5), z
+    # background angles: Legendre marginal in cos theta_l of the background events
+    x = ev[1][~sig]
+    c1, c2 = lam[12], lam[13]
+    cdf = lambda v: 0.5 * ((v + 1) + c1 * (v * v - 1) / 2 + c2 * 0.5 * (v ** 3 - v))
+    assert stats.kstest(x, cdf).pvalue > 1e-3
