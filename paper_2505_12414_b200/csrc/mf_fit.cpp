@@ -488,12 +488,16 @@ static mf_status fit_many(mf_model* m, int64_t n_toys, const double* starts, con
     std::vector<uint8_t> active((size_t)n_toys);
     const bool analytic = o.analytic_hessian != 0 && mf_model_has_hessian(m);
     std::vector<double> hess(analytic ? (size_t)n_toys * K * K : 0);
+    // the T fit states are independent: their host-side updates run on all cores (static schedule; the results do not
+    // depend on the thread count)
+#pragma omp parallel for schedule(static) if (n_toys >= 256)
     for (int64_t t = 0; t < n_toys; ++t) {
         st[t].init(K, starts + t * K, fixed, o);
         if (analytic) st[t].use_analytic_hessian();
     }
     for (;;) {
         int64_t n_active = 0;
+#pragma omp parallel for schedule(static) reduction(+ : n_active) if (n_toys >= 256)
         for (int64_t t = 0; t < n_toys; ++t) {
             active[t] = st[t].done() ? 0 : 1;
             if (active[t]) {
@@ -505,9 +509,11 @@ static mf_status fit_many(mf_model* m, int64_t n_toys, const double* starts, con
         const mf_status rc = analytic ? mf_nll_grad_hess_batch(m, n_toys, lam.data(), active.data(), nll.data(), grad.data(), hess.data())
                                       : mf_nll_grad_batch(m, n_toys, lam.data(), active.data(), nll.data(), grad.data());
         if (rc != MF_OK) return rc;
+#pragma omp parallel for schedule(static) if (n_toys >= 256)
         for (int64_t t = 0; t < n_toys; ++t)
             if (active[t]) st[t].feed(std::isfinite(nll[t]), nll[t], &grad[t * K], analytic ? &hess[t * K * K] : nullptr);
     }
+#pragma omp parallel for schedule(static) if (n_toys >= 256)
     for (int64_t t = 0; t < n_toys; ++t) st[t].result(&results[t]);
     return MF_OK;
 }
