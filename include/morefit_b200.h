@@ -18,9 +18,14 @@
  *   * All device work of a context is enqueued on the CUDA stream given at creation
  *     (borrowed, e.g. torch.cuda.current_stream().cuda_stream; NULL = the legacy default
  *     stream).  Calls on one context must not be made concurrently from several threads.
- *   * Results are bit-identical for identical inputs on the same GPU: per-thread, per-warp,
- *     per-block and final sums are all taken in a fixed order (PAPER.md:65 uses Kahan
- *     reduction kernels; here one compensated fixed-order pass).
+ *   * Results are bit-identical for identical inputs through the same entry point on the same
+ *     GPU: per-thread, per-warp, per-block and final sums are all taken in a fixed order
+ *     (PAPER.md:65 uses Kahan reduction kernels; here one compensated fixed-order pass,
+ *     SURVEY.md §8(a) S4/S5).  Different entry points tile the events differently (a lone call,
+ *     a pipelined series, many points per launch, toys): their results agree to summation
+ *     rounding (~1e-14 relative), not bit for bit.
+ *   * Successive evaluations on the stream overlap (programmatic dependent launch); results
+ *     still land in stream order.
  */
 #ifndef MOREFIT_B200_H
 #define MOREFIT_B200_H
