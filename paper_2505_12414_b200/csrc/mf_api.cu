@@ -9,6 +9,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "mf_internal.h"
@@ -413,6 +414,24 @@ static cudaError_t launch_pdl(void (*kernel)(const Args), int grid, cudaStream_t
     return cudaLaunchKernelEx(&cfg, kernel, a);
 }
 
+// The same for kernels with more than one parameter.
+template <class... KArgs, class... Args>
+static cudaError_t launch_pdl_v(void (*kernel)(KArgs...), int grid, int block, cudaStream_t stream, Args&&... args)
+{
+    static const bool no_pdl = std::getenv("MF_NO_PDL") != nullptr;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3((unsigned)block);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = no_pdl ? 0 : 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
+
 template <class M>
 static bool host_consts(const mf_model* m, const double* lam, typename M::Consts& c);
 template <>
@@ -643,8 +662,9 @@ static mf_status launch_batch(mf_model* m, int n_active, const double* lam_dev =
     a.bad_partials = m->b_bad;
     a.ticket = m->ticket + kRing;
     a.out = out_dev ? out_dev : m->d_bout;
-    batch_consts_kernel<M><<<(n_active + 127) / 128, 128, 0, ctx->stream>>>(a, n_active);
-    MF_CUDA(ctx, cudaGetLastError());
+    // both kernels are launched programmatically: the constants kernel of evaluation i+1 starts (and computes) while the
+    // batched kernel of evaluation i drains, and waits for it to complete only before overwriting the constants
+    MF_CUDA(ctx, launch_pdl_v(batch_consts_kernel<M>, (n_active + 127) / 128, 128, ctx->stream, a, n_active));
     MF_CUDA(ctx, launch_pdl(nll_grad_batch_kernel<M>, n_active * m->chunks, ctx->stream, a, M::BATCH_BLOCK));
     ctx->launches += 2;
     return MF_OK;
