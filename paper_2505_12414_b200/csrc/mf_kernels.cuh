@@ -457,7 +457,6 @@ __global__ void __launch_bounds__(M::BATCH_BLOCK, M::BATCH_RESIDENT_CTAS)
     nll_grad_batch_kernel(const __grid_constant__ BatchArgs<M> a)
 {
     constexpr int NACC = M::NACC;
-    constexpr int K = M::K;
     constexpr int kBlock = M::BATCH_BLOCK, kWarps = kBlock / 32;  // this kernel's own CTA size
     static_assert(kBlock >= 64 && NACC + 1 <= kBlock, "CTA too small for the reduction");
     __shared__ double sm[kWarps][NACC];
