@@ -359,3 +359,38 @@ def test_underflowed_pdf_is_flagged(mf, ctx):
     o_nll, o_g, o_bad = oracle.nll_grad(oracle.MASS, m, lam2, dg.MASS_LO, dg.MASS_HI)
     assert o_bad == 0
     assert_parity(nll, g, o_nll, o_g, "f = 0.9")
+
+
+def test_edge_cases_batch_and_points(mf, ctx):
+    """Empty toys, a single toy through the batch entries, and a bad point in a many-point call (nothing is enqueued)."""
+    import torch
+    # toys with zero events: every sum is 0
+    empty = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(np.zeros((3, 0)), dg.MASS_LO, dg.MASS_HI, n_toys=3))
+    nll, g = empty.nll_grad_batch(np.tile(np.array(dg.MASS_TRUTH), (3, 1)))
+    assert np.all(nll == 0.0) and np.all(g == 0.0)
+    # many points, one outside the domain: MF_ERR_PARAM_DOMAIN and the output buffer is untouched
+    m = dg.gen_mass(5000, seed=8)
+    model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(m, dg.MASS_LO, dg.MASS_HI))
+    pts = dg.gen_lambda_points(32, 3, dg.MASS_TRUTH, 3 * dg.mass_sigma_stat(5000))
+    pts[20, 0] = 1.5
+    out = torch.full((32, 6), -7.0, dtype=torch.float64, device="cuda")
+    with pytest.raises(mf.MoreFitError) as e:
+        model.nll_grad_points(pts, out.data_ptr())
+    assert e.value.status == mf.MF_ERR_PARAM_DOMAIN
+    torch.cuda.synchronize()
+    assert torch.all(out == -7.0)
+    # a point with P <= 0 for some event inside a many-point call: that row is +inf / NaN / n_bad > 0, the others are fine
+    am = ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ctx.dataset_upload(dg.gen_angular(3000, seed=4)))
+    apts = np.tile(np.array(dg.ANG_TRUTH), (16, 1))
+    apts[5, 0] = 3.0          # FL = 3: the PDF goes negative for many events
+    aout = torch.zeros((16, 10), dtype=torch.float64, device="cuda")
+    am.nll_grad_points(apts, aout.data_ptr())
+    torch.cuda.synchronize()
+    r = aout.cpu().numpy()
+    assert r[5, 0] == math.inf and np.all(np.isnan(r[5, 1:9])) and r[5, 9] > 0
+    n0, g0 = am.nll_grad(dg.ANG_TRUTH)
+    assert abs(r[4, 0] - n0) <= 1e-12 * abs(n0) and r[4, 9] == 0
+    # the 1-toy model through the batch entry points
+    n1, g1 = model.nll_grad_batch(np.array([dg.MASS_TRUTH]))
+    n2, g2 = model.nll_grad(dg.MASS_TRUTH)
+    assert n1[0] == n2 and np.array_equal(g1[0], g2)
