@@ -437,6 +437,27 @@ def run_mine(args) -> None:
     ms_per_step = ms / args.steps
     value = world * N_EVENTS * args.steps / (ms * 1e-3)
 
+    # the same steps as ONE KERNEL LAUNCH PER STEP (8 points per call -> pipelined single evaluations, every launch
+    # reading its replica's events from HBM): the number a minimiser sees when its points arrive one at a time
+    def run_single_launch_steps(count: int):
+        i = 0
+        while i < count:
+            p = i % N_POINTS
+            c = min(8 - p % 8, count - i)
+            models[(i // 8) % N_REPLICAS].nll_grad_points(pts_c[p:p + c], out_ptrs[p])
+            i += c
+
+    n_single = min(args.steps, 4000)
+    run_single_launch_steps(200)
+    torch.cuda.synchronize()
+    l0 = ctx.kernel_launches
+    e0.record()
+    run_single_launch_steps(n_single)
+    e1.record()
+    torch.cuda.synchronize()
+    single_us = _max_over_ranks(float(e0.elapsed_time(e1)), world) * 1e3 / n_single
+    single_launches = ctx.kernel_launches - l0
+
     # ---- e2e: public API with HOST (pinned) inputs, upload + model + evaluation every step
     pinned = torch.from_numpy(host0).pin_memory()
     host_view = pinned.numpy()
@@ -491,6 +512,10 @@ def run_mine(args) -> None:
         "peak_how": f"derived: {n_sm} SMs x {NOMINAL_FP64_LANES_PER_SM} fp64 lanes x {sm_max_mhz:.0f} MHz x 2 flop",
         "peak_measured_dfma_chain": 2.0 * measured_rate / 1e12,
         "frac_of_measured_dfma_chain": achieved_tflops / (2.0 * measured_rate / 1e12),
+        "one_launch_per_step": {"us_per_step": single_us, "steps": n_single, "gpu_launches": int(single_launches),
+                                "events_per_s": world * N_EVENTS / (single_us * 1e-6),
+                                "frac": 2.0 * MASS_FP64_INSTR_PER_EVENT * N_EVENTS / (single_us * 1e-6) / 1e12 / peak_tflops,
+                                "kernel": "nll_grad_kernel<MassModel>, programmatic dependent launch between steps"},
         "hbm_side": {"bytes_per_event": 8, "achieved_gbs": 8.0 * N_EVENTS / (ms_per_step * 1e-3) / 1e9,
                      "peak_gbs": peaks.get("hbm_gbs")},
     }
