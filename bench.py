@@ -328,12 +328,7 @@ def _other_workloads(torch, mf, ctx, peaks) -> dict:
     del bm, toys
     # the paper's own protocol (time per pseudo-experiment = generation + fit + HESSE), all on the device
     def toy_study(seed0):
-        ds = ctx.generate_mass(seed0, T, n, dg.MASS_TRUTH, dg.MASS_LO, dg.MASS_HI)
-        md = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ds)
-        out = md.fit_batch(np.array(dg.MASS_TRUTH))
-        md.close()
-        ds.close()
-        return out
+        return ctx.toy_study_mass(seed0, T, n, dg.MASS_TRUTH, dg.MASS_LO, dg.MASS_HI)
     toy_study(1)
     t = time.perf_counter()
     ts = toy_study(100_000)
@@ -346,8 +341,8 @@ def _other_workloads(torch, mf, ctx, peaks) -> dict:
     gds.close()
     res["toy_study_4096x1e4_on_device"] = {
         "ms_per_toy": 1e3 * ts_s / T, "toys_per_s": T / ts_s, "converged": int(ts.converged.sum()),
-        "what": "mf_generate_mass (4096 toys x 1e4 events, Philox4x32-10) + mf_model_create + mf_fit_batch (Newton on the "
-                "analytic Hessian + HESSE); no event crosses PCIe",
+        "what": "mf_toy_study_mass: mf_generate_mass (4096 toys x 1e4 events, Philox4x32-10) + mf_model_create + mf_fit_batch "
+                "(Newton on the analytic Hessian + HESSE); no event crosses PCIe",
         "generation_us": gen_us, "generated_events_per_s": T * n / (gen_us * 1e-6),
         "paper_context": "MoreFit OpenCL GPU (analytic), Titan V: 1.62 ms per toy at 1e4 events (PAPER.md:191); another machine"}
     # C0: N = 1e4, one call + full fit (latency bound: no roofline claim)

@@ -246,6 +246,12 @@ mf_status mf_fit(mf_model* model, const double* start, const uint8_t* fixed,
 mf_status mf_fit_batch(mf_model* model, int64_t n_toys, const double* starts,
                        const uint8_t* fixed, const mf_fit_opts* opts, mf_fit_result* results);
 
+/* The paper's toy study for the mass model (Listing 6: `toystudy.toy(...)`): generates n_toys
+ * pseudo-experiments of n_events events at lam_truth (mf_generate_mass, seeds seed0 + t), fits all of them concurrently from
+ * lam_truth (mf_fit_batch) and returns the n_toys fit results (host) with their HESSE covariances.  No event leaves the device. */
+mf_status mf_toy_study_mass(mf_ctx* ctx, uint64_t seed0, int64_t n_toys, int64_t n_events, const double* lam_truth, double lo,
+                            double hi, const mf_fit_opts* opts, mf_fit_result* results);
+
 /* ---- measurement helpers (not on the hot path) ------------------------ */
 
 /* fp64-pipe issue rate of this GPU in DFMA thread-instructions per second, measured with

@@ -36,7 +36,7 @@ EXPORTS = [
     "mf_model_create", "mf_model_destroy", "mf_model_nparams", "mf_model_n_events", "mf_model_n_toys",
     "mf_nll_grad", "mf_nll_grad_async", "mf_nll_grad_points", "mf_nll_grad_batch", "mf_nll_grad_batch_async",
     "mf_model_has_hessian", "mf_nll_grad_hess", "mf_nll_grad_hess_batch",
-    "mf_fit_opts_default", "mf_fit", "mf_fit_batch",
+    "mf_fit_opts_default", "mf_fit", "mf_fit_batch", "mf_toy_study_mass",
     "mf_probe_fp64_rate", "mf_probe_read_bandwidth", "mf_probe_math",
 ]
 
@@ -186,6 +186,9 @@ def load_library() -> ctypes.CDLL:
     lib.mf_fit.argtypes = [vp, dp, u8p, ctypes.POINTER(FitOpts), ctypes.POINTER(_FitResultC)]
     lib.mf_fit_batch.restype = ctypes.c_int
     lib.mf_fit_batch.argtypes = [vp, i64, dp, u8p, ctypes.POINTER(FitOpts), ctypes.POINTER(_FitResultC)]
+    lib.mf_toy_study_mass.restype = ctypes.c_int
+    lib.mf_toy_study_mass.argtypes = [vp, ctypes.c_uint64, i64, i64, dp, ctypes.c_double, ctypes.c_double, ctypes.POINTER(FitOpts),
+                                      ctypes.POINTER(_FitResultC)]
     lib.mf_probe_fp64_rate.restype = ctypes.c_int
     lib.mf_probe_fp64_rate.argtypes = [vp, dp]
     lib.mf_probe_read_bandwidth.restype = ctypes.c_int
@@ -292,6 +295,16 @@ class Context:
         self._children.add(ds)
         ds.ndim, ds.n_events, ds.n_toys = 3, int(n_events), int(n_toys)
         return ds
+
+    def toy_study_mass(self, seed0: int, n_toys: int, n_events: int, lam_truth, lo: float, hi: float,
+                       opts: "FitOpts | None" = None) -> "BatchFitResult":
+        """Generate, fit and HESSE n_toys pseudo-experiments of the mass model on the device."""
+        lam = np.ascontiguousarray(lam_truth, dtype=np.float64)
+        res = np.empty(int(n_toys), dtype=BatchFitResult._DT)
+        self._check(self._lib.mf_toy_study_mass(self._h, int(seed0), int(n_toys), int(n_events), _dp(lam), float(lo), float(hi),
+                                                None if opts is None else ctypes.byref(opts),
+                                                res.ctypes.data_as(ctypes.POINTER(_FitResultC))))
+        return BatchFitResult(res, int(n_toys), 4)
 
     def model_create(self, kind: int, dataset: "Dataset") -> "Model":
         return Model(self, kind, dataset)

@@ -388,3 +388,30 @@ extern "C" mf_status mf_dataset_download(const mf_dataset* ds, double* dst)
     if (cudaStreamSynchronize(ctx->stream) != cudaSuccess) return mf_fail(ctx, MF_ERR_CUDA, "mf_dataset_download: synchronise failed");
     return MF_OK;
 }
+
+// The paper's toy study (Listing 6 `toystudy::toy`): generate n_toys pseudo-experiments of n_events events at
+// lam_truth, fit all of them concurrently from lam_truth, HESSE.  Everything stays on the device.
+extern "C" mf_status mf_toy_study_mass(mf_ctx* ctx, uint64_t seed0, int64_t n_toys, int64_t n_events, const double* lam_truth,
+                                       double lo, double hi, const mf_fit_opts* opts, mf_fit_result* results)
+{
+    if (!ctx || !lam_truth || !results) return mf_fail(ctx, MF_ERR_ARG, "mf_toy_study_mass: NULL argument");
+    mf_dataset* ds = nullptr;
+    mf_status st = mf_generate_mass(ctx, seed0, n_toys, n_events, lam_truth, lo, hi, &ds);
+    if (st != MF_OK) return st;
+    mf_model* model = nullptr;
+    st = mf_model_create(ctx, MF_MASS_GAUSS_EXP, ds, &model);
+    mf_dataset_destroy(ds);
+    if (st != MF_OK) return st;
+    double* starts = new (std::nothrow) double[(size_t)n_toys * 4];
+    if (!starts) {
+        mf_model_destroy(model);
+        return mf_fail(ctx, MF_ERR_OOM, "mf_toy_study_mass: host allocation failed");
+    }
+    for (int64_t t = 0; t < n_toys; ++t)
+        for (int k = 0; k < 4; ++k) starts[t * 4 + k] = lam_truth[k];
+    if (n_toys == 1) st = mf_fit(model, starts, nullptr, opts, results);
+    else st = mf_fit_batch(model, n_toys, starts, nullptr, opts, results);
+    delete[] starts;
+    mf_model_destroy(model);
+    return st;
+}

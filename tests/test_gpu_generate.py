@@ -122,3 +122,16 @@ def test_generate_4d_matches_oracle_and_feeds_the_model(mf, ctx):
     assert abs(nll - o_nll) <= 1e-11 * abs(o_nll) and np.all(np.abs(g - o_g) <= 1e-9 * (1 + np.abs(o_g)))
     r = model.fit(lam)
     assert r.converged and np.all(np.abs((r.lam - np.array(lam)) / r.sigma) < 5)
+
+
+def test_toy_study_entry(mf, ctx):
+    """mf_toy_study_mass = generate + model + concurrent fits in one call; identical to doing the three steps by hand."""
+    T, n = 512, 5000
+    r = ctx.toy_study_mass(2024, T, n, dg.MASS_TRUTH, LO, HI)
+    ds = ctx.generate_mass(2024, T, n, dg.MASS_TRUTH, LO, HI)
+    r2 = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ds).fit_batch(np.array(dg.MASS_TRUTH))
+    assert r.converged.all() and np.array_equal(r.lam, r2.lam) and np.array_equal(r.cov, r2.cov)
+    pulls = (r.lam - np.array(dg.MASS_TRUTH)) / r.sigma
+    assert np.all(np.abs(pulls.mean(0)) < 0.25) and np.all(np.abs(pulls.std(0) - 1) < 0.15)
+    one = ctx.toy_study_mass(7, 1, 20_000, dg.MASS_TRUTH, LO, HI)
+    assert len(one) == 1 and one.converged[0]
