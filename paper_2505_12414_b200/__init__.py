@@ -220,6 +220,7 @@ class Context:
         self._lib = load_library()
         self._h = ctypes.c_void_p()
         self._children = weakref.WeakSet()   # live datasets / models, closed before the context
+        self._fit_buf = None                 # reused result buffer of the batched fits (fresh pages cost ~2 ms per 4096 toys)
         if stream is None:
             import torch  # device memory / streams come from PyTorch (plumbing only)
             if not torch.cuda.is_available():
@@ -229,6 +230,11 @@ class Context:
         if st != MF_OK:
             raise MoreFitError(st, "mf_ctx_create failed (no usable CUDA device?)")
         self.device = int(device)
+
+    def _fit_results(self, n_toys: int) -> np.ndarray:
+        if self._fit_buf is None or self._fit_buf.size < n_toys:
+            self._fit_buf = np.empty(n_toys, dtype=BatchFitResult._DT)
+        return self._fit_buf[:n_toys]
 
     def _check(self, st: int):
         if st != MF_OK:
@@ -300,7 +306,7 @@ class Context:
                        opts: "FitOpts | None" = None) -> "BatchFitResult":
         """Generate, fit and HESSE n_toys pseudo-experiments of the mass model on the device."""
         lam = np.ascontiguousarray(lam_truth, dtype=np.float64)
-        res = np.empty(int(n_toys), dtype=BatchFitResult._DT)
+        res = self._fit_results(int(n_toys))
         self._check(self._lib.mf_toy_study_mass(self._h, int(seed0), int(n_toys), int(n_events), _dp(lam), float(lo), float(hi),
                                                 None if opts is None else ctypes.byref(opts),
                                                 res.ctypes.data_as(ctypes.POINTER(_FitResultC))))
@@ -479,7 +485,7 @@ class Model:
         if starts.shape == (self.K,):
             starts = np.ascontiguousarray(np.broadcast_to(starts, (T, self.K)))
         fx = None if fixed is None else np.ascontiguousarray(fixed, dtype=np.uint8)
-        res = np.empty(T, dtype=BatchFitResult._DT)   # filled by the library (a ctypes array would be zeroed first: 3.5 ms)
+        res = self._ctx._fit_results(T)   # filled by the library; BatchFitResult copies what it keeps
         st = self._lib.mf_fit_batch(self._h, T, _dp(starts), _u8p(fx), None if opts is None else ctypes.byref(opts),
                                     res.ctypes.data_as(ctypes.POINTER(_FitResultC)))
         self._ctx._check(st)

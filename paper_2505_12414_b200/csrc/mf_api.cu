@@ -60,6 +60,31 @@ static cudaError_t host_slot_acquire(mf_ctx* ctx, double** h, double** d)
     std::memset(*h, 0, sizeof(double) * MF_HOST_SLOT_DOUBLES);
     return cudaSuccess;
 }
+// Pinned staging of a batched call: one grow-only block per context (cudaHostAlloc costs ~1 ms; a toy study creates a
+// model per call).  Batched calls are synchronous, so the block is free again when they return.
+static cudaError_t stage_views(mf_model* m)
+{
+    mf_ctx* ctx = m->ctx;
+    auto up = [](size_t x) { return (x + 255) / 256 * 256; };
+    const size_t T = (size_t)m->n_toys;
+    const size_t b_lam = up(sizeof(double) * T * m->K), b_ids = up(sizeof(int) * T), b_out = up(sizeof(double) * T * m->bout_row);
+    if (ctx->h_stage_bytes < b_lam + b_ids + b_out) {
+        if (ctx->h_stage) {
+            cudaStreamSynchronize(ctx->stream);
+            cudaFreeHost(ctx->h_stage);
+            ctx->h_stage = nullptr;
+            ctx->h_stage_bytes = 0;
+        }
+        const cudaError_t e = cudaHostAlloc(reinterpret_cast<void**>(&ctx->h_stage), b_lam + b_ids + b_out, cudaHostAllocDefault);
+        if (e != cudaSuccess) return e;
+        ctx->h_stage_bytes = b_lam + b_ids + b_out;
+    }
+    m->h_lam = reinterpret_cast<double*>(ctx->h_stage);
+    m->h_ids = reinterpret_cast<int*>(ctx->h_stage + b_lam);
+    m->h_bout = reinterpret_cast<double*>(ctx->h_stage + b_lam + b_ids);
+    return cudaSuccess;
+}
+
 static void host_slot_release(mf_ctx* ctx, double* h)
 {
     if (h && ctx && ctx->h_slab) ctx->free_slots.push_back((int)((h - ctx->h_slab) / MF_HOST_SLOT_DOUBLES));
@@ -108,10 +133,9 @@ extern "C" mf_status mf_ctx_create(int device, void* cuda_stream, mf_ctx** out)
 extern "C" void mf_ctx_destroy(mf_ctx* ctx)
 {
     if (!ctx) return;
-    if (ctx->h_slab) {
-        cudaStreamSynchronize(ctx->stream);
-        cudaFreeHost(ctx->h_slab);
-    }
+    if (ctx->h_slab || ctx->h_stage) cudaStreamSynchronize(ctx->stream);
+    if (ctx->h_slab) cudaFreeHost(ctx->h_slab);
+    if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
     cudaGetLastError();
     delete ctx;
 }
@@ -260,9 +284,6 @@ extern "C" void mf_model_destroy(mf_model* m)
     dev_free(m->ctx, m->d_ids);
     dev_free(m->ctx, m->d_bout);
     host_slot_release(m->ctx, m->h_out);
-    if (m->h_lam) cudaFreeHost(m->h_lam);
-    if (m->h_ids) cudaFreeHost(m->h_ids);
-    if (m->h_bout) cudaFreeHost(m->h_bout);
     devbuf_release(m->raw);
     cudaGetLastError();
     delete m;
@@ -371,9 +392,7 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
         MF_CUDA_M(dev_alloc(ctx, &m->d_ids, sizeof(int) * T));
         const int nout1 = (kind == MF_MASS_GAUSS_EXP ? MassHessModel::NOUT : kind == MF_ANGULAR_KSTMUMU ? AngularHessModel::NOUT : K + 1) + 1;  // widest output row + n_bad
         MF_CUDA_M(dev_alloc(ctx, &m->d_bout, sizeof(double) * T * nout1));
-        MF_CUDA_M(cudaHostAlloc(&m->h_lam, sizeof(double) * T * K, cudaHostAllocDefault));
-        MF_CUDA_M(cudaHostAlloc(&m->h_ids, sizeof(int) * T, cudaHostAllocDefault));
-        MF_CUDA_M(cudaHostAlloc(&m->h_bout, sizeof(double) * T * nout1, cudaHostAllocDefault));
+        m->bout_row = nout1;  // the pinned staging of these arrays lives in the context (stage_views)
     }
     {
         const cudaError_t e_sync = cudaStreamSynchronize(ctx->stream);
@@ -705,6 +724,7 @@ static mf_status eval_batch(mf_model* m, int64_t n_toys, const double* lambdas, 
         if (st == MF_OK && grad) std::memcpy(grad, g, sizeof(double) * K);
         return st;
     }
+    MF_CUDA(ctx, stage_views(m));
     int n_active = 0;
     for (int64_t t = 0; t < n_toys; ++t) {
         if (active && !active[t]) continue;

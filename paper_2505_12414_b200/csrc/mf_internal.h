@@ -18,6 +18,9 @@ struct mf_ctx {
     double* h_slab = nullptr;
     double* d_slab = nullptr;
     std::vector<int> free_slots;
+    // pinned staging of the batched (synchronous) calls, shared by all models of the context, grow-only
+    char* h_stage = nullptr;
+    size_t h_stage_bytes = 0;
 };
 
 constexpr int MF_HOST_SLOT_DOUBLES = 64;  // widest output row (angular Hessian: 45 + n_bad) and the done word
@@ -73,9 +76,10 @@ struct mf_model {
     double* d_lam = nullptr;          // device [n_toys][K]
     int* d_ids = nullptr;             // device [n_toys]
     double* d_bout = nullptr;         // device [n_toys][K+2]
-    double* h_lam = nullptr;          // pinned [n_toys][K]
-    int* h_ids = nullptr;             // pinned [n_toys]
-    double* h_bout = nullptr;         // pinned [n_toys][K+2]
+    double* h_lam = nullptr;          // views into the context's pinned staging block, set by every batched call:
+    int* h_ids = nullptr;             //   [n_toys][K], [n_toys], [n_toys][widest output row]
+    double* h_bout = nullptr;
+    int bout_row = 0;                 // widest output row + n_bad (doubles)
 };
 
 // Sets ctx->err and returns st (mf_api.cu).
