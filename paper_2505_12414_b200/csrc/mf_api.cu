@@ -9,6 +9,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <type_traits>
 #include <utility>
 #include <vector>
 
@@ -413,17 +414,18 @@ extern "C" int64_t mf_model_n_toys(const mf_model* m) { return m ? m->n_toys : 0
 // Launch with programmatic stream serialisation: the kernel may begin while its predecessor on the
 // stream (if that is one of ours) is still in its tail; see pdl_wait() in mf_kernels.cuh.
 template <class Args>
-static cudaError_t launch_pdl(void (*kernel)(const Args), int grid, cudaStream_t stream, const Args& a, int block = kBlock)
+static cudaError_t launch_pdl(void (*kernel)(const Args), int grid, cudaStream_t stream, const Args& a, int block = kBlock,
+                              size_t smem = 0)
 {
     static const bool no_pdl = std::getenv("MF_NO_PDL") != nullptr;  // ablation switch: plain stream order
     if (no_pdl) {
-        kernel<<<grid, block, 0, stream>>>(a);
+        kernel<<<grid, block, smem, stream>>>(a);
         return cudaGetLastError();
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)grid);
     cfg.blockDim = dim3((unsigned)block);
-    cfg.dynamicSmemBytes = 0;
+    cfg.dynamicSmemBytes = smem;
     cfg.stream = stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
@@ -502,6 +504,20 @@ static mf_status launch_single(mf_model* m, const double* lam, double* out_dev, 
     a.done_flag = signal_host ? reinterpret_cast<unsigned long long*>(m->d_out_mapped + MF_HOST_DONE_INDEX) : nullptr;
     a.done_value = m->seq + 1;
     const int grid = (pipelined && M::CTAS_PER_SM > 1 && m->grid > ctx->sm_count) ? std::max(ctx->sm_count, m->grid / 2) : m->grid;
+    if constexpr (std::is_same<M, AngularModel>::value || std::is_same<M, FourDModel>::value) {
+        // 9 / 12 columns per event, HBM bound: columns staged through shared memory by the bulk-copy engine
+        static const bool no_tma = std::getenv("MF_NO_TMA") != nullptr;  // ablation switch
+        if (!no_tma && m->n_pad >= 4 * kBlock) {
+            static const cudaError_t attr_set = cudaFuncSetAttribute(nll_grad_tma_kernel<M>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                                     (int)tma_smem_bytes<M>());
+            MF_CUDA(ctx, attr_set);
+            const int tgrid = (int)std::min<int64_t>((m->n_pad + kBlock - 1) / kBlock, 2 * (int64_t)ctx->sm_count);
+            MF_CUDA(ctx, launch_pdl(nll_grad_tma_kernel<M>, std::min(tgrid, m->grid), ctx->stream, a, kBlock, tma_smem_bytes<M>()));
+            ++m->seq;
+            ++ctx->launches;
+            return MF_OK;
+        }
+    }
     MF_CUDA(ctx, launch_pdl(nll_grad_kernel<M>, grid, ctx->stream, a));
     ++m->seq;
     ++ctx->launches;

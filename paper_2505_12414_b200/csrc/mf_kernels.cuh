@@ -391,10 +391,12 @@ __device__ __forceinline__ void final_combine(const double* p, int64_t stride_k,
     }
 }
 
-// ---- the fused single-dataset kernel (mf_nll_grad) ----------------------------------------------
+// ---- the fused single-dataset kernels (mf_nll_grad) ---------------------------------------------
 
+// S4 + S5 of a single-dataset evaluation: thread sums -> block partial in this evaluation's scratch slot -> the CTA
+// that draws the last ticket combines and finishes.  Called by every thread of every CTA.
 template <class M>
-__global__ void __launch_bounds__(kBlock, M::RESIDENT_CTAS) nll_grad_kernel(const __grid_constant__ EvalArgs<M> a)
+__device__ __forceinline__ void reduce_and_finish(const EvalArgs<M>& a, double* acc, unsigned bad)
 {
     constexpr int NACC = M::NACC;
     __shared__ double sm[kWarps][NACC];
@@ -402,16 +404,7 @@ __global__ void __launch_bounds__(kBlock, M::RESIDENT_CTAS) nll_grad_kernel(cons
     __shared__ unsigned sm_bad[kWarps];
     __shared__ unsigned s_bad_block;
     __shared__ bool s_last;
-
-    pdl_launch_dependents();
-    double acc[NACC];
-#pragma unroll
-    for (int k = 0; k < NACC; ++k) acc[k] = 0.0;
-    unsigned bad = 0;
     const int64_t G = gridDim.x;
-    accumulate<M>(a.col, a.n, a.n_items, blockIdx.x + G * (threadIdx.x >> 5), G * kWarps,
-                  [&]() -> const typename M::Consts& { return a.c; }, acc, bad);
-
     if (threadIdx.x == 0)
         while (gen_load(a.gen) < a.need) __nanosleep(64);  // slot still in use by evaluation e - kRing (rare)
     const double s = block_reduce<NACC>(acc, bad, sm, sm_bad, &s_bad_block);  // contains a __syncthreads()
@@ -430,6 +423,105 @@ __global__ void __launch_bounds__(kBlock, M::RESIDENT_CTAS) nll_grad_kernel(cons
             gen_store(a.gen, a.need + 1);  // releases the slot (and the ticket reset) to evaluation e + kRing
         }
     }
+}
+
+
+template <class M>
+__global__ void __launch_bounds__(kBlock, M::RESIDENT_CTAS) nll_grad_kernel(const __grid_constant__ EvalArgs<M> a)
+{
+    constexpr int NACC = M::NACC;
+    pdl_launch_dependents();
+    double acc[NACC];
+#pragma unroll
+    for (int k = 0; k < NACC; ++k) acc[k] = 0.0;
+    unsigned bad = 0;
+    const int64_t G = gridDim.x;
+    accumulate<M>(a.col, a.n, a.n_items, blockIdx.x + G * (threadIdx.x >> 5), G * kWarps,
+                  [&]() -> const typename M::Consts& { return a.c; }, acc, bad);
+
+    reduce_and_finish<M>(a, acc, bad);
+}
+
+// The same evaluation for the many-column, HBM-bound models, with the event columns staged through shared memory by
+// the bulk asynchronous copy engine (cp.async.bulk + mbarrier: "TMA" in its 1-D form): a tile is 256 consecutive events
+// of every column (NCOL x 2 KB), STAGES tiles are in flight per CTA whatever the register budget, thread t evaluates
+// event t of the tile.  Thread 0 re-arms a stage as soon as the CTA has consumed it.  Tiles are dealt block-cyclically.
+constexpr int kTmaStages = 4;
+
+template <class M>
+constexpr size_t tma_smem_bytes()
+{
+    return sizeof(double) * kTmaStages * M::NCOL * kBlock + sizeof(unsigned long long) * kTmaStages;
+}
+
+template <class M>
+__global__ void __launch_bounds__(kBlock, 2) nll_grad_tma_kernel(const __grid_constant__ EvalArgs<M> a)
+{
+    constexpr int NACC = M::NACC, NC = M::NCOL, TILE = kBlock, STAGES = kTmaStages;
+    extern __shared__ __align__(128) unsigned char tma_raw[];
+    double (*buf)[NC][TILE] = reinterpret_cast<double (*)[NC][TILE]>(tma_raw);
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(tma_raw + sizeof(double) * STAGES * NC * TILE);
+    const int tid = threadIdx.x;
+    const int64_t n_pad = a.n_items * kItem, n_tiles = (n_pad + TILE - 1) / TILE, G = gridDim.x;
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < STAGES; ++s)
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"((unsigned)__cvta_generic_to_shared(&bar[s])));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    pdl_launch_dependents();
+    auto issue = [&](int s, int64_t tile) {  // thread 0: arm stage s with tile `tile`
+        const int64_t first = tile * TILE;
+        const unsigned len = (unsigned)((n_pad - first < TILE) ? (n_pad - first) : TILE);  // multiple of 64 events
+        const unsigned bytes = len * (unsigned)sizeof(double);
+        const unsigned mb = (unsigned)__cvta_generic_to_shared(&bar[s]);
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mb), "r"(bytes * NC) : "memory");
+#pragma unroll
+        for (int c = 0; c < NC; ++c)
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                             (unsigned)__cvta_generic_to_shared(&buf[s][c][0])),
+                         "l"(a.col[c] + first), "r"(bytes), "r"(mb)
+                         : "memory");
+    };
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < STAGES; ++s)
+            if (blockIdx.x + s * G < n_tiles) issue(s, blockIdx.x + s * G);
+    }
+    double acc[NACC];
+#pragma unroll
+    for (int k = 0; k < NACC; ++k) acc[k] = 0.0;
+    unsigned bad = 0;
+    LogProd lp;
+    const double t_lane = mf_exp32_lane_entry();
+    int i = 0;
+    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += G, ++i) {
+        const int s = i % STAGES;
+        const unsigned phase = (unsigned)(i / STAGES) & 1u, mb = (unsigned)__cvta_generic_to_shared(&bar[s]);
+        unsigned done = 0;
+        while (!done)
+            asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                         : "=r"(done)
+                         : "r"(mb), "r"(phase)
+                         : "memory");
+        const int64_t e = tile * TILE + tid;
+        double x[NC];
+        if (e < n_pad) {
+#pragma unroll
+            for (int c = 0; c < NC; ++c) x[c] = buf[s][c][tid];
+        } else {
+#pragma unroll
+            for (int c = 0; c < NC; ++c) x[c] = 1.0;  // beyond the padded columns: any finite value, the lane is invalid
+        }
+        if ((tile + 1) * TILE <= a.n) M::template event<false>(x, a.c, acc, lp, bad, true, t_lane);
+        else M::template event<true>(x, a.c, acc, lp, bad, e < a.n, t_lane);
+        lp.renorm();
+        __syncthreads();  // the whole CTA has consumed stage s
+        if (tid == 0 && tile + STAGES * G < n_tiles) issue(s, tile + STAGES * G);
+    }
+    acc[0] = lp.log();
+    reduce_and_finish<M>(a, acc, bad);
 }
 
 // ---- the batched-toy kernels (mf_nll_grad_batch) -------------------------------------------------

@@ -525,7 +525,7 @@ struct FourDModel {
     static constexpr int RESIDENT_CTAS = 1;
     static constexpr int BATCH_RESIDENT_CTAS = 1;
     static constexpr int BATCH_BLOCK = 256;
-    static constexpr int CTAS_PER_SM = 1;  // 17 sums + two 12-column register buffers: needs > 128 registers
+    static constexpr int CTAS_PER_SM = 2;  // grid of the shared-memory-staged kernel (the register-buffer kernel, 255 registers, 1 resident CTA/SM, serves only n < 1024)
     using Consts = FourDConsts;
 
     template <bool PRED>
