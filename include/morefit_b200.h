@@ -121,7 +121,11 @@ mf_status mf_generate_angular(mf_ctx* ctx, uint64_t seed0, int64_t n_toys, int64
 /* The same for the 4D model (ndim = 4: m, cos theta_l, cos theta_K, phi; BASELINE.json configs[3]).  lam: host, the 16
  * parameters f, mu, sigma, tau, the 8 angular coefficients, cl1, cl2, ck1, ck2.  Signal (probability f): Gaussian mass and
  * angular accept-reject as above; background: exponential mass by inverse CDF, flat phi, (cos theta_l, cos theta_K) by
- * accept-reject of the Legendre product under 1/2 (1 + |c1| + |c2|) per factor.  Draw layout: mf_generate.cu. */
+ * accept-reject of the Legendre product under 1/2 (1 + |c1| + |c2|) per factor.
+ * Draw layout of event i (Philox counter (i, draw), two uniforms per draw): draw 0 = (component choice, background mass);
+ * signal: draws 1..64 Box-Muller mass candidates, draws 100+2k, 101+2k = angular proposal k (cos theta_l, cos theta_K |
+ * phi, accept); background: draw 1 = (phi, unused), draws 100+2k, 101+2k = Legendre proposal k (cos theta_l,
+ * cos theta_K | accept, unused). */
 mf_status mf_generate_4d(mf_ctx* ctx, uint64_t seed0, int64_t n_toys, int64_t n_events, const double* lam, double lo, double hi,
                          mf_dataset** out);
 
@@ -145,7 +149,7 @@ int64_t mf_model_n_toys(const mf_model* model);
 /* -ln L and d(-ln L)/d lambda_k at `lambda` over all events of a 1-toy dataset.
  *   lambda  host, K doubles.   nll  host, 1 double.   grad  host, K doubles or NULL.
  * One kernel launch (parameter-only constants of Eq. 3, are computed on
- * the host and passed as kernel arguments), then one stream synchronise.
+ * the host and passed as kernel arguments); the host then waits on a completion word in mapped memory.
  * MF_ERR_ARG if the dataset has n_toys != 1.  See mf_status for the domain / P<=0 cases. */
 mf_status mf_nll_grad(mf_model* model, const double* lambda, double* nll, double* grad);
 
@@ -160,10 +164,20 @@ mf_status mf_nll_grad_async(mf_model* model, const double* lambda, double* out_d
  *   lambdas  host, [n_points][K].   out_dev  DEVICE, [n_points][K+2], row p = [-ln L, grad, n_bad] at point p.
  * Fewer than 16 points: mf_nll_grad_async n_points times (one launch each, pipelined).  Otherwise ONE launch
  * whose CTA tile is (point, event chunk), the parameter-only constants of every point being derived on the host
- * and uploaded (the dataset is read from HBM once and re-read from L2 by the other points).
+ * and uploaded through a pinned staging ring (the dataset is read from HBM once and re-read from L2 by the other
+ * points).  No allocation, clearing or synchronisation per call once the model's scratch has grown to its size.
  * Every point is validated first: MF_ERR_PARAM_DOMAIN (nothing enqueued) if one is outside the domain
  * (for fewer than 16 points the earlier ones are enqueued). */
 mf_status mf_nll_grad_points(mf_model* model, int64_t n_points, const double* lambdas, double* out_dev);
+
+/* The same sweep with the results returned to the HOST: evaluates the n_points parameter points (as
+ * mf_nll_grad_points does), copies the results back and synchronises.
+ *   lambdas  host, [n_points][K].   nll  host, [n_points].   grad  host, [n_points][K] or NULL.
+ *   n_bad    host, 1 integer or NULL: number of points at which some event had P <= 0 (those points have
+ *            nll = +inf, grad = NaN; the call still returns MF_OK).
+ * MF_ERR_PARAM_DOMAIN (nothing evaluated) if a point is outside the parameter domain. */
+mf_status mf_nll_grad_sweep(mf_model* model, int64_t n_points, const double* lambdas, double* nll, double* grad,
+                            int64_t* n_bad);
 
 /* T pseudo-experiments at their own parameter points in ONE launch (BASELINE.json
  * configs[4]): a CTA tile is (toy, event chunk); the toys' parameter-only constants are
@@ -179,7 +193,10 @@ mf_status mf_nll_grad_batch(mf_model* model, int64_t n_toys, const double* lambd
 
 /* The same evaluation for ALL toys without host copies or synchronisation: lambdas_dev is DEVICE [n_toys][K],
  * out_dev DEVICE [n_toys][K+2], row t = [-ln L, grad, n_bad] of toy t (n_bad = -1: lambda_t outside the domain).
- * Two launches are enqueued on the context's stream (parameter-only constants, then the fused kernel). */
+ * Two launches are enqueued on the context's stream (parameter-only constants, then the fused kernel).
+ * lambdas_dev may have been written by the caller's own kernel enqueued earlier on the same stream (a device-side
+ * minimiser step): the constants kernel reads it only after the programmatic-launch wait, i.e. once that work has
+ * completed and its writes are visible. */
 mf_status mf_nll_grad_batch_async(mf_model* model, int64_t n_toys, const double* lambdas_dev, double* out_dev);
 
 /* ---- value + gradient + analytic Hessian ---------------------- */
@@ -252,20 +269,15 @@ mf_status mf_fit_batch(mf_model* model, int64_t n_toys, const double* starts,
 mf_status mf_toy_study_mass(mf_ctx* ctx, uint64_t seed0, int64_t n_toys, int64_t n_events, const double* lam_truth, double lo,
                             double hi, const mf_fit_opts* opts, mf_fit_result* results);
 
-/* ---- measurement helpers (not on the hot path) ------------------------ */
+/* ---- multi-GPU: S5 across ranks ------------------------------------------------------ */
 
-/* fp64-pipe issue rate of this GPU in DFMA thread-instructions per second, measured with
- * register-only DFMA chains (nominal B200: 148 SMs x 64 lanes x 1.965 GHz = 1.86e13). */
-mf_status mf_probe_fp64_rate(mf_ctx* ctx, double* dfma_per_second);
-/* Read bandwidth in bytes/s of a `bytes`-sized device buffer that one kernel reads `repeats`
- * times with 16-byte loads: L2 bandwidth when bytes fits the L2 and repeats > 1, HBM otherwise. */
-mf_status mf_probe_read_bandwidth(mf_ctx* ctx, size_t bytes, int repeats, double* bytes_per_second);
-/* Evaluates the kernels' own device math element by element, for the accuracy tests:
- * op 0 = exp (finite x < 709; x <= -708 gives 0), 1 = log (positive normal x), 2 = reciprocal,
- * 3 = the table-by-shuffle exp the event loops use (same domain; x below about -708 gives a value in
- *     [2^-1022, 2^-1021], which the kernels treat as zero, instead of 0).
- * x_host, y_host: host, n doubles. */
-mf_status mf_probe_math(mf_ctx* ctx, int op, int64_t n, const double* x_host, double* y_host);
+/* Combines the partial sums of n_ranks event shards of ONE dataset (each rank's mf_nll_grad on its shard: -ln L and the
+ * gradient are sums over events, Eq. 1) into the totals.  Host arithmetic, no device needed.
+ *   rows  host, [n_ranks][width], rank r's `width` partial sums in row r (gathered by the caller, e.g. all_gather).
+ *   out   host, [width].
+ * Every column is added in RANK ORDER with two-sum compensation, so all ranks obtain bit-identical totals whatever the
+ * collective's reduction tree; a column holding +inf or NaN (a shard with P <= 0) is added plainly and propagates. */
+mf_status mf_combine_partials(int n_ranks, int width, const double* rows, double* out);
 
 #ifdef __cplusplus
 }

@@ -34,10 +34,10 @@ EXPORTS = [
     "mf_ctx_create", "mf_ctx_destroy", "mf_last_error", "mf_ctx_kernel_launches",
     "mf_dataset_upload", "mf_generate_mass", "mf_generate_angular", "mf_generate_4d", "mf_dataset_download", "mf_dataset_destroy", "mf_dataset_n_events", "mf_dataset_n_toys",
     "mf_model_create", "mf_model_destroy", "mf_model_nparams", "mf_model_n_events", "mf_model_n_toys",
-    "mf_nll_grad", "mf_nll_grad_async", "mf_nll_grad_points", "mf_nll_grad_batch", "mf_nll_grad_batch_async",
+    "mf_nll_grad", "mf_nll_grad_async", "mf_nll_grad_points", "mf_nll_grad_sweep", "mf_nll_grad_batch", "mf_nll_grad_batch_async",
     "mf_model_has_hessian", "mf_nll_grad_hess", "mf_nll_grad_hess_batch",
     "mf_fit_opts_default", "mf_fit", "mf_fit_batch", "mf_toy_study_mass",
-    "mf_probe_fp64_rate", "mf_probe_read_bandwidth", "mf_probe_math",
+    "mf_combine_partials",
 ]
 
 
@@ -189,12 +189,10 @@ def load_library() -> ctypes.CDLL:
     lib.mf_toy_study_mass.restype = ctypes.c_int
     lib.mf_toy_study_mass.argtypes = [vp, ctypes.c_uint64, i64, i64, dp, ctypes.c_double, ctypes.c_double, ctypes.POINTER(FitOpts),
                                       ctypes.POINTER(_FitResultC)]
-    lib.mf_probe_fp64_rate.restype = ctypes.c_int
-    lib.mf_probe_fp64_rate.argtypes = [vp, dp]
-    lib.mf_probe_read_bandwidth.restype = ctypes.c_int
-    lib.mf_probe_read_bandwidth.argtypes = [vp, ctypes.c_size_t, ctypes.c_int, dp]
-    lib.mf_probe_math.restype = ctypes.c_int
-    lib.mf_probe_math.argtypes = [vp, ctypes.c_int, i64, dp, dp]
+    lib.mf_nll_grad_sweep.restype = ctypes.c_int
+    lib.mf_nll_grad_sweep.argtypes = [vp, i64, dp, dp, dp, ctypes.POINTER(i64)]
+    lib.mf_combine_partials.restype = ctypes.c_int
+    lib.mf_combine_partials.argtypes = [ctypes.c_int, ctypes.c_int, dp, dp]
     _lib = lib
     return lib
 
@@ -205,6 +203,18 @@ def _dp(a: np.ndarray):
 
 def _u8p(a):
     return None if a is None else a.ctypes.data_as(ctypes.POINTER(ctypes.c_uint8))
+
+
+def combine_partials(rows) -> np.ndarray:
+    """mf_combine_partials: rows [n_ranks][width] -> rank-ordered compensated column sums [width] (host only)."""
+    rows = np.ascontiguousarray(rows, dtype=np.float64)
+    if rows.ndim != 2:
+        raise ValueError("rows must be [n_ranks][width]")
+    out = np.empty(rows.shape[1], dtype=np.float64)
+    st = load_library().mf_combine_partials(rows.shape[0], rows.shape[1], _dp(rows), _dp(out))
+    if st != MF_OK:
+        raise MoreFitError(st, "mf_combine_partials")
+    return out
 
 
 def default_fit_opts() -> FitOpts:
@@ -243,25 +253,6 @@ class Context:
     @property
     def kernel_launches(self) -> int:
         return int(self._lib.mf_ctx_kernel_launches(self._h))
-
-    def probe_fp64_rate(self) -> float:
-        """Measured fp64-pipe rate (DFMA thread-instructions per second)."""
-        v = ctypes.c_double()
-        self._check(self._lib.mf_probe_fp64_rate(self._h, ctypes.byref(v)))
-        return float(v.value)
-
-    def probe_read_bandwidth(self, nbytes: int, repeats: int = 1) -> float:
-        """Measured read bandwidth (bytes/s) of an nbytes working set read `repeats` times."""
-        v = ctypes.c_double()
-        self._check(self._lib.mf_probe_read_bandwidth(self._h, int(nbytes), int(repeats), ctypes.byref(v)))
-        return float(v.value)
-
-    def probe_math(self, op: str, x) -> np.ndarray:
-        """The kernels' device exp / log / rcp evaluated element-wise (accuracy tests)."""
-        x = np.ascontiguousarray(x, dtype=np.float64)
-        y = np.empty_like(x)
-        self._check(self._lib.mf_probe_math(self._h, {"exp": 0, "log": 1, "rcp": 2, "exp32": 3}[op], x.size, _dp(x), _dp(y)))
-        return y
 
     def dataset_upload(self, columns, lo=None, hi=None, n_toys: int = 1) -> "Dataset":
         """columns: numpy array [ndim][n_toys*n_events] (or 1-D for ndim = 1; [n_toys][n_events] for
@@ -428,6 +419,19 @@ class Model:
         if lam.ndim != 2 or lam.shape[1] != self.K:
             raise ValueError(f"lambdas must be [n][{self.K}]")
         self._ctx._check(self._lib.mf_nll_grad_points(self._h, lam.shape[0], _dp(lam), ctypes.c_void_p(out_dev_ptr)))
+
+    def nll_grad_sweep(self, lambdas, want_grad: bool = True):
+        """lambdas [n][K] (host) -> (nll [n], grad [n][K], number of points with P <= 0 events), results on the host."""
+        lam = np.ascontiguousarray(lambdas, dtype=np.float64)
+        if lam.ndim != 2 or lam.shape[1] != self.K:
+            raise ValueError(f"lambdas must be [n][{self.K}]")
+        n = lam.shape[0]
+        nll = np.empty(n)
+        grad = np.empty((n, self.K)) if want_grad else None
+        nbad = ctypes.c_int64(0)
+        self._ctx._check(self._lib.mf_nll_grad_sweep(self._h, n, _dp(lam), _dp(nll), None if grad is None else _dp(grad),
+                                                     ctypes.byref(nbad)))
+        return nll, grad, int(nbad.value)
 
     def nll_grad_batch(self, lambdas, active=None):
         """lambdas [T][K] -> (nll [T], grad [T][K]); inactive toys are NaN in the returned arrays."""

@@ -134,9 +134,13 @@ extern "C" mf_status mf_ctx_create(int device, void* cuda_stream, mf_ctx** out)
 extern "C" void mf_ctx_destroy(mf_ctx* ctx)
 {
     if (!ctx) return;
-    if (ctx->h_slab || ctx->h_stage) cudaStreamSynchronize(ctx->stream);
+    cudaStreamSynchronize(ctx->stream);
     if (ctx->h_slab) cudaFreeHost(ctx->h_slab);
     if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
+    for (int i = 0; i < mf_ctx::kPointStages; ++i) {
+        if (ctx->h_pts[i]) cudaFreeHost(ctx->h_pts[i]);
+        if (ctx->pts_copied[i]) cudaEventDestroy(ctx->pts_copied[i]);
+    }
     cudaGetLastError();
     delete ctx;
 }
@@ -284,6 +288,8 @@ extern "C" void mf_model_destroy(mf_model* m)
     dev_free(m->ctx, m->d_consts_ok);
     dev_free(m->ctx, m->d_ids);
     dev_free(m->ctx, m->d_bout);
+    dev_free(m->ctx, m->p_blk);
+    dev_free(m->ctx, m->d_sweep);
     host_slot_release(m->ctx, m->h_out);
     devbuf_release(m->raw);
     cudaGetLastError();
@@ -364,7 +370,8 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
             ++ctx->launches;
         }
         MF_CUDA_M(cudaGetLastError());
-        MF_CUDA_M(cudaMemcpyAsync(&m->h_sum_m, m->d_sum_m, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        dev_free(ctx, d_part);  // stream-ordered: released after the finish kernel
+        d_part = nullptr;
     }
     // launch geometry: persistent-style grid, CTAS_PER_SM CTAs per SM (one wave), never more CTAs than 8-warp groups of items
     const int64_t n_items = m->n_pad / kItem;
@@ -395,11 +402,8 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
         MF_CUDA_M(dev_alloc(ctx, &m->d_bout, sizeof(double) * T * nout1));
         m->bout_row = nout1;  // the pinned staging of these arrays lives in the context (stage_views)
     }
-    {
-        const cudaError_t e_sync = cudaStreamSynchronize(ctx->stream);
-        dev_free(ctx, d_part);
-        MF_CUDA_M(e_sync);
-    }
+    // nothing here needs the host to wait: the kernels read sum_i m_i from device memory, so a model is ready to be
+    // evaluated (in stream order) as soon as this returns
 #undef MF_CUDA_M
     *out = m;
     return MF_OK;
@@ -413,15 +417,14 @@ extern "C" int64_t mf_model_n_toys(const mf_model* m) { return m ? m->n_toys : 0
 
 // Launch with programmatic stream serialisation: the kernel may begin while its predecessor on the
 // stream (if that is one of ours) is still in its tail; see pdl_wait() in mf_kernels.cuh.
-template <class Args>
-static cudaError_t launch_pdl(void (*kernel)(const Args), int grid, cudaStream_t stream, const Args& a, int block = kBlock,
-                              size_t smem = 0)
+// allow == false: plain stream order.  The FIRST launch on a model after mf_model_create is made that way: its
+// predecessors are the S0/S1 kernels (padding, range check, basis columns, sum_i m_i), whose output the event loop reads
+// ahead of any griddepcontrol.wait, and model creation does not synchronise the host any more.
+template <class... KArgs, class... Args>
+static cudaError_t launch_pdl_v(void (*kernel)(KArgs...), int grid, int block, size_t smem, cudaStream_t stream, bool allow,
+                                Args&&... args)
 {
-    static const bool no_pdl = std::getenv("MF_NO_PDL") != nullptr;  // ablation switch: plain stream order
-    if (no_pdl) {
-        kernel<<<grid, block, smem, stream>>>(a);
-        return cudaGetLastError();
-    }
+    static const bool no_pdl = std::getenv("MF_NO_PDL") != nullptr;  // ablation switch: plain stream order everywhere
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)grid);
     cfg.blockDim = dim3((unsigned)block);
@@ -429,28 +432,25 @@ static cudaError_t launch_pdl(void (*kernel)(const Args), int grid, cudaStream_t
     cfg.stream = stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, kernel, a);
-}
-
-// The same for kernels with more than one parameter.
-template <class... KArgs, class... Args>
-static cudaError_t launch_pdl_v(void (*kernel)(KArgs...), int grid, int block, cudaStream_t stream, Args&&... args)
-{
-    static const bool no_pdl = std::getenv("MF_NO_PDL") != nullptr;
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)grid);
-    cfg.blockDim = dim3((unsigned)block);
-    cfg.dynamicSmemBytes = 0;
-    cfg.stream = stream;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = no_pdl ? 0 : 1;
+    attr[0].val.programmaticStreamSerializationAllowed = (no_pdl || !allow) ? 0 : 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
+
+template <class Args>
+static cudaError_t launch_pdl(void (*kernel)(const Args), int grid, cudaStream_t stream, const Args& a, int block = kBlock,
+                              size_t smem = 0, bool allow = true)
+{
+    return launch_pdl_v(kernel, grid, block, smem, stream, allow, a);
+}
+
+// true exactly once per model: its first launch must not overlap the S0/S1 kernels
+static bool take_fresh(mf_model* m)
+{
+    const bool f = m->fresh;
+    m->fresh = false;
+    return f;
 }
 
 template <class M>
@@ -493,7 +493,7 @@ static mf_status launch_single(mf_model* m, const double* lam, double* out_dev, 
     for (int i = 0; i < M::NCOL; ++i) a.col[i] = m->col[i];
     a.n = m->n_events;
     a.n_items = m->n_pad / kItem;
-    a.sum_m = m->h_sum_m;
+    a.sum_m = m->d_sum_m;
     const int slot = (int)(m->seq % kRing);
     a.partials = m->partials + (int64_t)slot * m->nacc * m->grid;
     a.bad_partials = m->bad_partials + (int64_t)slot * m->grid;
@@ -512,13 +512,14 @@ static mf_status launch_single(mf_model* m, const double* lam, double* out_dev, 
                                                                      (int)tma_smem_bytes<M>());
             MF_CUDA(ctx, attr_set);
             const int tgrid = (int)std::min<int64_t>((m->n_pad + kBlock - 1) / kBlock, 2 * (int64_t)ctx->sm_count);
-            MF_CUDA(ctx, launch_pdl(nll_grad_tma_kernel<M>, std::min(tgrid, m->grid), ctx->stream, a, kBlock, tma_smem_bytes<M>()));
+            MF_CUDA(ctx, launch_pdl(nll_grad_tma_kernel<M>, std::min(tgrid, m->grid), ctx->stream, a, kBlock, tma_smem_bytes<M>(),
+                                    !take_fresh(m)));
             ++m->seq;
             ++ctx->launches;
             return MF_OK;
         }
     }
-    MF_CUDA(ctx, launch_pdl(nll_grad_kernel<M>, grid, ctx->stream, a));
+    MF_CUDA(ctx, launch_pdl(nll_grad_kernel<M>, grid, ctx->stream, a, kBlock, 0, !take_fresh(m)));
     ++m->seq;
     ++ctx->launches;
     return MF_OK;
@@ -548,15 +549,46 @@ extern "C" mf_status mf_nll_grad_async(mf_model* m, const double* lambda, double
 
 // Several parameter points on ONE dataset in one launch: the batched kernel with every slot reading toy 0.
 // The parameter-only constants are derived on the host (which also validates every point before anything is
-// enqueued) and uploaded; a CTA is (point, event chunk); chunk sums are combined per point in fixed order.
+// enqueued), written into a pinned staging block and copied to the model's grow-only scratch; a CTA is
+// (point, event chunk); chunk sums are combined per point in fixed order.  Nothing is allocated, freed or cleared per
+// call once the scratch has reached its size (the tickets are left at zero by the kernel itself).
+static cudaError_t points_stage(mf_ctx* ctx, size_t bytes, char** h, int* stage)
+{
+    const int s = (int)(ctx->pts_seq++ % mf_ctx::kPointStages);
+    if (ctx->pts_copied[s]) {
+        const cudaError_t e = cudaEventSynchronize(ctx->pts_copied[s]);  // the copy that last used this block (long done)
+        if (e != cudaSuccess) return e;
+    } else {
+        const cudaError_t e = cudaEventCreateWithFlags(&ctx->pts_copied[s], cudaEventDisableTiming);
+        if (e != cudaSuccess) return e;
+    }
+    if (ctx->h_pts_bytes[s] < bytes) {
+        if (ctx->h_pts[s]) cudaFreeHost(ctx->h_pts[s]);
+        ctx->h_pts[s] = nullptr;
+        ctx->h_pts_bytes[s] = 0;
+        const size_t want = std::max<size_t>(bytes, 64 * 1024);
+        const cudaError_t e = cudaHostAlloc(reinterpret_cast<void**>(&ctx->h_pts[s]), want, cudaHostAllocDefault);
+        if (e != cudaSuccess) return e;
+        ctx->h_pts_bytes[s] = want;
+    }
+    *h = ctx->h_pts[s];
+    *stage = s;
+    return cudaSuccess;
+}
+
 template <class M>
 static mf_status launch_points(mf_model* m, int64_t n_points, const double* lambdas, double* out_dev)
 {
     mf_ctx* ctx = m->ctx;
     const int K = M::K;
-    std::vector<typename M::Consts> hc((size_t)n_points);
+    using Consts = typename M::Consts;
+    const size_t b_consts = sizeof(Consts) * n_points;
+    char* h_blk = nullptr;
+    int stage = 0;
+    MF_CUDA(ctx, points_stage(ctx, b_consts, &h_blk, &stage));
+    Consts* hc = reinterpret_cast<Consts*>(h_blk);
     for (int64_t p = 0; p < n_points; ++p)
-        if (!host_consts<M>(m, lambdas + p * K, hc[(size_t)p]))
+        if (!host_consts<M>(m, lambdas + p * K, hc[p]))
             return mf_fail(ctx, MF_ERR_PARAM_DOMAIN, "mf_nll_grad_points: lambda " + std::to_string((long long)p) +
                                                          " is outside the parameter domain");
     // CTAs: whole waves of the resident capacity, about 64k events per CTA
@@ -564,14 +596,29 @@ static mf_status launch_points(mf_model* m, int64_t n_points, const double* lamb
     static const int64_t per_cta = std::getenv("MF_POINTS_CTA_EVENTS") ? std::atoll(std::getenv("MF_POINTS_CTA_EVENTS")) : 65536;  // tuning knob
     const int64_t waves = std::max<int64_t>(1, (n_points * m->n_pad + slots * per_cta - 1) / (slots * per_cta));
     const int64_t max_chunks = std::max<int64_t>(1, (m->n_pad / kItem + M::BATCH_BLOCK / 32 - 1) / (M::BATCH_BLOCK / 32));
-    const int chunks = (int)std::max<int64_t>(1, std::min<int64_t>(max_chunks, waves * slots / n_points));
-    // scratch from the stream-ordered pool: [consts | ok | partials | bad | ticket]
-    const size_t b_consts = sizeof(typename M::Consts) * n_points, b_ok = sizeof(int) * n_points;
-    const size_t b_part = sizeof(double) * n_points * M::NACC * chunks, b_bad = sizeof(unsigned) * n_points * chunks;
-    const size_t b_ticket = sizeof(unsigned) * n_points;
+    const int64_t chunks64 = std::max<int64_t>(1, std::min<int64_t>(max_chunks, waves * slots / n_points));
+    if (n_points * chunks64 > (int64_t)0x7fffffff)
+        return mf_fail(ctx, MF_ERR_ARG, "mf_nll_grad_points: n_points x event chunks exceeds the grid limit; split the call");
+    const int chunks = (int)chunks64;
+    // device scratch [consts | ok | partials | bad | ticket], laid out for the largest (points, chunks) seen so far
     auto up = [](size_t x) { return (x + 255) / 256 * 256; };
-    char* blk = nullptr;
-    MF_CUDA(ctx, dev_alloc(ctx, &blk, up(b_consts) + up(b_ok) + up(b_part) + up(b_bad) + up(b_ticket)));
+    if (n_points > m->p_points || chunks > m->p_chunks || !m->p_blk) {
+        const int64_t P = std::max<int64_t>(n_points, m->p_points);
+        const int C = std::max(chunks, m->p_chunks);
+        const size_t bytes = up(sizeof(FourDConsts) * P) + up(sizeof(int) * P) + up(sizeof(double) * P * MF_MAX_NACC * C) +
+                             up(sizeof(unsigned) * P * C) + up(sizeof(unsigned) * P);
+        dev_free(ctx, m->p_blk);  // stream-ordered: after the launches that still use it
+        m->p_blk = nullptr;
+        MF_CUDA(ctx, dev_alloc(ctx, &m->p_blk, bytes));
+        m->p_bytes = bytes;
+        m->p_points = P;
+        m->p_chunks = C;
+        // ok flags non-zero (every point is validated on the host), tickets zero (the kernel leaves them at zero)
+        MF_CUDA(ctx, cudaMemsetAsync(m->p_blk + up(sizeof(FourDConsts) * P), 0xFF, up(sizeof(int) * P), ctx->stream));
+        MF_CUDA(ctx, cudaMemsetAsync(m->p_blk + bytes - up(sizeof(unsigned) * P), 0, up(sizeof(unsigned) * P), ctx->stream));
+    }
+    const int64_t P = m->p_points;
+    const int C = m->p_chunks;
     BatchArgs<M> a;
     for (int i = 0; i < M::NCOL; ++i) a.col[i] = m->col[i];
     a.toy_stride = 0;
@@ -583,19 +630,23 @@ static mf_status launch_points(mf_model* m, int64_t n_points, const double* lamb
     a.mb = m->mb;
     a.sum_m = m->d_sum_m;
     a.lam = nullptr;
-    a.consts = reinterpret_cast<typename M::Consts*>(blk);
-    a.consts_ok = reinterpret_cast<int*>(blk + up(b_consts));
-    a.partials = reinterpret_cast<double*>(blk + up(b_consts) + up(b_ok));
-    a.bad_partials = reinterpret_cast<unsigned*>(blk + up(b_consts) + up(b_ok) + up(b_part));
-    a.ticket = reinterpret_cast<unsigned*>(blk + up(b_consts) + up(b_ok) + up(b_part) + up(b_bad));
+    a.lam_external = 0;
+    char* q = m->p_blk;
+    a.consts = reinterpret_cast<Consts*>(q);
+    q += up(sizeof(FourDConsts) * P);
+    a.consts_ok = reinterpret_cast<int*>(q);
+    q += up(sizeof(int) * P);
+    a.partials = reinterpret_cast<double*>(q);
+    q += up(sizeof(double) * P * MF_MAX_NACC * C);
+    a.bad_partials = reinterpret_cast<unsigned*>(q);
+    q += up(sizeof(unsigned) * P * C);
+    a.ticket = reinterpret_cast<unsigned*>(q);
     a.ids = nullptr;
     a.out = out_dev;
-    cudaError_t e = cudaMemcpyAsync(a.consts, hc.data(), b_consts, cudaMemcpyHostToDevice, ctx->stream);  // pageable: staged before return
-    if (e == cudaSuccess) e = cudaMemsetAsync(a.consts_ok, 0xFF, b_ok, ctx->stream);                    // non-zero = ok
-    if (e == cudaSuccess) e = cudaMemsetAsync(a.ticket, 0, b_ticket, ctx->stream);
-    if (e == cudaSuccess) e = launch_pdl(nll_grad_batch_kernel<M>, (int)(n_points * chunks), ctx->stream, a, M::BATCH_BLOCK);
-    dev_free(ctx, blk);
-    MF_CUDA(ctx, e);
+    MF_CUDA(ctx, cudaMemcpyAsync(a.consts, hc, b_consts, cudaMemcpyHostToDevice, ctx->stream));  // pinned: asynchronous
+    MF_CUDA(ctx, cudaEventRecord(ctx->pts_copied[stage], ctx->stream));
+    take_fresh(m);  // the copy above precedes the launch: the kernel cannot start before the S1 kernels have completed
+    MF_CUDA(ctx, launch_pdl(nll_grad_batch_kernel<M>, (int)(n_points * chunks), ctx->stream, a, M::BATCH_BLOCK));
     ++ctx->launches;
     return MF_OK;
 }
@@ -619,6 +670,50 @@ extern "C" mf_status mf_nll_grad_points(mf_model* m, int64_t n_points, const dou
     case MF_ANGULAR_KSTMUMU: return launch_points<AngularModel>(m, n_points, lambdas, out_dev);
     default: return launch_points<FourDModel>(m, n_points, lambdas, out_dev);
     }
+}
+
+// The same sweep with HOST results: one call evaluates n_points parameter points and returns when the values are on the
+// host (BASELINE.json configs[1] as a user of the library sees it).
+extern "C" mf_status mf_nll_grad_sweep(mf_model* m, int64_t n_points, const double* lambdas, double* nll, double* grad,
+                                       int64_t* n_bad)
+{
+    if (!m || !lambdas || !nll || n_points < 0) return mf_fail(m ? m->ctx : nullptr, MF_ERR_ARG, "mf_nll_grad_sweep: bad argument");
+    if (n_points == 0) return MF_OK;
+    mf_ctx* ctx = m->ctx;
+    const int K = m->K, row = K + 2;
+    if (m->p_sweep_rows < n_points) {
+        dev_free(ctx, m->d_sweep);
+        m->d_sweep = nullptr;
+        m->p_sweep_rows = 0;
+        MF_CUDA(ctx, dev_alloc(ctx, &m->d_sweep, sizeof(double) * n_points * row));
+        m->p_sweep_rows = n_points;
+    }
+    const mf_status st = mf_nll_grad_points(m, n_points, lambdas, m->d_sweep);
+    if (st != MF_OK) return st;
+    // results through the context's pinned staging block (grow-only), then scattered to the caller's arrays
+    const size_t bytes = sizeof(double) * n_points * row;
+    if (ctx->h_stage_bytes < bytes) {
+        if (ctx->h_stage) {
+            cudaStreamSynchronize(ctx->stream);
+            cudaFreeHost(ctx->h_stage);
+            ctx->h_stage = nullptr;
+            ctx->h_stage_bytes = 0;
+        }
+        MF_CUDA(ctx, cudaHostAlloc(reinterpret_cast<void**>(&ctx->h_stage), bytes, cudaHostAllocDefault));
+        ctx->h_stage_bytes = bytes;
+    }
+    double* h = reinterpret_cast<double*>(ctx->h_stage);
+    MF_CUDA(ctx, cudaMemcpyAsync(h, m->d_sweep, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    MF_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    int64_t bad_points = 0;
+    for (int64_t p = 0; p < n_points; ++p) {
+        const double* o = h + p * row;
+        nll[p] = o[0];
+        if (grad) std::memcpy(grad + p * K, o + 1, sizeof(double) * K);
+        if (o[K + 1] != 0.0) ++bad_points;
+    }
+    if (n_bad) *n_bad = bad_points;
+    return MF_OK;
 }
 
 // One synchronous evaluation: value, gradient and (hess != NULL, mass model) the K x K Hessian.
@@ -690,6 +785,7 @@ static mf_status launch_batch(mf_model* m, int n_active, const double* lam_dev =
     a.mb = m->mb;
     a.sum_m = m->d_sum_m;
     a.lam = lam_dev ? lam_dev : m->d_lam;
+    a.lam_external = lam_dev ? 1 : 0;
     a.consts = static_cast<typename M::Consts*>(m->d_consts);
     a.consts_ok = m->d_consts_ok;
     a.ids = (n_active == m->n_toys) ? nullptr : m->d_ids;
@@ -699,7 +795,7 @@ static mf_status launch_batch(mf_model* m, int n_active, const double* lam_dev =
     a.out = out_dev ? out_dev : m->d_bout;
     // both kernels are launched programmatically: the constants kernel of evaluation i+1 starts (and computes) while the
     // batched kernel of evaluation i drains, and waits for it to complete only before overwriting the constants
-    MF_CUDA(ctx, launch_pdl_v(batch_consts_kernel<M>, (n_active + 127) / 128, 128, ctx->stream, a, n_active));
+    MF_CUDA(ctx, launch_pdl_v(batch_consts_kernel<M>, (n_active + 127) / 128, 128, 0, ctx->stream, !take_fresh(m), a, n_active));
     MF_CUDA(ctx, launch_pdl(nll_grad_batch_kernel<M>, n_active * m->chunks, ctx->stream, a, M::BATCH_BLOCK));
     ctx->launches += 2;
     return MF_OK;

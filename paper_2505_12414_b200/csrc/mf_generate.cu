@@ -3,7 +3,7 @@
 //
 // Counter-based instead of the paper's jump-seeded Xoshiro streams: event i of toy t draws from Philox4x32-10 with
 // key = seed0 + t and counter = (i, draw), so any thread can generate any event and the result does not depend on the
-// launch geometry.  Recipe (restated independently in oracle/gen.py, which is test infrastructure):
+// launch geometry.  Recipe:
 //   draw 0 -> (uA, uB); signal if uA < f, else background m = lo + log1p(uB expm1(tau w)) / tau  (lo + uB w at tau == 0);
 //   signal: draws 1, 2, ... -> Box-Muller z = sqrt(-2 ln u1) cos(2 pi u2), m = mu + sigma z, first m inside [lo, hi]
 //   (after 64 rejected draws the last one is clamped).  u = ((w_hi 2^32 + w_lo) >> 11 + 1/2) 2^-53.
@@ -146,7 +146,12 @@ __device__ __forceinline__ double legendre2(double x, double c1, double c2)
     return 0.5 * (1.0 + c1 * x + c2 * 0.5 * (3.0 * x * x - 1.0));
 }
 
-// data: [4][n_toys][n_pad] (m, cos theta_l, cos theta_K, phi); recipe: see oracle/gen.py gen_4d_event / the header
+// data: [4][n_toys][n_pad] (m, cos theta_l, cos theta_K, phi).  Draw layout of one event (two uniforms per draw):
+//   draw 0 -> (uA, uB): signal if uA < f; background mass from uB by the inverse CDF (as generate_mass_kernel);
+//   signal:     draws 1..64 Box-Muller mass candidates (first inside the range); draws 100 + 2k -> (cos theta_l, cos theta_K)
+//               and 101 + 2k -> (phi, accept) of angular proposal k, accepted when accept * pmax < P(Omega);
+//   background: draw 1 -> (phi, unused); draws 100 + 2k -> (cos theta_l, cos theta_K) and 101 + 2k -> (accept, unused) of
+//               Legendre proposal k, accepted when accept * bound < l(cos theta_l) l(cos theta_K).
 __global__ void __launch_bounds__(256) generate_4d_kernel(double* __restrict__ data, int64_t n_toys, int64_t n, int64_t n_pad,
                                                           unsigned long long seed0, const __grid_constant__ FourDGenArgs g)
 {

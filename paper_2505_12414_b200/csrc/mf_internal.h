@@ -21,6 +21,13 @@ struct mf_ctx {
     // pinned staging of the batched (synchronous) calls, shared by all models of the context, grow-only
     char* h_stage = nullptr;
     size_t h_stage_bytes = 0;
+    // pinned staging of the parameter-only constants of mf_nll_grad_points: a ring of blocks, each guarded by an event
+    // recorded after its host-to-device copy, so that successive calls never wait for one another's copies
+    static constexpr int kPointStages = 4;
+    char* h_pts[kPointStages] = {};
+    size_t h_pts_bytes[kPointStages] = {};
+    cudaEvent_t pts_copied[kPointStages] = {};
+    unsigned pts_seq = 0;
 };
 
 constexpr int MF_HOST_SLOT_DOUBLES = 64;  // widest output row (angular Hessian: 45 + n_bad) and the done word
@@ -46,6 +53,7 @@ struct mf_dataset {
 };
 
 constexpr int MF_MAX_COLS = 12;
+constexpr int MF_MAX_NACC = 17;  // accumulators of the widest value+gradient model (points-mode scratch layout)
 
 struct mf_model {
     mf_ctx* ctx = nullptr;
@@ -56,7 +64,6 @@ struct mf_model {
     mf_devbuf* raw = nullptr;         // shared with the dataset
     double* cache = nullptr;          // [9][n_toys][n_pad] angular basis columns (S1), or NULL
     double* d_sum_m = nullptr;        // device [n_toys]: event-only constants sum_i m_i (S1), NULL without a mass dimension
-    double h_sum_m = 0.0;             // its value for toy 0 (single-dataset evaluation)
     const double* col[MF_MAX_COLS] = {};  // column base pointers, stride between toys = n_pad
     // single-dataset evaluation
     int grid = 1;                     // CTAs of the fused kernel
@@ -65,6 +72,7 @@ struct mf_model {
     unsigned* ticket = nullptr;       // device, kRing (single) + n_toys (batch)
     unsigned long long* gen = nullptr;  // device [kRing]: evaluations completed per scratch slot
     unsigned long long seq = 0;       // evaluations enqueued so far (evaluation e uses slot e % kRing)
+    bool fresh = true;                // no kernel of this model launched yet: its first launch is made in plain stream order
     double* h_out = nullptr;          // pinned + mapped host slot: the output row, the 64-bit done word at MF_HOST_DONE_INDEX
     double* d_out_mapped = nullptr;   // device alias of h_out
     // batched evaluation
@@ -80,6 +88,13 @@ struct mf_model {
     int* h_ids = nullptr;             //   [n_toys][K], [n_toys], [n_toys][widest output row]
     double* h_bout = nullptr;
     int bout_row = 0;                 // widest output row + n_bad (doubles)
+    // many-points evaluation (mf_nll_grad_points / mf_nll_grad_sweep): grow-only scratch, reused by every call
+    char* p_blk = nullptr;            // device [consts | ok | partials | bad | ticket]
+    size_t p_bytes = 0;
+    int64_t p_points = 0;             // points and chunks the block was laid out for (tickets are zero between calls)
+    int p_chunks = 0;
+    double* d_sweep = nullptr;        // device [p_sweep_rows][K+2] results of mf_nll_grad_sweep
+    int64_t p_sweep_rows = 0;
 };
 
 // Sets ctx->err and returns st (mf_api.cu).

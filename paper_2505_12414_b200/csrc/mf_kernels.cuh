@@ -37,7 +37,7 @@ struct EvalArgs {
     int64_t n;                   // valid events
     int64_t n_items;             // n_pad / 64
     typename M::Consts c;        // parameter-only constants (S2), computed on the host
-    double sum_m;                // event-only constant sum_i m_i (0 for models without a mass dimension)
+    const double* sum_m;         // device: event-only constant sum_i m_i (S1), or NULL for models without a mass dimension
     // scratch slot of this evaluation (ring of kRing slots, so that successive evaluations do not
     // serialise on one scratch area; see "pipelining" below)
     double* partials;            // [NACC][gridDim.x]
@@ -61,6 +61,8 @@ struct BatchArgs {
     double ma, mb;               // mass range for the constants prologue
     const double* sum_m;         // [n_toys] event-only constants sum_i m_i per toy, or NULL
     const double* lam;           // [n_active][K]
+    int lam_external;            // 1: lam was written by the caller's own work on the stream (mf_nll_grad_batch_async), so it
+                                 // may only be read after griddepcontrol.wait; 0: written by a stream-ordered copy of ours
     typename M::Consts* consts;  // [n_active] parameter-only constants (S2), written by batch_consts_kernel
     int* consts_ok;              // [n_active] 0 = lambda outside the parameter domain
     const int* ids;              // [n_active] toy index of each active slot; NULL = identity (all toys active)
@@ -416,8 +418,8 @@ __device__ __forceinline__ void reduce_and_finish(const EvalArgs<M>& a, double* 
     if (threadIdx.x == 0) s_last = (ticket_take(a.ticket) == gridDim.x - 1);
     __syncthreads();
     if (s_last) {
-        final_combine<M>(a.partials, G, (int)G, a.bad_partials, a.c, (double)a.n, a.sum_m, s_sum, a.out, a.done_flag,
-                         a.done_value);
+        final_combine<M>(a.partials, G, (int)G, a.bad_partials, a.c, (double)a.n, a.sum_m ? __ldg(a.sum_m) : 0.0, s_sum, a.out,
+                         a.done_flag, a.done_value);
         if (threadIdx.x == 0) {  // every partial has been read: final_combine synchronises the CTA before its thread 0 returns
             *a.ticket = 0u;
             gen_store(a.gen, a.need + 1);  // releases the slot (and the ticket reset) to evaluation e + kRing
@@ -536,6 +538,10 @@ __global__ void __launch_bounds__(128) batch_consts_kernel(const __grid_constant
     const int slot = blockIdx.x * blockDim.x + threadIdx.x;
     if (slot >= n_active) return;
     typename M::Consts c;
+    // lambda written by the caller's preceding work on the stream is complete and visible only after the wait (a
+    // programmatic launch may start this kernel before its predecessor has flushed); our own stream-ordered copy is
+    // complete before this kernel can start, and the constants are then derived while the previous evaluation drains
+    if (a.lam_external) pdl_wait();
     const int ok = make_consts<M>(a.lam + (int64_t)slot * M::K, a.ma, a.mb, c) ? 1 : 0;
     pdl_wait();
     a.consts[slot] = c;
@@ -561,7 +567,9 @@ __global__ void __launch_bounds__(M::BATCH_BLOCK, M::BATCH_RESIDENT_CTAS)
 
     pdl_launch_dependents();
     const int slot = blockIdx.x / a.chunks, chunk = blockIdx.x % a.chunks;
-    const int64_t toy = a.shared_data ? 0 : a.ids ? a.ids[slot] : slot;  // ids == NULL: every toy is active
+    // ids == NULL: every toy is active.  ids is only ever the library's own array, filled by a stream-ordered copy that is
+    // complete before the constants kernel (this kernel's predecessor) can start, so it may be read ahead of the wait.
+    const int64_t toy = a.shared_data ? 0 : a.ids ? a.ids[slot] : slot;
     if (a.chunks == 1 && !a.shared_data) {
         // this CTA streams its toy's columns once from HBM: ask for them now (L2 prefetch, 128-byte lines), so
         // that they arrive while the constants are fetched and the first loads of the event loop hit L2

@@ -1,13 +1,16 @@
-// mf_probe.cu — the two roofline denominators that MEASURED_PEAKS.json does not hold
-// (SURVEY.md §7 step 0): the fp64-pipe issue rate (register-only DFMA chains) and the read
-// bandwidth of a working set that is re-read in a loop (L2-resident when it fits the 126 MB
-// L2, HBM otherwise).  Measurement helpers only; nothing on the hot path calls them.
+// mf_probe.cu — measurement and test probes, built into their OWN library (lib/libmorefit_b200_probe.so, declared in
+// mf_probe.h); they are not part of the product library nor of its public header.
+//   * the two roofline denominators that MEASURED_PEAKS.json does not hold: the fp64-pipe issue
+//     rate (register-only DFMA chains) and the read bandwidth of a working set that is re-read in a loop (L2-resident
+//     when it fits the 126 MB L2, HBM otherwise) — used by bench.py;
+//   * element-wise evaluation of the kernels' own device math (mf_math.cuh) — used by the accuracy tests.
+// Every entry takes the CUDA device and stream directly and returns 0 or the cudaError_t that stopped it.
 #include <cuda_runtime.h>
 
-#include <string>
+#include <cstdint>
 
-#include "mf_internal.h"
 #include "mf_math.cuh"
+#include "mf_probe.h"
 
 namespace {
 
@@ -57,17 +60,33 @@ __global__ void __launch_bounds__(256) math_kernel(int op, int64_t n, const doub
 
 }  // namespace
 
-#define MF_CUDA(ctx, call)                                                                        \
-    do {                                                                                          \
-        cudaError_t e__ = (call);                                                                 \
-        if (e__ != cudaSuccess)                                                                   \
-            return mf_fail(ctx, MF_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e__)); \
+#define MF_CUDA(ctx, call)                  \
+    do {                                    \
+        cudaError_t e__ = (call);           \
+        if (e__ != cudaSuccess) return (int)e__; \
     } while (0)
 
-extern "C" mf_status mf_probe_fp64_rate(mf_ctx* ctx, double* dfma_per_second)
+struct ProbeCtx {
+    int device;
+    cudaStream_t stream;
+    int sm_count;
+};
+
+static int probe_ctx(int device, void* stream, ProbeCtx* c)
 {
-    if (!ctx || !dfma_per_second) return mf_fail(ctx, MF_ERR_ARG, "mf_probe_fp64_rate: NULL argument");
-    MF_CUDA(ctx, cudaSetDevice(ctx->device));
+    c->device = device;
+    c->stream = static_cast<cudaStream_t>(stream);
+    c->sm_count = 0;
+    MF_CUDA(c, cudaSetDevice(device));
+    MF_CUDA(c, cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device));
+    return 0;
+}
+
+extern "C" int mfp_fp64_rate(int device, void* stream, double* dfma_per_second)
+{
+    if (!dfma_per_second) return (int)cudaErrorInvalidValue;
+    ProbeCtx pc, *ctx = &pc;
+    if (const int e = probe_ctx(device, stream, ctx)) return e;
     double* d_out = nullptr;
     MF_CUDA(ctx, cudaMalloc(&d_out, sizeof(double)));
     cudaEvent_t e0, e1;
@@ -78,7 +97,6 @@ extern "C" mf_status mf_probe_fp64_rate(mf_ctx* ctx, double* dfma_per_second)
     for (int rep = 0; rep < 6; ++rep) {
         MF_CUDA(ctx, cudaEventRecord(e0, ctx->stream));
         dfma_chain_kernel<<<grid, 256, 0, ctx->stream>>>(d_out, iters, 0.999999, 1e-9);
-        ++ctx->launches;
         MF_CUDA(ctx, cudaEventRecord(e1, ctx->stream));
         MF_CUDA(ctx, cudaEventSynchronize(e1));
         float ms = 0;
@@ -90,14 +108,14 @@ extern "C" mf_status mf_probe_fp64_rate(mf_ctx* ctx, double* dfma_per_second)
     cudaEventDestroy(e1);
     cudaFree(d_out);
     *dfma_per_second = best;
-    return MF_OK;
+    return 0;
 }
 
-extern "C" mf_status mf_probe_read_bandwidth(mf_ctx* ctx, size_t bytes, int repeats, double* bytes_per_second)
+extern "C" int mfp_read_bandwidth(int device, void* stream, size_t bytes, int repeats, double* bytes_per_second)
 {
-    if (!ctx || !bytes_per_second || bytes < 4096 || repeats < 1)
-        return mf_fail(ctx, MF_ERR_ARG, "mf_probe_read_bandwidth: bad argument");
-    MF_CUDA(ctx, cudaSetDevice(ctx->device));
+    if (!bytes_per_second || bytes < 4096 || repeats < 1) return (int)cudaErrorInvalidValue;
+    ProbeCtx pc, *ctx = &pc;
+    if (const int e = probe_ctx(device, stream, ctx)) return e;
     const size_t n_vec = bytes / sizeof(double2);
     double2* buf = nullptr;
     double* d_out = nullptr;
@@ -112,7 +130,6 @@ extern "C" mf_status mf_probe_read_bandwidth(mf_ctx* ctx, size_t bytes, int repe
     for (int rep = 0; rep < 4; ++rep) {
         MF_CUDA(ctx, cudaEventRecord(e0, ctx->stream));
         read_kernel<<<grid, 256, 0, ctx->stream>>>(buf, n_vec, repeats, d_out);
-        ++ctx->launches;
         MF_CUDA(ctx, cudaEventRecord(e1, ctx->stream));
         MF_CUDA(ctx, cudaEventSynchronize(e1));
         float ms = 0;
@@ -125,23 +142,23 @@ extern "C" mf_status mf_probe_read_bandwidth(mf_ctx* ctx, size_t bytes, int repe
     cudaFree(buf);
     cudaFree(d_out);
     *bytes_per_second = best;
-    return MF_OK;
+    return 0;
 }
 
-extern "C" mf_status mf_probe_math(mf_ctx* ctx, int op, int64_t n, const double* x_host, double* y_host)
+extern "C" int mfp_math(int device, void* stream, int op, int64_t n, const double* x_host, double* y_host)
 {
-    if (!ctx || !x_host || !y_host || n < 1 || op < 0 || op > 3) return mf_fail(ctx, MF_ERR_ARG, "mf_probe_math: bad argument");
-    MF_CUDA(ctx, cudaSetDevice(ctx->device));
+    if (!x_host || !y_host || n < 1 || op < 0 || op > 3) return (int)cudaErrorInvalidValue;
+    ProbeCtx pc, *ctx = &pc;
+    if (const int e = probe_ctx(device, stream, ctx)) return e;
     double *dx = nullptr, *dy = nullptr;
     MF_CUDA(ctx, cudaMalloc(&dx, sizeof(double) * n));
     MF_CUDA(ctx, cudaMalloc(&dy, sizeof(double) * n));
     MF_CUDA(ctx, cudaMemcpyAsync(dx, x_host, sizeof(double) * n, cudaMemcpyHostToDevice, ctx->stream));
     math_kernel<<<(int)((n + 255) / 256 > 1184 ? 1184 : (n + 255) / 256), 256, 0, ctx->stream>>>(op, n, dx, dy);
-    ++ctx->launches;
     MF_CUDA(ctx, cudaGetLastError());
     MF_CUDA(ctx, cudaMemcpyAsync(y_host, dy, sizeof(double) * n, cudaMemcpyDeviceToHost, ctx->stream));
     MF_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     cudaFree(dx);
     cudaFree(dy);
-    return MF_OK;
+    return 0;
 }

@@ -11,8 +11,8 @@ likelihood are independent, and so are pseudo-experiments):
   that all ranks hold bit-identical results and the result does not depend on the collective's
   reduction tree (an all-reduce's order may).  K+1 <= 17 doubles: latency bound on any fabric.
 
-Nothing here computes likelihoods; it is plumbing over ``torch.distributed`` (gloo on CPU in the tests,
-nccl on GPUs).
+Nothing here computes anything: it is plumbing over ``torch.distributed`` (gloo on CPU in the tests, nccl on
+GPUs); the rank-ordered compensated sum itself is the library's ``mf_combine_partials`` (host C).
 """
 from __future__ import annotations
 
@@ -42,27 +42,11 @@ def shard_events(n_events: int, rank: int, world: int) -> tuple[int, int]:
     return first, last - first
 
 
-def _two_sum(a: np.ndarray, b: np.ndarray):
-    s = a + b
-    bb = s - a
-    return s, (a - (s - bb)) + (b - bb)
-
-
 def ordered_sum(rows: np.ndarray) -> np.ndarray:
-    """Compensated sum of rows[0], rows[1], ... in that order (fp64 two-sum; any +inf / NaN propagates)."""
+    """Compensated sum of rows[0], rows[1], ... in that order: the library's mf_combine_partials (host C)."""
+    from . import combine_partials as _c
     rows = np.asarray(rows, dtype=np.float64)
-    s = np.zeros(rows.shape[1:], dtype=np.float64)
-    c = np.zeros_like(s)
-    for r in rows:
-        with np.errstate(invalid="ignore"):
-            s, e = _two_sum(s, r)
-            c = c + e
-    out = s + c
-    bad = ~np.isfinite(rows).all(axis=0)
-    if np.any(bad):
-        plain = rows.sum(axis=0)
-        out = np.where(bad, plain, out)
-    return out
+    return _c(rows.reshape(rows.shape[0], -1)).reshape(rows.shape[1:])
 
 
 def combine_partials(local: np.ndarray, group=None) -> np.ndarray:

@@ -51,7 +51,7 @@ def test_c1_points_mode_full_size(mf, ctx):
     torch.cuda.synchronize()
     res = out.cpu().numpy()
     assert np.all(np.isfinite(res)) and np.all(res[:, 5] == 0)
-    for p in (0, 137, 499, 500, 999):      # sampled outputs, both calls, first and last slots
+    for p in range(1000):                  # every output of both calls (the oracle needs ~12 s for the 1e9 event evaluations)
         o_nll, o_g, _ = oracle.nll_grad(oracle.MASS, m, pts[p], dg.MASS_LO, dg.MASS_HI, nthreads=oracle.max_threads())
         check(res[p, 0], res[p, 1:5], o_nll, o_g, f"C1 point {p}")
     # properties that hold for every point: the lone-call kernel agrees with the points-mode kernel
@@ -86,12 +86,36 @@ def test_c2_full_size(mf, ctx):
         check(nll, g, o_nll, o_g, "C2")
 
 
+def _check_full_size_fit(r, o_nll, o_g, truth, what):
+    """The fitted point satisfies the ORACLE's stationarity condition: a Newton step from it, taken with the oracle's
+    gradient and the fit's covariance, is below 1e-6 sigma in every parameter (north_star's fit tolerance)."""
+    assert r.converged, what
+    assert abs(r.nll - o_nll) <= NLL_RTOL * abs(o_nll), what
+    step = r.cov @ o_g
+    assert np.max(np.abs(step) / r.sigma) < 1e-6, (what, step, r.sigma)
+    pull = (r.lam - np.array(truth)) / r.sigma
+    assert np.all(np.abs(pull) < 5), (what, pull)
+
+
+def test_c2_full_fit(mf, ctx):
+    """C2's full fit (N = 1e6, all 8 coefficients free, from the truth) checked at full size like C1's."""
+    ev = dg.gen_angular(1_000_000, seed=2)
+    model = ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ctx.dataset_upload(ev))
+    r = model.fit(dg.ANG_TRUTH)
+    o_nll, o_g, _ = oracle.nll_grad(oracle.ANGULAR, ev, r.lam, nthreads=oracle.max_threads())
+    _check_full_size_fit(r, o_nll, o_g, dg.ANG_TRUTH, "C2 fit")
+
+
 def test_c3_full_size(mf, ctx):
     ev = dg.gen_4d(2_000_000, seed=3)
     model = ctx.model_create(mf.MF_MASS_X_ANGULAR, ctx.dataset_upload(ev, dg.MASS_LO, dg.MASS_HI))
     nll, g = model.nll_grad(dg.FOURD_TRUTH)
     o_nll, o_g, _ = oracle.nll_grad(oracle.FOURD, ev, dg.FOURD_TRUTH, dg.MASS_LO, dg.MASS_HI, nthreads=oracle.max_threads())
     check(nll, g, o_nll, o_g, "C3")
+    # C3's full fit (16 free parameters, from the truth) at full size
+    r = model.fit(dg.FOURD_TRUTH)
+    o_nll, o_g, _ = oracle.nll_grad(oracle.FOURD, ev, r.lam, dg.MASS_LO, dg.MASS_HI, nthreads=oracle.max_threads())
+    _check_full_size_fit(r, o_nll, o_g, dg.FOURD_TRUTH, "C3 fit")
 
 
 def test_c4_full_size(mf, ctx):
@@ -103,7 +127,7 @@ def test_c4_full_size(mf, ctx):
     lams = dg.gen_lambda_points(T, 4242, dg.MASS_TRUTH, 3 * dg.mass_sigma_stat(n))
     nll, g = model.nll_grad_batch(lams)
     assert np.all(np.isfinite(nll)) and np.all(np.isfinite(g))
-    for t in (0, 1, 777, 2048, 4095):
+    for t in range(T):                     # every toy (4.1e7 oracle event evaluations, a few seconds)
         o_nll, o_g, _ = oracle.nll_grad(oracle.MASS, toys[t], lams[t], dg.MASS_LO, dg.MASS_HI)
         check(nll[t], g[t], o_nll, o_g, f"C4 toy {t}")
     # a 1-toy model of the same events gives the same numbers (same kernel arithmetic, different tiling)

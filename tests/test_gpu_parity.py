@@ -271,24 +271,25 @@ def _ulp_err(y, ref):
 
 def test_device_math_accuracy(mf, ctx):
     """The kernels' own exp / log / reciprocal (mf_math.cuh) against numpy's libm: a few ulp at most."""
+    from paper_2505_12414_b200 import probe
     rng = np.random.default_rng(0)
     x = np.concatenate([rng.uniform(-707.9, 700.0, 200_000), rng.uniform(-5, 5, 200_000), [0.0, -0.0, 1e-300, -1e-300]])
-    y = ctx.probe_math("exp", x)
+    y = probe.math("exp", x)
     assert np.max(_ulp_err(y, np.exp(x))) <= 2.0
-    assert np.all(ctx.probe_math("exp", np.array([-708.0, -750.0, -1e4, -1e300])) == 0.0)
-    y32 = ctx.probe_math("exp32", x)   # the table-by-shuffle variant used inside the event loops
+    assert np.all(probe.math("exp", np.array([-708.0, -750.0, -1e4, -1e300])) == 0.0)
+    y32 = probe.math("exp32", x)   # the table-by-shuffle variant used inside the event loops
     assert np.max(_ulp_err(y32, np.exp(x))) <= 2.0
-    tiny = ctx.probe_math("exp32", np.array([-709.5, -750.0, -1e4, -9e11]))   # clamped, not flushed: callers treat < 2^-1000 as 0
+    tiny = probe.math("exp32", np.array([-709.5, -750.0, -1e4, -9e11]))   # clamped, not flushed: callers treat < 2^-1000 as 0
     assert np.all((tiny >= 2.0 ** -1022) & (tiny <= 2.0 ** -1021))
-    assert ctx.probe_math("exp32", np.array([0.0]))[0] == 1.0
+    assert probe.math("exp32", np.array([0.0]))[0] == 1.0
     v = np.concatenate([np.exp(rng.uniform(-700, 700, 200_000)), rng.uniform(0.5, 2.0, 200_000),
                         1.0 + rng.uniform(-1e-3, 1e-3, 100_000), [1.0, 2.0, 0.5, 2.2250738585072014e-308]])
-    lg = ctx.probe_math("log", v)
+    lg = probe.math("log", v)
     ref = np.log(v)
     # absolute error matters for sums of ln P: <= 2 ulp of max(|ln v|, ~0.35) (log is exact at 1)
     assert np.max(np.abs(lg - ref) / np.spacing(np.maximum(np.abs(ref), 0.35))) <= 2.0
-    assert ctx.probe_math("log", np.array([1.0]))[0] == 0.0
-    r = ctx.probe_math("rcp", v)
+    assert probe.math("log", np.array([1.0]))[0] == 0.0
+    r = probe.math("rcp", v)
     assert np.max(_ulp_err(r, 1.0 / v)) <= 2.0
 
 

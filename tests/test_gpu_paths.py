@@ -1,0 +1,281 @@
+"""GPU parity for every code path that is not the default single-evaluation one: many-point launches of the angular and
+4D models, batched toys of the 4D model, the register-buffer 4D kernel (n < 1024), the host-result sweep, the
+MF_NO_TMA / MF_NO_PDL ablation paths (subprocess: the switches are read once per process) and the sharded evaluation of
+paper_2505_12414_b200.dist with the CUDA path supplying the shard sums.  Every comparison is against the oracle."""
+import os
+import subprocess
+import sys
+import textwrap
+
+import numpy as np
+import pytest
+
+import mf_datagen as dg
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+NLL_RTOL = 1e-11
+GRAD_TOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def mf():
+    import paper_2505_12414_b200 as mf
+    from paper_2505_12414_b200 import build
+    build.build()
+    return mf
+
+
+@pytest.fixture(scope="module")
+def ctx(mf):
+    c = mf.Context(0)
+    yield c
+    c.close()
+
+
+def check(nll, grad, o_nll, o_grad, what):
+    assert abs(nll - o_nll) <= NLL_RTOL * abs(o_nll), f"{what}: nll {nll!r} vs oracle {o_nll!r}"
+    err = np.abs(grad - o_grad)
+    tol = GRAD_TOL * (1.0 + np.abs(o_grad))
+    assert np.all(err <= tol), f"{what}: grad err {err} tol {tol}"
+
+
+def _ang_points(n_pts, seed):
+    rng = np.random.default_rng(seed)
+    pts = np.tile(np.array(dg.ANG_TRUTH), (n_pts, 1)) + rng.uniform(-0.03, 0.03, (n_pts, 8))
+    pts[0] = dg.ANG_TRUTH
+    return pts
+
+
+def _fourd_points(n_pts, seed):
+    rng = np.random.default_rng(seed)
+    pts = np.tile(np.array(dg.FOURD_TRUTH), (n_pts, 1))
+    scale = np.array([0.02, 0.002, 0.001, 0.2] + [0.03] * 8 + [0.05] * 4)
+    pts += rng.uniform(-1, 1, (n_pts, 16)) * scale
+    pts[0] = dg.FOURD_TRUTH
+    return pts
+
+
+@pytest.mark.parametrize("n,n_pts", [(20_011, 16), (150_000, 64)])
+def test_points_mode_angular_vs_oracle(mf, ctx, n, n_pts):
+    """launch_points<AngularModel>: every row of a >= 16-point call against the oracle."""
+    import torch
+    ev = dg.gen_angular(n, seed=21)
+    model = ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ctx.dataset_upload(ev))
+    pts = _ang_points(n_pts, 5)
+    out = torch.full((n_pts, 10), float("nan"), dtype=torch.float64, device="cuda")
+    model.nll_grad_points(pts, out.data_ptr())
+    torch.cuda.synchronize()
+    res = out.cpu().numpy()
+    assert np.all(res[:, 9] == 0)
+    for p in range(n_pts):
+        o_nll, o_g, _ = oracle.nll_grad(oracle.ANGULAR, ev, pts[p], nthreads=oracle.max_threads())
+        check(res[p, 0], res[p, 1:9], o_nll, o_g, f"angular points row {p}")
+
+
+@pytest.mark.parametrize("n,n_pts", [(30_001, 16), (100_000, 64)])
+def test_points_mode_fourd_vs_oracle(mf, ctx, n, n_pts):
+    """launch_points<FourDModel>: every row against the oracle."""
+    import torch
+    ev = dg.gen_4d(n, seed=23)
+    model = ctx.model_create(mf.MF_MASS_X_ANGULAR, ctx.dataset_upload(ev, dg.MASS_LO, dg.MASS_HI))
+    pts = _fourd_points(n_pts, 6)
+    out = torch.full((n_pts, 18), float("nan"), dtype=torch.float64, device="cuda")
+    model.nll_grad_points(pts, out.data_ptr())
+    torch.cuda.synchronize()
+    res = out.cpu().numpy()
+    assert np.all(res[:, 17] == 0)
+    for p in range(n_pts):
+        o_nll, o_g, _ = oracle.nll_grad(oracle.FOURD, ev, pts[p], dg.MASS_LO, dg.MASS_HI, nthreads=oracle.max_threads())
+        check(res[p, 0], res[p, 1:17], o_nll, o_g, f"4D points row {p}")
+
+
+@pytest.mark.parametrize("n", [3000, 40_001])
+def test_batch_fourd_vs_oracle(mf, ctx, n):
+    """launch_batch<FourDModel>: T toys of the 4D model at their own lambda_t (40,001 events: two CTAs per toy)."""
+    T = 5
+    ev = np.stack([dg.gen_4d(n, seed=60 + t) for t in range(T)], axis=1)  # [4][T][n]
+    model = ctx.model_create(mf.MF_MASS_X_ANGULAR, ctx.dataset_upload(ev, dg.MASS_LO, dg.MASS_HI, n_toys=T))
+    lams = _fourd_points(T, 9)
+    nll, g = model.nll_grad_batch(lams)
+    for t in range(T):
+        o_nll, o_g, _ = oracle.nll_grad(oracle.FOURD, ev[:, t, :], lams[t], dg.MASS_LO, dg.MASS_HI)
+        check(nll[t], g[t], o_nll, o_g, f"4D toy {t}")
+
+
+@pytest.mark.parametrize("n", [1, 37, 640, 1023])
+def test_small_fourd_register_kernel_vs_oracle(mf, ctx, n):
+    """n_pad < 1024: nll_grad_kernel<FourDModel> (register buffers) instead of the shared-memory-staged kernel."""
+    ev = dg.gen_4d(n, seed=70 + n)
+    model = ctx.model_create(mf.MF_MASS_X_ANGULAR, ctx.dataset_upload(ev, dg.MASS_LO, dg.MASS_HI))
+    for lam in _fourd_points(3, n):
+        nll, g = model.nll_grad(lam)
+        o_nll, o_g, _ = oracle.nll_grad(oracle.FOURD, ev, lam, dg.MASS_LO, dg.MASS_HI)
+        check(nll, g, o_nll, o_g, f"4D n={n}")
+
+
+@pytest.mark.parametrize("n", [37, 640])
+def test_small_angular_register_kernel_vs_oracle(mf, ctx, n):
+    ev = dg.gen_angular(n, seed=80 + n)
+    model = ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ctx.dataset_upload(ev))
+    for lam in _ang_points(3, n):
+        nll, g = model.nll_grad(lam)
+        o_nll, o_g, _ = oracle.nll_grad(oracle.ANGULAR, ev, lam)
+        check(nll, g, o_nll, o_g, f"angular n={n}")
+
+
+def test_sweep_host_results_vs_oracle(mf, ctx):
+    """mf_nll_grad_sweep: host lambda points in, host results out; both branches (< 16 and >= 16 points)."""
+    n = 50_003
+    m = dg.gen_mass(n, seed=9)
+    model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(m, dg.MASS_LO, dg.MASS_HI))
+    for n_pts in (5, 40):
+        pts = dg.gen_lambda_points(n_pts, 31, dg.MASS_TRUTH, 3 * dg.mass_sigma_stat(n))
+        nll, g, nbad = model.nll_grad_sweep(pts)
+        assert nbad == 0
+        for p in range(n_pts):
+            o_nll, o_g, _ = oracle.nll_grad(oracle.MASS, m, pts[p], dg.MASS_LO, dg.MASS_HI)
+            check(nll[p], g[p], o_nll, o_g, f"sweep {n_pts} row {p}")
+    # repeated calls reuse the model's scratch; a larger call grows it
+    pts = dg.gen_lambda_points(200, 32, dg.MASS_TRUTH, 3 * dg.mass_sigma_stat(n))
+    a = model.nll_grad_sweep(pts)
+    b = model.nll_grad_sweep(pts)
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+    o_nll, o_g, _ = oracle.nll_grad(oracle.MASS, m, pts[199], dg.MASS_LO, dg.MASS_HI)
+    check(a[0][199], a[1][199], o_nll, o_g, "sweep 200 row 199")
+    # a point with P <= 0 is counted, not an error
+    am = ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ctx.dataset_upload(dg.gen_angular(3000, seed=4)))
+    apts = np.tile(np.array(dg.ANG_TRUTH), (20, 1))
+    apts[7, 0] = 3.0
+    nll, g, nbad = am.nll_grad_sweep(apts)
+    assert nbad == 1 and nll[7] == np.inf and np.all(np.isnan(g[7])) and np.isfinite(nll[6])
+
+
+def test_first_evaluation_after_create_is_ordered(mf, ctx):
+    """mf_model_create no longer synchronises: the first launch on a fresh model must still see the S0/S1 kernels' output
+    (padding, basis columns, sum_i m_i).  Create-then-evaluate immediately, many times, for every entry point."""
+    import torch
+    ev = dg.gen_4d(200_003, seed=12)
+    o_nll, o_g, _ = oracle.nll_grad(oracle.FOURD, ev, dg.FOURD_TRUTH, dg.MASS_LO, dg.MASS_HI, nthreads=oracle.max_threads())
+    d_ev = [torch.from_numpy(np.ascontiguousarray(ev[j])).cuda() for j in range(4)]
+    pts = np.tile(np.array(dg.FOURD_TRUTH), (16, 1))
+    for rep in range(6):
+        ds = ctx.dataset_upload(d_ev, dg.MASS_LO, dg.MASS_HI)
+        model = ctx.model_create(mf.MF_MASS_X_ANGULAR, ds)
+        if rep % 2 == 0:
+            nll, g = model.nll_grad(dg.FOURD_TRUTH)
+            check(nll, g, o_nll, o_g, f"fresh model rep {rep}")
+        else:
+            nll, g, _ = model.nll_grad_sweep(pts)
+            check(nll[15], g[15], o_nll, o_g, f"fresh model sweep rep {rep}")
+        model.close()
+        ds.close()
+
+
+_ABLATION = textwrap.dedent("""
+    import numpy as np, sys
+    sys.path.insert(0, {root!r})
+    import mf_datagen as dg, oracle, paper_2505_12414_b200 as mf
+    import torch
+    ctx = mf.Context(0)
+    def check(nll, g, o):
+        assert abs(nll - o[0]) <= 1e-11 * abs(o[0]), (nll, o[0])
+        assert np.all(np.abs(g - o[1]) <= 1e-9 * (1 + np.abs(o[1]))), (g, o[1])
+    ev = dg.gen_angular(50_021, seed=2)
+    am = ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ctx.dataset_upload(ev))
+    for _ in range(3):
+        nll, g = am.nll_grad(dg.ANG_TRUTH)
+    check(nll, g, oracle.nll_grad(oracle.ANGULAR, ev, dg.ANG_TRUTH))
+    ev4 = dg.gen_4d(50_021, seed=3)
+    fm = ctx.model_create(mf.MF_MASS_X_ANGULAR, ctx.dataset_upload(ev4, dg.MASS_LO, dg.MASS_HI))
+    nll, g = fm.nll_grad(dg.FOURD_TRUTH)
+    check(nll, g, oracle.nll_grad(oracle.FOURD, ev4, dg.FOURD_TRUTH, dg.MASS_LO, dg.MASS_HI))
+    m = dg.gen_mass(100_003, seed=5)
+    mm = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(m, dg.MASS_LO, dg.MASS_HI))
+    pts = dg.gen_lambda_points(40, 77, dg.MASS_TRUTH, 3 * dg.mass_sigma_stat(100_003))
+    out = torch.zeros((40, 6), dtype=torch.float64, device="cuda")
+    for p in range(0, 40, 8):                       # pipelined single launches (< 16 points per call)
+        mm.nll_grad_points(pts[p:p + 8], out[p].data_ptr())
+    torch.cuda.synchronize()
+    r = out.cpu().numpy()
+    for p in (0, 13, 39):
+        check(r[p, 0], r[p, 1:5], oracle.nll_grad(oracle.MASS, m, pts[p], dg.MASS_LO, dg.MASS_HI))
+    nllb, gb, _ = mm.nll_grad_sweep(pts)            # one many-point launch
+    check(nllb[17], gb[17], oracle.nll_grad(oracle.MASS, m, pts[17], dg.MASS_LO, dg.MASS_HI))
+    toys = dg.gen_mass_toys(6, 3000, first_seed=9)
+    bm = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(toys, dg.MASS_LO, dg.MASS_HI, n_toys=6))
+    lam = np.tile(np.array(dg.MASS_TRUTH), (6, 1))
+    bn, bg = bm.nll_grad_batch(lam)
+    check(bn[5], bg[5], oracle.nll_grad(oracle.MASS, toys[5], lam[5], dg.MASS_LO, dg.MASS_HI))
+    r = mm.fit(dg.MASS_START)
+    assert r.converged
+    print("ablation ok")
+""")
+
+
+@pytest.mark.parametrize("switch", ["MF_NO_TMA", "MF_NO_PDL"])
+def test_ablation_switches_vs_oracle(mf, switch):
+    """The MF_NO_TMA=1 (register-buffer kernels for the angular / 4D models) and MF_NO_PDL=1 (plain stream order) paths
+    that DESIGN.md quotes numbers for, against the oracle."""
+    env = dict(os.environ)
+    env[switch] = "1"
+    p = subprocess.run([sys.executable, "-c", _ABLATION.format(root=ROOT)], env=env, capture_output=True, text=True, timeout=600)
+    assert p.returncode == 0 and "ablation ok" in p.stdout, p.stdout[-2000:] + p.stderr[-4000:]
+
+
+_DIST_WORKER = textwrap.dedent("""
+    import os, sys
+    import numpy as np
+    sys.path.insert(0, {root!r})
+    import torch.distributed as dist
+    import mf_datagen as dg, oracle
+    import paper_2505_12414_b200 as mf
+    from paper_2505_12414_b200 import dist as mfd
+    rank, world = int(sys.argv[1]), int(sys.argv[2])
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=sys.argv[3], RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    ctx = mf.Context(0)
+    # (a) one dataset, events sharded over the ranks: each rank's CUDA evaluation of its shard, rank-ordered combine
+    n = 100_037
+    ev = dg.gen_4d(n, seed=33)
+    first, count = mfd.shard_events(n, rank, world)
+    model = ctx.model_create(mf.MF_MASS_X_ANGULAR, ctx.dataset_upload(ev[:, first:first + count], dg.MASS_LO, dg.MASS_HI))
+    nll, g = model.nll_grad(dg.FOURD_TRUTH)
+    tot = mfd.combine_partials(np.concatenate([[nll], g]))
+    o_nll, o_g, _ = oracle.nll_grad(oracle.FOURD, ev, dg.FOURD_TRUTH, dg.MASS_LO, dg.MASS_HI)
+    assert abs(tot[0] - o_nll) <= 1e-11 * abs(o_nll), (tot[0], o_nll)
+    assert np.all(np.abs(tot[1:] - o_g) <= 1e-9 * (1 + np.abs(o_g)))
+    # (b) toys dealt to the ranks in contiguous blocks, per-toy rows gathered in toy order
+    T, ne = 11, 2000
+    toys = dg.gen_mass_toys(T, ne, first_seed=500)
+    t0, tc = mfd.shard_toys(T, rank, world)
+    bm = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(toys[t0:t0 + tc], dg.MASS_LO, dg.MASS_HI, n_toys=tc))
+    lam = np.tile(np.array(dg.MASS_TRUTH), (tc, 1))
+    bn, bg = bm.nll_grad_batch(lam)
+    rows = mfd.gather_toy_rows(np.concatenate([bn[:, None], bg], axis=1), T)
+    for t in range(T):
+        o_nll, o_g, _ = oracle.nll_grad(oracle.MASS, toys[t], dg.MASS_TRUTH, dg.MASS_LO, dg.MASS_HI)
+        assert abs(rows[t, 0] - o_nll) <= 1e-11 * abs(o_nll)
+        assert np.all(np.abs(rows[t, 1:] - o_g) <= 1e-9 * (1 + np.abs(o_g)))
+    dist.barrier()
+    dist.destroy_process_group()
+    print("dist ok", rank)
+""")
+
+
+def test_dist_with_cuda_shard_sums(mf):
+    """paper_2505_12414_b200.dist over gloo, world_size 2, both ranks on cuda:0 (independent kernels: no rank waits for
+    another on the device): the shard sums come from the CUDA path, the totals are compared with the oracle."""
+    import socket
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = str(s.getsockname()[1])
+    s.close()
+    code = _DIST_WORKER.format(root=ROOT)
+    procs = [subprocess.Popen([sys.executable, "-c", code, str(r), "2", port], stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True)
+             for r in range(2)]
+    outs = [p.communicate(timeout=600) for p in procs]
+    for r, (p, (so, se)) in enumerate(zip(procs, outs)):
+        assert p.returncode == 0 and f"dist ok {r}" in so, so[-2000:] + se[-4000:]
