@@ -135,6 +135,7 @@ extern "C" void mf_ctx_destroy(mf_ctx* ctx)
 {
     if (!ctx) return;
     cudaStreamSynchronize(ctx->stream);
+    if (ctx->p_blk) cudaFreeAsync(ctx->p_blk, ctx->stream);
     if (ctx->h_slab) cudaFreeHost(ctx->h_slab);
     if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
     for (int i = 0; i < mf_ctx::kPointStages; ++i) {
@@ -288,7 +289,6 @@ extern "C" void mf_model_destroy(mf_model* m)
     dev_free(m->ctx, m->d_consts_ok);
     dev_free(m->ctx, m->d_ids);
     dev_free(m->ctx, m->d_bout);
-    dev_free(m->ctx, m->p_blk);
     dev_free(m->ctx, m->d_sweep);
     host_slot_release(m->ctx, m->h_out);
     devbuf_release(m->raw);
@@ -602,23 +602,25 @@ static mf_status launch_points(mf_model* m, int64_t n_points, const double* lamb
     const int chunks = (int)chunks64;
     // device scratch [consts | ok | partials | bad | ticket], laid out for the largest (points, chunks) seen so far
     auto up = [](size_t x) { return (x + 255) / 256 * 256; };
-    if (n_points > m->p_points || chunks > m->p_chunks || !m->p_blk) {
-        const int64_t P = std::max<int64_t>(n_points, m->p_points);
-        const int C = std::max(chunks, m->p_chunks);
+    if (n_points > ctx->p_points || chunks > ctx->p_chunks || !ctx->p_blk) {
+        const int64_t P = std::max<int64_t>(n_points, ctx->p_points);
+        const int C = std::max(chunks, ctx->p_chunks);
         const size_t bytes = up(sizeof(FourDConsts) * P) + up(sizeof(int) * P) + up(sizeof(double) * P * MF_MAX_NACC * C) +
                              up(sizeof(unsigned) * P * C) + up(sizeof(unsigned) * P);
-        dev_free(ctx, m->p_blk);  // stream-ordered: after the launches that still use it
-        m->p_blk = nullptr;
-        MF_CUDA(ctx, dev_alloc(ctx, &m->p_blk, bytes));
-        m->p_bytes = bytes;
-        m->p_points = P;
-        m->p_chunks = C;
+        dev_free(ctx, ctx->p_blk);  // stream-ordered: after the launches that still use it
+        ctx->p_blk = nullptr;
+        ctx->p_points = 0;
+        ctx->p_chunks = 0;
+        MF_CUDA(ctx, dev_alloc(ctx, &ctx->p_blk, bytes));
+        ctx->p_bytes = bytes;
+        ctx->p_points = P;
+        ctx->p_chunks = C;
         // ok flags non-zero (every point is validated on the host), tickets zero (the kernel leaves them at zero)
-        MF_CUDA(ctx, cudaMemsetAsync(m->p_blk + up(sizeof(FourDConsts) * P), 0xFF, up(sizeof(int) * P), ctx->stream));
-        MF_CUDA(ctx, cudaMemsetAsync(m->p_blk + bytes - up(sizeof(unsigned) * P), 0, up(sizeof(unsigned) * P), ctx->stream));
+        MF_CUDA(ctx, cudaMemsetAsync(ctx->p_blk + up(sizeof(FourDConsts) * P), 0xFF, up(sizeof(int) * P), ctx->stream));
+        MF_CUDA(ctx, cudaMemsetAsync(ctx->p_blk + bytes - up(sizeof(unsigned) * P), 0, up(sizeof(unsigned) * P), ctx->stream));
     }
-    const int64_t P = m->p_points;
-    const int C = m->p_chunks;
+    const int64_t P = ctx->p_points;
+    const int C = ctx->p_chunks;
     BatchArgs<M> a;
     for (int i = 0; i < M::NCOL; ++i) a.col[i] = m->col[i];
     a.toy_stride = 0;
@@ -631,7 +633,7 @@ static mf_status launch_points(mf_model* m, int64_t n_points, const double* lamb
     a.sum_m = m->d_sum_m;
     a.lam = nullptr;
     a.lam_external = 0;
-    char* q = m->p_blk;
+    char* q = ctx->p_blk;
     a.consts = reinterpret_cast<Consts*>(q);
     q += up(sizeof(FourDConsts) * P);
     a.consts_ok = reinterpret_cast<int*>(q);

@@ -28,6 +28,13 @@ struct mf_ctx {
     size_t h_pts_bytes[kPointStages] = {};
     cudaEvent_t pts_copied[kPointStages] = {};
     unsigned pts_seq = 0;
+    // device scratch of the many-points evaluation (mf_nll_grad_points / mf_nll_grad_sweep), shared by all models of the
+    // context (every launch is ordered on the one stream, and the kernel touches the scratch only after its programmatic
+    // wait): grow-only, laid out as [consts | ok | partials | bad | ticket] for the largest (points, chunks) seen so far
+    char* p_blk = nullptr;
+    size_t p_bytes = 0;
+    int64_t p_points = 0;
+    int p_chunks = 0;
 };
 
 constexpr int MF_HOST_SLOT_DOUBLES = 64;  // widest output row (angular Hessian: 45 + n_bad) and the done word
@@ -88,12 +95,7 @@ struct mf_model {
     int* h_ids = nullptr;             //   [n_toys][K], [n_toys], [n_toys][widest output row]
     double* h_bout = nullptr;
     int bout_row = 0;                 // widest output row + n_bad (doubles)
-    // many-points evaluation (mf_nll_grad_points / mf_nll_grad_sweep): grow-only scratch, reused by every call
-    char* p_blk = nullptr;            // device [consts | ok | partials | bad | ticket]
-    size_t p_bytes = 0;
-    int64_t p_points = 0;             // points and chunks the block was laid out for (tickets are zero between calls)
-    int p_chunks = 0;
-    double* d_sweep = nullptr;        // device [p_sweep_rows][K+2] results of mf_nll_grad_sweep
+    double* d_sweep = nullptr;        // device [p_sweep_rows][K+2] results of mf_nll_grad_sweep (grow-only)
     int64_t p_sweep_rows = 0;
 };
 
