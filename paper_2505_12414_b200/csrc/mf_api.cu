@@ -358,7 +358,7 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
     }
     if (kind != MF_ANGULAR_KSTMUMU) {
         // S1: sum_i m_i per toy (ln P_i contains tau m_i: its sum is an event-only constant times tau)
-        MF_CUDA_M(dev_alloc(ctx, &m->d_sum_m, sizeof(double) * m->n_toys));
+        MF_CUDA_M(dev_alloc(ctx, &m->d_sum_m, sizeof(double2) * m->n_toys));
         const int chunks = (int)std::max<int64_t>(1, std::min<int64_t>(m->n_pad / 8192, 512));
         if (chunks > 1) MF_CUDA_M(dev_alloc(ctx, &d_part, sizeof(double2) * m->n_toys * chunks));
         column_sum_kernel<<<(unsigned)(m->n_toys * chunks), 256, 0, ctx->stream>>>(raw, m->n_events, m->n_pad, chunks, d_part,
@@ -374,7 +374,12 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
         d_part = nullptr;
     }
     // launch geometry: persistent-style grid, CTAS_PER_SM CTAs per SM (one wave), never more CTAs than 8-warp groups of items
-    const int64_t n_items = m->n_pad / kItem;
+    // work units dealt to warps: 64-event items, or 256-event groups for the one-column mass model
+    const int64_t n_items = (kind == MF_MASS_GAUSS_EXP) ? (m->n_pad / kItem + kGroupItems - 1) / kGroupItems : m->n_pad / kItem;
+    if (n_items > (int64_t)0x3fffffff) {
+        mf_model_destroy(m);
+        return mf_fail(ctx, MF_ERR_ARG, "mf_model_create: more than 2^30 work units per toy");
+    }
     const int ctas_per_sm = (kind == MF_MASS_X_ANGULAR) ? FourDModel::CTAS_PER_SM
                             : (kind == MF_ANGULAR_KSTMUMU) ? AngularModel::CTAS_PER_SM : MassModel::CTAS_PER_SM;
     m->grid = (int)std::max<int64_t>(1, std::min<int64_t>((n_items + kWarps - 1) / kWarps, ctas_per_sm * (int64_t)ctx->sm_count));
@@ -595,7 +600,8 @@ static mf_status launch_points(mf_model* m, int64_t n_points, const double* lamb
     const int64_t slots = (int64_t)M::BATCH_RESIDENT_CTAS * ctx->sm_count;
     static const int64_t per_cta = std::getenv("MF_POINTS_CTA_EVENTS") ? std::atoll(std::getenv("MF_POINTS_CTA_EVENTS")) : 65536;  // tuning knob
     const int64_t waves = std::max<int64_t>(1, (n_points * m->n_pad + slots * per_cta - 1) / (slots * per_cta));
-    const int64_t max_chunks = std::max<int64_t>(1, (m->n_pad / kItem + M::BATCH_BLOCK / 32 - 1) / (M::BATCH_BLOCK / 32));
+    const int64_t units = (M::NCOL == 1) ? (m->n_pad / kItem + kGroupItems - 1) / kGroupItems : m->n_pad / kItem;  // per warp: groups or items
+    const int64_t max_chunks = std::max<int64_t>(1, (units + M::BATCH_BLOCK / 32 - 1) / (M::BATCH_BLOCK / 32));
     const int64_t chunks64 = std::max<int64_t>(1, std::min<int64_t>(max_chunks, waves * slots / n_points));
     if (n_points * chunks64 > (int64_t)0x7fffffff)
         return mf_fail(ctx, MF_ERR_ARG, "mf_nll_grad_points: n_points x event chunks exceeds the grid limit; split the call");

@@ -70,7 +70,7 @@ struct mf_model {
     double ma = 0, mb = 0;            // mass normalisation range [m_a, m_b]
     mf_devbuf* raw = nullptr;         // shared with the dataset
     double* cache = nullptr;          // [9][n_toys][n_pad] angular basis columns (S1), or NULL
-    double* d_sum_m = nullptr;        // device [n_toys]: event-only constants sum_i m_i (S1), NULL without a mass dimension
+    double2* d_sum_m = nullptr;       // device [n_toys]: event-only constants sum_i m_i as (hi, lo) (S1), NULL without a mass dimension
     const double* col[MF_MAX_COLS] = {};  // column base pointers, stride between toys = n_pad
     // single-dataset evaluation
     int grid = 1;                     // CTAs of the fused kernel

@@ -37,7 +37,7 @@ struct EvalArgs {
     int64_t n;                   // valid events
     int64_t n_items;             // n_pad / 64
     typename M::Consts c;        // parameter-only constants (S2), computed on the host
-    const double* sum_m;         // device: event-only constant sum_i m_i (S1), or NULL for models without a mass dimension
+    const double2* sum_m;        // device: event-only constant sum_i m_i as (hi, lo) (S1), or NULL for models without a mass dimension
     // scratch slot of this evaluation (ring of kRing slots, so that successive evaluations do not
     // serialise on one scratch area; see "pipelining" below)
     double* partials;            // [NACC][gridDim.x]
@@ -59,7 +59,7 @@ struct BatchArgs {
     int64_t n_items;             // n_pad / 64 per toy
     int chunks;                  // CTAs per toy
     double ma, mb;               // mass range for the constants prologue
-    const double* sum_m;         // [n_toys] event-only constants sum_i m_i per toy, or NULL
+    const double2* sum_m;        // [n_toys] event-only constants sum_i m_i per toy as (hi, lo), or NULL
     const double* lam;           // [n_active][K]
     int lam_external;            // 1: lam was written by the caller's own work on the stream (mf_nll_grad_batch_async), so it
                                  // may only be read after griddepcontrol.wait; 0: written by a stream-ordered copy of ours
@@ -188,14 +188,84 @@ __device__ __forceinline__ void compute_group(int64_t n, int64_t n_items, int64_
     lp.renorm();  // at most 2U mantissas in [1,2) since the last one
 }
 
-// Items j0, j0 + step, j0 + 2 step, ... < n_items.  Two schedules:
-//  * PREFETCH == 0 (many columns, HBM bound): U items per iteration, software-pipelined with two register
-//    buffers (the loads of the next group are in flight while the current group is evaluated);
-//  * PREFETCH == D > 0 (one column, ALU bound): a rolling window of D items per thread — the slot of the
-//    item being evaluated is refilled at once with the item D steps ahead, so D 16-byte loads per
-//    thread stay in flight (memory latency x bandwidth needs ~44 KB in flight per SM).
-// get_c() yields the parameter-only constants; it is called AFTER the first loads have been issued (rolling
-// schedule), so that a kernel which must first fetch them (batched toys) overlaps that with the data latency.
+// The event loop of one warp for the one-column (ALU-bound) models.  The unit is a GROUP of kGroupItems = 4 consecutive
+// items = 256 consecutive events = 2 KB: lane l owns events 2l, 2l+1 of each of the four 64-event rows, read as four
+// 16-byte loads at immediate offsets from ONE pointer (one 64-bit pointer add and one 32-bit counter per group).
+// Groups g0, g0 + gstep, ... .  Latency: while a group is evaluated the warp's NEXT group is prefetched into L1 (four
+// prefetch instructions, no registers), so the loads at the top of the next iteration hit L1; keeping the next group in
+// registers instead (a second buffer, or a refill of the first) made ptxas copy the buffer twice per iteration.
+// FAST selects the model's fast event body (M::events<E, true>; decided per parameter point, M::is_fast).  The last,
+// partial group of the dataset (fewer than four items, or a ragged last item) is evaluated item by item by the warp it
+// falls to; only a ragged item is predicated.
+constexpr int kGroupItems = 4;
+constexpr int kGroupEvents = 2 * kGroupItems;  // per thread
+
+__device__ __forceinline__ void load_group4(const double2* __restrict__ p, double (&m)[kGroupEvents])
+{
+#pragma unroll
+    for (int i = 0; i < kGroupItems; ++i) {
+        const double2 v = __ldg(p + 32 * i);
+        m[2 * i] = v.x;
+        m[2 * i + 1] = v.y;
+    }
+}
+
+__device__ __forceinline__ void prefetch_group4(const double2* p)
+{
+#pragma unroll
+    for (int i = 0; i < kGroupItems; ++i) asm volatile("prefetch.global.L1 [%0];" ::"l"(p + 32 * i));
+}
+
+template <class M, bool FAST>
+__device__ __forceinline__ void group_loop(const double* col0, int64_t n, int64_t n_items, int g0, int gstep, int lane,
+                                           const typename M::Consts& c, double* acc, LogProd& lp, unsigned& bad, double t_lane)
+{
+    constexpr int E = M::EVENTS_PER_CALL;  // events the model evaluates together (interleaved instruction streams)
+    static_assert(kGroupEvents % E == 0, "a group is a whole number of calls");
+    const int n_full = (int)((n / kItem) / kGroupItems);  // groups 0 .. n_full-1 hold 256 valid events
+    const double2* p = reinterpret_cast<const double2*>(col0) + (int64_t)g0 * (32 * kGroupItems) + lane;
+    const int64_t pstep = (int64_t)gstep * (32 * kGroupItems);
+    // this warp's full groups: g0, g0 + gstep, ... < n_full
+    int left = (g0 < n_full) ? (n_full - g0 + gstep - 1) / gstep : 0;
+    const int g = g0 + left * gstep;  // this warp's first group index >= n_full
+    while (left > 0) {
+        double m[kGroupEvents];
+        load_group4(p, m);
+        --left;
+        p += (left > 0) ? pstep : 0;  // after the last group: prefetches that group again (harmless)
+        prefetch_group4(p);
+#pragma unroll
+        for (int q = 0; q < kGroupEvents / E; ++q) {
+            const double(&mq)[E] = *reinterpret_cast<const double(*)[E]>(&m[q * E]);
+            M::template events<E, FAST>(mq, c, acc, lp, bad, t_lane);
+            lp.renorm();
+        }
+    }
+    // the dataset's last, partial group: index n_full, if it exists and is one of this warp's
+    if (g == n_full && (int64_t)n_full * kGroupItems < n_items) {
+        const int64_t n_full_items = n / kItem;
+#pragma unroll 1
+        for (int64_t j = (int64_t)n_full * kGroupItems; j < n_items; ++j) {
+            const double2 v = __ldg(reinterpret_cast<const double2*>(col0) + j * 32 + lane);
+            const double x2[2] = {v.x, v.y};
+            if (j < n_full_items) {
+                M::template events<2, FAST>(x2, c, acc, lp, bad, t_lane);
+            } else {
+                const int64_t e = kItem * j + 2 * lane;
+                M::template event<true>(&x2[0], c, acc, lp, bad, e < n, t_lane);
+                M::template event<true>(&x2[1], c, acc, lp, bad, e + 1 < n, t_lane);
+            }
+            lp.renorm();
+        }
+    }
+}
+
+// The events of one warp.  Two schedules:
+//  * one column, ALU bound (M::NCOL == 1): 256-event groups j0, j0 + step, ... (group_loop above);
+//  * many columns, HBM bound: items (64 events) j0, j0 + step, ..., U items per iteration, software-pipelined with two
+//    register buffers (the loads of the next group are in flight while the current group is evaluated).
+// get_c() yields the parameter-only constants; it is called AFTER the first loads have been issued, so that a kernel
+// which must first fetch them (batched toys) overlaps that with the data latency.
 template <class M, class GetC>
 __device__ __forceinline__ void accumulate(const double* const* col, int64_t n, int64_t n_items, int64_t j0,
                                            int64_t step, GetC get_c, double* acc, unsigned& bad)
@@ -203,74 +273,18 @@ __device__ __forceinline__ void accumulate(const double* const* col, int64_t n, 
     const int lane = threadIdx.x & 31;
     const double t_lane = mf_exp32_lane_entry();
     LogProd lp;
-    if constexpr (M::PREFETCH > 0) {
-        constexpr int D = M::PREFETCH;
-        double buf[D][2][M::NCOL];
-#pragma unroll
-        for (int u = 0; u < D; ++u)
-            if (j0 + u * step < n_items) load_item<M>(col, j0 + u * step, lane, buf[u][0], buf[u][1]);
+    if constexpr (M::NCOL == 1) {
+        const int g0 = (int)j0, gstep = (int)step;  // group indices fit 32 bits (n_pad / 256; the host checks)
+        if (g0 < (int)((n / kItem) / kGroupItems))
+            prefetch_group4(reinterpret_cast<const double2*>(col[0]) + (int64_t)g0 * (32 * kGroupItems) + lane);
         decltype(auto) c = get_c();
-        constexpr int U = M::ITEMS_PER_ITER;  // items evaluated together: 2U independent events interleaved
-        static_assert(D % U == 0, "PREFETCH must be a multiple of ITEMS_PER_ITER");
-        const int64_t n_full = n / kItem;  // items 0 .. n_full-1 have 64 valid events
-        for (int64_t j = j0; j < n_items; j += D * step) {
-#pragma unroll
-            for (int u = 0; u < D; u += U) {
-                const int64_t ju = j + u * step;
-                if (ju < n_items) {
-                    // take the group out of the window and refill its slots at once (measured: refilling
-                    // after the evaluation saves the copies but costs the HBM-fed batch kernel 15%)
-                    double x[U][2][M::NCOL];
-#pragma unroll
-                    for (int v = 0; v < U; ++v) {
-#pragma unroll
-                        for (int q = 0; q < M::NCOL; ++q) {
-                            x[v][0][q] = buf[u + v][0][q];
-                            x[v][1][q] = buf[u + v][1][q];
-                        }
-                        const int64_t jn = ju + (v + D) * step;
-                        if (jn < n_items) load_item<M>(col, jn, lane, buf[u + v][0], buf[u + v][1]);
-                    }
-                    if (ju + (U - 1) * step < n_full) {
-                        if constexpr (M::NCOL == 1) {  // one column: the model evaluates the 2U events together
-                            double xs[2 * U];
-#pragma unroll
-                            for (int v = 0; v < U; ++v) {
-                                xs[2 * v] = x[v][0][0];
-                                xs[2 * v + 1] = x[v][1][0];
-                            }
-                            M::template events<2 * U>(xs, c, acc, lp, bad, t_lane);
-                        } else {
-#pragma unroll
-                            for (int v = 0; v < U; ++v) {
-                                M::template event<false>(x[v][0], c, acc, lp, bad, true, t_lane);
-                                M::template event<false>(x[v][1], c, acc, lp, bad, true, t_lane);
-                            }
-                        }
-                    } else {
-                        // the last, partial group of this warp (and the ragged last item of the dataset): full items
-                        // still go through the vectorised body, two events at a time; only a ragged item is predicated
-#pragma unroll
-                        for (int v = 0; v < U; ++v) {
-                            const int64_t jv = ju + v * step;
-                            if (jv < n_full) {
-                                if constexpr (M::NCOL == 1) {
-                                    const double xs[2] = {x[v][0][0], x[v][1][0]};
-                                    M::template events<2>(xs, c, acc, lp, bad, t_lane);
-                                } else {
-                                    M::template event<false>(x[v][0], c, acc, lp, bad, true, t_lane);
-                                    M::template event<false>(x[v][1], c, acc, lp, bad, true, t_lane);
-                                }
-                            } else if (jv < n_items) {
-                                const int64_t e = kItem * jv + 2 * lane;
-                                M::template event<true>(x[v][0], c, acc, lp, bad, e < n, t_lane);
-                                M::template event<true>(x[v][1], c, acc, lp, bad, e + 1 < n, t_lane);
-                            }
-                        }
-                    }
-                    lp.renorm();
-                }
-            }
+        if constexpr (M::HAS_FAST) {
+            if (M::is_fast(c))  // uniform over the CTA: one parameter point per CTA
+                group_loop<M, true>(col[0], n, n_items, g0, gstep, lane, c, acc, lp, bad, t_lane);
+            else
+                group_loop<M, false>(col[0], n, n_items, g0, gstep, lane, c, acc, lp, bad, t_lane);
+        } else {
+            group_loop<M, false>(col[0], n, n_items, g0, gstep, lane, c, acc, lp, bad, t_lane);
         }
     } else {
         decltype(auto) c = get_c();
@@ -335,7 +349,7 @@ __device__ __forceinline__ double block_reduce(double* acc, unsigned bad, double
 // previous kernel on the stream (outputs land in stream order).
 template <class M, int WARPS = kWarps>
 __device__ __forceinline__ void final_combine(const double* p, int64_t stride_k, int count, const unsigned* badp,
-                                              const typename M::Consts& c, double n, double sum_m, double* s_sum,
+                                              const typename M::Consts& c, double n, double2 sum_m, double* s_sum,
                                               double* out, unsigned long long* done_flag = nullptr,
                                               unsigned long long done_value = 0)
 {
@@ -418,8 +432,8 @@ __device__ __forceinline__ void reduce_and_finish(const EvalArgs<M>& a, double* 
     if (threadIdx.x == 0) s_last = (ticket_take(a.ticket) == gridDim.x - 1);
     __syncthreads();
     if (s_last) {
-        final_combine<M>(a.partials, G, (int)G, a.bad_partials, a.c, (double)a.n, a.sum_m ? __ldg(a.sum_m) : 0.0, s_sum, a.out,
-                         a.done_flag, a.done_value);
+        final_combine<M>(a.partials, G, (int)G, a.bad_partials, a.c, (double)a.n, a.sum_m ? __ldg(a.sum_m) : make_double2(0.0, 0.0),
+                         s_sum, a.out, a.done_flag, a.done_value);
         if (threadIdx.x == 0) {  // every partial has been read: final_combine synchronises the CTA before its thread 0 returns
             *a.ticket = 0u;
             gen_store(a.gen, a.need + 1);  // releases the slot (and the ticket reset) to evaluation e + kRing
@@ -591,7 +605,7 @@ __global__ void __launch_bounds__(M::BATCH_BLOCK, M::BATCH_RESIDENT_CTAS)
     }
     constexpr int NOUT = M::NOUT;  // -ln L, gradient (and Hessian for the *Hess models); n_bad follows at [NOUT]
     double* out = a.out + (int64_t)slot * (NOUT + 1);
-    const double sum_m = a.sum_m ? a.sum_m[toy] : 0.0;
+    const double2 sum_m = a.sum_m ? a.sum_m[toy] : make_double2(0.0, 0.0);
     const double* col[M::NCOL];
 #pragma unroll
     for (int i = 0; i < M::NCOL; ++i) col[i] = a.col[i] + toy * a.toy_stride;
@@ -651,7 +665,8 @@ __global__ void __launch_bounds__(M::BATCH_BLOCK, M::BATCH_RESIDENT_CTAS)
 
 // ---- S1: event-only constants: sum_i m_i per toy ------------------------------
 
-// Deterministic two-level sum.  Level 1: CTA (toy, chunk) sums events [chunk * len, (chunk+1) * len) of its
+// Deterministic two-level sum, returned as a (hi, lo) pair: the fast path of the mass model forms
+// sum_i (m_i - mu) = sum_i m_i - N mu from it, two terms that nearly cancel.  Level 1: CTA (toy, chunk) sums events [chunk * len, (chunk+1) * len) of its
 // toy — thread t Kahan-sums events t, t + 256, ..., the 256 (sum, compensation) pairs are merged by a
 // fixed two-sum tree in shared memory — and writes the pair to part[toy][chunk].  Level 2 (chunks > 1):
 // one thread per toy adds the chunk pairs in chunk order.
@@ -664,8 +679,14 @@ __device__ __forceinline__ void two_sum_acc(double& s, double& lo, double b, dou
     s = t;
 }
 
+__device__ __forceinline__ double2 fast_two_sum(double hi, double lo)  // |hi| >= |lo|: renormalised (hi, lo) pair
+{
+    const double s = hi + lo;
+    return make_double2(s, lo - (s - hi));
+}
+
 __global__ void __launch_bounds__(256) column_sum_kernel(const double* __restrict__ col, int64_t n, int64_t n_pad,
-                                                         int chunks, double2* __restrict__ part, double* __restrict__ out)
+                                                         int chunks, double2* __restrict__ part, double2* __restrict__ out)
 {
     __shared__ double sh[256], sl[256];
     const int toy = blockIdx.x / chunks, chunk = blockIdx.x % chunks;
@@ -693,13 +714,13 @@ __global__ void __launch_bounds__(256) column_sum_kernel(const double* __restric
     }
     if (threadIdx.x == 0) {
         if (chunks == 1)
-            out[toy] = sh[0] + sl[0];
+            out[toy] = fast_two_sum(sh[0], sl[0]);
         else
             part[blockIdx.x] = make_double2(sh[0], sl[0]);
     }
 }
 
-__global__ void column_sum_finish_kernel(const double2* __restrict__ part, int chunks, int64_t n_toys, double* __restrict__ out)
+__global__ void column_sum_finish_kernel(const double2* __restrict__ part, int chunks, int64_t n_toys, double2* __restrict__ out)
 {
     const int64_t toy = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (toy >= n_toys) return;
@@ -708,7 +729,7 @@ __global__ void column_sum_finish_kernel(const double2* __restrict__ part, int c
         const double2 p = part[toy * chunks + c];
         two_sum_acc(s, lo, p.x, p.y);
     }
-    out[toy] = s + lo;
+    out[toy] = fast_two_sum(s, lo);
 }
 
 // ---- S1: event-only precompute (Listing 4) ------------------

@@ -79,6 +79,12 @@ struct MassConsts {
     double ct;       // mu - m_a - ktau:  m - d ln N2/d tau = d + ct
     double n1mm, n1ms, n1ss;  // d2 ln N1 / d(mu, sigma)^2
     double n2tt;     // d2 ln N2 / d tau^2 = w^2 L'(tau w / 2) / 4
+    // 1.0 if this parameter point allows the event loop's fast path (MassModel::events<E, true>), else 0.0:
+    //   * 1 - f >= 1/4, so that D = (1-f) + f R >= 1/4 and the sums over r = 1/D can be derived from those over u = R/D
+    //     (f u + (1-f) r = 1 for every event) without amplifying their rounding by more than 4;
+    //   * every exponent argument lies in (-700, 69): no clamp in the exponential, D < 2^100, so the product of 8 factors D
+    //     cannot leave the normal range and no event can have "P <= 0".
+    double fast;
 };
 
 // derivative of the Langevin function, 1/x^2 - 1/sinh^2(x) (series below |x| = 0.1: cancellation)
@@ -146,6 +152,13 @@ MF_HD inline bool mass_consts(const double* lam, double ma, double mb, MassConst
     // ... and whose most negative one is beyond the range in which mf_exp32 reduces its argument
     const double dmax = fmax(fabs(ma - mu), fabs(mb - mu));
     if (!(-c.nb0 * dmax * dmax + fabs(tau) * mmax + fabs(c.lnk) < 1e12)) return false;
+    // bounds of ln R = -b0 d^2 - tau m + lnk over the range: -b0 d^2 <= 0
+    const double arg_hi = c.lnk + fabs(tau) * mmax, arg_lo = c.nb0 * dmax * dmax - fabs(tau) * mmax + c.lnk;
+#ifdef MF_MASS_NO_FAST
+    c.fast = 0.0;  // ablation: always the general path
+#else
+    c.fast = (c.omf >= 0.25 && arg_hi < 69.0 && arg_lo > -700.0) ? 1.0 : 0.0;
+#endif
     return true;
 }
 
@@ -218,11 +231,8 @@ struct MassModel {
     static constexpr int NACC = 6;  // ln prod D, and with u = (G/N1)/P', r = (E/N2)/P' (P' = P N2 e^{-tau m}, d = m - mu):
                                     // sum u, sum r, sum u d, sum u d^2, sum r d
     // tuning knobs (defaults = the measured best on B200)
-#ifndef MF_MASS_U
-#define MF_MASS_U 4
-#endif
-#ifndef MF_MASS_PREFETCH
-#define MF_MASS_PREFETCH 4
+#ifndef MF_MASS_EVENTS
+#define MF_MASS_EVENTS 8
 #endif
 #ifndef MF_MASS_GRID
 #define MF_MASS_GRID 2
@@ -230,8 +240,7 @@ struct MassModel {
 #ifndef MF_MASS_RESIDENT
 #define MF_MASS_RESIDENT 2
 #endif
-    static constexpr int ITEMS_PER_ITER = MF_MASS_U;    // x2 independent events in flight per thread
-    static constexpr int PREFETCH = MF_MASS_PREFETCH;   // rolling window of 16-byte loads in flight per thread (0: double buffer)
+    static constexpr int EVENTS_PER_CALL = MF_MASS_EVENTS;  // independent events interleaved per thread (a 256-event group is 8 per thread)
     static constexpr int CTAS_PER_SM = MF_MASS_GRID;    // grid of a lone (synchronous) evaluation: CTAs per SM
 #ifndef MF_MASS_BATCH_RESIDENT
 #define MF_MASS_BATCH_RESIDENT 4
@@ -267,9 +276,18 @@ struct MassModel {
         }
     }
 
-    // E full events at once (the fast path of the event loop), written operation by operation across the E
+    static constexpr bool HAS_FAST = true;
+    static MF_D bool is_fast(const Consts& c) { return c.fast != 0.0; }
+
+    // E full events at once (the body of the event loop), written operation by operation across the E
     // events so that the instruction stream is interleaved as issued and constants are shared operands.
-    template <int E>
+    // FAST (Consts::fast, decided per parameter point where the constants are made): D is known to lie in [1/4, 2^100], so
+    //   * the E factors are multiplied by a tree and enter the running product as ONE bounded factor: one exponent
+    //     extraction per E events (the caller's renorm()) instead of one per event, and no "P <= 0" test;
+    //   * the exponential needs no clamp;
+    //   * sum r and sum r d are not accumulated: f u + (1-f) r = 1 gives them from sum u, sum u d and the event-only
+    //     constant sum_i m_i (finish).  24 fp64 instructions per event instead of 26.
+    template <int E, bool FAST>
     static MF_D void events(const double (&m)[E], const Consts& c, double* acc, LogProd& lp, unsigned& bad, double t_lane)
     {
         double d[E], t[E], arg[E], R[E], D[E], r[E], u[E];
@@ -281,34 +299,88 @@ struct MassModel {
         for (int e = 0; e < E; ++e) t[e] = d[e] * d[e];
 #pragma unroll
         for (int e = 0; e < E; ++e) arg[e] = fma(c.nb0, t[e], arg[e]);
-        mf_exp32_v<E>(arg, t_lane, R);
+        mf_exp32_v<E, FAST>(arg, t_lane, R);
 #pragma unroll
         for (int e = 0; e < E; ++e) D[e] = fma(c.f, R[e], c.omf);
+        if constexpr (FAST) {
+            static_assert(E <= 8 && (E & (E - 1)) == 0, "the product of E factors below 2^100 must stay below 2^900");
+            // product tree of the E factors: P[l][i] = product of factors i 2^l .. (i+1) 2^l - 1
+            constexpr int L = (E == 8) ? 3 : (E == 4) ? 2 : (E == 2) ? 1 : 0;  // levels of the tree
+            double P[4][E];
 #pragma unroll
-        for (int e = 0; e < E; ++e) r[e] = mf_rcp(D[e]);
+            for (int e = 0; e < E; ++e) P[0][e] = D[e];
 #pragma unroll
-        for (int e = 0; e < E; ++e) u[e] = R[e] * r[e];
+            for (int l = 0; l < L; ++l)
 #pragma unroll
-        for (int e = 0; e < E; ++e) {
-            lp.mul(D[e], bad);
-            acc[1] += u[e];
-            acc[2] += r[e];
-            acc[3] = fma(u[e], d[e], acc[3]);
-            acc[4] = fma(u[e], t[e], acc[4]);
-            acc[5] = fma(r[e], d[e], acc[5]);
+                for (int i = 0; i < (E >> (l + 1)); ++i) P[l + 1][i] = P[l][2 * i] * P[l][2 * i + 1];
+            lp.mul_bounded(P[L][0]);
+            // ONE Newton reciprocal for the E events, of the root of the tree, pushed back down: the reciprocal of a node is
+            // its sibling's product times the parent's reciprocal (2 - 2/E multiplications per event instead of a 3-DFMA
+            // Newton step, a MUFU and a register move each)
+            double I[4][E];
+            I[L][0] = mf_rcp(P[L][0]);
+#pragma unroll
+            for (int l = L; l > 0; --l)
+#pragma unroll
+                for (int i = 0; i < (E >> l); ++i) {
+                    I[l - 1][2 * i] = P[l - 1][2 * i + 1] * I[l][i];
+                    I[l - 1][2 * i + 1] = P[l - 1][2 * i] * I[l][i];
+                }
+#pragma unroll
+            for (int e = 0; e < E; ++e) u[e] = R[e] * I[0][e];
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                acc[1] += u[e];
+                acc[3] = fma(u[e], d[e], acc[3]);
+                acc[4] = fma(u[e], t[e], acc[4]);
+            }
+        } else {
+#pragma unroll
+            for (int e = 0; e < E; ++e) r[e] = mf_rcp(D[e]);
+#pragma unroll
+            for (int e = 0; e < E; ++e) u[e] = R[e] * r[e];
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                lp.mul(D[e], bad);
+                acc[1] += u[e];
+                acc[2] += r[e];
+                acc[3] = fma(u[e], d[e], acc[3]);
+                acc[4] = fma(u[e], t[e], acc[4]);
+                acc[5] = fma(r[e], d[e], acc[5]);
+            }
         }
     }
 
     // ln P = tau m - ln N2 + ln D
     // d ln P/df = u - r;  d/dmu = f u (d/sigma^2 - kmu);  d/dsigma = f u (d^2/sigma^3 - ksig);
     // d/dtau = (1-f) r (m - m_a - ktau) = (1-f) r (d + mu - m_a - ktau)
-    static MF_D void finish(const Consts& c, const double* s, double n, double sum_m, double* out)
+    // sum_m = (hi, lo) of the event-only constant sum_i m_i.
+    static MF_D void finish_general(const Consts& c, const double* s, double n, double2 sum_m, double* out)
     {
-        out[0] = -(s[0] + fma(c.tau, sum_m, n * c.lnc2));
+        out[0] = -(s[0] + fma(c.tau, sum_m.x, fma(c.tau, sum_m.y, n * c.lnc2)));
         out[1] = -(s[1] - s[2]);
         out[2] = -c.f * diff_of_products(c.is2, s[3], c.kmu, s[1]);
         out[3] = -c.f * diff_of_products(c.is3, s[4], c.ksig, s[1]);
         out[4] = -c.omf * fma((c.mu - c.ma) - c.ktau, s[2], s[5]);
+    }
+
+    // Fast path: s[2] (sum r) and s[5] (sum r d) were not accumulated.  With f u + (1-f) r = 1 for every event:
+    //   (1-f) sum r   = N - f sum u            ->  sum u - sum r = (sum u - N) / (1-f)
+    //   (1-f) sum r d = sum d - f sum u d,   sum d = sum_i m_i - N mu  (double-double: the two terms nearly cancel)
+    static MF_D void finish(const Consts& c, const double* s, double n, double2 sum_m, double* out)
+    {
+        if (c.fast == 0.0) {
+            finish_general(c, s, n, sum_m, out);
+            return;
+        }
+        const double Su = s[1], Sud = s[3], Sut = s[4];
+        const double p = n * c.mu, pe = fma(n, c.mu, -p);       // N mu = p + pe exactly
+        const double Sd = (sum_m.x - p) + (sum_m.y - pe);
+        out[0] = -(s[0] + fma(c.tau, sum_m.x, fma(c.tau, sum_m.y, n * c.lnc2)));
+        out[1] = -(Su - n) / c.omf;
+        out[2] = -c.f * diff_of_products(c.is2, Sud, c.kmu, Su);
+        out[3] = -c.f * diff_of_products(c.is3, Sut, c.ksig, Su);
+        out[4] = -fma(c.ct, fma(-c.f, Su, n), fma(-c.f, Sud, Sd));
     }
 };
 
@@ -327,15 +399,18 @@ struct MassHessModel {
     static constexpr int NCOL = 1;
     static constexpr int NOUT = 1 + 4 + 10;
     static constexpr int NACC = 13;
-    static constexpr int ITEMS_PER_ITER = 2;  // 4 events at once (13 sums leave fewer registers)
-    static constexpr int PREFETCH = 4;
+    static constexpr int EVENTS_PER_CALL = 4;  // 4 events at once (13 sums leave fewer registers)
     static constexpr int CTAS_PER_SM = 2;
     static constexpr int RESIDENT_CTAS = 2;
     static constexpr int BATCH_RESIDENT_CTAS = 4;
     static constexpr int BATCH_BLOCK = 128;
     using Consts = MassConsts;
+    static constexpr bool HAS_FAST = true;
+    static MF_D bool is_fast(const Consts& c) { return c.fast != 0.0; }
 
-    template <int E>
+    // FAST: as MassModel's, but only the integer side (no clamp, one exponent extraction per E events, no "P <= 0" test);
+    // all 13 sums are accumulated.
+    template <int E, bool FAST>
     static MF_D void events(const double (&m)[E], const Consts& c, double* acc, LogProd& lp, unsigned& bad, double t_lane)
     {
         double d[E], t[E], arg[E], R[E], D[E], r[E], u[E], z[E];
@@ -347,7 +422,7 @@ struct MassHessModel {
         for (int e = 0; e < E; ++e) t[e] = d[e] * d[e];
 #pragma unroll
         for (int e = 0; e < E; ++e) arg[e] = fma(c.nb0, t[e], arg[e]);
-        mf_exp32_v<E>(arg, t_lane, R);
+        mf_exp32_v<E, FAST>(arg, t_lane, R);
 #pragma unroll
         for (int e = 0; e < E; ++e) D[e] = fma(c.f, R[e], c.omf);
 #pragma unroll
@@ -356,9 +431,20 @@ struct MassHessModel {
         for (int e = 0; e < E; ++e) u[e] = R[e] * r[e];
 #pragma unroll
         for (int e = 0; e < E; ++e) z[e] = u[e] * r[e];
+        if constexpr (FAST) {
+            static_assert(E <= 8, "the product of E factors below 2^100 must stay below 2^900");
+            double P[E];
+#pragma unroll
+            for (int e = 0; e < E; ++e) P[e] = D[e];
+#pragma unroll
+            for (int s = 1; s < E; s <<= 1)
+#pragma unroll
+                for (int e = 0; e + s < E; e += 2 * s) P[e] *= P[e + s];
+            lp.mul_bounded(P[0]);
+        }
 #pragma unroll
         for (int e = 0; e < E; ++e) {
-            lp.mul(D[e], bad);
+            if constexpr (!FAST) lp.mul(D[e], bad);
             acc[1] += u[e];
             acc[2] += r[e];
             acc[3] = fma(u[e], d[e], acc[3]);
@@ -386,7 +472,7 @@ struct MassHessModel {
         LogProd lp2;
         unsigned bad2 = 0;
         const double m1[1] = {x[0]};
-        events<1>(m1, c, tmp, lp2, bad2, t_lane);
+        events<1, false>(m1, c, tmp, lp2, bad2, t_lane);
         if (!PRED || valid) {
 #pragma unroll
             for (int k = 1; k < NACC; ++k) acc[k] += tmp[k];
@@ -396,9 +482,9 @@ struct MassHessModel {
         }
     }
 
-    static MF_D void finish(const Consts& c, const double* s, double n, double sum_m, double* out)
+    static MF_D void finish(const Consts& c, const double* s, double n, double2 sum_m, double* out)
     {
-        MassModel::finish(c, s, n, sum_m, out);
+        MassModel::finish_general(c, s, n, sum_m, out);
         const double Su = s[1], Sr = s[2], Sud = s[3], Sud2 = s[4];
         const double Suu = s[6], Srr = s[7], Sz = s[8], Szd = s[9], Szd2 = s[10], Szd3 = s[11], Szd4 = s[12];
         const double fo = c.f * c.omf, ct = c.ct, kmu = c.kmu, ksig = c.ksig, is2 = c.is2, is3 = c.is3;
@@ -431,6 +517,7 @@ struct MassHessModel {
 };
 
 struct AngularModel {
+    static constexpr bool HAS_FAST = false;
     static constexpr int K = 8;
     static constexpr int NCOL = 9;  // h_0..h_8 (cached, already times 9/(32 pi))
     static constexpr int NOUT = K + 1;
@@ -458,7 +545,7 @@ struct AngularModel {
         }
     }
 
-    static MF_D void finish(const Consts&, const double* s, double, double, double* out)
+    static MF_D void finish(const Consts&, const double* s, double, double2, double* out)
     {
 #pragma unroll
         for (int k = 0; k < NACC; ++k) out[k] = -s[k];
@@ -470,6 +557,7 @@ struct AngularModel {
 // 36 more sums than AngularModel; still one pass over the nine cached columns.
 // Output: -ln L, gradient[8], then the upper triangle (k <= l, row by row) of d2(-ln L).
 struct AngularHessModel {
+    static constexpr bool HAS_FAST = false;
     static constexpr int K = 8;
     static constexpr int NCOL = 9;
     static constexpr int NOUT = 1 + 8 + 36;
@@ -506,7 +594,7 @@ struct AngularHessModel {
         }
     }
 
-    static MF_D void finish(const Consts&, const double* s, double, double, double* out)
+    static MF_D void finish(const Consts&, const double* s, double, double2, double* out)
     {
 #pragma unroll
         for (int k = 0; k < 9; ++k) out[k] = -s[k];
@@ -516,6 +604,7 @@ struct AngularHessModel {
 };
 
 struct FourDModel {
+    static constexpr bool HAS_FAST = false;
     static constexpr int K = 16;
     static constexpr int NCOL = 12;  // m, cos theta_l, cos theta_K, h_0..h_8
     static constexpr int NOUT = K + 1;
@@ -576,9 +665,9 @@ struct FourDModel {
     }
 
     // ln P = tau m - ln N2 + ln D
-    static MF_D void finish(const Consts& c, const double* s, double n, double sum_m, double* out)
+    static MF_D void finish(const Consts& c, const double* s, double n, double2 sum_m, double* out)
     {
-        out[0] = -(s[0] + fma(c.m.tau, sum_m, n * c.m.lnc2));
+        out[0] = -(s[0] + fma(c.m.tau, sum_m.x, fma(c.m.tau, sum_m.y, n * c.m.lnc2)));
 #pragma unroll
         for (int k = 1; k < NACC; ++k) out[k] = -s[k];
     }
