@@ -53,6 +53,14 @@ def _load():
         lib.mfo_nll_grad.restype = ctypes.c_int64
         lib.mfo_nll_grad.argtypes = [ctypes.c_int, ctypes.c_int64, dpp, dp, ctypes.c_double,
                                      ctypes.c_double, ctypes.c_int, dp, dp]
+        lib.mfo_nll_grad_w.restype = ctypes.c_int64
+        lib.mfo_nll_grad_w.argtypes = [ctypes.c_int, ctypes.c_int64, dpp, dp, dp, ctypes.c_double,
+                                       ctypes.c_double, ctypes.c_int, dp, dp]
+        lib.mfo_nll_grad_hess_w.restype = ctypes.c_int64
+        lib.mfo_nll_grad_hess_w.argtypes = [ctypes.c_int, ctypes.c_int64, dpp, dp, dp, ctypes.c_double, ctypes.c_double,
+                                            dp, dp, dp, dp]
+        lib.mfo_hess_points.restype = ctypes.c_int
+        lib.mfo_hess_points.argtypes = [ctypes.c_int, ctypes.c_int64, dpp, dp, ctypes.c_double, ctypes.c_double, dp, dp, dp]
         lib.mfo_pdf.restype = ctypes.c_int
         lib.mfo_pdf.argtypes = [ctypes.c_int, ctypes.c_int64, dpp, dp, ctypes.c_double,
                                 ctypes.c_double, dp, dp]
@@ -105,39 +113,90 @@ def max_threads() -> int:
     return int(_load().mfo_max_threads())
 
 
+def _weights(weights, n: int):
+    if weights is None:
+        return None
+    w = np.ascontiguousarray(weights, dtype=np.float64)
+    if w.shape != (n,):
+        raise ValueError(f"weights must have shape ({n},)")
+    return w
+
+
 def nll_grad(kind: int, events, lam, lo: float = 0.0, hi: float = 0.0, nthreads: int = 1,
-             want_grad: bool = True):
-    """(-ln L, d(-ln L)/d lambda, n_bad) over all events (Eq. 1)."""
+             want_grad: bool = True, weights=None):
+    """(-ln L, d(-ln L)/d lambda, n_bad) over all events (Eq. 1); with ``weights`` the weighted sums
+    -sum_i w_i ln P_i (reading R23)."""
     lib = _load()
     cols, n = _columns(kind, events)
     lam = np.ascontiguousarray(lam, dtype=np.float64)
     if not check_domain(kind, lam):
         raise ValueError("parameter outside its domain")
+    w = _weights(weights, n)
     nll = ctypes.c_double(0.0)
     grad = np.zeros(NPARAMS[kind], dtype=np.float64)
-    nbad = lib.mfo_nll_grad(kind, n, _colptrs(cols), _dptr(lam), lo, hi, int(nthreads),
-                            ctypes.byref(nll), _dptr(grad) if want_grad else None)
+    if w is None:
+        nbad = lib.mfo_nll_grad(kind, n, _colptrs(cols), _dptr(lam), lo, hi, int(nthreads),
+                                ctypes.byref(nll), _dptr(grad) if want_grad else None)
+    else:
+        nbad = lib.mfo_nll_grad_w(kind, n, _colptrs(cols), _dptr(w), _dptr(lam), lo, hi, int(nthreads),
+                                  ctypes.byref(nll), _dptr(grad) if want_grad else None)
     if nbad < 0:
         raise ValueError("bad argument")
     return float(nll.value), (grad if want_grad else None), int(nbad)
 
 
-def nll_grad_hess(kind: int, events, lam, lo: float = 0.0, hi: float = 0.0):
-    """(-ln L, gradient [K], Hessian [K][K], n_bad) for the mass and angular kinds (analytic second derivatives,
-    PAPER.md:39, 53)."""
+def nll_grad_hess(kind: int, events, lam, lo: float = 0.0, hi: float = 0.0, weights=None, want_fisher: bool = False):
+    """(-ln L, gradient [K], Hessian [K][K], n_bad) from the analytic second derivatives (PAPER.md:39, 53;
+    SURVEY.md §8(f)-1), all three kinds, optionally weighted.  ``want_fisher``: also returns
+    sum_i w_i^2 s_i s_i^T (s = d ln P/d lambda, reading R23) as a fifth element, before n_bad."""
     lib = _load()
     cols, n = _columns(kind, events)
     lam = np.ascontiguousarray(lam, dtype=np.float64)
     if not check_domain(kind, lam):
         raise ValueError("parameter outside its domain")
+    w = _weights(weights, n)
+    K = NPARAMS[kind]
+    nll = ctypes.c_double(0.0)
+    grad = np.zeros(K, dtype=np.float64)
+    hess = np.zeros((K, K), dtype=np.float64)
+    fisher = np.zeros((K, K), dtype=np.float64)
+    nbad = lib.mfo_nll_grad_hess_w(kind, n, _colptrs(cols), _dptr(w) if w is not None else None, _dptr(lam), lo, hi,
+                                   ctypes.byref(nll), _dptr(grad), _dptr(hess), _dptr(fisher))
+    if nbad < 0:
+        raise ValueError("bad argument")
+    if want_fisher:
+        return float(nll.value), grad, hess, fisher, int(nbad)
+    return float(nll.value), grad, hess, int(nbad)
+
+
+def nll_grad_hess_unweighted_c(kind: int, events, lam, lo: float = 0.0, hi: float = 0.0):
+    """mfo_nll_grad_hess as first written (mass and angular kinds only); kept so that a test can show that the weighted
+    routine with w = NULL reproduces it bit for bit."""
+    lib = _load()
+    cols, n = _columns(kind, events)
+    lam = np.ascontiguousarray(lam, dtype=np.float64)
     K = NPARAMS[kind]
     nll = ctypes.c_double(0.0)
     grad = np.zeros(K, dtype=np.float64)
     hess = np.zeros((K, K), dtype=np.float64)
     nbad = lib.mfo_nll_grad_hess(kind, n, _colptrs(cols), _dptr(lam), lo, hi, ctypes.byref(nll), _dptr(grad), _dptr(hess))
     if nbad < 0:
-        raise ValueError("bad argument (no analytic Hessian for this kind)")
+        raise ValueError("bad argument (mass and angular kinds only)")
     return float(nll.value), grad, hess, int(nbad)
+
+
+def hess_points(kind: int, events, lam, lo: float = 0.0, hi: float = 0.0):
+    """Per event: P [n], d ln P/d lambda [n][K], d2 ln P/d lambda^2 [n][K][K]."""
+    lib = _load()
+    cols, n = _columns(kind, events)
+    lam = np.ascontiguousarray(lam, dtype=np.float64)
+    K = NPARAMS[kind]
+    P = np.empty(n)
+    g = np.empty((n, K))
+    H = np.empty((n, K, K))
+    if lib.mfo_hess_points(kind, n, _colptrs(cols), _dptr(lam), lo, hi, _dptr(P), _dptr(g), _dptr(H)) != 0:
+        raise ValueError("bad argument")
+    return P, g, H
 
 
 def mass_hess_points(m, lam, lo: float, hi: float):
@@ -204,6 +263,7 @@ class FitResult:
     converged: bool
     n_iter: int = 0
     history: list = field(default_factory=list)
+    cov_hesse: np.ndarray | None = None   # H^-1 (equals cov for an unweighted fit)
 
     @property
     def sigma(self):
@@ -211,7 +271,7 @@ class FitResult:
 
 
 def fit(kind: int, events, start, fixed=None, lo: float = 0.0, hi: float = 0.0,
-        opts: FitOptions | None = None, nthreads: int = 1) -> FitResult:
+        opts: FitOptions | None = None, nthreads: int = 1, weights=None) -> FitResult:
     """Quasi-Newton fit of SURVEY.md §8(c) "Fit", in the order stated there:
 
     1. seed the inverse Hessian with a central-difference Hessian of the analytic gradient
@@ -220,6 +280,10 @@ def fit(kind: int, events, start, fixed=None, lo: float = 0.0, hi: float = 0.0,
        non-finite points, domain errors and P<=0 points, until EDM = g^T H^-1 g / 2 < edm_tol;
     3. polish: central-difference Hessian of the analytic gradient, then Newton steps with
        that Hessian until max_k |step_k|/sigma_k < polish_tol; cov = H^-1.
+
+    With ``weights`` the minimised function is -sum_i w_i ln P_i and the returned covariance is the sandwich
+    H^-1 F H^-1 with F = sum_i w_i^2 s_i s_i^T evaluated at the minimum (reading R23); the
+    convergence test keeps using H^-1 (``cov_hesse``).
     """
     o = opts or FitOptions()
     K = NPARAMS[kind]
@@ -234,7 +298,7 @@ def fit(kind: int, events, start, fixed=None, lo: float = 0.0, hi: float = 0.0,
         calls += 1
         if not check_domain(kind, xx):
             return math.inf, None
-        v, g, nbad = nll_grad(kind, events, xx, lo, hi, nthreads)
+        v, g, nbad = nll_grad(kind, events, xx, lo, hi, nthreads, weights=weights)
         if nbad or not math.isfinite(v) or not np.all(np.isfinite(g)):
             return math.inf, None
         return v, g[idx]
@@ -328,4 +392,9 @@ def fit(kind: int, events, start, fixed=None, lo: float = 0.0, hi: float = 0.0,
 
     cov_full = np.zeros((K, K))
     cov_full[np.ix_(idx, idx)] = cov
-    return FitResult(lam=x, cov=cov_full, nll=f, n_calls=calls, converged=converged, n_iter=n_iter)
+    cov_hesse = cov_full
+    if weights is not None:
+        fisher = nll_grad_hess(kind, events, x, lo, hi, weights=weights, want_fisher=True)[3]
+        cov_full = np.zeros((K, K))
+        cov_full[np.ix_(idx, idx)] = cov @ fisher[np.ix_(idx, idx)] @ cov
+    return FitResult(lam=x, cov=cov_full, nll=f, n_calls=calls, converged=converged, n_iter=n_iter, cov_hesse=cov_hesse)

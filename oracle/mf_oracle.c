@@ -34,8 +34,12 @@
  * Pins (tests/test_oracle_*.py): unit integral by quadrature, positivity, score identity,
  * finite differences, scipy truncnorm/truncexpon, Gaussian closed-form MLE, the printed
  * constants of Listing 4, closed-form angular marginals, hand-evaluated points of Eq. 4.
- * The analytic Hessian at the end of the file (mass and angular kinds) has its own pins
+ * The analytic Hessian at the end of the file (all three kinds) has its own pins
  * (tests/test_oracle_hessian.py): finite differences of the pinned gradient and the information identity.
+ * Weighted sums and the Fisher matrix of weighted fits (reading R23: -ln L_w = -sum w_i ln P_i; covariance
+ * H^-1 F H^-1 with F = sum w_i^2 s_i s_i^T) are pinned there too: unit weights reproduce the unweighted sums bit for
+ * bit, integer weights equal event duplication, the sums rebuilt from the pinned per-event quantities, the closed
+ * forms of a weighted Gaussian (MLE, H, F, sandwich), invariance under a rescaling of the weights, unit pull width.
  */
 #include <math.h>
 #include <stddef.h>
@@ -268,8 +272,9 @@ void mfo_angular_terms(double cl, double ck, double phi, double *out /*[11]*/)
     for (int j = 0; j < 11; ++j) out[j] *= 9.0 / (32.0 * MFO_PI);
 }
 
-static void chunk_sums(int kind, const double *const *cols, int64_t i0, int64_t i1, const double *lam,
-                       double lo, double hi, int K, int want_grad, long double *acc /*[K+1]*/, int64_t *nbad)
+static void chunk_sums(int kind, const double *const *cols, const double *w /* event weights or NULL (= 1) */, int64_t i0,
+                       int64_t i1, const double *lam, double lo, double hi, int K, int want_grad,
+                       long double *acc /*[K+1]*/, int64_t *nbad)
 {
     for (int k = 0; k <= K; ++k) acc[k] = 0.0L;
     int64_t bad = 0;
@@ -277,9 +282,10 @@ static void chunk_sums(int kind, const double *const *cols, int64_t i0, int64_t 
         double g[MFO_MAXK];
         const double P = eval_event(kind, cols, i, lam, lo, hi, want_grad ? g : NULL);
         if (!(P > 0.0)) { ++bad; continue; }
-        acc[0] += (long double)log(P);
+        const long double wi = w ? (long double)w[i] : 1.0L; /* times 1.0L is exact: the unweighted sums are unchanged */
+        acc[0] += wi * (long double)log(P);
         if (want_grad)
-            for (int k = 0; k < K; ++k) acc[1 + k] += (long double)g[k];
+            for (int k = 0; k < K; ++k) acc[1 + k] += wi * (long double)g[k];
     }
     *nbad = bad;
 }
@@ -289,8 +295,23 @@ static void chunk_sums(int kind, const double *const *cols, int64_t i0, int64_t 
  * grad may be NULL.  Returns the number of events with P <= 0 or NaN (then *nll = +inf,
  * grad = NaN), or -1 on a bad argument.
  */
+int64_t mfo_nll_grad_w(int kind, int64_t n, const double *const *cols, const double *w, const double *lam, double lo,
+                       double hi, int nthreads, double *nll, double *grad);
+
 int64_t mfo_nll_grad(int kind, int64_t n, const double *const *cols, const double *lam, double lo,
                      double hi, int nthreads, double *nll, double *grad)
+{
+    return mfo_nll_grad_w(kind, n, cols, NULL, lam, lo, hi, nthreads, nll, grad);
+}
+
+/*
+ * The same with event weights w_i ("weighted fits"; reading R23):
+ *     -ln L_w(lambda) = - sum_i w_i ln P(x_i | lambda),   gradient likewise.
+ * w == NULL means w_i = 1 (bit-identical to the unweighted sums).  Weights may be negative (sWeights); an event
+ * with P <= 0 is counted as bad whatever its weight.
+ */
+int64_t mfo_nll_grad_w(int kind, int64_t n, const double *const *cols, const double *w, const double *lam, double lo,
+                       double hi, int nthreads, double *nll, double *grad)
 {
     const int K = mfo_nparams(kind);
     if (K < 0 || n < 0) return -1;
@@ -304,7 +325,7 @@ int64_t mfo_nll_grad(int kind, int64_t n, const double *const *cols, const doubl
 #endif
     for (int c = 0; c < nthreads; ++c) {
         const int64_t i0 = n * c / nthreads, i1 = n * (c + 1) / nthreads;
-        chunk_sums(kind, cols, i0, i1, lam, lo, hi, K, want_grad, part[c], &bad[c]);
+        chunk_sums(kind, cols, w, i0, i1, lam, lo, hi, K, want_grad, part[c], &bad[c]);
     }
     long double tot[MFO_MAXK + 1];
     int64_t nbad = 0;
@@ -412,7 +433,8 @@ int mfo_mass_hess_points(int64_t n, const double *m, const double *lam, double l
  * -ln L, its gradient and its Hessian (row-major K x K, symmetric) over n events, for the mass (K = 4) and
  * angular (K = 8) kinds.  Angular: P = A is linear in its coefficients, so d2 ln P / da db = -A_a A_b / A^2.
  * Sums in long double, single pass in event order.  Returns the number of events with P <= 0 (then nll = +inf,
- * everything else NaN), -1 on a bad argument (including the 4D kind, for which no analytic Hessian is defined here).
+ * everything else NaN), -1 on a bad argument (including the 4D kind: its Hessian is reached through
+ * mfo_nll_grad_hess_w below, which with w = NULL returns for the mass and angular kinds exactly what this routine does).
  */
 int64_t mfo_nll_grad_hess(int kind, int64_t n, const double *const *cols, const double *lam, double lo, double hi,
                           double *nll, double *grad, double *hess)
@@ -455,5 +477,192 @@ int64_t mfo_nll_grad_hess(int kind, int64_t n, const double *const *cols, const 
     *nll = (double)(-s0);
     for (int i = 0; i < K; ++i) grad[i] = (double)(-sg[i]);
     for (int i = 0; i < K * K; ++i) hess[i] = (double)(-sh[i]);
+    return 0;
+}
+
+/* ================================================================================================
+ * 4D model: second derivatives, again through the derivatives of P:
+ *     P = f s(m; mu, sigma) A(Omega; a) + (1 - f) b(m; tau) L(Omega; c),   d2 ln P / dx dy = P_xy / P - P_x P_y / P^2.
+ * A is linear in its eight coefficients and L = l(cos theta_l; cl1, cl2) l(cos theta_K; ck1, ck2) / (2 pi) is linear in
+ * each Legendre coefficient, so the only non-zero second derivatives of P are
+ *     (f, x) for every other x;  (mu|sigma, mu|sigma);  (mu|sigma, a_k);  (tau, tau);  (tau, c);  (cl_i, ck_j).
+ * Pins (tests/test_oracle_hessian.py): Richardson central differences of the pinned gradient, and the information
+ * identity  int P (l_xy + l_x l_y) dm dOmega = 0  for all 136 pairs on the quadrature grid of test_oracle_4d.py.
+ * ================================================================================================ */
+
+/* s = G/N1, b = e^{tau m}/N2 and their first and second parameter derivatives for one mass value
+ * (the same formulas as in mass_event_hess, collected for the 4D model). */
+typedef struct {
+    double s, s_m, s_s, s_mm, s_ms, s_ss; /* signal shape and its (mu, sigma) derivatives */
+    double b, b_t, b_tt;                  /* background shape and its tau derivatives */
+} mass_parts;
+
+static void mass_shape_derivs(double m, double mu, double sigma, double tau, double a, double b, mass_parts *o)
+{
+    const double s2 = sigma * sigma, s3 = s2 * sigma, s4 = s2 * s2;
+    const double d = m - mu;
+    const double N1 = norm_gauss(mu, sigma, a, b);
+    const double ga = gauss_density(a, mu, sigma), gb = gauss_density(b, mu, sigma);
+    const double da = a - mu, db = b - mu;
+    const double N1_m = ga - gb;
+    const double N1_s = (da * ga - db * gb) / sigma;
+    const double ga_s = ga * (da * da / s3 - 1.0 / sigma), gb_s = gb * (db * db / s3 - 1.0 / sigma);
+    const double N1_mm = ga * da / s2 - gb * db / s2;
+    const double N1_ms = ga_s - gb_s;
+    const double N1_ss = (da * ga_s - db * gb_s) / sigma - (da * ga - db * gb) / s2;
+    const double s = gauss_density(m, mu, sigma) / N1;
+    const double al_m = d / s2 - N1_m / N1;
+    const double al_s = d * d / s3 - 1.0 / sigma - N1_s / N1;
+    const double al_mm = -1.0 / s2 - (N1_mm / N1 - (N1_m / N1) * (N1_m / N1));
+    const double al_ms = -2.0 * d / s3 - (N1_ms / N1 - (N1_m / N1) * (N1_s / N1));
+    const double al_ss = -3.0 * d * d / s4 + 1.0 / s2 - (N1_ss / N1 - (N1_s / N1) * (N1_s / N1));
+    o->s = s;
+    o->s_m = s * al_m;
+    o->s_s = s * al_s;
+    o->s_mm = s * (al_m * al_m + al_mm);
+    o->s_ms = s * (al_m * al_s + al_ms);
+    o->s_ss = s * (al_s * al_s + al_ss);
+    const double bb = exp(tau * m) / norm_exp(tau, a, b);
+    const double be = m - dlognorm_exp_dtau(tau, a, b);
+    o->b = bb;
+    o->b_t = bb * be;
+    o->b_tt = bb * (be * be - d2lognorm_exp_dtau2(tau, a, b));
+}
+
+/* P, g[16] = d ln P / d lambda, H[16][16] = d2 ln P / d lambda^2 (full, symmetric) for one 4D event.
+ * lambda = (f, mu, sigma, tau, FL..S9, cl1, cl2, ck1, ck2). */
+static double fourd_event_hess(double m, double cl, double ck, double phi, const double *lam, double a, double b,
+                               double *g, double *H)
+{
+    const double f = lam[0], mu = lam[1], sigma = lam[2], tau = lam[3];
+    const double cl1 = lam[12], cl2 = lam[13], ck1 = lam[14], ck2 = lam[15];
+    mass_parts q;
+    mass_shape_derivs(m, mu, sigma, tau, a, b, &q);
+    double dA[8];
+    const double A = angular_value(cl, ck, phi, lam + 4, dA);
+    const double Ll = legendre2(cl, cl1, cl2), Lk = legendre2(ck, ck1, ck2);
+    const double twopi = 2.0 * MFO_PI;
+    const double L = Ll * Lk / twopi;
+    /* dl/dc1 = x/2, dl/dc2 = (3x^2 - 1)/4 */
+    const double dLl[2] = {0.5 * cl, 0.5 * 0.5 * (3.0 * cl * cl - 1.0)};
+    const double dLk[2] = {0.5 * ck, 0.5 * 0.5 * (3.0 * ck * ck - 1.0)};
+    const double dL[4] = {dLl[0] * Lk / twopi, dLl[1] * Lk / twopi, Ll * dLk[0] / twopi, Ll * dLk[1] / twopi};
+    const double P = f * q.s * A + (1.0 - f) * q.b * L;
+    double P1[16], P2[16][16];
+    for (int i = 0; i < 16; ++i)
+        for (int j = 0; j < 16; ++j) P2[i][j] = 0.0;
+    P1[0] = q.s * A - q.b * L;
+    P1[1] = f * q.s_m * A;
+    P1[2] = f * q.s_s * A;
+    P1[3] = (1.0 - f) * q.b_t * L;
+    for (int k = 0; k < 8; ++k) P1[4 + k] = f * q.s * dA[k];
+    for (int k = 0; k < 4; ++k) P1[12 + k] = (1.0 - f) * q.b * dL[k];
+    /* row f */
+    P2[0][1] = q.s_m * A;
+    P2[0][2] = q.s_s * A;
+    P2[0][3] = -q.b_t * L;
+    for (int k = 0; k < 8; ++k) P2[0][4 + k] = q.s * dA[k];
+    for (int k = 0; k < 4; ++k) P2[0][12 + k] = -q.b * dL[k];
+    /* (mu, sigma) block and its couplings to the angular coefficients */
+    P2[1][1] = f * q.s_mm * A;
+    P2[1][2] = f * q.s_ms * A;
+    P2[2][2] = f * q.s_ss * A;
+    for (int k = 0; k < 8; ++k) {
+        P2[1][4 + k] = f * q.s_m * dA[k];
+        P2[2][4 + k] = f * q.s_s * dA[k];
+    }
+    /* tau and the Legendre coefficients */
+    P2[3][3] = (1.0 - f) * q.b_tt * L;
+    for (int k = 0; k < 4; ++k) P2[3][12 + k] = (1.0 - f) * q.b_t * dL[k];
+    for (int i = 0; i < 2; ++i)
+        for (int j = 0; j < 2; ++j) P2[12 + i][14 + j] = (1.0 - f) * q.b * dLl[i] * dLk[j] / twopi;
+    for (int i = 0; i < 16; ++i)
+        for (int j = 0; j < i; ++j) P2[i][j] = P2[j][i];
+    for (int i = 0; i < 16; ++i) g[i] = P1[i] / P;
+    for (int i = 0; i < 16; ++i)
+        for (int j = 0; j < 16; ++j) H[i * 16 + j] = P2[i][j] / P - (P1[i] / P) * (P1[j] / P);
+    return P;
+}
+
+/* P, gradient and full Hessian of ln P for one event of any kind (g[K], H[K*K]). */
+static double event_hess(int kind, const double *const *cols, int64_t e, const double *lam, double lo, double hi, double *g,
+                         double *H)
+{
+    if (kind == MFO_MASS) {
+        double h[10];
+        const double P = mass_event_hess(cols[0][e], lam, lo, hi, g, h);
+        int q = 0;
+        for (int i = 0; i < 4; ++i)
+            for (int j = i; j < 4; ++j, ++q) H[i * 4 + j] = H[j * 4 + i] = h[q];
+        return P;
+    }
+    if (kind == MFO_ANGULAR) {
+        double dA[8];
+        const double P = angular_value(cols[0][e], cols[1][e], cols[2][e], lam, dA);
+        for (int i = 0; i < 8; ++i) g[i] = dA[i] / P;
+        for (int i = 0; i < 8; ++i)
+            for (int j = 0; j < 8; ++j) H[i * 8 + j] = -(dA[i] / P) * (dA[j] / P);
+        return P;
+    }
+    return fourd_event_hess(cols[0][e], cols[1][e], cols[2][e], cols[3][e], lam, lo, hi, g, H);
+}
+
+/* exposed for the quadrature pins: per-event P [n], d ln P [n][K], d2 ln P [n][K][K] */
+int mfo_hess_points(int kind, int64_t n, const double *const *cols, const double *lam, double lo, double hi, double *P,
+                    double *g, double *H)
+{
+    const int K = mfo_nparams(kind);
+    if (K < 0) return -1;
+    for (int64_t e = 0; e < n; ++e) P[e] = event_hess(kind, cols, e, lam, lo, hi, g + e * K, H + e * K * K);
+    return 0;
+}
+
+/*
+ * Weighted second-order sums for every kind ("the Fisher information matrix can be
+ * calculated analytically, which is required for weighted fits [22]"; reading R23):
+ *     -ln L_w = - sum_i w_i ln P_i
+ *     grad    = - sum_i w_i  d ln P_i / d lambda
+ *     hess    = - sum_i w_i  d2 ln P_i / d lambda^2                 (K x K, may be NULL)
+ *     fisher  =   sum_i w_i^2 (d ln P_i/d lambda)(d ln P_i/d lambda)^T   (K x K, may be NULL)
+ * The covariance of a weighted fit is  hess^-1 fisher hess^-1  at the minimum (the sandwich of [22]); for w_i = 1 its
+ * expectation equals hess^-1.  w == NULL means w_i = 1: hess is then what mfo_nll_grad_hess returns, bit for bit, and
+ * this is also the only route to the 4D Hessian.  Sums in long double, one pass in event order.
+ * Returns the number of events with P <= 0 (then nll = +inf, everything else NaN), -1 on a bad argument.
+ */
+int64_t mfo_nll_grad_hess_w(int kind, int64_t n, const double *const *cols, const double *w, const double *lam, double lo,
+                            double hi, double *nll, double *grad, double *hess, double *fisher)
+{
+    const int K = mfo_nparams(kind);
+    if (K < 0 || n < 0) return -1;
+    long double s0 = 0.0L, sg[MFO_MAXK], sh[MFO_MAXK * MFO_MAXK], sf[MFO_MAXK * MFO_MAXK];
+    for (int i = 0; i < K; ++i) sg[i] = 0.0L;
+    for (int i = 0; i < K * K; ++i) sh[i] = sf[i] = 0.0L;
+    int64_t bad = 0;
+    for (int64_t e = 0; e < n; ++e) {
+        double g[MFO_MAXK], H[MFO_MAXK * MFO_MAXK];
+        const double P = event_hess(kind, cols, e, lam, lo, hi, g, H);
+        if (!(P > 0.0)) { ++bad; continue; }
+        const long double wi = w ? (long double)w[e] : 1.0L;
+        s0 += wi * (long double)log(P);
+        for (int i = 0; i < K; ++i) sg[i] += wi * (long double)g[i];
+        for (int i = 0; i < K * K; ++i) sh[i] += wi * (long double)H[i];
+        for (int i = 0; i < K; ++i)
+            for (int j = 0; j < K; ++j) sf[i * K + j] += wi * wi * (long double)(g[i] * g[j]);
+    }
+    if (bad) {
+        *nll = INFINITY;
+        for (int i = 0; i < K; ++i) grad[i] = NAN;
+        for (int i = 0; i < K * K; ++i) {
+            if (hess) hess[i] = NAN;
+            if (fisher) fisher[i] = NAN;
+        }
+        return bad;
+    }
+    *nll = (double)(-s0);
+    for (int i = 0; i < K; ++i) grad[i] = (double)(-sg[i]);
+    for (int i = 0; i < K * K; ++i) {
+        if (hess) hess[i] = (double)(-sh[i]);
+        if (fisher) fisher[i] = (double)sf[i];
+    }
     return 0;
 }
