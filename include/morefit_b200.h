@@ -100,6 +100,13 @@ int64_t mf_ctx_kernel_launches(const mf_ctx* ctx);
 mf_status mf_dataset_upload(mf_ctx* ctx, int ndim, int64_t n_events, int64_t n_toys,
                             const double* const* columns, mf_mem where,
                             const double* lo, const double* hi, mf_dataset** out);
+/* Event weights ("weighted fits"; reading R23): models created on the dataset
+ * AFTER this call evaluate  -ln L_w = -sum_i w_i ln P(x_i | lambda)  (gradient and Hessian likewise) and mf_fit returns the
+ * sandwich covariance H^-1 F H^-1 with F = sum_i w_i^2 s_i s_i^T (mf_nll_grad_hess_fisher).
+ *   weights   n_events doubles in `where` memory (copied; any sign, e.g. sWeights), or NULL: back to unweighted.
+ * Only datasets with n_toys == 1.  MF_ERR_DATA_RANGE if a weight is NaN/inf.  Weighted models are evaluated by the
+ * second-order kernels (one launch pair per parameter point); the batched-toy entry points do not take weights. */
+mf_status mf_dataset_set_weights(mf_dataset* ds, const double* weights, mf_mem where);
 void mf_dataset_destroy(mf_dataset* ds);
 int64_t mf_dataset_n_events(const mf_dataset* ds);
 int64_t mf_dataset_n_toys(const mf_dataset* ds);
@@ -201,15 +208,27 @@ mf_status mf_nll_grad_batch_async(mf_model* model, int64_t n_toys, const double*
 
 /* ---- value + gradient + analytic Hessian ---------------------- */
 
-/* 1 if the model family has the analytic Hessian kernel (MF_MASS_GAUSS_EXP, MF_ANGULAR_KSTMUMU), else 0
- * (MF_MASS_X_ANGULAR: the fit driver then uses finite differences of the gradient). */
+/* 1 if the analytic Hessian is available for this model: every family on a single dataset (n_toys == 1); with
+ * n_toys > 1 (mf_nll_grad_hess_batch) the mass and angular families (the fit driver then uses finite differences of the
+ * gradient for batched 4D toys). */
 int mf_model_has_hessian(const mf_model* model);
+/* 1 if the model was created on a dataset with event weights. */
+int mf_model_is_weighted(const mf_model* model);
 
-/* As mf_nll_grad, plus hess (host, K*K doubles, row-major, symmetric) = d2(-ln L)/d lambda_k d lambda_l, from one
- * launch that accumulates the second-derivative sums beside the value and the gradient (mass: seven more moment sums;
- * angular: the 36 products of the score components).
- * MF_ERR_ARG for a model family without the Hessian kernel; on MF_NONPOSITIVE_PDF hess is NaN. */
+/* As mf_nll_grad, plus hess (host, K*K doubles, row-major, symmetric) = d2(-ln L)/d lambda_k d lambda_l from the same
+ * pass over the data.  Unweighted mass and angular models: one launch that accumulates the second-derivative sums in
+ * registers (mass: seven more moment sums; angular: the 36 products of the score components).  The 4D model (136
+ * second-derivative sums) and every weighted model: the second-order kernel, which forms S^T diag(w) S and the
+ * P_ab / P terms as fp64 tensor-core contractions over the event index (mf_second.cuh).
+ * On MF_NONPOSITIVE_PDF hess is NaN. */
 mf_status mf_nll_grad_hess(mf_model* model, const double* lambda, double* nll, double* grad, double* hess);
+
+/* As mf_nll_grad_hess, plus fisher (host, K*K, row-major, symmetric) = sum_i w_i^2 s_i s_i^T with s_i = d ln P_i/d lambda
+ * (w_i = 1 without weights): the matrix PAPER.md:53 calls the Fisher information matrix "required for weighted fits";
+ * the covariance of a weighted fit is hess^-1 fisher hess^-1 at the minimum (reading R23).  Any model family,
+ * n_toys == 1; hess may be NULL.  One launch pair (second-order kernel + combine). */
+mf_status mf_nll_grad_hess_fisher(mf_model* model, const double* lambda, double* nll, double* grad, double* hess,
+                                  double* fisher);
 
 /* As mf_nll_grad_batch, plus hess (host, [n_toys][K*K]); inactive toys are left untouched. */
 mf_status mf_nll_grad_hess_batch(mf_model* model, int64_t n_toys, const double* lambdas, const uint8_t* active,
@@ -237,7 +256,8 @@ void mf_fit_opts_default(mf_fit_opts* opts);
 
 typedef struct {
     double lambda_hat[MF_MAX_PARAMS];               /* fitted parameters (fixed ones = start) */
-    double cov[MF_MAX_PARAMS * MF_MAX_PARAMS];      /* row-major K x K inverse Hessian (HESSE); 0 for fixed */
+    double cov[MF_MAX_PARAMS * MF_MAX_PARAMS];      /* row-major K x K inverse Hessian (HESSE); 0 for fixed.
+                                                       Weighted model: the sandwich H^-1 F H^-1 (reading R23) */
     double nll_min;
     int n_calls;                                    /* value+gradient evaluations used */
     int n_iter;                                     /* BFGS iterations */
@@ -246,7 +266,7 @@ typedef struct {
 
 /* Minimises -ln L from `start` (host, K).  fixed: host, K bytes (1 = keep at start; paper:
  * the parameter `constant` flag) or NULL.  opts NULL = defaults.
- * With the analytic Hessian (opts->analytic_hessian, mass model): Newton steps with Armijo backtracking on the
+ * With the analytic Hessian (opts->analytic_hessian, every family with n_toys == 1): Newton steps with Armijo backtracking on the
  * Hessian returned by every evaluation, then Newton polish; cov = H^-1 at the minimum.
  * Otherwise (SURVEY.md §8(c) "Fit"): central-difference Hessian of the analytic gradient
  * at the start point seeds the inverse metric; BFGS with Armijo backtracking that rejects

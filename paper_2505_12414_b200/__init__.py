@@ -32,10 +32,10 @@ _STATUS_NAMES = ["MF_OK", "MF_ERR_ARG", "MF_ERR_CUDA", "MF_ERR_OOM", "MF_ERR_DAT
 
 EXPORTS = [
     "mf_ctx_create", "mf_ctx_destroy", "mf_last_error", "mf_ctx_kernel_launches",
-    "mf_dataset_upload", "mf_generate_mass", "mf_generate_angular", "mf_generate_4d", "mf_dataset_download", "mf_dataset_destroy", "mf_dataset_n_events", "mf_dataset_n_toys",
+    "mf_dataset_upload", "mf_generate_mass", "mf_generate_angular", "mf_generate_4d", "mf_dataset_download", "mf_dataset_set_weights", "mf_dataset_destroy", "mf_dataset_n_events", "mf_dataset_n_toys",
     "mf_model_create", "mf_model_destroy", "mf_model_nparams", "mf_model_n_events", "mf_model_n_toys",
     "mf_nll_grad", "mf_nll_grad_async", "mf_nll_grad_points", "mf_nll_grad_sweep", "mf_nll_grad_batch", "mf_nll_grad_batch_async",
-    "mf_model_has_hessian", "mf_nll_grad_hess", "mf_nll_grad_hess_batch",
+    "mf_model_has_hessian", "mf_model_is_weighted", "mf_nll_grad_hess", "mf_nll_grad_hess_fisher", "mf_nll_grad_hess_batch",
     "mf_fit_opts_default", "mf_fit", "mf_fit_batch", "mf_toy_study_mass",
     "mf_combine_partials",
 ]
@@ -148,6 +148,8 @@ def load_library() -> ctypes.CDLL:
     lib.mf_generate_4d.argtypes = [vp, ctypes.c_uint64, i64, i64, dp, ctypes.c_double, ctypes.c_double, ctypes.POINTER(vp)]
     lib.mf_dataset_download.restype = ctypes.c_int
     lib.mf_dataset_download.argtypes = [vp, dp]
+    lib.mf_dataset_set_weights.restype = ctypes.c_int
+    lib.mf_dataset_set_weights.argtypes = [vp, vp, ctypes.c_int]
     lib.mf_dataset_destroy.restype = None
     lib.mf_dataset_destroy.argtypes = [vp]
     lib.mf_dataset_n_events.restype = i64
@@ -178,6 +180,10 @@ def load_library() -> ctypes.CDLL:
     lib.mf_model_has_hessian.argtypes = [vp]
     lib.mf_nll_grad_hess.restype = ctypes.c_int
     lib.mf_nll_grad_hess.argtypes = [vp, dp, dp, dp, dp]
+    lib.mf_model_is_weighted.restype = ctypes.c_int
+    lib.mf_model_is_weighted.argtypes = [vp]
+    lib.mf_nll_grad_hess_fisher.restype = ctypes.c_int
+    lib.mf_nll_grad_hess_fisher.argtypes = [vp, dp, dp, dp, dp, dp]
     lib.mf_nll_grad_hess_batch.restype = ctypes.c_int
     lib.mf_nll_grad_hess_batch.argtypes = [vp, i64, dp, u8p, dp, dp, dp]
     lib.mf_fit_opts_default.restype = None
@@ -360,6 +366,16 @@ class Dataset:
         ctx._children.add(self)
         self.ndim, self.n_events, self.n_toys = ndim, total // n_toys, int(n_toys)
 
+    def set_weights(self, weights) -> None:
+        """Event weights (host array of n_events doubles, or None for unweighted); models created afterwards are weighted."""
+        if weights is None:
+            self._ctx._check(self._lib.mf_dataset_set_weights(self._h, None, MF_HOST))
+            return
+        w = np.ascontiguousarray(weights, dtype=np.float64)
+        if w.shape != (self.n_events,):
+            raise ValueError(f"weights must have shape ({self.n_events},)")
+        self._ctx._check(self._lib.mf_dataset_set_weights(self._h, ctypes.c_void_p(w.ctypes.data), MF_HOST))
+
     def download(self) -> np.ndarray:
         """The events as a host array [ndim][n_toys][n_events]."""
         out = np.empty((self.ndim, self.n_toys, self.n_events), dtype=np.float64)
@@ -457,6 +473,20 @@ class Model:
         hess = np.empty((self.K, self.K))
         self._ctx._check(self._lib.mf_nll_grad_hess(self._h, _dp(lam), ctypes.byref(nll), _dp(grad), _dp(hess)))
         return float(nll.value), grad, hess
+
+    @property
+    def weighted(self) -> bool:
+        return bool(self._lib.mf_model_is_weighted(self._h))
+
+    def nll_grad_hess_fisher(self, lam):
+        """(-ln L, gradient [K], Hessian [K][K], Fisher matrix sum w^2 s s^T [K][K]) from one pass (tensor-core contraction)."""
+        lam = np.ascontiguousarray(lam, dtype=np.float64)
+        nll = ctypes.c_double()
+        grad = np.empty(self.K)
+        hess = np.empty((self.K, self.K))
+        fisher = np.empty((self.K, self.K))
+        self._ctx._check(self._lib.mf_nll_grad_hess_fisher(self._h, _dp(lam), ctypes.byref(nll), _dp(grad), _dp(hess), _dp(fisher)))
+        return float(nll.value), grad, hess, fisher
 
     def nll_grad_hess_batch(self, lambdas, active=None):
         """lambdas [T][K] -> (nll [T], grad [T][K], hess [T][K][K]); inactive toys are NaN."""

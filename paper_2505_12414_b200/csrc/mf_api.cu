@@ -15,6 +15,7 @@
 
 #include "mf_internal.h"
 #include "mf_kernels.cuh"
+#include "mf_second.cuh"
 
 using namespace mf;
 
@@ -263,8 +264,59 @@ extern "C" void mf_dataset_destroy(mf_dataset* ds)
 {
     if (!ds) return;
     devbuf_release(ds->raw);
+    devbuf_release(ds->wts);
     delete ds;
 }
+// Event weights (reading R23): one more device column, padding 0.
+extern "C" mf_status mf_dataset_set_weights(mf_dataset* ds, const double* weights, mf_mem where)
+{
+    if (!ds) return MF_ERR_ARG;
+    mf_ctx* ctx = ds->ctx;
+    if (ds->n_toys != 1) return mf_fail(ctx, MF_ERR_ARG, "mf_dataset_set_weights: weighted datasets must have n_toys == 1");
+    MF_CUDA(ctx, cudaSetDevice(ctx->device));
+    if (!weights) {  // back to unweighted (models created before keep their weights)
+        devbuf_release(ds->wts);
+        ds->wts = nullptr;
+        return MF_OK;
+    }
+    mf_devbuf* buf = new (std::nothrow) mf_devbuf();
+    if (!buf) return mf_fail(ctx, MF_ERR_OOM, "mf_dataset_set_weights: host allocation failed");
+    buf->stream = ctx->stream;
+    buf->bytes = (size_t)std::max<int64_t>(ds->n_pad, 1) * sizeof(double);
+    unsigned long long* d_count = nullptr;
+    unsigned long long n_out = 0;
+    cudaError_t e = dev_alloc(ctx, &buf->p, buf->bytes);
+    if (e == cudaSuccess) e = dev_alloc(ctx, &d_count, sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemsetAsync(d_count, 0, sizeof(unsigned long long), ctx->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(buf->p, 0, buf->bytes, ctx->stream);
+    if (e == cudaSuccess && ds->n_events > 0) {
+        e = cudaMemcpyAsync(buf->p, weights, sizeof(double) * ds->n_events,
+                            where == MF_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, ctx->stream);
+        if (e == cudaSuccess) {
+            const int grid = (int)std::min<int64_t>((ds->n_events + 255) / 256, 8 * (int64_t)ctx->sm_count);
+            range_check_kernel<<<grid, 256, 0, ctx->stream>>>(buf->p, 1, ds->n_events, ds->n_pad, -1.7976931348623157e308,
+                                                              1.7976931348623157e308, d_count);  // finite, any sign
+            ++ctx->launches;
+            e = cudaGetLastError();
+        }
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&n_out, d_count, sizeof(n_out), cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (d_count) cudaFreeAsync(d_count, ctx->stream);
+    if (e != cudaSuccess) {
+        devbuf_release(buf);
+        return mf_fail(ctx, e == cudaErrorMemoryAllocation ? MF_ERR_OOM : MF_ERR_CUDA,
+                       std::string("mf_dataset_set_weights: ") + cudaGetErrorString(e));
+    }
+    if (n_out) {
+        devbuf_release(buf);
+        return mf_fail(ctx, MF_ERR_DATA_RANGE, "mf_dataset_set_weights: " + std::to_string(n_out) + " weights are not finite");
+    }
+    devbuf_release(ds->wts);
+    ds->wts = buf;
+    return MF_OK;
+}
+
 extern "C" int64_t mf_dataset_n_events(const mf_dataset* ds) { return ds ? ds->n_events : 0; }
 extern "C" int64_t mf_dataset_n_toys(const mf_dataset* ds) { return ds ? ds->n_toys : 0; }
 
@@ -290,8 +342,14 @@ extern "C" void mf_model_destroy(mf_model* m)
     dev_free(m->ctx, m->d_ids);
     dev_free(m->ctx, m->d_bout);
     dev_free(m->ctx, m->d_sweep);
+    dev_free(m->ctx, m->s_partials);
+    dev_free(m->ctx, m->s_bad);
+    dev_free(m->ctx, m->s_sums);
+    dev_free(m->ctx, m->s_ticket);
+    dev_free(m->ctx, m->s_out);
     host_slot_release(m->ctx, m->h_out);
     devbuf_release(m->raw);
+    devbuf_release(m->wts);
     cudaGetLastError();
     delete m;
 }
@@ -323,6 +381,8 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
     m->mb = ds->hi[0];
     m->raw = ds->raw;
     ++m->raw->refs;
+    m->wts = ds->wts;
+    if (m->wts) ++m->wts->refs;
 #define MF_CUDA_M(call)                                                                               \
     do {                                                                                              \
         cudaError_t e__ = (call);                                                                     \
@@ -530,13 +590,139 @@ static mf_status launch_single(mf_model* m, const double* lam, double* out_dev, 
     return MF_OK;
 }
 
+
+// ---- second-order sums by tensor-core contraction (mf_second.cuh): weighted models, the 4D Hessian, the Fisher matrix ----
+
+template <class S>
+static bool second_consts(const mf_model* m, const double* lam, typename S::Consts& c);
+template <>
+bool second_consts<MassSecond>(const mf_model* m, const double* lam, MassConsts& c)
+{
+    return mass_consts(lam, m->ma, m->mb, c);
+}
+template <>
+bool second_consts<AngularSecond>(const mf_model*, const double* lam, AngularConsts& c)
+{
+    return angular_consts(lam, c);
+}
+template <>
+bool second_consts<FourDSecond>(const mf_model* m, const double* lam, FourDConsts& c)
+{
+    return fourd_consts(lam, m->ma, m->mb, c);
+}
+
+// grow-only pinned staging block of the context (shared with the batched calls; every user is synchronous)
+static mf_status stage_reserve(mf_ctx* ctx, size_t bytes)
+{
+    if (ctx->h_stage_bytes >= bytes) return MF_OK;
+    if (ctx->h_stage) {
+        cudaStreamSynchronize(ctx->stream);
+        cudaFreeHost(ctx->h_stage);
+        ctx->h_stage = nullptr;
+        ctx->h_stage_bytes = 0;
+    }
+    MF_CUDA(ctx, cudaHostAlloc(reinterpret_cast<void**>(&ctx->h_stage), bytes, cudaHostAllocDefault));
+    ctx->h_stage_bytes = bytes;
+    return MF_OK;
+}
+
+// MODE 0: -ln L and gradient; 1: + Hessian; 2: + Fisher matrix sum w^2 s s^T.  out_dev NULL = the model's own buffer.
+// Output row: -ln L, gradient [K], Hessian upper triangle row by row [K(K+1)/2], Fisher likewise, n_bad.
+template <class S, int MODE>
+static mf_status launch_second(mf_model* m, const double* lam, double* out_dev)
+{
+    using L = SecondLayout<S, MODE>;
+    using LW = SecondLayout<S, 2>;  // scratch is sized for the widest mode
+    mf_ctx* ctx = m->ctx;
+    SecondArgs<S> a;
+    if (!second_consts<S>(m, lam, a.c)) return mf_fail(ctx, MF_ERR_PARAM_DOMAIN, "lambda outside the parameter domain");
+    if (!m->s_partials) {
+        const int64_t n_tiles = (m->n_pad + kBlock - 1) / kBlock;
+        m->s_grid = (int)std::max<int64_t>(1, std::min<int64_t>(n_tiles, ctx->sm_count));
+        MF_CUDA(ctx, dev_alloc(ctx, &m->s_partials, sizeof(double) * LW::NQ * m->s_grid));
+        MF_CUDA(ctx, dev_alloc(ctx, &m->s_bad, sizeof(unsigned) * m->s_grid));
+        MF_CUDA(ctx, dev_alloc(ctx, &m->s_sums, sizeof(double) * LW::NQ));
+        MF_CUDA(ctx, dev_alloc(ctx, &m->s_ticket, sizeof(unsigned)));
+        MF_CUDA(ctx, cudaMemsetAsync(m->s_ticket, 0, sizeof(unsigned), ctx->stream));
+        MF_CUDA(ctx, dev_alloc(ctx, &m->s_out, sizeof(double) * (LW::NOUT + 1)));
+    }
+    for (int i = 0; i < S::NCOL; ++i) a.col[i] = m->col[i];
+    a.w = m->wts ? m->wts->p : nullptr;
+    a.n = m->n_events;
+    a.n_pad = m->n_pad;
+    a.partials = m->s_partials;
+    a.bad_partials = m->s_bad;
+    static const cudaError_t attr_set = cudaFuncSetAttribute(nll_second_kernel<S, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                             (int)L::smem_bytes());
+    MF_CUDA(ctx, attr_set);
+    take_fresh(m);  // plain stream order: these launches never overlap their predecessors
+    nll_second_kernel<S, MODE><<<m->s_grid, kBlock, L::smem_bytes(), ctx->stream>>>(a);
+    SecondCombineArgs<S> cb;
+    cb.partials = m->s_partials;
+    cb.bad_partials = m->s_bad;
+    cb.G = m->s_grid;
+    cb.sums = m->s_sums;
+    cb.ticket = m->s_ticket;
+    cb.c = a.c;
+    cb.out = out_dev ? out_dev : m->s_out;
+    second_combine_kernel<S, MODE><<<(L::NQ + kWarps - 1) / kWarps, kBlock, 0, ctx->stream>>>(cb);
+    MF_CUDA(ctx, cudaGetLastError());
+    ctx->launches += 2;
+    return MF_OK;
+}
+
+template <int MODE>
+static mf_status dispatch_second(mf_model* m, const double* lam, double* out_dev)
+{
+    switch (m->kind) {
+    case MF_MASS_GAUSS_EXP: return launch_second<MassSecond, MODE>(m, lam, out_dev);
+    case MF_ANGULAR_KSTMUMU: return launch_second<AngularSecond, MODE>(m, lam, out_dev);
+    default: return launch_second<FourDSecond, MODE>(m, lam, out_dev);
+    }
+}
+
+// Synchronous second-order evaluation; hess / fisher (host, K x K, row-major, symmetric) may be NULL.
+static mf_status second_sync(mf_model* m, const double* lambda, double* nll, double* grad, double* hess, double* fisher,
+                             const char* who)
+{
+    mf_ctx* ctx = m->ctx;
+    const int K = m->K, NH = K * (K + 1) / 2;
+    const int mode = fisher ? 2 : hess ? 1 : 0;
+    const mf_status st = mode == 2 ? dispatch_second<2>(m, lambda, nullptr) : mode == 1 ? dispatch_second<1>(m, lambda, nullptr)
+                                                                                       : dispatch_second<0>(m, lambda, nullptr);
+    if (st != MF_OK) return st;
+    const int nout = 1 + K + (mode >= 1 ? NH : 0) + (mode >= 2 ? NH : 0);
+    const mf_status sr = stage_reserve(ctx, sizeof(double) * (nout + 1));
+    if (sr != MF_OK) return sr;
+    double* h = reinterpret_cast<double*>(ctx->h_stage);
+    MF_CUDA(ctx, cudaMemcpyAsync(h, m->s_out, sizeof(double) * (nout + 1), cudaMemcpyDeviceToHost, ctx->stream));
+    MF_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    *nll = h[0];
+    if (grad) std::memcpy(grad, h + 1, sizeof(double) * K);
+    int q = 1 + K;
+    if (mode >= 1)
+        for (int i = 0; i < K; ++i)
+            for (int j = i; j < K; ++j, ++q)
+                if (hess) hess[i * K + j] = hess[j * K + i] = h[q];
+    if (mode >= 2)
+        for (int i = 0; i < K; ++i)
+            for (int j = i; j < K; ++j, ++q) fisher[i * K + j] = fisher[j * K + i] = h[q];
+    if (h[nout] != 0.0)
+        return mf_fail(ctx, MF_NONPOSITIVE_PDF,
+                       std::string(who) + ": P <= 0 for " + std::to_string((long long)h[nout]) + " events at this lambda");
+    return MF_OK;
+}
+
+// true where an evaluation goes through the second-order kernels: weighted models, and the Hessian of the 4D model
+static bool uses_second(const mf_model* m, bool hess) { return m->wts != nullptr || (hess && m->kind == MF_MASS_X_ANGULAR); }
+
 static mf_status dispatch_single(mf_model* m, const double* lam, double* out_dev, bool pipelined = false,
                                  bool signal_host = false, bool hess = false)
 {
     if (hess) {
         if (m->kind == MF_MASS_GAUSS_EXP) return launch_single<MassHessModel>(m, lam, out_dev, pipelined, signal_host);
         if (m->kind == MF_ANGULAR_KSTMUMU) return launch_single<AngularHessModel>(m, lam, out_dev, false, signal_host);
-        return mf_fail(m->ctx, MF_ERR_ARG, "no analytic Hessian kernel for this model family (MF_MASS_X_ANGULAR)");
+        return mf_fail(m->ctx, MF_ERR_ARG, "internal: the 4D Hessian goes through the second-order kernel");
     }
     switch (m->kind) {
     case MF_MASS_GAUSS_EXP: return launch_single<MassModel>(m, lam, out_dev, pipelined, signal_host);
@@ -549,6 +735,7 @@ extern "C" mf_status mf_nll_grad_async(mf_model* m, const double* lambda, double
 {
     if (!m || !lambda || !out_dev) return mf_fail(m ? m->ctx : nullptr, MF_ERR_ARG, "mf_nll_grad_async: NULL argument");
     if (m->n_toys != 1) return mf_fail(m->ctx, MF_ERR_ARG, "mf_nll_grad_async: dataset has n_toys != 1; use mf_nll_grad_batch");
+    if (uses_second(m, false)) return dispatch_second<0>(m, lambda, out_dev);
     return dispatch_single(m, lambda, out_dev);
 }
 
@@ -665,6 +852,13 @@ extern "C" mf_status mf_nll_grad_points(mf_model* m, int64_t n_points, const dou
         return mf_fail(m ? m->ctx : nullptr, MF_ERR_ARG, "mf_nll_grad_points: bad argument");
     if (m->n_toys != 1) return mf_fail(m->ctx, MF_ERR_ARG, "mf_nll_grad_points: dataset has n_toys != 1");
     if (n_points == 0) return MF_OK;
+    if (uses_second(m, false)) {  // weighted: one second-order evaluation (gradient mode) per point, in stream order
+        for (int64_t p = 0; p < n_points; ++p) {
+            const mf_status st = dispatch_second<0>(m, lambdas + p * m->K, out_dev + p * (m->K + 2));
+            if (st != MF_OK) return st;
+        }
+        return MF_OK;
+    }
     if (n_points < 16) {  // few points: back-to-back pipelined single evaluations are faster (measured cross-over ~12)
         for (int64_t p = 0; p < n_points; ++p) {
             const mf_status st = dispatch_single(m, lambdas + p * m->K, out_dev + p * (m->K + 2), n_points > 1);
@@ -763,6 +957,7 @@ extern "C" mf_status mf_nll_grad(mf_model* m, const double* lambda, double* nll,
 {
     if (!m || !lambda || !nll) return mf_fail(m ? m->ctx : nullptr, MF_ERR_ARG, "mf_nll_grad: NULL argument");
     if (m->n_toys != 1) return mf_fail(m->ctx, MF_ERR_ARG, "mf_nll_grad: dataset has n_toys != 1; use mf_nll_grad_batch");
+    if (uses_second(m, false)) return second_sync(m, lambda, nll, grad, nullptr, nullptr, "mf_nll_grad");
     return eval_sync(m, lambda, nll, grad, nullptr, "mf_nll_grad");
 }
 
@@ -770,13 +965,27 @@ extern "C" mf_status mf_nll_grad_hess(mf_model* m, const double* lambda, double*
 {
     if (!m || !lambda || !nll || !hess) return mf_fail(m ? m->ctx : nullptr, MF_ERR_ARG, "mf_nll_grad_hess: NULL argument");
     if (m->n_toys != 1) return mf_fail(m->ctx, MF_ERR_ARG, "mf_nll_grad_hess: dataset has n_toys != 1; use mf_nll_grad_hess_batch");
+    if (uses_second(m, true)) return second_sync(m, lambda, nll, grad, hess, nullptr, "mf_nll_grad_hess");
     return eval_sync(m, lambda, nll, grad, hess, "mf_nll_grad_hess");
 }
 
+extern "C" mf_status mf_nll_grad_hess_fisher(mf_model* m, const double* lambda, double* nll, double* grad, double* hess,
+                                             double* fisher)
+{
+    if (!m || !lambda || !nll || !fisher)
+        return mf_fail(m ? m->ctx : nullptr, MF_ERR_ARG, "mf_nll_grad_hess_fisher: NULL argument");
+    if (m->n_toys != 1) return mf_fail(m->ctx, MF_ERR_ARG, "mf_nll_grad_hess_fisher: dataset has n_toys != 1");
+    return second_sync(m, lambda, nll, grad, hess, fisher, "mf_nll_grad_hess_fisher");
+}
+
+// 1: mf_nll_grad_hess is available (every family on a single dataset; batched toys: mass and angular families)
 extern "C" int mf_model_has_hessian(const mf_model* m)
 {
-    return m && (m->kind == MF_MASS_GAUSS_EXP || m->kind == MF_ANGULAR_KSTMUMU) ? 1 : 0;
+    if (!m) return 0;
+    return (m->n_toys == 1 || m->kind == MF_MASS_GAUSS_EXP || m->kind == MF_ANGULAR_KSTMUMU) ? 1 : 0;
 }
+
+extern "C" int mf_model_is_weighted(const mf_model* m) { return m && m->wts ? 1 : 0; }
 
 template <class M>
 static mf_status launch_batch(mf_model* m, int n_active, const double* lam_dev = nullptr, double* out_dev = nullptr)
@@ -829,12 +1038,13 @@ static mf_status eval_batch(mf_model* m, int64_t n_toys, const double* lambdas, 
     const int K = m->K;
     if (n_toys != m->n_toys) return mf_fail(ctx, MF_ERR_ARG, std::string(who) + ": n_toys does not match the dataset");
     if (hess && !mf_model_has_hessian(m))
-        return mf_fail(ctx, MF_ERR_ARG, "no analytic Hessian kernel for this model family (MF_MASS_X_ANGULAR)");
+        return mf_fail(ctx, MF_ERR_ARG, "no batched analytic Hessian kernel for this model family (MF_MASS_X_ANGULAR)");
     if (m->n_toys < 2 && !m->d_lam) {
         // a 1-toy dataset evaluated through the batch entry: same result as the single call
         if (active && !active[0]) return MF_OK;
         double g[MF_MAX_PARAMS];
-        const mf_status st = eval_sync(m, lambdas, nll, g, hess, who);
+        const mf_status st = uses_second(m, hess != nullptr) ? second_sync(m, lambdas, nll, g, hess, nullptr, who)
+                                                             : eval_sync(m, lambdas, nll, g, hess, who);
         if (st == MF_ERR_PARAM_DOMAIN || st == MF_NONPOSITIVE_PDF) {
             *nll = INFINITY;
             if (grad) for (int k = 0; k < K; ++k) grad[k] = NAN;

@@ -462,6 +462,29 @@ static mf_status fit_one(mf_model* m, const double* start, const uint8_t* fixed,
     }
     st.result(result);
     if (st.failed_start()) return mf_fail(m->ctx, first == MF_OK ? MF_NONPOSITIVE_PDF : first, "mf_fit: invalid start point");
+    if (mf_model_is_weighted(m)) {
+        // weighted fit: cov = H^-1 F H^-1 with F = sum_i w_i^2 s_i s_i^T at the minimum (reading R23);
+        // result->cov holds H^-1 over the free parameters (zero rows / columns for the fixed ones)
+        const int K = m->K;
+        double f = 0, g[KM], F[KM * KM];
+        const mf_status rc = mf_nll_grad_hess_fisher(m, result->lambda_hat, &f, g, nullptr, F);
+        if (rc != MF_OK) return rc;
+        double T[KM * KM], C[KM * KM];
+        for (int i = 0; i < K; ++i)
+            for (int j = 0; j < K; ++j) {
+                double s = 0.0;
+                for (int k = 0; k < K; ++k) s += result->cov[i * K + k] * F[k * K + j];
+                T[i * K + j] = s;
+            }
+        for (int i = 0; i < K; ++i)
+            for (int j = 0; j < K; ++j) {
+                double s = 0.0;
+                for (int k = 0; k < K; ++k) s += T[i * K + k] * result->cov[k * K + j];
+                C[i * K + j] = s;
+            }
+        for (int i = 0; i < K; ++i)
+            for (int j = 0; j <= i; ++j) result->cov[i * K + j] = result->cov[j * K + i] = 0.5 * (C[i * K + j] + C[j * K + i]);
+    }
     return MF_OK;
 }
 
@@ -486,7 +509,7 @@ static mf_status fit_many(mf_model* m, int64_t n_toys, const double* starts, con
     std::vector<FitStateT<KM>> st((size_t)n_toys);
     std::vector<double> lam((size_t)n_toys * K), nll((size_t)n_toys), grad((size_t)n_toys * K);
     std::vector<uint8_t> active((size_t)n_toys);
-    const bool analytic = o.analytic_hessian != 0 && mf_model_has_hessian(m);
+    const bool analytic = o.analytic_hessian != 0 && mf_model_has_hessian(m);  // n_toys > 1: mass and angular families
     std::vector<double> hess(analytic ? (size_t)n_toys * K * K : 0);
     // the T fit states are independent: their host-side updates run on all cores (static schedule; the results do not
     // depend on the thread count)

@@ -57,6 +57,7 @@ struct mf_dataset {
     int64_t n_toys = 1;
     double lo[MF_MAX_DIMS] = {0, 0, 0, 0}, hi[MF_MAX_DIMS] = {0, 0, 0, 0};
     mf_devbuf* raw = nullptr;  // [ndim][n_toys][n_pad]
+    mf_devbuf* wts = nullptr;  // [n_pad] event weights (padding 0), or NULL: unweighted (mf_dataset_set_weights)
 };
 
 constexpr int MF_MAX_COLS = 12;
@@ -97,6 +98,14 @@ struct mf_model {
     int bout_row = 0;                 // widest output row + n_bad (doubles)
     double* d_sweep = nullptr;        // device [p_sweep_rows][K+2] results of mf_nll_grad_sweep (grow-only)
     int64_t p_sweep_rows = 0;
+    // second-order sums by tensor-core contraction (mf_second.cuh): weighted models, the 4D Hessian, the Fisher matrix
+    mf_devbuf* wts = nullptr;         // shared with the dataset; NULL = unweighted
+    int s_grid = 0;                   // CTAs of nll_second_kernel
+    double* s_partials = nullptr;     // device [NQ of the widest mode][s_grid]
+    unsigned* s_bad = nullptr;        // device [s_grid]
+    double* s_sums = nullptr;         // device [NQ]
+    unsigned* s_ticket = nullptr;     // device, one word, zero between launches
+    double* s_out = nullptr;          // device [NOUT + 1] of the widest mode
 };
 
 // Sets ctx->err and returns st (mf_api.cu).

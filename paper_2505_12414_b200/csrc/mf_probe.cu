@@ -30,6 +30,39 @@ __global__ void __launch_bounds__(256) dfma_chain_kernel(double* out, int iters,
     if (s == 123.456) out[0] = s;  // never true for these inputs; keeps the chains alive
 }
 
+// fp64 tensor-core rate (DMMA m8n8k4) and whether it shares the issue rate of the vector fp64 pipe: N_MMA independent
+// accumulator tiles and N_FMA independent DFMA chains per warp and iteration (either may be 0).
+__device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+template <int N_MMA, int N_FMA>
+__global__ void __launch_bounds__(256) dmma_mix_kernel(double* out, int iters, double a, double b)
+{
+    double c[8][2], x[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        c[i][0] = threadIdx.x + i;
+        c[i][1] = threadIdx.x - i;
+        x[i] = threadIdx.x + 0.5 * i;
+    }
+#pragma unroll 1
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+#pragma unroll
+            for (int i = 0; i < N_MMA; ++i) dmma(c[i][0], c[i][1], a, b);
+#pragma unroll
+            for (int i = 0; i < N_FMA; ++i) x[i] = fma(x[i], a, b);
+        }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += c[i][0] + c[i][1] + x[i];
+    if (s == 123.456) out[0] = s;
+}
+
 __global__ void __launch_bounds__(256) read_kernel(const double2* __restrict__ p, size_t n_vec, int repeats, double* out)
 {
     double s = 0.0;
@@ -108,6 +141,50 @@ extern "C" int mfp_fp64_rate(int device, void* stream, double* dfma_per_second)
     cudaEventDestroy(e1);
     cudaFree(d_out);
     *dfma_per_second = best;
+    return 0;
+}
+
+template <int N_MMA, int N_FMA>
+static int time_mix(ProbeCtx* ctx, double* d_out, double* seconds)
+{
+    cudaEvent_t e0, e1;
+    MF_CUDA(ctx, cudaEventCreate(&e0));
+    MF_CUDA(ctx, cudaEventCreate(&e1));
+    const int grid = ctx->sm_count * 4, iters = 2048;
+    double best = 1e30;
+    for (int rep = 0; rep < 5; ++rep) {
+        MF_CUDA(ctx, cudaEventRecord(e0, ctx->stream));
+        dmma_mix_kernel<N_MMA, N_FMA><<<grid, 256, 0, ctx->stream>>>(d_out, iters, 0.999999, 1e-9);
+        MF_CUDA(ctx, cudaEventRecord(e1, ctx->stream));
+        MF_CUDA(ctx, cudaEventSynchronize(e1));
+        float ms = 0;
+        MF_CUDA(ctx, cudaEventElapsedTime(&ms, e0, e1));
+        if (rep > 0 && ms * 1e-3 < best) best = ms * 1e-3;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    *seconds = best;
+    return 0;
+}
+
+extern "C" int mfp_dmma_rate(int device, void* stream, double* out4)
+{
+    if (!out4) return (int)cudaErrorInvalidValue;
+    ProbeCtx pc, *ctx = &pc;
+    if (const int e = probe_ctx(device, stream, ctx)) return e;
+    double* d_out = nullptr;
+    MF_CUDA(ctx, cudaMalloc(&d_out, sizeof(double)));
+    const double warps = (double)ctx->sm_count * 4 * 8, steps = 2048.0 * 4;
+    double t_mma = 0, t_fma = 0, t_both = 0, t_both2 = 0;
+    if (const int e = time_mix<4, 0>(ctx, d_out, &t_mma)) return e;
+    if (const int e = time_mix<0, 8>(ctx, d_out, &t_fma)) return e;
+    if (const int e = time_mix<4, 8>(ctx, d_out, &t_both)) return e;
+    if (const int e = time_mix<1, 8>(ctx, d_out, &t_both2)) return e;
+    cudaFree(d_out);
+    out4[0] = warps * steps * 4 * 256.0 / t_mma;        // DMMA alone: fp64 FMAs per second (m8n8k4 = 256 FMAs)
+    out4[1] = warps * steps * 8 * 32.0 / t_fma;         // DFMA alone: FMAs per second
+    out4[2] = t_both / (t_mma + t_fma);                 // 4 DMMA + 8 DFMA: 1.0 = the two serialise, max/sum = they overlap fully
+    out4[3] = t_both2 / (t_fma + 0.25 * t_mma);         // 1 DMMA + 8 DFMA
     return 0;
 }
 

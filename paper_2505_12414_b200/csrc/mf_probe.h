@@ -11,6 +11,10 @@ extern "C" {
 /* fp64-pipe issue rate of the GPU in DFMA thread-instructions per second, measured with register-only DFMA chains
  * (nominal B200: 148 SMs x 64 lanes x 1.965 GHz = 1.86e13). */
 int mfp_fp64_rate(int device, void* stream, double* dfma_per_second);
+/* fp64 tensor-core (DMMA m8n8k4) rate: out4[0] = fp64 FMAs per second with DMMA alone, out4[1] = with DFMA alone,
+ * out4[2] = time(4 DMMA + 8 DFMA per step) / (time of each alone, added): 1.0 means the two serialise,
+ * out4[3] = the same for 1 DMMA + 8 DFMA per step. */
+int mfp_dmma_rate(int device, void* stream, double* out4);
 /* Read bandwidth in bytes/s of a `bytes`-sized device buffer that one kernel reads `repeats` times with 16-byte loads:
  * L2 bandwidth when bytes fits the L2 and repeats > 1, HBM otherwise. */
 int mfp_read_bandwidth(int device, void* stream, size_t bytes, int repeats, double* bytes_per_second);

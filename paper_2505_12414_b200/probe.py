@@ -24,6 +24,8 @@ def _load() -> ctypes.CDLL:
         dp, vp = ctypes.POINTER(ctypes.c_double), ctypes.c_void_p
         lib.mfp_fp64_rate.restype = ctypes.c_int
         lib.mfp_fp64_rate.argtypes = [ctypes.c_int, vp, dp]
+        lib.mfp_dmma_rate.restype = ctypes.c_int
+        lib.mfp_dmma_rate.argtypes = [ctypes.c_int, vp, dp]
         lib.mfp_read_bandwidth.restype = ctypes.c_int
         lib.mfp_read_bandwidth.argtypes = [ctypes.c_int, vp, ctypes.c_size_t, ctypes.c_int, dp]
         lib.mfp_math.restype = ctypes.c_int
@@ -42,6 +44,13 @@ def fp64_rate(device: int = 0, stream: int = 0) -> float:
     v = ctypes.c_double()
     _check(_load().mfp_fp64_rate(int(device), ctypes.c_void_p(stream), ctypes.byref(v)), "mfp_fp64_rate")
     return float(v.value)
+
+
+def dmma_rate(device: int = 0, stream: int = 0) -> dict:
+    """fp64 tensor-core rate against the vector fp64 pipe (see mf_probe.h)."""
+    out = (ctypes.c_double * 4)()
+    _check(_load().mfp_dmma_rate(int(device), ctypes.c_void_p(stream), out), "mfp_dmma_rate")
+    return {"dmma_fma_per_s": out[0], "dfma_fma_per_s": out[1], "mix_4dmma_8dfma_vs_sum": out[2], "mix_1dmma_8dfma_vs_sum": out[3]}
 
 
 def read_bandwidth(nbytes: int, repeats: int = 1, device: int = 0, stream: int = 0) -> float:

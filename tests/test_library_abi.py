@@ -65,7 +65,7 @@ def test_probe_library_is_separate(lib):
     text = open(os.path.join(ROOT, "paper_2505_12414_b200", "csrc", "mf_probe.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     names = sorted(set(re.findall(r"\b(mfp_[a-z0-9_]+)\s*\(", text)))
-    assert names == ["mfp_fp64_rate", "mfp_math", "mfp_read_bandwidth"]
+    assert names == ["mfp_dmma_rate", "mfp_fp64_rate", "mfp_math", "mfp_read_bandwidth"]
     probe = ctypes.CDLL(build.PROBE_LIB_PATH)
     for n in names:
         assert hasattr(probe, n) and not hasattr(lib, n)
