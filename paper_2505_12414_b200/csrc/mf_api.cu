@@ -637,8 +637,8 @@ static mf_status launch_second(mf_model* m, const double* lam, double* out_dev)
     SecondArgs<S> a;
     if (!second_consts<S>(m, lam, a.c)) return mf_fail(ctx, MF_ERR_PARAM_DOMAIN, "lambda outside the parameter domain");
     if (!m->s_partials) {
-        const int64_t n_tiles = (m->n_pad + kBlock - 1) / kBlock;
-        m->s_grid = (int)std::max<int64_t>(1, std::min<int64_t>(n_tiles, ctx->sm_count));
+        const int64_t n_cta_items = (m->n_pad / kSecondItem + 11) / 12;  // at least one item per warp of the smallest CTA
+        m->s_grid = (int)std::max<int64_t>(1, std::min<int64_t>(n_cta_items, ctx->sm_count));
         MF_CUDA(ctx, dev_alloc(ctx, &m->s_partials, sizeof(double) * LW::NQ * m->s_grid));
         MF_CUDA(ctx, dev_alloc(ctx, &m->s_bad, sizeof(unsigned) * m->s_grid));
         MF_CUDA(ctx, dev_alloc(ctx, &m->s_sums, sizeof(double) * LW::NQ));
@@ -656,7 +656,7 @@ static mf_status launch_second(mf_model* m, const double* lam, double* out_dev)
                                                              (int)L::smem_bytes());
     MF_CUDA(ctx, attr_set);
     take_fresh(m);  // plain stream order: these launches never overlap their predecessors
-    nll_second_kernel<S, MODE><<<m->s_grid, kBlock, L::smem_bytes(), ctx->stream>>>(a);
+    nll_second_kernel<S, MODE><<<m->s_grid, L::THREADS, L::smem_bytes(), ctx->stream>>>(a);
     SecondCombineArgs<S> cb;
     cb.partials = m->s_partials;
     cb.bad_partials = m->s_bad;

@@ -20,7 +20,7 @@
 //   X[8]      X_0 = 1, then event-only quantities.
 // Tile sums (each an 8 x 8 tile of doubles):
 //   XY[tj]      = sum_i w_i X_r(i) Y_{8 tj + c}(i)                      (row 0: the weighted gradient sums)
-//   YY[ti<=tj]  = sum_i w_i Y_{8 ti + r}(i) Y_{8 tj + c}(i)             (MODE >= 1)
+//   YY[ti<=tj]  = sum_i w_i Y_{8 ti + r}(i) Y_{8 tj + c}(i)             (MODE >= 1; score tiles only: 8 ti, 8 tj < K)
 //   FF[ti<=tj]  = the same with w_i^2                                  (MODE == 2)
 // plus the plain per-thread sum of w_i ln D_i.  S::finish turns the combined sums into the outputs.
 #pragma once
@@ -35,8 +35,8 @@ __device__ __forceinline__ void dmma_m8n8k4(double& c0, double& c1, double a, do
                  : "d"(a), "d"(b));
 }
 
-constexpr int kSecondStages = 3;
 constexpr int kSecondRow = 36;  // doubles per row of the per-warp vector buffer: 32 events + 4 (conflict-free fragment reads)
+constexpr int kSecondItem = 32;  // events per warp item: one per lane
 
 template <class S>
 struct SecondArgs {
@@ -50,72 +50,45 @@ struct SecondArgs {
 
 template <class S, int MODE>
 struct SecondLayout {
-    static constexpr int NT = S::NY / 8;
-    static constexpr int NYY = NT * (NT + 1) / 2;
+    static constexpr int NT = S::NY / 8;          // Y tiles (scores, then helpers)
+    static constexpr int NTK = (S::K + 7) / 8;    // Y tiles that hold scores: only their products enter YY and FF
+    static constexpr int NYY = NTK * (NTK + 1) / 2;
     static constexpr int NTILES = NT + (MODE >= 1 ? NYY : 0) + (MODE >= 2 ? NYY : 0);
     static constexpr int NQ = 1 + 64 * NTILES;  // quantity 0: sum w ln D
     static constexpr int NV = 8 + S::NY + 1;    // X, Y, w
     static constexpr int K = S::K;
     static constexpr int NH = K * (K + 1) / 2;
     static constexpr int NOUT = 1 + K + (MODE >= 1 ? NH : 0) + (MODE >= 2 ? NH : 0);  // n_bad follows at [NOUT]
+    // CTA size: 16 warps where the register budget allows (128 per thread), else 12; one CTA per SM
+    static constexpr int THREADS = (S::NY > 8 && MODE >= 2) ? 384 : 512;
+    static constexpr int WARPS = THREADS / 32;
     __host__ __device__ static constexpr int yy_tile(int ti, int tj)  // ti <= tj, row-major upper triangle
     {
-        return ti * NT - ti * (ti - 1) / 2 + (tj - ti);
+        return ti * NTK - ti * (ti - 1) / 2 + (tj - ti);
     }
-    static constexpr size_t smem_bytes()
-    {
-        return sizeof(double) * ((size_t)kSecondStages * (S::NCOL + 1) * kBlock + (size_t)kWarps * NV * kSecondRow) +
-               sizeof(double2) * kLogTableSize + sizeof(unsigned long long) * kSecondStages;
-    }
+    static constexpr size_t smem_bytes() { return sizeof(double) * (size_t)WARPS * NV * kSecondRow + sizeof(double2) * kLogTableSize; }
 };
 
+// Warps are independent: a warp item is 32 consecutive events, one per lane, read with one coalesced 256-byte load per
+// column; items are dealt block-cyclically over all warps of the grid; the next item's lines are requested from L2 while
+// the current one is evaluated.  No CTA-wide barrier inside the event loop.
 template <class S, int MODE>
-__global__ void __launch_bounds__(kBlock, 1) nll_second_kernel(const __grid_constant__ SecondArgs<S> a)
+__global__ void __launch_bounds__(SecondLayout<S, MODE>::THREADS, 1) nll_second_kernel(const __grid_constant__ SecondArgs<S> a)
 {
     using L = SecondLayout<S, MODE>;
-    constexpr int NC = S::NCOL + 1, TILE = kBlock, STAGES = kSecondStages, NT = L::NT, NYY = L::NYY, NV = L::NV, RS = kSecondRow;
+    constexpr int NT = L::NT, NTK = L::NTK, NYY = L::NYY, NV = L::NV, RS = kSecondRow, WARPS = L::WARPS, THREADS = L::THREADS;
     extern __shared__ __align__(128) unsigned char sec_raw[];
-    double (*buf)[NC][TILE] = reinterpret_cast<double (*)[NC][TILE]>(sec_raw);
-    double (*sv)[NV][RS] = reinterpret_cast<double (*)[NV][RS]>(sec_raw + sizeof(double) * STAGES * NC * TILE);
-    double2* s_tab = reinterpret_cast<double2*>(sec_raw + sizeof(double) * (STAGES * NC * TILE + kWarps * NV * RS));
-    unsigned long long* bar = reinterpret_cast<unsigned long long*>(s_tab + kLogTableSize);
-    __shared__ double s_w0[kWarps];
-    __shared__ unsigned s_wbad[kWarps];
+    double (*sv)[NV][RS] = reinterpret_cast<double (*)[NV][RS]>(sec_raw);
+    double2* s_tab = reinterpret_cast<double2*>(sec_raw + sizeof(double) * WARPS * NV * RS);
+    __shared__ double s_w0[WARPS];
+    __shared__ unsigned s_wbad[WARPS];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int fg = lane >> 2, ft = lane & 3;  // fragment coordinates: row / column group and event within the group of four
     const bool weighted = a.w != nullptr;
-    const int ncopy = weighted ? NC : NC - 1;
-    const int64_t n_pad = a.n_pad, n_tiles = (n_pad + TILE - 1) / TILE, G = gridDim.x;
-    if (tid == 0) {
-#pragma unroll
-        for (int s = 0; s < STAGES; ++s)
-            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"((unsigned)__cvta_generic_to_shared(&bar[s])));
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
+    const int64_t n_items = a.n_pad / kSecondItem, G = gridDim.x;
     load_log_table(s_tab);
     __syncthreads();
-    auto issue = [&](int s, int64_t tile) {  // thread 0: arm stage s with tile `tile`
-        const int64_t first = tile * TILE;
-        const unsigned len = (unsigned)((n_pad - first < TILE) ? (n_pad - first) : TILE);  // multiple of 64 events
-        const unsigned bytes = len * (unsigned)sizeof(double);
-        const unsigned mb = (unsigned)__cvta_generic_to_shared(&bar[s]);
-        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mb), "r"(bytes * ncopy) : "memory");
-#pragma unroll
-        for (int c = 0; c < NC; ++c) {
-            const double* src = (c < S::NCOL) ? a.col[c < S::NCOL ? c : 0] : a.w;
-            if (c < ncopy)
-                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                                 (unsigned)__cvta_generic_to_shared(&buf[s][c][0])),
-                             "l"(src + first), "r"(bytes), "r"(mb)
-                             : "memory");
-        }
-    };
-    if (tid == 0) {
-#pragma unroll
-        for (int s = 0; s < STAGES; ++s)
-            if (blockIdx.x + s * G < n_tiles) issue(s, blockIdx.x + s * G);
-    }
     double cxy[NT][2], cyy[MODE >= 1 ? NYY : 1][2], cff[MODE >= 2 ? NYY : 1][2];
 #pragma unroll
     for (int i = 0; i < NT; ++i) cxy[i][0] = cxy[i][1] = 0.0;
@@ -126,27 +99,19 @@ __global__ void __launch_bounds__(kBlock, 1) nll_second_kernel(const __grid_cons
     double acc0 = 0.0;
     unsigned bad = 0;
     const double t_lane = mf_exp32_lane_entry();
-    int it = 0;
-    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += G, ++it) {
-        const int s = it % STAGES;
-        const unsigned phase = (unsigned)(it / STAGES) & 1u, mb = (unsigned)__cvta_generic_to_shared(&bar[s]);
-        unsigned done = 0;
-        while (!done)
-            asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
-                         : "=r"(done)
-                         : "r"(mb), "r"(phase)
-                         : "memory");
-        const int64_t e = tile * TILE + tid;
-        const bool valid = e < a.n;
+    const int64_t step = G * WARPS;
+    for (int64_t item = blockIdx.x + G * warp; item < n_items; item += step) {
+        const int64_t e = item * kSecondItem + lane;
         double x[S::NCOL], wgt = 1.0;
-        if (e < n_pad) {
 #pragma unroll
-            for (int c = 0; c < S::NCOL; ++c) x[c] = buf[s][c][tid];
-            if (weighted) wgt = buf[s][NC - 1][tid];
-        } else {
-#pragma unroll
-            for (int c = 0; c < S::NCOL; ++c) x[c] = S::kPadValue;  // beyond the padded columns: any valid event value, weight 0
+        for (int c = 0; c < S::NCOL; ++c) x[c] = __ldg(a.col[c] + e);
+        if (weighted) wgt = __ldg(a.w + e);
+        if (item + step < n_items) {  // next item of this warp: 256 bytes per column = two lines
+            const int64_t en = (item + step) * kSecondItem;
+            if (lane < 2 * S::NCOL) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.col[lane >> 1] + en + 16 * (lane & 1)));
+            if (weighted && lane >= 30) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.w + en + 16 * (lane & 1)));
         }
+        const bool valid = e < a.n;
         if (!valid) wgt = 0.0;
         {
             double X[8], Y[S::NY];
@@ -163,7 +128,7 @@ __global__ void __launch_bounds__(kBlock, 1) nll_second_kernel(const __grid_cons
         }
         __syncwarp();
         // the warp's 32 events, four per DMMA: lane (fg, ft) supplies row / column fg of event ft of the group
-#pragma unroll 2
+#pragma unroll
         for (int q = 0; q < 8; ++q) {
             const int ev = 4 * q + ft;
             const double wv = sv[warp][NV - 1][ev];
@@ -175,23 +140,22 @@ __global__ void __launch_bounds__(kBlock, 1) nll_second_kernel(const __grid_cons
             for (int tj = 0; tj < NT; ++tj) dmma_m8n8k4(cxy[tj][0], cxy[tj][1], xa, y[tj]);
             if constexpr (MODE >= 1) {
 #pragma unroll
-                for (int ti = 0; ti < NT; ++ti) {
+                for (int ti = 0; ti < NTK; ++ti) {
                     const double ya = y[ti] * wv;
 #pragma unroll
-                    for (int tj = ti; tj < NT; ++tj) dmma_m8n8k4(cyy[L::yy_tile(ti, tj)][0], cyy[L::yy_tile(ti, tj)][1], ya, y[tj]);
+                    for (int tj = ti; tj < NTK; ++tj) dmma_m8n8k4(cyy[L::yy_tile(ti, tj)][0], cyy[L::yy_tile(ti, tj)][1], ya, y[tj]);
                     if constexpr (MODE >= 2) {
                         const double yaa = ya * wv;
 #pragma unroll
-                        for (int tj = ti; tj < NT; ++tj) dmma_m8n8k4(cff[L::yy_tile(ti, tj)][0], cff[L::yy_tile(ti, tj)][1], yaa, y[tj]);
+                        for (int tj = ti; tj < NTK; ++tj) dmma_m8n8k4(cff[L::yy_tile(ti, tj)][0], cff[L::yy_tile(ti, tj)][1], yaa, y[tj]);
                     }
                 }
             }
         }
-        __syncthreads();  // the whole CTA has consumed stage s (and every warp its vector buffer)
-        if (tid == 0 && tile + STAGES * G < n_tiles) issue(s, tile + STAGES * G);
+        __syncwarp();  // every lane has read the vectors before the next item overwrites them
     }
     // ---- warp -> block: tile accumulators through the (now free) vector buffers, summed in warp order
-    static_assert(sizeof(double) * 64 * L::NTILES <= sizeof(double) * NV * RS, "a warp's tiles fit its vector buffer");
+    static_assert(64 * L::NTILES <= NV * RS, "a warp's tiles fit its vector buffer");
     double* red = &sv[warp][0][0];  // [NTILES][64], element (row, col) of a tile at 8 row + col = 2 lane + {0, 1}
 #pragma unroll
     for (int i = 0; i < NT; ++i) {
@@ -220,17 +184,17 @@ __global__ void __launch_bounds__(kBlock, 1) nll_second_kernel(const __grid_cons
         s_wbad[warp] = bad;
     }
     __syncthreads();
-    for (int q = tid; q < 64 * L::NTILES; q += kBlock) {
+    for (int q = tid; q < 64 * L::NTILES; q += THREADS) {
         double s = 0.0;
 #pragma unroll
-        for (int w = 0; w < kWarps; ++w) s += (&sv[w][0][0])[q];
+        for (int w = 0; w < WARPS; ++w) s += (&sv[w][0][0])[q];
         a.partials[(int64_t)(1 + q) * G + blockIdx.x] = s;
     }
     if (tid == 0) {
         double s = 0.0;
         unsigned b = 0;
 #pragma unroll
-        for (int w = 0; w < kWarps; ++w) {
+        for (int w = 0; w < WARPS; ++w) {
             s += s_w0[w];
             b += s_wbad[w];
         }
@@ -373,7 +337,6 @@ __device__ __forceinline__ void second_out_index(int o, int& kind, int& a, int& 
 // Helpers: Y4 = u, Y5 = r, Y6 = 1.  X = (1, d, d^2, d^3, d^4).
 struct MassSecond {
     static constexpr int K = 4, NCOL = 1, NY = 8;
-    static constexpr double kPadValue = 0.0;
     using Consts = MassConsts;
     static MF_D double vectors(const double* x, const Consts& c, double* X, double* Y, double t_lane)
     {
@@ -436,7 +399,6 @@ struct MassSecond {
 // Angular model: P linear in its coefficients, y_k = h_{k+1} / P = s_k, no second derivatives of P.
 struct AngularSecond {
     static constexpr int K = 8, NCOL = 9, NY = 8;
-    static constexpr double kPadValue = 1.0;
     using Consts = AngularConsts;
     static MF_D double vectors(const double* x, const Consts& c, double* X, double* Y, double)
     {
@@ -471,7 +433,6 @@ struct AngularSecond {
 // Helpers: Y16 = us, Y17 = ub, Y18 = qq cl, Y19 = qq p2l, Y20 = 1.  X = (1, d, d^2, d^3, d^4, ck, p2k).
 struct FourDSecond {
     static constexpr int K = 16, NCOL = 12, NY = 24;
-    static constexpr double kPadValue = 1.0;
     using Consts = FourDConsts;
     static MF_D double vectors(const double* x, const Consts& c, double* X, double* Y, double t_lane)
     {
