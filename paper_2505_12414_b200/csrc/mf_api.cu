@@ -16,6 +16,7 @@
 #include "mf_internal.h"
 #include "mf_kernels.cuh"
 #include "mf_second.cuh"
+#include "mf_points.cuh"
 
 using namespace mf;
 
@@ -768,6 +769,82 @@ static cudaError_t points_stage(mf_ctx* ctx, size_t bytes, char** h, int* stage)
     return cudaSuccess;
 }
 
+// Device scratch of the many-points evaluations, [consts | ok | partials | bad | ticket], grow-only, laid out for the largest
+// (points, chunks) seen so far; ok flags non-zero (every point is validated on the host), tickets zero (the kernels leave
+// them at zero).
+static mf_status points_scratch(mf_ctx* ctx, int64_t n_points, int chunks)
+{
+    auto up = [](size_t x) { return (x + 255) / 256 * 256; };
+    if (n_points > ctx->p_points || chunks > ctx->p_chunks || !ctx->p_blk) {
+        const int64_t P = std::max<int64_t>(n_points, ctx->p_points);
+        const int C = std::max(chunks, ctx->p_chunks);
+        const size_t bytes = up(sizeof(FourDConsts) * P) + up(sizeof(int) * P) + up(sizeof(double) * P * MF_MAX_NACC * C) +
+                             up(sizeof(unsigned) * P * C) + up(sizeof(unsigned) * P);
+        dev_free(ctx, ctx->p_blk);  // stream-ordered: after the launches that still use it
+        ctx->p_blk = nullptr;
+        ctx->p_points = 0;
+        ctx->p_chunks = 0;
+        MF_CUDA(ctx, dev_alloc(ctx, &ctx->p_blk, bytes));
+        ctx->p_bytes = bytes;
+        ctx->p_points = P;
+        ctx->p_chunks = C;
+        MF_CUDA(ctx, cudaMemsetAsync(ctx->p_blk + up(sizeof(FourDConsts) * P), 0xFF, up(sizeof(int) * P), ctx->stream));
+        MF_CUDA(ctx, cudaMemsetAsync(ctx->p_blk + bytes - up(sizeof(unsigned) * P), 0, up(sizeof(unsigned) * P), ctx->stream));
+    }
+    return MF_OK;
+}
+
+// The angular model's many-points evaluation as two tensor-core contractions (mf_points.cuh): one pass over the data per
+// 64 points.  out_dev rows are K + 2 = 10 doubles.
+static mf_status launch_points_angular_mma(mf_model* m, int64_t n_points, const double* lambdas, double* out_dev)
+{
+    mf_ctx* ctx = m->ctx;
+    for (int64_t i = 0; i < n_points * 8; ++i)
+        if (!std::isfinite(lambdas[i]))
+            return mf_fail(ctx, MF_ERR_PARAM_DOMAIN, "mf_nll_grad_points: lambda " + std::to_string((long long)(i / 8)) +
+                                                         " is outside the parameter domain");
+    const int64_t n_groups = m->n_pad / 8;
+    static const int pass_env = std::getenv("MF_POINTS_PER_PASS") ? std::atoi(std::getenv("MF_POINTS_PER_PASS")) : 0;  // tuning knob
+    const int per_pass = (pass_env == 16 || pass_env == 32 || pass_env == 64) ? pass_env : n_points > 32 ? 64 : n_points > 16 ? 32 : 16;
+    const int ctas_per_sm = per_pass == 64 ? 1 : 2;
+    const int G = (int)std::max<int64_t>(1, std::min<int64_t>((n_groups + kWarps - 1) / kWarps, ctas_per_sm * (int64_t)ctx->sm_count));
+    {
+        const mf_status ss = points_scratch(ctx, n_points, G);
+        if (ss != MF_OK) return ss;
+    }
+    auto up = [](size_t x) { return (x + 255) / 256 * 256; };
+    const int64_t P = ctx->p_points;
+    const int C = ctx->p_chunks;
+    char* h_blk = nullptr;
+    int stage = 0;
+    const size_t b_coef = sizeof(double) * 8 * n_points;
+    MF_CUDA(ctx, points_stage(ctx, b_coef, &h_blk, &stage));
+    std::memcpy(h_blk, lambdas, b_coef);
+    AngPointsArgs a;
+    for (int i = 0; i < 9; ++i) a.col[i] = m->col[i];
+    a.n = m->n_events;
+    a.n_pad = m->n_pad;
+    char* q = ctx->p_blk;
+    a.coef = reinterpret_cast<const double*>(q);
+    q += up(sizeof(FourDConsts) * P) + up(sizeof(int) * P);
+    a.partials = reinterpret_cast<double*>(q);
+    q += up(sizeof(double) * P * MF_MAX_NACC * C);
+    a.bad_partials = reinterpret_cast<unsigned*>(q);
+    a.n_points = (int)n_points;
+    MF_CUDA(ctx, cudaMemcpyAsync(q = ctx->p_blk, h_blk, b_coef, cudaMemcpyHostToDevice, ctx->stream));
+    MF_CUDA(ctx, cudaEventRecord(ctx->pts_copied[stage], ctx->stream));
+    take_fresh(m);
+    const dim3 grid((unsigned)G, (unsigned)((n_points + per_pass - 1) / per_pass));
+    if (per_pass == 64) angular_points_mma_kernel<8><<<grid, kBlock, 0, ctx->stream>>>(a);
+    else if (per_pass == 32) angular_points_mma_kernel<4><<<grid, kBlock, 0, ctx->stream>>>(a);
+    else angular_points_mma_kernel<2><<<grid, kBlock, 0, ctx->stream>>>(a);
+    angular_points_combine_kernel<<<(unsigned)((n_points + kWarps - 1) / kWarps), kBlock, 0, ctx->stream>>>(
+        a.partials, a.bad_partials, G, (int)n_points, out_dev);
+    MF_CUDA(ctx, cudaGetLastError());
+    ctx->launches += 2;
+    return MF_OK;
+}
+
 template <class M>
 static mf_status launch_points(mf_model* m, int64_t n_points, const double* lambdas, double* out_dev)
 {
@@ -793,25 +870,11 @@ static mf_status launch_points(mf_model* m, int64_t n_points, const double* lamb
     if (n_points * chunks64 > (int64_t)0x7fffffff)
         return mf_fail(ctx, MF_ERR_ARG, "mf_nll_grad_points: n_points x event chunks exceeds the grid limit; split the call");
     const int chunks = (int)chunks64;
-    // device scratch [consts | ok | partials | bad | ticket], laid out for the largest (points, chunks) seen so far
-    auto up = [](size_t x) { return (x + 255) / 256 * 256; };
-    if (n_points > ctx->p_points || chunks > ctx->p_chunks || !ctx->p_blk) {
-        const int64_t P = std::max<int64_t>(n_points, ctx->p_points);
-        const int C = std::max(chunks, ctx->p_chunks);
-        const size_t bytes = up(sizeof(FourDConsts) * P) + up(sizeof(int) * P) + up(sizeof(double) * P * MF_MAX_NACC * C) +
-                             up(sizeof(unsigned) * P * C) + up(sizeof(unsigned) * P);
-        dev_free(ctx, ctx->p_blk);  // stream-ordered: after the launches that still use it
-        ctx->p_blk = nullptr;
-        ctx->p_points = 0;
-        ctx->p_chunks = 0;
-        MF_CUDA(ctx, dev_alloc(ctx, &ctx->p_blk, bytes));
-        ctx->p_bytes = bytes;
-        ctx->p_points = P;
-        ctx->p_chunks = C;
-        // ok flags non-zero (every point is validated on the host), tickets zero (the kernel leaves them at zero)
-        MF_CUDA(ctx, cudaMemsetAsync(ctx->p_blk + up(sizeof(FourDConsts) * P), 0xFF, up(sizeof(int) * P), ctx->stream));
-        MF_CUDA(ctx, cudaMemsetAsync(ctx->p_blk + bytes - up(sizeof(unsigned) * P), 0, up(sizeof(unsigned) * P), ctx->stream));
+    {
+        const mf_status ss = points_scratch(ctx, n_points, chunks);
+        if (ss != MF_OK) return ss;
     }
+    auto up = [](size_t x) { return (x + 255) / 256 * 256; };
     const int64_t P = ctx->p_points;
     const int C = ctx->p_chunks;
     BatchArgs<M> a;
@@ -869,7 +932,11 @@ extern "C" mf_status mf_nll_grad_points(mf_model* m, int64_t n_points, const dou
     if (n_points > (int64_t)1 << 20) return mf_fail(m->ctx, MF_ERR_ARG, "mf_nll_grad_points: more than 2^20 points per call");
     switch (m->kind) {
     case MF_MASS_GAUSS_EXP: return launch_points<MassModel>(m, n_points, lambdas, out_dev);
-    case MF_ANGULAR_KSTMUMU: return launch_points<AngularModel>(m, n_points, lambdas, out_dev);
+    case MF_ANGULAR_KSTMUMU: {
+        static const bool no_mma = std::getenv("MF_NO_POINTS_MMA") != nullptr;  // ablation switch: the (point, chunk) kernel
+        return no_mma ? launch_points<AngularModel>(m, n_points, lambdas, out_dev)
+                      : launch_points_angular_mma(m, n_points, lambdas, out_dev);
+    }
     default: return launch_points<FourDModel>(m, n_points, lambdas, out_dev);
     }
 }

@@ -1,0 +1,216 @@
+// mf_points.cuh — many parameter points on ONE dataset in a single pass over the data, angular model
+// ("multi-lambda evaluation in one pass ... the only case where F C becomes a real contraction worth
+// testing on tensor cores"; north_star: "tensor cores only if the batched angular basis product F(N x K) C(K x M) is shown
+// by ncu to be a real contraction").
+//
+// With M parameter points the cached-basis model is two contractions around one reciprocal:
+//     P[p][e]   = sum_k a_pk h_k(e)            (k = 0..8, a_p0 = 1)        [M x 9] . [9 x N]
+//     r[p][e]   = 1 / P[p][e],   ln L_p = sum_e ln P[p][e]                 (log of the running product, LogProd)
+//     G[p][k]   = sum_e r[p][e] h_k(e)         (k = 1..8)                  [M x N] . [N x 8]
+// Both run as DMMA m8n8k4 (mma.sync f64) on 8 points x 8 events at a time:
+//   step 1: A = coefficients (8 points x 4 k, registers, loaded once), B = basis values (4 k x 8 events), two k-steps for
+//           h_1..h_8, the accumulator tile initialised with the coefficient-free h_0 -> lane (g, t) holds
+//           P(point g; events 2t, 2t+1);
+//   step 2: A = r (8 points x 4 events) — exactly the two values each lane already holds if k-step j takes events
+//           {2t + j}: no transposition, no shuffle; B = h_{1+g}(event 2t + j), one 16-byte load -> G tile (8 points x 8 k).
+// Every 8-event group is loaded once (two layouts, 576 B each, straight from L2 / HBM in 64-byte segments) and serves all
+// the points of the pass, so the arithmetic intensity grows with M and the kernel is bound by the fp64 pipe: per
+// (point, event) pair 4/64 DMMA (each holds the pipe of its SM sub-partition for 16 clocks) + one reciprocal (3 DFMA) + one
+// DMUL, i.e. 0.31 pipe-clocks per pair per SM, the same as the hand-written DFMA form — which however issues 2.4
+// instructions per pair instead of 0.6 and whose three-register DFMAs run at 2/3 rate.
+#pragma once
+#include "mf_kernels.cuh"
+#include "mf_second.cuh"  // dmma_m8n8k4
+
+namespace mf {
+
+struct AngPointsArgs {
+    const double* col[9];   // h_0..h_8
+    int64_t n, n_pad;
+    const double* coef;     // device [n_points][8]: FL, S3, S4, S5, AFB, S7, S8, S9 per point
+    int n_points;
+    double* partials;       // [n_points][9][G]
+    unsigned* bad_partials; // [n_points][G]
+};
+
+// NPB point blocks of 8 points per CTA pass; grid = (G, ceil(n_points / (8 NPB))).
+template <int NPB>
+__global__ void __launch_bounds__(kBlock, (NPB <= 4) ? 2 : 1) angular_points_mma_kernel(const __grid_constant__ AngPointsArgs a)
+{
+    __shared__ double red[kWarps][NPB][8][9];
+    __shared__ unsigned red_bad[kWarps][NPB][8];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int fg = lane >> 2, ft = lane & 3;
+    const int64_t G = gridDim.x;
+    const int p0 = blockIdx.y * (8 * NPB);  // first point of this pass
+    // step-1 A fragments: lane (fg, ft) holds the coefficient of h_{1 + 4 kk + ft} of point p = p0 + 8 pb + fg
+    double ca[NPB][2];
+#pragma unroll
+    for (int pb = 0; pb < NPB; ++pb) {
+        const int p = p0 + 8 * pb + fg;
+        const bool live = p < a.n_points;
+#pragma unroll
+        for (int kk = 0; kk < 2; ++kk) ca[pb][kk] = live ? __ldg(a.coef + (int64_t)p * 8 + 4 * kk + ft) : 0.0;
+    }
+    double g[NPB][2];
+    LogProd lp[NPB];
+    unsigned bad[NPB];
+#pragma unroll
+    for (int pb = 0; pb < NPB; ++pb) {
+        g[pb][0] = g[pb][1] = 0.0;
+        bad[pb] = 0;
+    }
+    const int64_t n_groups = a.n_pad / 8, step = G * kWarps;
+    // fragments of a group: f1[kk] = h_{1 + 4 kk + ft}(event fg), f2 = h_{1 + fg}(events 2 ft, 2 ft + 1),
+    // f0 = h_0(events 2 ft, 2 ft + 1): the coefficient-free term, the initial value of every P tile
+    struct Frag {
+        double f1[2];
+        double2 f2, f0;
+    };
+    auto load = [&](int64_t grp, Frag& f) {
+        const int64_t e0 = grp * 8;
+        f.f1[0] = __ldg(a.col[1 + ft] + e0 + fg);
+        f.f1[1] = __ldg(a.col[5 + ft] + e0 + fg);
+        f.f2 = __ldg(reinterpret_cast<const double2*>(a.col[1 + fg] + e0) + ft);
+        f.f0 = __ldg(reinterpret_cast<const double2*>(a.col[0] + e0) + ft);
+    };
+    // One group for all the point blocks of the pass, written stage by stage across the NPB independent blocks so that
+    // dependent instructions are NPB apart.  Only the dataset's last groups can hold padded events (copies of the last
+    // event): there `masked` makes them contribute exactly nothing.
+    auto process = [&](int64_t grp, const Frag& f) {
+        const double2 f2 = f.f2;
+        double c[NPB][2], r[NPB][2];
+#pragma unroll
+        for (int pb = 0; pb < NPB; ++pb) {
+            c[pb][0] = f.f0.x;
+            c[pb][1] = f.f0.y;
+        }
+#pragma unroll
+        for (int kk = 0; kk < 2; ++kk)
+#pragma unroll
+            for (int pb = 0; pb < NPB; ++pb) dmma_m8n8k4(c[pb][0], c[pb][1], ca[pb][kk], f.f1[kk]);
+        const bool masked = grp * 8 + 8 > a.n;  // warp-uniform
+        const int64_t e = grp * 8 + 2 * ft;
+        const bool v0 = e < a.n, v1 = e + 1 < a.n;
+        if (masked) {
+#pragma unroll
+            for (int pb = 0; pb < NPB; ++pb) {
+                c[pb][0] = v0 ? c[pb][0] : 1.0;
+                c[pb][1] = v1 ? c[pb][1] : 1.0;
+            }
+        }
+#pragma unroll
+        for (int pb = 0; pb < NPB; ++pb) {
+            r[pb][0] = mf_rcp(c[pb][0]);
+            r[pb][1] = mf_rcp(c[pb][1]);
+        }
+        if (masked) {
+#pragma unroll
+            for (int pb = 0; pb < NPB; ++pb) {
+                r[pb][0] = v0 ? r[pb][0] : 0.0;
+                r[pb][1] = v1 ? r[pb][1] : 0.0;
+            }
+        }
+#pragma unroll
+        for (int pb = 0; pb < NPB; ++pb) dmma_m8n8k4(g[pb][0], g[pb][1], r[pb][0], f2.x);
+#pragma unroll
+        for (int pb = 0; pb < NPB; ++pb) dmma_m8n8k4(g[pb][0], g[pb][1], r[pb][1], f2.y);
+#pragma unroll
+        for (int pb = 0; pb < NPB; ++pb) {
+            lp[pb].mul(c[pb][0], bad[pb]);
+            lp[pb].mul(c[pb][1], bad[pb]);
+        }
+    };
+    // two fragment buffers used alternately (no register copies, which would wait for the loads): the next group of this
+    // warp is in flight while the current one is evaluated
+    Frag fa, fb;
+    int64_t gi = blockIdx.x + G * warp;
+    unsigned since_renorm = 0;
+    if (gi < n_groups) load(gi, fa);
+    while (gi < n_groups) {
+        if (gi + step < n_groups) load(gi + step, fb);
+        process(gi, fa);
+        gi += step;
+        if (gi >= n_groups) break;
+        if (gi + step < n_groups) load(gi + step, fa);
+        process(gi, fb);
+        gi += step;
+        if (++since_renorm == 128) {  // 512 mantissas in [1, 2) per running product since the last one
+            since_renorm = 0;
+#pragma unroll
+            for (int pb = 0; pb < NPB; ++pb) lp[pb].renorm();
+        }
+    }
+    // lane (fg, ft): ln of the product over its events for point fg of every block; sum over the four ft lanes
+#pragma unroll
+    for (int pb = 0; pb < NPB; ++pb) {
+        double l = lp[pb].log();
+        l += __shfl_xor_sync(0xffffffffu, l, 1);
+        l += __shfl_xor_sync(0xffffffffu, l, 2);
+        unsigned b = bad[pb];
+        b += __shfl_xor_sync(0xffffffffu, b, 1);
+        b += __shfl_xor_sync(0xffffffffu, b, 2);
+        if (ft == 0) {
+            red[warp][pb][fg][0] = l;
+            red_bad[warp][pb][fg] = b;
+        }
+        red[warp][pb][fg][1 + 2 * ft] = g[pb][0];
+        red[warp][pb][fg][2 + 2 * ft] = g[pb][1];
+    }
+    __syncthreads();
+    for (int q = threadIdx.x; q < NPB * 8 * 10; q += kBlock) {
+        const int pl = q / 10, k = q % 10;  // local point, quantity (9: bad count)
+        const int p = p0 + pl;
+        if (p >= a.n_points) continue;
+        if (k < 9) {
+            double s = 0.0;
+#pragma unroll
+            for (int w = 0; w < kWarps; ++w) s += red[w][pl >> 3][pl & 7][k];
+            a.partials[((int64_t)p * 9 + k) * G + blockIdx.x] = s;
+        } else {
+            unsigned b = 0;
+#pragma unroll
+            for (int w = 0; w < kWarps; ++w) b += red_bad[w][pl >> 3][pl & 7];
+            a.bad_partials[(int64_t)p * G + blockIdx.x] = b;
+        }
+    }
+}
+
+// One warp per point: fixed-order Kahan sums of the CTA partials, then out[p] = (-ln L, gradient[8], n_bad).
+__global__ void __launch_bounds__(kBlock) angular_points_combine_kernel(const double* __restrict__ partials,
+                                                                       const unsigned* __restrict__ bad_partials, int G,
+                                                                       int n_points, double* __restrict__ out)
+{
+    const int lane = threadIdx.x & 31, p = blockIdx.x * kWarps + (threadIdx.x >> 5);
+    if (p >= n_points) return;
+    unsigned nb = 0;
+    for (int i = lane; i < G; i += 32) nb += __ldcg(bad_partials + (int64_t)p * G + i);
+    nb = __reduce_add_sync(0xffffffffu, nb);
+    double* o = out + (int64_t)p * 10;
+    for (int k = 0; k < 9; ++k) {
+        const double* pk = partials + ((int64_t)p * 9 + k) * G;
+        double s = 0.0, cc = 0.0;
+        for (int i = lane; i < G; i += 32) {
+            const double y = __ldcg(pk + i) - cc;
+            const double t = s + y;
+            cc = (t - s) - y;
+            s = t;
+        }
+        double lo = -cc;
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+            const double s2 = __shfl_down_sync(0xffffffffu, s, off);
+            const double lo2 = __shfl_down_sync(0xffffffffu, lo, off);
+            const double t = s + s2;
+            const double bb = t - s;
+            const double e = (s - (t - bb)) + (s2 - bb);
+            lo = (lo + lo2) + e;
+            s = t;
+        }
+        if (lane == 0)
+            o[k] = !nb ? -(s + lo) : (k == 0) ? __longlong_as_double(0x7ff0000000000000LL) : __longlong_as_double(0x7ff8000000000000LL);
+    }
+    if (lane == 0) o[9] = (double)nb;
+}
+
+}  // namespace mf

@@ -2,6 +2,7 @@
 4D models, batched toys of the 4D model, the register-buffer 4D kernel (n < 1024), the host-result sweep, the
 MF_NO_TMA / MF_NO_PDL ablation paths (subprocess: the switches are read once per process) and the sharded evaluation of
 paper_2505_12414_b200.dist with the CUDA path supplying the shard sums.  Every comparison is against the oracle."""
+import math
 import os
 import subprocess
 import sys
@@ -58,9 +59,10 @@ def _fourd_points(n_pts, seed):
     return pts
 
 
-@pytest.mark.parametrize("n,n_pts", [(20_011, 16), (150_000, 64)])
+@pytest.mark.parametrize("n,n_pts", [(20_011, 16), (150_000, 64), (1, 16), (10_007, 17), (20_011, 40), (5_000, 100)])
 def test_points_mode_angular_vs_oracle(mf, ctx, n, n_pts):
-    """launch_points<AngularModel>: every row of a >= 16-point call against the oracle."""
+    """The angular many-points kernel (two tensor-core contractions, mf_points.cuh): every row of a >= 16-point call
+    against the oracle, with ragged event counts, partly filled point blocks and more than one 64-point pass."""
     import torch
     ev = dg.gen_angular(n, seed=21)
     model = ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ctx.dataset_upload(ev))
@@ -73,6 +75,28 @@ def test_points_mode_angular_vs_oracle(mf, ctx, n, n_pts):
     for p in range(n_pts):
         o_nll, o_g, _ = oracle.nll_grad(oracle.ANGULAR, ev, pts[p], nthreads=oracle.max_threads())
         check(res[p, 0], res[p, 1:9], o_nll, o_g, f"angular points row {p}")
+
+
+def test_points_mode_angular_bad_point(mf, ctx):
+    """A point at which the PDF goes negative for some events gets +inf / NaN and the count; its neighbours are unaffected."""
+    import torch
+    ev = dg.gen_angular(4_000, seed=22)
+    model = ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ctx.dataset_upload(ev))
+    pts = _ang_points(20, 7)
+    pts[11, 1] = 5.0
+    out = torch.full((20, 10), float("nan"), dtype=torch.float64, device="cuda")
+    model.nll_grad_points(pts, out.data_ptr())
+    torch.cuda.synchronize()
+    res = out.cpu().numpy()
+    _, _, nbad = oracle.nll_grad(oracle.ANGULAR, ev, pts[11])
+    assert nbad > 0 and res[11, 9] == nbad and res[11, 0] == math.inf and np.all(np.isnan(res[11, 1:9]))
+    for p in (10, 12):
+        o_nll, o_g, _ = oracle.nll_grad(oracle.ANGULAR, ev, pts[p])
+        check(res[p, 0], res[p, 1:9], o_nll, o_g, f"row {p}")
+    pts[3, 2] = np.nan
+    with pytest.raises(mf.MoreFitError) as e:
+        model.nll_grad_points(pts, out.data_ptr())
+    assert e.value.status == mf.MF_ERR_PARAM_DOMAIN
 
 
 @pytest.mark.parametrize("n,n_pts", [(30_001, 16), (100_000, 64)])
@@ -188,6 +212,13 @@ _ABLATION = textwrap.dedent("""
     for _ in range(3):
         nll, g = am.nll_grad(dg.ANG_TRUTH)
     check(nll, g, oracle.nll_grad(oracle.ANGULAR, ev, dg.ANG_TRUTH))
+    apts = np.tile(np.array(dg.ANG_TRUTH), (20, 1)) + np.random.default_rng(3).uniform(-0.03, 0.03, (20, 8))
+    aout = torch.zeros((20, 10), dtype=torch.float64, device="cuda")
+    am.nll_grad_points(apts, aout.data_ptr())      # >= 16 points: the many-points kernel of the angular model
+    torch.cuda.synchronize()
+    ar = aout.cpu().numpy()
+    for p in (0, 7, 19):
+        check(ar[p, 0], ar[p, 1:9], oracle.nll_grad(oracle.ANGULAR, ev, apts[p]))
     ev4 = dg.gen_4d(50_021, seed=3)
     fm = ctx.model_create(mf.MF_MASS_X_ANGULAR, ctx.dataset_upload(ev4, dg.MASS_LO, dg.MASS_HI))
     nll, g = fm.nll_grad(dg.FOURD_TRUTH)
@@ -215,7 +246,7 @@ _ABLATION = textwrap.dedent("""
 """)
 
 
-@pytest.mark.parametrize("switch", ["MF_NO_TMA", "MF_NO_PDL"])
+@pytest.mark.parametrize("switch", ["MF_NO_TMA", "MF_NO_PDL", "MF_NO_POINTS_MMA"])
 def test_ablation_switches_vs_oracle(mf, switch):
     """The MF_NO_TMA=1 (register-buffer kernels for the angular / 4D models) and MF_NO_PDL=1 (plain stream order) paths
     that DESIGN.md quotes numbers for, against the oracle."""
