@@ -50,9 +50,10 @@ K_PARAMS = 4
 METRIC = "nll_grad_event_evals_per_s"
 UNIT = "events/s"
 WORKLOAD = "C1: 1D Gaussian+exponential mass model, N=1e6 fp64 events, K=4, NLL+gradient at 1000 seeded lambda points"
-# fp64-pipe thread-instructions per event of the shipped mass kernel's fast path (counted from
-# SASS); never more than the plain two-exponential form's hand count (100).
-MASS_FP64_INSTR_PER_EVENT = 26.0
+# fp64-pipe thread-instructions per event of the shipped mass kernel's fast path, counted in its SASS (177 DFMA/DMUL/DADD
+# per 8-event call = 22.1 per event, DESIGN.md §7 "Roofline"); the shipped kernel's count, never more than
+# the plain two-exponential form's hand count (100).  Round 1 credited 26 (that kernel's count).
+MASS_FP64_INSTR_PER_EVENT = 22.1
 POINTS_PER_CALL = 500  # evaluations per mf_nll_grad_points call (ONE launch: CTA tile = (point, event chunk))
 NOMINAL_FP64_LANES_PER_SM = 64  # B200: 4 SMSPs x 16 fp64 FMA lanes
 SINGLE_LAUNCH_STEPS = 4000      # evaluations of the one-launch-per-evaluation leg (fixed, whatever --steps says)
@@ -252,6 +253,8 @@ def _other_workloads(torch, mf, ctx, peaks, traffic_all) -> dict:
     hbm = float(peaks.get("hbm_gbs", 0.0)) or 6650.0
     hbm_how = "MEASURED_PEAKS.json hbm_gbs" if peaks.get("hbm_gbs") else "fallback of B200_PROFILING.md (6.65 TB/s)"
     res = {"hbm_peak_source": hbm_how}
+    n_sm_ = torch.cuda.get_device_properties(0).multi_processor_count
+    sm_mhz_ = float(peaks.get("sm_max_mhz", 1965.0))
     # C2: 3D angular, N = 1e6, nine cached basis columns = 72 B/event (HBM bound)
     ev = dg.gen_angular(1_000_000, seed=2)
     ms = [ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ctx.dataset_upload(ev)) for _ in range(6)]   # 6 x 72 MB = 432 MB > 3 x L2
@@ -266,6 +269,30 @@ def _other_workloads(torch, mf, ctx, peaks, traffic_all) -> dict:
     r = ms[0].fit(dg.ANG_TRUTH)
     res["C2_angular_1e6"]["fit_s"] = time.perf_counter() - t
     res["C2_angular_1e6"]["fit_calls"] = r.n_calls
+    # many parameter points in ONE pass over the data: two fp64 tensor-core contractions, 64 points per pass
+    mp = {}
+    for M in (64, 1000):
+        ptsM = np.tile(np.array(dg.ANG_TRUTH), (M, 1)) + np.random.default_rng(5).uniform(-0.03, 0.03, (M, 8))
+        oM = torch.zeros((M, 10), dtype=torch.float64, device="cuda")
+        for _ in range(3):
+            ms[0].nll_grad_points(ptsM, oM.data_ptr())
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = 20
+        e0.record()
+        for i_ in range(reps):
+            ms[i_ % len(ms)].nll_grad_points(ptsM, oM.data_ptr())
+        e1.record()
+        torch.cuda.synchronize()
+        usM = float(e0.elapsed_time(e1)) * 1e3 / reps / M
+        if not np.all(np.isfinite(oM.cpu().numpy()[:, :9])):
+            raise RuntimeError("non-finite result in the angular many-points workload")
+        # pipe work per (point, event) pair: 4/64 DMMA of 256 FMAs + reciprocal (3 DFMA) + 1 DMUL = 20 FMA-equivalents
+        mp[f"us_per_evaluation_{M}_points"] = usM
+        mp[f"frac_of_fp64_peak_{M}_points"] = 20.0 * 1e6 / (usM * 1e-6) / (n_sm_ * NOMINAL_FP64_LANES_PER_SM * sm_mhz_ * 1e6)
+    mp["kernel"] = "angular_points_mma_kernel<8> + angular_points_combine_kernel (mf_nll_grad_points)"
+    mp["bound"] = "alu (fp64 pipe, DMMA shares it with DFMA): 20 FMA-equivalents per (point, event) pair incl. tile padding"
+    res["C2_angular_1e6"]["many_points"] = mp
     del ms, ev
     # C3: 4D, N = 2e6, 12 columns = 96 B/event (192 MB > L2)
     ev = dg.gen_4d(2_000_000, seed=3)
@@ -278,11 +305,36 @@ def _other_workloads(torch, mf, ctx, peaks, traffic_all) -> dict:
                                      "frac": gbs / hbm if hbm else None, "bytes_per_event": 96,
                                      "traffic": traffic_all.get("nll_grad_tma_kernel<FourDModel>")},
                         "l2": "2 model replicas x 192 MB of columns, alternating every evaluation"}
+    m4.fit(dg.FOURD_TRUTH)
     t = time.perf_counter()
     r = m4.fit(dg.FOURD_TRUTH)
     res["C3_4d_2e6"]["fit_s"] = time.perf_counter() - t
     res["C3_4d_2e6"]["fit_calls"] = r.n_calls
-    del m4, m4s, ev
+    res["C3_4d_2e6"]["fit"] = "mf_fit: Newton steps on the analytic Hessian (second-order kernel: S^T S by fp64 tensor-core contraction) + HESSE"
+    # value + gradient + analytic Hessian (136 second derivatives), and with the Fisher matrix, per synchronous call
+    def sync_us(f, n=20):
+        f()
+        t0 = time.perf_counter()
+        for _ in range(n):
+            f()
+        return (time.perf_counter() - t0) / n * 1e6
+    res["C3_4d_2e6"]["second_order"] = {
+        "kernel": "nll_second_kernel<FourDSecond, 1|2> + second_combine_kernel",
+        "us_per_call_value_gradient_hessian": sync_us(lambda: m4.nll_grad_hess(dg.FOURD_TRUTH)),
+        "us_per_call_with_fisher_matrix": sync_us(lambda: m4.nll_grad_hess_fisher(dg.FOURD_TRUTH)),
+        "us_per_call_value_gradient": sync_us(lambda: m4.nll_grad(dg.FOURD_TRUTH)),
+        "what": "synchronous host calls (launch pair + D2H of the result row + stream synchronise included)"}
+    # weighted fit of the same events: every evaluation through the second-order kernel, sandwich covariance
+    dsw = ctx.dataset_upload(ev, dg.MASS_LO, dg.MASS_HI)
+    dsw.set_weights(np.random.default_rng(77).uniform(0.5, 1.5, ev.shape[1]))
+    m4w = ctx.model_create(mf.MF_MASS_X_ANGULAR, dsw)
+    m4w.fit(dg.FOURD_TRUTH)
+    t = time.perf_counter()
+    rw = m4w.fit(dg.FOURD_TRUTH)
+    res["C3_4d_2e6"]["weighted_fit"] = {"fit_s": time.perf_counter() - t, "fit_calls": rw.n_calls, "converged": bool(rw.converged),
+                                        "us_per_call_value_gradient": sync_us(lambda: m4w.nll_grad(dg.FOURD_TRUTH)),
+                                        "what": "weights uniform in [0.5, 1.5]; covariance = H^-1 F H^-1 (mf_nll_grad_hess_fisher at the minimum)"}
+    del m4, m4s, m4w, dsw, ev
     # C4: 4096 toys x 1e4 events (328 MB > L2), one launch for all toys; then all toys fitted concurrently
     T, n = 4096, 10_000
     toys = dg.gen_mass_toys(T, n, first_seed=0)

@@ -73,11 +73,17 @@ def test_mass_hessian_batch_parity(mf, ctx):
 def test_hessian_status(mf, ctx):
     ev = dg.gen_4d(1000, seed=3)
     amodel = ctx.model_create(mf.MF_MASS_X_ANGULAR, ctx.dataset_upload(ev, LO, HI))
-    assert not amodel.has_hessian                 # no Hessian kernel for the 4D family: the fit uses finite differences
-    with pytest.raises(mf.MoreFitError) as e:
-        amodel.nll_grad_hess(dg.FOURD_TRUTH)
-    assert e.value.status == mf.MF_ERR_ARG
+    assert amodel.has_hessian                     # single dataset: every family (4D through the second-order kernel)
     assert amodel.fit(dg.FOURD_TRUTH).converged
+    ofd = mf.default_fit_opts()
+    ofd.analytic_hessian = 0                      # the finite-difference mode stays available (register kernel, n_pad < 1024)
+    assert amodel.fit(dg.FOURD_TRUTH, opts=ofd).converged
+    toys4 = np.stack([dg.gen_4d(500, seed=s) for s in (1, 2)], axis=1)      # [4][2][500]
+    bmodel = ctx.model_create(mf.MF_MASS_X_ANGULAR, ctx.dataset_upload(toys4, LO, HI, n_toys=2))
+    assert not bmodel.has_hessian                 # batched 4D toys: no batched Hessian kernel, the fit uses finite differences
+    with pytest.raises(mf.MoreFitError) as e:
+        bmodel.nll_grad_hess_batch(np.tile(np.array(dg.FOURD_TRUTH), (2, 1)))
+    assert e.value.status == mf.MF_ERR_ARG
     m = dg.gen_mass(1000, seed=0)
     model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(m, LO, HI))
     with pytest.raises(mf.MoreFitError) as e:
