@@ -444,8 +444,19 @@ def _other_workloads(torch, mf, ctx, peaks, traffic_all) -> dict:
     lat = (time.perf_counter() - t) / 200
     t = time.perf_counter()
     r = m0.fit(dg.MASS_START)
-    res["C0_mass_1e4"] = {"sync_call_us": lat * 1e6, "fit_s": time.perf_counter() - t, "fit_calls": r.n_calls,
-                          "converged": bool(r.converged)}
+    fit_s0 = time.perf_counter() - t
+    m0.serve(True)          # resident evaluation kernel: no launch, no completion latency per call (mf_server.cuh)
+    for _ in range(50):
+        m0.nll_grad(dg.MASS_START)
+    t = time.perf_counter()
+    for _ in range(200):
+        m0.nll_grad(dg.MASS_START)
+    lat_served = (time.perf_counter() - t) / 200
+    m0.serve(False)
+    res["C0_mass_1e4"] = {"sync_call_us": lat * 1e6, "served_call_us": lat_served * 1e6, "fit_s": fit_s0, "fit_calls": r.n_calls,
+                          "converged": bool(r.converged),
+                          "what": "Python-level synchronous mf_nll_grad calls (ctypes marshalling included; from C: 13.0 us by launch, "
+                                  "8.5 us served, profiles/r2_server_latency.md); mf_fit serves its own evaluations"}
     # C1's full fit from the BASELINE start point (N = 1e6)
     m1 = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(dg.gen_mass(N_EVENTS, seed=1), dg.MASS_LO, dg.MASS_HI))
     m1.fit(dg.MASS_START)

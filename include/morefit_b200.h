@@ -206,6 +206,17 @@ mf_status mf_nll_grad_batch(mf_model* model, int64_t n_toys, const double* lambd
  * completed and its writes are visible. */
 mf_status mf_nll_grad_batch_async(mf_model* model, int64_t n_toys, const double* lambdas_dev, double* out_dev);
 
+/* Resident evaluation kernel for the minimiser's one-point-at-a-time pattern (at small N an evaluation
+ * costs its kernel submission).  on = 1: from the next mf_nll_grad / mf_nll_grad_hess on, the model's CTAs stay resident on
+ * a stream of their own (one per SM, at most half an SM's registers) and are fed through mapped pinned memory: the call
+ * writes the parameter-only constants and a request number, the last CTA writes the result and the number back; no kernel
+ * launch and no completion latency per call.  The kernel leaves on mf_model_serve(model, 0), mf_model_destroy, or by
+ * itself after 5 ms without a request (it is relaunched on the next call).  mf_fit serves its own evaluations this way
+ * for the duration of the fit.  Only unweighted MF_MASS_GAUSS_EXP models with n_toys == 1 and n_events > 0 (MF_ERR_ARG
+ * otherwise).  Other calls on the model or the context are unaffected and may run beside the resident kernel. */
+mf_status mf_model_serve(mf_model* model, int on);
+int mf_model_is_served(const mf_model* model);
+
 /* ---- value + gradient + analytic Hessian ---------------------- */
 
 /* 1 if the analytic Hessian is available for this model: every family on a single dataset (n_toys == 1); with

@@ -35,7 +35,7 @@ EXPORTS = [
     "mf_dataset_upload", "mf_generate_mass", "mf_generate_angular", "mf_generate_4d", "mf_dataset_download", "mf_dataset_set_weights", "mf_dataset_destroy", "mf_dataset_n_events", "mf_dataset_n_toys",
     "mf_model_create", "mf_model_destroy", "mf_model_nparams", "mf_model_n_events", "mf_model_n_toys",
     "mf_nll_grad", "mf_nll_grad_async", "mf_nll_grad_points", "mf_nll_grad_sweep", "mf_nll_grad_batch", "mf_nll_grad_batch_async",
-    "mf_model_has_hessian", "mf_model_is_weighted", "mf_nll_grad_hess", "mf_nll_grad_hess_fisher", "mf_nll_grad_hess_batch",
+    "mf_model_serve", "mf_model_is_served", "mf_model_has_hessian", "mf_model_is_weighted", "mf_nll_grad_hess", "mf_nll_grad_hess_fisher", "mf_nll_grad_hess_batch",
     "mf_fit_opts_default", "mf_fit", "mf_fit_batch", "mf_toy_study_mass",
     "mf_combine_partials",
 ]
@@ -180,6 +180,10 @@ def load_library() -> ctypes.CDLL:
     lib.mf_model_has_hessian.argtypes = [vp]
     lib.mf_nll_grad_hess.restype = ctypes.c_int
     lib.mf_nll_grad_hess.argtypes = [vp, dp, dp, dp, dp]
+    lib.mf_model_serve.restype = ctypes.c_int
+    lib.mf_model_serve.argtypes = [vp, ctypes.c_int]
+    lib.mf_model_is_served.restype = ctypes.c_int
+    lib.mf_model_is_served.argtypes = [vp]
     lib.mf_model_is_weighted.restype = ctypes.c_int
     lib.mf_model_is_weighted.argtypes = [vp]
     lib.mf_nll_grad_hess_fisher.restype = ctypes.c_int
@@ -473,6 +477,11 @@ class Model:
         hess = np.empty((self.K, self.K))
         self._ctx._check(self._lib.mf_nll_grad_hess(self._h, _dp(lam), ctypes.byref(nll), _dp(grad), _dp(hess)))
         return float(nll.value), grad, hess
+
+    def serve(self, on: bool = True) -> None:
+        """Keep a resident evaluation kernel for this model (mass model, single dataset): nll_grad / nll_grad_hess then
+        cost no kernel launch.  serve(False) stops it."""
+        self._ctx._check(self._lib.mf_model_serve(self._h, 1 if on else 0))
 
     @property
     def weighted(self) -> bool:

@@ -17,6 +17,7 @@
 #include "mf_kernels.cuh"
 #include "mf_second.cuh"
 #include "mf_points.cuh"
+#include "mf_server.cuh"
 
 using namespace mf;
 
@@ -136,6 +137,15 @@ extern "C" mf_status mf_ctx_create(int device, void* cuda_stream, mf_ctx** out)
 extern "C" void mf_ctx_destroy(mf_ctx* ctx)
 {
     if (!ctx) return;
+    for (mf_model* m : ctx->serving)  // resident kernels of models the caller has not destroyed
+        if (m->srv_running) {
+            for (int l = 0; l < 4; ++l) reinterpret_cast<volatile unsigned long long*>(m->h_req)[8 * l] = ~0ull;  // kServerExit
+            m->srv_running = false;
+        }
+    if (ctx->server_stream) {
+        cudaStreamSynchronize(ctx->server_stream);
+        cudaStreamDestroy(ctx->server_stream);
+    }
     cudaStreamSynchronize(ctx->stream);
     if (ctx->p_blk) cudaFreeAsync(ctx->p_blk, ctx->stream);
     if (ctx->h_slab) cudaFreeHost(ctx->h_slab);
@@ -323,12 +333,31 @@ extern "C" int64_t mf_dataset_n_toys(const mf_dataset* ds) { return ds ? ds->n_t
 
 // ------------------------------------------------------------------------------ S1: model
 
+// stops a model's resident kernel (if any) and forgets the model in the context's list
+static void server_stop_for_destroy(mf_model* m)
+{
+    if (m->srv_running) {
+        for (int l = 0; l < 4; ++l) reinterpret_cast<volatile unsigned long long*>(m->h_req)[8 * l] = ~0ull;  // kServerExit
+        cudaStreamSynchronize(m->ctx->server_stream);
+        cudaGetLastError();
+        m->srv_running = false;
+    }
+    auto& v = m->ctx->serving;
+    v.erase(std::remove(v.begin(), v.end(), m), v.end());
+}
+
 extern "C" void mf_model_destroy(mf_model* m)
 {
     if (!m) return;
     // device memory is freed in stream order; the pinned result slot is recycled at once, so no evaluation of this
     // model may still be in flight
+    server_stop_for_destroy(m);
     if (m->seq > 0 || m->n_toys > 1) cudaStreamSynchronize(m->ctx->stream);
+    dev_free(m->ctx, m->srv_relay);
+    dev_free(m->ctx, m->srv_partials);
+    dev_free(m->ctx, m->srv_bad);
+    dev_free(m->ctx, m->srv_ticket);
+    host_slot_release(m->ctx, m->h_req);
     dev_free(m->ctx, m->cache);
     dev_free(m->ctx, m->d_sum_m);
     dev_free(m->ctx, m->partials);
@@ -985,11 +1014,181 @@ extern "C" mf_status mf_nll_grad_sweep(mf_model* m, int64_t n_points, const doub
     return MF_OK;
 }
 
+
+// ---- resident evaluation kernel (mf_server.cuh) ---------------------------------------------------------------------
+
+static bool server_applicable(const mf_model* m)
+{
+    static const bool off = std::getenv("MF_NO_SERVER") != nullptr;  // ablation switch: every evaluation is a launch
+    return !off && m->kind == MF_MASS_GAUSS_EXP && m->n_toys == 1 && !m->wts && m->n_events > 0 && m->srv_failures < 3;
+}
+
+// Writes a request into the mapped slot: per 64-byte line the payload words first, then the line's request number
+// (x86 keeps the store order; the device reads a line atomically).  c == NULL: the numbers only.
+static void server_post(mf_model* m, unsigned long long seq, const MassConsts* c, int kind)
+{
+    volatile unsigned long long* req = reinterpret_cast<volatile unsigned long long*>(m->h_req);
+    if (c) {
+        unsigned long long pay[kServerReqPayload] = {};
+        pay[0] = (unsigned long long)kind;
+        static_assert(sizeof(MassConsts) + 8 <= sizeof(pay), "request payload too small");
+        std::memcpy(pay + 1, c, sizeof(MassConsts));
+        for (int l = 0; l < kServerReqLines; ++l)
+            for (int j = 0; j < 7; ++j) req[8 * l + 1 + j] = pay[7 * l + j];
+    }
+    std::atomic_thread_fence(std::memory_order_release);
+    for (int l = 0; l < kServerReqLines; ++l) req[8 * l] = seq;
+}
+
+static void server_stop(mf_model* m)
+{
+    if (!m->srv_running) return;
+    server_post(m, kServerExit, nullptr, 0);
+    cudaStreamSynchronize(m->ctx->server_stream);
+    cudaGetLastError();
+    m->srv_running = false;
+    server_post(m, m->srv_seq, nullptr, 0);  // not a new request for the next kernel
+}
+
+// Launches the resident kernel.  pending: request srv_seq has been written and is to be served by this kernel.
+static mf_status server_launch(mf_model* m, bool pending)
+{
+    mf_ctx* ctx = m->ctx;
+    if (!ctx->server_stream) MF_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->server_stream, cudaStreamNonBlocking));
+    const int64_t n_groups = (m->n_pad / kItem + kGroupItems - 1) / kGroupItems;
+    const int G = (int)std::max<int64_t>(1, std::min<int64_t>((n_groups + kWarps - 1) / kWarps, ctx->sm_count));
+    if (!m->h_req) {
+        MF_CUDA(ctx, host_slot_acquire(ctx, &m->h_req, &m->d_req_mapped));
+        MF_CUDA(ctx, dev_alloc(ctx, reinterpret_cast<char**>(&m->srv_relay), sizeof(ServerRelay)));
+        MF_CUDA(ctx, dev_alloc(ctx, &m->srv_partials, sizeof(double) * MassHessModel::NACC * ctx->sm_count));
+        MF_CUDA(ctx, dev_alloc(ctx, &m->srv_bad, sizeof(unsigned) * ctx->sm_count));
+        MF_CUDA(ctx, dev_alloc(ctx, &m->srv_ticket, sizeof(unsigned)));
+        MF_CUDA(ctx, cudaMemsetAsync(m->srv_ticket, 0, sizeof(unsigned), ctx->stream));
+        MF_CUDA(ctx, cudaMemsetAsync(m->srv_relay, 0, sizeof(ServerRelay), ctx->stream));
+        ctx->serving.push_back(m);
+    }
+    // everything enqueued on the work stream (S0 / S1 kernels, the scratch set-up above) is complete before the kernel starts
+    MF_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    const unsigned long long first = pending ? m->srv_seq - 1 : m->srv_seq;
+    if (!pending) server_post(m, first, nullptr, 0);
+    reinterpret_cast<volatile unsigned long long*>(m->h_out)[kServerRepExited] = 0ull;
+    MF_CUDA(ctx, cudaMemcpyAsync(&static_cast<ServerRelay*>(m->srv_relay)->seq, &first, sizeof(first), cudaMemcpyHostToDevice,
+                                 ctx->server_stream));  // pageable source: staged before the call returns
+    ServerArgs a;
+    a.col0 = m->col[0];
+    a.n = m->n_events;
+    a.n_items = m->n_pad / kItem;
+    a.sum_m = m->d_sum_m;
+    a.req = reinterpret_cast<const unsigned long long*>(m->d_req_mapped);
+    a.rep = m->d_out_mapped;
+    a.relay = static_cast<ServerRelay*>(m->srv_relay);
+    a.partials = m->srv_partials;
+    a.bad_partials = m->srv_bad;
+    a.ticket = m->srv_ticket;
+    a.first_seq = first;
+    static const unsigned long long idle_us = std::getenv("MF_SERVER_IDLE_US") ? std::strtoull(std::getenv("MF_SERVER_IDLE_US"), nullptr, 10) : 5000;
+    a.idle_ns = idle_us * 1000ull;
+    nll_server_kernel<<<G, kBlock, 0, ctx->server_stream>>>(a);
+    MF_CUDA(ctx, cudaGetLastError());
+    m->srv_running = true;
+    m->fresh = false;
+    ++ctx->launches;
+    return MF_OK;
+}
+
+// One evaluation through the resident kernel.  *handled = false: the server gave up (a tool serialises kernels): the caller
+// evaluates by launch.
+static mf_status server_eval_sync(mf_model* m, const double* lambda, double* nll, double* grad, double* hess, const char* who,
+                                  bool* handled)
+{
+    mf_ctx* ctx = m->ctx;
+    const int K = m->K;
+    *handled = true;
+    MassConsts c;
+    if (!mass_consts(lambda, m->ma, m->mb, c)) return mf_fail(ctx, MF_ERR_PARAM_DOMAIN, "lambda outside the parameter domain");
+    if (!m->h_req) {  // first use: set up and launch, then issue the request
+        const mf_status st = server_launch(m, false);
+        if (st != MF_OK) return st;
+    }
+    const unsigned long long want = ++m->srv_seq;
+    server_post(m, want, &c, hess ? 1 : 0);
+    if (!m->srv_running) {
+        const mf_status st = server_launch(m, true);
+        if (st != MF_OK) return st;
+    }
+    volatile unsigned long long* rep = reinterpret_cast<volatile unsigned long long*>(m->h_out);
+    for (unsigned spins = 1; rep[kServerRepDone] != want; ++spins) {
+        if ((spins & 0x3FFF) == 0 && rep[kServerRepExited] != 0 && rep[kServerRepDone] != want) {
+            // the kernel left (idle time-out racing with this request, or a tool ran it to completion before we could ask)
+            cudaStreamSynchronize(ctx->server_stream);
+            m->srv_running = false;
+            if (++m->srv_failures >= 3) {  // give up on the server for this model
+                *handled = false;
+                return MF_OK;
+            }
+            const mf_status st = server_launch(m, true);
+            if (st != MF_OK) return st;
+        }
+        if ((spins & 0xFFFFF) == 0) {
+            const cudaError_t q = cudaStreamQuery(ctx->server_stream);
+            if (q != cudaErrorNotReady && q != cudaSuccess) return mf_fail(ctx, MF_ERR_CUDA, std::string(who) + ": " + cudaGetErrorString(q));
+        }
+    }
+    std::atomic_thread_fence(std::memory_order_acquire);
+    m->srv_failures = 0;
+    *nll = m->h_out[0];
+    if (grad) std::memcpy(grad, m->h_out + 1, sizeof(double) * K);
+    const int nout = hess ? 1 + K + K * (K + 1) / 2 : K + 1;
+    if (hess) {
+        int q = 1 + K;
+        for (int i = 0; i < K; ++i)
+            for (int j = i; j < K; ++j, ++q) hess[i * K + j] = hess[j * K + i] = m->h_out[q];
+    }
+    if (m->h_out[nout] != 0.0)
+        return mf_fail(ctx, MF_NONPOSITIVE_PDF, "P <= 0 for " + std::to_string((long long)m->h_out[nout]) + " events at this lambda");
+    return MF_OK;
+}
+
+extern "C" mf_status mf_model_serve(mf_model* m, int on)
+{
+    if (!m) return MF_ERR_ARG;
+    if (on) {
+        if (!server_applicable(m))
+            return mf_fail(m->ctx, MF_ERR_ARG, "mf_model_serve: only unweighted MF_MASS_GAUSS_EXP models on a single non-empty dataset");
+        m->srv_on = true;
+    } else {
+        m->srv_on = false;
+        server_stop(m);
+    }
+    return MF_OK;
+}
+
+extern "C" int mf_model_is_served(const mf_model* m) { return m && m->srv_on ? 1 : 0; }
+
+mf_status mf_server_begin(mf_model* m)
+{
+    if (server_applicable(m)) m->srv_on = true;
+    return MF_OK;
+}
+
+void mf_server_end(mf_model* m, bool was_on)
+{
+    if (!was_on) {
+        m->srv_on = false;
+        server_stop(m);
+    }
+}
+
 // One synchronous evaluation: value, gradient and (hess != NULL, mass model) the K x K Hessian.
 static mf_status eval_sync(mf_model* m, const double* lambda, double* nll, double* grad, double* hess, const char* who)
 {
     mf_ctx* ctx = m->ctx;
     const int K = m->K;
+    if (m->srv_on && server_applicable(m)) {  // resident kernel: no launch, no completion latency
+        bool handled = false;
+        const mf_status ss = server_eval_sync(m, lambda, nll, grad, hess, who, &handled);
+        if (handled) return ss;
+    }
     // the last CTA writes the result, then the done word, to mapped pinned memory; the host spins on the
     // done word (a stream synchronise costs ~20 us of driver latency per call, the kernel 4-30 us)
     const mf_status st = dispatch_single(m, lambda, m->d_out_mapped, false, true, hess != nullptr);

@@ -450,6 +450,14 @@ static mf_status fit_one(mf_model* m, const double* start, const uint8_t* fixed,
     st.init(m->K, start, fixed, o);
     const bool analytic = o.analytic_hessian != 0 && mf_model_has_hessian(m);
     if (analytic) st.use_analytic_hessian();
+    // the minimiser asks for one point at a time: serve the evaluations from a resident kernel for the duration of the fit
+    // where the model family has one (kernel submission dominates at small N)
+    struct Serve {
+        mf_model* m;
+        bool was_on;
+        explicit Serve(mf_model* mm) : m(mm), was_on(mf_model_is_served(mm) != 0) { mf_server_begin(m); }
+        ~Serve() { mf_server_end(m, was_on); }
+    } serve(m);
     mf_status first = MF_OK;
     bool is_first = true;
     while (!st.done()) {

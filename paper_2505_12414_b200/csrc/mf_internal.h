@@ -31,6 +31,8 @@ struct mf_ctx {
     // device scratch of the many-points evaluation (mf_nll_grad_points / mf_nll_grad_sweep), shared by all models of the
     // context (every launch is ordered on the one stream, and the kernel touches the scratch only after its programmatic
     // wait): grow-only, laid out as [consts | ok | partials | bad | ticket] for the largest (points, chunks) seen so far
+    cudaStream_t server_stream = nullptr;  // resident evaluation kernels (mf_model_serve) run here, beside the work stream
+    std::vector<struct mf_model*> serving;  // models whose resident kernel may be running
     char* p_blk = nullptr;
     size_t p_bytes = 0;
     int64_t p_points = 0;
@@ -106,7 +108,22 @@ struct mf_model {
     double* s_sums = nullptr;         // device [NQ]
     unsigned* s_ticket = nullptr;     // device, one word, zero between launches
     double* s_out = nullptr;          // device [NOUT + 1] of the widest mode
+    // resident evaluation kernel (mf_server.cuh; mass model, n_toys == 1, unweighted)
+    bool srv_on = false;              // requested (mf_model_serve, or for the duration of mf_fit)
+    bool srv_running = false;         // a kernel has been launched and has not been seen to leave
+    int srv_failures = 0;             // relaunches that did not produce an answer (tools that serialise kernels): then disabled
+    unsigned long long srv_seq = 0;   // last request number issued
+    double* h_req = nullptr;          // mapped pinned request slot (64 words) and its device alias
+    double* d_req_mapped = nullptr;
+    void* srv_relay = nullptr;        // device: ServerRelay
+    double* srv_partials = nullptr;   // device [13][grid]
+    unsigned* srv_bad = nullptr;
+    unsigned* srv_ticket = nullptr;
 };
+
+// mf_api.cu: resident evaluation kernel
+mf_status mf_server_begin(mf_model* m);  // used by mf_fit: serve for the duration of the fit (no-op where not applicable)
+void mf_server_end(mf_model* m, bool was_on);
 
 // Sets ctx->err and returns st (mf_api.cu).
 mf_status mf_fail(mf_ctx* ctx, mf_status st, const std::string& msg);
