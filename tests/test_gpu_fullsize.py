@@ -116,6 +116,53 @@ def test_c3_full_size(mf, ctx):
     r = model.fit(dg.FOURD_TRUTH)
     o_nll, o_g, _ = oracle.nll_grad(oracle.FOURD, ev, r.lam, dg.MASS_LO, dg.MASS_HI, nthreads=oracle.max_threads())
     _check_full_size_fit(r, o_nll, o_g, dg.FOURD_TRUTH, "C3 fit")
+    assert r.n_calls <= 12, r.n_calls           # Newton on the analytic Hessian (round 1: 100 evaluations by finite differences)
+    # the 136-entry analytic Hessian and the Fisher matrix at full size (second-order kernel) against the oracle
+    nll, g, H, F = model.nll_grad_hess_fisher(dg.FOURD_TRUTH)
+    o = oracle.nll_grad_hess(oracle.FOURD, ev, dg.FOURD_TRUTH, dg.MASS_LO, dg.MASS_HI, want_fisher=True)
+    check(nll, g, o[0], o[1], "C3 second-order")
+    for A, B, what in ((H, o[2], "Hessian"), (F, o[3], "Fisher")):
+        scale = 1.0 + np.sqrt(np.abs(np.outer(np.diag(B), np.diag(B))))
+        assert np.all(np.abs(A - B) <= 1e-9 * scale), (what, np.max(np.abs(A - B) / scale))
+
+
+def test_c2_many_points_full_size(mf, ctx):
+    """Every point of a 64-point call on C2 (1e6 events, one pass over the data: mf_points.cuh) against the oracle."""
+    import torch
+    ev = dg.gen_angular(1_000_000, seed=2)
+    model = ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ctx.dataset_upload(ev))
+    pts = np.tile(np.array(dg.ANG_TRUTH), (64, 1)) + np.random.default_rng(5).uniform(-0.03, 0.03, (64, 8))
+    out = torch.full((64, 10), float("nan"), dtype=torch.float64, device="cuda")
+    model.nll_grad_points(pts, out.data_ptr())
+    torch.cuda.synchronize()
+    res = out.cpu().numpy()
+    assert np.all(res[:, 9] == 0)
+    for p in range(64):
+        o_nll, o_g, _ = oracle.nll_grad(oracle.ANGULAR, ev, pts[p], nthreads=oracle.max_threads())
+        check(res[p, 0], res[p, 1:9], o_nll, o_g, f"C2 point {p}")
+
+
+def test_c1_weighted_full_size(mf, ctx):
+    """C1's events with weights: value, gradient, Hessian and Fisher matrix at N = 1e6, and the weighted fit."""
+    m = dg.gen_mass(1_000_000, seed=1)
+    w = np.random.default_rng(91).choice([0.2, 1.8], m.size)
+    ds = ctx.dataset_upload(m, dg.MASS_LO, dg.MASS_HI)
+    ds.set_weights(w)
+    model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ds)
+    nll, g, H, F = model.nll_grad_hess_fisher(dg.MASS_START)
+    o = oracle.nll_grad_hess(oracle.MASS, m, dg.MASS_START, dg.MASS_LO, dg.MASS_HI, weights=w, want_fisher=True)
+    check(nll, g, o[0], o[1], "C1 weighted")
+    for A, B, what in ((H, o[2], "Hessian"), (F, o[3], "Fisher")):
+        scale = 1.0 + np.sqrt(np.abs(np.outer(np.diag(B), np.diag(B))))
+        assert np.all(np.abs(A - B) <= 1e-9 * scale), (what, np.max(np.abs(A - B) / scale))
+    r = model.fit(dg.MASS_START)
+    assert r.converged
+    o_nll, o_g, o_H, o_F, _ = oracle.nll_grad_hess(oracle.MASS, m, r.lam, dg.MASS_LO, dg.MASS_HI, weights=w, want_fisher=True)
+    Hi = np.linalg.inv(o_H)
+    sand = Hi @ o_F @ Hi                          # the oracle's sandwich covariance at the fitted point
+    sig = np.sqrt(np.diag(sand))
+    assert np.max(np.abs(Hi @ o_g) / sig) < 1e-6  # the oracle's Newton step from the fitted point
+    assert np.max(np.abs(r.cov - sand) / np.sqrt(np.outer(np.diag(sand), np.diag(sand)))) < 1e-6
 
 
 def test_c4_full_size(mf, ctx):
