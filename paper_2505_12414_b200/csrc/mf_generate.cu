@@ -16,6 +16,7 @@
 #include <string>
 
 #include "mf_internal.h"
+#include "mf_math.cuh"
 
 namespace {
 
@@ -24,8 +25,9 @@ __device__ __forceinline__ void philox4x32_10(unsigned c0, unsigned c1, unsigned
 {
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
-        const unsigned hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
-        const unsigned hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        const unsigned long long p0 = (unsigned long long)0xD2511F53u * c0, p1 = (unsigned long long)0xCD9E8D57u * c2;  // one wide multiply each
+        const unsigned hi0 = (unsigned)(p0 >> 32), lo0 = (unsigned)p0;
+        const unsigned hi1 = (unsigned)(p1 >> 32), lo1 = (unsigned)p1;
         const unsigned n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
         c0 = n0;
         c1 = lo1;
@@ -54,49 +56,62 @@ __device__ __forceinline__ void uniforms(unsigned long long seed, unsigned long 
     ub = uniform53(w[2], w[3]);
 }
 
-// data: [n_toys][n_pad]; the padding of each toy row repeats its last event (as mf_dataset_upload does)
+// data: [n_toys][n_pad]; the padding of each toy row repeats its last event (as mf_dataset_upload does).
+// grid = (slots, toys): no 64-bit division per event.  The transforms use the path's own logarithm (mf_log, table in
+// shared memory) and cospi instead of the library's log / log1p / cos (which made the kernel instruction-issue bound:
+// 785 us for 4.1e7 events); the results differ from the recipe evaluated with correctly rounded functions by a few ulp
+// of the Box-Muller variate and far less than an ulp of m for the background (ln(1 + x) with x in (-1, 0]: the absolute
+// error 1.1e-16 of forming 1 + x is divided by |tau| and added to lo ~ 5).
 __global__ void __launch_bounds__(256) generate_mass_kernel(double* __restrict__ data, int64_t n_toys, int64_t n, int64_t n_pad,
                                                             unsigned long long seed0, double f, double mu, double sigma,
-                                                            double tau, double lo, double hi, double em1)
+                                                            double tau, double lo, double hi, double em1, double inv_tau)
 {
+    __shared__ double2 s_tab[mf::kLogTableSize];
+    mf::load_log_table(s_tab);
+    __syncthreads();
     const double w = hi - lo;
-    for (int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; idx < n_toys * n_pad; idx += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t toy = idx / n_pad, slot = idx % n_pad;
-        if (n == 0) {
-            data[idx] = 0.0;
-            continue;
-        }
-        const unsigned long long ev = (unsigned long long)(slot < n ? slot : n - 1), seed = seed0 + (unsigned long long)toy;
-        double ua, ub, m;
-        uniforms(seed, ev, 0u, ua, ub);
-        if (ua < f) {
-            m = mu;
-            bool ok = false;
-            for (unsigned k = 1; k <= 64 && !ok; ++k) {
-                double u1, u2;
-                uniforms(seed, ev, k, u1, u2);
-                const double z = sqrt(-2.0 * log(u1)) * cos(2.0 * 3.141592653589793238462643383279502884 * u2);
-                m = fma(sigma, z, mu);
-                ok = (m >= lo && m <= hi);
+    for (int64_t toy = blockIdx.y; toy < n_toys; toy += gridDim.y) {
+        double* row = data + toy * n_pad;
+        const unsigned long long seed = seed0 + (unsigned long long)toy;
+        for (int64_t slot = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; slot < n_pad; slot += (int64_t)gridDim.x * blockDim.x) {
+            if (n == 0) {
+                row[slot] = 0.0;
+                continue;
             }
-            if (!ok) m = fmin(fmax(m, lo), hi);
-        } else {
-            m = (tau == 0.0) ? fma(ub, w, lo) : lo + log1p(ub * em1) / tau;
-            m = fmin(fmax(m, lo), hi);
+            const unsigned long long ev = (unsigned long long)(slot < n ? slot : n - 1);
+            double ua, ub, m;
+            uniforms(seed, ev, 0u, ua, ub);
+            if (ua < f) {
+                m = mu;
+                bool ok = false;
+                for (unsigned k = 1; k <= 64 && !ok; ++k) {
+                    double u1, u2;
+                    uniforms(seed, ev, k, u1, u2);
+                    const double z = sqrt(-2.0 * mf::mf_log(u1, s_tab)) * cospi(2.0 * u2);
+                    m = fma(sigma, z, mu);
+                    ok = (m >= lo && m <= hi);
+                }
+                if (!ok) m = fmin(fmax(m, lo), hi);
+            } else {
+                m = (tau == 0.0) ? fma(ub, w, lo) : fma(mf::mf_log(fma(ub, em1, 1.0), s_tab), inv_tau, lo);
+                m = fmin(fmax(m, lo), hi);
+            }
+            row[slot] = m;
         }
-        data[idx] = m;
     }
 }
 
 // Eq. 4, term by term, for the accept decision
-__device__ __forceinline__ double angular_pdf(double cl, double ck, double phi, const double* a)
+// phi = pi phi_turns: sine and cosine by sincospi of the half-turn count (no argument reduction of a rounded phi), the
+// double angle by the addition formulas
+__device__ __forceinline__ double angular_pdf(double cl, double ck, double phi_turns, const double* a)
 {
     const double cl2 = cl * cl, ck2 = ck * ck, sl2 = 1.0 - cl2, sk2 = 1.0 - ck2;
     const double sl = sqrt(sl2), sk = sqrt(sk2);
     const double c2l = 2.0 * cl2 - 1.0, s2l = 2.0 * sl * cl, s2k = 2.0 * sk * ck;
-    double sp, cp, s2p, c2p;
-    sincos(phi, &sp, &cp);
-    sincos(2.0 * phi, &s2p, &c2p);
+    double sp, cp;
+    sincospi(phi_turns, &sp, &cp);
+    const double s2p = 2.0 * sp * cp, c2p = (cp - sp) * (cp + sp);
     const double FL = a[0];
     return (9.0 / (32.0 * 3.141592653589793238462643383279502884)) *
            (0.75 * (1.0 - FL) * sk2 + FL * ck2 + 0.25 * (1.0 - FL) * sk2 * c2l - FL * ck2 * c2l + a[1] * sk2 * sl2 * c2p +
@@ -126,7 +141,7 @@ __global__ void __launch_bounds__(256) generate_angular_kernel(double* __restric
                 cl = 2.0 * u1 - 1.0;
                 ck = 2.0 * u2 - 1.0;
                 phi = 3.141592653589793238462643383279502884 * (2.0 * u3 - 1.0);
-                if (u4 * g.pmax < angular_pdf(cl, ck, phi, g.a)) break;
+                if (u4 * g.pmax < angular_pdf(cl, ck, 2.0 * u3 - 1.0, g.a)) break;
             }
         }
         data[idx] = cl;
@@ -181,7 +196,7 @@ __global__ void __launch_bounds__(256) generate_4d_kernel(double* __restrict__ d
                     cl = 2.0 * u1 - 1.0;
                     ck = 2.0 * u2 - 1.0;
                     phi = pi * (2.0 * u3 - 1.0);
-                    if (u4 * g.ang.pmax < angular_pdf(cl, ck, phi, g.ang.a)) break;
+                    if (u4 * g.ang.pmax < angular_pdf(cl, ck, 2.0 * u3 - 1.0, g.ang.a)) break;
                 }
             } else {
                 const double w = g.hi - g.lo;
@@ -362,9 +377,10 @@ extern "C" mf_status mf_generate_mass(mf_ctx* ctx, uint64_t seed0, int64_t n_toy
     buf->bytes = (size_t)(total > 0 ? total : 1) * sizeof(double);
     cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&buf->p), buf->bytes, ctx->stream);
     if (e == cudaSuccess && total > 0) {
-        const int grid = (int)std::min<int64_t>((total + 255) / 256, 32 * (int64_t)ctx->sm_count);
-        generate_mass_kernel<<<grid, 256, 0, ctx->stream>>>(buf->p, n_toys, n_events, ds->n_pad, seed0, f, mu, sigma, tau, lo, hi,
-                                                             std::expm1(tau * (hi - lo)));
+        const unsigned gy = (unsigned)std::min<int64_t>(n_toys, 65535);
+        const unsigned gx = (unsigned)std::max<int64_t>(1, std::min<int64_t>((ds->n_pad + 255) / 256, 32 * (int64_t)ctx->sm_count / gy));
+        generate_mass_kernel<<<dim3(gx, gy), 256, 0, ctx->stream>>>(buf->p, n_toys, n_events, ds->n_pad, seed0, f, mu, sigma, tau, lo,
+                                                                     hi, std::expm1(tau * (hi - lo)), tau != 0.0 ? 1.0 / tau : 0.0);
         ++ctx->launches;
         e = cudaGetLastError();
     }
