@@ -614,6 +614,7 @@ def run_mine(args) -> None:
     n_sm = torch.cuda.get_device_properties(local).multi_processor_count
     peak_tflops = 2.0 * n_sm * NOMINAL_FP64_LANES_PER_SM * sm_max_mhz * 1e6 / 1e12
     measured_rate = probe.fp64_rate(local, torch.cuda.current_stream(local).cuda_stream)
+    dmma = probe.dmma_rate(local, torch.cuda.current_stream(local).cuda_stream)   # fp64 tensor-core rate, DMMA + DFMA mix
     n_launches_timed = max(int(launches), 1)
     us_per_launch = 1e3 * ms / n_launches_timed
     achieved_tflops = 2.0 * MASS_FP64_INSTR_PER_EVENT * N_EVENTS * POINTS_PER_CALL / (us_per_launch * 1e-6) / 1e12
@@ -630,6 +631,8 @@ def run_mine(args) -> None:
         "launches_timed": n_launches_timed, "us_per_launch": us_per_launch, "evaluations_per_launch": POINTS_PER_CALL,
         "peak_how": f"derived: {n_sm} SMs x {NOMINAL_FP64_LANES_PER_SM} fp64 lanes x {sm_max_mhz:.0f} MHz x 2 flop",
         "peak_measured_dfma_chain": 2.0 * measured_rate / 1e12,
+        "peak_measured_dmma": 2.0 * dmma["dmma_fma_per_s"] / 1e12,
+        "dmma_plus_dfma_time_over_sum_of_times": dmma["mix_4dmma_8dfma_vs_sum"],
         "frac_of_measured_dfma_chain": achieved_tflops / (2.0 * measured_rate / 1e12),
         "one_launch_per_evaluation": {"us_per_evaluation": single_us, "evaluations": n_single, "gpu_launches": int(single_launches),
                                       "events_per_s": world * N_EVENTS / (single_us * 1e-6),
