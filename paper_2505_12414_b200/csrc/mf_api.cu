@@ -17,6 +17,7 @@
 #include "mf_kernels.cuh"
 #include "mf_second.cuh"
 #include "mf_points.cuh"
+#include "mf_points4d.cuh"
 #include "mf_server.cuh"
 
 using namespace mf;
@@ -874,6 +875,100 @@ static mf_status launch_points_angular_mma(mf_model* m, int64_t n_points, const 
     return MF_OK;
 }
 
+// The 4D model's many-points evaluation in one pass over the data (mf_points4d.cuh): 32 points per pass.  out_dev rows are
+// K + 2 = 18 doubles.  *handled = false: a point has f = 0 or f = 1 exactly (ln f and 1/f, 1/(1-f) are folded into the
+// per-point constants): the caller uses the (point, chunk) kernel.
+static mf_status launch_points_fourd_mma(mf_model* m, int64_t n_points, const double* lambdas, double* out_dev, bool* handled)
+{
+    mf_ctx* ctx = m->ctx;
+    *handled = true;
+    const int64_t n_groups = m->n_pad / 8;
+    const int G = (int)std::max<int64_t>(1, std::min<int64_t>((n_groups + kWarps - 1) / kWarps, 2 * (int64_t)ctx->sm_count));  // 2 CTAs per SM
+    char* h_blk = nullptr;
+    int stage = 0;
+    const size_t per_point = sizeof(double) * (16 + kP4PointConsts + kP4FinishConsts);
+    static_assert(sizeof(double) * (16 + kP4PointConsts + kP4FinishConsts) <= sizeof(FourDConsts), "per-point block fits the scratch layout");
+    MF_CUDA(ctx, points_stage(ctx, per_point * n_points, &h_blk, &stage));
+    double* h_coef = reinterpret_cast<double*>(h_blk);
+    double* h_pc = h_coef + 16 * n_points;
+    double* h_fc = h_pc + kP4PointConsts * n_points;
+    const double mref = 0.5 * (m->ma + m->mb);
+    for (int64_t p = 0; p < n_points; ++p) {
+        const double* lam = lambdas + p * 16;
+        FourDConsts c;
+        if (!fourd_consts(lam, m->ma, m->mb, c))
+            return mf_fail(ctx, MF_ERR_PARAM_DOMAIN, "mf_nll_grad_points: lambda " + std::to_string((long long)p) +
+                                                         " is outside the parameter domain");
+        if (!(c.m.f > 0.0 && c.m.f < 1.0)) {
+            *handled = false;
+            return MF_OK;
+        }
+        std::memcpy(h_coef + 16 * p, lam, sizeof(double) * 16);
+        double* pc = h_pc + kP4PointConsts * p;
+        pc[0] = c.m.mu - mref;
+        pc[1] = c.m.nb0;
+        pc[2] = c.m.tau;
+        pc[3] = c.m.lnk - c.m.tau * mref + std::log(c.m.f);
+        pc[4] = c.m.is2;
+        pc[5] = c.m.kmu;
+        pc[6] = c.m.is3;
+        pc[7] = c.m.ksig;
+        pc[8] = (mref - c.m.ma) - c.m.ktau;
+        pc[9] = 0.0;
+        double* fc = h_fc + kP4FinishConsts * p;
+        fc[0] = 1.0 / c.m.f;
+        fc[1] = 1.0 / c.m.omf;
+        fc[2] = c.m.tau;
+        fc[3] = c.m.lnc2;
+        fc[4] = c.kappa;
+        fc[5] = 0.0;
+    }
+    {
+        const mf_status ss = points_scratch(ctx, n_points, G);
+        if (ss != MF_OK) return ss;
+    }
+    auto up = [](size_t x) { return (x + 255) / 256 * 256; };
+    const int64_t P = ctx->p_points;
+    const int C = ctx->p_chunks;
+    FourDPointsArgs a;
+    for (int i = 0; i < 12; ++i) a.col[i] = m->col[i];
+    a.n = m->n_events;
+    a.n_pad = m->n_pad;
+    a.mref = mref;
+    char* q = ctx->p_blk;
+    double* d_blk = reinterpret_cast<double*>(q);
+    a.coef = d_blk;
+    a.pconst = d_blk + 16 * n_points;
+    const double* d_fc = d_blk + (16 + kP4PointConsts) * n_points;
+    q += up(sizeof(FourDConsts) * P) + up(sizeof(int) * P);
+    a.partials = reinterpret_cast<double*>(q);
+    q += up(sizeof(double) * P * MF_MAX_NACC * C);
+    a.bad_partials = reinterpret_cast<unsigned*>(q);
+    a.n_points = (int)n_points;
+    MF_CUDA(ctx, cudaMemcpyAsync(d_blk, h_blk, per_point * n_points, cudaMemcpyHostToDevice, ctx->stream));
+    MF_CUDA(ctx, cudaEventRecord(ctx->pts_copied[stage], ctx->stream));
+    take_fresh(m);
+    static const int pass_env4 = std::getenv("MF_POINTS4D_PER_PASS") ? std::atoi(std::getenv("MF_POINTS4D_PER_PASS")) : 0;  // tuning knob
+    const int per_pass = (pass_env4 == 16 || pass_env4 == 24 || pass_env4 == 32) ? pass_env4 : 16;
+    const dim3 grid((unsigned)G, (unsigned)((n_points + per_pass - 1) / per_pass));
+    const size_t smem4 = sizeof(double) * 2 * kBlock * kP4StageDoubles;  // 48 KB: above the default dynamic limit with the static part
+    static const cudaError_t attr4 = [&] {
+        cudaError_t e = cudaFuncSetAttribute(fourd_points_mma_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem4);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(fourd_points_mma_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem4);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(fourd_points_mma_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem4);
+        return e;
+    }();
+    MF_CUDA(ctx, attr4);
+    if (per_pass == 32) fourd_points_mma_kernel<4><<<grid, kBlock, smem4, ctx->stream>>>(a);
+    else if (per_pass == 24) fourd_points_mma_kernel<3><<<grid, kBlock, smem4, ctx->stream>>>(a);
+    else fourd_points_mma_kernel<2><<<grid, kBlock, smem4, ctx->stream>>>(a);
+    fourd_points_combine_kernel<<<(unsigned)((n_points + kWarps - 1) / kWarps), kBlock, 0, ctx->stream>>>(
+        a.partials, a.bad_partials, G, (int)n_points, d_fc, m->d_sum_m, (double)m->n_events, out_dev);
+    MF_CUDA(ctx, cudaGetLastError());
+    ctx->launches += 2;
+    return MF_OK;
+}
+
 template <class M>
 static mf_status launch_points(mf_model* m, int64_t n_points, const double* lambdas, double* out_dev)
 {
@@ -966,7 +1061,15 @@ extern "C" mf_status mf_nll_grad_points(mf_model* m, int64_t n_points, const dou
         return no_mma ? launch_points<AngularModel>(m, n_points, lambdas, out_dev)
                       : launch_points_angular_mma(m, n_points, lambdas, out_dev);
     }
-    default: return launch_points<FourDModel>(m, n_points, lambdas, out_dev);
+    default: {
+        static const bool no_mma4 = std::getenv("MF_NO_POINTS_MMA") != nullptr;
+        if (!no_mma4) {
+            bool handled = false;
+            const mf_status st = launch_points_fourd_mma(m, n_points, lambdas, out_dev, &handled);
+            if (handled || st != MF_OK) return st;
+        }
+        return launch_points<FourDModel>(m, n_points, lambdas, out_dev);
+    }
     }
 }
 

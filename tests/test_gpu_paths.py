@@ -99,9 +99,10 @@ def test_points_mode_angular_bad_point(mf, ctx):
     assert e.value.status == mf.MF_ERR_PARAM_DOMAIN
 
 
-@pytest.mark.parametrize("n,n_pts", [(30_001, 16), (100_000, 64)])
+@pytest.mark.parametrize("n,n_pts", [(30_001, 16), (100_000, 64), (1, 16), (10_007, 17), (5_000, 41)])
 def test_points_mode_fourd_vs_oracle(mf, ctx, n, n_pts):
-    """launch_points<FourDModel>: every row against the oracle."""
+    """The 4D many-points kernel (mf_points4d.cuh: one pass over the data per 16 points, tensor-core contractions around
+    the per-pair exponential): every row against the oracle, ragged event counts, partly filled point blocks."""
     import torch
     ev = dg.gen_4d(n, seed=23)
     model = ctx.model_create(mf.MF_MASS_X_ANGULAR, ctx.dataset_upload(ev, dg.MASS_LO, dg.MASS_HI))
@@ -114,6 +115,38 @@ def test_points_mode_fourd_vs_oracle(mf, ctx, n, n_pts):
     for p in range(n_pts):
         o_nll, o_g, _ = oracle.nll_grad(oracle.FOURD, ev, pts[p], dg.MASS_LO, dg.MASS_HI, nthreads=oracle.max_threads())
         check(res[p, 0], res[p, 1:17], o_nll, o_g, f"4D points row {p}")
+
+
+def test_points_mode_fourd_edge_points(mf, ctx):
+    """Points with f = 0 or f = 1 exactly go through the (point, chunk) kernel (the one-pass kernel folds ln f, 1/f and
+    1/(1-f) into its constants); a point outside the parameter domain is refused; a point with P <= 0 events is flagged."""
+    import torch
+    ev = dg.gen_4d(6_000, seed=24)
+    model = ctx.model_create(mf.MF_MASS_X_ANGULAR, ctx.dataset_upload(ev, dg.MASS_LO, dg.MASS_HI))
+    pts = _fourd_points(20, 8)
+    pts[5, 0] = 0.0
+    pts[9, 0] = 1.0
+    out = torch.full((20, 18), float("nan"), dtype=torch.float64, device="cuda")
+    model.nll_grad_points(pts, out.data_ptr())
+    torch.cuda.synchronize()
+    res = out.cpu().numpy()
+    for p in (4, 5, 9, 19):
+        o_nll, o_g, nbad = oracle.nll_grad(oracle.FOURD, ev, pts[p], dg.MASS_LO, dg.MASS_HI)
+        assert nbad == 0 and res[p, 17] == 0
+        check(res[p, 0], res[p, 1:17], o_nll, o_g, f"4D edge row {p}")
+    pts = _fourd_points(20, 8)
+    pts[7, 5] = 5.0                       # S3 = 5: the signal's angular PDF goes negative for many events
+    model.nll_grad_points(pts, out.data_ptr())
+    torch.cuda.synchronize()
+    res = out.cpu().numpy()
+    _, _, nbad = oracle.nll_grad(oracle.FOURD, ev, pts[7], dg.MASS_LO, dg.MASS_HI)
+    assert nbad > 0 and res[7, 17] == nbad and res[7, 0] == math.inf and np.all(np.isnan(res[7, 1:17]))
+    o_nll, o_g, _ = oracle.nll_grad(oracle.FOURD, ev, pts[8], dg.MASS_LO, dg.MASS_HI)
+    check(res[8, 0], res[8, 1:17], o_nll, o_g, "row beside a bad point")
+    pts[3, 2] = -0.01                     # sigma < 0
+    with pytest.raises(mf.MoreFitError) as e:
+        model.nll_grad_points(pts, out.data_ptr())
+    assert e.value.status == mf.MF_ERR_PARAM_DOMAIN
 
 
 @pytest.mark.parametrize("n", [3000, 40_001])
