@@ -835,7 +835,9 @@ static mf_status launch_points_angular_mma(mf_model* m, int64_t n_points, const 
                                                          " is outside the parameter domain");
     const int64_t n_groups = m->n_pad / 8;
     static const int pass_env = std::getenv("MF_POINTS_PER_PASS") ? std::atoi(std::getenv("MF_POINTS_PER_PASS")) : 0;  // tuning knob
-    const int per_pass = (pass_env == 16 || pass_env == 32 || pass_env == 64) ? pass_env : n_points > 32 ? 64 : n_points > 16 ? 32 : 16;
+    // measured (C2, 1e6 events): 32 points per pass at 2 CTAs per SM (124 registers) 1.62 us per evaluation at 1000 points,
+    // 64 per pass at 1 CTA per SM (212 registers) 1.85 us
+    const int per_pass = (pass_env == 16 || pass_env == 32 || pass_env == 64) ? pass_env : n_points > 16 ? 32 : 16;
     const int ctas_per_sm = per_pass == 64 ? 1 : 2;
     const int G = (int)std::max<int64_t>(1, std::min<int64_t>((n_groups + kWarps - 1) / kWarps, ctas_per_sm * (int64_t)ctx->sm_count));
     {
@@ -865,9 +867,9 @@ static mf_status launch_points_angular_mma(mf_model* m, int64_t n_points, const 
     MF_CUDA(ctx, cudaEventRecord(ctx->pts_copied[stage], ctx->stream));
     take_fresh(m);
     const dim3 grid((unsigned)G, (unsigned)((n_points + per_pass - 1) / per_pass));
-    if (per_pass == 64) angular_points_mma_kernel<8><<<grid, kBlock, 0, ctx->stream>>>(a);
-    else if (per_pass == 32) angular_points_mma_kernel<4><<<grid, kBlock, 0, ctx->stream>>>(a);
-    else angular_points_mma_kernel<2><<<grid, kBlock, 0, ctx->stream>>>(a);
+    if (per_pass == 64) angular_points_mma_kernel<8><<<grid, kBlock, ang_points_smem<8>(), ctx->stream>>>(a);
+    else if (per_pass == 32) angular_points_mma_kernel<4><<<grid, kBlock, ang_points_smem<4>(), ctx->stream>>>(a);
+    else angular_points_mma_kernel<2><<<grid, kBlock, ang_points_smem<2>(), ctx->stream>>>(a);
     angular_points_combine_kernel<<<(unsigned)((n_points + kWarps - 1) / kWarps), kBlock, 0, ctx->stream>>>(
         a.partials, a.bad_partials, G, (int)n_points, out_dev);
     MF_CUDA(ctx, cudaGetLastError());

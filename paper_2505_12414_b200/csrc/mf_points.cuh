@@ -13,8 +13,8 @@
 //           P(point g; events 2t, 2t+1);
 //   step 2: A = r (8 points x 4 events) — exactly the two values each lane already holds if k-step j takes events
 //           {2t + j}: no transposition, no shuffle; B = h_{1+g}(event 2t + j), one 16-byte load -> G tile (8 points x 8 k).
-// Every 8-event group is loaded once (two layouts, 576 B each, straight from L2 / HBM in 64-byte segments) and serves all
-// the points of the pass, so the arithmetic intensity grows with M and the kernel is bound by the fp64 pipe: per
+// Every 8-event group is fetched once per pass (two layouts, 576 B each, 64-byte segments from L2 / HBM, staged per lane in
+// shared memory by cp.async so that the loads in flight cost no registers) and serves all the points of the pass, so the arithmetic intensity grows with M and the kernel is bound by the fp64 pipe: per
 // (point, event) pair 4/64 DMMA (each holds the pipe of its SM sub-partition for 16 clocks) + one reciprocal (3 DFMA) + one
 // DMUL, i.e. 0.31 pipe-clocks per pair per SM, the same as the hand-written DFMA form — which however issues 2.4
 // instructions per pair instead of 0.6 and whose three-register DFMAs run at 2/3 rate.
@@ -33,11 +33,21 @@ struct AngPointsArgs {
     unsigned* bad_partials; // [n_points][G]
 };
 
-// NPB point blocks of 8 points per CTA pass; grid = (G, ceil(n_points / (8 NPB))).
+// NPB point blocks of 8 points per CTA pass; grid = (G, ceil(n_points / (8 NPB))); dynamic shared memory: ang_points_smem<NPB>().
+template <int NPB>
+constexpr size_t ang_points_smem()
+{
+    return sizeof(double) * ((2 * kBlock * 6 > kWarps * NPB * 8 * 9) ? 2 * kBlock * 6 : kWarps * NPB * 8 * 9);
+}
+
 template <int NPB>
 __global__ void __launch_bounds__(kBlock, (NPB <= 4) ? 2 : 1) angular_points_mma_kernel(const __grid_constant__ AngPointsArgs a)
 {
-    __shared__ double red[kWarps][NPB][8][9];
+    // dynamic shared memory: per-lane staging of the event fragments (two stages filled by cp.async: loads in flight cost no
+    // registers), reused after the event loop for the cross-warp reduction
+    extern __shared__ __align__(16) unsigned char ap_raw[];
+    double (*stg)[kBlock][6] = reinterpret_cast<double (*)[kBlock][6]>(ap_raw);
+    double (*red)[NPB][8][9] = reinterpret_cast<double (*)[NPB][8][9]>(ap_raw);
     __shared__ unsigned red_bad[kWarps][NPB][8];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int fg = lane >> 2, ft = lane & 3;
@@ -67,12 +77,22 @@ __global__ void __launch_bounds__(kBlock, (NPB <= 4) ? 2 : 1) angular_points_mma
         double f1[2];
         double2 f2, f0;
     };
-    auto load = [&](int64_t grp, Frag& f) {
+    // issue: this lane's values of group grp -> stage st (asynchronous copies); fetch: stage st -> fragments
+    auto issue = [&](int64_t grp, int st) {
         const int64_t e0 = grp * 8;
-        f.f1[0] = __ldg(a.col[1 + ft] + e0 + fg);
-        f.f1[1] = __ldg(a.col[5 + ft] + e0 + fg);
-        f.f2 = __ldg(reinterpret_cast<const double2*>(a.col[1 + fg] + e0) + ft);
-        f.f0 = __ldg(reinterpret_cast<const double2*>(a.col[0] + e0) + ft);
+        const unsigned dst = (unsigned)__cvta_generic_to_shared(&stg[st][threadIdx.x][0]);
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(a.col[1 + ft] + e0 + fg) : "memory");
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst + 8u), "l"(a.col[5 + ft] + e0 + fg) : "memory");
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst + 16u), "l"(a.col[1 + fg] + e0 + 2 * ft) : "memory");
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst + 32u), "l"(a.col[0] + e0 + 2 * ft) : "memory");
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    auto fetch = [&](int st, Frag& f) {
+        const double* q = &stg[st][threadIdx.x][0];
+        f.f1[0] = q[0];
+        f.f1[1] = q[1];
+        f.f2 = *reinterpret_cast<const double2*>(q + 2);
+        f.f0 = *reinterpret_cast<const double2*>(q + 4);
     };
     // One group for all the point blocks of the pass, written stage by stage across the NPB independent blocks so that
     // dependent instructions are NPB apart.  Only the dataset's last groups can hold padded events (copies of the last
@@ -121,26 +141,29 @@ __global__ void __launch_bounds__(kBlock, (NPB <= 4) ? 2 : 1) angular_points_mma
             lp[pb].mul(c[pb][1], bad[pb]);
         }
     };
-    // two fragment buffers used alternately (no register copies, which would wait for the loads): the next group of this
-    // warp is in flight while the current one is evaluated
-    Frag fa, fb;
     int64_t gi = blockIdx.x + G * warp;
     unsigned since_renorm = 0;
-    if (gi < n_groups) load(gi, fa);
+    int st = 0;
+    if (gi < n_groups) issue(gi, 0);
     while (gi < n_groups) {
-        if (gi + step < n_groups) load(gi + step, fb);
-        process(gi, fa);
+        if (gi + step < n_groups) {
+            issue(gi + step, st ^ 1);
+            asm volatile("cp.async.wait_group 1;" ::: "memory");  // everything but the group just requested has landed
+        } else {
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+        }
+        Frag f;
+        fetch(st, f);
+        process(gi, f);
         gi += step;
-        if (gi >= n_groups) break;
-        if (gi + step < n_groups) load(gi + step, fa);
-        process(gi, fb);
-        gi += step;
-        if (++since_renorm == 128) {  // 512 mantissas in [1, 2) per running product since the last one
+        st ^= 1;
+        if (++since_renorm == 256) {  // 512 mantissas in [1, 2) per running product since the last one
             since_renorm = 0;
 #pragma unroll
             for (int pb = 0; pb < NPB; ++pb) lp[pb].renorm();
         }
     }
+    __syncthreads();  // the staging area becomes the reduction buffer
     // lane (fg, ft): ln of the product over its events for point fg of every block; sum over the four ft lanes
 #pragma unroll
     for (int pb = 0; pb < NPB; ++pb) {
