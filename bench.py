@@ -290,7 +290,7 @@ def _other_workloads(torch, mf, ctx, peaks, traffic_all) -> dict:
         # pipe work per (point, event) pair: 4/64 DMMA of 256 FMAs + reciprocal (3 DFMA) + 1 DMUL = 20 FMA-equivalents
         mp[f"us_per_evaluation_{M}_points"] = usM
         mp[f"frac_of_fp64_peak_{M}_points"] = 20.0 * 1e6 / (usM * 1e-6) / (n_sm_ * NOMINAL_FP64_LANES_PER_SM * sm_mhz_ * 1e6)
-    mp["kernel"] = "angular_points_mma_kernel<8> + angular_points_combine_kernel (mf_nll_grad_points)"
+    mp["kernel"] = "angular_points_mma_kernel<4> + angular_points_combine_kernel (mf_nll_grad_points), 32 points per pass"
     mp["bound"] = "alu (fp64 pipe, DMMA shares it with DFMA): 20 FMA-equivalents per (point, event) pair incl. tile padding"
     res["C2_angular_1e6"]["many_points"] = mp
     del ms, ev
@@ -305,6 +305,27 @@ def _other_workloads(torch, mf, ctx, peaks, traffic_all) -> dict:
                                      "frac": gbs / hbm if hbm else None, "bytes_per_event": 96,
                                      "traffic": traffic_all.get("nll_grad_tma_kernel<FourDModel>")},
                         "l2": "2 model replicas x 192 MB of columns, alternating every evaluation"}
+    # many parameter points in ONE pass over the data per 16 points (mf_points4d.cuh)
+    mp4 = {}
+    for M in (64, 256):
+        ptsM = np.tile(np.array(dg.FOURD_TRUTH), (M, 1))
+        ptsM += np.random.default_rng(6).uniform(-1, 1, (M, 16)) * np.array([0.02, 0.002, 0.001, 0.2] + [0.03] * 8 + [0.05] * 4)
+        oM = torch.zeros((M, 18), dtype=torch.float64, device="cuda")
+        for _ in range(2):
+            m4.nll_grad_points(ptsM, oM.data_ptr())
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for i_ in range(6):
+            m4s[i_ % 2].nll_grad_points(ptsM, oM.data_ptr())
+        e1.record()
+        torch.cuda.synchronize()
+        if not np.all(np.isfinite(oM.cpu().numpy()[:, :17])):
+            raise RuntimeError("non-finite result in the 4D many-points workload")
+        mp4[f"us_per_evaluation_{M}_points"] = float(e0.elapsed_time(e1)) * 1e3 / 6 / M
+    mp4["kernel"] = "fourd_points_mma_kernel<2> + fourd_points_combine_kernel (mf_nll_grad_points), 16 points per pass"
+    mp4["single_launch_us_per_evaluation"] = us
+    res["C3_4d_2e6"]["many_points"] = mp4
     m4.fit(dg.FOURD_TRUTH)
     t = time.perf_counter()
     r = m4.fit(dg.FOURD_TRUTH)
