@@ -410,14 +410,18 @@ class Model:
         self.n_toys = int(self._lib.mf_model_n_toys(self._h))
 
     def nll_grad(self, lam, want_grad: bool = True):
-        """(-ln L, gradient) at lam; raises MoreFitError on a domain error or P <= 0."""
-        lam = np.ascontiguousarray(lam, dtype=np.float64)
-        if lam.shape != (self.K,):
-            raise ValueError(f"lambda must have {self.K} entries")
-        nll = ctypes.c_double()
-        grad = np.empty(self.K, dtype=np.float64)
-        self._ctx._check(self._lib.mf_nll_grad(self._h, _dp(lam), ctypes.byref(nll), _dp(grad) if want_grad else None))
-        return float(nll.value), (grad if want_grad else None)
+        """(-ln L, gradient) at lam; raises MoreFitError on a domain error or P <= 0.  (Marshalling buffers and their
+        pointers are made once per model: this call is what a minimiser loops over.)"""
+        io = self.__dict__.get("_io")
+        if io is None:
+            lam_b, grad_b, nll_b = np.empty(self.K), np.empty(self.K), ctypes.c_double()
+            io = self._io = (lam_b, grad_b, nll_b, _dp(lam_b), _dp(grad_b), ctypes.byref(nll_b), self._lib.mf_nll_grad)
+        lam_b, grad_b, nll_b, p_lam, p_grad, p_nll, fn = io
+        lam_b[:] = lam                       # raises on a wrong length; converts to float64
+        st = fn(self._h, p_lam, p_nll, p_grad if want_grad else None)
+        if st != MF_OK:
+            self._ctx._check(st)
+        return nll_b.value, (grad_b.copy() if want_grad else None)
 
     def nll_grad_status(self, lam):
         """Like nll_grad but returns (status, nll, grad) instead of raising."""
