@@ -219,9 +219,7 @@ int mf_model_is_served(const mf_model* model);
 
 /* ---- value + gradient + analytic Hessian ---------------------- */
 
-/* 1 if the analytic Hessian is available for this model: every family on a single dataset (n_toys == 1); with
- * n_toys > 1 (mf_nll_grad_hess_batch) the mass and angular families (the fit driver then uses finite differences of the
- * gradient for batched 4D toys). */
+/* 1 if the analytic Hessian is available for this model (every family, single datasets and batched toys). */
 int mf_model_has_hessian(const mf_model* model);
 /* 1 if the model was created on a dataset with event weights. */
 int mf_model_is_weighted(const mf_model* model);
@@ -241,7 +239,8 @@ mf_status mf_nll_grad_hess(mf_model* model, const double* lambda, double* nll, d
 mf_status mf_nll_grad_hess_fisher(mf_model* model, const double* lambda, double* nll, double* grad, double* hess,
                                   double* fisher);
 
-/* As mf_nll_grad_batch, plus hess (host, [n_toys][K*K]); inactive toys are left untouched. */
+/* As mf_nll_grad_batch, plus hess (host, [n_toys][K*K]); inactive toys are left untouched.  Mass and angular families: one
+ * launch for all toys; the 4D family: the second-order kernel toy by toy, in stream order, one synchronisation at the end. */
 mf_status mf_nll_grad_hess_batch(mf_model* model, int64_t n_toys, const double* lambdas, const uint8_t* active,
                                  double* nll, double* grad, double* hess);
 

@@ -494,7 +494,7 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
         MF_CUDA_M(dev_alloc(ctx, &m->d_consts, sizeof(FourDConsts) * T));  // the largest Consts
         MF_CUDA_M(dev_alloc(ctx, &m->d_consts_ok, sizeof(int) * T));
         MF_CUDA_M(dev_alloc(ctx, &m->d_ids, sizeof(int) * T));
-        const int nout1 = (kind == MF_MASS_GAUSS_EXP ? MassHessModel::NOUT : kind == MF_ANGULAR_KSTMUMU ? AngularHessModel::NOUT : K + 1) + 1;  // widest output row + n_bad
+        const int nout1 = 1 + K + K * (K + 1) / 2 + 1;  // widest output row (value, gradient, Hessian triangle) + n_bad
         MF_CUDA_M(dev_alloc(ctx, &m->d_bout, sizeof(double) * T * nout1));
         m->bout_row = nout1;  // the pinned staging of these arrays lives in the context (stage_views)
     }
@@ -660,7 +660,7 @@ static mf_status stage_reserve(mf_ctx* ctx, size_t bytes)
 // MODE 0: -ln L and gradient; 1: + Hessian; 2: + Fisher matrix sum w^2 s s^T.  out_dev NULL = the model's own buffer.
 // Output row: -ln L, gradient [K], Hessian upper triangle row by row [K(K+1)/2], Fisher likewise, n_bad.
 template <class S, int MODE>
-static mf_status launch_second(mf_model* m, const double* lam, double* out_dev)
+static mf_status launch_second(mf_model* m, const double* lam, double* out_dev, int64_t toy = 0)
 {
     using L = SecondLayout<S, MODE>;
     using LW = SecondLayout<S, 2>;  // scratch is sized for the widest mode
@@ -677,7 +677,7 @@ static mf_status launch_second(mf_model* m, const double* lam, double* out_dev)
         MF_CUDA(ctx, cudaMemsetAsync(m->s_ticket, 0, sizeof(unsigned), ctx->stream));
         MF_CUDA(ctx, dev_alloc(ctx, &m->s_out, sizeof(double) * (LW::NOUT + 1)));
     }
-    for (int i = 0; i < S::NCOL; ++i) a.col[i] = m->col[i];
+    for (int i = 0; i < S::NCOL; ++i) a.col[i] = m->col[i] + toy * m->n_pad;  // columns are [toy][n_pad]
     a.w = m->wts ? m->wts->p : nullptr;
     a.n = m->n_events;
     a.n_pad = m->n_pad;
@@ -1349,12 +1349,8 @@ extern "C" mf_status mf_nll_grad_hess_fisher(mf_model* m, const double* lambda, 
     return second_sync(m, lambda, nll, grad, hess, fisher, "mf_nll_grad_hess_fisher");
 }
 
-// 1: mf_nll_grad_hess is available (every family on a single dataset; batched toys: mass and angular families)
-extern "C" int mf_model_has_hessian(const mf_model* m)
-{
-    if (!m) return 0;
-    return (m->n_toys == 1 || m->kind == MF_MASS_GAUSS_EXP || m->kind == MF_ANGULAR_KSTMUMU) ? 1 : 0;
-}
+// 1: the analytic Hessian is available (every family, single datasets and batched toys)
+extern "C" int mf_model_has_hessian(const mf_model* m) { return m ? 1 : 0; }
 
 extern "C" int mf_model_is_weighted(const mf_model* m) { return m && m->wts ? 1 : 0; }
 
@@ -1408,8 +1404,6 @@ static mf_status eval_batch(mf_model* m, int64_t n_toys, const double* lambdas, 
     mf_ctx* ctx = m->ctx;
     const int K = m->K;
     if (n_toys != m->n_toys) return mf_fail(ctx, MF_ERR_ARG, std::string(who) + ": n_toys does not match the dataset");
-    if (hess && !mf_model_has_hessian(m))
-        return mf_fail(ctx, MF_ERR_ARG, "no batched analytic Hessian kernel for this model family (MF_MASS_X_ANGULAR)");
     if (m->n_toys < 2 && !m->d_lam) {
         // a 1-toy dataset evaluated through the batch entry: same result as the single call
         if (active && !active[0]) return MF_OK;
@@ -1437,8 +1431,17 @@ static mf_status eval_batch(mf_model* m, int64_t n_toys, const double* lambdas, 
     MF_CUDA(ctx, cudaMemcpyAsync(m->d_lam, m->h_lam, sizeof(double) * n_active * K, cudaMemcpyHostToDevice, ctx->stream));
     if (n_active < n_toys)
         MF_CUDA(ctx, cudaMemcpyAsync(m->d_ids, m->h_ids, sizeof(int) * n_active, cudaMemcpyHostToDevice, ctx->stream));
-    mf_status st;
-    if (hess) {
+    mf_status st = MF_OK;
+    std::vector<int> invalid;  // 4D Hessian: slots whose lambda is outside the parameter domain
+    if (hess && m->kind == MF_MASS_X_ANGULAR) {
+        // batched 4D toys: the second-order kernel (tensor-core contraction) toy by toy, in stream order
+        const int row4 = 1 + K + K * (K + 1) / 2 + 1;
+        for (int s = 0; s < n_active; ++s) {
+            const mf_status ss = launch_second<FourDSecond, 1>(m, m->h_lam + (int64_t)s * K, m->d_bout + (int64_t)s * row4, m->h_ids[s]);
+            if (ss == MF_ERR_PARAM_DOMAIN) invalid.push_back(s);
+            else if (ss != MF_OK) return ss;
+        }
+    } else if (hess) {
         st = (m->kind == MF_MASS_GAUSS_EXP) ? launch_batch<MassHessModel>(m, n_active) : launch_batch<AngularHessModel>(m, n_active);
     } else {
         switch (m->kind) {
@@ -1451,6 +1454,11 @@ static mf_status eval_batch(mf_model* m, int64_t n_toys, const double* lambdas, 
     const int row = (hess ? 1 + K + K * (K + 1) / 2 : K + 1) + 1;
     MF_CUDA(ctx, cudaMemcpyAsync(m->h_bout, m->d_bout, sizeof(double) * n_active * row, cudaMemcpyDeviceToHost, ctx->stream));
     MF_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    for (int s : invalid) {  // as the batched kernels report a domain error: +inf, NaN
+        double* o = m->h_bout + (int64_t)s * row;
+        o[0] = INFINITY;
+        for (int k = 1; k < row - 1; ++k) o[k] = NAN;
+    }
     for (int s = 0; s < n_active; ++s) {
         const int64_t t = m->h_ids[s];
         const double* o = m->h_bout + (int64_t)s * row;

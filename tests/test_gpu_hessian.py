@@ -80,10 +80,7 @@ def test_hessian_status(mf, ctx):
     assert amodel.fit(dg.FOURD_TRUTH, opts=ofd).converged
     toys4 = np.stack([dg.gen_4d(500, seed=s) for s in (1, 2)], axis=1)      # [4][2][500]
     bmodel = ctx.model_create(mf.MF_MASS_X_ANGULAR, ctx.dataset_upload(toys4, LO, HI, n_toys=2))
-    assert not bmodel.has_hessian                 # batched 4D toys: no batched Hessian kernel, the fit uses finite differences
-    with pytest.raises(mf.MoreFitError) as e:
-        bmodel.nll_grad_hess_batch(np.tile(np.array(dg.FOURD_TRUTH), (2, 1)))
-    assert e.value.status == mf.MF_ERR_ARG
+    assert bmodel.has_hessian                     # batched 4D toys: the second-order kernel toy by toy
     m = dg.gen_mass(1000, seed=0)
     model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(m, LO, HI))
     with pytest.raises(mf.MoreFitError) as e:
@@ -165,3 +162,28 @@ def test_angular_hessian_batch_and_fit(mf, ctx):
     assert r.converged and np.max(np.abs(r.lam - o.lam) / o.sigma) < 1e-6
     assert np.max(np.abs(r.sigma / o.sigma - 1)) < 1e-5
     assert r.n_calls <= 12
+
+
+def test_fourd_hessian_batch_and_toy_fits(mf, ctx):
+    """mf_nll_grad_hess_batch for 4D toys (second-order kernel toy by toy) against the oracle, with an inactive toy and a toy
+    whose lambda is outside the parameter domain; then all toys fitted concurrently by Newton steps on that Hessian."""
+    T, n = 5, 3_001
+    toys = np.stack([dg.gen_4d(n, seed=70 + t) for t in range(T)], axis=1)          # [4][T][n]
+    model = ctx.model_create(mf.MF_MASS_X_ANGULAR, ctx.dataset_upload(toys, LO, HI, n_toys=T))
+    lams = np.tile(np.array(dg.FOURD_TRUTH), (T, 1))
+    lams[1, 4:12] += 0.02
+    lams[3, 2] = -0.01                            # sigma < 0
+    active = np.ones(T, dtype=np.uint8)
+    active[2] = 0
+    nll, g, H = model.nll_grad_hess_batch(lams, active)
+    assert math.isnan(nll[2]) and np.all(np.isnan(H[2]))
+    assert nll[3] == math.inf and np.all(np.isnan(g[3])) and np.all(np.isnan(H[3]))
+    for t in (0, 1, 4):
+        o_nll, o_g, o_H, bad = oracle.nll_grad_hess(oracle.FOURD, toys[:, t, :], lams[t], LO, HI)
+        assert bad == 0
+        check(nll[t], g[t], H[t], o_nll, o_g, o_H, f"4D toy {t}")
+    fr = model.fit_batch(np.array(dg.FOURD_TRUTH))
+    assert np.all(fr.converged) and np.all(fr.n_calls <= 12), fr.n_calls
+    for t in (0, 4):
+        o = oracle.fit(oracle.FOURD, toys[:, t, :], dg.FOURD_TRUTH, lo=LO, hi=HI)
+        assert np.max(np.abs(fr.lam[t] - o.lam) / o.sigma) < 1e-6
