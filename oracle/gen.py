@@ -6,10 +6,13 @@ The recipe, followed step by step, one event 
   RNG     Philox4x32-10 (Salmon et al., "Parallel random numbers: as easy as 1, 2, 3", SC'11), written out below.
           key = (seed mod 2^32, seed >> 32) with seed = seed0 + toy; counter = (event mod 2^32, event >> 32, draw, 0).
           One call gives four 32-bit words w0..w3 = two uniforms  u = ((w_hi * 2^32 + w_lo) >> 11 + 1/2) * 2^-53  in (0, 1).
-  event   draw 0: (uA, uB).  Signal if uA < f, else background.
-          background:  m = lo + log1p(uB * expm1(tau w)) / tau   (tau != 0),  lo + uB w  (tau == 0),  w = hi - lo; clamped to [lo, hi].
-          signal: draws k = 1, 2, ...: (u1, u2), z = sqrt(-2 ln u1) cos(2 pi u2), m = mu + sigma z; the first m in [lo, hi] is taken
-          (after 64 rejected draws the last m is clamped into the range).
+  event   (mass model; round 2: ONE Philox block per event in the common case, all four words used)
+          draw k gives  s = (w0 + 1/2) 2^-32,  u = ((w1 2^32 + w2) >> 11 + 1/2) 2^-53,  v = (w3 + 1/2) 2^-32.
+          draw 0: signal if s < f, else background.
+          background:  m = lo + log1p(u * expm1(tau w)) / tau   (tau != 0),  lo + u w  (tau == 0),  w = hi - lo; clamped to [lo, hi].
+          signal: z = sqrt(-2 ln u) cos(2 pi v), m = mu + sigma z, with (u, v) of draw 0; if m is outside [lo, hi], (u, v) of
+          draws 1, 2, ... until it is inside (after 64 rejected draws the last m is clamped into the range).
+          (The angular and 4D recipes below keep two 53-bit uniforms per draw.)
 
 The CUDA path implements the same recipe in its own code (mf_generate.cu); uniform words are bit-identical, the
 floating-point transforms agree to a few ulp.  Pins (tests/test_oracle_gen.py): the published Philox4x32-10 known-answer
@@ -49,21 +52,28 @@ def uniforms(seed: int, event: int, draw: int):
     return _uniform(w[0], w[1]), _uniform(w[2], w[3])
 
 
+def mass_draw(seed: int, event: int, draw: int):
+    """(s, u, v) of one Philox block: s, v with 32 bits, u with 53 bits, all in (0, 1)."""
+    w = philox4x32_10((event & _MASK, event >> 32, draw, 0), (seed & _MASK, seed >> 32))
+    return (w[0] + 0.5) * 2.0 ** -32, _uniform(w[1], w[2]), (w[3] + 0.5) * 2.0 ** -32
+
+
 def gen_mass_event(seed: int, event: int, lam, lo: float, hi: float):
     """(m, is_signal, number of draws used) of one event."""
     f, mu, sigma, tau = [float(x) for x in lam]
-    ua, ub = uniforms(seed, event, 0)
-    if ua < f:
+    s, u, v = mass_draw(seed, event, 0)
+    if s < f:
         m = mu
-        for k in range(1, 65):
-            u1, u2 = uniforms(seed, event, k)
-            z = math.sqrt(-2.0 * math.log(u1)) * math.cos(2.0 * math.pi * u2)
+        for k in range(0, 65):
+            if k:
+                _, u, v = mass_draw(seed, event, k)
+            z = math.sqrt(-2.0 * math.log(u)) * math.cos(2.0 * math.pi * v)
             m = mu + sigma * z
             if lo <= m <= hi:
                 return m, True, k + 1
         return min(max(m, lo), hi), True, 65
     w = hi - lo
-    m = lo + ub * w if tau == 0.0 else lo + math.log1p(ub * math.expm1(tau * w)) / tau
+    m = lo + u * w if tau == 0.0 else lo + math.log1p(u * math.expm1(tau * w)) / tau
     return min(max(m, lo), hi), False, 1
 
 
@@ -129,8 +139,8 @@ def gen_angular_toys(seed0: int, n_toys: int, n_events: int, a) -> np.ndarray:
 # ---------------------------------------------------------------- 4D model (BASELINE.json configs[3])
 #
 #   draw 0: (uA, uB).  Signal if uA < f.
-#   signal:      mass from draws 1..64 exactly as in gen_mass_event; angles by the angular accept-reject above with the
-#                proposals taken from draws 100 + 2k, 101 + 2k.
+#   signal:      mass from draws k = 1..64: (u1, u2) -> mu + sigma sqrt(-2 ln u1) cos(2 pi u2), the first inside [lo, hi]; angles by
+#                the angular accept-reject above with the proposals taken from draws 100 + 2k, 101 + 2k.
 #   background:  mass from uB by the inverse CDF; draw 1: (u1, -) -> phi = pi (2 u1 - 1);
 #                (cos theta_l, cos theta_K) by accept-reject of the Legendre product l(x; cl1, cl2) l(y; ck1, ck2),
 #                l(x; c1, c2) = 1/2 [1 + c1 x + c2 (3 x^2 - 1)/2], under the bound lmax(c1, c2) = 1/2 (1 + |c1| + |c2|) per factor:

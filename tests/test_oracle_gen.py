@@ -49,7 +49,7 @@ def test_signal_fraction_and_redraws():
     sig = np.array([s for _, s, _ in r])
     draws = np.array([k for _, s, k in r if s])
     assert abs(sig.mean() - 0.5) < 0.03
-    assert 1.3 < (draws - 1).mean() < 1.8   # expected 1 / P(accept) = 1 / 0.655 = 1.53 Gaussian draws per signal event
+    assert 1.3 < draws.mean() < 1.8         # expected 1 / P(accept) = 1 / 0.655 = 1.53 Gaussian draws per signal event (draw 0 is the first)
 
 
 def test_angular_generator_pdf_is_the_pinned_oracle_pdf():
