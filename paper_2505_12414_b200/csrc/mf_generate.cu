@@ -3,10 +3,12 @@
 //
 // Counter-based instead of the paper's jump-seeded Xoshiro streams: event i of toy t draws from Philox4x32-10 with
 // key = seed0 + t and counter = (i, draw), so any thread can generate any event and the result does not depend on the
-// launch geometry.  Recipe:
-//   draw 0 -> (uA, uB); signal if uA < f, else background m = lo + log1p(uB expm1(tau w)) / tau  (lo + uB w at tau == 0);
-//   signal: draws 1, 2, ... -> Box-Muller z = sqrt(-2 ln u1) cos(2 pi u2), m = mu + sigma z, first m inside [lo, hi]
-//   (after 64 rejected draws the last one is clamped).  u = ((w_hi 2^32 + w_lo) >> 11 + 1/2) 2^-53.
+// launch geometry.  Recipe of the mass model (one block per event in the common case, all four words w0..w3 of a draw used):
+//   s = (w0 + 1/2) 2^-32,  u = ((w1 2^32 + w2) >> 11 + 1/2) 2^-53,  v = (w3 + 1/2) 2^-32;
+//   draw 0: signal if s < f, else background m = lo + log1p(u expm1(tau w)) / tau  (lo + u w at tau == 0);
+//   signal: Box-Muller z = sqrt(-2 ln u) cos(2 pi v), m = mu + sigma z from draw 0; if outside [lo, hi], (u, v) of draws
+//   1, 2, ... until inside (after 64 rejected draws the last one is clamped).
+// The angular and 4D recipes take two 53-bit uniforms ((w0, w1), (w2, w3)) per draw; their layouts are at their kernels.
 // The events are written straight into the dataset's padded structure of arrays: no host copy.
 #include <cuda_runtime.h>
 
@@ -79,23 +81,27 @@ __global__ void __launch_bounds__(256) generate_mass_kernel(double* __restrict__
                 continue;
             }
             const unsigned long long ev = (unsigned long long)(slot < n ? slot : n - 1);
-            double ua, ub, m;
-            uniforms(seed, ev, 0u, ua, ub);
-            if (ua < f) {
-                m = mu;
+            // draw 0: s = (w0 + 1/2) 2^-32 chooses the component, u = 53 bits of (w1, w2), v = (w3 + 1/2) 2^-32.
+            // Both components need ONE logarithm of a function of u: ln u (Box-Muller radius) or ln(1 + u expm1(tau w))
+            // (inverse CDF of the exponential), so the common path has no divergent branch.
+            unsigned wd[4];
+            philox4x32_10((unsigned)ev, (unsigned)(ev >> 32), 0u, 0u, (unsigned)seed, (unsigned)(seed >> 32), wd);
+            const bool sig = ((double)wd[0] + 0.5) * 0x1p-32 < f;
+            double u = uniform53(wd[1], wd[2]), v = ((double)wd[3] + 0.5) * 0x1p-32;
+            const double L = mf::mf_log(sig ? u : fma(u, em1, 1.0), s_tab);
+            const double zs = sqrt(-2.0 * L) * cospi(2.0 * v);
+            double m = sig ? fma(sigma, zs, mu) : (tau == 0.0) ? fma(u, w, lo) : fma(L, inv_tau, lo);
+            if (sig && !(m >= lo && m <= hi)) {  // rare: the Gaussian draw fell outside the range: further blocks
                 bool ok = false;
                 for (unsigned k = 1; k <= 64 && !ok; ++k) {
-                    double u1, u2;
-                    uniforms(seed, ev, k, u1, u2);
-                    const double z = sqrt(-2.0 * mf::mf_log(u1, s_tab)) * cospi(2.0 * u2);
-                    m = fma(sigma, z, mu);
+                    philox4x32_10((unsigned)ev, (unsigned)(ev >> 32), k, 0u, (unsigned)seed, (unsigned)(seed >> 32), wd);
+                    u = uniform53(wd[1], wd[2]);
+                    v = ((double)wd[3] + 0.5) * 0x1p-32;
+                    m = fma(sigma, sqrt(-2.0 * mf::mf_log(u, s_tab)) * cospi(2.0 * v), mu);
                     ok = (m >= lo && m <= hi);
                 }
-                if (!ok) m = fmin(fmax(m, lo), hi);
-            } else {
-                m = (tau == 0.0) ? fma(ub, w, lo) : fma(mf::mf_log(fma(ub, em1, 1.0), s_tab), inv_tau, lo);
-                m = fmin(fmax(m, lo), hi);
             }
+            m = fmin(fmax(m, lo), hi);
             row[slot] = m;
         }
     }
