@@ -150,6 +150,7 @@ extern "C" void mf_ctx_destroy(mf_ctx* ctx)
     cudaStreamSynchronize(ctx->stream);
     if (ctx->p_blk) cudaFreeAsync(ctx->p_blk, ctx->stream);
     if (ctx->h_slab) cudaFreeHost(ctx->h_slab);
+    if (ctx->h_big) cudaFreeHost(ctx->h_big);
     if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
     for (int i = 0; i < mf_ctx::kPointStages; ++i) {
         if (ctx->h_pts[i]) cudaFreeHost(ctx->h_pts[i]);
@@ -660,7 +661,8 @@ static mf_status stage_reserve(mf_ctx* ctx, size_t bytes)
 // MODE 0: -ln L and gradient; 1: + Hessian; 2: + Fisher matrix sum w^2 s s^T.  out_dev NULL = the model's own buffer.
 // Output row: -ln L, gradient [K], Hessian upper triangle row by row [K(K+1)/2], Fisher likewise, n_bad.
 template <class S, int MODE>
-static mf_status launch_second(mf_model* m, const double* lam, double* out_dev, int64_t toy = 0)
+static mf_status launch_second(mf_model* m, const double* lam, double* out_dev, int64_t toy = 0,
+                               unsigned long long* done_flag = nullptr, unsigned long long done_value = 0)
 {
     using L = SecondLayout<S, MODE>;
     using LW = SecondLayout<S, 2>;  // scratch is sized for the widest mode
@@ -696,6 +698,8 @@ static mf_status launch_second(mf_model* m, const double* lam, double* out_dev, 
     cb.ticket = m->s_ticket;
     cb.c = a.c;
     cb.out = out_dev ? out_dev : m->s_out;
+    cb.done_flag = done_flag;
+    cb.done_value = done_value;
     second_combine_kernel<S, MODE><<<(L::NQ + kWarps - 1) / kWarps, kBlock, 0, ctx->stream>>>(cb);
     MF_CUDA(ctx, cudaGetLastError());
     ctx->launches += 2;
@@ -703,12 +707,13 @@ static mf_status launch_second(mf_model* m, const double* lam, double* out_dev, 
 }
 
 template <int MODE>
-static mf_status dispatch_second(mf_model* m, const double* lam, double* out_dev)
+static mf_status dispatch_second(mf_model* m, const double* lam, double* out_dev, unsigned long long* done_flag = nullptr,
+                                 unsigned long long done_value = 0)
 {
     switch (m->kind) {
-    case MF_MASS_GAUSS_EXP: return launch_second<MassSecond, MODE>(m, lam, out_dev);
-    case MF_ANGULAR_KSTMUMU: return launch_second<AngularSecond, MODE>(m, lam, out_dev);
-    default: return launch_second<FourDSecond, MODE>(m, lam, out_dev);
+    case MF_MASS_GAUSS_EXP: return launch_second<MassSecond, MODE>(m, lam, out_dev, 0, done_flag, done_value);
+    case MF_ANGULAR_KSTMUMU: return launch_second<AngularSecond, MODE>(m, lam, out_dev, 0, done_flag, done_value);
+    default: return launch_second<FourDSecond, MODE>(m, lam, out_dev, 0, done_flag, done_value);
     }
 }
 
@@ -719,15 +724,33 @@ static mf_status second_sync(mf_model* m, const double* lambda, double* nll, dou
     mf_ctx* ctx = m->ctx;
     const int K = m->K, NH = K * (K + 1) / 2;
     const int mode = fisher ? 2 : hess ? 1 : 0;
-    const mf_status st = mode == 2 ? dispatch_second<2>(m, lambda, nullptr) : mode == 1 ? dispatch_second<1>(m, lambda, nullptr)
-                                                                                       : dispatch_second<0>(m, lambda, nullptr);
-    if (st != MF_OK) return st;
     const int nout = 1 + K + (mode >= 1 ? NH : 0) + (mode >= 2 ? NH : 0);
-    const mf_status sr = stage_reserve(ctx, sizeof(double) * (nout + 1));
-    if (sr != MF_OK) return sr;
-    double* h = reinterpret_cast<double*>(ctx->h_stage);
-    MF_CUDA(ctx, cudaMemcpyAsync(h, m->s_out, sizeof(double) * (nout + 1), cudaMemcpyDeviceToHost, ctx->stream));
-    MF_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    // the combine kernel writes the result row and then a done word into mapped pinned memory; the host spins on the word
+    // (a D2H copy + stream synchronise costs ~25 us per call, the kernels 60-110 us)
+    constexpr int kBigDoubles = 512, kBigDone = 511;
+    if (!ctx->h_big) {
+        MF_CUDA(ctx, cudaHostAlloc(reinterpret_cast<void**>(&ctx->h_big), sizeof(double) * kBigDoubles, cudaHostAllocMapped));
+        MF_CUDA(ctx, cudaHostGetDevicePointer(reinterpret_cast<void**>(&ctx->d_big), ctx->h_big, 0));
+        std::memset(ctx->h_big, 0, sizeof(double) * kBigDoubles);
+    }
+    const unsigned long long want = ++ctx->big_seq;
+    unsigned long long* d_done = reinterpret_cast<unsigned long long*>(ctx->d_big + kBigDone);
+    const mf_status st = mode == 2   ? dispatch_second<2>(m, lambda, ctx->d_big, d_done, want)
+                         : mode == 1 ? dispatch_second<1>(m, lambda, ctx->d_big, d_done, want)
+                                     : dispatch_second<0>(m, lambda, ctx->d_big, d_done, want);
+    if (st != MF_OK) return st;
+    volatile unsigned long long* done = reinterpret_cast<volatile unsigned long long*>(ctx->h_big + kBigDone);
+    for (unsigned spins = 1; *done != want; ++spins) {
+        if ((spins & 0xFFFF) == 0) {
+            const cudaError_t qy = cudaStreamQuery(ctx->stream);
+            if (qy != cudaErrorNotReady && *done != want) {
+                if (qy == cudaSuccess) continue;
+                return mf_fail(ctx, MF_ERR_CUDA, std::string(who) + ": " + cudaGetErrorString(qy));
+            }
+        }
+    }
+    std::atomic_thread_fence(std::memory_order_acquire);
+    const double* h = ctx->h_big;
     *nll = h[0];
     if (grad) std::memcpy(grad, h + 1, sizeof(double) * K);
     int q = 1 + K;

@@ -31,6 +31,10 @@ struct mf_ctx {
     // device scratch of the many-points evaluation (mf_nll_grad_points / mf_nll_grad_sweep), shared by all models of the
     // context (every launch is ordered on the one stream, and the kernel touches the scratch only after its programmatic
     // wait): grow-only, laid out as [consts | ok | partials | bad | ticket] for the largest (points, chunks) seen so far
+    // mapped pinned result row of the synchronous second-order calls (up to 1 + 16 + 136 + 136 + 1 doubles) and its done word
+    double* h_big = nullptr;
+    double* d_big = nullptr;
+    unsigned long long big_seq = 0;
     cudaStream_t server_stream = nullptr;  // resident evaluation kernels (mf_model_serve) run here, beside the work stream
     std::vector<struct mf_model*> serving;  // models whose resident kernel may be running
     char* p_blk = nullptr;

@@ -214,6 +214,8 @@ struct SecondCombineArgs {
     unsigned* ticket;              // zero on entry, reset by the last CTA
     typename S::Consts c;
     double* out;                   // [NOUT + 1]
+    unsigned long long* done_flag; // mapped host word that receives done_value after `out` is written, or NULL
+    unsigned long long done_value;
 };
 
 template <class S, int MODE>
@@ -267,6 +269,14 @@ __global__ void __launch_bounds__(kBlock) second_combine_kernel(const __grid_con
     if (threadIdx.x == 0) {
         a.out[L::NOUT] = (double)nb;
         *a.ticket = 0u;
+    }
+    if (a.done_flag) {  // synchronous call: `out` is mapped host memory and the host spins on this word
+        __threadfence_system();
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            __threadfence_system();
+            *reinterpret_cast<volatile unsigned long long*>(a.done_flag) = a.done_value;
+        }
     }
 }
 
