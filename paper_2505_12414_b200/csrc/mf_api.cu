@@ -1071,7 +1071,8 @@ extern "C" mf_status mf_nll_grad_points(mf_model* m, int64_t n_points, const dou
         }
         return MF_OK;
     }
-    if (n_points < 16) {  // few points: back-to-back pipelined single evaluations are faster (measured cross-over ~12)
+    static const int min_batch = std::getenv("MF_POINTS_MIN_BATCH") ? std::atoi(std::getenv("MF_POINTS_MIN_BATCH")) : 16;  // tuning knob
+    if (n_points < min_batch) {  // few points: back-to-back pipelined single evaluations are faster (measured cross-over ~12)
         for (int64_t p = 0; p < n_points; ++p) {
             const mf_status st = dispatch_single(m, lambdas + p * m->K, out_dev + p * (m->K + 2), n_points > 1);
             if (st != MF_OK) return st;
