@@ -461,6 +461,18 @@ def _other_workloads(torch, mf, ctx, peaks, traffic_all) -> dict:
                 "(Newton on the analytic Hessian + HESSE); no event crosses PCIe",
         "generation_us": gen_us, "generated_events_per_s": T * n / (gen_us * 1e-6),
         "paper_context": "MoreFit OpenCL GPU (analytic), Titan V: 1.62 ms per toy at 1e4 events (PAPER.md:191); another machine"}
+    # the paper's second benchmark (Table 3): angular pseudo-experiments, generation + fit + HESSE
+    Ta = 1024
+    ctx.toy_study_angular(1, Ta, n, dg.ANG_TRUTH)
+    t = time.perf_counter()
+    tsa = ctx.toy_study_angular(200_000, Ta, n, dg.ANG_TRUTH)
+    tsa_s = time.perf_counter() - t
+    res["toy_study_angular_1024x1e4_on_device"] = {
+        "ms_per_toy": 1e3 * tsa_s / Ta, "toys_per_s": Ta / tsa_s, "converged": int(tsa.converged.sum()),
+        "mean_calls_per_toy": float(tsa.n_calls.mean()),
+        "what": "mf_toy_study_angular: mf_generate_angular (accept-reject, 1024 toys x 1e4 events) + mf_model_create (basis cache) + "
+                "mf_fit_batch (Newton on the analytic Hessian + HESSE); no event crosses PCIe",
+        "paper_context": "MoreFit OpenCL GPU (analytic), Titan V: 2.39 ms per toy at 1e4 events (PAPER.md:224); another machine, other truth values"}
     # C0: N = 1e4, one call + full fit (latency bound: no roofline claim)
     m0 = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(dg.gen_mass(10_000, seed=0), dg.MASS_LO, dg.MASS_HI))
     m0.nll_grad(dg.MASS_START)

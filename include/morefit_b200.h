@@ -305,6 +305,12 @@ mf_status mf_fit_batch(mf_model* model, int64_t n_toys, const double* starts,
 mf_status mf_toy_study_mass(mf_ctx* ctx, uint64_t seed0, int64_t n_toys, int64_t n_events, const double* lam_truth, double lo,
                             double hi, const mf_fit_opts* opts, mf_fit_result* results);
 
+/* The same for the angular model (the paper's second benchmark, Table 3): n_toys pseudo-experiments of
+ * n_events events generated by accept-reject at a_truth (mf_generate_angular, seeds seed0 + t), fitted concurrently from
+ * a_truth with Newton steps on the analytic Hessian, HESSE covariances returned.  a_truth: host, 8 doubles. */
+mf_status mf_toy_study_angular(mf_ctx* ctx, uint64_t seed0, int64_t n_toys, int64_t n_events, const double* a_truth,
+                               const mf_fit_opts* opts, mf_fit_result* results);
+
 /* ---- multi-GPU: S5 across ranks ------------------------------------------------------ */
 
 /* Combines the partial sums of n_ranks event shards of ONE dataset (each rank's mf_nll_grad on its shard: -ln L and the

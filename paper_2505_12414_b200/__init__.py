@@ -36,7 +36,7 @@ EXPORTS = [
     "mf_model_create", "mf_model_destroy", "mf_model_nparams", "mf_model_n_events", "mf_model_n_toys",
     "mf_nll_grad", "mf_nll_grad_async", "mf_nll_grad_points", "mf_nll_grad_sweep", "mf_nll_grad_batch", "mf_nll_grad_batch_async",
     "mf_model_serve", "mf_model_is_served", "mf_model_has_hessian", "mf_model_is_weighted", "mf_nll_grad_hess", "mf_nll_grad_hess_fisher", "mf_nll_grad_hess_batch",
-    "mf_fit_opts_default", "mf_fit", "mf_fit_batch", "mf_toy_study_mass",
+    "mf_fit_opts_default", "mf_fit", "mf_fit_batch", "mf_toy_study_mass", "mf_toy_study_angular",
     "mf_combine_partials",
 ]
 
@@ -199,6 +199,8 @@ def load_library() -> ctypes.CDLL:
     lib.mf_toy_study_mass.restype = ctypes.c_int
     lib.mf_toy_study_mass.argtypes = [vp, ctypes.c_uint64, i64, i64, dp, ctypes.c_double, ctypes.c_double, ctypes.POINTER(FitOpts),
                                       ctypes.POINTER(_FitResultC)]
+    lib.mf_toy_study_angular.restype = ctypes.c_int
+    lib.mf_toy_study_angular.argtypes = [vp, ctypes.c_uint64, i64, i64, dp, ctypes.POINTER(FitOpts), ctypes.POINTER(_FitResultC)]
     lib.mf_nll_grad_sweep.restype = ctypes.c_int
     lib.mf_nll_grad_sweep.argtypes = [vp, i64, dp, dp, dp, ctypes.POINTER(i64)]
     lib.mf_combine_partials.restype = ctypes.c_int
@@ -312,6 +314,17 @@ class Context:
                                                 None if opts is None else ctypes.byref(opts),
                                                 res.ctypes.data_as(ctypes.POINTER(_FitResultC))))
         return BatchFitResult(res, int(n_toys), 4)
+
+    def toy_study_angular(self, seed0: int, n_toys: int, n_events: int, a_truth, opts: "FitOpts | None" = None) -> "BatchFitResult":
+        """Generate (accept-reject), fit and HESSE n_toys pseudo-experiments of the angular model on the device."""
+        a = np.ascontiguousarray(a_truth, dtype=np.float64)
+        if a.shape != (8,):
+            raise ValueError("a_truth must have 8 entries")
+        res = self._fit_results(int(n_toys))
+        self._check(self._lib.mf_toy_study_angular(self._h, int(seed0), int(n_toys), int(n_events), _dp(a),
+                                                   None if opts is None else ctypes.byref(opts),
+                                                   res.ctypes.data_as(ctypes.POINTER(_FitResultC))))
+        return BatchFitResult(res, int(n_toys), 8)
 
     def model_create(self, kind: int, dataset: "Dataset") -> "Model":
         return Model(self, kind, dataset)

@@ -130,29 +130,66 @@ struct AngGenArgs {
     double pmax;
 };
 
-// data: [3][n_toys][n_pad] (cos theta_l, cos theta_K, phi).  Proposal k of an event uses draws 2k and 2k+1.
+// data: [3][n_toys][n_pad] (cos theta_l, cos theta_K, phi).  Proposal k of an event uses draws 2k and 2k+1; the event is its
+// first accepted proposal (a pure function of (seed, event index)).
+// Work distribution: accept-reject with ~10 % efficiency leaves a warp that walks 32 events in lock step waiting for its
+// slowest lane (35 proposals against a mean of 10).  Here every warp owns a contiguous chunk of the flattened (toy, slot)
+// index space and its lanes are persistent workers: a lane whose event has been accepted writes it and takes the next
+// unassigned index of the chunk (ballot + prefix count), so all 32 lanes keep proposing until the chunk is exhausted.
+constexpr int kGenChunk = 256;  // indices per warp chunk (the last proposals of a chunk run on a thinning warp)
+
 __global__ void __launch_bounds__(256) generate_angular_kernel(double* __restrict__ data, int64_t n_toys, int64_t n, int64_t n_pad,
                                                                unsigned long long seed0, const __grid_constant__ AngGenArgs g)
 {
     const int64_t per_dim = n_toys * n_pad;
-    for (int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; idx < per_dim; idx += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t toy = idx / n_pad, slot = idx % n_pad;
-        double cl = 0.0, ck = 0.0, phi = 0.0;
-        if (n > 0) {
-            const unsigned long long ev = (unsigned long long)(slot < n ? slot : n - 1), seed = seed0 + (unsigned long long)toy;
-            for (unsigned k = 0; k < 4096; ++k) {
-                double u1, u2, u3, u4;
-                uniforms(seed, ev, 2 * k, u1, u2);
-                uniforms(seed, ev, 2 * k + 1, u3, u4);
-                cl = 2.0 * u1 - 1.0;
-                ck = 2.0 * u2 - 1.0;
-                phi = 3.141592653589793238462643383279502884 * (2.0 * u3 - 1.0);
-                if (u4 * g.pmax < angular_pdf(cl, ck, 2.0 * u3 - 1.0, g.a)) break;
+    const int lane = threadIdx.x & 31;
+    const int64_t n_chunks = (per_dim + kGenChunk - 1) / kGenChunk;
+    const int64_t warps = (int64_t)gridDim.x * (blockDim.x >> 5), w0 = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    for (int64_t ch = w0; ch < n_chunks; ch += warps) {
+        const int64_t first = ch * kGenChunk, end = (first + kGenChunk < per_dim) ? first + kGenChunk : per_dim;
+        int64_t next = first + 32;          // next unassigned index of the chunk (warp-uniform)
+        int64_t idx = first + lane;         // this lane's current index
+        bool active = idx < end;
+        unsigned long long ev = 0, seed = 0;
+        unsigned k = 0;
+        auto start = [&]() {                // set up the event of index idx
+            const int64_t toy = idx / n_pad, slot = idx % n_pad;
+            ev = (unsigned long long)(slot < n ? slot : n - 1);
+            seed = seed0 + (unsigned long long)toy;
+            k = 0;
+        };
+        if (active && n > 0) start();
+        while (__any_sync(0xffffffffu, active)) {
+            bool finished = false;
+            double cl = 0.0, ck = 0.0, phi = 0.0;
+            if (active) {
+                if (n > 0) {
+                    double u1, u2, u3, u4;
+                    uniforms(seed, ev, 2 * k, u1, u2);
+                    uniforms(seed, ev, 2 * k + 1, u3, u4);
+                    cl = 2.0 * u1 - 1.0;
+                    ck = 2.0 * u2 - 1.0;
+                    phi = 3.141592653589793238462643383279502884 * (2.0 * u3 - 1.0);
+                    finished = (u4 * g.pmax < angular_pdf(cl, ck, 2.0 * u3 - 1.0, g.a)) || (k == 4095u);
+                    ++k;
+                } else {
+                    finished = true;        // empty toys: zeros
+                }
+                if (finished) {
+                    data[idx] = cl;
+                    data[per_dim + idx] = ck;
+                    data[2 * per_dim + idx] = phi;
+                }
             }
+            // lanes that finished take the next unassigned indices, in lane order
+            const unsigned need = __ballot_sync(0xffffffffu, active && finished);
+            if (active && finished) {
+                idx = next + __popc(need & ((1u << lane) - 1u));
+                active = idx < end;
+                if (active && n > 0) start();
+            }
+            next += __popc(need);
         }
-        data[idx] = cl;
-        data[per_dim + idx] = ck;
-        data[2 * per_dim + idx] = phi;
     }
 }
 
@@ -176,54 +213,87 @@ __device__ __forceinline__ double legendre2(double x, double c1, double c2)
 __global__ void __launch_bounds__(256) generate_4d_kernel(double* __restrict__ data, int64_t n_toys, int64_t n, int64_t n_pad,
                                                           unsigned long long seed0, const __grid_constant__ FourDGenArgs g)
 {
+    // persistent lanes over warp chunks of the flattened (toy, slot) index space, as generate_angular_kernel
     const int64_t per_dim = n_toys * n_pad;
     const double pi = 3.141592653589793238462643383279502884;
-    for (int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; idx < per_dim; idx += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t toy = idx / n_pad, slot = idx % n_pad;
-        double m = 0.0, cl = 0.0, ck = 0.0, phi = 0.0;
-        if (n > 0) {
-            const unsigned long long ev = (unsigned long long)(slot < n ? slot : n - 1), seed = seed0 + (unsigned long long)toy;
+    const int lane = threadIdx.x & 31;
+    const int64_t n_chunks = (per_dim + kGenChunk - 1) / kGenChunk;
+    const int64_t warps = (int64_t)gridDim.x * (blockDim.x >> 5), w0 = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    for (int64_t ch = w0; ch < n_chunks; ch += warps) {
+        const int64_t first = ch * kGenChunk, end = (first + kGenChunk < per_dim) ? first + kGenChunk : per_dim;
+        int64_t next = first + 32;
+        int64_t idx = first + lane;
+        bool active = idx < end;
+        unsigned long long ev = 0, seed = 0;
+        unsigned k = 0;
+        bool sig = false;
+        double m = 0.0, phi_bkg = 0.0;
+        auto start = [&]() {  // component, mass (and the background's phi) of the event of index idx; proposals start at k = 0
+            const int64_t toy = idx / n_pad, slot = idx % n_pad;
+            ev = (unsigned long long)(slot < n ? slot : n - 1);
+            seed = seed0 + (unsigned long long)toy;
+            k = 0;
             double ua, ub;
             uniforms(seed, ev, 0u, ua, ub);
-            if (ua < g.f) {
+            sig = ua < g.f;
+            if (sig) {
                 m = g.mu;
                 bool ok = false;
-                for (unsigned k = 1; k <= 64 && !ok; ++k) {
+                for (unsigned q = 1; q <= 64 && !ok; ++q) {
                     double u1, u2;
-                    uniforms(seed, ev, k, u1, u2);
+                    uniforms(seed, ev, q, u1, u2);
                     m = fma(g.sigma, sqrt(-2.0 * log(u1)) * cos(2.0 * pi * u2), g.mu);
                     ok = (m >= g.lo && m <= g.hi);
                 }
                 if (!ok) m = fmin(fmax(m, g.lo), g.hi);
-                for (unsigned k = 0; k < 4096; ++k) {
+            } else {
+                const double w = g.hi - g.lo;
+                m = (g.tau == 0.0) ? fma(ub, w, g.lo) : g.lo + log1p(ub * g.em1) / g.tau;
+                m = fmin(fmax(m, g.lo), g.hi);
+                double u1, u2;
+                uniforms(seed, ev, 1u, u1, u2);
+                phi_bkg = pi * (2.0 * u1 - 1.0);
+            }
+        };
+        if (active && n > 0) start();
+        while (__any_sync(0xffffffffu, active)) {
+            bool finished = false;
+            double cl = 0.0, ck = 0.0, phi = 0.0;
+            if (active) {
+                if (n > 0) {
                     double u1, u2, u3, u4;
                     uniforms(seed, ev, 100 + 2 * k, u1, u2);
                     uniforms(seed, ev, 101 + 2 * k, u3, u4);
                     cl = 2.0 * u1 - 1.0;
                     ck = 2.0 * u2 - 1.0;
-                    phi = pi * (2.0 * u3 - 1.0);
-                    if (u4 * g.ang.pmax < angular_pdf(cl, ck, 2.0 * u3 - 1.0, g.ang.a)) break;
+                    if (sig) {
+                        phi = pi * (2.0 * u3 - 1.0);
+                        finished = u4 * g.ang.pmax < angular_pdf(cl, ck, 2.0 * u3 - 1.0, g.ang.a);
+                    } else {
+                        phi = phi_bkg;
+                        finished = u3 * g.bound < legendre2(cl, g.cl1, g.cl2) * legendre2(ck, g.ck1, g.ck2);
+                    }
+                    finished = finished || (k == 4095u);
+                    ++k;
+                } else {
+                    finished = true;
+                    m = 0.0;
                 }
-            } else {
-                const double w = g.hi - g.lo;
-                m = (g.tau == 0.0) ? fma(ub, w, g.lo) : g.lo + log1p(ub * g.em1) / g.tau;
-                m = fmin(fmax(m, g.lo), g.hi);
-                double u1, u2, u3, u4;
-                uniforms(seed, ev, 1u, u1, u2);
-                phi = pi * (2.0 * u1 - 1.0);
-                for (unsigned k = 0; k < 4096; ++k) {
-                    uniforms(seed, ev, 100 + 2 * k, u1, u2);
-                    uniforms(seed, ev, 101 + 2 * k, u3, u4);
-                    cl = 2.0 * u1 - 1.0;
-                    ck = 2.0 * u2 - 1.0;
-                    if (u3 * g.bound < legendre2(cl, g.cl1, g.cl2) * legendre2(ck, g.ck1, g.ck2)) break;
+                if (finished) {
+                    data[idx] = m;
+                    data[per_dim + idx] = cl;
+                    data[2 * per_dim + idx] = ck;
+                    data[3 * per_dim + idx] = phi;
                 }
             }
+            const unsigned need = __ballot_sync(0xffffffffu, active && finished);
+            if (active && finished) {
+                idx = next + __popc(need & ((1u << lane) - 1u));
+                active = idx < end;
+                if (active && n > 0) start();
+            }
+            next += __popc(need);
         }
-        data[idx] = m;
-        data[per_dim + idx] = cl;
-        data[2 * per_dim + idx] = ck;
-        data[3 * per_dim + idx] = phi;
     }
 }
 
@@ -283,7 +353,8 @@ extern "C" mf_status mf_generate_4d(mf_ctx* ctx, uint64_t seed0, int64_t n_toys,
     buf->bytes = (size_t)(per_dim > 0 ? 4 * per_dim : 1) * sizeof(double);
     cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&buf->p), buf->bytes, ctx->stream);
     if (e == cudaSuccess && per_dim > 0) {
-        const int grid = (int)std::min<int64_t>((per_dim + 255) / 256, 32 * (int64_t)ctx->sm_count);
+        const int64_t chunks = (per_dim + kGenChunk - 1) / kGenChunk;
+        const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((chunks + 7) / 8, 32 * (int64_t)ctx->sm_count));
         generate_4d_kernel<<<grid, 256, 0, ctx->stream>>>(buf->p, n_toys, n_events, ds->n_pad, seed0, g);
         ++ctx->launches;
         e = cudaGetLastError();
@@ -336,7 +407,8 @@ extern "C" mf_status mf_generate_angular(mf_ctx* ctx, uint64_t seed0, int64_t n_
     buf->bytes = (size_t)(per_dim > 0 ? 3 * per_dim : 1) * sizeof(double);
     cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&buf->p), buf->bytes, ctx->stream);
     if (e == cudaSuccess && per_dim > 0) {
-        const int grid = (int)std::min<int64_t>((per_dim + 255) / 256, 32 * (int64_t)ctx->sm_count);
+        const int64_t chunks = (per_dim + kGenChunk - 1) / kGenChunk;
+        const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((chunks + 7) / 8, 32 * (int64_t)ctx->sm_count));
         generate_angular_kernel<<<grid, 256, 0, ctx->stream>>>(buf->p, n_toys, n_events, ds->n_pad, seed0, g);
         ++ctx->launches;
         e = cudaGetLastError();
@@ -442,3 +514,29 @@ extern "C" mf_status mf_toy_study_mass(mf_ctx* ctx, uint64_t seed0, int64_t n_to
     mf_model_destroy(model);
     return st;
 }
+
+extern "C" mf_status mf_toy_study_angular(mf_ctx* ctx, uint64_t seed0, int64_t n_toys, int64_t n_events, const double* a_truth,
+                                          const mf_fit_opts* opts, mf_fit_result* results)
+{
+    if (!ctx || !a_truth || !results) return mf_fail(ctx, MF_ERR_ARG, "mf_toy_study_angular: NULL argument");
+    mf_dataset* ds = nullptr;
+    mf_status st = mf_generate_angular(ctx, seed0, n_toys, n_events, a_truth, &ds);
+    if (st != MF_OK) return st;
+    mf_model* model = nullptr;
+    st = mf_model_create(ctx, MF_ANGULAR_KSTMUMU, ds, &model);
+    mf_dataset_destroy(ds);
+    if (st != MF_OK) return st;
+    double* starts = new (std::nothrow) double[(size_t)n_toys * 8];
+    if (!starts) {
+        mf_model_destroy(model);
+        return mf_fail(ctx, MF_ERR_OOM, "mf_toy_study_angular: host allocation failed");
+    }
+    for (int64_t t = 0; t < n_toys; ++t)
+        for (int k = 0; k < 8; ++k) starts[t * 8 + k] = a_truth[k];
+    if (n_toys == 1) st = mf_fit(model, starts, nullptr, opts, results);
+    else st = mf_fit_batch(model, n_toys, starts, nullptr, opts, results);
+    delete[] starts;
+    mf_model_destroy(model);
+    return st;
+}
+

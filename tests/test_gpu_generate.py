@@ -135,3 +135,17 @@ def test_toy_study_entry(mf, ctx):
     assert np.all(np.abs(pulls.mean(0)) < 0.25) and np.all(np.abs(pulls.std(0) - 1) < 0.15)
     one = ctx.toy_study_mass(7, 1, 20_000, dg.MASS_TRUTH, LO, HI)
     assert len(one) == 1 and one.converged[0]
+
+
+def test_toy_study_angular(mf, ctx):
+    """mf_toy_study_angular = generate + model + concurrent fits in one call: identical to the three steps by hand; pulls sane."""
+    T, n = 64, 4_000
+    r = ctx.toy_study_angular(77, T, n, dg.ANG_TRUTH)
+    ds = ctx.generate_angular(77, T, n, dg.ANG_TRUTH)
+    byhand = ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ds).fit_batch(np.array(dg.ANG_TRUTH))
+    assert np.all(r.converged) and np.array_equal(r.lam, byhand.lam) and np.array_equal(r.nll, byhand.nll)
+    pulls = (r.lam - np.array(dg.ANG_TRUTH)) / r.sigma
+    assert np.all(np.abs(pulls.mean(0)) < 0.6) and np.all(np.abs(pulls.std(0) - 1) < 0.4)
+    one = ctx.toy_study_angular(5, 1, 20_000, dg.ANG_TRUTH)
+    assert bool(one.converged[0])
+
