@@ -1050,6 +1050,8 @@ static mf_status launch_points(mf_model* m, int64_t n_points, const double* lamb
     a.ticket = reinterpret_cast<unsigned*>(q);
     a.ids = nullptr;
     a.out = out_dev;
+    a.ahead = 0;  // one dataset for every point: it comes from L2 anyway
+    a.n_active = (int)n_points;
     MF_CUDA(ctx, cudaMemcpyAsync(a.consts, hc, b_consts, cudaMemcpyHostToDevice, ctx->stream));  // pinned: asynchronous
     MF_CUDA(ctx, cudaEventRecord(ctx->pts_copied[stage], ctx->stream));
     take_fresh(m);  // the copy above precedes the launch: the kernel cannot start before the S1 kernels have completed
@@ -1401,10 +1403,26 @@ static mf_status launch_batch(mf_model* m, int n_active, const double* lam_dev =
     a.bad_partials = m->b_bad;
     a.ticket = m->ticket + kRing;
     a.out = out_dev ? out_dev : m->d_bout;
+    a.n_active = n_active;
+    a.ahead = 0;
+    if (m->chunks == 1 && M::NCOL == 1) {
+        static const int env_ahead = [] { const char* e = getenv("MF_BATCH_AHEAD"); return e ? atoi(e) : -1; }();
+        a.ahead = env_ahead >= 0 ? env_ahead : ctx->sm_count;  // measured on B200: 74 .. 296 slots alike, 592 and 0 slower
+    }
     // both kernels are launched programmatically: the constants kernel of evaluation i+1 starts (and computes) while the
     // batched kernel of evaluation i drains, and waits for it to complete only before overwriting the constants
     MF_CUDA(ctx, launch_pdl_v(batch_consts_kernel<M>, (n_active + 127) / 128, 128, 0, ctx->stream, !take_fresh(m), a, n_active));
-    MF_CUDA(ctx, launch_pdl(nll_grad_batch_kernel<M>, n_active * m->chunks, ctx->stream, a, M::BATCH_BLOCK));
+    if constexpr (M::NCOL == 1) {
+        // one-column toys come from HBM: events staged through shared memory by cp.async, 3 groups deep (0: direct loads)
+        static const int env_stages = [] { const char* e = getenv("MF_BATCH_STAGES"); return e ? atoi(e) : 3; }();
+        const int stages = env_stages;
+        if (stages == 2) MF_CUDA(ctx, launch_pdl(nll_grad_batch_kernel<M, 2>, n_active * m->chunks, ctx->stream, a, M::BATCH_BLOCK));
+        else if (stages == 3) MF_CUDA(ctx, launch_pdl(nll_grad_batch_kernel<M, 3>, n_active * m->chunks, ctx->stream, a, M::BATCH_BLOCK));
+        else if (stages == 4) MF_CUDA(ctx, launch_pdl(nll_grad_batch_kernel<M, 4>, n_active * m->chunks, ctx->stream, a, M::BATCH_BLOCK));
+        else MF_CUDA(ctx, launch_pdl(nll_grad_batch_kernel<M>, n_active * m->chunks, ctx->stream, a, M::BATCH_BLOCK));
+    } else {
+        MF_CUDA(ctx, launch_pdl(nll_grad_batch_kernel<M>, n_active * m->chunks, ctx->stream, a, M::BATCH_BLOCK));
+    }
     ctx->launches += 2;
     return MF_OK;
 }

@@ -70,6 +70,10 @@ struct BatchArgs {
     unsigned* bad_partials;      // [n_active][chunks]
     unsigned* ticket;            // [n_active]
     double* out;                 // [n_active][K+2]
+    int ahead;                   // > 0 (chunks == 1, one-column models): the CTA of slot s requests, group by group while it
+                                 // evaluates its own toy, the events of slot s + ahead from HBM into L2 (ahead = the number of
+                                 // co-resident CTAs: the CTA that will follow it on its SM); 0: off
+    int n_active;
 };
 
 template <class M>
@@ -216,9 +220,66 @@ __device__ __forceinline__ void prefetch_group4(const double2* p)
     for (int i = 0; i < kGroupItems; ++i) asm volatile("prefetch.global.L1 [%0];" ::"l"(p + 32 * i));
 }
 
-template <class M, bool FAST>
+// pf_bytes != 0: while group g is evaluated, the same group of ANOTHER dataset (pf_bytes further on: the toy that the next
+// CTA on this SM will evaluate) is requested from HBM into L2 — one 64-byte-strided prefetch per lane covers the 2 KB.
+// STG > 0: the warp's groups are staged through shared memory by per-lane asynchronous copies (cp.async, 16 bytes each, every
+// lane copies and later reads only its own four double2), STG groups deep: the copies of the next STG - 1 groups are in
+// flight while a group is evaluated, at no cost in registers.  For data that come from HBM (batched toys), where the L1
+// prefetch of the direct form does not cover the latency (ncu: 22 % of the warp samples on the first use of a loaded value).
+// stg: this warp's staging area, STG x 4 x 32 double2.
+// state of the staging pipeline of one warp (STG > 0): started by stage_begin() BEFORE the parameter-only constants are
+// waited for, so that the first copies are in flight during that wait
+struct StagePipe {
+    const double2* pi;  // next group to request
+    unsigned s0;        // shared-memory address of this lane's slot in stage 0, item 0
+    int ahead;          // groups requested and not yet evaluated
+};
+
+__device__ __forceinline__ void stage_issue(unsigned s0, const double2* src, int st)
+{
+#pragma unroll
+    for (int i = 0; i < kGroupItems; ++i)
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s0 + (unsigned)((st * kGroupItems + i) * 32 * 16)),
+                     "l"(src + 32 * i)
+                     : "memory");
+}
+
+// this warp's full groups g0, g0 + gstep, ... < n_full: pointer of lane `lane` into the first, pointer step, count
+__device__ __forceinline__ int group_range(const double* col0, int64_t n, int g0, int gstep, int lane, const double2*& p,
+                                           int64_t& pstep)
+{
+    const int n_full = (int)((n / kItem) / kGroupItems);
+    p = reinterpret_cast<const double2*>(col0) + (int64_t)g0 * (32 * kGroupItems) + lane;
+    pstep = (int64_t)gstep * (32 * kGroupItems);
+    return (g0 < n_full) ? (n_full - g0 + gstep - 1) / gstep : 0;
+}
+
+template <int STG>
+__device__ __forceinline__ void stage_begin(StagePipe& sp, const double* col0, int64_t n, int g0, int gstep, int lane, double2* stg,
+                                            int64_t pf_bytes)
+{
+    const double2* p;
+    int64_t pstep;
+    const int left = group_range(col0, n, g0, gstep, lane, p, pstep);
+    sp.pi = p;
+    sp.s0 = (unsigned)__cvta_generic_to_shared(stg + lane);
+    sp.ahead = 0;
+#pragma unroll
+    for (int k = 0; k < STG - 1; ++k) {  // groups 0 .. STG-2 of this warp (one commit per slot, empty if the warp has fewer)
+        if (k < left) {
+            stage_issue(sp.s0, sp.pi, k);
+            if (pf_bytes) asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(sp.pi) + pf_bytes));
+            sp.pi += pstep;
+            ++sp.ahead;
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    }
+}
+
+template <class M, bool FAST, int STG = 0>
 __device__ __forceinline__ void group_loop(const double* col0, int64_t n, int64_t n_items, int g0, int gstep, int lane,
-                                           const typename M::Consts& c, double* acc, LogProd& lp, unsigned& bad, double t_lane)
+                                           const typename M::Consts& c, double* acc, LogProd& lp, unsigned& bad, double t_lane,
+                                           int64_t pf_bytes = 0, double2* stg = nullptr, StagePipe* spp = nullptr)
 {
     constexpr int E = M::EVENTS_PER_CALL;  // events the model evaluates together (interleaved instruction streams)
     static_assert(kGroupEvents % E == 0, "a group is a whole number of calls");
@@ -228,17 +289,52 @@ __device__ __forceinline__ void group_loop(const double* col0, int64_t n, int64_
     // this warp's full groups: g0, g0 + gstep, ... < n_full
     int left = (g0 < n_full) ? (n_full - g0 + gstep - 1) / gstep : 0;
     const int g = g0 + left * gstep;  // this warp's first group index >= n_full
-    while (left > 0) {
-        double m[kGroupEvents];
-        load_group4(p, m);
-        --left;
-        p += (left > 0) ? pstep : 0;  // after the last group: prefetches that group again (harmless)
-        prefetch_group4(p);
+    if constexpr (STG > 0) {
+        const unsigned s0 = spp->s0;
+        const double2* pi = spp->pi;
+        int ahead = spp->ahead;
+        int st = 0, st_in = STG - 1;
+        while (left > 0) {
+            if (ahead < left) {  // one more group of this warp to request
+                stage_issue(s0, pi, st_in);
+                if (pf_bytes) asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(pi) + pf_bytes));
+                pi += pstep;
+                ++ahead;
+            }
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            asm volatile("cp.async.wait_group %0;" ::"n"(STG - 1) : "memory");  // the oldest group has landed
+            double m[kGroupEvents];
 #pragma unroll
-        for (int q = 0; q < kGroupEvents / E; ++q) {
-            const double(&mq)[E] = *reinterpret_cast<const double(*)[E]>(&m[q * E]);
-            M::template events<E, FAST>(mq, c, acc, lp, bad, t_lane);
-            lp.renorm();
+            for (int i = 0; i < kGroupItems; ++i) {
+                const double2 v = stg[(st * kGroupItems + i) * 32 + lane];
+                m[2 * i] = v.x;
+                m[2 * i + 1] = v.y;
+            }
+            --left;
+            --ahead;
+            st = (st + 1 == STG) ? 0 : st + 1;
+            st_in = (st_in + 1 == STG) ? 0 : st_in + 1;
+#pragma unroll
+            for (int q = 0; q < kGroupEvents / E; ++q) {
+                const double(&mq)[E] = *reinterpret_cast<const double(*)[E]>(&m[q * E]);
+                M::template events<E, FAST>(mq, c, acc, lp, bad, t_lane);
+                lp.renorm();
+            }
+        }
+    } else {
+        while (left > 0) {
+            double m[kGroupEvents];
+            load_group4(p, m);
+            if (pf_bytes) asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(p) + pf_bytes));
+            --left;
+            p += (left > 0) ? pstep : 0;  // after the last group: prefetches that group again (harmless)
+            prefetch_group4(p);
+#pragma unroll
+            for (int q = 0; q < kGroupEvents / E; ++q) {
+                const double(&mq)[E] = *reinterpret_cast<const double(*)[E]>(&m[q * E]);
+                M::template events<E, FAST>(mq, c, acc, lp, bad, t_lane);
+                lp.renorm();
+            }
         }
     }
     // the dataset's last, partial group: index n_full, if it exists and is one of this warp's
@@ -266,25 +362,33 @@ __device__ __forceinline__ void group_loop(const double* col0, int64_t n, int64_
 //    register buffers (the loads of the next group are in flight while the current group is evaluated).
 // get_c() yields the parameter-only constants; it is called AFTER the first loads have been issued, so that a kernel
 // which must first fetch them (batched toys) overlaps that with the data latency.
-template <class M, class GetC>
+template <class M, int STG = 0, class GetC>
 __device__ __forceinline__ void accumulate(const double* const* col, int64_t n, int64_t n_items, int64_t j0,
-                                           int64_t step, GetC get_c, double* acc, unsigned& bad)
+                                           int64_t step, GetC get_c, double* acc, unsigned& bad, int64_t pf_delta = 0,
+                                           double2* stg = nullptr)
 {
     const int lane = threadIdx.x & 31;
     const double t_lane = mf_exp32_lane_entry();
     LogProd lp;
     if constexpr (M::NCOL == 1) {
         const int g0 = (int)j0, gstep = (int)step;  // group indices fit 32 bits (n_pad / 256; the host checks)
-        if (g0 < (int)((n / kItem) / kGroupItems))
-            prefetch_group4(reinterpret_cast<const double2*>(col[0]) + (int64_t)g0 * (32 * kGroupItems) + lane);
+        // lane l's pointer is 16 l bytes into the group; its prefetch goes to byte 64 l of the other dataset's group
+        const int64_t pf_bytes = pf_delta ? pf_delta * (int64_t)sizeof(double) + 48 * lane : 0;
+        StagePipe sp;
+        if constexpr (STG > 0) {
+            stage_begin<STG>(sp, col[0], n, g0, gstep, lane, stg, pf_bytes);
+        } else {
+            if (g0 < (int)((n / kItem) / kGroupItems))
+                prefetch_group4(reinterpret_cast<const double2*>(col[0]) + (int64_t)g0 * (32 * kGroupItems) + lane);
+        }
         decltype(auto) c = get_c();
         if constexpr (M::HAS_FAST) {
             if (M::is_fast(c))  // uniform over the CTA: one parameter point per CTA
-                group_loop<M, true>(col[0], n, n_items, g0, gstep, lane, c, acc, lp, bad, t_lane);
+                group_loop<M, true, STG>(col[0], n, n_items, g0, gstep, lane, c, acc, lp, bad, t_lane, pf_bytes, stg, &sp);
             else
-                group_loop<M, false>(col[0], n, n_items, g0, gstep, lane, c, acc, lp, bad, t_lane);
+                group_loop<M, false, STG>(col[0], n, n_items, g0, gstep, lane, c, acc, lp, bad, t_lane, pf_bytes, stg, &sp);
         } else {
-            group_loop<M, false>(col[0], n, n_items, g0, gstep, lane, c, acc, lp, bad, t_lane);
+            group_loop<M, false, STG>(col[0], n, n_items, g0, gstep, lane, c, acc, lp, bad, t_lane, pf_bytes, stg, &sp);
         }
     } else {
         decltype(auto) c = get_c();
@@ -564,12 +668,14 @@ __global__ void __launch_bounds__(128) batch_consts_kernel(const __grid_constant
 
 // CTA <-> (toy, event chunk)
 
-template <class M>
+// STG > 0 (one-column models, one CTA per toy): the events are staged through shared memory, STG groups deep (group_loop)
+template <class M, int STG = 0>
 __global__ void __launch_bounds__(M::BATCH_BLOCK, M::BATCH_RESIDENT_CTAS)
     nll_grad_batch_kernel(const __grid_constant__ BatchArgs<M> a)
 {
     constexpr int NACC = M::NACC;
     constexpr int kBlock = M::BATCH_BLOCK, kWarps = kBlock / 32;  // this kernel's own CTA size
+    __shared__ __align__(16) double2 s_stage[(STG > 0 ? STG : 1) * kGroupItems * 32 * (STG > 0 ? kWarps : 0) + 1];
     static_assert(kBlock >= 64 && NACC + 1 <= kBlock, "CTA too small for the reduction");
     __shared__ double sm[kWarps][NACC];
     __shared__ double s_sum[NACC];
@@ -578,15 +684,22 @@ __global__ void __launch_bounds__(M::BATCH_BLOCK, M::BATCH_RESIDENT_CTAS)
     __shared__ bool s_last;
     __shared__ typename M::Consts s_c;
     __shared__ int s_ok;
+    __shared__ double2 s_summ;
 
     pdl_launch_dependents();
     const int slot = blockIdx.x / a.chunks, chunk = blockIdx.x % a.chunks;
     // ids == NULL: every toy is active.  ids is only ever the library's own array, filled by a stream-ordered copy that is
     // complete before the constants kernel (this kernel's predecessor) can start, so it may be read ahead of the wait.
     const int64_t toy = a.shared_data ? 0 : a.ids ? a.ids[slot] : slot;
-    if (a.chunks == 1 && !a.shared_data) {
+    int64_t pf_delta = 0;  // doubles from this toy's events to those of the toy `ahead` slots further on
+    if (M::NCOL == 1 && a.ahead > 0 && slot + a.ahead < a.n_active) {
+        const int64_t next = a.ids ? a.ids[slot + a.ahead] : slot + a.ahead;
+        pf_delta = (next - toy) * a.toy_stride;
+    }
+    if (a.chunks == 1 && !a.shared_data && (a.ahead <= 0 || slot < a.ahead)) {
         // this CTA streams its toy's columns once from HBM: ask for them now (L2 prefetch, 128-byte lines), so
         // that they arrive while the constants are fetched and the first loads of the event loop hit L2
+        // (with `ahead` only the first wave: later toys were requested by their predecessors)
         const int64_t lines = (a.n_items * kItem * (int64_t)sizeof(double) + 127) / 128;
 #pragma unroll
         for (int q = 0; q < M::NCOL; ++q) {
@@ -602,10 +715,11 @@ __global__ void __launch_bounds__(M::BATCH_BLOCK, M::BATCH_RESIDENT_CTAS)
         if (threadIdx.x < W)
             reinterpret_cast<double*>(&s_c)[threadIdx.x] = reinterpret_cast<const double*>(a.consts + slot)[threadIdx.x];
         if (threadIdx.x == 0) s_ok = a.consts_ok[slot];
+        // the event-only constant of the toy (S1, complete long ago): fetched now, not when thread 0 finishes the toy
+        if (threadIdx.x == kBlock - 1) s_summ = a.sum_m ? a.sum_m[toy] : make_double2(0.0, 0.0);
     }
     constexpr int NOUT = M::NOUT;  // -ln L, gradient (and Hessian for the *Hess models); n_bad follows at [NOUT]
     double* out = a.out + (int64_t)slot * (NOUT + 1);
-    const double2 sum_m = a.sum_m ? a.sum_m[toy] : make_double2(0.0, 0.0);
     const double* col[M::NCOL];
 #pragma unroll
     for (int i = 0; i < M::NCOL; ++i) col[i] = a.col[i] + toy * a.toy_stride;
@@ -616,12 +730,12 @@ __global__ void __launch_bounds__(M::BATCH_BLOCK, M::BATCH_RESIDENT_CTAS)
     unsigned bad = 0;
     const int64_t C = a.chunks;
     // the constants become visible (barrier) only after the first event loads are in flight
-    accumulate<M>(col, a.n, a.n_items, chunk + C * (threadIdx.x >> 5), C * kWarps,
-                  [&]() -> const typename M::Consts& {
-                      __syncthreads();
-                      return s_c;
-                  },
-                  acc, bad);
+    accumulate<M, STG>(col, a.n, a.n_items, chunk + C * (threadIdx.x >> 5), C * kWarps,
+                       [&]() -> const typename M::Consts& {
+                           __syncthreads();
+                           return s_c;
+                       },
+                       acc, bad, pf_delta, s_stage + (threadIdx.x >> 5) * (STG * kGroupItems * 32));
     if (!s_ok) {  // outside the parameter domain (the sums above are garbage and unused): +inf / NaN, n_bad = -1
         if (chunk == 0 && threadIdx.x <= NOUT)
             out[threadIdx.x] = threadIdx.x == 0       ? __longlong_as_double(0x7ff0000000000000LL)
@@ -630,11 +744,18 @@ __global__ void __launch_bounds__(M::BATCH_BLOCK, M::BATCH_RESIDENT_CTAS)
         return;
     }
     const typename M::Consts& c = s_c;
+    const double2 sum_m = s_summ;
 
     const double s = block_reduce<NACC, kWarps>(acc, bad, sm, sm_bad, &s_bad_block);
     if (a.chunks == 1) {  // the CTA holds the toy's complete sums: no cross-CTA pass
-        if (threadIdx.x < NACC) s_sum[threadIdx.x] = s;
-        __syncthreads();
+        if constexpr (NACC + 1 <= 32) {  // the block sums and the bad count are held by threads of warp 0
+            if (threadIdx.x >= 32) return;
+            if (threadIdx.x < NACC) s_sum[threadIdx.x] = s;
+            __syncwarp();
+        } else {
+            if (threadIdx.x < NACC) s_sum[threadIdx.x] = s;
+            __syncthreads();
+        }
         if (threadIdx.x == 0) {
             const unsigned nb = s_bad_block;
             double o[NOUT];
