@@ -861,7 +861,7 @@ static mf_status launch_points_angular_mma(mf_model* m, int64_t n_points, const 
     // measured (C2, 1e6 events): 32 points per pass at 2 CTAs per SM (124 registers) 1.62 us per evaluation at 1000 points,
     // 64 per pass at 1 CTA per SM (212 registers) 1.85 us
     const int per_pass = (pass_env == 16 || pass_env == 32 || pass_env == 64) ? pass_env : n_points > 16 ? 32 : 16;
-    const int ctas_per_sm = per_pass == 64 ? 1 : 2;
+    const int ctas_per_sm = per_pass == 64 ? 1 : per_pass == 16 ? 3 : 2;
     const int G = (int)std::max<int64_t>(1, std::min<int64_t>((n_groups + kWarps - 1) / kWarps, ctas_per_sm * (int64_t)ctx->sm_count));
     {
         const mf_status ss = points_scratch(ctx, n_points, G);

@@ -41,7 +41,7 @@ constexpr size_t ang_points_smem()
 }
 
 template <int NPB>
-__global__ void __launch_bounds__(kBlock, (NPB <= 4) ? 2 : 1) angular_points_mma_kernel(const __grid_constant__ AngPointsArgs a)
+__global__ void __launch_bounds__(kBlock, (NPB <= 2) ? 3 : (NPB <= 4) ? 2 : 1) angular_points_mma_kernel(const __grid_constant__ AngPointsArgs a)
 {
     // dynamic shared memory: per-lane staging of the event fragments (two stages filled by cp.async: loads in flight cost no
     // registers), reused after the event loop for the cross-warp reduction
@@ -78,13 +78,19 @@ __global__ void __launch_bounds__(kBlock, (NPB <= 4) ? 2 : 1) angular_points_mma
         double2 f2, f0;
     };
     // issue: this lane's values of group grp -> stage st (asynchronous copies); fetch: stage st -> fragments
+    // this lane's four source pointers at group 0 (set once: no indexed loads of the column table in the loop)
+    const double* const src_a = a.col[1 + ft] + fg;
+    const double* const src_b = a.col[5 + ft] + fg;
+    const double* const src_c = a.col[1 + fg] + 2 * ft;
+    const double* const src_d = a.col[0] + 2 * ft;
+    const unsigned dst0 = (unsigned)__cvta_generic_to_shared(&stg[0][threadIdx.x][0]);
     auto issue = [&](int64_t grp, int st) {
         const int64_t e0 = grp * 8;
-        const unsigned dst = (unsigned)__cvta_generic_to_shared(&stg[st][threadIdx.x][0]);
-        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(a.col[1 + ft] + e0 + fg) : "memory");
-        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst + 8u), "l"(a.col[5 + ft] + e0 + fg) : "memory");
-        asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst + 16u), "l"(a.col[1 + fg] + e0 + 2 * ft) : "memory");
-        asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst + 32u), "l"(a.col[0] + e0 + 2 * ft) : "memory");
+        const unsigned dst = dst0 + (unsigned)(st * (int)sizeof(stg[0]));
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src_a + e0) : "memory");
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst + 8u), "l"(src_b + e0) : "memory");
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst + 16u), "l"(src_c + e0) : "memory");
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst + 32u), "l"(src_d + e0) : "memory");
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
     auto fetch = [&](int st, Frag& f) {
@@ -135,10 +141,30 @@ __global__ void __launch_bounds__(kBlock, (NPB <= 4) ? 2 : 1) angular_points_mma
         for (int pb = 0; pb < NPB; ++pb) dmma_m8n8k4(g[pb][0], g[pb][1], r[pb][0], f2.x);
 #pragma unroll
         for (int pb = 0; pb < NPB; ++pb) dmma_m8n8k4(g[pb][0], g[pb][1], r[pb][1], f2.y);
+        // ln L: the PDF values of a group are multiplied into the running products as they are when all of them lie in
+        // [2^-60, 2^16) (one integer max per value decides; the exponent is then extracted every fourth group: at most
+        // 8 x 60 bits of drift); otherwise (a bad or an extreme value somewhere in the lane's 2 NPB values) the general
+        // multiplication, which extracts every exponent and counts the bad events
+        constexpr int kLo = (1023 - 60) << 20;
+        constexpr unsigned kRange = 76u << 20;
+        unsigned u = 0;
 #pragma unroll
         for (int pb = 0; pb < NPB; ++pb) {
-            lp[pb].mul(c[pb][0], bad[pb]);
-            lp[pb].mul(c[pb][1], bad[pb]);
+            u = max(u, (unsigned)(__double2hiint(c[pb][0]) - kLo));
+            u = max(u, (unsigned)(__double2hiint(c[pb][1]) - kLo));
+        }
+        if (u < kRange) {
+#pragma unroll
+            for (int pb = 0; pb < NPB; ++pb) {
+                lp[pb].mul_bounded(c[pb][0]);
+                lp[pb].mul_bounded(c[pb][1]);
+            }
+        } else {
+#pragma unroll
+            for (int pb = 0; pb < NPB; ++pb) {
+                lp[pb].mul(c[pb][0], bad[pb]);
+                lp[pb].mul(c[pb][1], bad[pb]);
+            }
         }
     };
     int64_t gi = blockIdx.x + G * warp;
@@ -157,7 +183,7 @@ __global__ void __launch_bounds__(kBlock, (NPB <= 4) ? 2 : 1) angular_points_mma
         process(gi, f);
         gi += step;
         st ^= 1;
-        if (++since_renorm == 256) {  // 512 mantissas in [1, 2) per running product since the last one
+        if (++since_renorm == 4) {  // 8 factors in [2^-60, 2^16) (or mantissas in [1, 2)) per running product since the last one
             since_renorm = 0;
 #pragma unroll
             for (int pb = 0; pb < NPB; ++pb) lp[pb].renorm();

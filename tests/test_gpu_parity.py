@@ -201,6 +201,33 @@ def test_batch_parity(mf, ctx, n_events):
     assert nll2[1] == nll[1] and np.array_equal(g2[1], g[1])
 
 
+def test_batch_many_toys_active_subset(mf, ctx):
+    """More toys than CTAs resident at once (the kernel then requests the events of the toy `ahead` slots further on while it
+    evaluates its own, through the list of active toys), ragged toy length (not a multiple of the 256-event group), an active
+    subset: EVERY active toy against the oracle; inactive rows untouched; a second call with all toys active."""
+    T, n = 700, 1337
+    toys = dg.gen_mass_toys(T, n, first_seed=4000)
+    model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(toys, dg.MASS_LO, dg.MASS_HI, n_toys=T))
+    lams = dg.gen_lambda_points(T, 6, dg.MASS_TRUTH, 3 * dg.mass_sigma_stat(n))
+    active = (np.random.default_rng(8).uniform(size=T) < 0.6).astype(np.uint8)
+    active[0] = 0
+    active[T - 1] = 1
+    nll, g = model.nll_grad_batch(lams, active)
+    for t in range(T):
+        if not active[t]:
+            assert math.isnan(nll[t]) and np.all(np.isnan(g[t]))
+            continue
+        o_nll, o_g, _ = oracle.nll_grad(oracle.MASS, toys[t], lams[t], dg.MASS_LO, dg.MASS_HI)
+        assert_parity(nll[t], g[t], o_nll, o_g, f"toy {t} (subset)")
+    nll_all, g_all = model.nll_grad_batch(lams)
+    for t in range(T):
+        if active[t]:  # the same toy at the same point: the same bits, whatever its slot and neighbours
+            assert nll_all[t] == nll[t] and np.array_equal(g_all[t], g[t])
+        else:
+            o_nll, o_g, _ = oracle.nll_grad(oracle.MASS, toys[t], lams[t], dg.MASS_LO, dg.MASS_HI)
+            assert_parity(nll_all[t], g_all[t], o_nll, o_g, f"toy {t} (all)")
+
+
 def test_batch_angular_parity(mf, ctx):
     T, n = 3, 4000
     ev = np.stack([dg.gen_angular(n, seed=40 + t) for t in range(T)], axis=1)  # [3][T][n]

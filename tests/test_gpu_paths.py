@@ -273,18 +273,26 @@ _ABLATION = textwrap.dedent("""
     lam = np.tile(np.array(dg.MASS_TRUTH), (6, 1))
     bn, bg = bm.nll_grad_batch(lam)
     check(bn[5], bg[5], oracle.nll_grad(oracle.MASS, toys[5], lam[5], dg.MASS_LO, dg.MASS_HI))
+    toys = dg.gen_mass_toys(400, 700, first_seed=20)     # more toys than resident CTAs of a small grid, ragged groups
+    bm2 = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(toys, dg.MASS_LO, dg.MASS_HI, n_toys=400))
+    lam = np.tile(np.array(dg.MASS_TRUTH), (400, 1))
+    bn, bg = bm2.nll_grad_batch(lam)
+    for t in (0, 147, 148, 399):
+        check(bn[t], bg[t], oracle.nll_grad(oracle.MASS, toys[t], lam[t], dg.MASS_LO, dg.MASS_HI))
     r = mm.fit(dg.MASS_START)
     assert r.converged
     print("ablation ok")
 """)
 
 
-@pytest.mark.parametrize("switch", ["MF_NO_TMA", "MF_NO_PDL", "MF_NO_POINTS_MMA"])
+@pytest.mark.parametrize("switch", ["MF_NO_TMA", "MF_NO_PDL", "MF_NO_POINTS_MMA", "MF_BATCH_STAGES=0", "MF_BATCH_STAGES=2"])
 def test_ablation_switches_vs_oracle(mf, switch):
-    """The MF_NO_TMA=1 (register-buffer kernels for the angular / 4D models) and MF_NO_PDL=1 (plain stream order) paths
-    that DESIGN.md quotes numbers for, against the oracle."""
+    """The MF_NO_TMA=1 (register-buffer kernels for the angular / 4D models), MF_NO_PDL=1 (plain stream order),
+    MF_NO_POINTS_MMA=1 and MF_BATCH_STAGES=0 (batched toys with direct loads) paths that DESIGN.md quotes numbers for,
+    against the oracle."""
     env = dict(os.environ)
-    env[switch] = "1"
+    name, _, value = switch.partition("=")
+    env[name] = value or "1"
     p = subprocess.run([sys.executable, "-c", _ABLATION.format(root=ROOT)], env=env, capture_output=True, text=True, timeout=600)
     assert p.returncode == 0 and "ablation ok" in p.stdout, p.stdout[-2000:] + p.stderr[-4000:]
 
