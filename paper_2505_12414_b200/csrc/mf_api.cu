@@ -849,6 +849,24 @@ static mf_status points_scratch(mf_ctx* ctx, int64_t n_points, int chunks)
 
 // The angular model's many-points evaluation as two tensor-core contractions (mf_points.cuh): one pass over the data per
 // 64 points.  out_dev rows are K + 2 = 10 doubles.
+// Width of the grid (G, passes) of the many-points kernels: G CTAs share the events of one pass.  Whole waves: the smallest
+// G >= slots / 4 for which G x passes fills its waves of `slots` resident CTAs to >= 97 % (measured, C2: 64 points 1.89 us per
+// evaluation at G = 296 -> 1.78 at 148; 128 points 1.69 -> 1.54 at G = 74; CTAs of different passes on one SM read the same
+// events: L1 hits).  MF_POINTS_G overrides (tuning knob).
+static int points_grid_width(int slots, int64_t passes, int64_t n_groups)
+{
+    static const int g_env = std::getenv("MF_POINTS_G") ? std::atoi(std::getenv("MF_POINTS_G")) : 0;
+    int g_pick = slots;
+    for (int g = std::max(1, slots / 4); g < slots; ++g) {
+        const int64_t ctas = g * passes, waves = (ctas + slots - 1) / slots;
+        if ((double)ctas >= 0.97 * (double)(waves * slots)) {
+            g_pick = g;
+            break;
+        }
+    }
+    return (int)std::max<int64_t>(1, std::min<int64_t>((n_groups + kWarps - 1) / kWarps, g_env > 0 ? g_env : g_pick));
+}
+
 static mf_status launch_points_angular_mma(mf_model* m, int64_t n_points, const double* lambdas, double* out_dev)
 {
     mf_ctx* ctx = m->ctx;
@@ -862,7 +880,7 @@ static mf_status launch_points_angular_mma(mf_model* m, int64_t n_points, const 
     // 64 per pass at 1 CTA per SM (212 registers) 1.85 us
     const int per_pass = (pass_env == 16 || pass_env == 32 || pass_env == 64) ? pass_env : n_points > 16 ? 32 : 16;
     const int ctas_per_sm = per_pass == 64 ? 1 : per_pass == 16 ? 3 : 2;
-    const int G = (int)std::max<int64_t>(1, std::min<int64_t>((n_groups + kWarps - 1) / kWarps, ctas_per_sm * (int64_t)ctx->sm_count));
+    const int G = points_grid_width(ctas_per_sm * ctx->sm_count, (n_points + per_pass - 1) / per_pass, n_groups);
     {
         const mf_status ss = points_scratch(ctx, n_points, G);
         if (ss != MF_OK) return ss;
@@ -908,7 +926,9 @@ static mf_status launch_points_fourd_mma(mf_model* m, int64_t n_points, const do
     mf_ctx* ctx = m->ctx;
     *handled = true;
     const int64_t n_groups = m->n_pad / 8;
-    const int G = (int)std::max<int64_t>(1, std::min<int64_t>((n_groups + kWarps - 1) / kWarps, 2 * (int64_t)ctx->sm_count));  // 2 CTAs per SM
+    static const int pass_env4 = std::getenv("MF_POINTS4D_PER_PASS") ? std::atoi(std::getenv("MF_POINTS4D_PER_PASS")) : 0;  // tuning knob
+    const int per_pass = (pass_env4 == 16 || pass_env4 == 24 || pass_env4 == 32) ? pass_env4 : 16;
+    const int G = points_grid_width(2 * ctx->sm_count, (n_points + per_pass - 1) / per_pass, n_groups);  // 2 CTAs per SM
     char* h_blk = nullptr;
     int stage = 0;
     const size_t per_point = sizeof(double) * (16 + kP4PointConsts + kP4FinishConsts);
@@ -973,8 +993,6 @@ static mf_status launch_points_fourd_mma(mf_model* m, int64_t n_points, const do
     MF_CUDA(ctx, cudaMemcpyAsync(d_blk, h_blk, per_point * n_points, cudaMemcpyHostToDevice, ctx->stream));
     MF_CUDA(ctx, cudaEventRecord(ctx->pts_copied[stage], ctx->stream));
     take_fresh(m);
-    static const int pass_env4 = std::getenv("MF_POINTS4D_PER_PASS") ? std::atoi(std::getenv("MF_POINTS4D_PER_PASS")) : 0;  // tuning knob
-    const int per_pass = (pass_env4 == 16 || pass_env4 == 24 || pass_env4 == 32) ? pass_env4 : 16;
     const dim3 grid((unsigned)G, (unsigned)((n_points + per_pass - 1) / per_pass));
     const size_t smem4 = sizeof(double) * 2 * kBlock * kP4StageDoubles;  // 48 KB: above the default dynamic limit with the static part
     static const cudaError_t attr4 = [&] {
