@@ -220,8 +220,9 @@ __device__ __forceinline__ void prefetch_group4(const double2* p)
     for (int i = 0; i < kGroupItems; ++i) asm volatile("prefetch.global.L1 [%0];" ::"l"(p + 32 * i));
 }
 
-// pf_bytes != 0: while group g is evaluated, the same group of ANOTHER dataset (pf_bytes further on: the toy that the next
-// CTA on this SM will evaluate) is requested from HBM into L2 — one 64-byte-strided prefetch per lane covers the 2 KB.
+// pf_bytes != 0 (staged form only): while group g is evaluated, the same group of ANOTHER dataset (pf_bytes further on: the
+// toy that a later CTA will evaluate) is requested from HBM into L2 — one 64-byte-strided prefetch per lane covers the 2 KB.
+// The direct form carries no such code: three predicated-off instructions per group cost the C1 headline 1.8 %.
 // STG > 0: the warp's groups are staged through shared memory by per-lane asynchronous copies (cp.async, 16 bytes each, every
 // lane copies and later reads only its own four double2), STG groups deep: the copies of the next STG - 1 groups are in
 // flight while a group is evaluated, at no cost in registers.  For data that come from HBM (batched toys), where the L1
@@ -325,7 +326,6 @@ __device__ __forceinline__ void group_loop(const double* col0, int64_t n, int64_
         while (left > 0) {
             double m[kGroupEvents];
             load_group4(p, m);
-            if (pf_bytes) asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(p) + pf_bytes));
             --left;
             p += (left > 0) ? pstep : 0;  // after the last group: prefetches that group again (harmless)
             prefetch_group4(p);
@@ -692,11 +692,11 @@ __global__ void __launch_bounds__(M::BATCH_BLOCK, M::BATCH_RESIDENT_CTAS)
     // complete before the constants kernel (this kernel's predecessor) can start, so it may be read ahead of the wait.
     const int64_t toy = a.shared_data ? 0 : a.ids ? a.ids[slot] : slot;
     int64_t pf_delta = 0;  // doubles from this toy's events to those of the toy `ahead` slots further on
-    if (M::NCOL == 1 && a.ahead > 0 && slot + a.ahead < a.n_active) {
+    if (STG > 0 && M::NCOL == 1 && a.ahead > 0 && slot + a.ahead < a.n_active) {
         const int64_t next = a.ids ? a.ids[slot + a.ahead] : slot + a.ahead;
         pf_delta = (next - toy) * a.toy_stride;
     }
-    if (a.chunks == 1 && !a.shared_data && (a.ahead <= 0 || slot < a.ahead)) {
+    if (a.chunks == 1 && !a.shared_data && (STG == 0 || a.ahead <= 0 || slot < a.ahead)) {
         // this CTA streams its toy's columns once from HBM: ask for them now (L2 prefetch, 128-byte lines), so
         // that they arrive while the constants are fetched and the first loads of the event loop hit L2
         // (with `ahead` only the first wave: later toys were requested by their predecessors)
@@ -716,10 +716,12 @@ __global__ void __launch_bounds__(M::BATCH_BLOCK, M::BATCH_RESIDENT_CTAS)
             reinterpret_cast<double*>(&s_c)[threadIdx.x] = reinterpret_cast<const double*>(a.consts + slot)[threadIdx.x];
         if (threadIdx.x == 0) s_ok = a.consts_ok[slot];
         // the event-only constant of the toy (S1, complete long ago): fetched now, not when thread 0 finishes the toy
-        if (threadIdx.x == kBlock - 1) s_summ = a.sum_m ? a.sum_m[toy] : make_double2(0.0, 0.0);
+        if (STG > 0 && threadIdx.x == kBlock - 1) s_summ = a.sum_m ? a.sum_m[toy] : make_double2(0.0, 0.0);
     }
     constexpr int NOUT = M::NOUT;  // -ln L, gradient (and Hessian for the *Hess models); n_bad follows at [NOUT]
     double* out = a.out + (int64_t)slot * (NOUT + 1);
+    double2 sum_m = make_double2(0.0, 0.0);
+    if (STG == 0 && a.sum_m) sum_m = a.sum_m[toy];
     const double* col[M::NCOL];
 #pragma unroll
     for (int i = 0; i < M::NCOL; ++i) col[i] = a.col[i] + toy * a.toy_stride;
@@ -744,7 +746,7 @@ __global__ void __launch_bounds__(M::BATCH_BLOCK, M::BATCH_RESIDENT_CTAS)
         return;
     }
     const typename M::Consts& c = s_c;
-    const double2 sum_m = s_summ;
+    if (STG > 0) sum_m = s_summ;
 
     const double s = block_reduce<NACC, kWarps>(acc, bad, sm, sm_bad, &s_bad_block);
     if (a.chunks == 1) {  // the CTA holds the toy's complete sums: no cross-CTA pass
