@@ -195,9 +195,10 @@ __device__ __forceinline__ void compute_group(int64_t n, int64_t n_items, int64_
 // The event loop of one warp for the one-column (ALU-bound) models.  The unit is a GROUP of kGroupItems = 4 consecutive
 // items = 256 consecutive events = 2 KB: lane l owns events 2l, 2l+1 of each of the four 64-event rows, read as four
 // 16-byte loads at immediate offsets from ONE pointer (one 64-bit pointer add and one 32-bit counter per group).
-// Groups g0, g0 + gstep, ... .  Latency: while a group is evaluated the warp's NEXT group is prefetched into L1 (four
-// prefetch instructions, no registers), so the loads at the top of the next iteration hit L1; keeping the next group in
-// registers instead (a second buffer, or a refill of the first) made ptxas copy the buffer twice per iteration.
+// Groups g0, g0 + gstep, ... .  Latency: direct form (data from L2: one dataset, many points or launches): the other three
+// warps of the SM sub-partition cover the L2 latency of the four loads; an L1 prefetch of the next group (round 1) was
+// measured to do nothing (ncu: 5 % L1 hit rate on those loads; without it the C1 sweep is 0.7 % faster) and keeping the next
+// group in registers made ptxas copy the buffer twice per iteration.  Staged form (data from HBM: batched toys): below.
 // FAST selects the model's fast event body (M::events<E, true>; decided per parameter point, M::is_fast).  The last,
 // partial group of the dataset (fewer than four items, or a ragged last item) is evaluated item by item by the warp it
 // falls to; only a ragged item is predicated.
@@ -214,19 +215,12 @@ __device__ __forceinline__ void load_group4(const double2* __restrict__ p, doubl
     }
 }
 
-__device__ __forceinline__ void prefetch_group4(const double2* p)
-{
-#pragma unroll
-    for (int i = 0; i < kGroupItems; ++i) asm volatile("prefetch.global.L1 [%0];" ::"l"(p + 32 * i));
-}
-
 // pf_bytes != 0 (staged form only): while group g is evaluated, the same group of ANOTHER dataset (pf_bytes further on: the
 // toy that a later CTA will evaluate) is requested from HBM into L2 — one 64-byte-strided prefetch per lane covers the 2 KB.
-// The direct form carries no such code: three predicated-off instructions per group cost the C1 headline 1.8 %.
 // STG > 0: the warp's groups are staged through shared memory by per-lane asynchronous copies (cp.async, 16 bytes each, every
 // lane copies and later reads only its own four double2), STG groups deep: the copies of the next STG - 1 groups are in
-// flight while a group is evaluated, at no cost in registers.  For data that come from HBM (batched toys), where the L1
-// prefetch of the direct form does not cover the latency (ncu: 22 % of the warp samples on the first use of a loaded value).
+// flight while a group is evaluated, at no cost in registers.  For data that come from HBM (batched toys), where the
+// direct form leaves the latency exposed (ncu: 22 % of the warp samples on the first use of a loaded value).
 // stg: this warp's staging area, STG x 4 x 32 double2.
 // state of the staging pipeline of one warp (STG > 0): started by stage_begin() BEFORE the parameter-only constants are
 // waited for, so that the first copies are in flight during that wait
@@ -327,8 +321,7 @@ __device__ __forceinline__ void group_loop(const double* col0, int64_t n, int64_
             double m[kGroupEvents];
             load_group4(p, m);
             --left;
-            p += (left > 0) ? pstep : 0;  // after the last group: prefetches that group again (harmless)
-            prefetch_group4(p);
+            p += pstep;
 #pragma unroll
             for (int q = 0; q < kGroupEvents / E; ++q) {
                 const double(&mq)[E] = *reinterpret_cast<const double(*)[E]>(&m[q * E]);
@@ -375,12 +368,7 @@ __device__ __forceinline__ void accumulate(const double* const* col, int64_t n, 
         // lane l's pointer is 16 l bytes into the group; its prefetch goes to byte 64 l of the other dataset's group
         const int64_t pf_bytes = pf_delta ? pf_delta * (int64_t)sizeof(double) + 48 * lane : 0;
         StagePipe sp;
-        if constexpr (STG > 0) {
-            stage_begin<STG>(sp, col[0], n, g0, gstep, lane, stg, pf_bytes);
-        } else {
-            if (g0 < (int)((n / kItem) / kGroupItems))
-                prefetch_group4(reinterpret_cast<const double2*>(col[0]) + (int64_t)g0 * (32 * kGroupItems) + lane);
-        }
+        if constexpr (STG > 0) stage_begin<STG>(sp, col[0], n, g0, gstep, lane, stg, pf_bytes);
         decltype(auto) c = get_c();
         if constexpr (M::HAS_FAST) {
             if (M::is_fast(c))  // uniform over the CTA: one parameter point per CTA
