@@ -311,6 +311,29 @@ mf_status mf_toy_study_mass(mf_ctx* ctx, uint64_t seed0, int64_t n_toys, int64_t
 mf_status mf_toy_study_angular(mf_ctx* ctx, uint64_t seed0, int64_t n_toys, int64_t n_events, const double* a_truth,
                                const mf_fit_opts* opts, mf_fit_result* results);
 
+/* ---- an evaluation that allocates nothing ------------------------------------------------------------------ */
+
+/* For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it):
+ * ONE evaluation of -ln L(lambda) and its gradient for the mass model (Eq. 1; Eq. 2 / Eq. 3) on
+ * events the caller already holds on the device, with no dataset or model object.  The kernel's cross-CTA scratch (one row of
+ * partial sums per 8192 events, the completion ticket) is a fixed array of 246,016 bytes in the library's device image, held
+ * by every GPU that loads the library until the process exits; nothing is allocated or freed by this call (no cudaMalloc,
+ * cudaFree, cudaHostAlloc, no stream-ordered pool), it enqueues one 256-byte memset and one kernel and does not synchronise.
+ *   m_dev    device, n doubles, 16-byte aligned, unpadded; NOT range-checked: every event must lie in [lo, hi].
+ *   n        0 <= n <= MF_NOALLOC_MAX_EVENTS; more: MF_ERR_ARG, text in mf_last_error, nothing enqueued.
+ *   lambda   host, 4 doubles (f, mu, sigma, tau), read before the call returns; MF_ERR_PARAM_DOMAIN as for mf_nll_grad.
+ *   out_dev  device, 6 doubles, written in stream order: -ln L, the 4 gradient components, n_bad (events with P <= 0;
+ *            when non-zero the value is +inf and the gradient NaN).
+ *   stream   a cudaStream_t, or NULL for the context's stream.
+ * Every call on a device shares the one scratch array: calls ordered on one stream are safe (the ticket word is cleared on
+ * the stream before each kernel, rows are overwritten before they are read); calls that OVERLAP on the GPU — two streams,
+ * two host threads, parallel graph branches — race on it and return garbage.  The first call on a device resolves the
+ * array's device address (cudaGetSymbolAddress): make it once outside stream capture.  The result agrees with mf_nll_grad
+ * to rounding (not bit for bit: fixed 8192-event chunks, general event body) and does not depend on the SM count. */
+#define MF_NOALLOC_MAX_EVENTS 33554432 /* 2^25 */
+mf_status mf_nll_grad_mass_noalloc(mf_ctx* ctx, const double* m_dev, int64_t n, double lo, double hi, const double* lambda,
+                                   double* out_dev, void* stream);
+
 /* ---- multi-GPU: S5 across ranks ------------------------------------------------------ */
 
 /* Combines the partial sums of n_ranks event shards of ONE dataset (each rank's mf_nll_grad on its shard: -ln L and the

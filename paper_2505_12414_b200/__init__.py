@@ -37,8 +37,9 @@ EXPORTS = [
     "mf_nll_grad", "mf_nll_grad_async", "mf_nll_grad_points", "mf_nll_grad_sweep", "mf_nll_grad_batch", "mf_nll_grad_batch_async",
     "mf_model_serve", "mf_model_is_served", "mf_model_has_hessian", "mf_model_is_weighted", "mf_nll_grad_hess", "mf_nll_grad_hess_fisher", "mf_nll_grad_hess_batch",
     "mf_fit_opts_default", "mf_fit", "mf_fit_batch", "mf_toy_study_mass", "mf_toy_study_angular",
-    "mf_combine_partials",
+    "mf_combine_partials", "mf_nll_grad_mass_noalloc",
 ]
+MF_NOALLOC_MAX_EVENTS = 1 << 25
 
 
 class MoreFitError(RuntimeError):
@@ -201,6 +202,8 @@ def load_library() -> ctypes.CDLL:
                                       ctypes.POINTER(_FitResultC)]
     lib.mf_toy_study_angular.restype = ctypes.c_int
     lib.mf_toy_study_angular.argtypes = [vp, ctypes.c_uint64, i64, i64, dp, ctypes.POINTER(FitOpts), ctypes.POINTER(_FitResultC)]
+    lib.mf_nll_grad_mass_noalloc.restype = ctypes.c_int
+    lib.mf_nll_grad_mass_noalloc.argtypes = [vp, vp, i64, ctypes.c_double, ctypes.c_double, dp, vp, vp]
     lib.mf_nll_grad_sweep.restype = ctypes.c_int
     lib.mf_nll_grad_sweep.argtypes = [vp, i64, dp, dp, dp, ctypes.POINTER(i64)]
     lib.mf_combine_partials.restype = ctypes.c_int
@@ -325,6 +328,17 @@ class Context:
                                                    None if opts is None else ctypes.byref(opts),
                                                    res.ctypes.data_as(ctypes.POINTER(_FitResultC))))
         return BatchFitResult(res, int(n_toys), 8)
+
+    def nll_grad_mass_noalloc(self, m_dev_ptr: int, n: int, lo: float, hi: float, lam, out_dev_ptr: int, stream: int = 0) -> None:
+        """mf_nll_grad_mass_noalloc: one mass-model evaluation on n device-resident events (16-byte aligned pointer) that
+        allocates nothing (fixed scratch in the library image, n <= MF_NOALLOC_MAX_EVENTS); 6 doubles (-ln L, gradient,
+        n_bad) are written to out_dev_ptr in stream order.  Calls that overlap on the GPU race on the scratch."""
+        lam = np.ascontiguousarray(lam, dtype=np.float64)
+        if lam.shape != (4,):
+            raise ValueError("lam must have 4 entries")
+        self._check(self._lib.mf_nll_grad_mass_noalloc(self._h, ctypes.c_void_p(int(m_dev_ptr)), int(n), float(lo), float(hi),
+                                                       _dp(lam), ctypes.c_void_p(int(out_dev_ptr)),
+                                                       ctypes.c_void_p(int(stream)) if stream else None))
 
     def model_create(self, kind: int, dataset: "Dataset") -> "Model":
         return Model(self, kind, dataset)

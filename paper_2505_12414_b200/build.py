@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB_DIR = os.path.join(HERE, "lib")
 LIB_PATH = os.path.join(LIB_DIR, "libmorefit_b200.so")
-SOURCES = ["mf_api.cu", "mf_fit.cpp", "mf_dist.cpp", "mf_generate.cu"]
+SOURCES = ["mf_api.cu", "mf_fit.cpp", "mf_dist.cpp", "mf_generate.cu", "mf_noalloc.cu"]
 PROBE_LIB_PATH = os.path.join(LIB_DIR, "libmorefit_b200_probe.so")
 PROBE_SOURCES = ["mf_probe.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
