@@ -1434,7 +1434,17 @@ static mf_status launch_batch(mf_model* m, int n_active, const double* lam_dev =
         // one-column toys come from HBM: events staged through shared memory by cp.async, 3 groups deep (0: direct loads)
         static const int env_stages = [] { const char* e = getenv("MF_BATCH_STAGES"); return e ? atoi(e) : 3; }();
         const int stages = env_stages;
-        if (stages == 2) MF_CUDA(ctx, launch_pdl(nll_grad_batch_kernel<M, 2>, n_active * m->chunks, ctx->stream, a, M::BATCH_BLOCK));
+        // CTA size by the number of active toys (BatchShape, mf_kernels.cuh): measured cross-overs at 24 and 40 toys per SM
+        static const int env_block = [] { const char* e = getenv("MF_BATCH_BLOCK"); return e ? atoi(e) : 0; }();  // tuning knob
+        const int block = (m->chunks != 1 || stages != 3)                ? 0
+                          : (env_block == 32 || env_block == 64)         ? env_block
+                          : env_block                                    ? 0
+                          : (n_active >= 40 * (int64_t)ctx->sm_count)    ? 32
+                          : (n_active >= 24 * (int64_t)ctx->sm_count)    ? 64
+                                                                         : 0;
+        if (block == 32) MF_CUDA(ctx, launch_pdl(nll_grad_batch_kernel<M, 3, 32>, n_active, ctx->stream, a, 32));
+        else if (block == 64) MF_CUDA(ctx, launch_pdl(nll_grad_batch_kernel<M, 3, 64>, n_active, ctx->stream, a, 64));
+        else if (stages == 2) MF_CUDA(ctx, launch_pdl(nll_grad_batch_kernel<M, 2>, n_active * m->chunks, ctx->stream, a, M::BATCH_BLOCK));
         else if (stages == 3) MF_CUDA(ctx, launch_pdl(nll_grad_batch_kernel<M, 3>, n_active * m->chunks, ctx->stream, a, M::BATCH_BLOCK));
         else if (stages == 4) MF_CUDA(ctx, launch_pdl(nll_grad_batch_kernel<M, 4>, n_active * m->chunks, ctx->stream, a, M::BATCH_BLOCK));
         else MF_CUDA(ctx, launch_pdl(nll_grad_batch_kernel<M>, n_active * m->chunks, ctx->stream, a, M::BATCH_BLOCK));

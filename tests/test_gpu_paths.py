@@ -285,10 +285,12 @@ _ABLATION = textwrap.dedent("""
 """)
 
 
-@pytest.mark.parametrize("switch", ["MF_NO_TMA", "MF_NO_PDL", "MF_NO_POINTS_MMA", "MF_BATCH_STAGES=0", "MF_BATCH_STAGES=2"])
+@pytest.mark.parametrize("switch", ["MF_NO_TMA", "MF_NO_PDL", "MF_NO_POINTS_MMA", "MF_BATCH_STAGES=0", "MF_BATCH_STAGES=2",
+                                    "MF_BATCH_BLOCK=32", "MF_BATCH_BLOCK=64"])
 def test_ablation_switches_vs_oracle(mf, switch):
     """The MF_NO_TMA=1 (register-buffer kernels for the angular / 4D models), MF_NO_PDL=1 (plain stream order),
-    MF_NO_POINTS_MMA=1 and MF_BATCH_STAGES=0 (batched toys with direct loads) paths that DESIGN.md quotes numbers for,
+    MF_NO_POINTS_MMA=1, MF_BATCH_STAGES=0 (batched toys with direct loads) and MF_BATCH_BLOCK=32 / 64 (the one- and two-warp
+    CTAs that the library picks by itself from 5920 / 3552 active toys on) paths that DESIGN.md quotes numbers for,
     against the oracle."""
     env = dict(os.environ)
     name, _, value = switch.partition("=")
