@@ -238,10 +238,13 @@ extern "C" mf_status mf_dataset_upload(mf_ctx* ctx, int ndim, int64_t n_events, 
         const cudaMemcpyKind kind = (where == MF_HOST) ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
         for (int j = 0; j < ndim; ++j) {
             double* dst = buf->p + (int64_t)j * per_dim;
-            // toy rows of n_events doubles -> rows of n_pad doubles
-            MF_CUDA_C(cudaMemcpy2DAsync(dst, (size_t)ds->n_pad * sizeof(double), columns[j],
-                                        (size_t)n_events * sizeof(double), (size_t)n_events * sizeof(double),
-                                        (size_t)n_toys, kind, ctx->stream));
+            // toy rows of n_events doubles -> rows of n_pad doubles; one row (or no padding): a plain 1-D copy
+            if (n_toys == 1 || ds->n_pad == n_events)
+                MF_CUDA_C(cudaMemcpyAsync(dst, columns[j], (size_t)n_toys * n_events * sizeof(double), kind, ctx->stream));
+            else
+                MF_CUDA_C(cudaMemcpy2DAsync(dst, (size_t)ds->n_pad * sizeof(double), columns[j],
+                                            (size_t)n_events * sizeof(double), (size_t)n_events * sizeof(double),
+                                            (size_t)n_toys, kind, ctx->stream));
         }
         if (ds->n_pad > n_events) {
             const int64_t rows = (int64_t)ndim * n_toys;
