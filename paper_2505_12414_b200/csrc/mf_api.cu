@@ -914,7 +914,7 @@ static mf_status launch_points_angular_mma(mf_model* m, int64_t n_points, const 
     if (per_pass == 64) angular_points_mma_kernel<8><<<grid, kBlock, ang_points_smem<8>(), ctx->stream>>>(a);
     else if (per_pass == 32) angular_points_mma_kernel<4><<<grid, kBlock, ang_points_smem<4>(), ctx->stream>>>(a);
     else angular_points_mma_kernel<2><<<grid, kBlock, ang_points_smem<2>(), ctx->stream>>>(a);
-    angular_points_combine_kernel<<<(unsigned)((n_points + kWarps - 1) / kWarps), kBlock, 0, ctx->stream>>>(
+    angular_points_combine_kernel<<<(unsigned)n_points, kAngCombineThreads, 0, ctx->stream>>>(
         a.partials, a.bad_partials, G, (int)n_points, out_dev);
     MF_CUDA(ctx, cudaGetLastError());
     ctx->launches += 2;
@@ -1008,7 +1008,7 @@ static mf_status launch_points_fourd_mma(mf_model* m, int64_t n_points, const do
     if (per_pass == 32) fourd_points_mma_kernel<4><<<grid, kBlock, smem4, ctx->stream>>>(a);
     else if (per_pass == 24) fourd_points_mma_kernel<3><<<grid, kBlock, smem4, ctx->stream>>>(a);
     else fourd_points_mma_kernel<2><<<grid, kBlock, smem4, ctx->stream>>>(a);
-    fourd_points_combine_kernel<<<(unsigned)((n_points + kWarps - 1) / kWarps), kBlock, 0, ctx->stream>>>(
+    fourd_points_combine_kernel<<<(unsigned)n_points, kP4CombineThreads, 0, ctx->stream>>>(
         a.partials, a.bad_partials, G, (int)n_points, d_fc, m->d_sum_m, (double)m->n_events, out_dev);
     MF_CUDA(ctx, cudaGetLastError());
     ctx->launches += 2;

@@ -225,41 +225,72 @@ __global__ void __launch_bounds__(kBlock, (NPB <= 2) ? 3 : (NPB <= 4) ? 2 : 1) a
     }
 }
 
-// One warp per point: fixed-order Kahan sums of the CTA partials, then out[p] = (-ln L, gradient[8], n_bad).
-__global__ void __launch_bounds__(kBlock) angular_points_combine_kernel(const double* __restrict__ partials,
-                                                                       const unsigned* __restrict__ bad_partials, int G,
-                                                                       int n_points, double* __restrict__ out)
+// Fixed-order compensated sum of G partials by one warp: lane l adds partials l, l + 32, ... (Kahan), the 32 (sum, compensation)
+// pairs are merged by a two-sum tree.  The loads of a lane are issued eight at a time, independently of the running sum.
+__device__ __forceinline__ double warp_combine_partials(const double* __restrict__ pk, int G, int lane)
 {
-    const int lane = threadIdx.x & 31, p = blockIdx.x * kWarps + (threadIdx.x >> 5);
-    if (p >= n_points) return;
-    unsigned nb = 0;
-    for (int i = lane; i < G; i += 32) nb += __ldcg(bad_partials + (int64_t)p * G + i);
-    nb = __reduce_add_sync(0xffffffffu, nb);
-    double* o = out + (int64_t)p * 10;
-    for (int k = 0; k < 9; ++k) {
-        const double* pk = partials + ((int64_t)p * 9 + k) * G;
-        double s = 0.0, cc = 0.0;
-        for (int i = lane; i < G; i += 32) {
-            const double y = __ldcg(pk + i) - cc;
-            const double t = s + y;
-            cc = (t - s) - y;
-            s = t;
-        }
-        double lo = -cc;
+    double s = 0.0, cc = 0.0;
+    for (int base = lane; base < G; base += 256) {
+        double v[8];
 #pragma unroll
-        for (int off = 16; off > 0; off >>= 1) {
-            const double s2 = __shfl_down_sync(0xffffffffu, s, off);
-            const double lo2 = __shfl_down_sync(0xffffffffu, lo, off);
-            const double t = s + s2;
-            const double bb = t - s;
-            const double e = (s - (t - bb)) + (s2 - bb);
-            lo = (lo + lo2) + e;
-            s = t;
-        }
-        if (lane == 0)
-            o[k] = !nb ? -(s + lo) : (k == 0) ? __longlong_as_double(0x7ff0000000000000LL) : __longlong_as_double(0x7ff8000000000000LL);
+        for (int j = 0; j < 8; ++j) v[j] = (base + 32 * j < G) ? __ldcg(pk + base + 32 * j) : 0.0;
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+            if (base + 32 * j < G) {
+                const double y = v[j] - cc;
+                const double t = s + y;
+                cc = (t - s) - y;
+                s = t;
+            }
     }
-    if (lane == 0) o[9] = (double)nb;
+    double lo = -cc;
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        const double s2 = __shfl_down_sync(0xffffffffu, s, off);
+        const double lo2 = __shfl_down_sync(0xffffffffu, lo, off);
+        const double t = s + s2;
+        const double bb = t - s;
+        const double e = (s - (t - bb)) + (s2 - bb);
+        lo = (lo + lo2) + e;
+        s = t;
+    }
+    return s + lo;  // lane 0
+}
+
+__device__ __forceinline__ unsigned warp_combine_bad(const unsigned* __restrict__ bp, int G, int lane)
+{
+    unsigned nb = 0;
+    for (int i = lane; i < G; i += 32) nb += __ldcg(bp + i);
+    return __reduce_add_sync(0xffffffffu, nb);
+}
+
+// One CTA per point, one warp per quantity (9 sums + the bad-event count): out[p] = (-ln L, gradient[8], n_bad).  (One warp per
+// POINT walking its 9 rows one after the other took 16 us whatever the number of points: a chain of dependent L2 round trips.)
+constexpr int kAngCombineThreads = 32 * 10;
+__global__ void __launch_bounds__(kAngCombineThreads) angular_points_combine_kernel(const double* __restrict__ partials,
+                                                                                   const unsigned* __restrict__ bad_partials, int G,
+                                                                                   int n_points, double* __restrict__ out)
+{
+    __shared__ double s_sum[9];
+    __shared__ unsigned s_nb;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, p = blockIdx.x;
+    if (p >= n_points) return;
+    if (w < 9) {
+        const double s = warp_combine_partials(partials + ((int64_t)p * 9 + w) * G, G, lane);
+        if (lane == 0) s_sum[w] = s;
+    } else {
+        const unsigned nb = warp_combine_bad(bad_partials + (int64_t)p * G, G, lane);
+        if (lane == 0) s_nb = nb;
+    }
+    __syncthreads();
+    const unsigned nb = s_nb;
+    double* o = out + (int64_t)p * 10;
+    if (threadIdx.x < 9)
+        o[threadIdx.x] = !nb                ? -s_sum[threadIdx.x]
+                         : (threadIdx.x == 0) ? __longlong_as_double(0x7ff0000000000000LL)
+                                              : __longlong_as_double(0x7ff8000000000000LL);
+    else if (threadIdx.x == 9)
+        o[9] = (double)nb;
 }
 
 }  // namespace mf

@@ -261,60 +261,50 @@ __global__ void __launch_bounds__(kBlock, 2) fourd_points_mma_kernel(const __gri
     }
 }
 
-// One warp per point: fixed-order Kahan sums of the CTA partials, then the K + 2 = 18 outputs.
+// One CTA per point, one warp per quantity (17 sums + the bad-event count; warp_combine_partials, mf_points.cuh), then the
+// K + 2 = 18 outputs.
 // Sums: 0 ln prod D; 1 sum ws; 2 sum ws h_mu; 3 sum ws h_sigma; 4 sum wb h_tau'; 5..12 angular; 13, 14 cl1, cl2; 15, 16 ck1, ck2 (/ kappa).
-__global__ void __launch_bounds__(kBlock) fourd_points_combine_kernel(const double* __restrict__ partials,
-                                                                     const unsigned* __restrict__ bad_partials, int G, int n_points,
-                                                                     const double* __restrict__ fconst, const double2* __restrict__ sum_m,
-                                                                     double n, double* __restrict__ out)
+constexpr int kP4CombineThreads = 32 * 18;
+__global__ void __launch_bounds__(kP4CombineThreads) fourd_points_combine_kernel(const double* __restrict__ partials,
+                                                                                const unsigned* __restrict__ bad_partials, int G,
+                                                                                int n_points, const double* __restrict__ fconst,
+                                                                                const double2* __restrict__ sum_m, double n,
+                                                                                double* __restrict__ out)
 {
-    const int lane = threadIdx.x & 31, p = blockIdx.x * kWarps + (threadIdx.x >> 5);
+    __shared__ double s[17];
+    __shared__ unsigned s_nb;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, p = blockIdx.x;
     if (p >= n_points) return;
-    unsigned nb = 0;
-    for (int i = lane; i < G; i += 32) nb += __ldcg(bad_partials + (int64_t)p * G + i);
-    nb = __reduce_add_sync(0xffffffffu, nb);
-    double s[17];
-    for (int k = 0; k < 17; ++k) {
-        const double* pk = partials + ((int64_t)p * 17 + k) * G;
-        double v = 0.0, cc = 0.0;
-        for (int i = lane; i < G; i += 32) {
-            const double y = __ldcg(pk + i) - cc;
-            const double t = v + y;
-            cc = (t - v) - y;
-            v = t;
-        }
-        double lo = -cc;
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) {
-            const double s2 = __shfl_down_sync(0xffffffffu, v, off);
-            const double lo2 = __shfl_down_sync(0xffffffffu, lo, off);
-            const double t = v + s2;
-            const double bb = t - v;
-            const double e = (v - (t - bb)) + (s2 - bb);
-            lo = (lo + lo2) + e;
-            v = t;
-        }
-        s[k] = v + lo;
+    if (w < 17) {
+        const double v = warp_combine_partials(partials + ((int64_t)p * 17 + w) * G, G, lane);
+        if (lane == 0) s[w] = v;
+    } else {
+        const unsigned b = warp_combine_bad(bad_partials + (int64_t)p * G, G, lane);
+        if (lane == 0) s_nb = b;
     }
-    if (lane != 0) return;
+    __syncthreads();
+    const int k = threadIdx.x;
+    if (k > 17) return;
+    const unsigned nb = s_nb;
+    double* op = out + (int64_t)p * 18;
+    if (k == 17) {
+        op[17] = (double)nb;
+        return;
+    }
     const double* fc = fconst + (int64_t)p * kP4FinishConsts;
     const double inv_f = fc[0], inv_omf = fc[1], tau = fc[2], lnc2 = fc[3], kappa = fc[4];
-    const double2 sm = __ldg(sum_m);
-    double o[17];
-    o[0] = -(s[0] + fma(tau, sm.x, fma(tau, sm.y, n * lnc2)));
-    o[1] = -(inv_f * s[1] - inv_omf * (n - s[1]));  // sum (R A - L') / D from sum ws: ws / f - (1 - ws) / (1 - f)
-    o[2] = -s[2];
-    o[3] = -s[3];
-    o[4] = -s[4];
-#pragma unroll
-    for (int k = 5; k < 15; ++k) o[k] = -s[k];
-    o[15] = -kappa * s[15];
-    o[16] = -kappa * s[16];
-    double* op = out + (int64_t)p * 18;
-#pragma unroll
-    for (int k = 0; k < 17; ++k)
-        op[k] = !nb ? o[k] : (k == 0) ? __longlong_as_double(0x7ff0000000000000LL) : __longlong_as_double(0x7ff8000000000000LL);
-    op[17] = (double)nb;
+    double o;
+    if (k == 0) {
+        const double2 sm = __ldg(sum_m);
+        o = -(s[0] + fma(tau, sm.x, fma(tau, sm.y, n * lnc2)));
+    } else if (k == 1) {
+        o = -(inv_f * s[1] - inv_omf * (n - s[1]));  // sum (R A - L') / D from sum ws: ws / f - (1 - ws) / (1 - f)
+    } else if (k >= 15) {
+        o = -kappa * s[k];
+    } else {
+        o = -s[k];
+    }
+    op[k] = !nb ? o : (k == 0) ? __longlong_as_double(0x7ff0000000000000LL) : __longlong_as_double(0x7ff8000000000000LL);
 }
 
 }  // namespace mf
