@@ -599,12 +599,19 @@ def run_mine(args) -> None:
     host_view = pinned.numpy()
     e2e_steps = max(3, min(args.steps, 30))
 
+    e2e_parts = []   # host seconds of the pieces of every timed step: upload, model, sweep, destroy
+
     def e2e_step(i: int):
+        t0 = time.perf_counter()
         ds = ctx.dataset_upload(host_view, dg.MASS_LO, dg.MASS_HI)
+        t1 = time.perf_counter()
         md = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ds)
+        t2 = time.perf_counter()
         nll, g, nbad = md.nll_grad_sweep(pts_c)
+        t3 = time.perf_counter()
         md.close()
         ds.close()
+        e2e_parts.append((t1 - t0, t2 - t1, t3 - t2, time.perf_counter() - t3))
         return nll, nbad
 
     for i in range(3):
@@ -612,10 +619,12 @@ def run_mine(args) -> None:
     torch.cuda.synchronize()
     _barrier(world)
     t = time.perf_counter()
+    e2e_parts.clear()
     for i in range(e2e_steps):
         nll_h, nbad = e2e_step(i)
     torch.cuda.synchronize()
     e2e_s = _max_over_ranks(time.perf_counter() - t, world)
+    e2e_median_ms = [round(float(v) * 1e3, 4) for v in np.median(np.array(e2e_parts), axis=0)]
     if nbad or not np.all(np.isfinite(nll_h)):
         raise RuntimeError("non-finite NLL in the e2e steps")
     # the smallest e2e unit a minimiser sees: upload + model + ONE synchronous evaluation + destroy
@@ -636,7 +645,8 @@ def run_mine(args) -> None:
            "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps,
            "what": "per step: mf_dataset_upload (pinned host -> device, 8 MB) + mf_model_create + mf_nll_grad_sweep "
                    "(1000 host lambda points -> 1000 x (-lnL, gradient) on the host) + destroy",
-           "upload_plus_one_evaluation_ms": e2e_single_ms}
+           "upload_plus_one_evaluation_ms": e2e_single_ms,
+           "median_ms_upload_model_sweep_destroy": e2e_median_ms}
 
     if rank != 0:
         return

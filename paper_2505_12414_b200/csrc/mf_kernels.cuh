@@ -433,6 +433,45 @@ __device__ __forceinline__ double block_reduce(double* acc, unsigned bad, double
     return s;
 }
 
+// Fixed-order compensated sum of G partials by one warp: lane l adds partials l, l + 32, ... (Kahan), the 32 (sum, compensation)
+// pairs are merged by a two-sum tree.  The loads of a lane are issued eight at a time, independently of the running sum.
+__device__ __forceinline__ double warp_combine_partials(const double* __restrict__ pk, int G, int lane)
+{
+    double s = 0.0, cc = 0.0;
+    for (int base = lane; base < G; base += 256) {
+        double v[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) v[j] = (base + 32 * j < G) ? __ldcg(pk + base + 32 * j) : 0.0;
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+            if (base + 32 * j < G) {
+                const double y = v[j] - cc;
+                const double t = s + y;
+                cc = (t - s) - y;
+                s = t;
+            }
+    }
+    double lo = -cc;
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        const double s2 = __shfl_down_sync(0xffffffffu, s, off);
+        const double lo2 = __shfl_down_sync(0xffffffffu, lo, off);
+        const double t = s + s2;
+        const double bb = t - s;
+        const double e = (s - (t - bb)) + (s2 - bb);
+        lo = (lo + lo2) + e;
+        s = t;
+    }
+    return s + lo;  // lane 0
+}
+
+__device__ __forceinline__ unsigned warp_combine_bad(const unsigned* __restrict__ bp, int G, int lane)
+{
+    unsigned nb = 0;
+    for (int i = lane; i < G; i += 32) nb += __ldcg(bp + i);
+    return __reduce_add_sync(0xffffffffu, nb);
+}
+
 // ---- S5: fixed-order compensated combine of `count` partials per quantity, then M::finish ---------
 
 // Called by every thread of the CTA that drew the last ticket.  Warp w combines quantities w, w + 8,

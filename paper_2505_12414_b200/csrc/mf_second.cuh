@@ -228,26 +228,8 @@ __global__ void __launch_bounds__(kBlock) second_combine_kernel(const __grid_con
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int q = blockIdx.x * kWarps + w;
     if (q < L::NQ) {
-        const double* pk = a.partials + (int64_t)q * a.G;
-        double s = 0.0, cc = 0.0;
-        for (int i = lane; i < a.G; i += 32) {
-            const double y = __ldcg(pk + i) - cc;
-            const double t = s + y;
-            cc = (t - s) - y;
-            s = t;
-        }
-        double lo = -cc;
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) {
-            const double s2 = __shfl_down_sync(0xffffffffu, s, off);
-            const double lo2 = __shfl_down_sync(0xffffffffu, lo, off);
-            const double t = s + s2;
-            const double bb = t - s;
-            const double e = (s - (t - bb)) + (s2 - bb);
-            lo = (lo + lo2) + e;
-            s = t;
-        }
-        if (lane == 0) a.sums[q] = s + lo;
+        const double s = warp_combine_partials(a.partials + (int64_t)q * a.G, a.G, lane);
+        if (lane == 0) a.sums[q] = s;
     }
     __syncthreads();
     if (threadIdx.x == 0) s_last = (ticket_take(a.ticket) == gridDim.x - 1);
