@@ -6,7 +6,8 @@ fp64 events, 4 free parameters, "repeated NLL+gradient calls at 1,000 random par
 +-3 sigma_stat of truth".  One STEP = one complete SWEEP of the hot path over that workload: all 1,000
 seeded lambda points evaluated on one dataset replica (S2 parameter-only constants on the host, S3
 per-event value + gradient, S4/S5 reductions, S6 K+2 doubles out per point) = 1e9 event evaluations,
-issued as two mf_nll_grad_points calls of 500 points (= two kernel launches).  `value` = events/s;
+issued as ONE mf_nll_grad_points call of 1,000 points (= one kernel launch; two calls of 500 points cost 1.8 % more:
+≈ 30 us per call of kernel tail and hand-over).  `value` = events/s;
 `us_per_evaluation` = ms_per_step / 1000 points is printed beside it.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl mine|reference]
@@ -15,7 +16,7 @@ Timing rules followed: W >= 3 warm-up steps of the SAME call shape as the timed 
 over R = 32 dataset replicas (256 MB > the 126 MB L2), so every sweep first reads its events from HBM
 ("l2" in config); CUDA events on the launching stream; max over ranks; SM clocks and throttle reasons
 sampled (NVML, separate process) during the timed region.  The number does not depend on --steps: the
-driver's `--steps 20 --warmup 5` times 40 launches (~46 ms).
+driver's `--steps 20 --warmup 5` times 20 launches (~31 ms).
 
 `e2e` is the same step through the public API with HOST inputs: mf_dataset_upload from pinned host memory,
 mf_model_create, mf_nll_grad_sweep (1,000 host lambda points in, 1,000 x (K+1) host results out), destroy.
@@ -54,7 +55,7 @@ WORKLOAD = "C1: 1D Gaussian+exponential mass model, N=1e6 fp64 events, K=4, NLL+
 # per 8-event call = 22.1 per event, DESIGN.md §7 "Roofline"); the shipped kernel's count, never more than
 # the plain two-exponential form's hand count (100).  Round 1 credited 26 (that kernel's count).
 MASS_FP64_INSTR_PER_EVENT = 22.1
-POINTS_PER_CALL = 500  # evaluations per mf_nll_grad_points call (ONE launch: CTA tile = (point, event chunk))
+POINTS_PER_CALL = 1000  # evaluations per mf_nll_grad_points call (ONE launch: CTA tile = (point, event chunk))
 NOMINAL_FP64_LANES_PER_SM = 64  # B200: 4 SMSPs x 16 fp64 FMA lanes
 SINGLE_LAUNCH_STEPS = 4000      # evaluations of the one-launch-per-evaluation leg (fixed, whatever --steps says)
 REF_POINTS_PER_STEP = 8         # reference arm: lambda points of the sweep evaluated per step (bounded sample)
