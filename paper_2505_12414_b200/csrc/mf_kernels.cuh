@@ -744,8 +744,11 @@ __global__ void __launch_bounds__(BatchShape<M, BLOCK>::kThreads, BatchShape<M, 
             for (int64_t l = threadIdx.x; l < lines; l += kBlock) asm volatile("prefetch.global.L2 [%0];" ::"l"(base + 128 * l));
         }
     }
-    // S2 for this toy: parameter-only constants of lambda_t (batch_consts_kernel, the previous launch)
-    pdl_wait();
+    // S2 for this toy: parameter-only constants of lambda_t (batch_consts_kernel, the previous launch).  Many points on one
+    // dataset (shared_data): the host wrote the constants before the launch (pinned, device-mapped memory, or a stream-ordered
+    // copy), so the event loop does NOT wait for the previous kernel on the stream: under a programmatic launch the CTAs of this
+    // call fill the tail of the previous one; the wait comes before the first write to the scratch the calls share (below).
+    if (!a.shared_data) pdl_wait();
     {
         constexpr int W = (int)(sizeof(typename M::Consts) / sizeof(double));
         static_assert(sizeof(typename M::Consts) % sizeof(double) == 0 && W <= kBlock, "Consts is an array of doubles");
