@@ -358,6 +358,7 @@ extern "C" void mf_model_destroy(mf_model* m)
     // model may still be in flight
     server_stop_for_destroy(m);
     if (m->seq > 0 || m->n_toys > 1) cudaStreamSynchronize(m->ctx->stream);
+    if (m->s1_done) cudaEventDestroy(m->s1_done);
     dev_free(m->ctx, m->srv_relay);
     dev_free(m->ctx, m->srv_partials);
     dev_free(m->ctx, m->srv_bad);
@@ -504,6 +505,11 @@ extern "C" mf_status mf_model_create(mf_ctx* ctx, mf_model_kind kind, const mf_d
     }
     // nothing here needs the host to wait: the kernels read sum_i m_i from device memory, so a model is ready to be
     // evaluated (in stream order) as soon as this returns
+    if (cudaEventCreateWithFlags(&m->s1_done, cudaEventDisableTiming) == cudaSuccess)
+        cudaEventRecord(m->s1_done, ctx->stream);
+    else
+        m->s1_done = nullptr;
+    cudaGetLastError();
 #undef MF_CUDA_M
     *out = m;
     return MF_OK;
@@ -545,12 +551,18 @@ static cudaError_t launch_pdl(void (*kernel)(const Args), int grid, cudaStream_t
     return launch_pdl_v(kernel, grid, block, smem, stream, allow, a);
 }
 
-// true exactly once per model: its first launch must not overlap the S0/S1 kernels
+// true at most once per model: its first launch must not overlap the S0/S1 kernels of mf_model_create — unless those have
+// completed by now (a model created ahead of time, the usual case: one event query)
 static bool take_fresh(mf_model* m)
 {
-    const bool f = m->fresh;
+    if (!m->fresh) return false;
     m->fresh = false;
-    return f;
+    if (m->s1_done) {
+        const cudaError_t e = cudaEventQuery(m->s1_done);
+        if (e == cudaSuccess) return false;
+        cudaGetLastError();  // cudaErrorNotReady is not an error
+    }
+    return true;
 }
 
 template <class M>

@@ -87,6 +87,7 @@ struct mf_model {
     unsigned long long* gen = nullptr;  // device [kRing]: evaluations completed per scratch slot
     unsigned long long seq = 0;       // evaluations enqueued so far (evaluation e uses slot e % kRing)
     bool fresh = true;                // no kernel of this model launched yet: its first launch is made in plain stream order
+    cudaEvent_t s1_done = nullptr;    // recorded behind the S0/S1 kernels of mf_model_create: once it has completed, `fresh` no longer matters
     double* h_out = nullptr;          // pinned + mapped host slot: the output row, the 64-bit done word at MF_HOST_DONE_INDEX
     double* d_out_mapped = nullptr;   // device alias of h_out
     // batched evaluation
