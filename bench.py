@@ -6,8 +6,8 @@ fp64 events, 4 free parameters, "repeated NLL+gradient calls at 1,000 random par
 +-3 sigma_stat of truth".  One STEP = one complete SWEEP of the hot path over that workload: all 1,000
 seeded lambda points evaluated on one dataset replica (S2 parameter-only constants on the host, S3
 per-event value + gradient, S4/S5 reductions, S6 K+2 doubles out per point) = 1e9 event evaluations,
-issued as ONE mf_nll_grad_points call of 1,000 points (= one kernel launch; two calls of 500 points cost 1.8 % more:
-≈ 30 us per call of kernel tail and hand-over).  `value` = events/s;
+issued as ONE mf_nll_grad_points call of 1,000 points (= one kernel launch; consecutive calls overlap on the GPU, so the
+number does not depend on how a sweep is cut into calls).  `value` = events/s;
 `us_per_evaluation` = ms_per_step / 1000 points is printed beside it.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl mine|reference]
