@@ -350,6 +350,59 @@ def test_points_and_pipelining(mf, ctx):
     torch.cuda.synchronize()
 
 
+def test_overlapping_points_calls(mf, ctx):
+    """Back-to-back mf_nll_grad_points calls overlap on the GPU (constants read in place, the wait only before the shared
+    scratch is written): 60 calls of varying size on two models, more than the staging ring holds, the same output rows
+    written again and again — every call gives bit for bit what the same call gives when the stream is drained first, all
+    rows match the oracle at sampled points, and a sweep (sub-calls of 128 points) agrees with them."""
+    import torch
+    n1, n2 = 300_007, 70_001
+    m1, m2 = dg.gen_mass(n1, seed=21), dg.gen_mass(n2, seed=22)
+    mod1 = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(m1, dg.MASS_LO, dg.MASS_HI))
+    mod2 = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(m2, dg.MASS_LO, dg.MASS_HI))
+    pts = dg.gen_lambda_points(350, 9, dg.MASS_TRUTH, 3 * dg.mass_sigma_stat(n2))   # offsets < 50, sizes <= 300
+    sizes = [16, 200, 33, 128, 64, 17, 300, 50, 20, 100]
+    calls = [((mod1, m1) if i % 3 else (mod2, m2), sizes[i % len(sizes)], (7 * i) % 50) for i in range(60)]
+    # reference: each call alone, the stream drained before and after
+    ref = []
+    for (mod, _), k, off in calls:
+        o = torch.full((k, 6), float("nan"), dtype=torch.float64, device="cuda")
+        torch.cuda.synchronize()
+        mod.nll_grad_points(pts[off:off + k], o.data_ptr())
+        torch.cuda.synchronize()
+        ref.append(o.cpu().numpy())
+    # the same calls back to back; calls i and i + 2 write the same rows of one buffer (stream order must hold)
+    bufs = [torch.full((300, 6), float("nan"), dtype=torch.float64, device="cuda") for _ in range(2)]
+    got = []
+    for i, ((mod, _), k, off) in enumerate(calls):
+        mod.nll_grad_points(pts[off:off + k], bufs[i % 2].data_ptr())
+        if i % 7 == 6:                      # read some results back mid-series (asynchronously ordered copy)
+            got.append((i, bufs[i % 2][:k].clone()))
+    torch.cuda.synchronize()
+    for i, t in got:
+        assert np.array_equal(t.cpu().numpy(), ref[i]), f"call {i}"
+    for i in (58, 59):                      # the last writers of the two buffers
+        k = calls[i][1]
+        assert np.array_equal(bufs[i % 2][:k].cpu().numpy(), ref[i]), f"call {i}"
+    for i in (0, 6, 13, 59):
+        (mod, ev), k, off = calls[i]
+        for p in (0, k - 1):
+            o_nll, o_g, _ = oracle.nll_grad(oracle.MASS, ev, pts[off + p], dg.MASS_LO, dg.MASS_HI)
+            assert_parity(ref[i][p, 0], ref[i][p, 1:5], o_nll, o_g, f"call {i} point {p}")
+    pts = pts[:300]
+    nll, g, nbad = mod1.nll_grad_sweep(pts)   # 300 points: three sub-calls
+    assert not nbad
+    for p in (0, 127, 128, 299):
+        o_nll, o_g, _ = oracle.nll_grad(oracle.MASS, m1, pts[p], dg.MASS_LO, dg.MASS_HI)
+        assert_parity(nll[p], g[p], o_nll, o_g, f"sweep point {p}")
+    bad = pts.copy()
+    bad[290, 2] = -1.0                        # in the last sub-call: the caller's arrays are not touched
+    with pytest.raises(mf.MoreFitError) as e:
+        mod1.nll_grad_sweep(bad)
+    assert e.value.status == mf.MF_ERR_PARAM_DOMAIN
+    torch.cuda.synchronize()
+
+
 def test_batch_async_parity(mf, ctx):
     """mf_nll_grad_batch_async (device pointers, no host copies) equals mf_nll_grad_batch bit for bit."""
     import torch
