@@ -571,15 +571,15 @@ def run_mine(args) -> None:
     us_per_eval = 1e3 * ms_per_step / N_POINTS
     value = world * N_EVENTS * N_POINTS * args.steps / (ms * 1e-3)
 
-    # the same evaluations as ONE KERNEL LAUNCH PER EVALUATION (8 points per call -> pipelined single evaluations, every
+    # the same evaluations as ONE KERNEL LAUNCH PER EVALUATION (7 points per call -> pipelined single evaluations, every
     # launch reading its replica's events from HBM): the number a minimiser sees when its points arrive one at a time.
     # Always SINGLE_LAUNCH_STEPS launches, whatever --steps says.
     def run_single_launch_steps(count: int):
         i = 0
         while i < count:
             p = i % N_POINTS
-            c = min(8 - p % 8, count - i)
-            models[(i // 8) % N_REPLICAS].nll_grad_points(pts_c[p:p + c], out_ptrs[p])
+            c = min(7 - p % 7, count - i, N_POINTS - p)   # < 8 points per call: the library launches them one by one
+            models[(i // 7) % N_REPLICAS].nll_grad_points(pts_c[p:p + c], out_ptrs[p])
             i += c
 
     n_single = SINGLE_LAUNCH_STEPS

@@ -169,10 +169,12 @@ mf_status mf_nll_grad_async(mf_model* model, const double* lambda, double* out_d
 /* n_points evaluations of the same dataset at n_points parameter points (BASELINE.json configs[1]:
  * "repeated NLL+gradient calls at 1,000 random parameter points"), enqueued without a host synchronisation.
  *   lambdas  host, [n_points][K].   out_dev  DEVICE, [n_points][K+2], row p = [-ln L, grad, n_bad] at point p.
- * Fewer than 16 points: mf_nll_grad_async n_points times (one launch each, pipelined).  Otherwise, by family:
+ * Few points (mass model: fewer than 8; angular, 4D: fewer than 16): mf_nll_grad_async n_points times (one launch each,
+ * pipelined).  Otherwise, by family:
  *   mass     ONE launch whose CTA tile is (point, event chunk), the parameter-only constants of every point derived on
- *            the host and uploaded through a pinned staging ring (the dataset is read from HBM once and re-read from L2
- *            by the other points; 8 B per event, ALU bound);
+ *            the host and read by the kernel in place from a pinned, device-mapped staging ring (the dataset is read from
+ *            HBM once and re-read from L2 by the other points; 8 B per event, ALU bound); consecutive calls overlap on the
+ *            GPU (outputs still land in stream order);
  *   angular  one pass over the nine cached columns per 32 points: P = h0 + A.H and G = R.H^T as fp64 tensor-core
  *            contractions on 8 points x 8 events (mf_points.cuh), then a combine launch;
  *   4D       one pass over the twelve columns per 16 points: tensor-core contractions around the per-pair exponential
@@ -180,7 +182,7 @@ mf_status mf_nll_grad_async(mf_model* model, const double* lambda, double* out_d
  * Weighted models: one second-order evaluation (gradient mode) per point.
  * No allocation, clearing or synchronisation per call once the model's scratch has grown to its size.
  * Every point is validated first: MF_ERR_PARAM_DOMAIN (nothing enqueued) if one is outside the domain
- * (for fewer than 16 points the earlier ones are enqueued). */
+ * (below the few-points threshold the earlier ones are enqueued). */
 mf_status mf_nll_grad_points(mf_model* model, int64_t n_points, const double* lambdas, double* out_dev);
 
 /* The same sweep with the results returned to the HOST: evaluates the n_points parameter points (as

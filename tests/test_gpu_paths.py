@@ -260,8 +260,10 @@ _ABLATION = textwrap.dedent("""
     mm = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(m, dg.MASS_LO, dg.MASS_HI))
     pts = dg.gen_lambda_points(40, 77, dg.MASS_TRUTH, 3 * dg.mass_sigma_stat(100_003))
     out = torch.zeros((40, 6), dtype=torch.float64, device="cuda")
-    for p in range(0, 40, 8):                       # pipelined single launches (< 16 points per call)
-        mm.nll_grad_points(pts[p:p + 8], out[p].data_ptr())
+    for p in range(0, 40, 5):                       # pipelined single launches (< 8 points per call)
+        mm.nll_grad_points(pts[p:p + 5], out[p].data_ptr())
+    for p in range(0, 40, 10):                      # small many-point calls (8 .. 15 points: one launch each)
+        mm.nll_grad_points(pts[p:p + 10], out[p].data_ptr())
     torch.cuda.synchronize()
     r = out.cpu().numpy()
     for p in (0, 13, 39):
