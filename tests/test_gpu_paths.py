@@ -59,7 +59,8 @@ def _fourd_points(n_pts, seed):
     return pts
 
 
-@pytest.mark.parametrize("n,n_pts", [(20_011, 16), (150_000, 64), (1, 16), (10_007, 17), (20_011, 40), (5_000, 100)])
+@pytest.mark.parametrize("n,n_pts", [(20_011, 16), (150_000, 64), (1, 16), (10_007, 17), (20_011, 40), (5_000, 100), (20_011, 6),
+                                     (20_011, 9)])
 def test_points_mode_angular_vs_oracle(mf, ctx, n, n_pts):
     """The angular many-points kernel (two tensor-core contractions, mf_points.cuh): every row of a >= 16-point call
     against the oracle, with ragged event counts, partly filled point blocks and more than one 64-point pass."""
@@ -99,7 +100,7 @@ def test_points_mode_angular_bad_point(mf, ctx):
     assert e.value.status == mf.MF_ERR_PARAM_DOMAIN
 
 
-@pytest.mark.parametrize("n,n_pts", [(30_001, 16), (100_000, 64), (1, 16), (10_007, 17), (5_000, 41)])
+@pytest.mark.parametrize("n,n_pts", [(30_001, 16), (100_000, 64), (1, 16), (10_007, 17), (5_000, 41), (30_001, 10), (30_001, 13)])
 def test_points_mode_fourd_vs_oracle(mf, ctx, n, n_pts):
     """The 4D many-points kernel (mf_points4d.cuh: one pass over the data per 16 points, tensor-core contractions around
     the per-pair exponential): every row against the oracle, ragged event counts, partly filled point blocks."""
