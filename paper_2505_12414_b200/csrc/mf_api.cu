@@ -903,11 +903,7 @@ static mf_status launch_points_angular_mma(mf_model* m, int64_t n_points, const 
     auto up = [](size_t x) { return (x + 255) / 256 * 256; };
     const int64_t P = ctx->p_points;
     const int C = ctx->p_chunks;
-    char* h_blk = nullptr;
-    int stage = 0;
     const size_t b_coef = sizeof(double) * 8 * n_points;
-    MF_CUDA(ctx, points_stage(ctx, b_coef, &h_blk, &stage));
-    std::memcpy(h_blk, lambdas, b_coef);
     AngPointsArgs a;
     for (int i = 0; i < 9; ++i) a.col[i] = m->col[i];
     a.n = m->n_events;
@@ -919,10 +915,44 @@ static mf_status launch_points_angular_mma(mf_model* m, int64_t n_points, const 
     q += up(sizeof(double) * P * MF_MAX_NACC * C);
     a.bad_partials = reinterpret_cast<unsigned*>(q);
     a.n_points = (int)n_points;
+    const dim3 grid((unsigned)G, (unsigned)((n_points + per_pass - 1) / per_pass));
+    static const bool copy_coef = std::getenv("MF_POINTS_COPY") != nullptr;
+    if (n_points <= kAngInlinePoints && per_pass != 64 && !copy_coef) {
+        // the coefficients travel in the parameter block: nothing sits between this call and the previous kernel on the stream,
+        // and both kernels are launched programmatically (mf_points.cuh): consecutive calls overlap
+        AngPointsInlineArgs ia;
+        ia.a = a;
+        ia.a.coef = nullptr;
+        std::memcpy(ia.coef, lambdas, b_coef);
+        const bool pdl_ok = !take_fresh(m);
+        auto launch = [&](auto kernel, dim3 g, int block, size_t smem, bool allow, auto&&... args) {
+            static const bool no_pdl = std::getenv("MF_NO_PDL") != nullptr;
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = g;
+            cfg.blockDim = dim3((unsigned)block);
+            cfg.dynamicSmemBytes = smem;
+            cfg.stream = ctx->stream;
+            cudaLaunchAttribute attr[1];
+            attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+            attr[0].val.programmaticStreamSerializationAllowed = 1;
+            cfg.attrs = attr;
+            cfg.numAttrs = (allow && !no_pdl) ? 1 : 0;
+            return cudaLaunchKernelEx(&cfg, kernel, args...);
+        };
+        if (per_pass == 32) MF_CUDA(ctx, launch(angular_points_mma_inline_kernel<4>, grid, kBlock, ang_points_smem<4>(), pdl_ok, ia));
+        else MF_CUDA(ctx, launch(angular_points_mma_inline_kernel<2>, grid, kBlock, ang_points_smem<2>(), pdl_ok, ia));
+        MF_CUDA(ctx, launch(angular_points_combine_kernel, dim3((unsigned)n_points), kAngCombineThreads, 0, true,
+                            (const double*)a.partials, (const unsigned*)a.bad_partials, G, (int)n_points, out_dev));
+        ctx->launches += 2;
+        return MF_OK;
+    }
+    char* h_blk = nullptr;
+    int stage = 0;
+    MF_CUDA(ctx, points_stage(ctx, b_coef, &h_blk, &stage));
+    std::memcpy(h_blk, lambdas, b_coef);
     MF_CUDA(ctx, cudaMemcpyAsync(q = ctx->p_blk, h_blk, b_coef, cudaMemcpyHostToDevice, ctx->stream));
     MF_CUDA(ctx, cudaEventRecord(ctx->pts_copied[stage], ctx->stream));
     take_fresh(m);
-    const dim3 grid((unsigned)G, (unsigned)((n_points + per_pass - 1) / per_pass));
     if (per_pass == 64) angular_points_mma_kernel<8><<<grid, kBlock, ang_points_smem<8>(), ctx->stream>>>(a);
     else if (per_pass == 32) angular_points_mma_kernel<4><<<grid, kBlock, ang_points_smem<4>(), ctx->stream>>>(a);
     else angular_points_mma_kernel<2><<<grid, kBlock, ang_points_smem<2>(), ctx->stream>>>(a);

@@ -27,10 +27,21 @@ namespace mf {
 struct AngPointsArgs {
     const double* col[9];   // h_0..h_8
     int64_t n, n_pad;
-    const double* coef;     // device [n_points][8]: FL, S3, S4, S5, AFB, S7, S8, S9 per point
+    const double* coef;     // device [n_points][8]: FL, S3, S4, S5, AFB, S7, S8, S9 per point; NULL: in the parameter block
     int n_points;
     double* partials;       // [n_points][9][G]
     unsigned* bad_partials; // [n_points][G]
+};
+
+// Calls of up to kAngInlinePoints points carry the coefficients in the kernel's parameter block (16 KB): no copy sits between
+// such a call and the previous kernel on the stream, so under the programmatic launch its CTAs start in the tail of the previous
+// call (both kernels release their successor at entry; the main kernel waits for its predecessor — the previous call's combine
+// kernel, which itself waited for that call's main kernel — only before it writes the partial sums the calls share, the
+// combine kernel before it reads them).
+constexpr int kAngInlinePoints = 256;
+struct AngPointsInlineArgs {
+    AngPointsArgs a;
+    double coef[kAngInlinePoints * 8];
 };
 
 // NPB point blocks of 8 points per CTA pass; grid = (G, ceil(n_points / (8 NPB))); dynamic shared memory: ang_points_smem<NPB>().
@@ -41,8 +52,25 @@ constexpr size_t ang_points_smem()
 }
 
 template <int NPB>
+__device__ __forceinline__ void angular_points_mma_body(const AngPointsArgs& a, const double* __restrict__ coef);
+
+template <int NPB>
 __global__ void __launch_bounds__(kBlock, (NPB <= 2) ? 3 : (NPB <= 4) ? 2 : 1) angular_points_mma_kernel(const __grid_constant__ AngPointsArgs a)
 {
+    angular_points_mma_body<NPB>(a, a.coef);
+}
+
+template <int NPB>
+__global__ void __launch_bounds__(kBlock, (NPB <= 2) ? 3 : (NPB <= 4) ? 2 : 1)
+    angular_points_mma_inline_kernel(const __grid_constant__ AngPointsInlineArgs ia)
+{
+    angular_points_mma_body<NPB>(ia.a, ia.coef);
+}
+
+template <int NPB>
+__device__ __forceinline__ void angular_points_mma_body(const AngPointsArgs& a, const double* __restrict__ coef)
+{
+    pdl_launch_dependents();
     // dynamic shared memory: per-lane staging of the event fragments (two stages filled by cp.async: loads in flight cost no
     // registers), reused after the event loop for the cross-warp reduction
     extern __shared__ __align__(16) unsigned char ap_raw[];
@@ -60,7 +88,7 @@ __global__ void __launch_bounds__(kBlock, (NPB <= 2) ? 3 : (NPB <= 4) ? 2 : 1) a
         const int p = p0 + 8 * pb + fg;
         const bool live = p < a.n_points;
 #pragma unroll
-        for (int kk = 0; kk < 2; ++kk) ca[pb][kk] = live ? __ldg(a.coef + (int64_t)p * 8 + 4 * kk + ft) : 0.0;
+        for (int kk = 0; kk < 2; ++kk) ca[pb][kk] = live ? coef[(int64_t)p * 8 + 4 * kk + ft] : 0.0;
     }
     double g[NPB][2];
     LogProd lp[NPB];
@@ -207,6 +235,7 @@ __global__ void __launch_bounds__(kBlock, (NPB <= 2) ? 3 : (NPB <= 4) ? 2 : 1) a
         red[warp][pb][fg][2 + 2 * ft] = g[pb][1];
     }
     __syncthreads();
+    pdl_wait();  // the partial sums are shared with the previous call, whose combine kernel must have read them
     for (int q = threadIdx.x; q < NPB * 8 * 10; q += kBlock) {
         const int pl = q / 10, k = q % 10;  // local point, quantity (9: bad count)
         const int p = p0 + pl;
@@ -235,6 +264,8 @@ __global__ void __launch_bounds__(kAngCombineThreads) angular_points_combine_ker
     __shared__ double s_sum[9];
     __shared__ unsigned s_nb;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, p = blockIdx.x;
+    pdl_launch_dependents();
+    pdl_wait();  // the main kernel of this call has completed
     if (p >= n_points) return;
     if (w < 9) {
         const double s = warp_combine_partials(partials + ((int64_t)p * 9 + w) * G, G, lane);

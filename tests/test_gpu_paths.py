@@ -232,6 +232,44 @@ def test_first_evaluation_after_create_is_ordered(mf, ctx):
         ds.close()
 
 
+def test_overlapping_angular_points_calls(mf, ctx):
+    """Angular many-points calls of up to 256 points carry their coefficients in the kernel parameters and overlap on the GPU:
+    40 back-to-back calls of varying size on two models, writing the same rows again and again, give bit for bit what each
+    call gives alone; sampled rows against the oracle; a 300-point call (copy path) in between."""
+    import torch
+    ev1, ev2 = dg.gen_angular(120_011, seed=31), dg.gen_angular(30_001, seed=32)
+    mod1 = ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ctx.dataset_upload(ev1))
+    mod2 = ctx.model_create(mf.MF_ANGULAR_KSTMUMU, ctx.dataset_upload(ev2))
+    pts = _ang_points(350, 12)
+    sizes = [6, 64, 17, 256, 33, 300, 16, 100]
+    calls = [((mod1, ev1) if i % 3 else (mod2, ev2), sizes[i % len(sizes)], (5 * i) % 50) for i in range(40)]
+    ref = []
+    for (mod, _), k, off in calls:
+        o = torch.full((k, 10), float("nan"), dtype=torch.float64, device="cuda")
+        torch.cuda.synchronize()
+        mod.nll_grad_points(pts[off:off + k], o.data_ptr())
+        torch.cuda.synchronize()
+        ref.append(o.cpu().numpy())
+    bufs = [torch.full((300, 10), float("nan"), dtype=torch.float64, device="cuda") for _ in range(2)]
+    got = []
+    for i, ((mod, _), k, off) in enumerate(calls):
+        mod.nll_grad_points(pts[off:off + k], bufs[i % 2].data_ptr())
+        if i % 5 == 4:
+            got.append((i, bufs[i % 2][:k].clone()))
+    torch.cuda.synchronize()
+    for i, t in got:
+        assert np.array_equal(t.cpu().numpy(), ref[i]), f"call {i}"
+    for i in (38, 39):
+        k = calls[i][1]
+        assert np.array_equal(bufs[i % 2][:k].cpu().numpy(), ref[i]), f"call {i}"
+    for i in (0, 3, 5, 39):
+        (mod, ev), k, off = calls[i]
+        for p in (0, k - 1):
+            o_nll, o_g, _ = oracle.nll_grad(oracle.ANGULAR, ev, pts[off + p])
+            assert abs(ref[i][p, 0] - o_nll) <= 1e-11 * abs(o_nll), (i, p)
+            assert np.all(np.abs(ref[i][p, 1:9] - o_g) <= 1e-9 * (1 + np.abs(o_g))), (i, p)
+
+
 _ABLATION = textwrap.dedent("""
     import numpy as np, sys
     sys.path.insert(0, {root!r})
