@@ -978,10 +978,23 @@ static mf_status launch_points_fourd_mma(mf_model* m, int64_t n_points, const do
     int stage = 0;
     const size_t per_point = sizeof(double) * (16 + kP4PointConsts + kP4FinishConsts);
     static_assert(sizeof(double) * (16 + kP4PointConsts + kP4FinishConsts) <= sizeof(FourDConsts), "per-point block fits the scratch layout");
-    MF_CUDA(ctx, points_stage(ctx, per_point * n_points, &h_blk, &stage));
-    double* h_coef = reinterpret_cast<double*>(h_blk);
-    double* h_pc = h_coef + 16 * n_points;
-    double* h_fc = h_pc + kP4PointConsts * n_points;
+    // up to kP4InlinePoints points: the per-point data travel in the kernels' parameter blocks (no copy, programmatic launches:
+    // consecutive calls overlap); more: through the pinned staging ring and a stream-ordered copy
+    static const bool copy_coef4 = std::getenv("MF_POINTS_COPY") != nullptr;
+    const bool inl = n_points <= kP4InlinePoints && per_pass == 16 && !copy_coef4;
+    FourDPointsInlineArgs ia;
+    FourDCombineInlineArgs ic;
+    double *h_coef, *h_pc, *h_fc;
+    if (inl) {
+        h_coef = ia.coef;
+        h_pc = ia.pconst;
+        h_fc = ic.fconst;
+    } else {
+        MF_CUDA(ctx, points_stage(ctx, per_point * n_points, &h_blk, &stage));
+        h_coef = reinterpret_cast<double*>(h_blk);
+        h_pc = h_coef + 16 * n_points;
+        h_fc = h_pc + kP4PointConsts * n_points;
+    }
     const double mref = 0.5 * (m->ma + m->mb);
     for (int64_t p = 0; p < n_points; ++p) {
         const double* lam = lambdas + p * 16;
@@ -1035,18 +1048,50 @@ static mf_status launch_points_fourd_mma(mf_model* m, int64_t n_points, const do
     q += up(sizeof(double) * P * MF_MAX_NACC * C);
     a.bad_partials = reinterpret_cast<unsigned*>(q);
     a.n_points = (int)n_points;
-    MF_CUDA(ctx, cudaMemcpyAsync(d_blk, h_blk, per_point * n_points, cudaMemcpyHostToDevice, ctx->stream));
-    MF_CUDA(ctx, cudaEventRecord(ctx->pts_copied[stage], ctx->stream));
-    take_fresh(m);
     const dim3 grid((unsigned)G, (unsigned)((n_points + per_pass - 1) / per_pass));
     const size_t smem4 = sizeof(double) * 2 * kBlock * kP4StageDoubles;  // 48 KB: above the default dynamic limit with the static part
     static const cudaError_t attr4 = [&] {
         cudaError_t e = cudaFuncSetAttribute(fourd_points_mma_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem4);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(fourd_points_mma_inline_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem4);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(fourd_points_mma_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem4);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(fourd_points_mma_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem4);
         return e;
     }();
     MF_CUDA(ctx, attr4);
+    if (inl) {
+        ia.a = a;
+        ia.a.coef = nullptr;
+        ia.a.pconst = nullptr;
+        ic.partials = a.partials;
+        ic.bad_partials = a.bad_partials;
+        ic.G = G;
+        ic.n_points = (int)n_points;
+        ic.sum_m = m->d_sum_m;
+        ic.n = (double)m->n_events;
+        ic.out = out_dev;
+        const bool pdl_ok = !take_fresh(m);
+        auto launch = [&](auto kernel, dim3 g, int block, size_t smem, bool allow, const auto& arg) {
+            static const bool no_pdl = std::getenv("MF_NO_PDL") != nullptr;
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = g;
+            cfg.blockDim = dim3((unsigned)block);
+            cfg.dynamicSmemBytes = smem;
+            cfg.stream = ctx->stream;
+            cudaLaunchAttribute attr[1];
+            attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+            attr[0].val.programmaticStreamSerializationAllowed = 1;
+            cfg.attrs = attr;
+            cfg.numAttrs = (allow && !no_pdl) ? 1 : 0;
+            return cudaLaunchKernelEx(&cfg, kernel, arg);
+        };
+        MF_CUDA(ctx, launch(fourd_points_mma_inline_kernel<2>, grid, kBlock, smem4, pdl_ok, ia));
+        MF_CUDA(ctx, launch(fourd_points_combine_inline_kernel, dim3((unsigned)n_points), kP4CombineThreads, 0, true, ic));
+        ctx->launches += 2;
+        return MF_OK;
+    }
+    MF_CUDA(ctx, cudaMemcpyAsync(d_blk, h_blk, per_point * n_points, cudaMemcpyHostToDevice, ctx->stream));
+    MF_CUDA(ctx, cudaEventRecord(ctx->pts_copied[stage], ctx->stream));
+    take_fresh(m);
     if (per_pass == 32) fourd_points_mma_kernel<4><<<grid, kBlock, smem4, ctx->stream>>>(a);
     else if (per_pass == 24) fourd_points_mma_kernel<3><<<grid, kBlock, smem4, ctx->stream>>>(a);
     else fourd_points_mma_kernel<2><<<grid, kBlock, smem4, ctx->stream>>>(a);

@@ -35,9 +35,36 @@ struct FourDPointsArgs {
     unsigned* bad_partials;      // [n_points][G]
 };
 
+// Calls of up to kP4InlinePoints points carry their per-point data in the kernels' parameter blocks (as the angular kernel's,
+// mf_points.cuh): no copy between such a call and the previous kernel on the stream, both kernels launched programmatically.
+constexpr int kP4InlinePoints = 96;
+struct FourDPointsInlineArgs {
+    FourDPointsArgs a;
+    double coef[kP4InlinePoints * 16];
+    double pconst[kP4InlinePoints * kP4PointConsts];
+};
+
+template <int NPB>
+__device__ __forceinline__ void fourd_points_mma_body(const FourDPointsArgs& a, const double* __restrict__ coef,
+                                                      const double* __restrict__ pconst);
+
 template <int NPB>
 __global__ void __launch_bounds__(kBlock, 2) fourd_points_mma_kernel(const __grid_constant__ FourDPointsArgs a)
 {
+    fourd_points_mma_body<NPB>(a, a.coef, a.pconst);
+}
+
+template <int NPB>
+__global__ void __launch_bounds__(kBlock, 2) fourd_points_mma_inline_kernel(const __grid_constant__ FourDPointsInlineArgs ia)
+{
+    fourd_points_mma_body<NPB>(ia.a, ia.coef, ia.pconst);
+}
+
+template <int NPB>
+__device__ __forceinline__ void fourd_points_mma_body(const FourDPointsArgs& a, const double* __restrict__ coef,
+                                                      const double* __restrict__ pconst)
+{
+    pdl_launch_dependents();
     // dynamic shared memory: the per-lane staging of the event fragments (two stages, filled by cp.async: loads in flight cost
     // no registers), reused after the event loop for the cross-warp reduction
     extern __shared__ __align__(16) unsigned char p4_raw[];
@@ -52,7 +79,7 @@ __global__ void __launch_bounds__(kBlock, 2) fourd_points_mma_kernel(const __gri
     const int p0 = blockIdx.y * (8 * NPB);
     for (int i = threadIdx.x; i < NPB * 8 * kP4PointConsts; i += kBlock) {
         const int p = p0 + i / kP4PointConsts;
-        (&s_pc[0][0])[i] = (p < a.n_points) ? __ldg(a.pconst + (int64_t)p0 * kP4PointConsts + i) : 0.0;
+        (&s_pc[0][0])[i] = (p < a.n_points) ? pconst[(int64_t)p0 * kP4PointConsts + i] : 0.0;
     }
     // A fragments of the first contractions: lane (fg, ft) holds, for point p = p0 + 8 pb + fg,
     //   ca[pb][kk] coefficient of h_{1 + 4 kk + ft};  cl_[pb] = (1, cl1, cl2, 0)[ft];  ck_[pb] = kappa (1, ck1, ck2, 0)[ft]
@@ -61,12 +88,12 @@ __global__ void __launch_bounds__(kBlock, 2) fourd_points_mma_kernel(const __gri
     for (int pb = 0; pb < NPB; ++pb) {
         const int p = p0 + 8 * pb + fg;
         const bool live = p < a.n_points;
-        const double* lam = a.coef + (int64_t)(live ? p : 0) * 16;
+        const double* lam = coef + (int64_t)(live ? p : 0) * 16;
 #pragma unroll
-        for (int kk = 0; kk < 2; ++kk) ca[pb][kk] = live ? __ldg(lam + 4 + 4 * kk + ft) : 0.0;
-        const double kappa = live ? (1.0 - __ldg(lam)) * kInv8Pi : 0.0;
-        cll[pb] = (ft == 0) ? 1.0 : (ft == 3 || !live) ? 0.0 : __ldg(lam + 11 + ft);
-        clk[pb] = (ft == 0) ? kappa : (ft == 3 || !live) ? 0.0 : kappa * __ldg(lam + 13 + ft);
+        for (int kk = 0; kk < 2; ++kk) ca[pb][kk] = live ? lam[4 + 4 * kk + ft] : 0.0;
+        const double kappa = live ? (1.0 - lam[0]) * kInv8Pi : 0.0;
+        cll[pb] = (ft == 0) ? 1.0 : (ft == 3 || !live) ? 0.0 : lam[11 + ft];
+        clk[pb] = (ft == 0) ? kappa : (ft == 3 || !live) ? 0.0 : kappa * lam[13 + ft];
     }
     __syncthreads();
     double gA[NPB][2], gL[NPB][2], gK[NPB][2];  // tiles: angular gradient; r LK x (cl, P2l, ...); r LL x (.., .., ck, P2k)
@@ -243,6 +270,7 @@ __global__ void __launch_bounds__(kBlock, 2) fourd_points_mma_kernel(const __gri
         }
     }
     __syncthreads();
+    pdl_wait();  // the partial sums are shared with the previous call, whose combine kernel must have read them
     for (int q = threadIdx.x; q < NPB * 8 * 18; q += kBlock) {
         const int pl = q / 18, k = q % 18;  // local point, quantity (17: bad count)
         const int p = p0 + pl;
@@ -265,12 +293,40 @@ __global__ void __launch_bounds__(kBlock, 2) fourd_points_mma_kernel(const __gri
 // K + 2 = 18 outputs.
 // Sums: 0 ln prod D; 1 sum ws; 2 sum ws h_mu; 3 sum ws h_sigma; 4 sum wb h_tau'; 5..12 angular; 13, 14 cl1, cl2; 15, 16 ck1, ck2 (/ kappa).
 constexpr int kP4CombineThreads = 32 * 18;
+struct FourDCombineInlineArgs {
+    const double* partials;
+    const unsigned* bad_partials;
+    int G, n_points;
+    const double2* sum_m;
+    double n;
+    double* out;
+    double fconst[kP4InlinePoints * kP4FinishConsts];
+};
+
+__device__ __forceinline__ void fourd_points_combine_body(const double* __restrict__ partials, const unsigned* __restrict__ bad_partials,
+                                                          int G, int n_points, const double* __restrict__ fconst,
+                                                          const double2* __restrict__ sum_m, double n, double* __restrict__ out);
+
 __global__ void __launch_bounds__(kP4CombineThreads) fourd_points_combine_kernel(const double* __restrict__ partials,
                                                                                 const unsigned* __restrict__ bad_partials, int G,
                                                                                 int n_points, const double* __restrict__ fconst,
                                                                                 const double2* __restrict__ sum_m, double n,
                                                                                 double* __restrict__ out)
 {
+    fourd_points_combine_body(partials, bad_partials, G, n_points, fconst, sum_m, n, out);
+}
+
+__global__ void __launch_bounds__(kP4CombineThreads) fourd_points_combine_inline_kernel(const __grid_constant__ FourDCombineInlineArgs c)
+{
+    fourd_points_combine_body(c.partials, c.bad_partials, c.G, c.n_points, c.fconst, c.sum_m, c.n, c.out);
+}
+
+__device__ __forceinline__ void fourd_points_combine_body(const double* __restrict__ partials, const unsigned* __restrict__ bad_partials,
+                                                          int G, int n_points, const double* __restrict__ fconst,
+                                                          const double2* __restrict__ sum_m, double n, double* __restrict__ out)
+{
+    pdl_launch_dependents();
+    pdl_wait();  // the main kernel of this call has completed
     __shared__ double s[17];
     __shared__ unsigned s_nb;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, p = blockIdx.x;

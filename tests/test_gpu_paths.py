@@ -270,6 +270,43 @@ def test_overlapping_angular_points_calls(mf, ctx):
             assert np.all(np.abs(ref[i][p, 1:9] - o_g) <= 1e-9 * (1 + np.abs(o_g))), (i, p)
 
 
+def test_overlapping_fourd_points_calls(mf, ctx):
+    """4D many-points calls of up to 96 points carry their per-point data in the kernel parameters and overlap on the GPU:
+    back-to-back calls of varying size, writing the same rows again and again, give bit for bit what each call gives alone;
+    sampled rows against the oracle; a 120-point call (copy path) in between."""
+    import torch
+    ev = dg.gen_4d(60_013, seed=41)
+    mod = ctx.model_create(mf.MF_MASS_X_ANGULAR, ctx.dataset_upload(ev, dg.MASS_LO, dg.MASS_HI))
+    pts = _fourd_points(170, 14)
+    sizes = [10, 64, 17, 96, 33, 120, 16]
+    calls = [(sizes[i % len(sizes)], (5 * i) % 50) for i in range(21)]
+    ref = []
+    for k, off in calls:
+        o = torch.full((k, 18), float("nan"), dtype=torch.float64, device="cuda")
+        torch.cuda.synchronize()
+        mod.nll_grad_points(pts[off:off + k], o.data_ptr())
+        torch.cuda.synchronize()
+        ref.append(o.cpu().numpy())
+    bufs = [torch.full((120, 18), float("nan"), dtype=torch.float64, device="cuda") for _ in range(2)]
+    got = []
+    for i, (k, off) in enumerate(calls):
+        mod.nll_grad_points(pts[off:off + k], bufs[i % 2].data_ptr())
+        if i % 4 == 3:
+            got.append((i, bufs[i % 2][:k].clone()))
+    torch.cuda.synchronize()
+    for i, t in got:
+        assert np.array_equal(t.cpu().numpy(), ref[i]), f"call {i}"
+    for i in (19, 20):
+        k = calls[i][0]
+        assert np.array_equal(bufs[i % 2][:k].cpu().numpy(), ref[i]), f"call {i}"
+    for i in (0, 3, 5, 20):
+        k, off = calls[i]
+        for p in (0, k - 1):
+            o_nll, o_g, _ = oracle.nll_grad(oracle.FOURD, ev, pts[off + p], dg.MASS_LO, dg.MASS_HI)
+            assert abs(ref[i][p, 0] - o_nll) <= 1e-11 * abs(o_nll), (i, p)
+            assert np.all(np.abs(ref[i][p, 1:17] - o_g) <= 1e-9 * (1 + np.abs(o_g))), (i, p)
+
+
 _ABLATION = textwrap.dedent("""
     import numpy as np, sys
     sys.path.insert(0, {root!r})
