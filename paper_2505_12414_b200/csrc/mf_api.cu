@@ -920,10 +920,6 @@ static mf_status launch_points_angular_mma(mf_model* m, int64_t n_points, const 
     if (n_points <= kAngInlinePoints && per_pass != 64 && !copy_coef) {
         // the coefficients travel in the parameter block: nothing sits between this call and the previous kernel on the stream,
         // and both kernels are launched programmatically (mf_points.cuh): consecutive calls overlap
-        AngPointsInlineArgs ia;
-        ia.a = a;
-        ia.a.coef = nullptr;
-        std::memcpy(ia.coef, lambdas, b_coef);
         const bool pdl_ok = !take_fresh(m);
         auto launch = [&](auto kernel, dim3 g, int block, size_t smem, bool allow, auto&&... args) {
             static const bool no_pdl = std::getenv("MF_NO_PDL") != nullptr;
@@ -939,8 +935,21 @@ static mf_status launch_points_angular_mma(mf_model* m, int64_t n_points, const 
             cfg.numAttrs = (allow && !no_pdl) ? 1 : 0;
             return cudaLaunchKernelEx(&cfg, kernel, args...);
         };
-        if (per_pass == 32) MF_CUDA(ctx, launch(angular_points_mma_inline_kernel<4>, grid, kBlock, ang_points_smem<4>(), pdl_ok, ia));
-        else MF_CUDA(ctx, launch(angular_points_mma_inline_kernel<2>, grid, kBlock, ang_points_smem<2>(), pdl_ok, ia));
+        if (n_points <= 32) {
+            AngPointsInlineArgs<32> ia;
+            ia.a = a;
+            ia.a.coef = nullptr;
+            std::memcpy(ia.coef, lambdas, b_coef);
+            if (per_pass == 32) MF_CUDA(ctx, launch(angular_points_mma_inline_kernel<4, 32>, grid, kBlock, ang_points_smem<4>(), pdl_ok, ia));
+            else MF_CUDA(ctx, launch(angular_points_mma_inline_kernel<2, 32>, grid, kBlock, ang_points_smem<2>(), pdl_ok, ia));
+        } else {
+            AngPointsInlineArgs<kAngInlinePoints> ia;
+            ia.a = a;
+            ia.a.coef = nullptr;
+            std::memcpy(ia.coef, lambdas, b_coef);
+            if (per_pass == 32) MF_CUDA(ctx, launch(angular_points_mma_inline_kernel<4, kAngInlinePoints>, grid, kBlock, ang_points_smem<4>(), pdl_ok, ia));
+            else MF_CUDA(ctx, launch(angular_points_mma_inline_kernel<2, kAngInlinePoints>, grid, kBlock, ang_points_smem<2>(), pdl_ok, ia));
+        }
         MF_CUDA(ctx, launch(angular_points_combine_kernel, dim3((unsigned)n_points), kAngCombineThreads, 0, true,
                             (const double*)a.partials, (const unsigned*)a.bad_partials, G, (int)n_points, out_dev));
         ctx->launches += 2;

@@ -39,9 +39,10 @@ struct AngPointsArgs {
 // kernel, which itself waited for that call's main kernel — only before it writes the partial sums the calls share, the
 // combine kernel before it reads them).
 constexpr int kAngInlinePoints = 256;
+template <int MAXP>  // 32 or kAngInlinePoints: small calls carry a small block (2 KB instead of 16 KB per launch)
 struct AngPointsInlineArgs {
     AngPointsArgs a;
-    double coef[kAngInlinePoints * 8];
+    double coef[MAXP * 8];
 };
 
 // NPB point blocks of 8 points per CTA pass; grid = (G, ceil(n_points / (8 NPB))); dynamic shared memory: ang_points_smem<NPB>().
@@ -60,9 +61,9 @@ __global__ void __launch_bounds__(kBlock, (NPB <= 2) ? 3 : (NPB <= 4) ? 2 : 1) a
     angular_points_mma_body<NPB>(a, a.coef);
 }
 
-template <int NPB>
+template <int NPB, int MAXP>
 __global__ void __launch_bounds__(kBlock, (NPB <= 2) ? 3 : (NPB <= 4) ? 2 : 1)
-    angular_points_mma_inline_kernel(const __grid_constant__ AngPointsInlineArgs ia)
+    angular_points_mma_inline_kernel(const __grid_constant__ AngPointsInlineArgs<MAXP> ia)
 {
     angular_points_mma_body<NPB>(ia.a, ia.coef);
 }
