@@ -169,7 +169,7 @@ mf_status mf_nll_grad_async(mf_model* model, const double* lambda, double* out_d
 /* n_points evaluations of the same dataset at n_points parameter points (BASELINE.json configs[1]:
  * "repeated NLL+gradient calls at 1,000 random parameter points"), enqueued without a host synchronisation.
  *   lambdas  host, [n_points][K].   out_dev  DEVICE, [n_points][K+2], row p = [-ln L, grad, n_bad] at point p.
- * Few points (mass model: fewer than 8; angular: fewer than 6; 4D: fewer than 10): mf_nll_grad_async n_points times (one launch each,
+ * Few points (mass model: fewer than 8, fewer than 4 up to 2e5 events; angular: fewer than 6; 4D: fewer than 10): mf_nll_grad_async n_points times (one launch each,
  * pipelined).  Otherwise, by family:
  *   mass     ONE launch whose CTA tile is (point, event chunk), the parameter-only constants of every point derived on
  *            the host and read by the kernel in place from a pinned, device-mapped staging ring (the dataset is read from

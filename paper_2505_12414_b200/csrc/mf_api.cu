@@ -1207,7 +1207,10 @@ extern "C" mf_status mf_nll_grad_points(mf_model* m, int64_t n_points, const dou
     // 2.86 / 1.31 at 1e4; 4 points 3.64 / 3.79 and 3.55 / 2.49.  Angular model (C2, L2-resident singles 7.7): one 16-point pass
     // costs ~40 us: 4 points 10.1, 8 points 5.1.  4D model (C3, singles 27.7): one pass ~245 us: 8 points 30.6, 12 points 20.4.
     static const int env_min_batch = std::getenv("MF_POINTS_MIN_BATCH") ? std::atoi(std::getenv("MF_POINTS_MIN_BATCH")) : 0;  // tuning knob
-    const int min_batch = env_min_batch > 0 ? env_min_batch : (m->kind == MF_MASS_GAUSS_EXP) ? 8 : (m->kind == MF_ANGULAR_KSTMUMU) ? 6 : 10;
+    const int min_batch = env_min_batch > 0                 ? env_min_batch
+                          : (m->kind == MF_MASS_GAUSS_EXP)  ? (m->n_pad <= 200000 ? 4 : 8)
+                          : (m->kind == MF_ANGULAR_KSTMUMU) ? 6
+                                                            : 10;
     if (n_points < min_batch) {
         for (int64_t p = 0; p < n_points; ++p) {
             const mf_status st = dispatch_single(m, lambdas + p * m->K, out_dev + p * (m->K + 2), n_points > 1);

@@ -336,7 +336,10 @@ _ABLATION = textwrap.dedent("""
     mm = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(m, dg.MASS_LO, dg.MASS_HI))
     pts = dg.gen_lambda_points(40, 77, dg.MASS_TRUTH, 3 * dg.mass_sigma_stat(100_003))
     out = torch.zeros((40, 6), dtype=torch.float64, device="cuda")
-    for p in range(0, 40, 5):                       # pipelined single launches (< 8 points per call)
+    for p in range(0, 39, 3):                       # pipelined single launches (< 4 points per call at this size)
+        mm.nll_grad_points(pts[p:p + 3], out[p].data_ptr())
+    mm.nll_grad_points(pts[39:40], out[39].data_ptr())
+    for p in range(0, 40, 5):                       # the smallest many-point calls
         mm.nll_grad_points(pts[p:p + 5], out[p].data_ptr())
     for p in range(0, 40, 10):                      # small many-point calls (8 .. 15 points: one launch each)
         mm.nll_grad_points(pts[p:p + 10], out[p].data_ptr())
