@@ -893,8 +893,8 @@ static mf_status launch_points_angular_mma(mf_model* m, int64_t n_points, const 
     static const int pass_env = std::getenv("MF_POINTS_PER_PASS") ? std::atoi(std::getenv("MF_POINTS_PER_PASS")) : 0;  // tuning knob
     // measured (C2, 1e6 events): 32 points per pass at 2 CTAs per SM (124 registers) 1.62 us per evaluation at 1000 points,
     // 64 per pass at 1 CTA per SM (212 registers) 1.85 us
-    const int per_pass = (pass_env == 16 || pass_env == 32 || pass_env == 64) ? pass_env : n_points > 16 ? 32 : 16;
-    const int ctas_per_sm = per_pass == 64 ? 1 : per_pass == 16 ? 3 : 2;
+    const int per_pass = (pass_env == 8 || pass_env == 16 || pass_env == 32 || pass_env == 64) ? pass_env : n_points > 16 ? 32 : n_points > 8 ? 16 : 8;
+    const int ctas_per_sm = per_pass == 64 ? 1 : per_pass <= 16 ? 3 : 2;
     const int G = points_grid_width(ctas_per_sm * ctx->sm_count, (n_points + per_pass - 1) / per_pass, n_groups);
     {
         const mf_status ss = points_scratch(ctx, n_points, G);
@@ -941,14 +941,16 @@ static mf_status launch_points_angular_mma(mf_model* m, int64_t n_points, const 
             ia.a.coef = nullptr;
             std::memcpy(ia.coef, lambdas, b_coef);
             if (per_pass == 32) MF_CUDA(ctx, launch(angular_points_mma_inline_kernel<4, 32>, grid, kBlock, ang_points_smem<4>(), pdl_ok, ia));
-            else MF_CUDA(ctx, launch(angular_points_mma_inline_kernel<2, 32>, grid, kBlock, ang_points_smem<2>(), pdl_ok, ia));
+            else if (per_pass == 16) MF_CUDA(ctx, launch(angular_points_mma_inline_kernel<2, 32>, grid, kBlock, ang_points_smem<2>(), pdl_ok, ia));
+            else MF_CUDA(ctx, launch(angular_points_mma_inline_kernel<1, 32>, grid, kBlock, ang_points_smem<1>(), pdl_ok, ia));
         } else {
             AngPointsInlineArgs<kAngInlinePoints> ia;
             ia.a = a;
             ia.a.coef = nullptr;
             std::memcpy(ia.coef, lambdas, b_coef);
             if (per_pass == 32) MF_CUDA(ctx, launch(angular_points_mma_inline_kernel<4, kAngInlinePoints>, grid, kBlock, ang_points_smem<4>(), pdl_ok, ia));
-            else MF_CUDA(ctx, launch(angular_points_mma_inline_kernel<2, kAngInlinePoints>, grid, kBlock, ang_points_smem<2>(), pdl_ok, ia));
+            else if (per_pass == 16) MF_CUDA(ctx, launch(angular_points_mma_inline_kernel<2, kAngInlinePoints>, grid, kBlock, ang_points_smem<2>(), pdl_ok, ia));
+            else MF_CUDA(ctx, launch(angular_points_mma_inline_kernel<1, kAngInlinePoints>, grid, kBlock, ang_points_smem<1>(), pdl_ok, ia));
         }
         MF_CUDA(ctx, launch(angular_points_combine_kernel, dim3((unsigned)n_points), kAngCombineThreads, 0, true,
                             (const double*)a.partials, (const unsigned*)a.bad_partials, G, (int)n_points, out_dev));
@@ -964,7 +966,8 @@ static mf_status launch_points_angular_mma(mf_model* m, int64_t n_points, const 
     take_fresh(m);
     if (per_pass == 64) angular_points_mma_kernel<8><<<grid, kBlock, ang_points_smem<8>(), ctx->stream>>>(a);
     else if (per_pass == 32) angular_points_mma_kernel<4><<<grid, kBlock, ang_points_smem<4>(), ctx->stream>>>(a);
-    else angular_points_mma_kernel<2><<<grid, kBlock, ang_points_smem<2>(), ctx->stream>>>(a);
+    else if (per_pass == 16) angular_points_mma_kernel<2><<<grid, kBlock, ang_points_smem<2>(), ctx->stream>>>(a);
+    else angular_points_mma_kernel<1><<<grid, kBlock, ang_points_smem<1>(), ctx->stream>>>(a);
     angular_points_combine_kernel<<<(unsigned)n_points, kAngCombineThreads, 0, ctx->stream>>>(
         a.partials, a.bad_partials, G, (int)n_points, out_dev);
     MF_CUDA(ctx, cudaGetLastError());
