@@ -1024,19 +1024,19 @@ static mf_status launch_points_fourd_mma(mf_model* m, int64_t n_points, const do
         pc[1] = c.m.nb0;
         pc[2] = c.m.tau;
         pc[3] = c.m.lnk - c.m.tau * mref + std::log(c.m.f);
-        pc[4] = c.m.is2;
-        pc[5] = c.m.kmu;
-        pc[6] = c.m.is3;
-        pc[7] = c.m.ksig;
-        pc[8] = (mref - c.m.ma) - c.m.ktau;
-        pc[9] = 0.0;
         double* fc = h_fc + kP4FinishConsts * p;
         fc[0] = 1.0 / c.m.f;
         fc[1] = 1.0 / c.m.omf;
         fc[2] = c.m.tau;
         fc[3] = c.m.lnc2;
         fc[4] = c.kappa;
-        fc[5] = 0.0;
+        fc[5] = c.m.is2;
+        fc[6] = c.m.kmu;
+        fc[7] = c.m.is3;
+        fc[8] = c.m.ksig;
+        fc[9] = (c.m.mu - c.m.ma) - c.m.ktau;
+        fc[10] = c.m.ma + c.m.ktau;
+        fc[11] = 0.0;
     }
     {
         const mf_status ss = points_scratch(ctx, n_points, G);

@@ -20,9 +20,10 @@
 
 namespace mf {
 
-constexpr int kP4PointConsts = 10;  // per point, in shared memory: mu', nb0, tau, q0, is2, kmu, is3, ksig, htau0, spare
+constexpr int kP4PointConsts = 4;   // per point, in shared memory: mu', nb0, tau, q0
 constexpr int kP4StageDoubles = 12;  // per lane and stage: f1[2], f2, f0, cl(fg), ck(fg), c2, m2 = 96 bytes
-constexpr int kP4FinishConsts = 6;  // per point, for the combine kernel: 1/f, 1/(1-f), tau, lnc2, kappa, spare
+constexpr int kP4FinishConsts = 12;  // per point, for the combine kernel: 1/f, 1/(1-f), tau, lnc2, kappa, is2, kmu, is3, ksig,
+                                     // mu - m_a - ktau, m_a + ktau, spare
 
 struct FourDPointsArgs {
     const double* col[12];       // m, cos theta_l, cos theta_K, h_0..h_8
@@ -97,13 +98,13 @@ __device__ __forceinline__ void fourd_points_mma_body(const FourDPointsArgs& a, 
     }
     __syncthreads();
     double gA[NPB][2], gL[NPB][2], gK[NPB][2];  // tiles: angular gradient; r LK x (cl, P2l, ...); r LL x (.., .., ck, P2k)
-    double ams[NPB][4];                         // per-thread: sum ws, ws h_mu, ws h_sigma, wb h_tau
+    double ams[NPB][3];                         // per-thread: sum ws, ws d, ws d^2 (d = m - mu)
     LogProd lp[NPB];
     unsigned bad[NPB];
 #pragma unroll
     for (int pb = 0; pb < NPB; ++pb) {
         gA[pb][0] = gA[pb][1] = gL[pb][0] = gL[pb][1] = gK[pb][0] = gK[pb][1] = 0.0;
-        ams[pb][0] = ams[pb][1] = ams[pb][2] = ams[pb][3] = 0.0;
+        ams[pb][0] = ams[pb][1] = ams[pb][2] = 0.0;
         bad[pb] = 0;
     }
     const double t_lane = mf_exp32_lane_entry();
@@ -173,8 +174,7 @@ __device__ __forceinline__ void fourd_points_mma_body(const FourDPointsArgs& a, 
 #pragma unroll
         for (int pb = 0; pb < NPB; ++pb) {
             const double* pc = s_pc[8 * pb + fg];
-            const double mu = pc[0], nb0 = pc[1], tau = pc[2], q0 = pc[3], is2 = pc[4], kmu = pc[5], is3 = pc[6], ksig = pc[7],
-                         ht0 = pc[8];
+            const double mu = pc[0], nb0 = pc[1], tau = pc[2], q0 = pc[3];
             const double m[2] = {f.m2.x, f.m2.y};
             double arg[2], d[2], t[2], R[2];
 #pragma unroll
@@ -194,14 +194,15 @@ __device__ __forceinline__ void fourd_points_mma_body(const FourDPointsArgs& a, 
                 if (masked && !v) r = 0.0;
                 lp[pb].mul(D, bad[pb]);
                 const double q = R[j] * r;                      // f (G/N1) / P
-                const double ws = q * A[pb][j], wb = Lp * r;
+                const double ws = q * A[pb][j];                 // signal weight of the event; the background's is 1 - ws
                 qa[pb][j] = q;
                 wl[pb][j] = r * LK[pb][j];
                 wk[pb][j] = r * LL[pb][j];
+                // raw moments of ws; the parameter-only factors and the background sums (from sum_i 1, sum_i m_i) are applied
+                // once per point by the combine kernel
                 ams[pb][0] += ws;
-                ams[pb][1] = fma(ws, fma(d[j], is2, -kmu), ams[pb][1]);
-                ams[pb][2] = fma(ws, fma(t[j], is3, -ksig), ams[pb][2]);
-                ams[pb][3] = fma(wb, m[j] + ht0, ams[pb][3]);
+                ams[pb][1] = fma(ws, d[j], ams[pb][1]);
+                ams[pb][2] = fma(ws, t[j], ams[pb][2]);
             }
         }
 #pragma unroll
@@ -243,7 +244,7 @@ __device__ __forceinline__ void fourd_points_mma_body(const FourDPointsArgs& a, 
     // lane (fg, ft) holds per-thread sums for point fg over its events: add the four ft lanes; tiles are complete per lane
 #pragma unroll
     for (int pb = 0; pb < NPB; ++pb) {
-        double v[5] = {lp[pb].log(), ams[pb][0], ams[pb][1], ams[pb][2], ams[pb][3]};
+        double v[5] = {lp[pb].log(), ams[pb][0], ams[pb][1], ams[pb][2], 0.0};
 #pragma unroll
         for (int i = 0; i < 5; ++i) {
             v[i] += __shfl_xor_sync(0xffffffffu, v[i], 1);
@@ -291,7 +292,7 @@ __device__ __forceinline__ void fourd_points_mma_body(const FourDPointsArgs& a, 
 
 // One CTA per point, one warp per quantity (17 sums + the bad-event count; warp_combine_partials, mf_points.cuh), then the
 // K + 2 = 18 outputs.
-// Sums: 0 ln prod D; 1 sum ws; 2 sum ws h_mu; 3 sum ws h_sigma; 4 sum wb h_tau'; 5..12 angular; 13, 14 cl1, cl2; 15, 16 ck1, ck2 (/ kappa).
+// Sums: 0 ln prod D; 1 sum ws; 2 sum ws d; 3 sum ws d^2; 4 unused; 5..12 angular; 13, 14 cl1, cl2; 15, 16 ck1, ck2 (/ kappa).
 constexpr int kP4CombineThreads = 32 * 18;
 struct FourDCombineInlineArgs {
     const double* partials;
@@ -355,6 +356,17 @@ __device__ __forceinline__ void fourd_points_combine_body(const double* __restri
         o = -(s[0] + fma(tau, sm.x, fma(tau, sm.y, n * lnc2)));
     } else if (k == 1) {
         o = -(inv_f * s[1] - inv_omf * (n - s[1]));  // sum (R A - L') / D from sum ws: ws / f - (1 - ws) / (1 - f)
+    } else if (k == 2) {  // d/dmu = -sum ws (d is2 - kmu): the two terms nearly cancel at a minimum
+        o = -diff_of_products(fc[5], s[2], fc[6], s[1]);
+    } else if (k == 3) {  // d/dsigma = -sum ws (d^2 is3 - ksig)
+        o = -diff_of_products(fc[7], s[3], fc[8], s[1]);
+    } else if (k == 4) {
+        // d/dtau = -sum wb (m - m_a - ktau) with wb = 1 - ws for every valid event:
+        //   sum_i (m_i - c) - sum ws (m - c),  c = m_a + ktau,  m - c = d + (mu - c);  sum_i m_i as its (hi, lo) pair
+        const double2 sm = __ldg(sum_m);
+        const double c = fc[10], pr = n * c, pe = fma(n, c, -pr);
+        const double all = (sm.x - pr) + (sm.y - pe);
+        o = -(all - fma(fc[9], s[1], s[2]));
     } else if (k >= 15) {
         o = -kappa * s[k];
     } else {
