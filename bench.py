@@ -615,8 +615,15 @@ def run_mine(args) -> None:
         e2e_parts.append((t1 - t0, t2 - t1, t3 - t2, time.perf_counter() - t3))
         return nll, nbad
 
-    for i in range(3):
+    # warm-up: at least 3 steps and at least 0.3 s of them.  The PCIe link of an otherwise busy GPU takes some tens of ms of
+    # host<->device traffic to reach its full speed (measured on this pool: the 8 MB upload takes 0.35-0.7 ms for the first
+    # 30-100 ms after the traffic starts, 0.19 ms afterwards; the device-only phases before this point move no data)
+    t_w = time.perf_counter()
+    i = 0
+    while i < 3 or time.perf_counter() - t_w < 0.3:
         e2e_step(i)
+        i += 1
+    e2e_warmup_steps = i
     torch.cuda.synchronize()
     _barrier(world)
     t = time.perf_counter()
@@ -647,7 +654,7 @@ def run_mine(args) -> None:
            "what": "per step: mf_dataset_upload (pinned host -> device, 8 MB) + mf_model_create + mf_nll_grad_sweep "
                    "(1000 host lambda points -> 1000 x (-lnL, gradient) on the host) + destroy",
            "upload_plus_one_evaluation_ms": e2e_single_ms,
-           "median_ms_upload_model_sweep_destroy": e2e_median_ms}
+           "median_ms_upload_model_sweep_destroy": e2e_median_ms, "warmup_steps": e2e_warmup_steps}
 
     if rank != 0:
         return
