@@ -228,6 +228,34 @@ def test_batch_many_toys_active_subset(mf, ctx):
             assert_parity(nll_all[t], g_all[t], o_nll, o_g, f"toy {t} (all)")
 
 
+def test_batch_cta_size_by_number_of_toys(mf, ctx):
+    """The library picks the toy kernel's CTA size from the number of active toys (4 warps, 2 warps from 24 toys per SM, 1 warp
+    from 40 per SM on: 3552 / 5920 on a B200): 6000 toys of 300 events cross both thresholds when evaluated in full and as
+    subsets of 4000 and 1000; sampled toys against the oracle, and a toy's result must not depend on which CTA size ran it
+    beyond the summation order (same tolerance)."""
+    T, n = 6000, 300
+    toys = dg.gen_mass_toys(T, n, first_seed=7000)
+    model = ctx.model_create(mf.MF_MASS_GAUSS_EXP, ctx.dataset_upload(toys, dg.MASS_LO, dg.MASS_HI, n_toys=T))
+    lams = dg.gen_lambda_points(T, 12, dg.MASS_TRUTH, 0.5 * dg.mass_sigma_stat(n))
+    results = []
+    for n_act in (T, 4000, 1000):
+        active = np.zeros(T, dtype=np.uint8)
+        active[np.random.default_rng(n_act).choice(T, n_act, replace=False)] = 1
+        active[0] = active[T - 1] = 1
+        nll, g = model.nll_grad_batch(lams, active)
+        results.append((active, nll, g))
+        for t in list(range(0, T, 397)) + [T - 1]:
+            if not active[t]:
+                continue
+            o_nll, o_g, _ = oracle.nll_grad(oracle.MASS, toys[t], lams[t], dg.MASS_LO, dg.MASS_HI)
+            assert_parity(nll[t], g[t], o_nll, o_g, f"{n_act} active, toy {t}")
+    (a0, n0, g0), (a1, n1, g1), (a2, n2, g2) = results
+    both = np.flatnonzero(a1 & a2)
+    assert len(both) > 100
+    assert np.all(np.abs(n0[both] - n2[both]) <= 1e-12 * np.abs(n0[both]))
+    assert np.all(np.abs(g1[both] - g2[both]) <= 1e-9 * (1 + np.abs(g2[both])))
+
+
 def test_batch_angular_parity(mf, ctx):
     T, n = 3, 4000
     ev = np.stack([dg.gen_angular(n, seed=40 + t) for t in range(T)], axis=1)  # [3][T][n]
