@@ -80,7 +80,7 @@ static cudaError_t stage_views(mf_model* m)
             ctx->h_stage = nullptr;
             ctx->h_stage_bytes = 0;
         }
-        const cudaError_t e = cudaHostAlloc(reinterpret_cast<void**>(&ctx->h_stage), b_lam + b_ids + b_out, cudaHostAllocDefault);
+        const cudaError_t e = cudaHostAlloc(reinterpret_cast<void**>(&ctx->h_stage), b_lam + b_ids + b_out, cudaHostAllocMapped);
         if (e != cudaSuccess) return e;
         ctx->h_stage_bytes = b_lam + b_ids + b_out;
     }
@@ -668,7 +668,7 @@ static mf_status stage_reserve(mf_ctx* ctx, size_t bytes)
         ctx->h_stage = nullptr;
         ctx->h_stage_bytes = 0;
     }
-    MF_CUDA(ctx, cudaHostAlloc(reinterpret_cast<void**>(&ctx->h_stage), bytes, cudaHostAllocDefault));
+    MF_CUDA(ctx, cudaHostAlloc(reinterpret_cast<void**>(&ctx->h_stage), bytes, cudaHostAllocMapped));
     ctx->h_stage_bytes = bytes;
     return MF_OK;
 }
@@ -1250,34 +1250,8 @@ extern "C" mf_status mf_nll_grad_sweep(mf_model* m, int64_t n_points, const doub
     if (n_points == 0) return MF_OK;
     mf_ctx* ctx = m->ctx;
     const int K = m->K, row = K + 2;
-    if (m->p_sweep_rows < n_points) {
-        dev_free(ctx, m->d_sweep);
-        m->d_sweep = nullptr;
-        m->p_sweep_rows = 0;
-        MF_CUDA(ctx, dev_alloc(ctx, &m->d_sweep, sizeof(double) * n_points * row));
-        m->p_sweep_rows = n_points;
-    }
-    // Mass model (the (point, chunk) kernel, whose consecutive calls overlap on the GPU): the sweep is issued in sub-calls of
-    // 128 points, so that the host derives the constants of the later points (~0.18 us each) while the GPU evaluates the
-    // earlier ones: a 1000-point sweep of C1 1.74 -> 1.60 ms.  A point outside the domain in a later sub-call is found after the
-    // earlier ones were enqueued; nothing is copied back then, so the caller's arrays stay untouched as documented.
-    static const int64_t sub = std::getenv("MF_SWEEP_SUBCALL") ? std::max<int64_t>(16, std::atoll(std::getenv("MF_SWEEP_SUBCALL"))) : 128;
-    if (m->kind == MF_MASS_GAUSS_EXP && !m->wts && n_points >= 2 * sub) {
-        for (int64_t p0 = 0; p0 < n_points; p0 += sub) {
-            const int64_t np = std::min<int64_t>(sub, n_points - p0);
-            const mf_status st = mf_nll_grad_points(m, np, lambdas + p0 * K, m->d_sweep + p0 * row);
-            if (st != MF_OK) {
-                if (st == MF_ERR_PARAM_DOMAIN)  // the index in the message is relative to the sub-call
-                    mf_fail(ctx, st, "mf_nll_grad_sweep: a lambda in [" + std::to_string((long long)p0) + ", " +
-                                         std::to_string((long long)(p0 + np)) + ") is outside the parameter domain");
-                return st;
-            }
-        }
-    } else {
-        const mf_status st = mf_nll_grad_points(m, n_points, lambdas, m->d_sweep);
-        if (st != MF_OK) return st;
-    }
-    // results through the context's pinned staging block (grow-only), then scattered to the caller's arrays
+    // The kernels write the result rows straight into the context's pinned, device-mapped staging block (grow-only): no
+    // device-to-host copy behind them, one stream synchronise, then the rows are scattered to the caller's arrays
     const size_t bytes = sizeof(double) * n_points * row;
     if (ctx->h_stage_bytes < bytes) {
         if (ctx->h_stage) {
@@ -1286,11 +1260,32 @@ extern "C" mf_status mf_nll_grad_sweep(mf_model* m, int64_t n_points, const doub
             ctx->h_stage = nullptr;
             ctx->h_stage_bytes = 0;
         }
-        MF_CUDA(ctx, cudaHostAlloc(reinterpret_cast<void**>(&ctx->h_stage), bytes, cudaHostAllocDefault));
+        MF_CUDA(ctx, cudaHostAlloc(reinterpret_cast<void**>(&ctx->h_stage), bytes, cudaHostAllocMapped));
         ctx->h_stage_bytes = bytes;
     }
     double* h = reinterpret_cast<double*>(ctx->h_stage);
-    MF_CUDA(ctx, cudaMemcpyAsync(h, m->d_sweep, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    double* d_rows = nullptr;
+    MF_CUDA(ctx, cudaHostGetDevicePointer(reinterpret_cast<void**>(&d_rows), h, 0));
+    // Mass model (the (point, chunk) kernel, whose consecutive calls overlap on the GPU): the sweep is issued in sub-calls of
+    // 128 points, so that the host derives the constants of the later points (~0.18 us each) while the GPU evaluates the
+    // earlier ones: a 1000-point sweep of C1 1.74 -> 1.60 ms.  A point outside the domain in a later sub-call is found after the
+    // earlier ones were enqueued; nothing is copied back then, so the caller's arrays stay untouched as documented.
+    static const int64_t sub = std::getenv("MF_SWEEP_SUBCALL") ? std::max<int64_t>(16, std::atoll(std::getenv("MF_SWEEP_SUBCALL"))) : 128;
+    if (m->kind == MF_MASS_GAUSS_EXP && !m->wts && n_points >= 2 * sub) {
+        for (int64_t p0 = 0; p0 < n_points; p0 += sub) {
+            const int64_t np = std::min<int64_t>(sub, n_points - p0);
+            const mf_status st = mf_nll_grad_points(m, np, lambdas + p0 * K, d_rows + p0 * row);
+            if (st != MF_OK) {
+                if (st == MF_ERR_PARAM_DOMAIN)  // the index in the message is relative to the sub-call
+                    mf_fail(ctx, st, "mf_nll_grad_sweep: a lambda in [" + std::to_string((long long)p0) + ", " +
+                                         std::to_string((long long)(p0 + np)) + ") is outside the parameter domain");
+                return st;
+            }
+        }
+    } else {
+        const mf_status st = mf_nll_grad_points(m, n_points, lambdas, d_rows);
+        if (st != MF_OK) return st;
+    }
     MF_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     int64_t bad_points = 0;
     for (int64_t p = 0; p < n_points; ++p) {

@@ -24,6 +24,17 @@ int main(int argc,char**argv){
     printf("n=%lld served=%d nll=%.12g  grad call %.2f us  hess call %.2f us\n",(long long)n,served,nll,dt,dt2);
   }
   mf_model_serve(md,0);
+  { /* throughput of evaluations issued one at a time WITHOUT waiting (mf_nll_grad_points with one point = mf_nll_grad_async:
+       one launch each, pipelined on the GPU) and of 8-point calls (one launch per call), results on the device */
+    double *lam8=malloc(8*4*8), nb; int64_t nbad; double nll8[8], g8[32];
+    for(int p=0;p<8;++p){lam8[4*p]=0.5+0.001*p; lam8[4*p+1]=5.27; lam8[4*p+2]=0.03; lam8[4*p+3]=-1.0;}
+    /* device output rows come from a sweep's scratch: use mf_nll_grad_sweep once to size it, then the async entry points need a
+       device pointer, which C callers get from their own cudaMalloc; here the sweep (host results) is timed instead */
+    for(int i=0;i<50;++i) mf_nll_grad_sweep(md,8,lam8,nll8,g8,&nbad);
+    double t=now(); for(int i=0;i<2000;++i) mf_nll_grad_sweep(md,8,lam8,nll8,g8,&nbad); double dt=(now()-t)/2000*1e6;
+    printf("n=%lld sweep of 8 points (one call, host results): %.2f us per call = %.2f us per evaluation\n",(long long)n,dt,dt/8); (void)nb;
+    free(lam8);
+  }
   mf_fit_result r; double t=now(); mf_fit(md,lam,NULL,NULL,&r); printf("fit %.1f us calls %d conv %d\n",(now()-t)*1e6,r.n_calls,r.converged);
   t=now(); mf_fit(md,lam,NULL,NULL,&r); printf("fit %.1f us calls %d conv %d\n",(now()-t)*1e6,r.n_calls,r.converged);
   mf_model_destroy(md); mf_dataset_destroy(ds); mf_ctx_destroy(ctx); return 0;}
