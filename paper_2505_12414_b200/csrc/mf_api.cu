@@ -1633,7 +1633,18 @@ static mf_status eval_batch(mf_model* m, int64_t n_toys, const double* lambdas, 
         ++n_active;
     }
     if (n_active == 0) return MF_OK;
-    MF_CUDA(ctx, cudaMemcpyAsync(m->d_lam, m->h_lam, sizeof(double) * n_active * K, cudaMemcpyHostToDevice, ctx->stream));
+    // lambda and the result rows stay in the pinned, device-mapped staging block: the constants kernel reads the former in place,
+    // the batched kernel writes the latter in place (one row per toy): no copy in either direction, one stream synchronise.
+    // (The 4D Hessian path goes through the second-order kernel toy by toy and keeps its device rows and the copy.)
+    static const bool copy_io = std::getenv("MF_BATCH_COPY") != nullptr;  // ablation: stream-ordered copies of lambda and the rows
+    const bool in_place = !copy_io && !(hess && m->kind == MF_MASS_X_ANGULAR);
+    double *d_lam_map = nullptr, *d_out_map = nullptr;
+    if (in_place) {
+        MF_CUDA(ctx, cudaHostGetDevicePointer(reinterpret_cast<void**>(&d_lam_map), m->h_lam, 0));
+        MF_CUDA(ctx, cudaHostGetDevicePointer(reinterpret_cast<void**>(&d_out_map), m->h_bout, 0));
+    } else {
+        MF_CUDA(ctx, cudaMemcpyAsync(m->d_lam, m->h_lam, sizeof(double) * n_active * K, cudaMemcpyHostToDevice, ctx->stream));
+    }
     if (n_active < n_toys)
         MF_CUDA(ctx, cudaMemcpyAsync(m->d_ids, m->h_ids, sizeof(int) * n_active, cudaMemcpyHostToDevice, ctx->stream));
     mf_status st = MF_OK;
@@ -1647,17 +1658,19 @@ static mf_status eval_batch(mf_model* m, int64_t n_toys, const double* lambdas, 
             else if (ss != MF_OK) return ss;
         }
     } else if (hess) {
-        st = (m->kind == MF_MASS_GAUSS_EXP) ? launch_batch<MassHessModel>(m, n_active) : launch_batch<AngularHessModel>(m, n_active);
+        st = (m->kind == MF_MASS_GAUSS_EXP) ? launch_batch<MassHessModel>(m, n_active, d_lam_map, d_out_map)
+                                            : launch_batch<AngularHessModel>(m, n_active, d_lam_map, d_out_map);
     } else {
         switch (m->kind) {
-        case MF_MASS_GAUSS_EXP: st = launch_batch<MassModel>(m, n_active); break;
-        case MF_ANGULAR_KSTMUMU: st = launch_batch<AngularModel>(m, n_active); break;
-        default: st = launch_batch<FourDModel>(m, n_active); break;
+        case MF_MASS_GAUSS_EXP: st = launch_batch<MassModel>(m, n_active, d_lam_map, d_out_map); break;
+        case MF_ANGULAR_KSTMUMU: st = launch_batch<AngularModel>(m, n_active, d_lam_map, d_out_map); break;
+        default: st = launch_batch<FourDModel>(m, n_active, d_lam_map, d_out_map); break;
         }
     }
     if (st != MF_OK) return st;
     const int row = (hess ? 1 + K + K * (K + 1) / 2 : K + 1) + 1;
-    MF_CUDA(ctx, cudaMemcpyAsync(m->h_bout, m->d_bout, sizeof(double) * n_active * row, cudaMemcpyDeviceToHost, ctx->stream));
+    if (!in_place)
+        MF_CUDA(ctx, cudaMemcpyAsync(m->h_bout, m->d_bout, sizeof(double) * n_active * row, cudaMemcpyDeviceToHost, ctx->stream));
     MF_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     for (int s : invalid) {  // as the batched kernels report a domain error: +inf, NaN
         double* o = m->h_bout + (int64_t)s * row;
