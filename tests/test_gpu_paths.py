@@ -367,11 +367,13 @@ _ABLATION = textwrap.dedent("""
 
 
 @pytest.mark.parametrize("switch", ["MF_NO_TMA", "MF_NO_PDL", "MF_NO_POINTS_MMA", "MF_BATCH_STAGES=0", "MF_BATCH_STAGES=2",
-                                    "MF_BATCH_BLOCK=32", "MF_BATCH_BLOCK=64"])
+                                    "MF_BATCH_BLOCK=32", "MF_BATCH_BLOCK=64", "MF_POINTS_COPY", "MF_BATCH_COPY"])
 def test_ablation_switches_vs_oracle(mf, switch):
     """The MF_NO_TMA=1 (register-buffer kernels for the angular / 4D models), MF_NO_PDL=1 (plain stream order),
     MF_NO_POINTS_MMA=1, MF_BATCH_STAGES=0 (batched toys with direct loads) and MF_BATCH_BLOCK=32 / 64 (the one- and two-warp
-    CTAs that the library picks by itself from 5920 / 3552 active toys on) paths that DESIGN.md quotes numbers for,
+    CTAs that the library picks by itself from 5920 / 3552 active toys on), MF_POINTS_COPY=1 (many-points calls fed by a
+    stream-ordered copy: no overlap of consecutive calls) and MF_BATCH_COPY=1 (batch calls with copies of lambda and the rows)
+    paths that DESIGN.md quotes numbers for,
     against the oracle."""
     env = dict(os.environ)
     name, _, value = switch.partition("=")
